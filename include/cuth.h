@@ -1,0 +1,146 @@
+/* cuth.h -- C ABI of the B200-native Jacobi-PCG hot path of CUTh-Solver (arxiv/paper_2606_17850).
+ *
+ * Boundary.  Everything behind these calls is hand-written CUDA for
+ * sm_100a; there is no CPU fallback.  Conventions shared by all calls:
+ *   - "_D" pointers are DEVICE pointers owned by the caller (allocate them with torch or cudaMalloc),
+ *     "_H" pointers are HOST pointers.  The library allocates no device memory of its own; its only
+ *     hidden host-side state is a cache of instantiated CUDA graphs keyed by the workspace address
+ *     (released by cuth_release_workspace / at process exit).
+ *   - Device buffers must be 16-byte aligned (torch gives 512).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call is
+ *     asynchronous on that stream and never synchronises with the host.
+ *   - Return value: CUTH_OK or a negative cuth_status_t for errors detectable on the host (bad
+ *     arguments, CUDA API failure).  NUMERICAL outcomes of a solve (converged / max-iters /
+ *     breakdown) are written to result_D->status on the device, because the call is asynchronous.
+ *   - Grid: nx * ny * nz cells, linear index i = x + nx*(y + ny*z), z = 0 bottom, z = nz-1 top
+ *     (convective).  All of nx, ny, nz must be >= 2 so that the diagonal offsets {1, nx, nx*ny}
+ *     are distinct and non-empty.  Index arithmetic is 64-bit.
+ */
+#ifndef CUTH_H_
+#define CUTH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  CUTH_OK = 0,
+  CUTH_ERR_NULL = -1,        /* a required pointer is NULL */
+  CUTH_ERR_DIMS = -2,        /* nx, ny or nz < 2, or N too large */
+  CUTH_ERR_VALUE = -3,       /* non-positive dx, dy, dz, rtol; negative h; bad enum value */
+  CUTH_ERR_SIZE = -4,        /* caller's buffer too small */
+  CUTH_ERR_ALIGN = -5,       /* device pointer not 16-byte aligned */
+  CUTH_ERR_CUDA = -6,        /* a CUDA runtime call failed (see cuth_last_cuda_error) */
+  CUTH_ERR_NOT_TRANSIENT = -7 /* cuth_transient_step on a matrix built without cvol/dt */
+} cuth_status_t;
+
+/* result_D->status values (device-side, numerical outcome of a solve) */
+enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN = 2, CUTH_SOLVE_RUNNING = 3 };
+
+enum { CUTH_FP64 = 0, CUTH_MIXED = 1 };            /* cuth_opts_t.precision / cuth_spmv precision */
+enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1 };
+
+/* The thermal problem of PAPER.md §III-B: eq. (4) (steady) and eq. (5) (backward
+ * Euler) on a box of cells with adiabatic sides/bottom (eq. (3)) and a Robin top
+ * (eq. (2)); T_amb = 0, so temperatures are rises above ambient. */
+typedef struct {
+  int64_t nx, ny, nz;
+  double dx, dy;              /* lateral cell size, m */
+  const double* dz_H;         /* [nz] layer thickness, m (host) */
+  const double* kappa_D;      /* conductivity W/m.K (DEVICE): nz values or nx*ny*nz values */
+  int32_t kappa_is_per_layer; /* 1: kappa_D has nz values, 0: one per cell */
+  double h_top;               /* W/m^2.K on the top face of layer nz-1 */
+  const double* cvol_H;       /* [nz] volumetric heat capacity J/m^3.K (host), or NULL => steady */
+  double dt;                  /* s; <= 0 => steady */
+} cuth_grid_t;
+
+typedef struct {
+  int32_t precision;          /* CUTH_FP64 or CUTH_MIXED (§IV-D) */
+  double rtol;                /* stop when ||b - A x||_2 <= rtol * ||b||_2 (true fp64 residual) */
+  int32_t max_iters;          /* cap on PCG iterations (Alg. 1 loop), > 0 */
+  int32_t true_resid_period;  /* MIXED early stage: evaluate b - A1 x every this many iterations
+                                 (20 steady, 5 transient); <= 0 => 20 */
+  int32_t preconditioner;     /* CUTH_PRECOND_JACOBI (M = diag A) or CUTH_PRECOND_NONE (M = I) */
+} cuth_opts_t;
+
+typedef struct {
+  int32_t status;             /* CUTH_SOLVE_* */
+  int32_t iterations;         /* PCG iterations done (Alg. 1 line 13 counter) */
+  int32_t promotions;         /* early->late switches (0 in FP64 mode, <= 1 in MIXED) */
+  int32_t true_resid_evals;   /* number of explicit b - A1 x evaluations */
+  double rel_resid_true;      /* last evaluated ||b - A1 x||_2 / ||b||_2 (fp64) */
+  double rel_resid_rec;       /* last recursive ||r||_2 / ||b||_2 */
+  int32_t switch_reason;      /* MIXED: 0 none, 1 = (14a), 2 = (14b), 3 = (14c), 4 = recursive converged */
+  int32_t switch_iteration;   /* iteration at which the switch happened */
+} cuth_result_t;
+
+/* Bytes of the caller-allocated device buffer that holds the matrix object (header, fp64 packed
+ * diagonals A1, fp32 copy A2, 1/D0, per-layer row sums).  0 on invalid dims. */
+size_t cuth_dia_bytes(const cuth_grid_t* grid);
+
+/* Bytes of the caller-allocated device workspace for cuth_pcg_solve / cuth_transient_step
+ * (control block, reduction partials, vectors r, p, mu and -- transient only -- b). */
+size_t cuth_workspace_bytes(const cuth_grid_t* grid, const cuth_opts_t* opts);
+
+/* Builder (hot-path step a0).  Computes from the cell fields the condensed-DIA ("Quad-Diag",
+ * PAPER.md:219, Fig. 4) matrix of eq. (4)/(5): only the main and the three upper diagonals
+ * (offsets 0, 1, nx, nx*ny), unpadded: diagonal k has exactly N - off[k] elements, element j =
+ * A[j, j+off[k]]; packed D0|D1|D2|D3 in one fp64 array `vals`, ptr = {0, N, 2N-1, 3N-1-nx,
+ * 4N-1-nx-nx*ny}.  Entries of A are stored (off-diagonals negative).  Where the +x / +y neighbour
+ * does not exist (x = nx-1, y = ny-1) the stored element is +0.0.  Also stored: the fp32 copy A2
+ * (round-to-nearest-even of vals), 1/D0 (fp64), and the exact row sums s(z) used by the MIXED
+ * operator.  Arithmetic: fp64 without FMA contraction, in the order DESIGN.md §4 states, so
+ * values are bit-identical to the oracle's.  dia_D: device buffer of >= cuth_dia_bytes(). */
+int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void* stream);
+
+/* View of the matrix object for the bit-exact layout test: device pointers to the packed fp64
+ * values and to the fp32 copy (same ptr/off), and the host copies of ptr[5], off[4].
+ * Any output pointer may be NULL.  Pure host arithmetic, no CUDA call. */
+int cuth_dia_view(const void* dia_D, const cuth_grid_t* grid, const double** vals_D, const float** vals32_D,
+                  const double** inv_diag_D, int64_t ptr_H[5], int64_t off_H[4]);
+
+/* SpMV (hot-path step a1), Alg. 2 read 0-based: y = A x with
+ * y[i] = D0[i] x[i] + sum_k ( Dk[i] x[i+off k] + Dk[i-off k] x[i-off k] ), out-of-range terms dropped.
+ * precision CUTH_FP64: fp64 matrix A1.  CUTH_MIXED: fp32-stored off-diagonals promoted to fp64
+ * ("FP64/32 SpMV with arithmetic decoupling") applied in difference form
+ * y_i = s_i x_i + sum_j g_ij (x_i - x_j) (DESIGN.md R-F3).  x_D, y_D: fp64 [N], distinct buffers. */
+int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const double* x_D, double* y_D,
+              void* stream);
+
+/* PCG solve (steps a1-a5), Alg. 1 with M = diag(A): x_D holds x0 on entry and
+ * the solution on exit.  The loop runs entirely on the device inside one CUDA graph (conditional
+ * WHILE node); convergence is decided on the device and verified on the true fp64 residual.
+ * MIXED: early stage on the fp32-stored operator, switch by eq. (14a)-(14c) with
+ * hot restart, late stage fp64.  b_D is read only.  work_D >= cuth_workspace_bytes().
+ * result_D: device cuth_result_t written when the solve ends.  b = 0 gives x = 0. */
+int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
+                   double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D, void* stream);
+
+/* One backward-Euler step (step a6), eq. (5): forms b = P_{n+1} + (C V/dt) T_n in
+ * one fused pass and solves A T_{n+1} = b warm-started from T_n.  power_D: W per cell [N];
+ * T_D: in T_n, out T_{n+1}.  The matrix must have been built with cvol_H and dt > 0. */
+int cuth_transient_step(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts,
+                        const double* power_D, double* T_D, void* work_D, size_t work_bytes,
+                        cuth_result_t* result_D, void* stream);
+
+/* Drops the cached CUDA graph(s) tied to this workspace address (call before freeing it). */
+int cuth_release_workspace(const void* work_D);
+
+/* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
+const char* cuth_last_cuda_error(void);
+
+/* Library version, e.g. 10000 = 1.0.0 */
+int cuth_version(void);
+
+/* Number of kernel launches the last cuth_pcg_solve/cuth_transient_step on this workspace will
+ * have made is data dependent; this returns the launches per PCG iteration of the graph body
+ * (used by bench.py to report gpu_launches = prologue + body * iterations + epilogue). */
+int cuth_launches_per_iteration(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUTH_H_ */

@@ -1,0 +1,14 @@
+"""cuth: B200-native Jacobi-PCG hot path of CUTh-Solver (arxiv/paper_2606_17850).
+
+Thin Python binding over the C-ABI library declared in include/cuth.h.  Every step of the
+path runs in the hand-written CUDA kernels of csrc/; this package only marshals arguments
+(torch tensors -> device pointers, current stream -> cudaStream_t).  There is no CPU fallback:
+importing `binding` without the compiled library, or calling it without a CUDA device, raises.
+"""
+from .binding import (  # noqa: F401
+    CuthError, Grid, Opts, Result, DiaMatrix, Solver,
+    cuth_dia_bytes, cuth_workspace_bytes, cuth_build_dia, cuth_dia_view, cuth_spmv,
+    cuth_pcg_solve, cuth_transient_step, cuth_release_workspace, cuth_version,
+    cuth_launches_per_iteration, load_library, exported_symbols,
+    FP64, MIXED, PRECOND_NONE, PRECOND_JACOBI,
+)

@@ -1,0 +1,271 @@
+"""ctypes binding with the same names as include/cuth.h (argument marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcuth.so")
+
+FP64, MIXED = 0, 1
+PRECOND_NONE, PRECOND_JACOBI = 0, 1
+STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}
+_ERR = {-1: "CUTH_ERR_NULL", -2: "CUTH_ERR_DIMS", -3: "CUTH_ERR_VALUE", -4: "CUTH_ERR_SIZE",
+        -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT"}
+
+
+class CuthError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = _ERR.get(code, str(code))
+        if code == -6:
+            msg += ": " + load_library().cuth_last_cuda_error().decode()
+        super().__init__(f"{where} failed: {msg}")
+
+
+class cuth_grid_t(C.Structure):
+    _fields_ = [("nx", C.c_int64), ("ny", C.c_int64), ("nz", C.c_int64),
+                ("dx", C.c_double), ("dy", C.c_double),
+                ("dz_H", C.c_void_p), ("kappa_D", C.c_void_p), ("kappa_is_per_layer", C.c_int32),
+                ("h_top", C.c_double), ("cvol_H", C.c_void_p), ("dt", C.c_double)]
+
+
+class cuth_opts_t(C.Structure):
+    _fields_ = [("precision", C.c_int32), ("rtol", C.c_double), ("max_iters", C.c_int32),
+                ("true_resid_period", C.c_int32), ("preconditioner", C.c_int32)]
+
+
+class cuth_result_t(C.Structure):
+    _fields_ = [("status", C.c_int32), ("iterations", C.c_int32), ("promotions", C.c_int32),
+                ("true_resid_evals", C.c_int32), ("rel_resid_true", C.c_double),
+                ("rel_resid_rec", C.c_double), ("switch_reason", C.c_int32),
+                ("switch_iteration", C.c_int32)]
+
+
+EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
+           "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
+           "cuth_version", "cuth_launches_per_iteration"]
+
+_lib = None
+
+
+def exported_symbols():
+    return list(EXPORTS)
+
+
+def load_library():
+    """dlopen the in-tree libcuth.so; fails loudly when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_17850_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, gp, op = C.c_void_p, C.POINTER(cuth_grid_t), C.POINTER(cuth_opts_t)
+    L.cuth_dia_bytes.restype = C.c_size_t
+    L.cuth_dia_bytes.argtypes = [gp]
+    L.cuth_workspace_bytes.restype = C.c_size_t
+    L.cuth_workspace_bytes.argtypes = [gp, op]
+    L.cuth_build_dia.restype = C.c_int
+    L.cuth_build_dia.argtypes = [gp, vp, C.c_size_t, vp]
+    L.cuth_dia_view.restype = C.c_int
+    L.cuth_dia_view.argtypes = [vp, gp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
+                                C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.cuth_spmv.restype = C.c_int
+    L.cuth_spmv.argtypes = [vp, gp, C.c_int, vp, vp, vp]
+    L.cuth_pcg_solve.restype = C.c_int
+    L.cuth_pcg_solve.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp, vp]
+    L.cuth_transient_step.restype = C.c_int
+    L.cuth_transient_step.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp, vp]
+    L.cuth_release_workspace.restype = C.c_int
+    L.cuth_release_workspace.argtypes = [vp]
+    L.cuth_last_cuda_error.restype = C.c_char_p
+    L.cuth_version.restype = C.c_int
+    L.cuth_launches_per_iteration.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise CuthError(rc, where)
+
+
+# ------------------------------------------------------------------ argument holders
+class Grid:
+    """Holds a cuth_grid_t and keeps the host arrays / device tensor it points to alive."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, kappa, h_top, cvol=None, dt=0.0):
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.n = self.nx * self.ny * self.nz
+        self._dz = np.ascontiguousarray(dz, dtype=np.float64)
+        self._cvol = None if cvol is None else np.ascontiguousarray(cvol, dtype=np.float64)
+        self.kappa = kappa          # torch CUDA float64 tensor (nz or n values) or None
+        per_layer = 1
+        kptr = None
+        if kappa is not None:
+            per_layer = 1 if kappa.numel() == self.nz else 0
+            kptr = kappa.data_ptr()
+        self.c = cuth_grid_t(self.nx, self.ny, self.nz, float(dx), float(dy),
+                             self._dz.ctypes.data, kptr, per_layer, float(h_top),
+                             None if self._cvol is None else self._cvol.ctypes.data, float(dt))
+
+    @property
+    def transient(self):
+        return self._cvol is not None and self.c.dt > 0
+
+    def ref(self):
+        return C.byref(self.c)
+
+
+def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI):
+    return cuth_opts_t(int(precision), float(rtol), int(max_iters), int(true_resid_period), int(preconditioner))
+
+
+@dataclass
+class Result:
+    status: int
+    iterations: int
+    promotions: int
+    true_resid_evals: int
+    rel_resid_true: float
+    rel_resid_rec: float
+    switch_reason: int
+    switch_iteration: int
+
+    @property
+    def status_name(self):
+        return STATUS_NAMES.get(self.status, "?")
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+# ------------------------------------------------------------------ the C calls, same names
+def cuth_dia_bytes(grid: Grid) -> int:
+    return int(load_library().cuth_dia_bytes(grid.ref()))
+
+
+def cuth_workspace_bytes(grid: Grid, opts) -> int:
+    return int(load_library().cuth_workspace_bytes(grid.ref(), C.byref(opts)))
+
+
+def cuth_build_dia(grid: Grid, dia, stream=None):
+    _check(load_library().cuth_build_dia(grid.ref(), _ptr(dia), dia.numel() * dia.element_size(),
+                                         stream or _stream()), "cuth_build_dia")
+
+
+def cuth_dia_view(dia, grid: Grid):
+    """Returns (vals_ptr, vals32_ptr, inv_diag_ptr, ptr[5], off[4]); pointers are device addresses."""
+    v, v32, dinv = C.c_void_p(), C.c_void_p(), C.c_void_p()
+    ptr = (C.c_int64 * 5)()
+    off = (C.c_int64 * 4)()
+    _check(load_library().cuth_dia_view(_ptr(dia), grid.ref(), C.byref(v), C.byref(v32), C.byref(dinv), ptr, off),
+           "cuth_dia_view")
+    return v.value, v32.value, dinv.value, list(ptr), list(off)
+
+
+def cuth_spmv(dia, grid: Grid, precision, x, y, stream=None):
+    _check(load_library().cuth_spmv(_ptr(dia), grid.ref(), int(precision), _ptr(x), _ptr(y), stream or _stream()),
+           "cuth_spmv")
+
+
+def cuth_pcg_solve(dia, grid: Grid, opts, b, x, work, result, stream=None):
+    _check(load_library().cuth_pcg_solve(_ptr(dia), grid.ref(), C.byref(opts), _ptr(b), _ptr(x), _ptr(work),
+                                         work.numel() * work.element_size(), _ptr(result), stream or _stream()),
+           "cuth_pcg_solve")
+
+
+def cuth_transient_step(dia, grid: Grid, opts, power, T, work, result, stream=None):
+    _check(load_library().cuth_transient_step(_ptr(dia), grid.ref(), C.byref(opts), _ptr(power), _ptr(T), _ptr(work),
+                                              work.numel() * work.element_size(), _ptr(result),
+                                              stream or _stream()), "cuth_transient_step")
+
+
+def cuth_release_workspace(work):
+    load_library().cuth_release_workspace(_ptr(work))
+
+
+def cuth_version() -> int:
+    return int(load_library().cuth_version())
+
+
+def cuth_launches_per_iteration() -> int:
+    return int(load_library().cuth_launches_per_iteration())
+
+
+# ------------------------------------------------------------------ convenience holders (allocation only)
+class DiaMatrix:
+    """Allocates the matrix buffer with torch and calls cuth_build_dia."""
+
+    def __init__(self, grid: Grid):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("cuth needs a CUDA device (no CPU fallback)")
+        self.grid = grid
+        nbytes = cuth_dia_bytes(grid)
+        if nbytes == 0:
+            raise CuthError(-2, "cuth_dia_bytes")
+        self.buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        cuth_build_dia(grid, self.buf)
+
+    def view(self):
+        """(vals fp64 [E], vals32 fp32 [E], inv_diag fp64 [N], ptr, off) as torch views of the buffer."""
+        import torch
+        v, v32, dinv, ptr, off = cuth_dia_view(self.buf, self.grid)
+        base = self.buf.data_ptr()
+        e = ptr[4]
+        vals = self.buf[v - base: v - base + 8 * e].view(torch.float64)
+        vals32 = self.buf[v32 - base: v32 - base + 4 * e].view(torch.float32)
+        inv = self.buf[dinv - base: dinv - base + 8 * self.grid.n].view(torch.float64)
+        return vals, vals32, inv, ptr, off
+
+    def spmv(self, x, precision=FP64, out=None):
+        import torch
+        y = torch.empty_like(x) if out is None else out
+        cuth_spmv(self.buf, self.grid, precision, x, y)
+        return y
+
+
+class Solver:
+    """Allocates workspace + result record once; solve()/step() enqueue without synchronising."""
+
+    def __init__(self, A: DiaMatrix, opts=None):
+        import torch
+        self.A = A
+        self.opts = opts or Opts()
+        self.work = torch.empty(cuth_workspace_bytes(A.grid, self.opts), dtype=torch.uint8, device="cuda")
+        self.result_dev = torch.zeros(C.sizeof(cuth_result_t), dtype=torch.uint8, device="cuda")
+
+    def solve(self, b, x):
+        cuth_pcg_solve(self.A.buf, self.A.grid, self.opts, b, x, self.work, self.result_dev)
+
+    def step(self, power, T):
+        cuth_transient_step(self.A.buf, self.A.grid, self.opts, power, T, self.work, self.result_dev)
+
+    def result(self) -> Result:
+        """Synchronising read-back of the device result record."""
+        raw = self.result_dev.cpu().numpy().tobytes()
+        r = cuth_result_t.from_buffer_copy(raw)
+        return Result(r.status, r.iterations, r.promotions, r.true_resid_evals, r.rel_resid_true,
+                      r.rel_resid_rec, r.switch_reason, r.switch_iteration)
+
+    def close(self):
+        cuth_release_workspace(self.work)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,160 @@
+// cuth_internal.cuh -- device-side structures and helpers shared by the cuth kernels.
+// Product code (CUDA, sm_100a).  Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/cuth.h"
+
+namespace cuth {
+
+constexpr int kAlign = 256;            // byte alignment of every section of the matrix object / workspace
+constexpr int kHeaderBytes = 512;
+constexpr uint64_t kMagic = 0x4355544844494131ull;  // "CUTHDIA1"
+constexpr int kMaxBlocks = 4096;       // upper bound on the grid of any reducing kernel
+constexpr int kNumPartialSlots = 4;    // partial-sum arrays (each kMaxBlocks doubles)
+
+// Host-computed placement of the sections inside the caller's matrix buffer.
+struct DiaLayout {
+  int64_t nx, ny, nz, n, nxny, e;
+  int64_t ptr[5], off[4];
+  size_t o_layers;   // dz[nz] | s[nz] | cap[nz] | cvol[nz]   (fp64)
+  size_t o_vals;     // fp64 [e]  packed D0|D1|D2|D3   (A1)
+  size_t o_vals32;   // fp32 [e]  same packing          (A2)
+  size_t o_dinv;     // fp64 [n]  1/D0
+  size_t bytes;
+};
+
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
+  if (!g || g->nx < 2 || g->ny < 2 || g->nz < 2) return false;
+  if (g->nx > (1ll << 31) / g->ny || g->nx * g->ny > (1ll << 31) / g->nz) return false;  // N < 2^31
+  L->nx = g->nx; L->ny = g->ny; L->nz = g->nz;
+  L->nxny = g->nx * g->ny;
+  L->n = L->nxny * g->nz;
+  L->off[0] = 0; L->off[1] = 1; L->off[2] = g->nx; L->off[3] = L->nxny;
+  L->ptr[0] = 0;
+  for (int k = 0; k < 4; ++k) L->ptr[k + 1] = L->ptr[k] + (L->n - L->off[k]);
+  L->e = L->ptr[4];
+  size_t o = kHeaderBytes;
+  L->o_layers = o; o = align_up(o + 4 * sizeof(double) * (size_t)g->nz);
+  L->o_vals = o;   o = align_up(o + sizeof(double) * (size_t)L->e);
+  L->o_vals32 = o; o = align_up(o + sizeof(float) * (size_t)L->e);
+  L->o_dinv = o;   o = align_up(o + sizeof(double) * (size_t)L->n);
+  L->bytes = o;
+  return true;
+}
+
+// Device view of the matrix handed to kernels by value.
+struct DiaDev {
+  const double* d0; const double* d1; const double* d2; const double* d3;   // fp64 diagonals (A1)
+  const float* f1; const float* f2; const float* f3;                        // fp32 off-diagonals (A2)
+  const double* dinv;       // 1/D0
+  const double* s_layer;    // exact row sums per layer: h dx dy [top] + C V / dt
+  const double* cap_layer;  // C V / dt per layer (0 when steady)
+  int64_t n, nx, nxny;
+};
+
+// Pointers and options of one solve; lives at the start of the workspace, written per call.
+struct Ctx {
+  DiaDev A;
+  const double* b;
+  double* x;
+  double* r;
+  double* p;
+  double* mu;
+  cuth_result_t* result;
+  double rtol;
+  int32_t precision, max_iters, period, jacobi;
+};
+
+// Scalars of the iteration; device resident, written only by "last block" epilogues.
+struct Ctl {
+  double rho, pAp, alpha, beta, rr, bb, tol2, sw2;
+  double tt, dd, tt_prev, rr_prev_eval;
+  int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
+  int32_t switch_reason, switch_it, conv_rec, zero_rhs, pad;
+  unsigned int ticket[8];
+};
+
+struct Workspace {
+  Ctx* ctx; Ctl* ctl; double* partials; double* r; double* p; double* mu; double* b;
+  size_t bytes;
+};
+
+inline Workspace carve_workspace(void* base, int64_t n, bool with_b) {
+  Workspace w;
+  char* c = (char*)base;
+  size_t o = 0;
+  w.ctx = (Ctx*)(c + o); o = align_up(o + sizeof(Ctx));
+  w.ctl = (Ctl*)(c + o); o = align_up(o + sizeof(Ctl));
+  w.partials = (double*)(c + o); o = align_up(o + sizeof(double) * kMaxBlocks * kNumPartialSlots);
+  w.r = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
+  w.p = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
+  w.mu = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
+  w.b = nullptr;
+  if (with_b) { w.b = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
+  w.bytes = o;
+  return w;
+}
+
+#ifdef __CUDACC__
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Sum of NV values over the block (blockDim.x multiple of 32, <= 1024); result valid in thread 0.
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* smem /* >= NV*32 */) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int k = 0; k < NV; ++k) v[k] = warp_sum(v[k]);
+  __syncthreads();
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < NV; ++k) smem[k * 32 + wid] = v[k];
+  }
+  __syncthreads();
+  if (wid == 0) {
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+      double t = lane < nw ? smem[k * 32 + lane] : 0.0;
+      v[k] = warp_sum(t);
+    }
+  }
+}
+
+// Grid-wide deterministic reduction: every block deposits NV partials, the last block to arrive
+// (atomic ticket) sums them in a fixed order.  Returns true in ALL threads of that last block,
+// with the totals valid in thread 0 only.
+template <int NV>
+__device__ __forceinline__ bool grid_sum_last_block(double (&v)[NV], double* partials, unsigned int* ticket,
+                                                    double* smem, int* s_flag) {
+  block_sum<NV>(v, smem);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int k = 0; k < NV; ++k) partials[k * kMaxBlocks + blockIdx.x] = v[k];
+    __threadfence();
+    unsigned int t = atomicAdd(ticket, 1u);
+    *s_flag = (t == gridDim.x - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  if (!*s_flag) return false;
+  __threadfence();
+#pragma unroll
+  for (int k = 0; k < NV; ++k) {
+    double a = 0.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) a += __ldcg(&partials[k * kMaxBlocks + b]);
+    v[k] = a;
+  }
+  block_sum<NV>(v, smem);
+  if (threadIdx.x == 0) *ticket = 0u;
+  return true;
+}
+#endif  // __CUDACC__
+
+}  // namespace cuth

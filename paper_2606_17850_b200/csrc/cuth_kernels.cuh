@@ -1,0 +1,350 @@
+// cuth_kernels.cuh -- the PCG hot-path kernels (steps a1-a6 of DESIGN.md §3).
+// Alg. 1 with M = diag(A); Alg. 2 for the SpMV.
+#pragma once
+#include "cuth_internal.cuh"
+
+namespace cuth {
+
+constexpr int kThreads = 256;
+constexpr int kRows = 2;        // rows per thread per tile (strided by blockDim for coalescing)
+
+// ---------------------------------------------------------------------------------------------
+// One row of y = A v, Alg. 2 read 0-based: 7 terms, out-of-range terms dropped.  The structural
+// zeros stored in D1/D2 (x = nx-1, y = ny-1) make the lateral wrap-around vanish by themselves,
+// so the operator is purely banded in the linear index i.
+// MIXED = false: fp64 matrix A1 (kernel K1 of the paper).
+// MIXED = true : fp32-stored off-diagonals promoted to fp64 (K3) and applied in
+//                difference form  y_i = s_i v_i + sum_j g_ij (v_i - v_j)   (DESIGN.md R-F3).
+template <bool MIXED>
+__device__ __forceinline__ double spmv_row(const DiaDev& A, const double* __restrict__ v, int64_t i, double vi) {
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx, up3 = i + np < n, lo3 = i >= np;
+  if (!MIXED) {
+    // issue all loads first
+    const double a0 = A.d0[i];
+    const double a1u = up1 ? A.d1[i] : 0.0, a1l = lo1 ? A.d1[i - 1] : 0.0;
+    const double a2u = up2 ? A.d2[i] : 0.0, a2l = lo2 ? A.d2[i - nx] : 0.0;
+    const double a3u = up3 ? A.d3[i] : 0.0, a3l = lo3 ? A.d3[i - np] : 0.0;
+    const double v1u = up1 ? v[i + 1] : 0.0, v1l = lo1 ? v[i - 1] : 0.0;
+    const double v2u = up2 ? v[i + nx] : 0.0, v2l = lo2 ? v[i - nx] : 0.0;
+    const double v3u = up3 ? v[i + np] : 0.0, v3l = lo3 ? v[i - np] : 0.0;
+    double acc = a0 * vi;
+    acc = fma(a1u, v1u, acc); acc = fma(a1l, v1l, acc);
+    acc = fma(a2u, v2u, acc); acc = fma(a2l, v2l, acc);
+    acc = fma(a3u, v3u, acc); acc = fma(a3l, v3l, acc);
+    return acc;
+  } else {
+    const float g1u = up1 ? A.f1[i] : 0.f, g1l = lo1 ? A.f1[i - 1] : 0.f;
+    const float g2u = up2 ? A.f2[i] : 0.f, g2l = lo2 ? A.f2[i - nx] : 0.f;
+    const float g3u = up3 ? A.f3[i] : 0.f, g3l = lo3 ? A.f3[i - np] : 0.f;
+    const double v1u = up1 ? v[i + 1] : vi, v1l = lo1 ? v[i - 1] : vi;
+    const double v2u = up2 ? v[i + nx] : vi, v2l = lo2 ? v[i - nx] : vi;
+    const double v3u = up3 ? v[i + np] : vi, v3l = lo3 ? v[i - np] : vi;
+    const unsigned z = (unsigned)i / (unsigned)np;
+    double acc = A.s_layer[z] * vi;
+    // stored entries are A's (negative); conductance g = -entry, y += g (vi - vj) = entry (vj - vi)
+    acc = fma((double)g1u, v1u - vi, acc); acc = fma((double)g1l, v1l - vi, acc);
+    acc = fma((double)g2u, v2u - vi, acc); acc = fma((double)g2l, v2l - vi, acc);
+    acc = fma((double)g3u, v3u - vi, acc); acc = fma((double)g3l, v3l - vi, acc);
+    return acc;
+  }
+}
+
+#define CUTH_TILE_LOOP(n_)                                                                   \
+  for (int64_t base = (int64_t)blockIdx.x * (kThreads * kRows); base < (n_);                 \
+       base += (int64_t)gridDim.x * (kThreads * kRows))
+
+// ---------------------------------------------------------------------------------------------
+// Standalone SpMV (cuth_spmv).
+template <bool MIXED>
+__global__ void __launch_bounds__(kThreads) k_spmv_only(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
+  CUTH_TILE_LOOP(A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < A.n) y[i] = spmv_row<MIXED>(A, x, i, x[i]);
+    }
+  }
+}
+
+// Writes the per-call context and clears the control block (plain launch before the graph).
+__global__ void k_set_ctx(Ctx c, Ctx* dst, Ctl* ctl) {
+  if (threadIdx.x == 0) {
+    *dst = c;
+    Ctl z;
+    memset(&z, 0, sizeof(z));
+    z.status = CUTH_SOLVE_RUNNING;
+    *ctl = z;
+  }
+}
+
+// rhs of eq. (5), T_amb = 0:  b = P + (C V / dt) T_n
+__global__ void __launch_bounds__(kThreads) k_transient_rhs(DiaDev A, const double* __restrict__ power,
+                                                           const double* __restrict__ t_n, double* __restrict__ b) {
+  CUTH_TILE_LOOP(A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < A.n) {
+        const unsigned z = (unsigned)i / (unsigned)A.nxny;
+        b[i] = __dadd_rn(power[i], __dmul_rn(A.cap_layer[z], t_n[i]));
+      }
+    }
+  }
+}
+
+// Alg. 1 lines 1-3: r0 = b - A1 x0, z0 = M^-1 r0, rho = r.z, ||r||^2, ||b||^2; p := 0, beta := 0
+// (the first k_pupdate then gives p0 = z0).
+__global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+                                                  cudaGraphConditionalHandle h_while) {
+  __shared__ double smem[3 * 32];
+  __shared__ int s_flag;
+  const Ctx c = *ctxp;
+  double acc[3] = {0.0, 0.0, 0.0};
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double bi = c.b[i];
+        const double ri = bi - spmv_row<false>(c.A, c.x, i, c.x[i]);
+        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+        c.r[i] = ri;
+        c.p[i] = 0.0;
+        acc[0] = fma(ri, zi, acc[0]);
+        acc[1] = fma(ri, ri, acc[1]);
+        acc[2] = fma(bi, bi, acc[2]);
+      }
+    }
+  }
+  if (grid_sum_last_block<3>(acc, partials, &ctl->ticket[0], smem, &s_flag) && threadIdx.x == 0) {
+    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->bb = acc[2];
+    ctl->tol2 = c.rtol * c.rtol * acc[2];
+    ctl->sw2 = c.rtol * acc[2];                  // (sqrt(rtol) ||b||)^2, eq. (14a) relative (R-G8)
+    ctl->beta = 0.0; ctl->alpha = 0.0;
+    ctl->tt = acc[1]; ctl->tt_prev = acc[1]; ctl->rr_prev_eval = acc[1];
+    ctl->stage = (c.precision == CUTH_MIXED) ? 0 : 1;
+    unsigned go = 1u;
+    if (acc[2] == 0.0) { ctl->zero_rhs = 1; ctl->status = CUTH_SOLVE_CONVERGED; ctl->tt = 0.0; ctl->rr = 0.0; go = 0u; }
+    else if (acc[1] <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }   // r0 IS the true residual
+    else if (!(acc[0] == acc[0]) || !(acc[1] == acc[1])) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
+    cudaGraphSetConditional(h_while, go);
+  }
+}
+
+// Alg. 1 line 12 (with line 10 recomputed): p = M^-1 r + beta p.
+__global__ void __launch_bounds__(kThreads) k_pupdate(const Ctx* __restrict__ ctxp, const Ctl* __restrict__ ctl) {
+  const Ctx c = *ctxp;
+  const double beta = ctl->beta;
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double ri = c.r[i];
+        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+        c.p[i] = fma(beta, c.p[i], zi);
+      }
+    }
+  }
+}
+
+// Alg. 1 line 6 + the p.mu half of line 7: mu = A p (stage-dependent operator), pAp = p.mu.
+template <bool MIXED>
+__device__ __forceinline__ void spmv_dot_body(const Ctx& c, double& acc) {
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double pi = c.p[i];
+        const double m = spmv_row<MIXED>(c.A, c.p, i, pi);
+        c.mu[i] = m;
+        acc = fma(pi, m, acc);
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(kThreads) k_spmv_dot(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
+  __shared__ double smem[32];
+  __shared__ int s_flag;
+  const Ctx c = *ctxp;
+  double acc[1] = {0.0};
+  if (ctl->stage == 0) spmv_dot_body<true>(c, acc[0]);
+  else spmv_dot_body<false>(c, acc[0]);
+  if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
+    const double pAp = acc[0];
+    ctl->pAp = pAp;
+    const double rho = ctl->rho;
+    if (!(pAp > 0.0) || !(pAp <= 1.79e308) || !(rho == rho)) {
+      ctl->alpha = 0.0;
+      ctl->status = CUTH_SOLVE_BREAKDOWN;
+    } else {
+      ctl->alpha = rho / pAp;            // Alg. 1 line 7
+    }
+  }
+}
+
+// Alg. 1 lines 8-11: x += alpha p, r -= alpha mu, z = M^-1 r, rho' = r.z, ||r||^2; the last block
+// forms beta, advances the iteration counter and takes the loop / policy decisions.
+__global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+                                                    cudaGraphConditionalHandle h_while,
+                                                    cudaGraphConditionalHandle h_if) {
+  __shared__ double smem[2 * 32];
+  __shared__ int s_flag;
+  const Ctx c = *ctxp;
+  const double alpha = ctl->alpha;
+  double acc[2] = {0.0, 0.0};
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double pi = c.p[i], mi = c.mu[i];
+        const double xi = fma(alpha, pi, c.x[i]);
+        const double ri = fma(-alpha, mi, c.r[i]);
+        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+        c.x[i] = xi;
+        c.r[i] = ri;
+        acc[0] = fma(ri, zi, acc[0]);
+        acc[1] = fma(ri, ri, acc[1]);
+      }
+    }
+  }
+  if (grid_sum_last_block<2>(acc, partials + kMaxBlocks, &ctl->ticket[2], smem, &s_flag) && threadIdx.x == 0) {
+    unsigned go = 1u, want = 0u;
+    if (ctl->status == CUTH_SOLVE_BREAKDOWN) {
+      go = 0u;
+    } else {
+      const double rho_new = acc[0], rr = acc[1];
+      ctl->beta = rho_new / ctl->rho;      // Alg. 1 line 11
+      ctl->rho = rho_new;
+      ctl->rr = rr;
+      const int it = ctl->it + 1;          // Alg. 1 line 13
+      ctl->it = it;
+      const int since = ctl->since_eval + 1;
+      ctl->since_eval = since;
+      const bool conv_rec = rr <= ctl->tol2;
+      const bool early = ctl->stage == 0;
+      const bool c14a = early && rr <= ctl->sw2;
+      const bool periodic = early && since >= c.period;
+      const bool capped = it >= c.max_iters;
+      const bool bad = !(rr == rr) || !(rho_new == rho_new);
+      ctl->conv_rec = conv_rec ? 1 : 0;
+      if (bad) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
+      else if (conv_rec || c14a || periodic || capped) want = 1u;
+    }
+    ctl->want_true = (int)want;
+    cudaGraphSetConditional(h_while, go);
+    cudaGraphSetConditional(h_if, want);
+  }
+}
+
+// True residual: t = b - A1 x in fp64 (stored in the mu buffer, which is dead here),
+// ||t||^2 and the drift ||t - r||^2; the last block applies the stopping rule and eq. (14a)-(14c).
+__global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+                                                        cudaGraphConditionalHandle h_while) {
+  __shared__ double smem[2 * 32];
+  __shared__ int s_flag;
+  const Ctx c = *ctxp;
+  double acc[2] = {0.0, 0.0};
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double ti = c.b[i] - spmv_row<false>(c.A, c.x, i, c.x[i]);
+        const double di = ti - c.r[i];
+        c.mu[i] = ti;
+        acc[0] = fma(ti, ti, acc[0]);
+        acc[1] = fma(di, di, acc[1]);
+      }
+    }
+  }
+  if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[3], smem, &s_flag) && threadIdx.x == 0) {
+    const double tt = acc[0], dd = acc[1];
+    const double rr = ctl->rr;
+    ctl->tt = tt; ctl->dd = dd;
+    ctl->evals += 1;
+    ctl->since_eval = 0;
+    unsigned go = 1u;
+    int restart = 0;
+    if (tt <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }
+    else if (ctl->it >= c.max_iters) { ctl->status = CUTH_SOLVE_MAX_ITERS; go = 0u; }
+    else if (ctl->stage == 1) {
+      // late stage: the recursive residual said "converged", the true one disagrees -> replace r,
+      // restart the direction (same rule as the oracle), keep iterating.
+      if (ctl->conv_rec) restart = 1;
+    } else {
+      int reason = 0;
+      if (ctl->conv_rec) reason = 4;
+      else if (rr <= ctl->sw2) reason = 1;                                        // (14a)
+      else if (dd >= 0.25 * tt) reason = 3;                                       // (14c): ||t-r|| >= 0.5 ||t||
+      else if (tt > 0.81 * ctl->tt_prev && rr <= 0.81 * ctl->rr_prev_eval) reason = 2;   // (14b), R-G9
+      if (reason) {
+        ctl->stage = 1; ctl->promotions += 1; ctl->switch_reason = reason; ctl->switch_it = ctl->it;
+        restart = 1;                                                              // hot restart
+      }
+    }
+    ctl->tt_prev = tt;
+    ctl->rr_prev_eval = rr;
+    ctl->restart = restart;
+    cudaGraphSetConditional(h_while, go);
+  }
+}
+
+// Hot restart: r := t (= b - A1 x, sitting in mu), z = M^-1 r, rho = r.z, beta := 0 so that
+// the next k_pupdate gives p = z (p's defining equation, Alg. 1 line 3).  No-op unless ctl->restart.
+__global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
+  __shared__ double smem[2 * 32];
+  __shared__ int s_flag;
+  if (!ctl->restart) return;
+  const Ctx c = *ctxp;
+  double acc[2] = {0.0, 0.0};
+  CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < c.A.n) {
+        const double ri = c.mu[i];
+        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+        c.r[i] = ri;
+        acc[0] = fma(ri, zi, acc[0]);
+        acc[1] = fma(ri, ri, acc[1]);
+      }
+    }
+  }
+  if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[4], smem, &s_flag) && threadIdx.x == 0) {
+    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->beta = 0.0; ctl->restart = 0; ctl->conv_rec = 0;
+  }
+}
+
+// Writes the result record; x := 0 when b = 0.
+__global__ void __launch_bounds__(kThreads) k_finalize(const Ctx* __restrict__ ctxp, Ctl* ctl) {
+  const Ctx c = *ctxp;
+  if (ctl->zero_rhs) {
+    CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        if (i < c.A.n) c.x[i] = 0.0;
+      }
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    cuth_result_t res;
+    res.status = ctl->status == CUTH_SOLVE_RUNNING ? CUTH_SOLVE_MAX_ITERS : ctl->status;
+    res.iterations = ctl->it;
+    res.promotions = ctl->promotions;
+    res.true_resid_evals = ctl->evals;
+    const double bb = ctl->bb;
+    res.rel_resid_true = bb > 0.0 ? sqrt(ctl->tt / bb) : 0.0;
+    res.rel_resid_rec = bb > 0.0 ? sqrt(ctl->rr / bb) : 0.0;
+    res.switch_reason = ctl->switch_reason;
+    res.switch_iteration = ctl->switch_it;
+    *c.result = res;
+  }
+}
+
+}  // namespace cuth

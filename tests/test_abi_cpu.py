@@ -1,0 +1,66 @@
+"""No-GPU checks of the C-ABI boundary: the library loads, exports every symbol include/cuth.h
+declares, and its pure-host entry points (sizes, layout view, argument errors) behave."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cu():
+    from paper_2606_17850_b200 import build
+    build.build()
+    import paper_2606_17850_b200 as cu
+    return cu
+
+
+def test_exports_match_header(cu):
+    hdr = open(os.path.join(ROOT, "include", "cuth.h")).read()
+    declared = set(re.findall(r"\b(cuth_[a-z0-9_]+)\s*\(", hdr))
+    declared -= {"cuth_status_t"}
+    lib = cu.load_library()
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert declared == set(cu.exported_symbols())
+
+
+def test_layout_closed_forms_host_side(cu):
+    for nx, ny, nz in [(4, 3, 2), (32, 32, 8), (256, 256, 16), (4096, 4096, 8)]:
+        g = cu.Grid(nx, ny, nz, 1e-6, 1e-6, np.full(nz, 1e-6), None, 1e4)
+        n = nx * ny * nz
+        lib = cu.load_library()
+        ptr = (C.c_int64 * 5)()
+        off = (C.c_int64 * 4)()
+        rc = lib.cuth_dia_view(C.c_void_p(4096), g.ref(), None, None, None, ptr, off)
+        assert rc == 0
+        assert list(off) == [0, 1, nx, nx * ny]
+        assert list(ptr) == [0, n, 2 * n - 1, 3 * n - 1 - nx, 4 * n - 1 - nx - nx * ny]
+        e = ptr[4]
+        assert cu.cuth_dia_bytes(g) >= 8 * e + 4 * e + 8 * n
+        assert cu.cuth_workspace_bytes(g, cu.Opts()) >= 3 * 8 * n
+
+
+def test_degenerate_dims_rejected(cu):
+    for dims in [(1, 4, 4), (4, 1, 4), (4, 4, 1), (0, 4, 4)]:
+        g = cu.Grid(*dims, 1e-6, 1e-6, np.full(max(dims[2], 1), 1e-6), None, 1e4)
+        assert cu.cuth_dia_bytes(g) == 0
+        lib = cu.load_library()
+        assert lib.cuth_build_dia(g.ref(), C.c_void_p(4096), 1 << 20, None) == -2   # CUTH_ERR_DIMS
+    g = cu.Grid(4, 4, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
+    lib = cu.load_library()
+    assert lib.cuth_build_dia(g.ref(), None, 1 << 20, None) == -1                   # NULL
+    assert lib.cuth_spmv(C.c_void_p(4096), g.ref(), 7, C.c_void_p(4096), C.c_void_p(8192), None) == -3
+    assert lib.cuth_spmv(C.c_void_p(4096), g.ref(), 0, C.c_void_p(4100), C.c_void_p(8192), None) == -5
+
+
+def test_no_cpu_fallback_without_device(cu):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    g = cu.Grid(4, 4, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
+    with pytest.raises(RuntimeError):
+        cu.DiaMatrix(g)
