@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- PCG time-to-solution and HBM roofline of the cuth hot path on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--precision fp64|mixed]
+  python bench.py --impl reference ...        # the CPU oracle on the host cores, bounded sample
+
+One "step" = one whole solve of the workload (cuth_pcg_solve to a verified true relative residual
+<= 1e-8; for config 5: one backward-Euler step) on synthetic seeded inputs (workloads/).  The default
+workload is BASELINE.json configs[2] (1024x1024x16, 16.8 M unknowns): the first of the two grids the
+metric's HBM target is quoted on, and the largest whose full solve keeps the default run within
+minutes.  N > 1: independent replicas, one per GPU ("replicas only", no collective on
+the data path); the time is the max over ranks.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "pcg_time_to_solution"
+UNIT = "s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def m_ratio(w):
+    return (4 * w.n - 1 - w.nx - w.nx * w.ny) / w.n
+
+
+def bytes_per_row(w, what):
+    """Algorithmic bytes per matrix row."""
+    m = m_ratio(w)
+    return {"spmv_fp64": 8 * m + 16, "spmv_mixed": 4 * (m - 1) + 16,
+            "iter_fp64": 8 * m + 88, "iter_mixed": 4 * (m - 1) + 88}[what]
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
+        "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown," \
+        "clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 8:
+                continue
+            try:
+                sm.append(float(c[0]))
+                mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm))
+        return out
+
+
+def cpu_oracle_sample(w, iters_for_extrapolation, budget_iters=None, out=None):
+    """Times the oracle (as it stands) on a bounded sample: a window of Alg.-1 iterations on the same
+    workload, extrapolated to the iteration count the solve needs."""
+    from oracle import oracle as O
+    t0 = time.time()
+    A = O.assemble_workload(w)
+    t_asm = time.time() - t0
+    b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
+    # size the window for ~10-20 s: ~176 B/row/iteration at a few GB/s per core
+    if budget_iters is None:
+        budget_iters = int(max(5, min(400, 1.2e9 / w.n)))
+    t0 = time.time()
+    O.pcg_window(A, b, np.zeros(w.n), budget_iters)
+    dt = time.time() - t0
+    s_per_it = dt / (budget_iters + 1)
+    if out is not None:
+        out["A"], out["b"] = A, b
+    return {"value": s_per_it * iters_for_extrapolation, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{budget_iters} Alg.-1 iterations of the CSR fp64 oracle on {w.name} timed "
+                      f"({dt:.2f} s, {s_per_it * 1e3:.2f} ms/iteration), extrapolated to "
+                      f"{iters_for_extrapolation} iterations; CSR assembly {t_asm:.1f} s not included",
+            "s_per_iteration": s_per_it, "assembly_s": t_asm}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = W.make_workload(args.config)
+    from oracle import oracle as O
+    A = O.assemble_workload(w)
+    b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
+    iters = int(max(3, min(200, 2.5e8 / w.n)))
+    nominal = {1: 288, 2: 1462, 3: 4500, 4: 8000, 5: 550}[args.config]
+    for _ in range(args.warmup):
+        O.pcg_window(A, b, np.zeros(w.n), 1)
+    t0 = time.time()
+    for _ in range(args.steps):
+        O.pcg_window(A, b, np.zeros(w.n), iters)
+    dt = (time.time() - t0) / args.steps
+    s_it = dt / (iters + 1)
+    val = s_it * nominal
+    sample = (f"each step = {iters} Alg.-1 iterations of the CSR fp64 oracle on {w.name} "
+              f"({s_it * 1e3:.2f} ms/iteration), extrapolated to the nominal {nominal} iterations of this config")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_unknowns": w.n, "rtol": w.rtol},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--precision", default=None, choices=["fp64", "mixed"])
+    ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel-reps", type=int, default=20)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2606_17850_b200 as cu
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the cuth path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = W.make_workload(args.config)
+    mixed = w.mixed if args.precision is None else (args.precision == "mixed")
+    prec = cu.MIXED if mixed else cu.FP64
+    kap = w.kappa_cell if w.kappa_cell is not None else w.kappa_layer
+    kap_d = torch.from_numpy(np.ascontiguousarray(kap)).cuda()
+    g = cu.Grid(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, kap_d, w.h_top, w.cvol, w.dt)
+    A = cu.DiaMatrix(g)
+    opts = cu.Opts(precision=prec, rtol=w.rtol, max_iters=200000, true_resid_period=w.true_resid_period)
+    S = cu.Solver(A, opts)
+    stream = torch.cuda.current_stream()
+
+    b_host = torch.from_numpy(w.power).pin_memory()
+    x_host = torch.empty(w.n, dtype=torch.float64).pin_memory()
+    b = b_host.cuda()
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+
+    def one_solve():
+        x.zero_()
+        if w.transient:
+            S.step(b, x)
+        else:
+            S.solve(b, x)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing (value)
+    for _ in range(args.warmup):
+        one_solve()
+    res = S.result()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    results = []
+    for e0, e1 in ev:
+        x.zero_()
+        e0.record(stream)
+        if w.transient:
+            S.step(b, x)
+        else:
+            S.solve(b, x)
+        e1.record(stream)
+        results.append(None)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    res = S.result()
+    ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+    ms_per_step = float(np.mean(ms))
+    t = torch.tensor([ms_per_step], device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_per_step = float(t.item())
+
+    # ---- end-to-end through the public API with HOST buffers (pinned), copies inside the timed region
+    barrier()
+    e2e_ms = []
+    for _ in range(max(1, min(args.steps, 3))):
+        t0 = torch.cuda.Event(enable_timing=True)
+        t1 = torch.cuda.Event(enable_timing=True)
+        t0.record(stream)
+        b.copy_(b_host, non_blocking=True)
+        x.zero_()
+        if w.transient:
+            S.step(b, x)
+        else:
+            S.solve(b, x)
+        x_host.copy_(x, non_blocking=True)
+        t1.record(stream)
+        torch.cuda.synchronize()
+        e2e_ms.append(t0.elapsed_time(t1))
+    e2e_t = torch.tensor([float(np.mean(e2e_ms))], device="cuda")
+    if world > 1:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    x_final = x_host.numpy().copy()
+
+    # ---- dominant kernels timed one by one with CUDA events (same launch configuration as in the graph)
+    peak, peak_src = peaks()
+    kern = {}
+    cu.cuth_profile_kernel(S.work, g, -1)
+    names = {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"}
+    for kid, nm in names.items():
+        for _ in range(3):
+            cu.cuth_profile_kernel(S.work, g, kid)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.kernel_reps):
+            cu.cuth_profile_kernel(S.work, g, kid)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        kern[nm] = e0.elapsed_time(e1) / args.kernel_reps
+    # standalone SpMV (cuth_spmv), both precisions
+    y = torch.empty_like(x)
+    spmv = {}
+    for nm, pr in (("fp64", cu.FP64), ("mixed", cu.MIXED)):
+        for _ in range(3):
+            cu.cuth_spmv(A.buf, g, pr, b, y)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.kernel_reps):
+            cu.cuth_spmv(A.buf, g, pr, b, y)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        tms = e0.elapsed_time(e1) / args.kernel_reps
+        spmv[nm] = {"ms": tms, "gbs": bytes_per_row(w, "spmv_" + nm) * w.n / tms / 1e6}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    it = res.iterations
+    early = res.switch_iteration if (mixed and res.promotions) else (it if mixed else 0)
+    late = it - early
+    iter_bytes = (early * bytes_per_row(w, "iter_mixed") + late * bytes_per_row(w, "iter_fp64")) * w.n
+    iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
+    stage_fp64 = (not mixed) or res.promotions > 0     # operator the armed profile kernels ran with
+    spmv_key = "spmv_fp64" if stage_fp64 else "spmv_mixed"
+    dom_bytes = bytes_per_row(w, spmv_key) * w.n
+    dom_ms = kern["k_spmv_dot"]
+    launches = args.steps * (1 + 1 + 3 * it + 2 * res.true_resid_evals + 1 + (1 if w.transient else 0))
+
+    line = {
+        "metric": METRIC, "value": ms_per_step * 1e-3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz],
+                   "precision": "mixed" if mixed else "fp64", "rtol": w.rtol, "preconditioner": "jacobi",
+                   "l2_policy": "inputs larger than L2 (matrix + vectors = %.1f GB)" %
+                                ((8 * m_ratio(w) + 48) * w.n / 1e9),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "iterations": it, "promotions": res.promotions, "true_resid_evals": res.true_resid_evals,
+        "switch_reason": res.switch_reason, "switch_iteration": res.switch_iteration,
+        "rel_resid_true": res.rel_resid_true, "status": res.status_name,
+        "us_per_iteration": ms_per_step * 1e3 / max(it, 1),
+        "solves_per_s": world / (ms_per_step * 1e-3),
+        "roofline": {"bound": "hbm", "kernel": "k_spmv_dot (%s operator)" % ("fp64" if stage_fp64 else "fp32-stored"),
+                     "achieved": dom_bytes / dom_ms / 1e6, "peak": peak, "unit": "GB/s",
+                     "frac": dom_bytes / dom_ms / 1e6 / peak, "traffic": None, "peak_source": peak_src,
+                     "ms_per_launch": dom_ms, "algorithmic_bytes_per_launch": dom_bytes},
+        "roofline_iteration": {"bound": "hbm", "achieved": iter_gbs, "peak": peak, "unit": "GB/s",
+                               "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
+                               "algorithmic_bytes_per_solve": iter_bytes,
+                               "note": "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
+                                       "x iterations / whole-solve time, true-residual checks included in the time"},
+        "kernels_ms": kern, "spmv": spmv,
+        "e2e": {"value": float(e2e_t.item()) * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8),
+                "d2h_bytes_per_step": int(w.n * 8)},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        keep = {}
+        line["cpu_baseline"] = cpu_oracle_sample(w, it, out=keep)
+        # property check of the timed result against the ORACLE's matrix (not timed)
+        from oracle import oracle as O
+        Ao, bb = keep["A"], keep["b"]
+        line["oracle_true_rel_resid_of_gpu_x"] = float(np.linalg.norm(bb - O.spmv(Ao, x_final)) / np.linalg.norm(bb))
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -140,6 +140,13 @@ int cuth_version(void);
  * (used by bench.py to report gpu_launches = prologue + body * iterations + epilogue). */
 int cuth_launches_per_iteration(void);
 
+/* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is
+ * still in this workspace, outside the graph and with the graph's launch configuration, so that it
+ * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the
+ * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = fused x/r update + dots,
+ * 3 = true residual.  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
+int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -280,6 +280,27 @@ int cuth_transient_step(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   return solve_common(dia_D, grid, opts, nullptr, power_D, T_D, work_D, work_bytes, result_D, stream);
 }
 
+int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  if (!work_D) return CUTH_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
+  const int blocks = grid_blocks(L.n);
+  cudaGraphConditionalHandle h0 = 0;
+  switch (kernel_id) {
+    case -1: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl); break;
+    case 0: k_pupdate<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl); break;
+    case 1: k_spmv_dot<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
+    case 2: k_update<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 3: k_true_resid<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
+    default: return CUTH_ERR_VALUE;
+  }
+  CU(cudaGetLastError());
+  return CUTH_OK;
+}
+
 int cuth_release_workspace(const void* work_D) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);

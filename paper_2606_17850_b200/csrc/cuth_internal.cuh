@@ -75,7 +75,7 @@ struct Ctl {
   double rho, pAp, alpha, beta, rr, bb, tol2, sw2;
   double tt, dd, tt_prev, rr_prev_eval;
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
-  int32_t switch_reason, switch_it, conv_rec, zero_rhs, pad;
+  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph;
   unsigned int ticket[8];
 };
 

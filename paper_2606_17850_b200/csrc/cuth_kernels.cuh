@@ -236,8 +236,7 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       else if (conv_rec || c14a || periodic || capped) want = 1u;
     }
     ctl->want_true = (int)want;
-    cudaGraphSetConditional(h_while, go);
-    cudaGraphSetConditional(h_if, want);
+    if (!ctl->no_graph) { cudaGraphSetConditional(h_while, go); cudaGraphSetConditional(h_if, want); }
   }
 }
 
@@ -290,7 +289,7 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
     ctl->tt_prev = tt;
     ctl->rr_prev_eval = rr;
     ctl->restart = restart;
-    cudaGraphSetConditional(h_while, go);
+    if (!ctl->no_graph) cudaGraphSetConditional(h_while, go);
   }
 }
 
@@ -319,6 +318,9 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
     ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->beta = 0.0; ctl->restart = 0; ctl->conv_rec = 0;
   }
 }
+
+// Measurement hook support: marks the control block as "outside a graph".
+__global__ void k_mark_no_graph(Ctl* ctl) { ctl->no_graph = 1; ctl->restart = 0; }
 
 // Writes the result record; x := 0 when b = 0.
 __global__ void __launch_bounds__(kThreads) k_finalize(const Ctx* __restrict__ ctxp, Ctl* ctl) {
