@@ -162,6 +162,9 @@ def main():
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-reps", type=int, default=20)
+    ap.add_argument("--profile-iters", type=int, default=0,
+                    help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
+                         "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -272,6 +275,10 @@ def main():
         e1.record(stream)
         torch.cuda.synchronize()
         kern[nm] = e0.elapsed_time(e1) / args.kernel_reps
+    for _ in range(args.profile_iters):
+        for kid in (0, 1, 2):
+            cu.cuth_profile_kernel(S.work, g, kid)
+    torch.cuda.synchronize()
     # standalone SpMV (cuth_spmv), both precisions
     y = torch.empty_like(x)
     spmv = {}
