@@ -140,6 +140,11 @@ int cuth_version(void);
  * (used by bench.py to report gpu_launches = prologue + body * iterations + epilogue). */
 int cuth_launches_per_iteration(void);
 
+/* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching
+ * when one x-y plane of the six streamed arrays no longer fits L2, flat 1-D streaming otherwise),
+ * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
+int cuth_set_traversal(int mode);
+
 /* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is
  * still in this workspace, outside the graph and with the graph's launch configuration, so that it
  * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the

@@ -48,7 +48,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal"]
 
 _lib = None
 
@@ -87,6 +87,8 @@ def load_library():
     L.cuth_last_cuda_error.restype = C.c_char_p
     L.cuth_version.restype = C.c_int
     L.cuth_launches_per_iteration.restype = C.c_int
+    L.cuth_set_traversal.restype = C.c_int
+    L.cuth_set_traversal.argtypes = [C.c_int]
     L.cuth_profile_kernel.restype = C.c_int
     L.cuth_profile_kernel.argtypes = [vp, gp, C.c_int, vp]
     _lib = L
@@ -202,6 +204,10 @@ def cuth_release_workspace(work):
 def cuth_profile_kernel(work, grid: Grid, kernel_id: int, stream=None):
     _check(load_library().cuth_profile_kernel(_ptr(work), grid.ref(), int(kernel_id), stream or _stream()),
            "cuth_profile_kernel")
+
+
+def cuth_set_traversal(mode: int):
+    _check(load_library().cuth_set_traversal(int(mode)), "cuth_set_traversal")
 
 
 def cuth_version() -> int:

@@ -3,6 +3,8 @@
 // IF{ k_true_resid, k_restart } } -> k_finalize.  Nothing in it synchronises with the host.
 #include <cmath>
 #include <cstdio>
+#include <atomic>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -34,6 +36,23 @@ static int check_grid(const cuth_grid_t* g, DiaLayout* L) {
   return CUTH_OK;
 }
 
+static std::atomic<int> g_traversal{0};   // 0 auto, 1 flat, 2 z-march (cuth_set_traversal)
+
+// Traversal choice: the flat kernel relies on L2 to keep the +-nx*ny neighbours (two planes of six
+// arrays, 96 B per plane cell); beyond ~1/3 of the 126 MB L2 that fails and z-marching wins.
+static bool use_zmarch(const DiaLayout& L) {
+  const int mode = g_traversal.load();
+  if (mode == 1) return false;
+  if (mode == 2) return true;
+  return L.nxny >= (1 << 19);
+}
+
+static int stencil_blocks(const DiaLayout& L) {
+  if (!use_zmarch(L)) return -1;
+  const int64_t tiles = ((L.nx + ZTX - 1) / ZTX) * ((L.ny + ZTY - 1) / ZTY);
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
+}
+
 static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   const char* base = (const char*)dia_D;
   const double* v = (const double*)(base + L.o_vals);
@@ -46,6 +65,8 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   A.s_layer = lay + L.nz;
   A.cap_layer = lay + 2 * L.nz;
   A.n = L.n; A.nx = L.nx; A.nxny = L.nxny;
+  A.ny = (int32_t)L.ny; A.nz = (int32_t)L.nz;
+  A.zmarch = use_zmarch(L) ? 1 : 0; A.pad = 0;
   return A;
 }
 
@@ -62,6 +83,7 @@ struct GraphEntry {
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t exec = nullptr;
   int64_t n = 0;
+  int sblocks = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -79,8 +101,9 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
 
-static int build_graph(const Workspace& w, int64_t n, GraphEntry* out) {
+static int build_graph(const Workspace& w, int64_t n, int sblocks, GraphEntry* out) {
   const int blocks = grid_blocks(n);
+  if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
   CU(cudaGraphCreate(&g, 0));
   cudaGraphConditionalHandle h_while, h_if;
@@ -90,7 +113,7 @@ static int build_graph(const Workspace& w, int64_t n, GraphEntry* out) {
 
   cudaGraphNode_t n_init, n_while, n_fin;
   { void* a[] = {&ctx, &ctl, &partials, &h_while};
-    CU(add_kernel(g, &n_init, nullptr, 0, (void*)k_init, blocks, a)); }
+    CU(add_kernel(g, &n_init, nullptr, 0, (void*)k_init, sblocks, a)); }
   cudaGraphNodeParams wp = {};
   wp.type = cudaGraphNodeTypeConditional;
   wp.conditional.handle = h_while;
@@ -105,7 +128,7 @@ static int build_graph(const Workspace& w, int64_t n, GraphEntry* out) {
   { void* a[] = {&ctx, &ctl};
     CU(add_kernel(body, &n_p, nullptr, 0, (void*)k_pupdate, blocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials};
-    CU(add_kernel(body, &n_s, &n_p, 1, (void*)k_spmv_dot, blocks, a)); }
+    CU(add_kernel(body, &n_s, &n_p, 1, (void*)k_spmv_dot, sblocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
     CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update, blocks, a)); }
   cudaGraphNodeParams ip = {};
@@ -117,23 +140,24 @@ static int build_graph(const Workspace& w, int64_t n, GraphEntry* out) {
   cudaGraph_t ifb = ip.conditional.phGraph_out[0];
   cudaGraphNode_t n_t, n_r;
   { void* a[] = {&ctx, &ctl, &partials, &h_while};
-    CU(add_kernel(ifb, &n_t, nullptr, 0, (void*)k_true_resid, blocks, a)); }
+    CU(add_kernel(ifb, &n_t, nullptr, 0, (void*)k_true_resid, sblocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials};
     CU(add_kernel(ifb, &n_r, &n_t, 1, (void*)k_restart, blocks, a)); }
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
-static int get_graph(const Workspace& w, void* work_D, int64_t n, cudaGraphExec_t* ex) {
+static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
   cudaGetDevice(&dev);
-  if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev)) {
+  if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
+                               it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)))) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -141,7 +165,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, cudaGraphExec_
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, &e);
+    int rc = build_graph(w, n, sblocks, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -194,7 +218,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   cudaGraphExec_t ex;
-  rc = get_graph(w, work_D, L.n, &ex);
+  rc = get_graph(w, work_D, L.n, stencil_blocks(L), &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -260,7 +284,8 @@ int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const d
   if (precision != CUTH_FP64 && precision != CUTH_MIXED) return CUTH_ERR_VALUE;
   if (x_D == y_D) return CUTH_ERR_VALUE;
   DiaDev A = dev_view(dia_D, L);
-  const int blocks = grid_blocks(L.n);
+  const int sb = stencil_blocks(L);
+  const int blocks = sb > 0 ? sb : grid_blocks(L.n);
   if (precision == CUTH_MIXED) k_spmv_only<true><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
   else k_spmv_only<false><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
   CU(cudaGetLastError());
@@ -288,16 +313,23 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
   cudaStream_t st = (cudaStream_t)stream;
   Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
   const int blocks = grid_blocks(L.n);
+  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
   cudaGraphConditionalHandle h0 = 0;
   switch (kernel_id) {
     case -1: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl); break;
     case 0: k_pupdate<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl); break;
-    case 1: k_spmv_dot<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
+    case 1: k_spmv_dot<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 2: k_update<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
-    case 3: k_true_resid<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
+    case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
   }
   CU(cudaGetLastError());
+  return CUTH_OK;
+}
+
+int cuth_set_traversal(int mode) {
+  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
+  g_traversal.store(mode);
   return CUTH_OK;
 }
 

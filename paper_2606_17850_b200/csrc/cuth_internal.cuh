@@ -12,7 +12,7 @@ namespace cuth {
 constexpr int kAlign = 256;            // byte alignment of every section of the matrix object / workspace
 constexpr int kHeaderBytes = 512;
 constexpr uint64_t kMagic = 0x4355544844494131ull;  // "CUTHDIA1"
-constexpr int kMaxBlocks = 4096;       // upper bound on the grid of any reducing kernel
+constexpr int kMaxBlocks = 8192;       // upper bound on the grid of any reducing kernel
 constexpr int kNumPartialSlots = 4;    // partial-sum arrays (each kMaxBlocks doubles)
 
 // Host-computed placement of the sections inside the caller's matrix buffer.
@@ -55,6 +55,8 @@ struct DiaDev {
   const double* s_layer;    // exact row sums per layer: h dx dy [top] + C V / dt
   const double* cap_layer;  // C V / dt per layer (0 when steady)
   int64_t n, nx, nxny;
+  int32_t ny, nz;
+  int32_t zmarch, pad;      // 1: march in z per thread (plane neighbours in registers), 0: flat 1-D streaming
 };
 
 // Pointers and options of one solve; lives at the start of the workspace, written per call.

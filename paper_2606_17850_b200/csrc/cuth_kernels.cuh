@@ -55,16 +55,89 @@ __device__ __forceinline__ double spmv_row(const DiaDev& A, const double* __rest
        base += (int64_t)gridDim.x * (kThreads * kRows))
 
 // ---------------------------------------------------------------------------------------------
+// z-marching form of the same operator for grids whose x-y plane is too large for the +-nx*ny
+// neighbours to survive in L2 (cfg 3, cfg 4): a CTA owns a ZTX x ZTY tile of the plane, each thread
+// owns one (x, y) column and walks z = 0..nz-1 keeping v[z-1], v[z], v[z+1] and D3[z-1] in
+// registers, so every matrix element and every vector element is fetched from HBM exactly once;
+// the in-plane neighbours (+-1, +-nx) come through L1/L2.
+constexpr int ZTX = 64, ZTY = 4;   // ZTX * ZTY == kThreads
+static_assert(ZTX * ZTY == kThreads, "tile must match the block size");
+
+template <bool MIXED, class F>
+__device__ __forceinline__ void zmarch_apply(const DiaDev& A, const double* __restrict__ v, F&& f) {
+  const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
+  const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
+  const int tiles_x = (nxi + ZTX - 1) / ZTX, tiles_y = (nyi + ZTY - 1) / ZTY;
+  const int ntiles = tiles_x * tiles_y;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int bx = t % tiles_x, by = t / tiles_x;
+    const int x = bx * ZTX + tx, y = by * ZTY + ty;
+    if (x >= nxi || y >= nyi) continue;
+    const int64_t c = x + nx * (int64_t)y;
+    double v_lo = 0.0, v_c = v[c];
+    double a3l = 0.0;     // D3[i - np] (fp64) or its fp32 value promoted
+#pragma unroll 2
+    for (int z = 0; z < nz; ++z) {
+      const int64_t i = c + (int64_t)z * np;
+      const bool up3 = z + 1 < nz, lo3 = z > 0;
+      const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx;
+      double acc, a3u, v_hi;
+      if (!MIXED) {
+        const double a0 = A.d0[i];
+        const double a1u = up1 ? A.d1[i] : 0.0, a1l = lo1 ? A.d1[i - 1] : 0.0;
+        const double a2u = up2 ? A.d2[i] : 0.0, a2l = lo2 ? A.d2[i - nx] : 0.0;
+        a3u = up3 ? A.d3[i] : 0.0;
+        v_hi = up3 ? v[i + np] : 0.0;
+        const double v1u = up1 ? v[i + 1] : 0.0, v1l = lo1 ? v[i - 1] : 0.0;
+        const double v2u = up2 ? v[i + nx] : 0.0, v2l = lo2 ? v[i - nx] : 0.0;
+        acc = a0 * v_c;
+        acc = fma(a1u, v1u, acc); acc = fma(a1l, v1l, acc);
+        acc = fma(a2u, v2u, acc); acc = fma(a2l, v2l, acc);
+        acc = fma(a3u, v_hi, acc); acc = fma(a3l, v_lo, acc);
+      } else {
+        const float g1u = up1 ? A.f1[i] : 0.f, g1l = lo1 ? A.f1[i - 1] : 0.f;
+        const float g2u = up2 ? A.f2[i] : 0.f, g2l = lo2 ? A.f2[i - nx] : 0.f;
+        a3u = up3 ? (double)A.f3[i] : 0.0;
+        v_hi = up3 ? v[i + np] : v_c;
+        const double v1u = up1 ? v[i + 1] : v_c, v1l = lo1 ? v[i - 1] : v_c;
+        const double v2u = up2 ? v[i + nx] : v_c, v2l = lo2 ? v[i - nx] : v_c;
+        acc = A.s_layer[z] * v_c;
+        acc = fma((double)g1u, v1u - v_c, acc); acc = fma((double)g1l, v1l - v_c, acc);
+        acc = fma((double)g2u, v2u - v_c, acc); acc = fma((double)g2l, v2l - v_c, acc);
+        acc = fma(a3u, v_hi - v_c, acc);
+        acc = fma(a3l, (lo3 ? v_lo : v_c) - v_c, acc);
+      }
+      f(i, v_c, acc);
+      v_lo = v_c; v_c = v_hi; a3l = a3u;
+    }
+  }
+}
+
+// y_i = (A v)_i handed to f(i, v_i, y_i) for every row, with the traversal chosen at build time.
+template <bool MIXED, class F>
+__device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restrict__ v, F&& f) {
+  if (A.zmarch) {
+    zmarch_apply<MIXED>(A, v, f);
+  } else {
+    CUTH_TILE_LOOP(A.n) {
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        if (i < A.n) {
+          const double vi = v[i];
+          f(i, vi, spmv_row<MIXED>(A, v, i, vi));
+        }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Standalone SpMV (cuth_spmv).
 template <bool MIXED>
 __global__ void __launch_bounds__(kThreads) k_spmv_only(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
-  CUTH_TILE_LOOP(A.n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < A.n) y[i] = spmv_row<MIXED>(A, x, i, x[i]);
-    }
-  }
+  apply_A<MIXED>(A, x, [&](int64_t i, double, double yi) { y[i] = yi; });
 }
 
 // Writes the per-call context and clears the control block (plain launch before the graph).
@@ -101,22 +174,16 @@ __global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp,
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   double acc[3] = {0.0, 0.0, 0.0};
-  CUTH_TILE_LOOP(c.A.n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < c.A.n) {
-        const double bi = c.b[i];
-        const double ri = bi - spmv_row<false>(c.A, c.x, i, c.x[i]);
-        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
-        c.r[i] = ri;
-        c.p[i] = 0.0;
-        acc[0] = fma(ri, zi, acc[0]);
-        acc[1] = fma(ri, ri, acc[1]);
-        acc[2] = fma(bi, bi, acc[2]);
-      }
-    }
-  }
+  apply_A<false>(c.A, c.x, [&](int64_t i, double, double ax) {
+    const double bi = c.b[i];
+    const double ri = bi - ax;
+    const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+    c.r[i] = ri;
+    c.p[i] = 0.0;
+    acc[0] = fma(ri, zi, acc[0]);
+    acc[1] = fma(ri, ri, acc[1]);
+    acc[2] = fma(bi, bi, acc[2]);
+  });
   if (grid_sum_last_block<3>(acc, partials, &ctl->ticket[0], smem, &s_flag) && threadIdx.x == 0) {
     ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->bb = acc[2];
     ctl->tol2 = c.rtol * c.rtol * acc[2];
@@ -152,18 +219,10 @@ __global__ void __launch_bounds__(kThreads) k_pupdate(const Ctx* __restrict__ ct
 // Alg. 1 line 6 + the p.mu half of line 7: mu = A p (stage-dependent operator), pAp = p.mu.
 template <bool MIXED>
 __device__ __forceinline__ void spmv_dot_body(const Ctx& c, double& acc) {
-  CUTH_TILE_LOOP(c.A.n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < c.A.n) {
-        const double pi = c.p[i];
-        const double m = spmv_row<MIXED>(c.A, c.p, i, pi);
-        c.mu[i] = m;
-        acc = fma(pi, m, acc);
-      }
-    }
-  }
+  apply_A<MIXED>(c.A, c.p, [&](int64_t i, double pi, double m) {
+    c.mu[i] = m;
+    acc = fma(pi, m, acc);
+  });
 }
 
 __global__ void __launch_bounds__(kThreads) k_spmv_dot(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
@@ -248,19 +307,13 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   double acc[2] = {0.0, 0.0};
-  CUTH_TILE_LOOP(c.A.n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < c.A.n) {
-        const double ti = c.b[i] - spmv_row<false>(c.A, c.x, i, c.x[i]);
-        const double di = ti - c.r[i];
-        c.mu[i] = ti;
-        acc[0] = fma(ti, ti, acc[0]);
-        acc[1] = fma(di, di, acc[1]);
-      }
-    }
-  }
+  apply_A<false>(c.A, c.x, [&](int64_t i, double, double ax) {
+    const double ti = c.b[i] - ax;
+    const double di = ti - c.r[i];
+    c.mu[i] = ti;
+    acc[0] = fma(ti, ti, acc[0]);
+    acc[1] = fma(di, di, acc[1]);
+  });
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[3], smem, &s_flag) && threadIdx.x == 0) {
     const double tt = acc[0], dd = acc[1];
     const double rr = ctl->rr;

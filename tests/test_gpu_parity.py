@@ -13,6 +13,15 @@ from gpu_util import grid_from_workload, to_dev, gpu_solve
 
 pytestmark = pytest.mark.gpu
 
+
+@pytest.fixture(params=["flat", "zmarch"], autouse=True)
+def traversal(request):
+    """Every parity case runs with both grid traversals of the kernels that apply A."""
+    import paper_2606_17850_b200 as cu
+    cu.cuth_set_traversal({"flat": 1, "zmarch": 2}[request.param])
+    yield request.param
+    cu.cuth_set_traversal(0)
+
 SMALL = [
     dict(cfg=1, nx=4, ny=3, nz=2, n_hot=1),
     dict(cfg=1, nx=7, ny=2, nz=5, n_hot=1),
