@@ -135,10 +135,10 @@ const char* cuth_last_cuda_error(void);
 /* Library version, e.g. 10000 = 1.0.0 */
 int cuth_version(void);
 
-/* Number of kernel launches the last cuth_pcg_solve/cuth_transient_step on this workspace will
- * have made is data dependent; this returns the launches per PCG iteration of the graph body
- * (used by bench.py to report gpu_launches = prologue + body * iterations + epilogue). */
-int cuth_launches_per_iteration(void);
+/* Kernel launches per PCG iteration of the graph body for this grid (2 on the fused path used for
+ * large planes, 3 on the flat path); bench.py reports gpu_launches = prologue + this * iterations +
+ * true-residual branches + epilogue. */
+int cuth_launches_per_iteration(const cuth_grid_t* grid);
 
 /* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching
  * when one x-y plane of the six streamed arrays no longer fits L2, flat 1-D streaming otherwise),
@@ -148,8 +148,8 @@ int cuth_set_traversal(int mode);
 /* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is
  * still in this workspace, outside the graph and with the graph's launch configuration, so that it
  * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the
- * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = fused x/r update + dots,
- * 3 = true residual.  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
+ * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual,
+ * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
 int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
 
 #ifdef __cplusplus

@@ -9,7 +9,7 @@ from typing import Optional
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libcuth.so")
+LIB_PATH = os.environ.get("CUTH_LIB", os.path.join(HERE, "libcuth.so"))   # CUTH_LIB: developer override
 
 FP64, MIXED = 0, 1
 PRECOND_NONE, PRECOND_JACOBI = 0, 1
@@ -87,6 +87,7 @@ def load_library():
     L.cuth_last_cuda_error.restype = C.c_char_p
     L.cuth_version.restype = C.c_int
     L.cuth_launches_per_iteration.restype = C.c_int
+    L.cuth_launches_per_iteration.argtypes = [gp]
     L.cuth_set_traversal.restype = C.c_int
     L.cuth_set_traversal.argtypes = [C.c_int]
     L.cuth_profile_kernel.restype = C.c_int
@@ -214,8 +215,8 @@ def cuth_version() -> int:
     return int(load_library().cuth_version())
 
 
-def cuth_launches_per_iteration() -> int:
-    return int(load_library().cuth_launches_per_iteration())
+def cuth_launches_per_iteration(grid: Grid) -> int:
+    return int(load_library().cuth_launches_per_iteration(grid.ref()))
 
 
 # ------------------------------------------------------------------ convenience holders (allocation only)

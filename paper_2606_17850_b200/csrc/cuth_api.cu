@@ -1,6 +1,9 @@
 // cuth_api.cu -- the C ABI of include/cuth.h: argument checks, CUDA-graph construction, launches.
-// The PCG loop is ONE CUDA graph per workspace: k_init -> WHILE{ k_pupdate, k_spmv_dot, k_update,
-// IF{ k_true_resid, k_restart } } -> k_finalize.  Nothing in it synchronises with the host.
+// The PCG loop is ONE CUDA graph per workspace.  Nothing in it synchronises with the host.
+//   small planes (flat traversal):  k_init -> WHILE{ k_pupdate, k_spmv_dot, k_update<x>,
+//                                   IF{ k_true_resid, k_restart } } -> k_finalize
+//   large planes (fused path):      k_init -> WHILE{ k_fused_pspmv, k_update<no x>,
+//                                   IF{ k_flush_x, k_true_resid, k_restart } } -> k_finalize
 #include <cmath>
 #include <cstdio>
 #include <atomic>
@@ -10,7 +13,7 @@
 #include <string>
 #include <unordered_map>
 
-#include "cuth_kernels.cuh"
+#include "cuth_fused.cuh"
 
 namespace cuth {
 
@@ -53,6 +56,11 @@ static int stencil_blocks(const DiaLayout& L) {
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
+static int fused_blocks(const DiaLayout& L) {
+  const int64_t tiles = ((L.nx + FTX - 1) / FTX) * ((L.ny + FTY - 1) / FTY);
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
+}
+
 static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   const char* base = (const char*)dia_D;
   const double* v = (const double*)(base + L.o_vals);
@@ -84,6 +92,7 @@ struct GraphEntry {
   cudaGraphExec_t exec = nullptr;
   int64_t n = 0;
   int sblocks = 0;
+  int fblocks = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -101,7 +110,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
 
-static int build_graph(const Workspace& w, int64_t n, int sblocks, GraphEntry* out) {
+static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -125,12 +134,19 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, GraphEntry* o
     CU(add_kernel(g, &n_fin, &n_while, 1, (void*)k_finalize, blocks, a)); }
 
   cudaGraphNode_t n_p, n_s, n_u, n_if;
-  { void* a[] = {&ctx, &ctl};
-    CU(add_kernel(body, &n_p, nullptr, 0, (void*)k_pupdate, blocks, a)); }
-  { void* a[] = {&ctx, &ctl, &partials};
-    CU(add_kernel(body, &n_s, &n_p, 1, (void*)k_spmv_dot, sblocks, a)); }
-  { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
-    CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update, blocks, a)); }
+  if (fblocks > 0) {
+    { void* a[] = {&ctx, &ctl, &partials};
+      CU(add_kernel(body, &n_s, nullptr, 0, (void*)k_fused_pspmv, fblocks, a)); }
+    { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
+      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a)); }
+  } else {
+    { void* a[] = {&ctx, &ctl};
+      CU(add_kernel(body, &n_p, nullptr, 0, (void*)k_pupdate, blocks, a)); }
+    { void* a[] = {&ctx, &ctl, &partials};
+      CU(add_kernel(body, &n_s, &n_p, 1, (void*)k_spmv_dot, sblocks, a)); }
+    { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
+      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<true>, blocks, a)); }
+  }
   cudaGraphNodeParams ip = {};
   ip.type = cudaGraphNodeTypeConditional;
   ip.conditional.handle = h_if;
@@ -138,26 +154,31 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, GraphEntry* o
   ip.conditional.size = 1;
   CU(cudaGraphAddNode(&n_if, body, &n_u, 1, &ip));
   cudaGraph_t ifb = ip.conditional.phGraph_out[0];
-  cudaGraphNode_t n_t, n_r;
+  cudaGraphNode_t n_f, n_t, n_r;
+  if (fblocks > 0) {
+    void* a[] = {&ctx, &ctl};
+    CU(add_kernel(ifb, &n_f, nullptr, 0, (void*)k_flush_x, blocks, a));
+  }
   { void* a[] = {&ctx, &ctl, &partials, &h_while};
-    CU(add_kernel(ifb, &n_t, nullptr, 0, (void*)k_true_resid, sblocks, a)); }
+    CU(add_kernel(ifb, &n_t, fblocks > 0 ? &n_f : nullptr, fblocks > 0 ? 1 : 0, (void*)k_true_resid, sblocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials};
     CU(add_kernel(ifb, &n_r, &n_t, 1, (void*)k_restart, blocks, a)); }
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
-static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, cudaGraphExec_t* ex) {
+static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
   cudaGetDevice(&dev);
   if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
-                               it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)))) {
+                               it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
+                               it->second.fblocks != fblocks)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -165,7 +186,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, c
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -208,7 +229,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   memset(&c, 0, sizeof c);
   c.A = A;
   c.b = transient ? w.b : b_D;
-  c.x = x_D; c.r = w.r; c.p = w.p; c.mu = w.mu;
+  c.x = x_D; c.r = w.r; c.p = w.p; c.p2 = w.p2; c.mu = w.mu;
   c.result = result_D;
   c.rtol = opts->rtol;
   c.precision = opts->precision;
@@ -218,7 +239,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   cudaGraphExec_t ex;
-  rc = get_graph(w, work_D, L.n, stencil_blocks(L), &ex);
+  rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -319,7 +340,9 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case -1: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl); break;
     case 0: k_pupdate<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl); break;
     case 1: k_spmv_dot<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
-    case 2: k_update<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 4: k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
+    case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
   }
@@ -348,6 +371,10 @@ const char* cuth_last_cuda_error(void) { return g_last_err.c_str(); }
 
 int cuth_version(void) { return 10000; }
 
-int cuth_launches_per_iteration(void) { return 3; }
+int cuth_launches_per_iteration(const cuth_grid_t* grid) {
+  DiaLayout L;
+  if (!make_layout(grid, &L)) return 0;
+  return use_zmarch(L) ? 2 : 3;
+}
 
 }  // extern "C"

@@ -66,6 +66,7 @@ struct Ctx {
   double* x;
   double* r;
   double* p;
+  double* p2;      // second direction buffer (fused path ping-pongs p between p and p2)
   double* mu;
   cuth_result_t* result;
   double rtol;
@@ -76,13 +77,14 @@ struct Ctx {
 struct Ctl {
   double rho, pAp, alpha, beta, rr, bb, tol2, sw2;
   double tt, dd, tt_prev, rr_prev_eval;
+  double xalpha;   // pending x += xalpha * p (fused path defers Alg. 1 line 8 by one kernel)
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
-  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph;
+  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, pad2, pad3;
   unsigned int ticket[8];
 };
 
 struct Workspace {
-  Ctx* ctx; Ctl* ctl; double* partials; double* r; double* p; double* mu; double* b;
+  Ctx* ctx; Ctl* ctl; double* partials; double* r; double* p; double* p2; double* mu; double* b;
   size_t bytes;
 };
 
@@ -95,6 +97,7 @@ inline Workspace carve_workspace(void* base, int64_t n, bool with_b) {
   w.partials = (double*)(c + o); o = align_up(o + sizeof(double) * kMaxBlocks * kNumPartialSlots);
   w.r = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
   w.p = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
+  w.p2 = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
   w.mu = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
   w.b = nullptr;
   if (with_b) { w.b = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
@@ -139,14 +142,17 @@ __device__ __forceinline__ bool grid_sum_last_block(double (&v)[NV], double* par
   block_sum<NV>(v, smem);
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int k = 0; k < NV; ++k) partials[k * kMaxBlocks + blockIdx.x] = v[k];
-    __threadfence();
-    unsigned int t = atomicAdd(ticket, 1u);
-    *s_flag = (t == gridDim.x - 1) ? 1 : 0;
+    for (int k = 0; k < NV; ++k) __stcg(&partials[k * kMaxBlocks + blockIdx.x], v[k]);
+    // Release-only ticket: orders the partial stores before the increment WITHOUT the L1 invalidation
+    // (CCTL.IVALL) that __threadfence() costs every CTA -- the in-plane stencil neighbours live in L1.
+    unsigned int t;
+    asm volatile("atom.release.gpu.global.add.u32 %0, [%1], %2;" : "=r"(t) : "l"(ticket), "r"(1u) : "memory");
+    const int last = (t == gridDim.x - 1) ? 1 : 0;
+    if (last) __threadfence();     // acquire side, paid by the single last CTA; partials are read with ld.cg
+    *s_flag = last;
   }
   __syncthreads();
   if (!*s_flag) return false;
-  __threadfence();
 #pragma unroll
   for (int k = 0; k < NV; ++k) {
     double a = 0.0;

@@ -60,7 +60,13 @@ __device__ __forceinline__ double spmv_row(const DiaDev& A, const double* __rest
 // owns one (x, y) column and walks z = 0..nz-1 keeping v[z-1], v[z], v[z+1] and D3[z-1] in
 // registers, so every matrix element and every vector element is fetched from HBM exactly once;
 // the in-plane neighbours (+-1, +-nx) come through L1/L2.
-constexpr int ZTX = 64, ZTY = 4;   // ZTX * ZTY == kThreads
+#ifndef CUTH_ZTX
+#define CUTH_ZTX 64
+#endif
+#ifndef CUTH_MINB
+#define CUTH_MINB 4
+#endif
+constexpr int ZTX = CUTH_ZTX, ZTY = kThreads / CUTH_ZTX;   // ZTX * ZTY == kThreads
 static_assert(ZTX * ZTY == kThreads, "tile must match the block size");
 
 template <bool MIXED, class F>
@@ -136,7 +142,7 @@ __device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restric
 // ---------------------------------------------------------------------------------------------
 // Standalone SpMV (cuth_spmv).
 template <bool MIXED>
-__global__ void __launch_bounds__(kThreads) k_spmv_only(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
+__global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_only(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
   apply_A<MIXED>(A, x, [&](int64_t i, double, double yi) { y[i] = yi; });
 }
 
@@ -225,7 +231,7 @@ __device__ __forceinline__ void spmv_dot_body(const Ctx& c, double& acc) {
   });
 }
 
-__global__ void __launch_bounds__(kThreads) k_spmv_dot(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
+__global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_dot(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
   __shared__ double smem[32];
   __shared__ int s_flag;
   const Ctx c = *ctxp;
@@ -247,6 +253,7 @@ __global__ void __launch_bounds__(kThreads) k_spmv_dot(const Ctx* __restrict__ c
 
 // Alg. 1 lines 8-11: x += alpha p, r -= alpha mu, z = M^-1 r, rho' = r.z, ||r||^2; the last block
 // forms beta, advances the iteration counter and takes the loop / policy decisions.
+template <bool UPDATE_X>
 __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                     cudaGraphConditionalHandle h_while,
                                                     cudaGraphConditionalHandle h_if) {
@@ -260,11 +267,9 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
     for (int k = 0; k < kRows; ++k) {
       const int64_t i = base + threadIdx.x + k * kThreads;
       if (i < c.A.n) {
-        const double pi = c.p[i], mi = c.mu[i];
-        const double xi = fma(alpha, pi, c.x[i]);
-        const double ri = fma(-alpha, mi, c.r[i]);
+        if (UPDATE_X) c.x[i] = fma(alpha, c.p[i], c.x[i]);
+        const double ri = fma(-alpha, c.mu[i], c.r[i]);
         const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
-        c.x[i] = xi;
         c.r[i] = ri;
         acc[0] = fma(ri, zi, acc[0]);
         acc[1] = fma(ri, ri, acc[1]);
@@ -320,6 +325,7 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
     ctl->tt = tt; ctl->dd = dd;
     ctl->evals += 1;
     ctl->since_eval = 0;
+    ctl->xalpha = 0.0;          // k_flush_x has just applied it (fused path)
     unsigned go = 1u;
     int restart = 0;
     if (tt <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }
@@ -378,6 +384,17 @@ __global__ void k_mark_no_graph(Ctl* ctl) { ctl->no_graph = 1; ctl->restart = 0;
 // Writes the result record; x := 0 when b = 0.
 __global__ void __launch_bounds__(kThreads) k_finalize(const Ctx* __restrict__ ctxp, Ctl* ctl) {
   const Ctx c = *ctxp;
+  const double xalpha = ctl->xalpha;
+  if (xalpha != 0.0 && !ctl->zero_rhs) {      // deferred x += alpha p of the last iteration (fused path)
+    const double* p = ctl->pcur ? c.p2 : c.p;
+    CUTH_TILE_LOOP(c.A.n) {
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        if (i < c.A.n) c.x[i] = fma(xalpha, p[i], c.x[i]);
+      }
+    }
+  }
   if (ctl->zero_rhs) {
     CUTH_TILE_LOOP(c.A.n) {
 #pragma unroll
