@@ -263,7 +263,10 @@ def main():
     peak, peak_src = peaks()
     kern = {}
     cu.cuth_profile_kernel(S.work, g, -1)
-    names = {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"}
+    fused = cu.cuth_launches_per_iteration(g) == 2
+    names = ({4: "k_fused_pspmv", 5: "k_update_nox", 3: "k_true_resid"} if fused else
+             {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"})
+    body_ids = (4, 5) if fused else (0, 1, 2)
     for kid, nm in names.items():
         for _ in range(3):
             cu.cuth_profile_kernel(S.work, g, kid)
@@ -276,7 +279,7 @@ def main():
         torch.cuda.synchronize()
         kern[nm] = e0.elapsed_time(e1) / args.kernel_reps
     for _ in range(args.profile_iters):
-        for kid in (0, 1, 2):
+        for kid in body_ids:
             cu.cuth_profile_kernel(S.work, g, kid)
     torch.cuda.synchronize()
     # standalone SpMV (cuth_spmv), both precisions
@@ -306,10 +309,16 @@ def main():
     iter_bytes = (early * bytes_per_row(w, "iter_mixed") + late * bytes_per_row(w, "iter_fp64")) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
     stage_fp64 = (not mixed) or res.promotions > 0     # operator the armed profile kernels ran with
-    spmv_key = "spmv_fp64" if stage_fp64 else "spmv_mixed"
-    dom_bytes = bytes_per_row(w, spmv_key) * w.n
-    dom_ms = kern["k_spmv_dot"]
-    launches = args.steps * (1 + 1 + 3 * it + 2 * res.true_resid_evals + 1 + (1 if w.transient else 0))
+    m = m_ratio(w)
+    if fused:      # K1: matrix + r, 1/D0, p, x read + p', mu, x written
+        dom_name, dom_ms = "k_fused_pspmv", kern["k_fused_pspmv"]
+        dom_bytes = ((8 * m if stage_fp64 else 4 * (m - 1)) + 56) * w.n
+    else:
+        dom_name, dom_ms = "k_spmv_dot", kern["k_spmv_dot"]
+        dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
+    per_it = 2 if fused else 3
+    per_eval = 3 if fused else 2
+    launches = args.steps * (1 + 1 + per_it * it + per_eval * res.true_resid_evals + 1 + (1 if w.transient else 0))
 
     line = {
         "metric": METRIC, "value": ms_per_step * 1e-3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -325,7 +334,7 @@ def main():
         "rel_resid_true": res.rel_resid_true, "status": res.status_name,
         "us_per_iteration": ms_per_step * 1e3 / max(it, 1),
         "solves_per_s": world / (ms_per_step * 1e-3),
-        "roofline": {"bound": "hbm", "kernel": "k_spmv_dot (%s operator)" % ("fp64" if stage_fp64 else "fp32-stored"),
+        "roofline": {"bound": "hbm", "kernel": "%s (%s operator)" % (dom_name, "fp64" if stage_fp64 else "fp32-stored"),
                      "achieved": dom_bytes / dom_ms / 1e6, "peak": peak, "unit": "GB/s",
                      "frac": dom_bytes / dom_ms / 1e6 / peak, "traffic": None, "peak_source": peak_src,
                      "ms_per_launch": dom_ms, "algorithmic_bytes_per_launch": dom_bytes},
