@@ -52,6 +52,23 @@ def bytes_per_row(w, what):
             "iter_fp64": 8 * m + 88, "iter_mixed": 4 * (m - 1) + 88}[what]
 
 
+def max_over_ranks(value_ms: float, world: int, device="cpu") -> float:
+    """Replicas-only multi-GPU timing: every rank times its own solve, the job's time is the MAX over
+    ranks (no data-path collective; this all_reduce of one float is measurement plumbing only)."""
+    if world <= 1:
+        return float(value_ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value_ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_seed_offset(rank: int) -> int:
+    """Each replica solves the same configuration (weak scaling: per-GPU work fixed)."""
+    return 0
+
+
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown," \
@@ -232,10 +249,7 @@ def main():
     res = S.result()
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     ms_per_step = float(np.mean(ms))
-    t = torch.tensor([ms_per_step], device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_per_step = float(t.item())
+    ms_per_step = max_over_ranks(ms_per_step, world, "cuda")
 
     # ---- end-to-end through the public API with HOST buffers (pinned), copies inside the timed region
     barrier()
@@ -254,9 +268,7 @@ def main():
         t1.record(stream)
         torch.cuda.synchronize()
         e2e_ms.append(t0.elapsed_time(t1))
-    e2e_t = torch.tensor([float(np.mean(e2e_ms))], device="cuda")
-    if world > 1:
-        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    e2e_ms_max = max_over_ranks(float(np.mean(e2e_ms)), world, "cuda")
     x_final = x_host.numpy().copy()
 
     # ---- dominant kernels timed one by one with CUDA events (same launch configuration as in the graph)
@@ -344,7 +356,7 @@ def main():
                                "note": "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv,
-        "e2e": {"value": float(e2e_t.item()) * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8),
+        "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8),
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,
     }
