@@ -29,6 +29,10 @@ sys.path.insert(0, ROOT)
 
 import workloads as W  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
+# kernel (profiles/r1b_cfg3_fp64_fused.md); null for workloads/kernels not captured.
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.4498e9}
+
 METRIC = "pcg_time_to_solution"
 UNIT = "s"
 
@@ -348,7 +352,8 @@ def main():
         "solves_per_s": world / (ms_per_step * 1e-3),
         "roofline": {"bound": "hbm", "kernel": "%s (%s operator)" % (dom_name, "fp64" if stage_fp64 else "fp32-stored"),
                      "achieved": dom_bytes / dom_ms / 1e6, "peak": peak, "unit": "GB/s",
-                     "frac": dom_bytes / dom_ms / 1e6 / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": dom_bytes / dom_ms / 1e6 / peak,
+                     "traffic": NCU_TRAFFIC_BYTES.get((w.name, dom_name, "fp64" if stage_fp64 else "mixed")), "peak_source": peak_src,
                      "ms_per_launch": dom_ms, "algorithmic_bytes_per_launch": dom_bytes},
         "roofline_iteration": {"bound": "hbm", "achieved": iter_gbs, "peak": peak, "unit": "GB/s",
                                "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
