@@ -183,6 +183,8 @@ def main():
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-reps", type=int, default=20)
+    ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
+                    help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
                          "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
@@ -203,6 +205,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
+    cu.cuth_set_traversal(args.traversal)
     w = W.make_workload(args.config)
     mixed = w.mixed if args.precision is None else (args.precision == "mixed")
     prec = cu.MIXED if mixed else cu.FP64

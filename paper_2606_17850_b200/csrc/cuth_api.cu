@@ -47,7 +47,7 @@ static bool use_zmarch(const DiaLayout& L) {
   const int mode = g_traversal.load();
   if (mode == 1) return false;
   if (mode == 2) return true;
-  return L.nxny >= (1 << 19);
+  return L.nxny >= (1 << 18);
 }
 
 static int stencil_blocks(const DiaLayout& L) {
@@ -236,6 +236,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.max_iters = opts->max_iters;
   c.period = opts->true_resid_period > 0 ? opts->true_resid_period : 20;
   c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
+  c.soft_restart = 1;         // promotion keeps p while the drift is small (DESIGN.md R-G11)
+  c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   cudaGraphExec_t ex;

@@ -70,7 +70,9 @@ struct Ctx {
   double* mu;
   cuth_result_t* result;
   double rtol;
+  double soft_drift2;   // soft restart allowed while ||t - r||^2 <= soft_drift2 * ||t||^2
   int32_t precision, max_iters, period, jacobi;
+  int32_t soft_restart, pad0;
 };
 
 // Scalars of the iteration; device resident, written only by "last block" epilogues.

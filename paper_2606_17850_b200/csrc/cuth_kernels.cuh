@@ -342,7 +342,10 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
       else if (tt > 0.81 * ctl->tt_prev && rr <= 0.81 * ctl->rr_prev_eval) reason = 2;   // (14b), R-G9
       if (reason) {
         ctl->stage = 1; ctl->promotions += 1; ctl->switch_reason = reason; ctl->switch_it = ctl->it;
-        restart = 1;                                                              // hot restart
+        // hot restart.  Small drift: r is recomputed, p keeps its history through its
+        // defining equation p = z + beta p ("preserving the established Krylov subspace");
+        // large drift ((14c)): the direction is rebuilt from scratch, p = z.
+        restart = (c.soft_restart && dd <= c.soft_drift2 * tt) ? 2 : 1;
       }
     }
     ctl->tt_prev = tt;
@@ -357,7 +360,8 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
 __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
   __shared__ double smem[2 * 32];
   __shared__ int s_flag;
-  if (!ctl->restart) return;
+  const int mode = ctl->restart;
+  if (!mode) return;
   const Ctx c = *ctxp;
   double acc[2] = {0.0, 0.0};
   CUTH_TILE_LOOP(c.A.n) {
@@ -374,7 +378,9 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
     }
   }
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[4], smem, &s_flag) && threadIdx.x == 0) {
-    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->beta = 0.0; ctl->restart = 0; ctl->conv_rec = 0;
+    // mode 1: beta = 0 => p = z.  mode 2: beta_k = rho(new r) / rho_k, with rho_k = rho_rec / beta_rec.
+    ctl->beta = (mode == 2 && ctl->rho > 0.0) ? ctl->beta * (acc[0] / ctl->rho) : 0.0;
+    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->restart = 0; ctl->conv_rec = 0;
   }
 }
 
