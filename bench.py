@@ -5,7 +5,7 @@
   python bench.py --impl reference ...        # the CPU oracle on the host cores, bounded sample
 
 One "step" = one whole solve of the workload (cuth_pcg_solve to a verified true relative residual
-<= 1e-8; for config 5: one backward-Euler step) on synthetic seeded inputs (workloads/).  The default
+<= 1e-8; for config 5: the whole 200-step backward-Euler trace) on synthetic seeded inputs (workloads/).  The default
 workload is BASELINE.json configs[2] (1024x1024x16, 16.8 M unknowns): the first of the two grids the
 metric's HBM target is quoted on, and the largest whose full solve keeps the default run within
 minutes.  N > 1: independent replicas, one per GPU ("replicas only", no collective on
@@ -183,6 +183,7 @@ def main():
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-reps", type=int, default=20)
+    ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,
@@ -217,17 +218,44 @@ def main():
     S = cu.Solver(A, opts)
     stream = torch.cuda.current_stream()
 
-    b_host = torch.from_numpy(w.power).pin_memory()
+    # Inputs.  Steady: one power map b.  Transient (cfg 5): the whole trace of n_steps power maps, each
+    # backward-Euler step warm-started from the previous one; ONE bench step = the whole trace.
+    nt = 1
+    if w.transient:
+        nt = args.transient_steps or w.n_steps
+        maps = [W.power_for_step(w, s + 1) for s in range(nt)]
+        b_host = torch.from_numpy(np.stack(maps)).pin_memory()
+        del maps
+    else:
+        b_host = torch.from_numpy(w.power).reshape(1, -1).pin_memory()
     x_host = torch.empty(w.n, dtype=torch.float64).pin_memory()
     b = b_host.cuda()
+    b_stage = torch.empty(w.n, dtype=torch.float64, device="cuda")
     x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    counters = torch.zeros(4, dtype=torch.int32, device="cuda")     # status, iterations, promotions, evals
+    early_acc = torch.zeros(1, dtype=torch.int32, device="cuda")   # iterations done on the fp32-stored operator
+    res_i32 = S.result_dev.view(torch.int32)
 
-    def one_solve():
+    def one_pass(from_host):
+        """One bench step: x0 = 0, then the solve (steady) or the nt-step trace (transient)."""
         x.zero_()
-        if w.transient:
-            S.step(b, x)
-        else:
-            S.solve(b, x)
+        counters.zero_()
+        early_acc.zero_()
+        for s in range(nt):
+            if from_host:
+                b_stage.copy_(b_host[s], non_blocking=True)
+                src = b_stage
+            else:
+                src = b[s]
+            if w.transient:
+                S.step(src, x)
+            else:
+                S.solve(src, x)
+            counters.add_(res_i32[:4])
+            if mixed:
+                early_acc.add_(torch.where(res_i32[2:3] > 0, res_i32[9:10], res_i32[1:2]))
+        if from_host:
+            x_host.copy_(x, non_blocking=True)
 
     def barrier():
         if world > 1:
@@ -236,27 +264,21 @@ def main():
 
     # ---- device-resident timing (value)
     for _ in range(args.warmup):
-        one_solve()
-    res = S.result()
+        one_pass(False)
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    results = []
     for e0, e1 in ev:
-        x.zero_()
         e0.record(stream)
-        if w.transient:
-            S.step(b, x)
-        else:
-            S.solve(b, x)
+        one_pass(False)
         e1.record(stream)
-        results.append(None)
     barrier()
     clocks = sampler.stop() if sampler else None
-    res = S.result()
+    res = S.result()                       # record of the last solve / last time step
+    cnt = counters.cpu().numpy()
+    total_its, total_promos, total_evals, worst_status = int(cnt[1]), int(cnt[2]), int(cnt[3]), int(cnt[0])
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
-    ms_per_step = float(np.mean(ms))
-    ms_per_step = max_over_ranks(ms_per_step, world, "cuda")
+    ms_per_step = max_over_ranks(float(np.mean(ms)), world, "cuda")
 
     # ---- end-to-end through the public API with HOST buffers (pinned), copies inside the timed region
     barrier()
@@ -265,13 +287,7 @@ def main():
         t0 = torch.cuda.Event(enable_timing=True)
         t1 = torch.cuda.Event(enable_timing=True)
         t0.record(stream)
-        b.copy_(b_host, non_blocking=True)
-        x.zero_()
-        if w.transient:
-            S.step(b, x)
-        else:
-            S.solve(b, x)
-        x_host.copy_(x, non_blocking=True)
+        one_pass(True)
         t1.record(stream)
         torch.cuda.synchronize()
         e2e_ms.append(t0.elapsed_time(t1))
@@ -306,12 +322,12 @@ def main():
     spmv = {}
     for nm, pr in (("fp64", cu.FP64), ("mixed", cu.MIXED)):
         for _ in range(3):
-            cu.cuth_spmv(A.buf, g, pr, b, y)
+            cu.cuth_spmv(A.buf, g, pr, b[0], y)
         e0 = torch.cuda.Event(enable_timing=True)
         e1 = torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(args.kernel_reps):
-            cu.cuth_spmv(A.buf, g, pr, b, y)
+            cu.cuth_spmv(A.buf, g, pr, b[0], y)
         e1.record(stream)
         torch.cuda.synchronize()
         tms = e0.elapsed_time(e1) / args.kernel_reps
@@ -322,8 +338,8 @@ def main():
             dist.destroy_process_group()
         return
 
-    it = res.iterations
-    early = res.switch_iteration if (mixed and res.promotions) else (it if mixed else 0)
+    it = total_its
+    early = int(early_acc.item()) if mixed else 0
     late = it - early
     iter_bytes = (early * bytes_per_row(w, "iter_mixed") + late * bytes_per_row(w, "iter_fp64")) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
@@ -337,7 +353,7 @@ def main():
         dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
     per_it = 2 if fused else 3
     per_eval = 3 if fused else 2
-    launches = args.steps * (1 + 1 + per_it * it + per_eval * res.true_resid_evals + 1 + (1 if w.transient else 0))
+    launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
 
     line = {
         "metric": METRIC, "value": ms_per_step * 1e-3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -345,12 +361,15 @@ def main():
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz],
                    "precision": "mixed" if mixed else "fp64", "rtol": w.rtol, "preconditioner": "jacobi",
-                   "l2_policy": "inputs larger than L2 (matrix + vectors = %.1f GB)" %
+                   "l2_policy": ("inputs larger than L2 (matrix + vectors = %.2f GB streamed per iteration)" if
+                                 (8 * m_ratio(w) + 48) * w.n > 126e6 else
+                                 "working set %.3f GB fits the 126 MB L2: L2-resident, latency-bound case, "
+                                 "no flush; HBM fractions are not meaningful here") %
                                 ((8 * m_ratio(w) + 48) * w.n / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "iterations": it, "promotions": res.promotions, "true_resid_evals": res.true_resid_evals,
+        "iterations": it, "promotions": total_promos, "true_resid_evals": total_evals, "time_steps": nt,
         "switch_reason": res.switch_reason, "switch_iteration": res.switch_iteration,
-        "rel_resid_true": res.rel_resid_true, "status": res.status_name,
+        "rel_resid_true": res.rel_resid_true, "status": res.status_name if worst_status == 0 else "not all steps converged",
         "us_per_iteration": ms_per_step * 1e3 / max(it, 1),
         "solves_per_s": world / (ms_per_step * 1e-3),
         "roofline": {"bound": "hbm", "kernel": "%s (%s operator)" % (dom_name, "fp64" if stage_fp64 else "fp32-stored"),
@@ -364,17 +383,18 @@ def main():
                                "note": "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv,
-        "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8),
+        "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,
     }
     if not args.no_cpu_baseline and world == 1:
         keep = {}
         line["cpu_baseline"] = cpu_oracle_sample(w, it, out=keep)
-        # property check of the timed result against the ORACLE's matrix (not timed)
-        from oracle import oracle as O
-        Ao, bb = keep["A"], keep["b"]
-        line["oracle_true_rel_resid_of_gpu_x"] = float(np.linalg.norm(bb - O.spmv(Ao, x_final)) / np.linalg.norm(bb))
+        if not w.transient:
+            # property check of the timed result against the ORACLE's matrix (not timed)
+            from oracle import oracle as O
+            Ao, bb = keep["A"], keep["b"]
+            line["oracle_true_rel_resid_of_gpu_x"] = float(np.linalg.norm(bb - O.spmv(Ao, x_final)) / np.linalg.norm(bb))
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
