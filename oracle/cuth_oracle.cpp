@@ -16,6 +16,8 @@
 //                         (PAPER.md:192-215): 4 unpadded upper diagonals, read off the CSR.
 //   oracle_pcg            Alg. 1 step by step, M = diag(A) (Jacobi, PAPER.md:231,
 //                         586) or M = I; stopping rule relative, verified on b - A x (R7).
+//   oracle_cheb_apply / oracle_lanczos / oracle_pcg_cheb   Alg. 3, Lanczos
+//                         and Alg. 1 with M^-1 = Alg. 3: the paper's own preconditioner.
 //   oracle_transient_rhs  right-hand side of eq. (5): b = P_{n+1} + (C V / dt) T_n  (T_amb = 0).
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form 1-D slab profile, dense Cholesky on
@@ -255,6 +257,113 @@ void oracle_pcg_window(int64_t n, const int64_t* rowptr, const int32_t* col, con
   int64_t it;
   double rel;
   oracle_pcg(n, rowptr, col, val, b, x, 0.0, iters, precond, &it, &rel, nullptr, 0);
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-1: the paper's own preconditioner.
+//
+// Alg. 3, Chebyshev polynomial preconditioning, step by step in the paper's order,
+// with the readings of DESIGN.md R-G16 for its garbles: z starts at 0, line 9 reads 2*sigma_1, and
+// rho_0 = 1/sigma_1 = delta/theta (PAPER.md:286 and 311 agree).  theta, delta from eq. (11b).
+// z = q(A) r with 1 - lambda q(lambda) = C_k((theta-lambda)/delta) / C_k(theta/delta)  (eq. (11a)).
+void oracle_cheb_apply(int64_t n, const int64_t* rowptr, const int32_t* col, const double* val, const double* r,
+                       double lmin, double lmax, int k, double* z) {
+  std::vector<double> rc(r, r + n), d(n), ad(n);
+  const double theta = (lmax + lmin) / 2.0, delta = (lmax - lmin) / 2.0;       // eq. (11b)
+  const double sigma1 = theta / delta;                                         // line 2
+  double rho = 1.0 / sigma1;                                                   // line 3
+  for (int64_t i = 0; i < n; ++i) { d[i] = rc[i] / theta; z[i] = 0.0; }        // line 4 (z = 0: R-G16)
+  for (int it = 0; it < k; ++it) {                                             // line 5
+    for (int64_t i = 0; i < n; ++i) z[i] = z[i] + d[i];                        // line 6
+    spmv(n, rowptr, col, val, d.data(), ad.data());                            // line 7
+    for (int64_t i = 0; i < n; ++i) rc[i] = rc[i] - ad[i];                     // line 8
+    const double rho_next = 1.0 / (2.0 * sigma1 - rho);                        // line 9
+    for (int64_t i = 0; i < n; ++i) d[i] = rho_next * rho * d[i] + (2.0 * rho_next / delta) * rc[i];   // line 10
+    rho = rho_next;
+  }
+}
+
+// Lanczos: m steps from the start vector v0 (normalised here), no reorthogonalisation;
+// alpha[0..m-1], beta[0..m-1] define the tridiagonal T (beta[j] couples j and j+1; beta[m-1] is the
+// residual norm).  fp64 (the paper runs this in fp32 on the GPU; the estimates only steer the
+// preconditioner).  Returns the number of steps done (stops early on an invariant subspace).
+int oracle_lanczos(int64_t n, const int64_t* rowptr, const int32_t* col, const double* val, const double* v0,
+                   int m, double* alpha, double* beta) {
+  std::vector<double> v(n), vp(n, 0.0), w(n);
+  const double nrm = std::sqrt(dot(n, v0, v0));
+  for (int64_t i = 0; i < n; ++i) v[i] = v0[i] / nrm;
+  double bprev = 0.0;
+  for (int j = 0; j < m; ++j) {
+    spmv(n, rowptr, col, val, v.data(), w.data());
+    for (int64_t i = 0; i < n; ++i) w[i] -= bprev * vp[i];
+    const double a = dot(n, w.data(), v.data());
+    for (int64_t i = 0; i < n; ++i) w[i] -= a * v[i];
+    const double bj = std::sqrt(dot(n, w.data(), w.data()));
+    alpha[j] = a;
+    beta[j] = bj;
+    if (!(bj > 0.0)) return j + 1;
+    for (int64_t i = 0; i < n; ++i) { vp[i] = v[i]; v[i] = w[i] / bj; }
+    bprev = bj;
+  }
+  return m;
+}
+
+// Alg. 1 with M^-1 = Alg. 3.  Same stopping rule as oracle_pcg (R-G7).
+int oracle_pcg_cheb(int64_t n, const int64_t* rowptr, const int32_t* col, const double* val, const double* b,
+                    double* x, double rtol, int64_t max_iters, double lmin, double lmax, int k,
+                    int64_t* iters_out, double* relres_true_out) {
+  std::vector<double> r(n), z(n), p(n), mu(n);
+  const double bnorm = std::sqrt(dot(n, b, b));
+  int64_t it = 0;
+  int status = 1;
+  if (bnorm == 0.0) {
+    std::memset(x, 0, sizeof(double) * n);
+    *iters_out = 0; *relres_true_out = 0.0;
+    return 0;
+  }
+  const double tol = rtol * bnorm;
+  spmv(n, rowptr, col, val, x, mu.data());
+  for (int64_t i = 0; i < n; ++i) r[i] = b[i] - mu[i];                         // line 1
+  oracle_cheb_apply(n, rowptr, col, val, r.data(), lmin, lmax, k, z.data());   // line 2
+  p = z;                                                                       // line 3
+  double rho = dot(n, r.data(), z.data());
+  double rnorm = std::sqrt(dot(n, r.data(), r.data()));
+  double rel_true = rnorm / bnorm;
+  for (;;) {
+    if (rnorm <= tol) {
+      spmv(n, rowptr, col, val, x, mu.data());
+      for (int64_t i = 0; i < n; ++i) mu[i] = b[i] - mu[i];
+      const double tn = std::sqrt(dot(n, mu.data(), mu.data()));
+      rel_true = tn / bnorm;
+      if (tn <= tol) { status = 0; break; }
+      r = mu;
+      oracle_cheb_apply(n, rowptr, col, val, r.data(), lmin, lmax, k, z.data());
+      p = z;
+      rho = dot(n, r.data(), z.data());
+      rnorm = tn;
+    }
+    if (it >= max_iters) { status = 1; break; }
+    spmv(n, rowptr, col, val, p.data(), mu.data());                            // line 6
+    const double pmu = dot(n, p.data(), mu.data());
+    if (!(pmu > 0.0) || !std::isfinite(pmu) || !std::isfinite(rho)) { status = 2; break; }
+    const double alpha = rho / pmu;                                            // line 7
+    for (int64_t i = 0; i < n; ++i) { x[i] += alpha * p[i]; r[i] -= alpha * mu[i]; }   // lines 8-9
+    oracle_cheb_apply(n, rowptr, col, val, r.data(), lmin, lmax, k, z.data()); // line 10
+    const double rho_new = dot(n, r.data(), z.data());
+    const double beta = rho_new / rho;                                         // line 11
+    for (int64_t i = 0; i < n; ++i) p[i] = z[i] + beta * p[i];                 // line 12
+    rho = rho_new;
+    rnorm = std::sqrt(dot(n, r.data(), r.data()));
+    ++it;
+  }
+  if (status != 0) {
+    spmv(n, rowptr, col, val, x, mu.data());
+    for (int64_t i = 0; i < n; ++i) mu[i] = b[i] - mu[i];
+    rel_true = std::sqrt(dot(n, mu.data(), mu.data())) / bnorm;
+  }
+  *iters_out = it;
+  *relres_true_out = rel_true;
+  return status;
 }
 
 }  // extern "C"

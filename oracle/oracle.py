@@ -133,3 +133,42 @@ def pcg_window(A: CSR, b, x0, iters: int, precond=1) -> np.ndarray:
     lib().oracle_pcg_window(C.c_int64(A.n), _p(A.rowptr), _p(A.col), _p(A.val), _p(b), _p(x),
                             C.c_int64(iters), C.c_int(precond))
     return x
+
+
+# ------------------------------------------------------------------ NEXT-1: Chebyshev + Lanczos
+def cheb_apply(A: CSR, r, lmin, lmax, k) -> np.ndarray:
+    """Alg. 3: z = q(A) r, degree-k Chebyshev preconditioner on [lmin, lmax]."""
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    z = np.empty(A.n, dtype=np.float64)
+    lib().oracle_cheb_apply(C.c_int64(A.n), _p(A.rowptr), _p(A.col), _p(A.val), _p(r), C.c_double(lmin),
+                            C.c_double(lmax), C.c_int(k), _p(z))
+    return z
+
+
+def lanczos(A: CSR, v0, m):
+    """m Lanczos steps: returns alpha[m'], beta[m'] of the tridiagonal T (m' <= m)."""
+    v0 = np.ascontiguousarray(v0, dtype=np.float64)
+    alpha = np.zeros(m)
+    beta = np.zeros(m)
+    done = lib().oracle_lanczos(C.c_int64(A.n), _p(A.rowptr), _p(A.col), _p(A.val), _p(v0), C.c_int(m),
+                                _p(alpha), _p(beta))
+    return alpha[:done], beta[:done]
+
+
+def ritz_extremes(alpha, beta):
+    """Extreme eigenvalues of T = tridiag(beta[:-1], alpha, beta[:-1]) (host, fp64, LAPACK)."""
+    import scipy.linalg as sla
+    w = sla.eigvalsh_tridiagonal(np.asarray(alpha), np.asarray(beta[:len(alpha) - 1]))
+    return float(w[0]), float(w[-1])
+
+
+def pcg_cheb(A: CSR, b, lmin, lmax, k, x0=None, rtol=1e-8, max_iters=200000) -> PCGResult:
+    """Alg. 1 with M^-1 = Alg. 3."""
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    x = np.zeros(A.n, dtype=np.float64) if x0 is None else np.array(x0, dtype=np.float64, copy=True)
+    it = C.c_int64(0)
+    rel = C.c_double(0.0)
+    st = lib().oracle_pcg_cheb(C.c_int64(A.n), _p(A.rowptr), _p(A.col), _p(A.val), _p(b), _p(x), C.c_double(rtol),
+                               C.c_int64(max_iters), C.c_double(lmin), C.c_double(lmax), C.c_int(k),
+                               C.byref(it), C.byref(rel))
+    return PCGResult(x, int(st), int(it.value), float(rel.value))
