@@ -41,7 +41,7 @@ typedef enum {
 enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN = 2, CUTH_SOLVE_RUNNING = 3 };
 
 enum { CUTH_FP64 = 0, CUTH_MIXED = 1 };            /* cuth_opts_t.precision / cuth_spmv precision */
-enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1 };
+enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1, CUTH_PRECOND_CHEBYSHEV = 2 };
 
 /* The thermal problem of PAPER.md §III-B: eq. (4) (steady) and eq. (5) (backward
  * Euler) on a box of cells with adiabatic sides/bottom (eq. (3)) and a Robin top
@@ -63,7 +63,11 @@ typedef struct {
   int32_t max_iters;          /* cap on PCG iterations (Alg. 1 loop), > 0 */
   int32_t true_resid_period;  /* MIXED early stage: evaluate b - A1 x every this many iterations
                                  (20 steady, 5 transient); <= 0 => 20 */
-  int32_t preconditioner;     /* CUTH_PRECOND_JACOBI (M = diag A) or CUTH_PRECOND_NONE (M = I) */
+  int32_t preconditioner;     /* CUTH_PRECOND_JACOBI (M = diag A), CUTH_PRECOND_NONE (M = I) or
+                                 CUTH_PRECOND_CHEBYSHEV (Alg. 3; needs the three fields below) */
+  int32_t cheb_degree;        /* k of Alg. 3 (the paper uses 30); 3 <= k <= 64 */
+  double cheb_lmin, cheb_lmax;/* spectral interval [alpha, beta] of eq. (10)-(11), e.g. from
+                                 cuth_lanczos_bounds; 0 < lmin < lmax, and lmax must bound the spectrum of A */
 } cuth_opts_t;
 
 typedef struct {
@@ -139,6 +143,23 @@ int cuth_version(void);
  * large planes, 3 on the flat path); bench.py reports gpu_launches = prologue + this * iterations +
  * true-residual branches + epilogue. */
 int cuth_launches_per_iteration(const cuth_grid_t* grid);
+
+/* Spectral-range estimate for the Chebyshev preconditioner: `steps` Lanczos iterations on
+ * the device (start vector v0_D, e.g. the right-hand side), the tridiagonal T copied to the host and its
+ * extreme eigenvalues found there in fp64 (bisection).  bounds_H[0] = smallest Ritz value, bounds_H[1] =
+ * largest Ritz value, bounds_H[2] = Gershgorin upper bound max_i sum_j |a_ij| (always >= lambda_max),
+ * bounds_H[3], bounds_H[4] = the interval to hand to cuth_opts_t.cheb_lmin / cheb_lmax: [Ritz min,
+ * min(1.05 * Ritz max, Gershgorin)].
+ * Uses the solver workspace (>= cuth_workspace_bytes).  This call SYNCHRONISES `stream` (setup, not hot path). */
+int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
+                        size_t work_bytes, double bounds_H[5], void* stream);
+
+/* One application of the Chebyshev polynomial preconditioner, z = q(A) r (Alg. 3), with the
+ * degree and interval of `opts` (preconditioner must be CUTH_PRECOND_CHEBYSHEV): k-1 stencil kernels, no
+ * reduction.  precision CUTH_FP64: fp64 vectors and matrix; CUTH_MIXED: fp32 vectors on the fp32-stored matrix
+ * (PAPER.md:376).  r_D, z_D fp64 [N], distinct.  work_D >= cuth_workspace_bytes(grid, opts). */
+int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* r_D,
+                    double* z_D, void* work_D, size_t work_bytes, void* stream);
 
 /* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching
  * when one x-y plane of the six streamed arrays no longer fits L2, flat 1-D streaming otherwise),

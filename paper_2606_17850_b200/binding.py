@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("CUTH_LIB", os.path.join(HERE, "libcuth.so"))   # CUTH_LIB: developer override
 
 FP64, MIXED = 0, 1
-PRECOND_NONE, PRECOND_JACOBI = 0, 1
+PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV = 0, 1, 2
 STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}
 _ERR = {-1: "CUTH_ERR_NULL", -2: "CUTH_ERR_DIMS", -3: "CUTH_ERR_VALUE", -4: "CUTH_ERR_SIZE",
         -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT"}
@@ -36,7 +36,8 @@ class cuth_grid_t(C.Structure):
 
 class cuth_opts_t(C.Structure):
     _fields_ = [("precision", C.c_int32), ("rtol", C.c_double), ("max_iters", C.c_int32),
-                ("true_resid_period", C.c_int32), ("preconditioner", C.c_int32)]
+                ("true_resid_period", C.c_int32), ("preconditioner", C.c_int32),
+                ("cheb_degree", C.c_int32), ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double)]
 
 
 class cuth_result_t(C.Structure):
@@ -48,7 +49,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply"]
 
 _lib = None
 
@@ -88,6 +89,10 @@ def load_library():
     L.cuth_version.restype = C.c_int
     L.cuth_launches_per_iteration.restype = C.c_int
     L.cuth_launches_per_iteration.argtypes = [gp]
+    L.cuth_lanczos_bounds.restype = C.c_int
+    L.cuth_lanczos_bounds.argtypes = [vp, gp, vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_double), vp]
+    L.cuth_cheb_apply.restype = C.c_int
+    L.cuth_cheb_apply.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp]
     L.cuth_set_traversal.restype = C.c_int
     L.cuth_set_traversal.argtypes = [C.c_int]
     L.cuth_profile_kernel.restype = C.c_int
@@ -128,8 +133,10 @@ class Grid:
         return C.byref(self.c)
 
 
-def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI):
-    return cuth_opts_t(int(precision), float(rtol), int(max_iters), int(true_resid_period), int(preconditioner))
+def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI,
+         cheb_degree=30, cheb_lmin=0.0, cheb_lmax=0.0):
+    return cuth_opts_t(int(precision), float(rtol), int(max_iters), int(true_resid_period), int(preconditioner),
+                       int(cheb_degree), float(cheb_lmin), float(cheb_lmax))
 
 
 @dataclass
@@ -207,6 +214,20 @@ def cuth_profile_kernel(work, grid: Grid, kernel_id: int, stream=None):
            "cuth_profile_kernel")
 
 
+def cuth_lanczos_bounds(dia, grid: Grid, v0, steps, work, stream=None):
+    """Returns (ritz_min, ritz_max, gershgorin_max, lmin, lmax); synchronises the stream."""
+    out = (C.c_double * 5)()
+    _check(load_library().cuth_lanczos_bounds(_ptr(dia), grid.ref(), _ptr(v0), int(steps), _ptr(work),
+                                              work.numel() * work.element_size(), out, stream or _stream()),
+           "cuth_lanczos_bounds")
+    return tuple(out)
+
+
+def cuth_cheb_apply(dia, grid: Grid, opts, r, z, work, stream=None):
+    _check(load_library().cuth_cheb_apply(_ptr(dia), grid.ref(), C.byref(opts), _ptr(r), _ptr(z), _ptr(work),
+                                          work.numel() * work.element_size(), stream or _stream()), "cuth_cheb_apply")
+
+
 def cuth_set_traversal(mode: int):
     _check(load_library().cuth_set_traversal(int(mode)), "cuth_set_traversal")
 
@@ -261,6 +282,23 @@ class Solver:
         self.opts = opts or Opts()
         self.work = torch.empty(cuth_workspace_bytes(A.grid, self.opts), dtype=torch.uint8, device="cuda")
         self.result_dev = torch.zeros(C.sizeof(cuth_result_t), dtype=torch.uint8, device="cuda")
+
+    def setup_chebyshev(self, v0, lanczos_steps=40, degree=30, lmin=None, lmax=None):
+        """Spectral range by Lanczos (cuth_lanczos_bounds) and switch this solver to the Chebyshev
+        preconditioner; only copies the interval the library returns into the options struct."""
+        import torch
+        lo, hi, gersh, rec_lo, rec_hi = cuth_lanczos_bounds(self.A.buf, self.A.grid, v0, lanczos_steps, self.work)
+        o = self.opts
+        self.opts = Opts(o.precision, o.rtol, o.max_iters, o.true_resid_period, PRECOND_CHEBYSHEV, degree,
+                         rec_lo if lmin is None else lmin, rec_hi if lmax is None else lmax)
+        need = cuth_workspace_bytes(self.A.grid, self.opts)
+        if need > self.work.numel():
+            cuth_release_workspace(self.work)
+            self.work = torch.empty(need, dtype=torch.uint8, device="cuda")
+        return lo, hi, gersh
+
+    def cheb_apply(self, r, z):
+        cuth_cheb_apply(self.A.buf, self.A.grid, self.opts, r, z, self.work)
 
     def solve(self, b, x):
         cuth_pcg_solve(self.A.buf, self.A.grid, self.opts, b, x, self.work, self.result_dev)

@@ -14,6 +14,7 @@
 #include <unordered_map>
 
 #include "cuth_fused.cuh"
+#include "cuth_cheb.cuh"
 
 namespace cuth {
 
@@ -93,6 +94,7 @@ struct GraphEntry {
   int64_t n = 0;
   int sblocks = 0;
   int fblocks = 0;
+  int chebkey = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -110,7 +112,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
 
-static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, GraphEntry* out) {
+static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -134,14 +136,35 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
     CU(add_kernel(g, &n_fin, &n_while, 1, (void*)k_finalize, blocks, a)); }
 
   cudaGraphNode_t n_p, n_s, n_u, n_if;
+  // Chebyshev: the body starts with the preconditioner z = q(A) r: k-1 stencil kernels, no reduction
+  // until the last one, which also forms rho = r.z and beta (Alg. 1 lines 10-11).
+  cudaGraphNode_t n_c = nullptr;
+  const int kdeg = chebkey >> 1;
+  if (kdeg > 0) {
+    const bool f32 = (chebkey & 1) != 0;
+    { void* a[] = {&ctx};
+      CU(add_kernel(body, &n_c, nullptr, 0, f32 ? (void*)k_cheb_first<float> : (void*)k_cheb_first<double>, sblocks, a)); }
+    for (int i = 1; i <= kdeg - 3; ++i) {
+      cudaGraphNode_t prev = n_c;
+      int step = i;
+      void* a[] = {&ctx, &step};
+      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, sblocks, a));
+    }
+    { cudaGraphNode_t prev = n_c;
+      int step = kdeg - 2;
+      void* a[] = {&ctx, &ctl, &partials, &step};
+      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_last<float> : (void*)k_cheb_last<double>, sblocks, a)); }
+  }
+  const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
+  const size_t ndep0 = n_c ? 1 : 0;
   if (fblocks > 0) {
     { void* a[] = {&ctx, &ctl, &partials};
-      CU(add_kernel(body, &n_s, nullptr, 0, (void*)k_fused_pspmv, fblocks, a)); }
+      CU(add_kernel(body, &n_s, dep0, ndep0, (void*)k_fused_pspmv, fblocks, a)); }
     { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
       CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a)); }
   } else {
     { void* a[] = {&ctx, &ctl};
-      CU(add_kernel(body, &n_p, nullptr, 0, (void*)k_pupdate, blocks, a)); }
+      CU(add_kernel(body, &n_p, dep0, ndep0, (void*)k_pupdate, blocks, a)); }
     { void* a[] = {&ctx, &ctl, &partials};
       CU(add_kernel(body, &n_s, &n_p, 1, (void*)k_spmv_dot, sblocks, a)); }
     { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
@@ -166,19 +189,20 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
-static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, cudaGraphExec_t* ex) {
+static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
+                     cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
   cudaGetDevice(&dev);
   if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
-                               it->second.fblocks != fblocks)) {
+                               it->second.fblocks != fblocks || it->second.chebkey != chebkey)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -186,7 +210,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -198,8 +222,33 @@ static int check_opts(const cuth_opts_t* o) {
   if (!o) return CUTH_ERR_NULL;
   if (!(o->rtol > 0.0) || o->max_iters <= 0) return CUTH_ERR_VALUE;
   if (o->precision != CUTH_FP64 && o->precision != CUTH_MIXED) return CUTH_ERR_VALUE;
-  if (o->preconditioner != CUTH_PRECOND_NONE && o->preconditioner != CUTH_PRECOND_JACOBI) return CUTH_ERR_VALUE;
+  if (o->preconditioner != CUTH_PRECOND_NONE && o->preconditioner != CUTH_PRECOND_JACOBI &&
+      o->preconditioner != CUTH_PRECOND_CHEBYSHEV)
+    return CUTH_ERR_VALUE;
+  if (o->preconditioner == CUTH_PRECOND_CHEBYSHEV &&
+      (o->cheb_degree < 3 || o->cheb_degree > kMaxChebDegree || !(o->cheb_lmin > 0.0) || !(o->cheb_lmax > o->cheb_lmin)))
+    return CUTH_ERR_VALUE;
   return CUTH_OK;
+}
+
+// Alg. 3 lines 2-3, 9-10 in fp64 on the host: theta, delta, sigma_1, rho_i and the two
+// coefficients of line 10 for every step; buffers of the preconditioner.
+static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
+  const int k = opts->cheb_degree;
+  const double theta = 0.5 * (opts->cheb_lmax + opts->cheb_lmin), delta = 0.5 * (opts->cheb_lmax - opts->cheb_lmin);
+  const double sigma1 = theta / delta;
+  double rho = 1.0 / sigma1;
+  for (int i = 0; i < k; ++i) {
+    const double rho_next = 1.0 / (2.0 * sigma1 - rho);
+    c->cheb_c1[i] = rho_next * rho;
+    c->cheb_c2[i] = 2.0 * rho_next / delta;
+    rho = rho_next;
+  }
+  c->cheb = k;
+  c->cheb_inv_theta = 1.0 / theta;
+  c->cz = w.cz; c->cd[0] = w.cd0; c->cd[1] = w.cd1; c->crc = w.crc; c->czc = w.czc;
+  c->jacobi = 0;
+  c->precision = opts->precision;
 }
 
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
@@ -218,7 +267,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   if (transient && !(grid->cvol_H && grid->dt > 0.0)) return CUTH_ERR_NOT_TRANSIENT;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
-  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
+  const bool cheb = opts->preconditioner == CUTH_PRECOND_CHEBYSHEV;
+  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, cheb);
   DiaDev A = dev_view(dia_D, L);
   const int blocks = grid_blocks(L.n);
   if (transient) {
@@ -236,15 +286,49 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.max_iters = opts->max_iters;
   c.period = opts->true_resid_period > 0 ? opts->true_resid_period : 20;
   c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
+  c.cheb = 0;
+  if (cheb) fill_cheb(&c, opts, w);
   c.soft_restart = 1;         // promotion keeps p while the drift is small (DESIGN.md R-G11)
   c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   cudaGraphExec_t ex;
-  rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0, &ex);
+  rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
+                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
+}
+
+
+// Extreme eigenvalues of the symmetric tridiagonal T (diagonal a[0..m), off-diagonal b[0..m-1)) by Sturm
+// bisection in fp64 on the host ("the solution of the spectrum of T is executed on CPUs").
+static int sturm_count(const double* a, const double* b, int m, double x) {   // #eigenvalues < x
+  int cnt = 0;
+  double q = a[0] - x;
+  if (q < 0) ++cnt;
+  for (int i = 1; i < m; ++i) {
+    if (q == 0.0) q = 1e-300;
+    q = a[i] - x - b[i - 1] * b[i - 1] / q;
+    if (q < 0) ++cnt;
+  }
+  return cnt;
+}
+static void tridiag_extremes(const double* a, const double* b, int m, double* lo, double* hi) {
+  double gl = a[0], gu = a[0];
+  for (int i = 0; i < m; ++i) {
+    const double r = (i > 0 ? fabs(b[i - 1]) : 0.0) + (i + 1 < m ? fabs(b[i]) : 0.0);
+    gl = fmin(gl, a[i] - r); gu = fmax(gu, a[i] + r);
+  }
+  for (int which = 0; which < 2; ++which) {
+    const int target = which == 0 ? 1 : m;          // smallest: count(x) >= 1; largest: count(x) >= m
+    double l = gl, u = gu;
+    for (int it = 0; it < 200 && u - l > 1e-15 * fmax(fabs(l), fabs(u)); ++it) {
+      const double mid = 0.5 * (l + u);
+      if (sturm_count(a, b, m, mid) >= target) u = mid; else l = mid;
+    }
+    *(which == 0 ? lo : hi) = 0.5 * (l + u);
+  }
 }
 
 }  // namespace cuth
@@ -260,10 +344,10 @@ size_t cuth_dia_bytes(const cuth_grid_t* grid) {
 }
 
 size_t cuth_workspace_bytes(const cuth_grid_t* grid, const cuth_opts_t* opts) {
-  (void)opts;
   DiaLayout L;
   if (!make_layout(grid, &L)) return 0;
-  return carve_workspace(nullptr, L.n, grid->cvol_H && grid->dt > 0.0).bytes;
+  return carve_workspace(nullptr, L.n, grid->cvol_H && grid->dt > 0.0,
+                         opts && opts->preconditioner == CUTH_PRECOND_CHEBYSHEV).bytes;
 }
 
 int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void* stream) {
@@ -347,6 +431,82 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
+  }
+  CU(cudaGetLastError());
+  return CUTH_OK;
+}
+
+int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
+                        size_t work_bytes, double bounds_H[5], void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  if (!dia_D || !v0_D || !work_D || !bounds_H) return CUTH_ERR_NULL;
+  if (steps < 2 || steps > 120) return CUTH_ERR_VALUE;
+  if (!aligned16(dia_D) || !aligned16(v0_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
+  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
+  if (work_bytes < w.bytes) return CUTH_ERR_SIZE;
+  cudaStream_t st = (cudaStream_t)stream;
+  DiaDev A = dev_view(dia_D, L);
+  const int blocks = grid_blocks(L.n);
+  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
+  LanczosScal* sc = (LanczosScal*)(w.partials + 3 * kMaxBlocks);
+  static_assert(sizeof(LanczosScal) <= sizeof(double) * kMaxBlocks, "LanczosScal must fit one partial slot");
+  CU(cudaMemsetAsync(sc, 0, sizeof(LanczosScal), st));
+  double* u_cur = w.r; double* u_prev = w.p; double* t = w.mu;
+  k_lanczos_init<<<blocks, kThreads, 0, st>>>(A, v0_D, u_cur, u_prev, sc, w.partials);
+  for (int j = 0; j < steps; ++j) {
+    k_lanczos_1<<<sb, kThreads, 0, st>>>(A, u_cur, u_prev, t, sc, w.partials);
+    k_lanczos_2<<<blocks, kThreads, 0, st>>>(L.n, u_cur, t, u_prev, sc, w.partials);
+    double* tmp = u_prev; u_prev = u_cur; u_cur = tmp;     // u_{j+1} was written over u_{j-1}
+  }
+  CU(cudaGetLastError());
+  LanczosScal h;
+  CU(cudaMemcpyAsync(&h, sc, sizeof h, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  int m = steps;
+  for (int j = 0; j < steps; ++j)
+    if (!(h.out_beta[j] > 0.0) || !(h.out_alpha[j] == h.out_alpha[j])) { m = j + 1; break; }   // invariant subspace
+  tridiag_extremes(h.out_alpha, h.out_beta, m, &bounds_H[0], &bounds_H[1]);
+  bounds_H[2] = h.out_beta[127];       // Gershgorin bound (k_lanczos_init)
+  // Interval handed to Alg. 3 (DESIGN.md R-C2): alpha = smallest Ritz value; beta = 1.05 x the largest Ritz
+  // value (Ritz values approach lambda_max from below), never above the Gershgorin bound.
+  bounds_H[3] = bounds_H[0];
+  bounds_H[4] = fmin(1.05 * bounds_H[1], bounds_H[2]);
+  return CUTH_OK;
+}
+
+int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* r_D,
+                    double* z_D, void* work_D, size_t work_bytes, void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  rc = check_opts(opts);
+  if (rc) return rc;
+  if (opts->preconditioner != CUTH_PRECOND_CHEBYSHEV) return CUTH_ERR_VALUE;
+  if (!dia_D || !r_D || !z_D || !work_D) return CUTH_ERR_NULL;
+  if (!aligned16(dia_D) || !aligned16(r_D) || !aligned16(z_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
+  if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, true);
+  Ctx c;
+  memset(&c, 0, sizeof c);
+  c.A = dev_view(dia_D, L);
+  c.r = const_cast<double*>(r_D);      // read only here
+  fill_cheb(&c, opts, w);
+  c.cz = z_D;
+  k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
+  const int blocks = grid_blocks(L.n);
+  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
+  const int k = opts->cheb_degree;
+  if (opts->precision == CUTH_MIXED) {
+    k_cheb_first<float><<<sb, kThreads, 0, st>>>(w.ctx);
+    for (int i = 1; i <= k - 3; ++i) k_cheb_mid<float><<<sb, kThreads, 0, st>>>(w.ctx, i);
+    k_cheb_last<float><<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, k - 2);
+  } else {
+    k_cheb_first<double><<<sb, kThreads, 0, st>>>(w.ctx);
+    for (int i = 1; i <= k - 3; ++i) k_cheb_mid<double><<<sb, kThreads, 0, st>>>(w.ctx, i);
+    k_cheb_last<double><<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, k - 2);
   }
   CU(cudaGetLastError());
   return CUTH_OK;

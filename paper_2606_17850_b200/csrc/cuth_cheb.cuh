@@ -1,0 +1,261 @@
+// cuth_cheb.cuh -- Chebyshev polynomial preconditioner (Alg. 3) and the Lanczos
+// spectral-range estimate: SURVEY.md §8(f) rank 1, the paper's own preconditioner.
+//
+// One apply z = q(A) r of degree k is k-1 stencil kernels with NO reduction inside:
+//   FIRST (i = 0)      d0 = r/theta (formed on the fly, also at the stencil neighbours: A d0 = (A r)/theta),
+//                      rc = r - A d0, z = d0, d1 = c1[0] d0 + c2[0] rc
+//   MID   (0 < i < k-2) rc -= A d_i, z += d_i, d_{i+1} = c1[i] d_i + c2[i] rc
+//   LAST  (i = k-2)    rc' = rc - A d_i, d_{k-1} = c1 d_i + c2 rc', z_out = z + d_i + d_{k-1}, rho = r.z_out
+// (Alg. 3's k-th SpMV and d-update feed nothing and are skipped: z is identical.)
+// Element type T of d, rc, z: double (FP64 mode, fp64 matrix A1) or float (MIXED mode: "FP32 for all
+// vector and scalar operations" of Alg. 3, on the fp32-stored matrix A2 in difference form).
+#pragma once
+#include "cuth_kernels.cuh"
+
+namespace cuth {
+
+// One row of A v with v stored as VT and arithmetic in T (T = double: A1 standard form; T = float: A2
+// difference form, DESIGN.md R-F3), flat traversal.
+template <class VT, class T>
+__device__ __forceinline__ T row_t(const DiaDev& A, const VT* __restrict__ v, int64_t i, T vi) {
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx, up3 = i + np < n, lo3 = i >= np;
+  if (sizeof(T) == 8) {
+    T acc = (T)A.d0[i] * vi;
+    acc += (T)(up1 ? A.d1[i] : 0.0) * (T)(up1 ? v[i + 1] : (VT)0);
+    acc += (T)(lo1 ? A.d1[i - 1] : 0.0) * (T)(lo1 ? v[i - 1] : (VT)0);
+    acc += (T)(up2 ? A.d2[i] : 0.0) * (T)(up2 ? v[i + nx] : (VT)0);
+    acc += (T)(lo2 ? A.d2[i - nx] : 0.0) * (T)(lo2 ? v[i - nx] : (VT)0);
+    acc += (T)(up3 ? A.d3[i] : 0.0) * (T)(up3 ? v[i + np] : (VT)0);
+    acc += (T)(lo3 ? A.d3[i - np] : 0.0) * (T)(lo3 ? v[i - np] : (VT)0);
+    return acc;
+  } else {
+    const unsigned z = (unsigned)i / (unsigned)np;
+    T acc = (T)A.s_layer[z] * vi;
+    acc += (T)(up1 ? A.f1[i] : 0.f) * ((T)(up1 ? v[i + 1] : (VT)vi) - vi);
+    acc += (T)(lo1 ? A.f1[i - 1] : 0.f) * ((T)(lo1 ? v[i - 1] : (VT)vi) - vi);
+    acc += (T)(up2 ? A.f2[i] : 0.f) * ((T)(up2 ? v[i + nx] : (VT)vi) - vi);
+    acc += (T)(lo2 ? A.f2[i - nx] : 0.f) * ((T)(lo2 ? v[i - nx] : (VT)vi) - vi);
+    acc += (T)(up3 ? A.f3[i] : 0.f) * ((T)(up3 ? v[i + np] : (VT)vi) - vi);
+    acc += (T)(lo3 ? A.f3[i - np] : 0.f) * ((T)(lo3 ? v[i - np] : (VT)vi) - vi);
+    return acc;
+  }
+}
+
+// f(i, v_i, (A v)_i) for every row; traversal as in apply_A (flat, or z-marching with the plane
+// neighbours in registers).
+template <class VT, class T, class F>
+__device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict__ v, F&& f) {
+  if (!A.zmarch) {
+    CUTH_TILE_LOOP(A.n) {
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        if (i < A.n) {
+          const T vi = (T)v[i];
+          f(i, vi, row_t<VT, T>(A, v, i, vi));
+        }
+      }
+    }
+    return;
+  }
+  const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
+  const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
+  const int tiles_x = (nxi + ZTX - 1) / ZTX, tiles_y = (nyi + ZTY - 1) / ZTY;
+  const int ntiles = tiles_x * tiles_y;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int bx = t % tiles_x, by = t / tiles_x;
+    const int x = bx * ZTX + tx, y = by * ZTY + ty;
+    if (x >= nxi || y >= nyi) continue;
+    const int64_t c = x + nx * (int64_t)y;
+    T v_lo = (T)0, v_c = (T)v[c], a3l = (T)0;
+#pragma unroll 2
+    for (int z = 0; z < nz; ++z) {
+      const int64_t i = c + (int64_t)z * np;
+      const bool up3 = z + 1 < nz;
+      const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx;
+      T acc, a3u, v_hi;
+      if (sizeof(T) == 8) {
+        const T a0 = (T)A.d0[i];
+        const T a1u = (T)(up1 ? A.d1[i] : 0.0), a1l = (T)(lo1 ? A.d1[i - 1] : 0.0);
+        const T a2u = (T)(up2 ? A.d2[i] : 0.0), a2l = (T)(lo2 ? A.d2[i - nx] : 0.0);
+        a3u = (T)(up3 ? A.d3[i] : 0.0);
+        v_hi = up3 ? (T)v[i + np] : (T)0;
+        const T v1u = up1 ? (T)v[i + 1] : (T)0, v1l = lo1 ? (T)v[i - 1] : (T)0;
+        const T v2u = up2 ? (T)v[i + nx] : (T)0, v2l = lo2 ? (T)v[i - nx] : (T)0;
+        acc = a0 * v_c;
+        acc += a1u * v1u; acc += a1l * v1l; acc += a2u * v2u; acc += a2l * v2l;
+        acc += a3u * v_hi; acc += a3l * v_lo;
+      } else {
+        const T a1u = (T)(up1 ? A.f1[i] : 0.f), a1l = (T)(lo1 ? A.f1[i - 1] : 0.f);
+        const T a2u = (T)(up2 ? A.f2[i] : 0.f), a2l = (T)(lo2 ? A.f2[i - nx] : 0.f);
+        a3u = (T)(up3 ? A.f3[i] : 0.f);
+        v_hi = up3 ? (T)v[i + np] : v_c;
+        const T v1u = up1 ? (T)v[i + 1] : v_c, v1l = lo1 ? (T)v[i - 1] : v_c;
+        const T v2u = up2 ? (T)v[i + nx] : v_c, v2l = lo2 ? (T)v[i - nx] : v_c;
+        acc = (T)A.s_layer[z] * v_c;
+        acc += a1u * (v1u - v_c); acc += a1l * (v1l - v_c);
+        acc += a2u * (v2u - v_c); acc += a2l * (v2l - v_c);
+        acc += a3u * (v_hi - v_c); acc += a3l * ((z > 0 ? v_lo : v_c) - v_c);
+      }
+      f(i, v_c, acc);
+      v_lo = v_c; v_c = v_hi; a3l = a3u;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Alg. 3 lines 1-4 and the first pass of lines 6-10.
+template <class T>
+__global__ void __launch_bounds__(kThreads, 4) k_cheb_first(const Ctx* __restrict__ ctxp) {
+  const Ctx c = *ctxp;
+  const T inv_theta = (T)c.cheb_inv_theta, c1 = (T)ctxp->cheb_c1[0], c2 = (T)ctxp->cheb_c2[0];
+  T* __restrict__ rc = (T*)c.crc;
+  T* __restrict__ zc = (T*)c.czc;
+  T* __restrict__ d1 = (T*)c.cd[1];
+  apply_A_t<double, T>(c.A, c.r, [&](int64_t i, T ri, T Ar) {
+    const T d0 = ri * inv_theta;                 // line 4
+    const T rci = ri - Ar * inv_theta;           // lines 7-8
+    rc[i] = rci;
+    zc[i] = d0;                                  // line 6
+    d1[i] = c1 * d0 + c2 * rci;                  // line 10
+  });
+}
+
+// Alg. 3 lines 6-10 for 0 < i < k-2.
+template <class T>
+__global__ void __launch_bounds__(kThreads, 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
+  const Ctx c = *ctxp;
+  const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
+  const T* __restrict__ din = (const T*)ctxp->cd[step & 1];
+  T* __restrict__ dout = (T*)ctxp->cd[(step + 1) & 1];
+  T* __restrict__ rc = (T*)c.crc;
+  T* __restrict__ zc = (T*)c.czc;
+  apply_A_t<T, T>(c.A, din, [&](int64_t i, T di, T Ad) {
+    const T rci = rc[i] - Ad;
+    rc[i] = rci;
+    zc[i] += di;
+    dout[i] = c1 * di + c2 * rci;
+  });
+}
+
+// Last stencil pass (i = k-2) + the two trailing z updates + rho = r.z (Alg. 1 lines 10-11).
+template <class T>
+__global__ void __launch_bounds__(kThreads, 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+                                                        int step) {
+  __shared__ double smem[32];
+  __shared__ int s_flag;
+  const Ctx c = *ctxp;
+  const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
+  const T* __restrict__ din = (const T*)ctxp->cd[step & 1];
+  const T* __restrict__ rc = (const T*)c.crc;
+  const T* __restrict__ zc = (const T*)c.czc;
+  double acc[1] = {0.0};
+  apply_A_t<T, T>(c.A, din, [&](int64_t i, T di, T Ad) {
+    const T rci = rc[i] - Ad;
+    const T dl = c1 * di + c2 * rci;             // d_{k-1}
+    const double zi = (double)(zc[i] + di + dl);
+    c.cz[i] = zi;
+    acc[0] = fma(c.r[i], zi, acc[0]);
+  });
+  if (grid_sum_last_block<1>(acc, partials + 3 * kMaxBlocks, &ctl->ticket[5], smem, &s_flag) && threadIdx.x == 0) {
+    const double rho_new = acc[0];
+    ctl->beta = ctl->beta_zero ? 0.0 : rho_new / ctl->rho;     // Alg. 1 line 11 (line 3 when restarting)
+    ctl->rho = rho_new;
+    ctl->beta_zero = 0;
+    if (!(rho_new == rho_new) || rho_new <= 0.0) ctl->status = CUTH_SOLVE_BREAKDOWN;   // q(A) not SPD: bad interval
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Lanczos on unnormalised vectors u_j (v_j = s_j u_j, s_j = 1/||u_j||):
+//   L1: t = s_j A u_j - beta_{j-1} s_{j-1} u_{j-1},  alpha_j = s_j (t . u_j)
+//   L2: u_{j+1} = t - alpha_j s_j u_j (overwrites u_{j-1}),  beta_j = ||u_{j+1}||
+struct LanczosScal { double s_cur, s_prev, beta_prev, alpha; double out_alpha[128], out_beta[128]; int j, pad; unsigned ticket[2]; };
+
+__global__ void __launch_bounds__(kThreads, 4) k_lanczos_1(DiaDev A, const double* __restrict__ u_cur,
+                                                         const double* __restrict__ u_prev, double* __restrict__ t,
+                                                         LanczosScal* sc, double* partials) {
+  __shared__ double smem[32];
+  __shared__ int s_flag;
+  const double s_cur = sc->s_cur, cprev = sc->beta_prev * sc->s_prev;
+  double acc[1] = {0.0};
+  apply_A<false>(A, u_cur, [&](int64_t i, double ui, double Au) {
+    const double ti = s_cur * Au - cprev * u_prev[i];
+    t[i] = ti;
+    acc[0] = fma(ti, ui, acc[0]);
+  });
+  if (grid_sum_last_block<1>(acc, partials, &sc->ticket[0], smem, &s_flag) && threadIdx.x == 0)
+    sc->alpha = s_cur * acc[0];
+}
+
+__global__ void __launch_bounds__(kThreads) k_lanczos_2(int64_t n, const double* __restrict__ u_cur,
+                                                       const double* __restrict__ t, double* __restrict__ u_next,
+                                                       LanczosScal* sc, double* partials) {
+  __shared__ double smem[32];
+  __shared__ int s_flag;
+  const double a = sc->alpha * sc->s_cur;
+  double acc[1] = {0.0};
+  CUTH_TILE_LOOP(n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < n) {
+        const double v = t[i] - a * u_cur[i];
+        u_next[i] = v;
+        acc[0] = fma(v, v, acc[0]);
+      }
+    }
+  }
+  if (grid_sum_last_block<1>(acc, partials + kMaxBlocks, &sc->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
+    const double beta = sqrt(acc[0]);
+    const int j = sc->j;
+    sc->out_alpha[j] = sc->alpha;
+    sc->out_beta[j] = beta;
+    sc->beta_prev = beta;
+    sc->s_prev = sc->s_cur;
+    sc->s_cur = beta > 0.0 ? 1.0 / beta : 0.0;
+    sc->j = j + 1;
+  }
+}
+
+// u_0 = v0, u_{-1} = 0, s_0 = 1/||v0||; also the Gershgorin bound max_i sum_j |a_ij| (into out_beta[127]).
+__global__ void __launch_bounds__(kThreads) k_lanczos_init(DiaDev A, const double* __restrict__ v0,
+                                                          double* __restrict__ u_cur, double* __restrict__ u_prev,
+                                                          LanczosScal* sc, double* partials) {
+  __shared__ double smem[2 * 32];
+  __shared__ int s_flag;
+  double acc[1] = {0.0};
+  double gmax = 0.0;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  CUTH_TILE_LOOP(n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < n) {
+        const double v = v0[i];
+        u_cur[i] = v;
+        u_prev[i] = 0.0;
+        acc[0] = fma(v, v, acc[0]);
+        double g = fabs(A.d0[i]);
+        if (i + 1 < n) g += fabs(A.d1[i]);
+        if (i >= 1) g += fabs(A.d1[i - 1]);
+        if (i + nx < n) g += fabs(A.d2[i]);
+        if (i >= nx) g += fabs(A.d2[i - nx]);
+        if (i + np < n) g += fabs(A.d3[i]);
+        if (i >= np) g += fabs(A.d3[i - np]);
+        gmax = fmax(gmax, g);
+      }
+    }
+  }
+  // max over the grid: positive doubles order like their bit patterns
+  for (int o = 16; o > 0; o >>= 1) gmax = fmax(gmax, __shfl_xor_sync(0xffffffffu, gmax, o));
+  if ((threadIdx.x & 31) == 0) atomicMax((unsigned long long*)&sc->out_beta[127], (unsigned long long)__double_as_longlong(gmax));
+  if (grid_sum_last_block<1>(acc, partials, &sc->ticket[0], smem, &s_flag) && threadIdx.x == 0) {
+    sc->s_cur = acc[0] > 0.0 ? 1.0 / sqrt(acc[0]) : 0.0;
+    sc->s_prev = 0.0; sc->beta_prev = 0.0; sc->j = 0;
+  }
+}
+
+}  // namespace cuth

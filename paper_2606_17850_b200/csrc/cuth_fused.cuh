@@ -38,6 +38,7 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
   const int ntiles = tiles_x * tiles_y;
   const int64_t n = A.n, nx = A.nx, np = A.nxny;
   const bool jac = c.jacobi != 0;
+  const double* __restrict__ zs = c.cheb ? c.cz : c.r;     // Chebyshev: z = q(A) r is a stored vector
   const bool do_x = xalpha != 0.0;
 
   for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
@@ -62,8 +63,8 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
     double pn_lo = 0.0, pn_c = 0.0, a3l = 0.0;
     {   // plane 0 of p'
       double ro = 0.0, dio = 1.0, po = 0.0, xo = 0.0, rh = 0.0, dih = 1.0, ph = 0.0;
-      if (own) { ro = c.r[col]; po = p_in[col]; if (jac) dio = A.dinv[col]; if (do_x) xo = c.x[col]; }
-      if (halo_in) { rh = c.r[hcol]; ph = p_in[hcol]; if (jac) dih = A.dinv[hcol]; }
+      if (own) { ro = zs[col]; po = p_in[col]; if (jac) dio = A.dinv[col]; if (do_x) xo = c.x[col]; }
+      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = A.dinv[hcol]; }
       if (own) {
         pn_c = fma(beta, po, ro * dio);
         p_out[col] = pn_c;
@@ -95,14 +96,14 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
         }
         if (up3) {
           const int64_t j = i + np;
-          ro = c.r[j]; po = p_in[j];
+          ro = zs[j]; po = p_in[j];
           if (jac) dio = A.dinv[j];
           if (do_x) xo = c.x[j];
         }
       }
       if (up3 && halo_in) {
         const int64_t j = hcol + (int64_t)(z + 1) * np;
-        rh = c.r[j]; ph = p_in[j];
+        rh = zs[j]; ph = p_in[j];
         if (jac) dih = A.dinv[j];
       }
       // ---- 2. plane z of p' (written during the previous step) is complete; the loads above fly

@@ -13,7 +13,8 @@ constexpr int kAlign = 256;            // byte alignment of every section of the
 constexpr int kHeaderBytes = 512;
 constexpr uint64_t kMagic = 0x4355544844494131ull;  // "CUTHDIA1"
 constexpr int kMaxBlocks = 8192;       // upper bound on the grid of any reducing kernel
-constexpr int kNumPartialSlots = 4;    // partial-sum arrays (each kMaxBlocks doubles)
+constexpr int kNumPartialSlots = 4;
+constexpr int kMaxChebDegree = 64;    // partial-sum arrays (each kMaxBlocks doubles)
 
 // Host-computed placement of the sections inside the caller's matrix buffer.
 struct DiaLayout {
@@ -72,7 +73,13 @@ struct Ctx {
   double rtol;
   double soft_drift2;   // soft restart allowed while ||t - r||^2 <= soft_drift2 * ||t||^2
   int32_t precision, max_iters, period, jacobi;
-  int32_t soft_restart, pad0;
+  int32_t soft_restart, cheb;     // cheb: degree k of the Chebyshev polynomial preconditioner, 0 = off
+  // Chebyshev preconditioner (Alg. 3): z = q(A) r.  cz: z (fp64) handed to the outer
+  // loop; cd[2]: d ping-pong; crc: inner residual; czc: inner z accumulator (element type T = double
+  // in FP64 mode, float in MIXED mode; buffers are sized for double).
+  double* cz; void* cd[2]; void* crc; void* czc;
+  double cheb_inv_theta;
+  double cheb_c1[kMaxChebDegree], cheb_c2[kMaxChebDegree];   // d_{i+1} = c1[i] d_i + c2[i] r_c
 };
 
 // Scalars of the iteration; device resident, written only by "last block" epilogues.
@@ -81,16 +88,17 @@ struct Ctl {
   double tt, dd, tt_prev, rr_prev_eval;
   double xalpha;   // pending x += xalpha * p (fused path defers Alg. 1 line 8 by one kernel)
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
-  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, pad2, pad3;
+  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, beta_zero, pad3;
   unsigned int ticket[8];
 };
 
 struct Workspace {
   Ctx* ctx; Ctl* ctl; double* partials; double* r; double* p; double* p2; double* mu; double* b;
+  double* cz; double* cd0; double* cd1; double* crc; double* czc;
   size_t bytes;
 };
 
-inline Workspace carve_workspace(void* base, int64_t n, bool with_b) {
+inline Workspace carve_workspace(void* base, int64_t n, bool with_b, bool with_cheb = false) {
   Workspace w;
   char* c = (char*)base;
   size_t o = 0;
@@ -103,6 +111,11 @@ inline Workspace carve_workspace(void* base, int64_t n, bool with_b) {
   w.mu = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n);
   w.b = nullptr;
   if (with_b) { w.b = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
+  w.cz = w.cd0 = w.cd1 = w.crc = w.czc = nullptr;
+  if (with_cheb) {
+    double** v[5] = {&w.cz, &w.cd0, &w.cd1, &w.crc, &w.czc};
+    for (int k = 0; k < 5; ++k) { *v[k] = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
+  }
   w.bytes = o;
   return w;
 }

@@ -197,6 +197,7 @@ __global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp,
     ctl->beta = 0.0; ctl->alpha = 0.0;
     ctl->tt = acc[1]; ctl->tt_prev = acc[1]; ctl->rr_prev_eval = acc[1];
     ctl->stage = (c.precision == CUTH_MIXED) ? 0 : 1;
+    ctl->beta_zero = 1;          // Chebyshev path: the first p is z (Alg. 1 line 3)
     unsigned go = 1u;
     if (acc[2] == 0.0) { ctl->zero_rhs = 1; ctl->status = CUTH_SOLVE_CONVERGED; ctl->tt = 0.0; ctl->rr = 0.0; go = 0u; }
     else if (acc[1] <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }   // r0 IS the true residual
@@ -209,12 +210,13 @@ __global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp,
 __global__ void __launch_bounds__(kThreads) k_pupdate(const Ctx* __restrict__ ctxp, const Ctl* __restrict__ ctl) {
   const Ctx c = *ctxp;
   const double beta = ctl->beta;
+  const double* __restrict__ zs = c.cheb ? c.cz : c.r;     // Chebyshev: z = q(A) r is a stored vector
   CUTH_TILE_LOOP(c.A.n) {
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
       const int64_t i = base + threadIdx.x + k * kThreads;
       if (i < c.A.n) {
-        const double ri = c.r[i];
+        const double ri = zs[i];
         const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
         c.p[i] = fma(beta, c.p[i], zi);
       }
@@ -282,8 +284,10 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       go = 0u;
     } else {
       const double rho_new = acc[0], rr = acc[1];
-      ctl->beta = rho_new / ctl->rho;      // Alg. 1 line 11
-      ctl->rho = rho_new;
+      if (!c.cheb) {                       // Chebyshev: rho and beta come from k_cheb_last
+        ctl->beta = rho_new / ctl->rho;    // Alg. 1 line 11
+        ctl->rho = rho_new;
+      }
       ctl->rr = rr;
       const int it = ctl->it + 1;          // Alg. 1 line 13
       ctl->it = it;
@@ -294,7 +298,7 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       const bool c14a = early && rr <= ctl->sw2;
       const bool periodic = early && since >= c.period;
       const bool capped = it >= c.max_iters;
-      const bool bad = !(rr == rr) || !(rho_new == rho_new);
+      const bool bad = !(rr == rr) || (!c.cheb && !(rho_new == rho_new));
       ctl->conv_rec = conv_rec ? 1 : 0;
       if (bad) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
       else if (conv_rec || c14a || periodic || capped) want = 1u;
@@ -379,8 +383,13 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
   }
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[4], smem, &s_flag) && threadIdx.x == 0) {
     // mode 1: beta = 0 => p = z.  mode 2: beta_k = rho(new r) / rho_k, with rho_k = rho_rec / beta_rec.
-    ctl->beta = (mode == 2 && ctl->rho > 0.0) ? ctl->beta * (acc[0] / ctl->rho) : 0.0;
-    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->restart = 0; ctl->conv_rec = 0;
+    if (c.cheb) {      // the next k_cheb_last forms rho(new r) and beta = rho_new / rho_k itself
+      ctl->beta_zero = (mode == 1) ? 1 : 0;
+    } else {
+      ctl->beta = (mode == 2 && ctl->rho > 0.0) ? ctl->beta * (acc[0] / ctl->rho) : 0.0;
+      ctl->rho = acc[0];
+    }
+    ctl->rr = acc[1]; ctl->restart = 0; ctl->conv_rec = 0;
   }
 }
 

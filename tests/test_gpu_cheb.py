@@ -1,0 +1,141 @@
+"""GPU parity of the Chebyshev path: Lanczos bounds, one preconditioner apply
+(Alg. 3) and the PCG solve, against the CPU oracle, in both grid traversals."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import oracle as O
+from gpu_util import grid_from_workload, to_dev
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    dict(cfg=1, nx=7, ny=5, nz=4, n_hot=1),
+    dict(cfg=1),
+    dict(cfg=3, nx=37, ny=29, nz=16, n_hot=8),
+    dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8),
+    dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),
+]
+
+
+@pytest.fixture(params=["flat", "zmarch"], autouse=True)
+def traversal(request):
+    import paper_2606_17850_b200 as cu
+    cu.cuth_set_traversal({"flat": 1, "zmarch": 2}[request.param])
+    yield request.param
+    cu.cuth_set_traversal(0)
+
+
+def _rhs(w):
+    return w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
+
+
+def _setup(w, prec, steps=20, degree=30):
+    import paper_2606_17850_b200 as cu
+    M = cu.DiaMatrix(grid_from_workload(w))
+    S = cu.Solver(M, cu.Opts(precision=prec, rtol=1e-8, true_resid_period=w.true_resid_period))
+    b = _rhs(w)
+    lo, hi, gersh = S.setup_chebyshev(to_dev(b), lanczos_steps=steps, degree=degree)
+    return M, S, b, lo, hi, gersh
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_lanczos_bounds_vs_oracle(kw):
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    steps = 12
+    M, S, b, lo, hi, gersh = _setup(w, cu.FP64, steps=steps)
+    a, bt = O.lanczos(A, b, steps)
+    lo_o, hi_o = O.ritz_extremes(a, bt)
+    assert hi == pytest.approx(hi_o, rel=1e-6)
+    assert lo == pytest.approx(lo_o, rel=1e-4)
+    rowsum = np.abs(A.to_scipy()).sum(axis=1).max()
+    assert gersh == pytest.approx(rowsum, rel=1e-12)
+    assert S.opts.cheb_lmin == lo and S.opts.cheb_lmax == min(1.05 * hi, gersh)
+
+
+@pytest.mark.parametrize("kw", CASES)
+@pytest.mark.parametrize("degree", [3, 4, 30])
+def test_cheb_apply_fp64_vs_oracle(kw, degree):
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    M, S, b, lo, hi, gersh = _setup(w, cu.FP64, degree=degree)
+    r = W.normal01(w.seed, 50, 51, np.arange(w.n)) * 1e-7
+    z = torch.empty(w.n, dtype=torch.float64, device="cuda")
+    S.cheb_apply(to_dev(r), z)
+    ref = O.cheb_apply(A, r, S.opts.cheb_lmin, S.opts.cheb_lmax, degree)
+    assert np.abs(z.cpu().numpy() - ref).max() <= 1e-10 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_cheb_apply_fp32_close_to_oracle(kw):
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    M, S, b, lo, hi, gersh = _setup(w, cu.MIXED)
+    r = W.normal01(w.seed, 50, 51, np.arange(w.n)) * 1e-7
+    z = torch.empty(w.n, dtype=torch.float64, device="cuda")
+    S.cheb_apply(to_dev(r), z)
+    ref = O.cheb_apply(A, r, S.opts.cheb_lmin, S.opts.cheb_lmax, 30)
+    # fp32 vectors and fp32-stored matrix: a preconditioner-grade approximation of the same operator
+    assert np.linalg.norm(z.cpu().numpy() - ref) <= 2e-3 * np.linalg.norm(ref)
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_pcg_cheb_fp64_vs_oracle(kw):
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    M, S, b, lo, hi, gersh = _setup(w, cu.FP64)
+    ref = O.pcg_cheb(A, b, S.opts.cheb_lmin, S.opts.cheb_lmax, 30)
+    assert ref.status == 0
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    S.solve(to_dev(b), x)
+    res = S.result()
+    xh = x.cpu().numpy()
+    assert res.status == 0, res
+    assert np.linalg.norm(b - O.spmv(A, xh)) <= 1e-8 * np.linalg.norm(b)
+    assert np.abs(xh - ref.x).max() <= 1e-6 * np.abs(ref.x).max()
+    assert abs(res.iterations - ref.iterations) <= max(3, 0.1 * ref.iterations)
+    jac = O.pcg(A, b)
+    assert np.abs(xh - jac.x).max() <= 1e-6 * np.abs(jac.x).max()      # same x whatever the preconditioner
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_pcg_cheb_mixed_vs_oracle(kw):
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    M, S, b, lo, hi, gersh = _setup(w, cu.MIXED)
+    ref = O.pcg(A, b)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    S.solve(to_dev(b), x)
+    res = S.result()
+    xh = x.cpu().numpy()
+    assert res.status == 0, res
+    assert np.linalg.norm(b - O.spmv(A, xh)) <= 1e-8 * np.linalg.norm(b)
+    assert np.abs(xh - ref.x).max() <= 1e-4
+    if w.n >= 8192:
+        assert res.iterations < ref.iterations / 2                      # far fewer outer iterations than Jacobi
+
+
+def test_cheb_bad_interval_rejected_or_reported():
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(1, nx=8, ny=6, nz=4, n_hot=1)
+    M = cu.DiaMatrix(grid_from_workload(w))
+    bad = cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_degree=30, cheb_lmin=1.0, cheb_lmax=0.5)
+    S = cu.Solver(M, bad)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    with pytest.raises(cu.CuthError) as e:
+        S.solve(to_dev(w.power), x)
+    assert e.value.code == -3
+    S2 = cu.Solver(M, cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_degree=2, cheb_lmin=1e-6, cheb_lmax=1e-3))
+    with pytest.raises(cu.CuthError):
+        S2.solve(to_dev(w.power), x)
