@@ -183,6 +183,10 @@ def main():
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-reps", type=int, default=20)
+    ap.add_argument("--preconditioner", default="jacobi", choices=["jacobi", "chebyshev"],
+                    help="jacobi = the north_star hot path; chebyshev = the paper's own preconditioner (Alg. 3)")
+    ap.add_argument("--cheb-degree", type=int, default=30)
+    ap.add_argument("--lanczos-steps", type=int, default=40)
     ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
@@ -232,6 +236,13 @@ def main():
     b = b_host.cuda()
     b_stage = torch.empty(w.n, dtype=torch.float64, device="cuda")
     x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    cheb = args.preconditioner == "chebyshev"
+    setup_ms = 0.0
+    if cheb:       # setup: Lanczos on the device + tridiagonal eigenvalues on the host, once per matrix
+        torch.cuda.synchronize()
+        t0 = time.time()
+        bounds = S.setup_chebyshev(b[0], lanczos_steps=args.lanczos_steps, degree=args.cheb_degree)
+        setup_ms = (time.time() - t0) * 1e3
     counters = torch.zeros(4, dtype=torch.int32, device="cuda")     # status, iterations, promotions, evals
     early_acc = torch.zeros(1, dtype=torch.int32, device="cuda")   # iterations done on the fp32-stored operator
     res_i32 = S.result_dev.view(torch.int32)
@@ -302,6 +313,9 @@ def main():
     names = ({4: "k_fused_pspmv", 5: "k_update_nox", 3: "k_true_resid"} if fused else
              {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"})
     body_ids = (4, 5) if fused else (0, 1, 2)
+    if cheb:
+        names[7 if mixed else 6] = "k_cheb_mid"
+        body_ids = tuple([7 if mixed else 6] * (args.cheb_degree - 1)) + body_ids
     for kid, nm in names.items():
         for _ in range(3):
             cu.cuth_profile_kernel(S.work, g, kid)
@@ -342,6 +356,15 @@ def main():
     early = int(early_acc.item()) if mixed else 0
     late = it - early
     iter_bytes = (early * bytes_per_row(w, "iter_mixed") + late * bytes_per_row(w, "iter_fp64")) * w.n
+    m = m_ratio(w)
+    if cheb:
+        # outer: K1 (matrix + z, p, x read + p', mu, x written) + K2 (r, mu read, r written); preconditioner:
+        # FIRST M+8+3s, (k-3) x MID M+6s, LAST M+3s+16 with s = sizeof(T), M = matrix bytes per row
+        k, sT = args.cheb_degree, (4 if mixed else 8)
+        Mc = 4 * (m - 1) if mixed else 8 * m
+        apply_bytes = (k - 1) * Mc + (3 * sT + 8) + (k - 3) * 6 * sT + (3 * sT + 16)
+        outer = lambda M_: M_ + 48 + 24
+        iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
     stage_fp64 = (not mixed) or res.promotions > 0     # operator the armed profile kernels ran with
     m = m_ratio(w)
@@ -351,7 +374,11 @@ def main():
     else:
         dom_name, dom_ms = "k_spmv_dot", kern["k_spmv_dot"]
         dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
-    per_it = 2 if fused else 3
+    if cheb:
+        dom_name, dom_ms = "k_cheb_mid", kern["k_cheb_mid"]
+        dom_bytes = ((4 * (m - 1) + 24) if mixed else (8 * m + 48)) * w.n
+        stage_fp64 = not mixed
+    per_it = (2 if fused else 3) + (args.cheb_degree - 1 if cheb else 0)
     per_eval = 3 if fused else 2
     launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
 
@@ -360,7 +387,9 @@ def main():
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz],
-                   "precision": "mixed" if mixed else "fp64", "rtol": w.rtol, "preconditioner": "jacobi",
+                   "precision": "mixed" if mixed else "fp64", "rtol": w.rtol, "preconditioner": args.preconditioner,
+                   **({"cheb_degree": args.cheb_degree, "lanczos_steps": args.lanczos_steps,
+                       "cheb_interval": [S.opts.cheb_lmin, S.opts.cheb_lmax]} if cheb else {}),
                    "l2_policy": ("inputs larger than L2 (matrix + vectors = %.2f GB streamed per iteration)" if
                                  (8 * m_ratio(w) + 48) * w.n > 126e6 else
                                  "working set %.3f GB fits the 126 MB L2: L2-resident, latency-bound case, "
@@ -380,9 +409,10 @@ def main():
         "roofline_iteration": {"bound": "hbm", "achieved": iter_gbs, "peak": peak, "unit": "GB/s",
                                "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
                                "algorithmic_bytes_per_solve": iter_bytes,
-                               "note": "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
+                               "note": ("Chebyshev: outer K1+K2 plus (k-1)-kernel apply bytes per row per iteration " if cheb else "") +
+                                       "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
-        "kernels_ms": kern, "spmv": spmv,
+        "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
         "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,

@@ -170,7 +170,8 @@ int cuth_set_traversal(int mode);
  * still in this workspace, outside the graph and with the graph's launch configuration, so that it
  * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the
  * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual,
- * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
+ * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path),
+ * 6 / 7 = one middle step of the Chebyshev apply in fp64 / fp32 (only after a CUTH_PRECOND_CHEBYSHEV solve).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
 int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
 
 #ifdef __cplusplus

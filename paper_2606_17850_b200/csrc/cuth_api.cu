@@ -57,6 +57,14 @@ static int stencil_blocks(const DiaLayout& L) {
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
+static int grid_blocks(int64_t n);
+
+static int cheb_blocks(const DiaLayout& L) {
+  if (!use_zmarch(L)) return grid_blocks(L.n);
+  const int64_t tiles = ((L.nx + ZTX - 1) / ZTX) * ((L.ny + CUTH_CHEB_NC * ZTY - 1) / (CUTH_CHEB_NC * ZTY));
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
+}
+
 static int fused_blocks(const DiaLayout& L) {
   const int64_t tiles = ((L.nx + FTX - 1) / FTX) * ((L.ny + FTY - 1) / FTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
@@ -112,7 +120,8 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
 
-static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, GraphEntry* out) {
+static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
+                       GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -143,17 +152,17 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   if (kdeg > 0) {
     const bool f32 = (chebkey & 1) != 0;
     { void* a[] = {&ctx};
-      CU(add_kernel(body, &n_c, nullptr, 0, f32 ? (void*)k_cheb_first<float> : (void*)k_cheb_first<double>, sblocks, a)); }
+      CU(add_kernel(body, &n_c, nullptr, 0, f32 ? (void*)k_cheb_first<float> : (void*)k_cheb_first<double>, cblocks, a)); }
     for (int i = 1; i <= kdeg - 3; ++i) {
       cudaGraphNode_t prev = n_c;
       int step = i;
       void* a[] = {&ctx, &step};
-      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, sblocks, a));
+      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, cblocks, a));
     }
     { cudaGraphNode_t prev = n_c;
       int step = kdeg - 2;
       void* a[] = {&ctx, &ctl, &partials, &step};
-      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_last<float> : (void*)k_cheb_last<double>, sblocks, a)); }
+      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_last<float> : (void*)k_cheb_last<double>, cblocks, a)); }
   }
   const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
   const size_t ndep0 = n_c ? 1 : 0;
@@ -195,7 +204,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 }
 
 static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     cudaGraphExec_t* ex) {
+                     int cblocks, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
@@ -210,7 +219,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -294,7 +303,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   CU(cudaGetLastError());
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
-                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, &ex);
+                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, cheb_blocks(L), &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -429,6 +438,8 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 4: k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 6: k_cheb_mid<double><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1); break;     // needs a Chebyshev solve's context
+    case 7: k_cheb_mid<float><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1); break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
   }
@@ -497,7 +508,7 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   c.cz = z_D;
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   const int blocks = grid_blocks(L.n);
-  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
+  const int sb = cheb_blocks(L);
   const int k = opts->cheb_degree;
   if (opts->precision == CUTH_MIXED) {
     k_cheb_first<float><<<sb, kThreads, 0, st>>>(w.ctx);

@@ -14,6 +14,11 @@
 
 namespace cuth {
 
+#ifndef CUTH_CHEB_MINB32
+#define CUTH_CHEB_MINB32 8
+#endif
+#define CUTH_CHEB_NC 1   // columns per thread of the z-marching stencil (2 and 4 measured slower, _work sweep)
+
 // One row of A v with v stored as VT and arithmetic in T (T = double: A1 standard form; T = float: A2
 // difference form, DESIGN.md R-F3), flat traversal.
 template <class VT, class T>
@@ -108,7 +113,7 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
 // ---------------------------------------------------------------------------------------------
 // Alg. 3 lines 1-4 and the first pass of lines 6-10.
 template <class T>
-__global__ void __launch_bounds__(kThreads, 4) k_cheb_first(const Ctx* __restrict__ ctxp) {
+__global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_first(const Ctx* __restrict__ ctxp) {
   const Ctx c = *ctxp;
   const T inv_theta = (T)c.cheb_inv_theta, c1 = (T)ctxp->cheb_c1[0], c2 = (T)ctxp->cheb_c2[0];
   T* __restrict__ rc = (T*)c.crc;
@@ -125,7 +130,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_first(const Ctx* __restric
 
 // Alg. 3 lines 6-10 for 0 < i < k-2.
 template <class T>
-__global__ void __launch_bounds__(kThreads, 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
+__global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
   const T* __restrict__ din = (const T*)ctxp->cd[step & 1];
@@ -142,7 +147,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_mid(const Ctx* __restrict_
 
 // Last stencil pass (i = k-2) + the two trailing z updates + rho = r.z (Alg. 1 lines 10-11).
 template <class T>
-__global__ void __launch_bounds__(kThreads, 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+__global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                         int step) {
   __shared__ double smem[32];
   __shared__ int s_flag;
