@@ -20,13 +20,16 @@ from gpu_util import grid_from_workload, to_dev
 pytestmark = pytest.mark.gpu
 
 
-def _solve(w, prec, b=None):
+def _solve(w, prec, b=None, chebyshev=False):
     import torch
     import paper_2606_17850_b200 as cu
     M = cu.DiaMatrix(grid_from_workload(w))
     S = cu.Solver(M, cu.Opts(precision=prec, rtol=1e-8, true_resid_period=w.true_resid_period))
+    bd = to_dev(w.power if b is None else b)
+    if chebyshev:
+        S.setup_chebyshev(bd, lanczos_steps=40, degree=30)
     x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
-    S.solve(to_dev(w.power if b is None else b), x)
+    S.solve(bd, x)
     res = S.result()
     xh = x.cpu().numpy()
     S.close()
@@ -64,11 +67,22 @@ def test_cfg3_full_size(mode):
             assert abs(s - w.power[i]) <= 1e-6 * np.abs(A.val[A.rowptr[i]:A.rowptr[i + 1]]).max() * x.max()
 
 
-@pytest.mark.parametrize("mode", ["fp64", "mixed"])
+def test_cfg3_full_size_chebyshev_mixed():
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(3)
+    A = O.assemble_workload(w)
+    x, res = _solve(w, cu.MIXED, chebyshev=True)
+    _check_invariants(w, A, w.power, x, res)
+    assert res.iterations < 1000                 # Jacobi needs 4499 (Table VII: 44-107 vs 647-1593)
+    xj, _ = _solve(w, cu.FP64)
+    assert np.abs(x - xj).max() <= 1e-4          # same temperatures as the Jacobi fp64 solve
+
+
+@pytest.mark.parametrize("mode", ["fp64", "mixed", "chebyshev-mixed"])
 def test_cfg4_full_size(mode):
     import paper_2606_17850_b200 as cu
     w = W.make_workload(4)
-    x, res = _solve(w, cu.FP64 if mode == "fp64" else cu.MIXED)
+    x, res = _solve(w, cu.FP64 if mode == "fp64" else cu.MIXED, chebyshev=mode.startswith("chebyshev"))
     assert res.status == 0, res
     xd = solve_layered(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.kappa_layer, w.h_top, w.power)
     err = np.abs(x - xd).max()
