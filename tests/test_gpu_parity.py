@@ -238,3 +238,63 @@ def test_transient_requires_transient_matrix():
     with pytest.raises(cu.CuthError) as e:
         S.step(to_dev(w.power), T)
     assert e.value.code == -7
+
+
+# ---------------------------------------------------------------- memory safety without a sanitizer
+@pytest.mark.parametrize("kw", [dict(cfg=1, nx=7, ny=5, nz=3, n_hot=1), dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),
+                                dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8)])
+@pytest.mark.parametrize("precond", ["jacobi", "chebyshev"])
+def test_no_out_of_bounds_canaries(kw, precond):
+    """compute-sanitizer is closed on this GPU pool, so: every caller-owned buffer (matrix object, workspace,
+    b, x, result) is carved out of a larger NaN-filled arena with the exact size the ABI asks for.  An
+    out-of-bounds WRITE would disturb the NaN guard words (checked bitwise); an out-of-bounds READ would pull
+    a NaN into the arithmetic (even 0 * NaN = NaN) and change the result, which must be bit-identical to the
+    run on ordinary allocations."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    g = grid_from_workload(w)
+    b_np = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
+
+    def run(guarded):
+        opts = cu.Opts(precision=cu.MIXED, rtol=1e-8, true_resid_period=5)
+        sizes = {"dia": cu.cuth_dia_bytes(g), "b": 8 * w.n, "x": 8 * w.n, "res": 64}
+        pad = 4096 if guarded else 0
+        bufs, arenas = {}, {}
+
+        def carve(name, nbytes):
+            tot = nbytes + 2 * pad
+            arena = torch.full((tot // 8 + 1,), float("nan"), dtype=torch.float64, device="cuda").view(torch.uint8)
+            arenas[name] = (arena, nbytes)
+            bufs[name] = arena[pad:pad + nbytes]
+
+        for k, v in sizes.items():
+            carve(k, v)
+        cu.cuth_build_dia(g, bufs["dia"])
+        bufs["b"].view(torch.float64).copy_(to_dev(b_np))
+        x = bufs["x"].view(torch.float64)
+        x.zero_()
+        if precond == "chebyshev":
+            carve("work0", cu.cuth_workspace_bytes(g, opts))
+            bounds = cu.cuth_lanczos_bounds(bufs["dia"], g, bufs["b"].view(torch.float64), 20, bufs["work0"])
+            opts = cu.Opts(precision=cu.MIXED, rtol=1e-8, true_resid_period=5, preconditioner=cu.PRECOND_CHEBYSHEV,
+                           cheb_degree=12, cheb_lmin=bounds[3], cheb_lmax=bounds[4])
+        carve("work", cu.cuth_workspace_bytes(g, opts))
+        cu.cuth_pcg_solve(bufs["dia"], g, opts, bufs["b"].view(torch.float64), x, bufs["work"], bufs["res"])
+        torch.cuda.synchronize()
+        cu.cuth_release_workspace(bufs["work"])
+        if guarded:
+            for name, (arena, nbytes) in arenas.items():
+                lo = arena[:pad].view(torch.int64)
+                hi = arena[pad + nbytes: pad + nbytes + pad - 8].view(torch.int64) if (pad + nbytes) % 8 == 0 else None
+                nanbits = torch.tensor([float("nan")], dtype=torch.float64, device="cuda").view(torch.int64)
+                assert bool((lo == nanbits).all()), f"guard below {name} overwritten"
+                if hi is not None:
+                    assert bool((hi == nanbits).all()), f"guard above {name} overwritten"
+        return x.clone().cpu().numpy(), bufs["res"][:8].view(torch.int32).cpu().numpy().copy()
+
+    x0, r0 = run(False)
+    x1, r1 = run(True)
+    assert r0[0] == 0 and r1[0] == 0
+    assert np.array_equal(r0, r1)
+    assert np.array_equal(x0.view(np.uint64), x1.view(np.uint64))
