@@ -152,7 +152,7 @@ def run_reference(args):
     A = O.assemble_workload(w)
     b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
     iters = int(max(3, min(200, 2.5e8 / w.n)))
-    nominal = {1: 288, 2: 1462, 3: 4500, 4: 8000, 5: 550}[args.config]
+    nominal = {1: 288, 2: 1462, 3: 4500, 4: 9791, 5: 580, 6: 1500}[args.config]
     for _ in range(args.warmup):
         O.pcg_window(A, b, np.zeros(w.n), 1)
     t0 = time.time()
@@ -178,7 +178,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--precision", default=None, choices=["fp64", "mixed"])
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

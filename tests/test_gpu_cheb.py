@@ -15,6 +15,7 @@ CASES = [
     dict(cfg=3, nx=37, ny=29, nz=16, n_hot=8),
     dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8),
     dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),
+    dict(cfg=6, nx=45, ny=38, nz=10, n_hot=6),     # paper-like anisotropic stack
 ]
 
 

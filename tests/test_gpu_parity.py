@@ -29,6 +29,7 @@ SMALL = [
     dict(cfg=3, nx=37, ny=29, nz=16, n_hot=8),     # per-cell lognormal kappa, ragged sizes
     dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8),     # transient matrix (C/dt on the diagonal)
     dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),     # several tiles + ragged tail (N = 69 680)
+    dict(cfg=6, nx=45, ny=38, nz=10, n_hot=6),     # paper-like anisotropic stack: dz 2-1000 um, 50 um cells
 ]
 
 

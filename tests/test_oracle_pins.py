@@ -249,6 +249,18 @@ def test_transient_step_vs_direct_and_energy_balance():
         T = r.x
 
 
+def test_paperlike_anisotropic_stack_vs_direct_solve():
+    # cfg 6: the paper's layer thicknesses 2-1000 um with 50 um cells: diagonals differ by 1e5
+    w = W.make_workload(6, nx=40, ny=36, nz=10, n_hot=6)
+    A = O.assemble_workload(w)
+    r = O.pcg(A, w.power, rtol=1e-9)
+    assert r.status == 0
+    xd = solve_layered(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.kappa_layer, w.h_top, w.power)
+    assert np.abs(r.x - xd).max() <= 1e-7 * np.abs(xd).max()
+    top = r.x.reshape(w.nz, -1)[w.nz - 1]
+    assert (w.h_top * w.dx * w.dy * top).sum() == pytest.approx(w.power.sum(), rel=1e-7)
+
+
 def test_pcg_lognormal_small_vs_cholesky():
     w = W.make_workload(3, nx=12, ny=10, nz=16, n_hot=6)
     A = O.assemble_workload(w)

@@ -29,8 +29,9 @@ CONFIG_NAMES = {
     3: "cfg3_steady_1024x1024x16_lognormal",
     4: "cfg4_steady_4096x4096x8",
     5: "cfg5_transient_512x512x16",
+    6: "cfg6_paperlike_anisotropic_256x256x10",
 }
-SEEDS = {1: 178501, 2: 178502, 3: 178503, 4: 178504, 5: 178505}
+SEEDS = {1: 178501, 2: 178502, 3: 178503, 4: 178504, 5: 178505, 6: 178506}
 
 # stream ids (the second key component)
 _ST_KAPPA_U1, _ST_KAPPA_U2 = 1, 2
@@ -46,6 +47,15 @@ S8P = [130.0, 2.0, 2.0, 130.0, 5.0, 400.0, 400.0, 400.0]
 _CV = {130.0: 1.63e6, 2.0: 2.2e6, 5.0: 2.0e6, 400.0: 3.45e6}
 
 W_PER_MM2 = 1.0e6  # 1 W/mm^2 in W/m^2
+
+# cfg 6: the layer THICKNESSES of the paper's 10-layer Memory-on-Logic stack,
+# bottom to top (logic bulk 10, logic FEOL 2, logic BEOL 10, hybrid bonding 2, memory BEOL 10,
+# memory FEOL 2, memory bulk 200, TIM 100, heat spreader 400, heat sink 1000 um).  Conductivities and the
+# lateral cell size are not given in the paper: this build's choice (Si 130, BEOL / bonding 2, TIM 5,
+# spreader and sink 400 W/m.K; 50 um cells).  Power on the two FEOL layers.  The floorplan power maps
+# (SPARC / EV6 / 9-core) are not available: the synthetic hotspot maps are used instead.
+PAPER_DZ_UM = [10.0, 2.0, 10.0, 2.0, 10.0, 2.0, 200.0, 100.0, 400.0, 1000.0]
+PAPER_KAPPA = [130.0, 130.0, 2.0, 2.0, 2.0, 130.0, 130.0, 5.0, 400.0, 400.0]
 
 
 def splitmix64(key: np.ndarray) -> np.ndarray:
@@ -156,10 +166,10 @@ def _sites(seed, nx, ny, n_sites):
 
 def make_workload(cfg: int, nx: int = 0, ny: int = 0, nz: int = 0, n_hot: int = -1,
                   seed: int = 0) -> Workload:
-    """Build config `cfg` (1..5).  nx/ny/nz/n_hot override the full size to get a
+    """Build config `cfg` (1..5 = BASELINE.json; 6 = paper-like anisotropic stack).  nx/ny/nz/n_hot override the full size to get a
     small grid with the same recipe (used by the parity tests)."""
     full = {1: (32, 32, 8, 4), 2: (256, 256, 16, 64), 3: (1024, 1024, 16, 1024),
-            4: (4096, 4096, 8, 4096), 5: (512, 512, 16, 256)}[cfg]
+            4: (4096, 4096, 8, 4096), 5: (512, 512, 16, 256), 6: (256, 256, 10, 64)}[cfg]
     nx = nx or full[0]
     ny = ny or full[1]
     nz = nz or full[2]
@@ -178,13 +188,23 @@ def make_workload(cfg: int, nx: int = 0, ny: int = 0, nz: int = 0, n_hot: int = 
     kappa_cell = None
     cvol = None
     dt = 0.0
-    mixed = cfg in (2, 3, 4, 5)
+    mixed = cfg in (2, 3, 4, 5, 6)
     period = 20
     n_steps = 0
     n_sites = 0
     extra = {}
 
-    if cfg in (1, 2):
+    if cfg == 6:
+        assert nz == 10, "cfg 6 is the paper's 10-layer stack"
+        dx = dy = 50.0e-6
+        dz = np.array(PAPER_DZ_UM) * 1e-6
+        kl = np.array(PAPER_KAPPA)
+        active = [1, 5]
+        bg = 0.05 * W_PER_MM2
+        for z in active:
+            q[z] += bg
+        _add_gaussian_hotspots(q, nx, ny, active, n_hot, seed, 1.0 * W_PER_MM2)
+    elif cfg in (1, 2):
         for z in active:
             q[z] += bg
         _add_gaussian_hotspots(q, nx, ny, active, n_hot, seed, 20.0 * W_PER_MM2)
