@@ -59,11 +59,20 @@ static int stencil_blocks(const DiaLayout& L) {
 
 static int grid_blocks(int64_t n);
 
+// fp32 Chebyshev middle step with two x-adjacent columns per thread: large planes with even nx
+static bool cheb_x2(const DiaLayout& L);
+static int cheb_x2_blocks(const DiaLayout& L) {
+  const int64_t tiles = ((L.nx + 2 * ZTX - 1) / (2 * ZTX)) * ((L.ny + ZTY - 1) / ZTY);
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
+}
+
 static int cheb_blocks(const DiaLayout& L) {
   if (!use_zmarch(L)) return grid_blocks(L.n);
   const int64_t tiles = ((L.nx + ZTX - 1) / ZTX) * ((L.ny + CUTH_CHEB_NC * ZTY - 1) / (CUTH_CHEB_NC * ZTY));
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
+
+static bool cheb_x2(const DiaLayout& L) { return use_zmarch(L) && (L.nx % 2 == 0); }
 
 static int fused_blocks(const DiaLayout& L) {
   const int64_t tiles = ((L.nx + FTX - 1) / FTX) * ((L.ny + FTY - 1) / FTY);
@@ -103,6 +112,7 @@ struct GraphEntry {
   int sblocks = 0;
   int fblocks = 0;
   int chebkey = 0;
+  int x2blocks = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -121,7 +131,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
 }
 
 static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
-                       GraphEntry* out) {
+                       int x2blocks, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -157,7 +167,10 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
       cudaGraphNode_t prev = n_c;
       int step = i;
       void* a[] = {&ctx, &step};
-      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, cblocks, a));
+      if (f32 && x2blocks > 0)
+        CU(add_kernel(body, &n_c, &prev, 1, (void*)k_cheb_mid_f32x2, x2blocks, a));
+      else
+        CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, cblocks, a));
     }
     { cudaGraphNode_t prev = n_c;
       int step = kdeg - 2;
@@ -198,20 +211,21 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
 static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     int cblocks, cudaGraphExec_t* ex) {
+                     int cblocks, int x2blocks, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
   cudaGetDevice(&dev);
   if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
-                               it->second.fblocks != fblocks || it->second.chebkey != chebkey)) {
+                               it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
+                               it->second.x2blocks != x2blocks)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -219,7 +233,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -303,7 +317,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   CU(cudaGetLastError());
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
-                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, cheb_blocks(L), &ex);
+                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -439,7 +453,10 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 4: k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 6: k_cheb_mid<double><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1); break;     // needs a Chebyshev solve's context
-    case 7: k_cheb_mid<float><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1); break;
+    case 7:
+      if (cheb_x2(L)) k_cheb_mid_f32x2<<<cheb_x2_blocks(L), kThreads, 0, st>>>(w.ctx, 1);
+      else k_cheb_mid<float><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1);
+      break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
   }
@@ -512,7 +529,10 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   const int k = opts->cheb_degree;
   if (opts->precision == CUTH_MIXED) {
     k_cheb_first<float><<<sb, kThreads, 0, st>>>(w.ctx);
-    for (int i = 1; i <= k - 3; ++i) k_cheb_mid<float><<<sb, kThreads, 0, st>>>(w.ctx, i);
+    for (int i = 1; i <= k - 3; ++i) {
+      if (cheb_x2(L)) k_cheb_mid_f32x2<<<cheb_x2_blocks(L), kThreads, 0, st>>>(w.ctx, i);
+      else k_cheb_mid<float><<<sb, kThreads, 0, st>>>(w.ctx, i);
+    }
     k_cheb_last<float><<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, k - 2);
   } else {
     k_cheb_first<double><<<sb, kThreads, 0, st>>>(w.ctx);

@@ -145,6 +145,61 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
   });
 }
 
+// The same middle step for T = float on large planes with even nx: each thread owns TWO x-adjacent columns,
+// so the vectors d, rc, zc move as 8-byte float2 (every row start is even => 8-byte aligned), the +-1
+// neighbours of the pair are each other (registers), and a thread keeps twice the bytes in flight -- the
+// 4-byte version is latency-bound (profiles/r1c_cfg3_cheb_mixed.md).  Matrix entries stay scalar loads: the
+// packed diagonals D2, D3 start at odd elements (R-G5b).  Tile = (2 ZTX) x ZTY columns per CTA.
+__global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __restrict__ ctxp, int step) {
+  const Ctx c = *ctxp;
+  const DiaDev& A = c.A;
+  const float c1 = (float)ctxp->cheb_c1[step], c2 = (float)ctxp->cheb_c2[step];
+  const float* __restrict__ din = (const float*)ctxp->cd[step & 1];
+  float* __restrict__ dout = (float*)ctxp->cd[(step + 1) & 1];
+  float* __restrict__ rc = (float*)c.crc;
+  float* __restrict__ zc = (float*)c.czc;
+  const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
+  const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
+  const int tiles_x = (nxi + 2 * ZTX - 1) / (2 * ZTX), tiles_y = (nyi + ZTY - 1) / ZTY;
+  const int ntiles = tiles_x * tiles_y;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  auto ld2 = [](const float* p) { return *reinterpret_cast<const float2*>(p); };
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int bx = t % tiles_x, by = t / tiles_x;
+    const int x = bx * 2 * ZTX + 2 * tx, y = by * ZTY + ty;
+    if (x >= nxi || y >= nyi) continue;                 // nx even: x + 1 < nx as well
+    const int64_t c0 = x + nx * (int64_t)y;
+    float2 v_lo = make_float2(0.f, 0.f), v_c = ld2(din + c0), a3l = make_float2(0.f, 0.f);
+#pragma unroll 2
+    for (int z = 0; z < nz; ++z) {
+      const int64_t i = c0 + (int64_t)z * np;
+      const bool up3 = z + 1 < nz, up2 = i + nx < n, lo2 = i >= nx, lo1 = i >= 1, up1 = i + 2 < n;
+      const float f1l = lo1 ? A.f1[i - 1] : 0.f, f1a = A.f1[i], f1b = up1 ? A.f1[i + 1] : 0.f;
+      const float f2u0 = up2 ? A.f2[i] : 0.f, f2u1 = up2 ? A.f2[i + 1] : 0.f;
+      const float f2l0 = lo2 ? A.f2[i - nx] : 0.f, f2l1 = lo2 ? A.f2[i + 1 - nx] : 0.f;
+      float2 a3u = make_float2(0.f, 0.f);
+      if (up3) { a3u.x = A.f3[i]; a3u.y = A.f3[i + 1]; }
+      const float2 v_hi = up3 ? ld2(din + i + np) : v_c;
+      const float2 v2u = up2 ? ld2(din + i + nx) : v_c, v2l = lo2 ? ld2(din + i - nx) : v_c;
+      const float vl = lo1 ? din[i - 1] : v_c.x, vr = up1 ? din[i + 2] : v_c.y;
+      const float2 rcv = ld2(rc + i), zcv = ld2(zc + i);
+      const float s = (float)A.s_layer[z];
+      float a0 = s * v_c.x, a1 = s * v_c.y;
+      a0 += f1a * (v_c.y - v_c.x);   a1 += f1a * (v_c.x - v_c.y);
+      a0 += f1l * (vl - v_c.x);      a1 += f1b * (vr - v_c.y);
+      a0 += f2u0 * (v2u.x - v_c.x);  a1 += f2u1 * (v2u.y - v_c.y);
+      a0 += f2l0 * (v2l.x - v_c.x);  a1 += f2l1 * (v2l.y - v_c.y);
+      a0 += a3u.x * (v_hi.x - v_c.x); a1 += a3u.y * (v_hi.y - v_c.y);
+      a0 += a3l.x * (v_lo.x - v_c.x); a1 += a3l.y * (v_lo.y - v_c.y);    // a3l = 0 at z = 0
+      const float2 rn = make_float2(rcv.x - a0, rcv.y - a1);
+      *reinterpret_cast<float2*>(rc + i) = rn;
+      *reinterpret_cast<float2*>(zc + i) = make_float2(zcv.x + v_c.x, zcv.y + v_c.y);
+      *reinterpret_cast<float2*>(dout + i) = make_float2(c1 * v_c.x + c2 * rn.x, c1 * v_c.y + c2 * rn.y);
+      v_lo = v_c; v_c = v_hi; a3l = a3u;
+    }
+  }
+}
+
 // Last stencil pass (i = k-2) + the two trailing z updates + rho = r.z (Alg. 1 lines 10-11).
 template <class T>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
