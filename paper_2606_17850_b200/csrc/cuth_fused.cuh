@@ -158,18 +158,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_fused_pspmv(const Ctx* __restri
   if (ctl->stage == 0) fused_pspmv_body<true>(c, p_in, p_out, beta, xalpha, sp, acc[0]);
   else fused_pspmv_body<false>(c, p_in, p_out, beta, xalpha, sp, acc[0]);
   if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
-    const double pAp = acc[0];
-    ctl->pAp = pAp;
     ctl->pcur = pcur ^ 1;
-    const double rho = ctl->rho;
-    if (!(pAp > 0.0) || !(pAp <= 1.79e308) || !(rho == rho)) {
-      ctl->alpha = 0.0; ctl->xalpha = 0.0;
-      ctl->status = CUTH_SOLVE_BREAKDOWN;
-    } else {
-      const double alpha = rho / pAp;      // Alg. 1 line 7
-      ctl->alpha = alpha;
-      ctl->xalpha = alpha;                 // x += alpha p is applied by the next K1 (or by k_flush_x)
-    }
+    policy_after_spmv(ctl, acc[0], true);       // Alg. 1 line 7; x += alpha p deferred to the next K1
   }
 }
 

@@ -2,6 +2,7 @@
 // Alg. 1 with M = diag(A); Alg. 2 for the SpMV.
 #pragma once
 #include "cuth_internal.cuh"
+#include "cuth_policy.cuh"
 
 namespace cuth {
 
@@ -191,17 +192,7 @@ __global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp,
     acc[2] = fma(bi, bi, acc[2]);
   });
   if (grid_sum_last_block<3>(acc, partials, &ctl->ticket[0], smem, &s_flag) && threadIdx.x == 0) {
-    ctl->rho = acc[0]; ctl->rr = acc[1]; ctl->bb = acc[2];
-    ctl->tol2 = c.rtol * c.rtol * acc[2];
-    ctl->sw2 = c.rtol * acc[2];                  // (sqrt(rtol) ||b||)^2, eq. (14a) relative (R-G8)
-    ctl->beta = 0.0; ctl->alpha = 0.0;
-    ctl->tt = acc[1]; ctl->tt_prev = acc[1]; ctl->rr_prev_eval = acc[1];
-    ctl->stage = (c.precision == CUTH_MIXED) ? 0 : 1;
-    ctl->beta_zero = 1;          // Chebyshev path: the first p is z (Alg. 1 line 3)
-    unsigned go = 1u;
-    if (acc[2] == 0.0) { ctl->zero_rhs = 1; ctl->status = CUTH_SOLVE_CONVERGED; ctl->tt = 0.0; ctl->rr = 0.0; go = 0u; }
-    else if (acc[1] <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }   // r0 IS the true residual
-    else if (!(acc[0] == acc[0]) || !(acc[1] == acc[1])) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
+    const unsigned go = policy_init(ctl, c, acc[0], acc[1], acc[2]);
     cudaGraphSetConditional(h_while, go);
   }
 }
@@ -241,15 +232,7 @@ __global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_dot(const Ctx* __r
   if (ctl->stage == 0) spmv_dot_body<true>(c, acc[0]);
   else spmv_dot_body<false>(c, acc[0]);
   if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
-    const double pAp = acc[0];
-    ctl->pAp = pAp;
-    const double rho = ctl->rho;
-    if (!(pAp > 0.0) || !(pAp <= 1.79e308) || !(rho == rho)) {
-      ctl->alpha = 0.0;
-      ctl->status = CUTH_SOLVE_BREAKDOWN;
-    } else {
-      ctl->alpha = rho / pAp;            // Alg. 1 line 7
-    }
+    policy_after_spmv(ctl, acc[0], false);      // Alg. 1 line 7
   }
 }
 
@@ -279,31 +262,8 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
     }
   }
   if (grid_sum_last_block<2>(acc, partials + kMaxBlocks, &ctl->ticket[2], smem, &s_flag) && threadIdx.x == 0) {
-    unsigned go = 1u, want = 0u;
-    if (ctl->status == CUTH_SOLVE_BREAKDOWN) {
-      go = 0u;
-    } else {
-      const double rho_new = acc[0], rr = acc[1];
-      if (!c.cheb) {                       // Chebyshev: rho and beta come from k_cheb_last
-        ctl->beta = rho_new / ctl->rho;    // Alg. 1 line 11
-        ctl->rho = rho_new;
-      }
-      ctl->rr = rr;
-      const int it = ctl->it + 1;          // Alg. 1 line 13
-      ctl->it = it;
-      const int since = ctl->since_eval + 1;
-      ctl->since_eval = since;
-      const bool conv_rec = rr <= ctl->tol2;
-      const bool early = ctl->stage == 0;
-      const bool c14a = early && rr <= ctl->sw2;
-      const bool periodic = early && since >= c.period;
-      const bool capped = it >= c.max_iters;
-      const bool bad = !(rr == rr) || (!c.cheb && !(rho_new == rho_new));
-      ctl->conv_rec = conv_rec ? 1 : 0;
-      if (bad) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
-      else if (conv_rec || c14a || periodic || capped) want = 1u;
-    }
-    ctl->want_true = (int)want;
+    unsigned go, want;
+    policy_after_update(ctl, c, acc[0], acc[1], go, want);
     if (!ctl->no_graph) { cudaGraphSetConditional(h_while, go); cudaGraphSetConditional(h_if, want); }
   }
 }
@@ -324,37 +284,7 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
     acc[1] = fma(di, di, acc[1]);
   });
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[3], smem, &s_flag) && threadIdx.x == 0) {
-    const double tt = acc[0], dd = acc[1];
-    const double rr = ctl->rr;
-    ctl->tt = tt; ctl->dd = dd;
-    ctl->evals += 1;
-    ctl->since_eval = 0;
-    ctl->xalpha = 0.0;          // k_flush_x has just applied it (fused path)
-    unsigned go = 1u;
-    int restart = 0;
-    if (tt <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }
-    else if (ctl->it >= c.max_iters) { ctl->status = CUTH_SOLVE_MAX_ITERS; go = 0u; }
-    else if (ctl->stage == 1) {
-      // late stage: the recursive residual said "converged", the true one disagrees -> replace r,
-      // restart the direction (same rule as the oracle), keep iterating.
-      if (ctl->conv_rec) restart = 1;
-    } else {
-      int reason = 0;
-      if (ctl->conv_rec) reason = 4;
-      else if (rr <= ctl->sw2) reason = 1;                                        // (14a)
-      else if (dd >= 0.25 * tt) reason = 3;                                       // (14c): ||t-r|| >= 0.5 ||t||
-      else if (tt > 0.81 * ctl->tt_prev && rr <= 0.81 * ctl->rr_prev_eval) reason = 2;   // (14b), R-G9
-      if (reason) {
-        ctl->stage = 1; ctl->promotions += 1; ctl->switch_reason = reason; ctl->switch_it = ctl->it;
-        // hot restart.  Small drift: r is recomputed, p keeps its history through its
-        // defining equation p = z + beta p ("preserving the established Krylov subspace");
-        // large drift ((14c)): the direction is rebuilt from scratch, p = z.
-        restart = (c.soft_restart && dd <= c.soft_drift2 * tt) ? 2 : 1;
-      }
-    }
-    ctl->tt_prev = tt;
-    ctl->rr_prev_eval = rr;
-    ctl->restart = restart;
+    const unsigned go = policy_after_true(ctl, c, acc[0], acc[1]);
     if (!ctl->no_graph) cudaGraphSetConditional(h_while, go);
   }
 }
@@ -382,14 +312,7 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
     }
   }
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[4], smem, &s_flag) && threadIdx.x == 0) {
-    // mode 1: beta = 0 => p = z.  mode 2: beta_k = rho(new r) / rho_k, with rho_k = rho_rec / beta_rec.
-    if (c.cheb) {      // the next k_cheb_last forms rho(new r) and beta = rho_new / rho_k itself
-      ctl->beta_zero = (mode == 1) ? 1 : 0;
-    } else {
-      ctl->beta = (mode == 2 && ctl->rho > 0.0) ? ctl->beta * (acc[0] / ctl->rho) : 0.0;
-      ctl->rho = acc[0];
-    }
-    ctl->rr = acc[1]; ctl->restart = 0; ctl->conv_rec = 0;
+    policy_after_restart(ctl, c, mode, acc[0], acc[1]);
   }
 }
 
@@ -420,17 +343,7 @@ __global__ void __launch_bounds__(kThreads) k_finalize(const Ctx* __restrict__ c
     }
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
-    cuth_result_t res;
-    res.status = ctl->status == CUTH_SOLVE_RUNNING ? CUTH_SOLVE_MAX_ITERS : ctl->status;
-    res.iterations = ctl->it;
-    res.promotions = ctl->promotions;
-    res.true_resid_evals = ctl->evals;
-    const double bb = ctl->bb;
-    res.rel_resid_true = bb > 0.0 ? sqrt(ctl->tt / bb) : 0.0;
-    res.rel_resid_rec = bb > 0.0 ? sqrt(ctl->rr / bb) : 0.0;
-    res.switch_reason = ctl->switch_reason;
-    res.switch_iteration = ctl->switch_it;
-    *c.result = res;
+    write_result(ctl, c);
   }
 }
 
