@@ -140,7 +140,7 @@ const char* cuth_last_cuda_error(void);
 int cuth_version(void);
 
 /* Kernel launches per PCG iteration of the graph body for this grid (2 on the fused path used for
- * large planes, 3 on the flat path); bench.py reports gpu_launches = prologue + this * iterations +
+ * large planes, 3 on the flat path, 0 when the whole solve is one persistent kernel); bench.py reports gpu_launches = prologue + this * iterations +
  * true-residual branches + epilogue. */
 int cuth_launches_per_iteration(const cuth_grid_t* grid);
 
@@ -165,6 +165,13 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * when one x-y plane of the six streamed arrays no longer fits L2, flat 1-D streaming otherwise),
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
+
+/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: for tiny grids (N <= 65536, flat
+ * traversal, Jacobi / no preconditioner) the whole solve is ONE persistent cooperative kernel whose
+ * iterations are separated by grid-wide barriers; everything else runs as the CUDA graph with conditional
+ * nodes.  1 = always the graph, 2 = the persistent kernel wherever it applies (any flat-traversal grid).
+ * Same arithmetic and policy code either way. */
+int cuth_set_loop_mode(int mode);
 
 /* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is
  * still in this workspace, outside the graph and with the graph's launch configuration, so that it

@@ -49,7 +49,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode"]
 
 _lib = None
 
@@ -93,6 +93,8 @@ def load_library():
     L.cuth_lanczos_bounds.argtypes = [vp, gp, vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_double), vp]
     L.cuth_cheb_apply.restype = C.c_int
     L.cuth_cheb_apply.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp]
+    L.cuth_set_loop_mode.restype = C.c_int
+    L.cuth_set_loop_mode.argtypes = [C.c_int]
     L.cuth_set_traversal.restype = C.c_int
     L.cuth_set_traversal.argtypes = [C.c_int]
     L.cuth_profile_kernel.restype = C.c_int
@@ -226,6 +228,10 @@ def cuth_lanczos_bounds(dia, grid: Grid, v0, steps, work, stream=None):
 def cuth_cheb_apply(dia, grid: Grid, opts, r, z, work, stream=None):
     _check(load_library().cuth_cheb_apply(_ptr(dia), grid.ref(), C.byref(opts), _ptr(r), _ptr(z), _ptr(work),
                                           work.numel() * work.element_size(), stream or _stream()), "cuth_cheb_apply")
+
+
+def cuth_set_loop_mode(mode: int):
+    _check(load_library().cuth_set_loop_mode(int(mode)), "cuth_set_loop_mode")
 
 
 def cuth_set_traversal(mode: int):

@@ -15,6 +15,7 @@
 
 #include "cuth_fused.cuh"
 #include "cuth_cheb.cuh"
+#include "cuth_persistent.cuh"
 
 namespace cuth {
 
@@ -40,6 +41,7 @@ static int check_grid(const cuth_grid_t* g, DiaLayout* L) {
   return CUTH_OK;
 }
 
+static std::atomic<int> g_loop_mode{0};   // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel (cuth_set_loop_mode)
 static std::atomic<int> g_traversal{0};   // 0 auto, 1 flat, 2 z-march (cuth_set_traversal)
 
 // Traversal choice: the flat kernel relies on L2 to keep the +-nx*ny neighbours (two planes of six
@@ -274,6 +276,33 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
   c->precision = opts->precision;
 }
 
+// Grid of the persistent kernel: every CTA must be co-resident (cooperative launch).
+static int persistent_blocks(int64_t n) {
+  static int cached = -1;
+  if (cached < 0) {
+    int dev = 0, sms = 0, coop = 0, occ = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pcg_persistent, kThreads, 0);
+    if (occ > 4) occ = 4;
+    cached = coop ? sms * occ : 0;
+    if (cached > kPersistMaxBlocks) cached = kPersistMaxBlocks;
+  }
+  int64_t need = (n + (int64_t)kThreads * kRows - 1) / ((int64_t)kThreads * kRows);
+  return (int)(need < cached ? need : cached);
+}
+
+static bool use_persistent(const DiaLayout& L, bool cheb) {
+  const int mode = g_loop_mode.load();
+  if (cheb || use_zmarch(L) || mode == 1) return false;
+  if (persistent_blocks(L.n) <= 0) return false;
+  // Measured on B200: a phase of the persistent kernel costs ~4.5 us (L2 round trips +
+  // grid.sync), a graph kernel node ~5 us: 14.1 vs 16.5 us per iteration at cfg 1 (8 k rows), 36.4 vs 34.6 us
+  // at cfg 2 (1 M rows), where the wider grid of the separate kernels wins.  Auto: persistent for tiny grids.
+  return mode == 2 || L.n <= (1 << 16);
+}
+
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
                         const double* power_D, double* x_D, void* work_D, size_t work_bytes,
                         cuth_result_t* result_D, void* stream) {
@@ -315,6 +344,12 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
+  if (use_persistent(L, cheb)) {
+    Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
+    void* args[] = {&ctxp, &ctlp, &part};
+    CU(cudaLaunchCooperativeKernel((void*)k_pcg_persistent, dim3(persistent_blocks(L.n)), dim3(kThreads), args, 0, st));
+    return CUTH_OK;
+  }
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
                  cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0, &ex);
@@ -543,6 +578,12 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   return CUTH_OK;
 }
 
+int cuth_set_loop_mode(int mode) {
+  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
+  g_loop_mode.store(mode);
+  return CUTH_OK;
+}
+
 int cuth_set_traversal(int mode) {
   if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
   g_traversal.store(mode);
@@ -567,6 +608,7 @@ int cuth_version(void) { return 10000; }
 int cuth_launches_per_iteration(const cuth_grid_t* grid) {
   DiaLayout L;
   if (!make_layout(grid, &L)) return 0;
+  if (use_persistent(L, false)) return 0;      // one persistent kernel for the whole solve
   return use_zmarch(L) ? 2 : 3;
 }
 
