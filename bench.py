@@ -187,6 +187,8 @@ def main():
                     help="jacobi = the north_star hot path; chebyshev = the paper's own preconditioner (Alg. 3)")
     ap.add_argument("--cheb-degree", type=int, default=30)
     ap.add_argument("--lanczos-steps", type=int, default=40)
+    ap.add_argument("--cheb-storage", default="fp32", choices=["fp32", "fp16"],
+                    help="MIXED Chebyshev: matrix copy the preconditioner reads (A2 fp32 / A3 fp16, Alg. 4)")
     ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
@@ -241,7 +243,8 @@ def main():
     if cheb:       # setup: Lanczos on the device + tridiagonal eigenvalues on the host, once per matrix
         torch.cuda.synchronize()
         t0 = time.time()
-        bounds = S.setup_chebyshev(b[0], lanczos_steps=args.lanczos_steps, degree=args.cheb_degree)
+        bounds = S.setup_chebyshev(b[0], lanczos_steps=args.lanczos_steps, degree=args.cheb_degree,
+                                   storage=cu.CHEB_A3_FP16 if args.cheb_storage == "fp16" else cu.CHEB_DEFAULT)
         setup_ms = (time.time() - t0) * 1e3
     counters = torch.zeros(4, dtype=torch.int32, device="cuda")     # status, iterations, promotions, evals
     early_acc = torch.zeros(1, dtype=torch.int32, device="cuda")   # iterations done on the fp32-stored operator
@@ -314,8 +317,10 @@ def main():
              {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"})
     body_ids = (4, 5) if fused else (0, 1, 2)
     if cheb:
-        names[7 if mixed else 6] = "k_cheb_mid"
-        body_ids = tuple([7 if mixed else 6] * (args.cheb_degree - 1)) + body_ids
+        h16 = mixed and args.cheb_storage == "fp16"
+        cid = 8 if h16 else (7 if mixed else 6)
+        names[cid] = "k_cheb_mid"
+        body_ids = tuple([cid] * (args.cheb_degree - 1)) + body_ids
     for kid, nm in names.items():
         for _ in range(3):
             cu.cuth_profile_kernel(S.work, g, kid)
@@ -361,7 +366,7 @@ def main():
         # outer: K1 (matrix + z, p, x read + p', mu, x written) + K2 (r, mu read, r written); preconditioner:
         # FIRST M+8+3s, (k-3) x MID M+6s, LAST M+3s+16 with s = sizeof(T), M = matrix bytes per row
         k, sT = args.cheb_degree, (4 if mixed else 8)
-        Mc = 4 * (m - 1) if mixed else 8 * m
+        Mc = (2 * (m - 1) if h16 else 4 * (m - 1)) if mixed else 8 * m
         apply_bytes = (k - 1) * Mc + (3 * sT + 8) + (k - 3) * 6 * sT + (3 * sT + 16)
         outer = lambda M_: M_ + 48 + 24
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
@@ -376,7 +381,7 @@ def main():
         dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
     if cheb:
         dom_name, dom_ms = "k_cheb_mid", kern["k_cheb_mid"]
-        dom_bytes = ((4 * (m - 1) + 24) if mixed else (8 * m + 48)) * w.n
+        dom_bytes = (((2 if h16 else 4) * (m - 1) + 24) if mixed else (8 * m + 48)) * w.n
         stage_fp64 = not mixed
     per_it = (2 if fused else 3) + (args.cheb_degree - 1 if cheb else 0)
     per_eval = 3 if fused else 2
@@ -389,7 +394,7 @@ def main():
         "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz],
                    "precision": "mixed" if mixed else "fp64", "rtol": w.rtol, "preconditioner": args.preconditioner,
                    **({"cheb_degree": args.cheb_degree, "lanczos_steps": args.lanczos_steps,
-                       "cheb_interval": [S.opts.cheb_lmin, S.opts.cheb_lmax]} if cheb else {}),
+                       "cheb_interval": [S.opts.cheb_lmin, S.opts.cheb_lmax], "cheb_storage": args.cheb_storage} if cheb else {}),
                    "l2_policy": ("inputs larger than L2 (matrix + vectors = %.2f GB streamed per iteration)" if
                                  (8 * m_ratio(w) + 48) * w.n > 126e6 else
                                  "working set %.3f GB fits the 126 MB L2: L2-resident, latency-bound case, "

@@ -42,6 +42,7 @@ enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN 
 
 enum { CUTH_FP64 = 0, CUTH_MIXED = 1 };            /* cuth_opts_t.precision / cuth_spmv precision */
 enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1, CUTH_PRECOND_CHEBYSHEV = 2 };
+enum { CUTH_CHEB_DEFAULT = 0, CUTH_CHEB_A3_FP16 = 1 };   /* cuth_opts_t.cheb_storage */
 
 /* The thermal problem of PAPER.md §III-B: eq. (4) (steady) and eq. (5) (backward
  * Euler) on a box of cells with adiabatic sides/bottom (eq. (3)) and a Robin top
@@ -68,6 +69,9 @@ typedef struct {
   int32_t cheb_degree;        /* k of Alg. 3 (the paper uses 30); 3 <= k <= 64 */
   double cheb_lmin, cheb_lmax;/* spectral interval [alpha, beta] of eq. (10)-(11), e.g. from
                                  cuth_lanczos_bounds; 0 < lmin < lmax, and lmax must bound the spectrum of A */
+  int32_t cheb_storage;       /* matrix the preconditioner multiplies by in MIXED mode: CUTH_CHEB_DEFAULT = the fp32
+                                 copy A2, CUTH_CHEB_A3_FP16 = the half-precision copy A3 promoted to fp32 on load
+                                 (Alg. 4 "arithmetic decoupling").  Ignored in FP64 mode. */
 } cuth_opts_t;
 
 typedef struct {
@@ -178,7 +182,8 @@ int cuth_set_loop_mode(int mode);
  * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the
  * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual,
  * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path),
- * 6 / 7 = one middle step of the Chebyshev apply in fp64 / fp32 (only after a CUTH_PRECOND_CHEBYSHEV solve).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
+ * 6 / 7 / 8 = one middle step of the Chebyshev apply in fp64 / fp32 on A2 / fp32 on the fp16 copy A3 (only
+ * after a CUTH_PRECOND_CHEBYSHEV solve).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
 int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
 
 #ifdef __cplusplus

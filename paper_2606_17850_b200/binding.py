@@ -13,6 +13,7 @@ LIB_PATH = os.environ.get("CUTH_LIB", os.path.join(HERE, "libcuth.so"))   # CUTH
 
 FP64, MIXED = 0, 1
 PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV = 0, 1, 2
+CHEB_DEFAULT, CHEB_A3_FP16 = 0, 1
 STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}
 _ERR = {-1: "CUTH_ERR_NULL", -2: "CUTH_ERR_DIMS", -3: "CUTH_ERR_VALUE", -4: "CUTH_ERR_SIZE",
         -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT"}
@@ -37,7 +38,8 @@ class cuth_grid_t(C.Structure):
 class cuth_opts_t(C.Structure):
     _fields_ = [("precision", C.c_int32), ("rtol", C.c_double), ("max_iters", C.c_int32),
                 ("true_resid_period", C.c_int32), ("preconditioner", C.c_int32),
-                ("cheb_degree", C.c_int32), ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double)]
+                ("cheb_degree", C.c_int32), ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double),
+                ("cheb_storage", C.c_int32)]
 
 
 class cuth_result_t(C.Structure):
@@ -136,9 +138,9 @@ class Grid:
 
 
 def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI,
-         cheb_degree=30, cheb_lmin=0.0, cheb_lmax=0.0):
+         cheb_degree=30, cheb_lmin=0.0, cheb_lmax=0.0, cheb_storage=CHEB_DEFAULT):
     return cuth_opts_t(int(precision), float(rtol), int(max_iters), int(true_resid_period), int(preconditioner),
-                       int(cheb_degree), float(cheb_lmin), float(cheb_lmax))
+                       int(cheb_degree), float(cheb_lmin), float(cheb_lmax), int(cheb_storage))
 
 
 @dataclass
@@ -289,14 +291,14 @@ class Solver:
         self.work = torch.empty(cuth_workspace_bytes(A.grid, self.opts), dtype=torch.uint8, device="cuda")
         self.result_dev = torch.zeros(C.sizeof(cuth_result_t), dtype=torch.uint8, device="cuda")
 
-    def setup_chebyshev(self, v0, lanczos_steps=40, degree=30, lmin=None, lmax=None):
+    def setup_chebyshev(self, v0, lanczos_steps=40, degree=30, lmin=None, lmax=None, storage=CHEB_DEFAULT):
         """Spectral range by Lanczos (cuth_lanczos_bounds) and switch this solver to the Chebyshev
         preconditioner; only copies the interval the library returns into the options struct."""
         import torch
         lo, hi, gersh, rec_lo, rec_hi = cuth_lanczos_bounds(self.A.buf, self.A.grid, v0, lanczos_steps, self.work)
         o = self.opts
         self.opts = Opts(o.precision, o.rtol, o.max_iters, o.true_resid_period, PRECOND_CHEBYSHEV, degree,
-                         rec_lo if lmin is None else lmin, rec_hi if lmax is None else lmax)
+                         rec_lo if lmin is None else lmin, rec_hi if lmax is None else lmax, storage)
         need = cuth_workspace_bytes(self.A.grid, self.opts)
         if need > self.work.numel():
             cuth_release_workspace(self.work)

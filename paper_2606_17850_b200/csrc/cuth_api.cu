@@ -90,6 +90,10 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   A.d0 = v + L.ptr[0]; A.d1 = v + L.ptr[1]; A.d2 = v + L.ptr[2]; A.d3 = v + L.ptr[3];
   A.f1 = f + L.ptr[1]; A.f2 = f + L.ptr[2]; A.f3 = f + L.ptr[3];
   A.dinv = (const double*)(base + L.o_dinv);
+  A.h1 = (const __half*)(base + L.o_h16);
+  A.h2 = (const __half*)(base + L.o_h16 + L.h16_stride);
+  A.h3 = (const __half*)(base + L.o_h16 + 2 * L.h16_stride);
+  A.h_scale = lay + 4 * L.nz;
   A.s_layer = lay + L.nz;
   A.cap_layer = lay + 2 * L.nz;
   A.n = L.n; A.nx = L.nx; A.nxny = L.nxny;
@@ -104,6 +108,25 @@ static int grid_blocks(int64_t n) {
   if (b > cap) b = cap;
   if (b < 1) b = 1;
   return (int)b;
+}
+
+// Chebyshev kernels by arithmetic / matrix storage: 0 = fp64 on A1, 1 = fp32 on A2, 2 = fp32 on the fp16 copy A3.
+static int cheb_code(const cuth_opts_t* o) {
+  if (o->precision != CUTH_MIXED) return 0;
+  return o->cheb_storage == CUTH_CHEB_A3_FP16 ? 2 : 1;
+}
+static void* cheb_first_fn(int code) {
+  return code == 0 ? (void*)k_cheb_first<double, MatF32> : code == 1 ? (void*)k_cheb_first<float, MatF32>
+                                                                     : (void*)k_cheb_first<float, MatF16>;
+}
+static void* cheb_mid_fn(int code, bool x2) {
+  if (code == 0) return (void*)k_cheb_mid<double, MatF32>;
+  if (x2) return code == 1 ? (void*)k_cheb_mid_f32x2<MatF32> : (void*)k_cheb_mid_f32x2<MatF16>;
+  return code == 1 ? (void*)k_cheb_mid<float, MatF32> : (void*)k_cheb_mid<float, MatF16>;
+}
+static void* cheb_last_fn(int code) {
+  return code == 0 ? (void*)k_cheb_last<double, MatF32> : code == 1 ? (void*)k_cheb_last<float, MatF32>
+                                                                    : (void*)k_cheb_last<float, MatF16>;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -160,24 +183,25 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   // Chebyshev: the body starts with the preconditioner z = q(A) r: k-1 stencil kernels, no reduction
   // until the last one, which also forms rho = r.z and beta (Alg. 1 lines 10-11).
   cudaGraphNode_t n_c = nullptr;
-  const int kdeg = chebkey >> 1;
+  const int kdeg = chebkey >> 2;
   if (kdeg > 0) {
-    const bool f32 = (chebkey & 1) != 0;
+    const int code = chebkey & 3;
+    const bool f32 = code != 0;
     { void* a[] = {&ctx};
-      CU(add_kernel(body, &n_c, nullptr, 0, f32 ? (void*)k_cheb_first<float> : (void*)k_cheb_first<double>, cblocks, a)); }
+      CU(add_kernel(body, &n_c, nullptr, 0, cheb_first_fn(code), cblocks, a)); }
     for (int i = 1; i <= kdeg - 3; ++i) {
       cudaGraphNode_t prev = n_c;
       int step = i;
       void* a[] = {&ctx, &step};
       if (f32 && x2blocks > 0)
-        CU(add_kernel(body, &n_c, &prev, 1, (void*)k_cheb_mid_f32x2, x2blocks, a));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, true), x2blocks, a));
       else
-        CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_mid<float> : (void*)k_cheb_mid<double>, cblocks, a));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, false), cblocks, a));
     }
     { cudaGraphNode_t prev = n_c;
       int step = kdeg - 2;
       void* a[] = {&ctx, &ctl, &partials, &step};
-      CU(add_kernel(body, &n_c, &prev, 1, f32 ? (void*)k_cheb_last<float> : (void*)k_cheb_last<double>, cblocks, a)); }
+      CU(add_kernel(body, &n_c, &prev, 1, cheb_last_fn(code), cblocks, a)); }
   }
   const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
   const size_t ndep0 = n_c ? 1 : 0;
@@ -251,7 +275,8 @@ static int check_opts(const cuth_opts_t* o) {
       o->preconditioner != CUTH_PRECOND_CHEBYSHEV)
     return CUTH_ERR_VALUE;
   if (o->preconditioner == CUTH_PRECOND_CHEBYSHEV &&
-      (o->cheb_degree < 3 || o->cheb_degree > kMaxChebDegree || !(o->cheb_lmin > 0.0) || !(o->cheb_lmax > o->cheb_lmin)))
+      (o->cheb_degree < 3 || o->cheb_degree > kMaxChebDegree || !(o->cheb_lmin > 0.0) || !(o->cheb_lmax > o->cheb_lmin) ||
+       (o->cheb_storage != CUTH_CHEB_DEFAULT && o->cheb_storage != CUTH_CHEB_A3_FP16)))
     return CUTH_ERR_VALUE;
   return CUTH_OK;
 }
@@ -352,7 +377,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   }
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
-                 cheb ? opts->cheb_degree * 2 + (opts->precision == CUTH_MIXED ? 1 : 0) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0, &ex);
+                 cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -487,11 +512,13 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 4: k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
-    case 6: k_cheb_mid<double><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1); break;     // needs a Chebyshev solve's context
-    case 7:
-      if (cheb_x2(L)) k_cheb_mid_f32x2<<<cheb_x2_blocks(L), kThreads, 0, st>>>(w.ctx, 1);
-      else k_cheb_mid<float><<<cheb_blocks(L), kThreads, 0, st>>>(w.ctx, 1);
-      break;
+    case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
+      const int code = kernel_id - 6;
+      const bool x2 = code != 0 && cheb_x2(L);
+      Ctx* ctxp = w.ctx; int step = 1;
+      void* args[] = {&ctxp, &step};
+      CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : cheb_blocks(L)), dim3(kThreads), args, 0, st));
+    } break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
   }
@@ -562,18 +589,20 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   const int blocks = grid_blocks(L.n);
   const int sb = cheb_blocks(L);
   const int k = opts->cheb_degree;
-  if (opts->precision == CUTH_MIXED) {
-    k_cheb_first<float><<<sb, kThreads, 0, st>>>(w.ctx);
-    for (int i = 1; i <= k - 3; ++i) {
-      if (cheb_x2(L)) k_cheb_mid_f32x2<<<cheb_x2_blocks(L), kThreads, 0, st>>>(w.ctx, i);
-      else k_cheb_mid<float><<<sb, kThreads, 0, st>>>(w.ctx, i);
-    }
-    k_cheb_last<float><<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, k - 2);
-  } else {
-    k_cheb_first<double><<<sb, kThreads, 0, st>>>(w.ctx);
-    for (int i = 1; i <= k - 3; ++i) k_cheb_mid<double><<<sb, kThreads, 0, st>>>(w.ctx, i);
-    k_cheb_last<double><<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, k - 2);
+  const int code = cheb_code(opts);
+  const bool x2 = code != 0 && cheb_x2(L);
+  Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
+  { void* a[] = {&ctxp};
+    CU(cudaLaunchKernel(cheb_first_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
+  for (int i = 1; i <= k - 3; ++i) {
+    int step = i;
+    void* a[] = {&ctxp, &step};
+    CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : sb), dim3(kThreads), a, 0, st));
   }
+  { int step = k - 2;
+    void* a[] = {&ctxp, &ctlp, &part, &step};
+    CU(cudaLaunchKernel(cheb_last_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
+  (void)blocks;
   CU(cudaGetLastError());
   return CUTH_OK;
 }

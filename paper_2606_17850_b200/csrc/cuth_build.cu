@@ -58,13 +58,44 @@ __global__ void __launch_bounds__(256) build_dia_kernel(BuildArgs a) {
   }
 }
 
+// A3: half-precision copy of the off-diagonals.  The entries of these matrices are
+// 1e-8..1 W/K, far below fp16's normal range, so they are stored times a power of two S chosen from the
+// largest |entry| (S * max in (2^13, 2^14]); the kernels multiply the accumulated sum by 1/S once.
+__global__ void __launch_bounds__(256) k_offdiag_absmax(const double* __restrict__ v, int64_t count, double* slot) {
+  double m = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) m = fmax(m, fabs(v[i]));
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) atomicMax((unsigned long long*)slot, (unsigned long long)__double_as_longlong(m));
+}
+
+__global__ void k_h16_scale(double* slot) {
+  const double m = __longlong_as_double((long long)((unsigned long long*)slot)[0]);
+  int e = 0;
+  if (m > 0.0) { frexp(m, &e); }                 // m = f * 2^e, f in [0.5, 1)
+  const double scale = ldexp(1.0, 14 - e);       // S * m in [2^13, 2^14)
+  slot[1] = scale;
+  slot[2] = 1.0 / scale;
+}
+
+__global__ void __launch_bounds__(256) k_make_h16(BuildArgs a, const double* slot, __half* h1, __half* h2, __half* h3) {
+  const double scale = slot[1];
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+    h1[i] = __double2half(i + 1 < a.n ? a.d1[i] * scale : 0.0);
+    h2[i] = __double2half(i + a.nx < a.n ? a.d2[i] * scale : 0.0);
+    h3[i] = __double2half(i + a.nxny < a.n ? a.d3[i] * scale : 0.0);
+  }
+}
+
 // Host side: fills the per-layer arrays, launches the kernel.  Called from cuth_api.cu.
 int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStream_t st, cudaError_t* err) {
   char* base = (char*)dia_D;
   const int nz = (int)g->nz;
   const bool transient = g->cvol_H != nullptr && g->dt > 0.0;
   // per-layer arrays inside the matrix object: dz | s | cap | cvol
-  double* h = new double[4 * nz];
+  double* h = new double[4 * nz + 4];
+  for (int k = 0; k < 4; ++k) h[4 * nz + k] = 0.0;
   for (int z = 0; z < nz; ++z) {
     const double axy = g->dx * g->dy;
     const double cap = transient ? g->cvol_H[z] * (axy * g->dz_H[z]) / g->dt : 0.0;
@@ -81,7 +112,7 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   for (int k = 0; k < 4; ++k) hdr[11 + k] = (unsigned long long)L.off[k];
   cudaError_t e = cudaMemcpyAsync(base, hdr, kHeaderBytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess)
-    e = cudaMemcpyAsync(base + L.o_layers, h, 4 * sizeof(double) * nz, cudaMemcpyHostToDevice, st);
+    e = cudaMemcpyAsync(base + L.o_layers, h, (4 * nz + 4) * sizeof(double), cudaMemcpyHostToDevice, st);
   delete[] h;   // pageable H2D copies are staged before cudaMemcpyAsync returns
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   BuildArgs a;
@@ -100,6 +131,12 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   int64_t blocks = (L.n + 255) / 256;
   if (blocks > 148 * 64) blocks = 148 * 64;
   build_dia_kernel<<<(unsigned)blocks, 256, 0, st>>>(a);
+  double* slot = (double*)(base + L.o_layers) + 4 * nz;
+  k_offdiag_absmax<<<(unsigned)blocks, 256, 0, st>>>(a.d1, L.e - L.n, slot);     // D1|D2|D3 are contiguous
+  k_h16_scale<<<1, 1, 0, st>>>(slot);
+  k_make_h16<<<(unsigned)blocks, 256, 0, st>>>(a, slot, (__half*)(base + L.o_h16),
+                                               (__half*)(base + L.o_h16 + L.h16_stride),
+                                               (__half*)(base + L.o_h16 + 2 * L.h16_stride));
   e = cudaGetLastError();
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   return CUTH_OK;

@@ -19,10 +19,38 @@ namespace cuth {
 #endif
 #define CUTH_CHEB_NC 1   // columns per thread of the z-marching stencil (2 and 4 measured slower, _work sweep)
 
+// Where the fp32-arithmetic operator takes its off-diagonal entries from: A2 (fp32) or A3 (fp16
+// times a power-of-two scale, promoted to fp32 on load: "arithmetic decoupling", Alg. 4).
+struct MatF32 {
+  // the packed A2 diagonals D2, D3 start at odd elements (R-G5b): pairs are two scalar loads
+  static __device__ __forceinline__ float2 p1(const DiaDev& A, int64_t i, float) { return make_float2(A.f1[i], A.f1[i + 1]); }
+  static __device__ __forceinline__ float2 p2(const DiaDev& A, int64_t i, float) { return make_float2(A.f2[i], A.f2[i + 1]); }
+  static __device__ __forceinline__ float2 p3(const DiaDev& A, int64_t i, float) { return make_float2(A.f3[i], A.f3[i + 1]); }
+  static __device__ __forceinline__ float inv(const DiaDev&) { return 1.f; }
+  static __device__ __forceinline__ float e1(const DiaDev& A, int64_t i, float) { return A.f1[i]; }
+  static __device__ __forceinline__ float e2(const DiaDev& A, int64_t i, float) { return A.f2[i]; }
+  static __device__ __forceinline__ float e3(const DiaDev& A, int64_t i, float) { return A.f3[i]; }
+};
+struct MatF16 {
+  // the three fp16 arrays are this library's own 256-B aligned copies, so an even index is a 4-byte
+  // aligned pair: one half2 load per pair of x-neighbours
+  static __device__ __forceinline__ float2 pair(const __half* p, int64_t i, float s) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(p + i));
+    return make_float2(f.x * s, f.y * s);
+  }
+  static __device__ __forceinline__ float2 p1(const DiaDev& A, int64_t i, float s) { return pair(A.h1, i, s); }
+  static __device__ __forceinline__ float2 p2(const DiaDev& A, int64_t i, float s) { return pair(A.h2, i, s); }
+  static __device__ __forceinline__ float2 p3(const DiaDev& A, int64_t i, float s) { return pair(A.h3, i, s); }
+  static __device__ __forceinline__ float inv(const DiaDev& A) { return (float)A.h_scale[2]; }
+  static __device__ __forceinline__ float e1(const DiaDev& A, int64_t i, float s) { return __half2float(A.h1[i]) * s; }
+  static __device__ __forceinline__ float e2(const DiaDev& A, int64_t i, float s) { return __half2float(A.h2[i]) * s; }
+  static __device__ __forceinline__ float e3(const DiaDev& A, int64_t i, float s) { return __half2float(A.h3[i]) * s; }
+};
+
 // One row of A v with v stored as VT and arithmetic in T (T = double: A1 standard form; T = float: A2
 // difference form, DESIGN.md R-F3), flat traversal.
-template <class VT, class T>
-__device__ __forceinline__ T row_t(const DiaDev& A, const VT* __restrict__ v, int64_t i, T vi) {
+template <class VT, class T, class M>
+__device__ __forceinline__ T row_t(const DiaDev& A, const VT* __restrict__ v, int64_t i, T vi, float ms) {
   const int64_t n = A.n, nx = A.nx, np = A.nxny;
   const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx, up3 = i + np < n, lo3 = i >= np;
   if (sizeof(T) == 8) {
@@ -37,20 +65,21 @@ __device__ __forceinline__ T row_t(const DiaDev& A, const VT* __restrict__ v, in
   } else {
     const unsigned z = (unsigned)i / (unsigned)np;
     T acc = (T)A.s_layer[z] * vi;
-    acc += (T)(up1 ? A.f1[i] : 0.f) * ((T)(up1 ? v[i + 1] : (VT)vi) - vi);
-    acc += (T)(lo1 ? A.f1[i - 1] : 0.f) * ((T)(lo1 ? v[i - 1] : (VT)vi) - vi);
-    acc += (T)(up2 ? A.f2[i] : 0.f) * ((T)(up2 ? v[i + nx] : (VT)vi) - vi);
-    acc += (T)(lo2 ? A.f2[i - nx] : 0.f) * ((T)(lo2 ? v[i - nx] : (VT)vi) - vi);
-    acc += (T)(up3 ? A.f3[i] : 0.f) * ((T)(up3 ? v[i + np] : (VT)vi) - vi);
-    acc += (T)(lo3 ? A.f3[i - np] : 0.f) * ((T)(lo3 ? v[i - np] : (VT)vi) - vi);
+    acc += (T)(up1 ? M::e1(A, i, ms) : 0.f) * ((T)(up1 ? v[i + 1] : (VT)vi) - vi);
+    acc += (T)(lo1 ? M::e1(A, i - 1, ms) : 0.f) * ((T)(lo1 ? v[i - 1] : (VT)vi) - vi);
+    acc += (T)(up2 ? M::e2(A, i, ms) : 0.f) * ((T)(up2 ? v[i + nx] : (VT)vi) - vi);
+    acc += (T)(lo2 ? M::e2(A, i - nx, ms) : 0.f) * ((T)(lo2 ? v[i - nx] : (VT)vi) - vi);
+    acc += (T)(up3 ? M::e3(A, i, ms) : 0.f) * ((T)(up3 ? v[i + np] : (VT)vi) - vi);
+    acc += (T)(lo3 ? M::e3(A, i - np, ms) : 0.f) * ((T)(lo3 ? v[i - np] : (VT)vi) - vi);
     return acc;
   }
 }
 
 // f(i, v_i, (A v)_i) for every row; traversal as in apply_A (flat, or z-marching with the plane
 // neighbours in registers).
-template <class VT, class T, class F>
+template <class VT, class T, class M, class F>
 __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict__ v, F&& f) {
+  const float ms = M::inv(A);
   if (!A.zmarch) {
     CUTH_TILE_LOOP(A.n) {
 #pragma unroll
@@ -58,7 +87,7 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
         const int64_t i = base + threadIdx.x + k * kThreads;
         if (i < A.n) {
           const T vi = (T)v[i];
-          f(i, vi, row_t<VT, T>(A, v, i, vi));
+          f(i, vi, row_t<VT, T, M>(A, v, i, vi, ms));
         }
       }
     }
@@ -93,9 +122,9 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
         acc += a1u * v1u; acc += a1l * v1l; acc += a2u * v2u; acc += a2l * v2l;
         acc += a3u * v_hi; acc += a3l * v_lo;
       } else {
-        const T a1u = (T)(up1 ? A.f1[i] : 0.f), a1l = (T)(lo1 ? A.f1[i - 1] : 0.f);
-        const T a2u = (T)(up2 ? A.f2[i] : 0.f), a2l = (T)(lo2 ? A.f2[i - nx] : 0.f);
-        a3u = (T)(up3 ? A.f3[i] : 0.f);
+        const T a1u = (T)(up1 ? M::e1(A, i, ms) : 0.f), a1l = (T)(lo1 ? M::e1(A, i - 1, ms) : 0.f);
+        const T a2u = (T)(up2 ? M::e2(A, i, ms) : 0.f), a2l = (T)(lo2 ? M::e2(A, i - nx, ms) : 0.f);
+        a3u = (T)(up3 ? M::e3(A, i, ms) : 0.f);
         v_hi = up3 ? (T)v[i + np] : v_c;
         const T v1u = up1 ? (T)v[i + 1] : v_c, v1l = lo1 ? (T)v[i - 1] : v_c;
         const T v2u = up2 ? (T)v[i + nx] : v_c, v2l = lo2 ? (T)v[i - nx] : v_c;
@@ -112,14 +141,14 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
 
 // ---------------------------------------------------------------------------------------------
 // Alg. 3 lines 1-4 and the first pass of lines 6-10.
-template <class T>
+template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_first(const Ctx* __restrict__ ctxp) {
   const Ctx c = *ctxp;
   const T inv_theta = (T)c.cheb_inv_theta, c1 = (T)ctxp->cheb_c1[0], c2 = (T)ctxp->cheb_c2[0];
   T* __restrict__ rc = (T*)c.crc;
   T* __restrict__ zc = (T*)c.czc;
   T* __restrict__ d1 = (T*)c.cd[1];
-  apply_A_t<double, T>(c.A, c.r, [&](int64_t i, T ri, T Ar) {
+  apply_A_t<double, T, M>(c.A, c.r, [&](int64_t i, T ri, T Ar) {
     const T d0 = ri * inv_theta;                 // line 4
     const T rci = ri - Ar * inv_theta;           // lines 7-8
     rc[i] = rci;
@@ -129,7 +158,7 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
 }
 
 // Alg. 3 lines 6-10 for 0 < i < k-2.
-template <class T>
+template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
@@ -137,7 +166,7 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
   T* __restrict__ dout = (T*)ctxp->cd[(step + 1) & 1];
   T* __restrict__ rc = (T*)c.crc;
   T* __restrict__ zc = (T*)c.czc;
-  apply_A_t<T, T>(c.A, din, [&](int64_t i, T di, T Ad) {
+  apply_A_t<T, T, M>(c.A, din, [&](int64_t i, T di, T Ad) {
     const T rci = rc[i] - Ad;
     rc[i] = rci;
     zc[i] += di;
@@ -150,6 +179,7 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
 // neighbours of the pair are each other (registers), and a thread keeps twice the bytes in flight -- the
 // 4-byte version is latency-bound (profiles/r1c_cfg3_cheb_mixed.md).  Matrix entries stay scalar loads: the
 // packed diagonals D2, D3 start at odd elements (R-G5b).  Tile = (2 ZTX) x ZTY columns per CTA.
+template <class M>
 __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __restrict__ ctxp, int step) {
   const Ctx c = *ctxp;
   const DiaDev& A = c.A;
@@ -164,6 +194,7 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
   const int ntiles = tiles_x * tiles_y;
   const int64_t n = A.n, nx = A.nx, np = A.nxny;
   auto ld2 = [](const float* p) { return *reinterpret_cast<const float2*>(p); };
+  const float ms = M::inv(A);
   for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
     const int bx = t % tiles_x, by = t / tiles_x;
     const int x = bx * 2 * ZTX + 2 * tx, y = by * ZTY + ty;
@@ -174,11 +205,14 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
     for (int z = 0; z < nz; ++z) {
       const int64_t i = c0 + (int64_t)z * np;
       const bool up3 = z + 1 < nz, up2 = i + nx < n, lo2 = i >= nx, lo1 = i >= 1, up1 = i + 2 < n;
-      const float f1l = lo1 ? A.f1[i - 1] : 0.f, f1a = A.f1[i], f1b = up1 ? A.f1[i + 1] : 0.f;
-      const float f2u0 = up2 ? A.f2[i] : 0.f, f2u1 = up2 ? A.f2[i + 1] : 0.f;
-      const float f2l0 = lo2 ? A.f2[i - nx] : 0.f, f2l1 = lo2 ? A.f2[i + 1 - nx] : 0.f;
-      float2 a3u = make_float2(0.f, 0.f);
-      if (up3) { a3u.x = A.f3[i]; a3u.y = A.f3[i + 1]; }
+      // entries of the pair (i, i+1); the element i+1 of D1 couples to i+2, which may not exist
+      const float f1l = lo1 ? M::e1(A, i - 1, ms) : 0.f;
+      float2 f1p = up1 ? M::p1(A, i, ms) : make_float2(M::e1(A, i, ms), 0.f);
+      const float f1a = f1p.x, f1b = f1p.y;
+      const float2 z2 = make_float2(0.f, 0.f);
+      const float2 f2u = up2 ? M::p2(A, i, ms) : z2, f2l = lo2 ? M::p2(A, i - nx, ms) : z2;
+      const float f2u0 = f2u.x, f2u1 = f2u.y, f2l0 = f2l.x, f2l1 = f2l.y;
+      const float2 a3u = up3 ? M::p3(A, i, ms) : z2;
       const float2 v_hi = up3 ? ld2(din + i + np) : v_c;
       const float2 v2u = up2 ? ld2(din + i + nx) : v_c, v2l = lo2 ? ld2(din + i - nx) : v_c;
       const float vl = lo1 ? din[i - 1] : v_c.x, vr = up1 ? din[i + 2] : v_c.y;
@@ -201,7 +235,7 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
 }
 
 // Last stencil pass (i = k-2) + the two trailing z updates + rho = r.z (Alg. 1 lines 10-11).
-template <class T>
+template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                         int step) {
   __shared__ double smem[32];
@@ -212,7 +246,7 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(
   const T* __restrict__ rc = (const T*)c.crc;
   const T* __restrict__ zc = (const T*)c.czc;
   double acc[1] = {0.0};
-  apply_A_t<T, T>(c.A, din, [&](int64_t i, T di, T Ad) {
+  apply_A_t<T, T, M>(c.A, din, [&](int64_t i, T di, T Ad) {
     const T rci = rc[i] - Ad;
     const T dl = c1 * di + c2 * rci;             // d_{k-1}
     const double zi = (double)(zc[i] + di + dl);

@@ -2,6 +2,7 @@
 // Product code (CUDA, sm_100a).  Shares nothing with oracle/.
 #pragma once
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -24,6 +25,8 @@ struct DiaLayout {
   size_t o_vals;     // fp64 [e]  packed D0|D1|D2|D3   (A1)
   size_t o_vals32;   // fp32 [e]  same packing          (A2)
   size_t o_dinv;     // fp64 [n]  1/D0
+  size_t o_h16;      // fp16 3 x [n] (each 256-B aligned): off-diagonals D1, D2, D3 times a power-of-two scale (A3)
+  size_t h16_stride; // bytes between the three fp16 arrays
   size_t bytes;
 };
 
@@ -40,10 +43,12 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
   for (int k = 0; k < 4; ++k) L->ptr[k + 1] = L->ptr[k] + (L->n - L->off[k]);
   L->e = L->ptr[4];
   size_t o = kHeaderBytes;
-  L->o_layers = o; o = align_up(o + 4 * sizeof(double) * (size_t)g->nz);
+  L->o_layers = o; o = align_up(o + (4 * (size_t)g->nz + 4) * sizeof(double));   // + absmax bits, scale, 1/scale, spare
   L->o_vals = o;   o = align_up(o + sizeof(double) * (size_t)L->e);
   L->o_vals32 = o; o = align_up(o + sizeof(float) * (size_t)L->e);
   L->o_dinv = o;   o = align_up(o + sizeof(double) * (size_t)L->n);
+  L->h16_stride = align_up(sizeof(__half) * (size_t)L->n);
+  L->o_h16 = o;    o = o + 3 * L->h16_stride;
   L->bytes = o;
   return true;
 }
@@ -52,6 +57,8 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
 struct DiaDev {
   const double* d0; const double* d1; const double* d2; const double* d3;   // fp64 diagonals (A1)
   const float* f1; const float* f2; const float* f3;                        // fp32 off-diagonals (A2)
+  const __half* h1; const __half* h2; const __half* h3;                     // fp16 off-diagonals x scale (A3)
+  const double* h_scale;    // [0] absmax bits, [1] scale (power of two), [2] 1/scale
   const double* dinv;       // 1/D0
   const double* s_layer;    // exact row sums per layer: h dx dy [top] + C V / dt
   const double* cap_layer;  // C V / dt per layer (0 when steady)

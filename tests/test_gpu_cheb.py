@@ -31,12 +31,12 @@ def _rhs(w):
     return w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
 
 
-def _setup(w, prec, steps=20, degree=30):
+def _setup(w, prec, steps=20, degree=30, storage=0):
     import paper_2606_17850_b200 as cu
     M = cu.DiaMatrix(grid_from_workload(w))
     S = cu.Solver(M, cu.Opts(precision=prec, rtol=1e-8, true_resid_period=w.true_resid_period))
     b = _rhs(w)
-    lo, hi, gersh = S.setup_chebyshev(to_dev(b), lanczos_steps=steps, degree=degree)
+    lo, hi, gersh = S.setup_chebyshev(to_dev(b), lanczos_steps=steps, degree=degree, storage=storage)
     return M, S, b, lo, hi, gersh
 
 
@@ -124,6 +124,30 @@ def test_pcg_cheb_mixed_vs_oracle(kw):
     assert np.abs(xh - ref.x).max() <= 1e-4
     if w.n >= 8192:
         assert res.iterations < ref.iterations / 2                      # far fewer outer iterations than Jacobi
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_cheb_fp16_matrix_apply_and_solve(kw):
+    """A3: half-precision off-diagonals (times a power-of-two scale), promoted to fp32 on load (Alg. 4's
+    arithmetic decoupling, PAPER.md:334, 344-374).  The apply is a 2^-11-accurate copy of the same operator;
+    the solve must still meet both parity bars, the outer loop and the true residual being fp64."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    M, S, b, lo, hi, gersh = _setup(w, cu.MIXED, storage=cu.CHEB_A3_FP16)
+    r = W.normal01(w.seed, 50, 51, np.arange(w.n)) * 1e-7
+    z = torch.empty(w.n, dtype=torch.float64, device="cuda")
+    S.cheb_apply(to_dev(r), z)
+    ref = O.cheb_apply(A, r, S.opts.cheb_lmin, S.opts.cheb_lmax, 30)
+    assert np.linalg.norm(z.cpu().numpy() - ref) <= 2e-2 * np.linalg.norm(ref)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    S.solve(to_dev(b), x)
+    res = S.result()
+    xh = x.cpu().numpy()
+    assert res.status == 0, res
+    assert np.linalg.norm(b - O.spmv(A, xh)) <= 1e-8 * np.linalg.norm(b)
+    assert np.abs(xh - O.pcg(A, b).x).max() <= 1e-4
 
 
 def test_cheb_bad_interval_rejected_or_reported():
