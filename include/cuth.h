@@ -40,7 +40,8 @@ typedef enum {
 /* result_D->status values (device-side, numerical outcome of a solve) */
 enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN = 2, CUTH_SOLVE_RUNNING = 3 };
 
-enum { CUTH_FP64 = 0, CUTH_MIXED = 1 };            /* cuth_opts_t.precision / cuth_spmv precision */
+enum { CUTH_FP64 = 0, CUTH_MIXED = 1,              /* cuth_opts_t.precision / cuth_spmv precision */
+       CUTH_ABLATION_STD32 = 2 };                  /* cuth_spmv only: fp32-rounded A2 in STANDARD form (ablation) */
 enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1, CUTH_PRECOND_CHEBYSHEV = 2 };
 enum { CUTH_CHEB_DEFAULT = 0, CUTH_CHEB_A3_FP16 = 1 };   /* cuth_opts_t.cheb_storage */
 
@@ -114,7 +115,9 @@ int cuth_dia_view(const void* dia_D, const cuth_grid_t* grid, const double** val
  * y[i] = D0[i] x[i] + sum_k ( Dk[i] x[i+off k] + Dk[i-off k] x[i-off k] ), out-of-range terms dropped.
  * precision CUTH_FP64: fp64 matrix A1.  CUTH_MIXED: fp32-stored off-diagonals promoted to fp64
  * ("FP64/32 SpMV with arithmetic decoupling") applied in difference form
- * y_i = s_i x_i + sum_j g_ij (x_i - x_j) (DESIGN.md R-F3).  x_D, y_D: fp64 [N], distinct buffers. */
+ * y_i = s_i x_i + sum_j g_ij (x_i - x_j) (DESIGN.md R-F3).  CUTH_ABLATION_STD32: the same fp32 copy applied
+ * literally in standard form (all four diagonals rounded): an ablation switch that reproduces the fixed-fp32
+ * drift of the paper's Table VI; no solver path uses it.  x_D, y_D: fp64 [N], distinct buffers. */
 int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const double* x_D, double* y_D,
               void* stream);
 

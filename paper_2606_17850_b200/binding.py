@@ -11,7 +11,7 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("CUTH_LIB", os.path.join(HERE, "libcuth.so"))   # CUTH_LIB: developer override
 
-FP64, MIXED = 0, 1
+FP64, MIXED, ABLATION_STD32 = 0, 1, 2
 PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV = 0, 1, 2
 CHEB_DEFAULT, CHEB_A3_FP16 = 0, 1
 STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}

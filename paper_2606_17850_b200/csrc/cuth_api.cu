@@ -88,7 +88,7 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   const double* lay = (const double*)(base + L.o_layers);
   DiaDev A;
   A.d0 = v + L.ptr[0]; A.d1 = v + L.ptr[1]; A.d2 = v + L.ptr[2]; A.d3 = v + L.ptr[3];
-  A.f1 = f + L.ptr[1]; A.f2 = f + L.ptr[2]; A.f3 = f + L.ptr[3];
+  A.f0 = f + L.ptr[0]; A.f1 = f + L.ptr[1]; A.f2 = f + L.ptr[2]; A.f3 = f + L.ptr[3];
   A.dinv = (const double*)(base + L.o_dinv);
   A.h1 = (const __half*)(base + L.o_h16);
   A.h2 = (const __half*)(base + L.o_h16 + L.h16_stride);
@@ -471,12 +471,13 @@ int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const d
   if (rc) return rc;
   if (!dia_D || !x_D || !y_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(y_D)) return CUTH_ERR_ALIGN;
-  if (precision != CUTH_FP64 && precision != CUTH_MIXED) return CUTH_ERR_VALUE;
+  if (precision != CUTH_FP64 && precision != CUTH_MIXED && precision != CUTH_ABLATION_STD32) return CUTH_ERR_VALUE;
   if (x_D == y_D) return CUTH_ERR_VALUE;
   DiaDev A = dev_view(dia_D, L);
   const int sb = stencil_blocks(L);
   const int blocks = sb > 0 ? sb : grid_blocks(L.n);
-  if (precision == CUTH_MIXED) k_spmv_only<true><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
+  if (precision == CUTH_ABLATION_STD32) k_spmv_std32<<<grid_blocks(L.n), kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
+  else if (precision == CUTH_MIXED) k_spmv_only<true><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
   else k_spmv_only<false><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
   CU(cudaGetLastError());
   return CUTH_OK;

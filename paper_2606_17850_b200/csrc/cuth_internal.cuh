@@ -56,6 +56,7 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
 // Device view of the matrix handed to kernels by value.
 struct DiaDev {
   const double* d0; const double* d1; const double* d2; const double* d3;   // fp64 diagonals (A1)
+  const float* f0;                                                          // fp32 main diagonal (A2), ablation only
   const float* f1; const float* f2; const float* f3;                        // fp32 off-diagonals (A2)
   const __half* h1; const __half* h2; const __half* h3;                     // fp16 off-diagonals x scale (A3)
   const double* h_scale;    // [0] absmax bits, [1] scale (power of two), [2] 1/scale

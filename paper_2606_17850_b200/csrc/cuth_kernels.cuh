@@ -147,6 +147,31 @@ __global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_only(DiaDev A, con
   apply_A<MIXED>(A, x, [&](int64_t i, double, double yi) { y[i] = yi; });
 }
 
+// ABLATION ONLY (Table VI of the paper): the paper's "FP64/32 SpMV with AD"
+// taken literally -- ALL four diagonals of the fp32-rounded copy A2 in standard form,
+// promoted to fp64.  Rounding D0 perturbs it by ~5e-11 W/K, the size of the whole convective term that
+// fixes the mean temperature, so b - A2 x has a floor of ~1e-2 ||b|| on these grids (DESIGN.md R-F3).  Not
+// used by any solver path; it exists so that the test suite can show why the difference form is used.
+__global__ void __launch_bounds__(kThreads) k_spmv_std32(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  CUTH_TILE_LOOP(n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < n) {
+        double acc = (double)A.f0[i] * x[i];
+        if (i + 1 < n) acc = fma((double)A.f1[i], x[i + 1], acc);
+        if (i >= 1) acc = fma((double)A.f1[i - 1], x[i - 1], acc);
+        if (i + nx < n) acc = fma((double)A.f2[i], x[i + nx], acc);
+        if (i >= nx) acc = fma((double)A.f2[i - nx], x[i - nx], acc);
+        if (i + np < n) acc = fma((double)A.f3[i], x[i + np], acc);
+        if (i >= np) acc = fma((double)A.f3[i - np], x[i - np], acc);
+        y[i] = acc;
+      }
+    }
+  }
+}
+
 // Writes the per-call context and clears the control block (plain launch before the graph).
 __global__ void k_set_ctx(Ctx c, Ctx* dst, Ctl* ctl) {
   if (threadIdx.x == 0) {

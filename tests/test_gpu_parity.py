@@ -98,6 +98,24 @@ def test_spmv_mixed_close_to_fp64(kw):
     assert np.allclose(ones, s.reshape(-1), rtol=1e-15, atol=0)
 
 
+def test_ablation_standard_form_fp32_has_a_residual_floor():
+    """Table VI of the paper: fixed fp32 drifts.  With the fp32-rounded matrix in STANDARD
+    form the exact solution has a relative residual of ~1e-2 on these grids (rounding D0 swamps the convective
+    term); in the difference form used by the MIXED operator it is ~1e-7 (F3)."""
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(2, nx=96, ny=96, nz=16, n_hot=12)
+    A = O.assemble_workload(w)
+    xs = O.pcg(A, w.power, rtol=1e-10).x
+    M = cu.DiaMatrix(grid_from_workload(w))
+    bn = np.linalg.norm(w.power)
+    r_std = np.linalg.norm(w.power - M.spmv(to_dev(xs), cu.ABLATION_STD32).cpu().numpy()) / bn
+    r_dif = np.linalg.norm(w.power - M.spmv(to_dev(xs), cu.MIXED).cpu().numpy()) / bn
+    r_f64 = np.linalg.norm(w.power - M.spmv(to_dev(xs), cu.FP64).cpu().numpy()) / bn
+    assert r_f64 <= 1e-9
+    assert r_dif <= 1e-6
+    assert r_std >= 1e-4 and r_std >= 1e3 * r_dif
+
+
 # ---------------------------------------------------------------- a1-a5: PCG, fp64 mode
 @pytest.mark.parametrize("kw", SMALL + [dict(cfg=2)])
 def test_pcg_fp64_vs_oracle(kw):
