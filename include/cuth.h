@@ -161,6 +161,11 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid);
 int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
                         size_t work_bytes, double bounds_H[5], void* stream);
 
+/* The host half of cuth_lanczos_bounds on its own (pure host, no CUDA): smallest and largest eigenvalue of
+ * the symmetric tridiagonal matrix with diagonal alpha_H[0..m) and off-diagonal beta_H[0..m-1), by Sturm
+ * bisection in fp64 (the spectrum of T is solved on the CPU). */
+int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, double out_H[2]);
+
 /* One application of the Chebyshev polynomial preconditioner, z = q(A) r (Alg. 3), with the
  * degree and interval of `opts` (preconditioner must be CUTH_PRECOND_CHEBYSHEV): k-1 stencil kernels, no
  * reduction.  precision CUTH_FP64: fp64 vectors and matrix; CUTH_MIXED: fp32 vectors on the fp32-stored matrix

@@ -51,7 +51,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes"]
 
 _lib = None
 
@@ -230,6 +230,17 @@ def cuth_lanczos_bounds(dia, grid: Grid, v0, steps, work, stream=None):
 def cuth_cheb_apply(dia, grid: Grid, opts, r, z, work, stream=None):
     _check(load_library().cuth_cheb_apply(_ptr(dia), grid.ref(), C.byref(opts), _ptr(r), _ptr(z), _ptr(work),
                                           work.numel() * work.element_size(), stream or _stream()), "cuth_cheb_apply")
+
+
+def cuth_tridiag_extremes(alpha, beta):
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    b = np.ascontiguousarray(beta, dtype=np.float64)
+    out = (C.c_double * 2)()
+    L = load_library()
+    L.cuth_tridiag_extremes.restype = C.c_int
+    _check(L.cuth_tridiag_extremes(a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), C.c_int(a.size), out),
+           "cuth_tridiag_extremes")
+    return out[0], out[1]
 
 
 def cuth_set_loop_mode(mode: int):

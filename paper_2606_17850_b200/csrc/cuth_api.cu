@@ -608,6 +608,13 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   return CUTH_OK;
 }
 
+int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, double out_H[2]) {
+  if (!alpha_H || !out_H || (m > 1 && !beta_H)) return CUTH_ERR_NULL;
+  if (m < 1) return CUTH_ERR_VALUE;
+  tridiag_extremes(alpha_H, beta_H, m, &out_H[0], &out_H[1]);
+  return CUTH_OK;
+}
+
 int cuth_set_loop_mode(int mode) {
   if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
   g_loop_mode.store(mode);

@@ -64,3 +64,22 @@ def test_no_cpu_fallback_without_device(cu):
     g = cu.Grid(4, 4, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
     with pytest.raises(RuntimeError):
         cu.DiaMatrix(g)
+
+
+def test_tridiag_extremes_vs_lapack(cu):
+    """Host half of the Lanczos setup (Sturm bisection) against LAPACK on random and on Lanczos tridiagonals."""
+    import scipy.linalg as sla
+    import workloads as W
+    for m, seed in ((1, 1), (2, 2), (7, 3), (40, 4), (120, 5)):
+        a = 1e-3 * (1.0 + W.uniform01(seed, 60, np.arange(m)))
+        b = 5e-4 * W.uniform01(seed, 61, np.arange(max(m - 1, 1)))
+        lo, hi = cu.cuth_tridiag_extremes(a, b[:max(m - 1, 0)] if m > 1 else np.zeros(1))
+        w = sla.eigvalsh_tridiagonal(a, b[:m - 1]) if m > 1 else a
+        assert lo == pytest.approx(w[0], rel=1e-12, abs=1e-18) and hi == pytest.approx(w[-1], rel=1e-12)
+    from oracle import oracle as O
+    wl = W.make_workload(1)
+    A = O.assemble_workload(wl)
+    al, be = O.lanczos(A, wl.power, 30)
+    lo, hi = cu.cuth_tridiag_extremes(al, be[:len(al) - 1])
+    lo_o, hi_o = O.ritz_extremes(al, be)
+    assert lo == pytest.approx(lo_o, rel=1e-9) and hi == pytest.approx(hi_o, rel=1e-12)
