@@ -314,7 +314,9 @@ def main():
     peak, peak_src = peaks()
     kern = {}
     cu.cuth_profile_kernel(S.work, g, -1)
-    fused = cu.cuth_launches_per_iteration(g) == 2
+    lpi = cu.cuth_launches_per_iteration(g)
+    persistent = (lpi == 0) and not (args.preconditioner == "chebyshev")   # whole solve = one cooperative kernel
+    fused = lpi == 2
     names = ({4: "k_fused_pspmv", 5: "k_update_nox", 3: "k_true_resid"} if fused else
              {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"})
     body_ids = (4, 5) if fused else (0, 1, 2)
@@ -388,6 +390,8 @@ def main():
     per_it = (2 if fused else 3) + (args.cheb_degree - 1 if cheb else 0)
     per_eval = 3 if fused else 2
     launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
+    if persistent:
+        launches = args.steps * nt * (2 + (1 if w.transient else 0))      # k_set_ctx + k_pcg_persistent
 
     line = {
         "metric": METRIC, "value": ms_per_step * 1e-3, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -420,6 +424,7 @@ def main():
                                        "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
+        "loop": "persistent cooperative kernel" if persistent else "cuda graph (conditional WHILE/IF nodes)",
         "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,

@@ -150,6 +150,27 @@ def test_cheb_fp16_matrix_apply_and_solve(kw):
     assert np.abs(xh - O.pcg(A, b).x).max() <= 1e-4
 
 
+def test_lanczos_invariant_subspace_on_a_tiny_grid():
+    """N = 8 < requested Lanczos steps: the Krylov space is exhausted (beta_j -> 0); the bounds must still be
+    the exact extreme eigenvalues and the Chebyshev solve must work."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(1, nx=2, ny=2, nz=2, n_hot=0)
+    A = O.assemble_workload(w)
+    lam = np.linalg.eigvalsh(A.to_scipy().toarray())
+    M = cu.DiaMatrix(grid_from_workload(w))
+    S = cu.Solver(M, cu.Opts(precision=cu.FP64))
+    v0 = W.uniform01(7, 70, np.arange(w.n)) + 0.1          # generic start vector (b is constant per layer here)
+    lo, hi, gersh = S.setup_chebyshev(to_dev(v0), lanczos_steps=20, degree=5)
+    assert lam[0] * (1 - 1e-6) <= lo <= lam[-1] and hi == pytest.approx(lam[-1], rel=1e-6)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    S.solve(to_dev(w.power), x)
+    res = S.result()
+    assert res.status == 0
+    xs = np.linalg.solve(A.to_scipy().toarray(), w.power)
+    assert np.abs(x.cpu().numpy() - xs).max() <= 1e-6 * np.abs(xs).max()
+
+
 def test_cheb_bad_interval_rejected_or_reported():
     import torch
     import paper_2606_17850_b200 as cu

@@ -26,6 +26,7 @@ def traversal(request):
     cu.cuth_set_loop_mode(0)
 
 SMALL = [
+    dict(cfg=1, nx=2, ny=2, nz=2, n_hot=0),        # the smallest grid the ABI accepts (N = 8)
     dict(cfg=1, nx=4, ny=3, nz=2, n_hot=1),
     dict(cfg=1, nx=7, ny=2, nz=5, n_hot=1),
     dict(cfg=1),                                   # BASELINE configs[0], full size
