@@ -178,6 +178,11 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
 
+/* Tuning knob, process-wide: variant of the fused kernel K1 on the z-marching path.  0 = automatic (two
+ * x-adjacent columns per thread with 16-byte vector traffic when nx is even, one column otherwise),
+ * 1 = always one column per thread, 2 = same as 0.  Results agree up to fp64 summation order. */
+int cuth_set_k1_variant(int mode);
+
 /* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: for tiny grids (N <= 65536, flat
  * traversal, Jacobi / no preconditioner) the whole solve is ONE persistent cooperative kernel whose
  * iterations are separated by grid-wide barriers; everything else runs as the CUDA graph with conditional

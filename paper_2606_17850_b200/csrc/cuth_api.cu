@@ -14,6 +14,7 @@
 #include <unordered_map>
 
 #include "cuth_fused.cuh"
+#include "cuth_fused_x2.cuh"
 #include "cuth_cheb.cuh"
 #include "cuth_persistent.cuh"
 
@@ -76,7 +77,14 @@ static int cheb_blocks(const DiaLayout& L) {
 
 static bool cheb_x2(const DiaLayout& L) { return use_zmarch(L) && (L.nx % 2 == 0); }
 
+static std::atomic<int> g_k1_variant{0};   // 0 auto (two columns per thread when nx is even), 1 one column, 2 two columns
+static bool fused_x2(const DiaLayout& L) { return (L.nx % 2 == 0) && g_k1_variant.load() != 1; }
+
 static int fused_blocks(const DiaLayout& L) {
+  if (fused_x2(L)) {
+    const int64_t t2 = ((L.nx + XTX - 1) / XTX) * ((L.ny + XTY - 1) / XTY);
+    return (int)(t2 < kMaxBlocks ? t2 : kMaxBlocks);
+  }
   const int64_t tiles = ((L.nx + FTX - 1) / FTX) * ((L.ny + FTY - 1) / FTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
@@ -138,6 +146,7 @@ struct GraphEntry {
   int fblocks = 0;
   int chebkey = 0;
   int x2blocks = 0;
+  int k1x2 = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -156,7 +165,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
 }
 
 static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
-                       int x2blocks, GraphEntry* out) {
+                       int x2blocks, int k1x2, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -207,7 +216,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   const size_t ndep0 = n_c ? 1 : 0;
   if (fblocks > 0) {
     { void* a[] = {&ctx, &ctl, &partials};
-      CU(add_kernel(body, &n_s, dep0, ndep0, (void*)k_fused_pspmv, fblocks, a)); }
+      CU(add_kernel(body, &n_s, dep0, ndep0, k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, fblocks, a)); }
     { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
       CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a)); }
   } else {
@@ -237,13 +246,13 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
 static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     int cblocks, int x2blocks, cudaGraphExec_t* ex) {
+                     int cblocks, int x2blocks, int k1x2, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
@@ -251,7 +260,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
                                it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
-                               it->second.x2blocks != x2blocks)) {
+                               it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -259,7 +268,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -377,7 +386,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   }
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
-                 cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0, &ex);
+                 cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0,
+                 (use_zmarch(L) && fused_x2(L)) ? 1 : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -511,7 +521,10 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 0: k_pupdate<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl); break;
     case 1: k_spmv_dot<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
-    case 4: k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
+    case 4:
+      if (fused_x2(L)) k_fused_pspmv_x2<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
+      else k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
+      break;
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
       const int code = kernel_id - 6;
@@ -612,6 +625,12 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
   if (!alpha_H || !out_H || (m > 1 && !beta_H)) return CUTH_ERR_NULL;
   if (m < 1) return CUTH_ERR_VALUE;
   tridiag_extremes(alpha_H, beta_H, m, &out_H[0], &out_H[1]);
+  return CUTH_OK;
+}
+
+int cuth_set_k1_variant(int mode) {
+  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
+  g_k1_variant.store(mode);
   return CUTH_OK;
 }
 

@@ -14,16 +14,18 @@ from gpu_util import grid_from_workload, to_dev, gpu_solve
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(params=["flat-graph", "flat-persistent", "zmarch"], autouse=True)
+@pytest.fixture(params=["flat-graph", "flat-persistent", "zmarch", "zmarch-k1x1"], autouse=True)
 def traversal(request):
     """Every parity case runs with both grid traversals of the kernels that apply A, and on the flat
     traversal with both homes of the loop (CUDA graph with conditional nodes / one persistent kernel)."""
     import paper_2606_17850_b200 as cu
-    cu.cuth_set_traversal(2 if request.param == "zmarch" else 1)
+    cu.cuth_set_traversal(2 if request.param.startswith("zmarch") else 1)
+    cu.cuth_set_k1_variant(1 if request.param == "zmarch-k1x1" else 0)
     cu.cuth_set_loop_mode(1 if request.param == "flat-graph" else 2)
     yield request.param
     cu.cuth_set_traversal(0)
     cu.cuth_set_loop_mode(0)
+    cu.cuth_set_k1_variant(0)
 
 SMALL = [
     dict(cfg=1, nx=2, ny=2, nz=2, n_hot=0),        # the smallest grid the ABI accepts (N = 8)
