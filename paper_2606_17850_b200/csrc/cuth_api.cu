@@ -56,7 +56,8 @@ static bool use_zmarch(const DiaLayout& L) {
 
 static int stencil_blocks(const DiaLayout& L) {
   if (!use_zmarch(L)) return -1;
-  const int64_t tiles = ((L.nx + ZTX - 1) / ZTX) * ((L.ny + ZTY - 1) / ZTY);
+  const int64_t wx = (L.nx % 2 == 0) ? 2 * ZTX : ZTX;      // two columns per thread when nx is even
+  const int64_t tiles = ((L.nx + wx - 1) / wx) * ((L.ny + ZTY - 1) / ZTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
@@ -106,7 +107,8 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   A.cap_layer = lay + 2 * L.nz;
   A.n = L.n; A.nx = L.nx; A.nxny = L.nxny;
   A.ny = (int32_t)L.ny; A.nz = (int32_t)L.nz;
-  A.zmarch = use_zmarch(L) ? 1 : 0; A.pad = 0;
+  A.zmarch = use_zmarch(L) ? 1 : 0;
+  A.x2 = (L.nx % 2 == 0) ? 1 : 0;
   return A;
 }
 

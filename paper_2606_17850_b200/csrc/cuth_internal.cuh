@@ -65,7 +65,8 @@ struct DiaDev {
   const double* cap_layer;  // C V / dt per layer (0 when steady)
   int64_t n, nx, nxny;
   int32_t ny, nz;
-  int32_t zmarch, pad;      // 1: march in z per thread (plane neighbours in registers), 0: flat 1-D streaming
+  int32_t zmarch, x2;       // zmarch 1: march in z per thread (plane neighbours in registers), 0: flat 1-D
+                            // streaming; x2 1: two x-adjacent columns per thread (nx even), 16-byte vector loads
 };
 
 // Pointers and options of one solve; lives at the start of the workspace, written per call.

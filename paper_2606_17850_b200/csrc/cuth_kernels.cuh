@@ -121,11 +121,85 @@ __device__ __forceinline__ void zmarch_apply(const DiaDev& A, const double* __re
   }
 }
 
+// The same traversal with two x-adjacent columns per thread (nx even: every row starts at an even index, so
+// v, D0 and D1 pairs are aligned 16-byte loads; D2 / D3 start at odd elements of the packed buffer, R-G5b,
+// and stay scalar; the fp32 copy likewise).  Halves the index / predicate instructions per row, which is
+// what bounds the one-column version (ncu: ~100 instructions per row, issue slots ~50 % busy).
+template <bool MIXED, class F>
+__device__ __forceinline__ void zmarch_apply_x2(const DiaDev& A, const double* __restrict__ v, F&& f) {
+  const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
+  const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
+  const int tiles_x = (nxi + 2 * ZTX - 1) / (2 * ZTX), tiles_y = (nyi + ZTY - 1) / ZTY;
+  const int ntiles = tiles_x * tiles_y;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  auto ld2 = [](const double* p) { return *reinterpret_cast<const double2*>(p); };
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int bx = t % tiles_x, by = t / tiles_x;
+    const int x = bx * 2 * ZTX + 2 * tx, y = by * ZTY + ty;
+    if (x >= nxi || y >= nyi) continue;
+    const int64_t c0 = x + nx * (int64_t)y;
+    double2 v_lo = make_double2(0.0, 0.0), v_c = ld2(v + c0);
+    double a3l0 = 0.0, a3l1 = 0.0;
+#pragma unroll 2
+    for (int z = 0; z < nz; ++z) {
+      const int64_t i = c0 + (int64_t)z * np;
+      const bool up3 = z + 1 < nz, up2 = i + nx < n, lo2 = i >= nx, lo1 = i >= 1, up1 = i + 2 < n;
+      double a1a, a1b = 0.0, a1l, a2u0 = 0.0, a2u1 = 0.0, a2l0 = 0.0, a2l1 = 0.0, a3u0 = 0.0, a3u1 = 0.0;
+      double2 d0 = make_double2(0.0, 0.0);
+      if (!MIXED) {
+        d0 = ld2(A.d0 + i);
+        if (up1) { const double2 d1 = ld2(A.d1 + i); a1a = d1.x; a1b = d1.y; } else { a1a = A.d1[i]; }
+        a1l = lo1 ? A.d1[i - 1] : 0.0;
+        if (up2) { a2u0 = A.d2[i]; a2u1 = A.d2[i + 1]; }
+        if (lo2) { a2l0 = A.d2[i - nx]; a2l1 = A.d2[i + 1 - nx]; }
+        if (up3) { a3u0 = A.d3[i]; a3u1 = A.d3[i + 1]; }
+      } else {
+        if (up1) { const float2 g = *reinterpret_cast<const float2*>(A.f1 + i); a1a = (double)g.x; a1b = (double)g.y; }
+        else { a1a = (double)A.f1[i]; }
+        a1l = lo1 ? (double)A.f1[i - 1] : 0.0;
+        if (up2) { a2u0 = (double)A.f2[i]; a2u1 = (double)A.f2[i + 1]; }
+        if (lo2) { a2l0 = (double)A.f2[i - nx]; a2l1 = (double)A.f2[i + 1 - nx]; }
+        if (up3) { a3u0 = (double)A.f3[i]; a3u1 = (double)A.f3[i + 1]; }
+      }
+      // absent neighbours: their matrix entry is 0 (standard form) / they take the centre value (difference form)
+      const double2 zero2 = make_double2(0.0, 0.0);
+      const double2 v_hi = up3 ? ld2(v + i + np) : (MIXED ? v_c : zero2);
+      const double2 v2u = up2 ? ld2(v + i + nx) : (MIXED ? v_c : zero2);
+      const double2 v2l = lo2 ? ld2(v + i - nx) : (MIXED ? v_c : zero2);
+      const double vl = lo1 ? v[i - 1] : (MIXED ? v_c.x : 0.0), vr = up1 ? v[i + 2] : (MIXED ? v_c.y : 0.0);
+      double y0, y1;
+      if (!MIXED) {
+        y0 = d0.x * v_c.x;              y1 = d0.y * v_c.y;
+        y0 = fma(a1a, v_c.y, y0);       y1 = fma(a1a, v_c.x, y1);
+        y0 = fma(a1l, vl, y0);          y1 = fma(a1b, vr, y1);
+        y0 = fma(a2u0, v2u.x, y0);      y1 = fma(a2u1, v2u.y, y1);
+        y0 = fma(a2l0, v2l.x, y0);      y1 = fma(a2l1, v2l.y, y1);
+        y0 = fma(a3u0, v_hi.x, y0);     y1 = fma(a3u1, v_hi.y, y1);
+        y0 = fma(a3l0, v_lo.x, y0);     y1 = fma(a3l1, v_lo.y, y1);
+      } else {
+        const double s = A.s_layer[z];
+        const double2 lo = z > 0 ? v_lo : v_c;
+        y0 = s * v_c.x;                         y1 = s * v_c.y;
+        y0 = fma(a1a, v_c.y - v_c.x, y0);       y1 = fma(a1a, v_c.x - v_c.y, y1);
+        y0 = fma(a1l, vl - v_c.x, y0);          y1 = fma(a1b, vr - v_c.y, y1);
+        y0 = fma(a2u0, v2u.x - v_c.x, y0);      y1 = fma(a2u1, v2u.y - v_c.y, y1);
+        y0 = fma(a2l0, v2l.x - v_c.x, y0);      y1 = fma(a2l1, v2l.y - v_c.y, y1);
+        y0 = fma(a3u0, v_hi.x - v_c.x, y0);     y1 = fma(a3u1, v_hi.y - v_c.y, y1);
+        y0 = fma(a3l0, lo.x - v_c.x, y0);       y1 = fma(a3l1, lo.y - v_c.y, y1);
+      }
+      f(i, v_c.x, y0);
+      f(i + 1, v_c.y, y1);
+      v_lo = v_c; v_c = v_hi; a3l0 = a3u0; a3l1 = a3u1;
+    }
+  }
+}
+
 // y_i = (A v)_i handed to f(i, v_i, y_i) for every row, with the traversal chosen at build time.
 template <bool MIXED, class F>
 __device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restrict__ v, F&& f) {
   if (A.zmarch) {
-    zmarch_apply<MIXED>(A, v, f);
+    if (A.x2) zmarch_apply_x2<MIXED>(A, v, f);
+    else zmarch_apply<MIXED>(A, v, f);
   } else {
     CUTH_TILE_LOOP(A.n) {
 #pragma unroll
