@@ -178,9 +178,10 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
 
-/* Tuning knob, process-wide: variant of the fused kernel K1 on the z-marching path.  0 = automatic (two
- * x-adjacent columns per thread with 16-byte vector traffic when nx is even, one column otherwise),
- * 1 = always one column per thread, 2 = same as 0.  Results agree up to fp64 summation order. */
+/* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle
+ * step).  0 = automatic: two x-adjacent columns per thread with 16-byte vector traffic when nx is even and the
+ * plane still yields >= 2048 CTAs (cfg 3, cfg 4), one column otherwise; 1 = always one column per thread;
+ * 2 = two columns whenever nx is even.  Results agree up to fp64 summation order. */
 int cuth_set_k1_variant(int mode);
 
 /* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: for tiny grids (N <= 65536, flat

@@ -54,9 +54,26 @@ static bool use_zmarch(const DiaLayout& L) {
   return L.nxny >= (1 << 18);
 }
 
+static std::atomic<int> g_k1_variant{0};   // 0 auto (two columns per thread when nx is even), 1 one column, 2 two columns
+// Two columns per thread halve the number of CTAs: worth it only while the grid still has several waves
+// (cfg 5, 512x512 columns: 512 CTAs on 444 slots ran 13 % slower than the one-column kernel's 1024 CTAs).
+static bool enough_tiles_x2(const DiaLayout& L, int wx, int wy) {
+  return ((L.nx + wx - 1) / wx) * ((L.ny + wy - 1) / wy) >= 2048;
+}
+static bool fused_x2(const DiaLayout& L) {
+  const int mode = g_k1_variant.load();
+  if (L.nx % 2 != 0 || mode == 1) return false;
+  return mode == 2 || enough_tiles_x2(L, XTX, XTY);
+}
+static bool zmarch_x2(const DiaLayout& L) {
+  const int mode = g_k1_variant.load();
+  if (L.nx % 2 != 0 || mode == 1) return false;
+  return mode == 2 || enough_tiles_x2(L, 2 * ZTX, ZTY);
+}
+
 static int stencil_blocks(const DiaLayout& L) {
   if (!use_zmarch(L)) return -1;
-  const int64_t wx = (L.nx % 2 == 0) ? 2 * ZTX : ZTX;      // two columns per thread when nx is even
+  const int64_t wx = zmarch_x2(L) ? 2 * ZTX : ZTX;         // two columns per thread (even nx, enough tiles)
   const int64_t tiles = ((L.nx + wx - 1) / wx) * ((L.ny + ZTY - 1) / ZTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
@@ -76,10 +93,7 @@ static int cheb_blocks(const DiaLayout& L) {
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
-static bool cheb_x2(const DiaLayout& L) { return use_zmarch(L) && (L.nx % 2 == 0); }
-
-static std::atomic<int> g_k1_variant{0};   // 0 auto (two columns per thread when nx is even), 1 one column, 2 two columns
-static bool fused_x2(const DiaLayout& L) { return (L.nx % 2 == 0) && g_k1_variant.load() != 1; }
+static bool cheb_x2(const DiaLayout& L) { return use_zmarch(L) && zmarch_x2(L); }
 
 static int fused_blocks(const DiaLayout& L) {
   if (fused_x2(L)) {
@@ -108,7 +122,7 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   A.n = L.n; A.nx = L.nx; A.nxny = L.nxny;
   A.ny = (int32_t)L.ny; A.nz = (int32_t)L.nz;
   A.zmarch = use_zmarch(L) ? 1 : 0;
-  A.x2 = (L.nx % 2 == 0) ? 1 : 0;
+  A.x2 = zmarch_x2(L) ? 1 : 0;
   return A;
 }
 

@@ -19,12 +19,14 @@ CASES = [
 ]
 
 
-@pytest.fixture(params=["flat", "zmarch"], autouse=True)
+@pytest.fixture(params=["flat", "zmarch", "zmarch-x1"], autouse=True)
 def traversal(request):
     import paper_2606_17850_b200 as cu
-    cu.cuth_set_traversal({"flat": 1, "zmarch": 2}[request.param])
+    cu.cuth_set_traversal(1 if request.param == "flat" else 2)
+    cu.cuth_set_k1_variant(1 if request.param == "zmarch-x1" else 2)       # 2: two columns per thread when nx is even
     yield request.param
     cu.cuth_set_traversal(0)
+    cu.cuth_set_k1_variant(0)
 
 
 def _rhs(w):

@@ -20,7 +20,7 @@ def traversal(request):
     traversal with both homes of the loop (CUDA graph with conditional nodes / one persistent kernel)."""
     import paper_2606_17850_b200 as cu
     cu.cuth_set_traversal(2 if request.param.startswith("zmarch") else 1)
-    cu.cuth_set_k1_variant(1 if request.param == "zmarch-k1x1" else 0)
+    cu.cuth_set_k1_variant(1 if request.param == "zmarch-k1x1" else 2)     # 2: two columns per thread when nx is even
     cu.cuth_set_loop_mode(1 if request.param == "flat-graph" else 2)
     yield request.param
     cu.cuth_set_traversal(0)
