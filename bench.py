@@ -30,8 +30,8 @@ sys.path.insert(0, ROOT)
 import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
-# kernel (profiles/r1b_cfg3_fp64_fused.md); null for workloads/kernels not captured.
-NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.4498e9,
+# kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.4477e9,   # profiles/r1e (two-column K1)
                      ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 12.055e9,     # profiles/r1d_cfg4_fp64.md
                      ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_mid", "mixed"): 0.5670e9}  # r1c (1-column kernel)
 
