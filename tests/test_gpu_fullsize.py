@@ -95,6 +95,20 @@ def test_cfg4_full_size(mode):
     _check_invariants(w, A, w.power, x, res)
 
 
+@pytest.mark.parametrize("mode", ["fp64", "mixed", "chebyshev-fp64", "chebyshev-mixed"])
+def test_cfg6_paperlike_stack_full_size(mode):
+    """cfg 6 (the paper's ten layer thicknesses; 256x256x10): layered, so the separable direct
+    solve is the truth for every unknown."""
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(6)
+    A = O.assemble_workload(w)
+    x, res = _solve(w, cu.FP64 if mode.endswith("fp64") else cu.MIXED, chebyshev=mode.startswith("chebyshev"))
+    xd = solve_layered(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.kappa_layer, w.h_top, w.power)
+    err = np.abs(x - xd).max()
+    assert err <= (1e-6 * np.abs(xd).max() if mode.endswith("fp64") else 1e-4), err
+    _check_invariants(w, A, w.power, x, res)
+
+
 def test_cfg5_full_size_200_steps():
     import torch
     import paper_2606_17850_b200 as cu
