@@ -33,7 +33,7 @@ import workloads as W  # noqa: E402
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
 NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.4477e9,   # profiles/r1e (two-column K1)
                      ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 12.055e9,     # profiles/r1d_cfg4_fp64.md
-                     ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_mid", "mixed"): 0.5670e9}  # r1c (1-column kernel)
+                     }
 
 METRIC = "pcg_time_to_solution"
 UNIT = "s"
@@ -368,10 +368,11 @@ def main():
     m = m_ratio(w)
     if cheb:
         # outer: K1 (matrix + z, p, x read + p', mu, x written) + K2 (r, mu read, r written); preconditioner:
-        # FIRST M+8+3s, (k-3) x MID M+6s, LAST M+3s+16 with s = sizeof(T), M = matrix bytes per row
+        # FIRST M+8+3s (2s in fp64), (k-3) x MID M+4s, LAST M+2s+16 with s = sizeof(T), M = matrix bytes per row
+        #
         k, sT = args.cheb_degree, (4 if mixed else 8)
         Mc = (2 * (m - 1) if h16 else 4 * (m - 1)) if mixed else 8 * m
-        apply_bytes = (k - 1) * Mc + (3 * sT + 8) + (k - 3) * 6 * sT + (3 * sT + 16)
+        apply_bytes = (k - 1) * Mc + ((3 if mixed else 2) * sT + 8) + (k - 3) * 4 * sT + (2 * sT + 16)
         outer = lambda M_: M_ + 48 + 24
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
@@ -385,7 +386,7 @@ def main():
         dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
     if cheb:
         dom_name, dom_ms = "k_cheb_mid", kern["k_cheb_mid"]
-        dom_bytes = (((2 if h16 else 4) * (m - 1) + 24) if mixed else (8 * m + 48)) * w.n
+        dom_bytes = (((2 if h16 else 4) * (m - 1) + 16) if mixed else (8 * m + 32)) * w.n
         stage_fp64 = not mixed
     per_it = (2 if fused else 3) + (args.cheb_degree - 1 if cheb else 0)
     per_eval = 3 if fused else 2

@@ -2,10 +2,10 @@
 // spectral-range estimate: SURVEY.md §8(f) rank 1, the paper's own preconditioner.
 //
 // One apply z = q(A) r of degree k is k-1 stencil kernels with NO reduction inside:
-//   FIRST (i = 0)      d0 = r/theta (formed on the fly, also at the stencil neighbours: A d0 = (A r)/theta),
-//                      rc = r - A d0, z = d0, d1 = c1[0] d0 + c2[0] rc
-//   MID   (0 < i < k-2) rc -= A d_i, z += d_i, d_{i+1} = c1[i] d_i + c2[i] rc
-//   LAST  (i = k-2)    rc' = rc - A d_i, d_{k-1} = c1 d_i + c2 rc', z_out = z + d_i + d_{k-1}, rho = r.z_out
+// with d and r_c eliminated in favour of the partial sums Z_j = d_0 + ... + d_{j-1} (see k_cheb_first below):
+//   FIRST (i = 0)       Z_1 = r/theta formed on the fly (A Z_1 = (A r)/theta), Z_2
+//   MID   (0 < i < k-2) Z_{i+2} = Z_{i+1} + c1[i] (Z_{i+1} - Z_i) + c2[i] (r - A Z_{i+1}), written over Z_i
+//   LAST  (i = k-2)     z = Z_k (fp64), rho = r.z
 // (Alg. 3's k-th SpMV and d-update feed nothing and are skipped: z is identical.)
 // Element type T of d, rc, z: double (FP64 mode, fp64 matrix A1) or float (MIXED mode: "FP32 for all
 // vector and scalar operations" of Alg. 3, on the fp32-stored matrix A2 in difference form).
@@ -140,42 +140,48 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------------
-// Alg. 3 lines 1-4 and the first pass of lines 6-10.
+// Alg. 3 with d and r_c eliminated.  With Z_j = d_0 + ... + d_{j-1} (Z_0 = 0, Z_1 = d_0 = r/theta, z = Z_k) the
+// algorithm's own identities d_i = Z_{i+1} - Z_i and r_c = r - A Z_{i+1} (lines 6, 8) turn line 10 into
+//     Z_{i+2} = Z_{i+1} + c1_i (Z_{i+1} - Z_i) + c2_i (r - A Z_{i+1}),      i = 0 .. k-2,
+// the same k-1 stencil passes, but a pass now reads Z_{i+1} (stencil), Z_i and r at its own cell and writes
+// Z_{i+2} over Z_i (in place: only the own cell of Z_i is ever read): M + 4s bytes per row instead of M + 6s
+// (s = sizeof(T)), and the residual is formed directly instead of by recurrence.  Two buffers Z[0], Z[1]
+// (Ctx.cd): at pass i the stencil input is Z[(i+1)&1], the old iterate / output is Z[i&1].  In fp32 mode the
+// first pass also leaves an fp32 copy of r (Ctx.crc) for the later passes.
+//
+// First pass (i = 0): Z_1 = r/theta formed on the fly (A Z_1 = (A r)/theta), Z_2 = Z_1 + c1_0 Z_1 + c2_0 (r - A Z_1).
 template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_first(const Ctx* __restrict__ ctxp) {
   const Ctx c = *ctxp;
   const T inv_theta = (T)c.cheb_inv_theta, c1 = (T)ctxp->cheb_c1[0], c2 = (T)ctxp->cheb_c2[0];
-  T* __restrict__ rc = (T*)c.crc;
-  T* __restrict__ zc = (T*)c.czc;
-  T* __restrict__ d1 = (T*)c.cd[1];
+  T* __restrict__ z1 = (T*)c.cd[1];
+  T* __restrict__ z2 = (T*)c.cd[0];
+  T* __restrict__ r32 = (T*)c.crc;
   apply_A_t<double, T, M>(c.A, c.r, [&](int64_t i, T ri, T Ar) {
-    const T d0 = ri * inv_theta;                 // line 4
-    const T rci = ri - Ar * inv_theta;           // lines 7-8
-    rc[i] = rci;
-    zc[i] = d0;                                  // line 6
-    d1[i] = c1 * d0 + c2 * rci;                  // line 10
+    const T Z1 = ri * inv_theta;                 // lines 4, 6
+    const T res = ri - Ar * inv_theta;           // r - A Z_1 (lines 7-8)
+    z1[i] = Z1;
+    z2[i] = Z1 + c1 * Z1 + c2 * res;             // line 10, then line 6 of the next pass
+    if (sizeof(T) == 4) r32[i] = ri;
   });
 }
 
-// Alg. 3 lines 6-10 for 0 < i < k-2.
+// Passes 0 < i < k-2.
 template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
-  const T* __restrict__ din = (const T*)ctxp->cd[step & 1];
-  T* __restrict__ dout = (T*)ctxp->cd[(step + 1) & 1];
-  T* __restrict__ rc = (T*)c.crc;
-  T* __restrict__ zc = (T*)c.czc;
-  apply_A_t<T, T, M>(c.A, din, [&](int64_t i, T di, T Ad) {
-    const T rci = rc[i] - Ad;
-    rc[i] = rci;
-    zc[i] += di;
-    dout[i] = c1 * di + c2 * rci;
+  const T* __restrict__ zcur = (const T*)ctxp->cd[(step + 1) & 1];
+  T* __restrict__ zold = (T*)ctxp->cd[step & 1];
+  const T* __restrict__ r32 = (const T*)c.crc;
+  apply_A_t<T, T, M>(c.A, zcur, [&](int64_t i, T zi, T Az) {
+    const T ri = sizeof(T) == 4 ? r32[i] : (T)c.r[i];
+    zold[i] = zi + c1 * (zi - zold[i]) + c2 * (ri - Az);
   });
 }
 
 // The same middle step for T = float on large planes with even nx: each thread owns TWO x-adjacent columns,
-// so the vectors d, rc, zc move as 8-byte float2 (every row start is even => 8-byte aligned), the +-1
+// so the vectors Z_{i+1}, Z_i, r move as 8-byte float2 (every row start is even => 8-byte aligned), the +-1
 // neighbours of the pair are each other (registers), and a thread keeps twice the bytes in flight -- the
 // 4-byte version is latency-bound (profiles/r1c_cfg3_cheb_mixed.md).  Matrix entries stay scalar loads: the
 // packed diagonals D2, D3 start at odd elements (R-G5b).  Tile = (2 ZTX) x ZTY columns per CTA.
@@ -184,10 +190,9 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
   const Ctx c = *ctxp;
   const DiaDev& A = c.A;
   const float c1 = (float)ctxp->cheb_c1[step], c2 = (float)ctxp->cheb_c2[step];
-  const float* __restrict__ din = (const float*)ctxp->cd[step & 1];
-  float* __restrict__ dout = (float*)ctxp->cd[(step + 1) & 1];
-  float* __restrict__ rc = (float*)c.crc;
-  float* __restrict__ zc = (float*)c.czc;
+  const float* __restrict__ din = (const float*)ctxp->cd[(step + 1) & 1];     // Z_{i+1}: stencil input
+  float* __restrict__ zold = (float*)ctxp->cd[step & 1];                      // Z_i in, Z_{i+2} out (in place)
+  const float* __restrict__ r32 = (const float*)c.crc;
   const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
   const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
   const int tiles_x = (nxi + 2 * ZTX - 1) / (2 * ZTX), tiles_y = (nyi + ZTY - 1) / ZTY;
@@ -216,7 +221,7 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
       const float2 v_hi = up3 ? ld2(din + i + np) : v_c;
       const float2 v2u = up2 ? ld2(din + i + nx) : v_c, v2l = lo2 ? ld2(din + i - nx) : v_c;
       const float vl = lo1 ? din[i - 1] : v_c.x, vr = up1 ? din[i + 2] : v_c.y;
-      const float2 rcv = ld2(rc + i), zcv = ld2(zc + i);
+      const float2 rv = ld2(r32 + i), zo = ld2(zold + i);
       const float s = (float)A.s_layer[z];
       float a0 = s * v_c.x, a1 = s * v_c.y;
       a0 += f1a * (v_c.y - v_c.x);   a1 += f1a * (v_c.x - v_c.y);
@@ -225,16 +230,14 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
       a0 += f2l0 * (v2l.x - v_c.x);  a1 += f2l1 * (v2l.y - v_c.y);
       a0 += a3u.x * (v_hi.x - v_c.x); a1 += a3u.y * (v_hi.y - v_c.y);
       a0 += a3l.x * (v_lo.x - v_c.x); a1 += a3l.y * (v_lo.y - v_c.y);    // a3l = 0 at z = 0
-      const float2 rn = make_float2(rcv.x - a0, rcv.y - a1);
-      *reinterpret_cast<float2*>(rc + i) = rn;
-      *reinterpret_cast<float2*>(zc + i) = make_float2(zcv.x + v_c.x, zcv.y + v_c.y);
-      *reinterpret_cast<float2*>(dout + i) = make_float2(c1 * v_c.x + c2 * rn.x, c1 * v_c.y + c2 * rn.y);
+      *reinterpret_cast<float2*>(zold + i) = make_float2(v_c.x + c1 * (v_c.x - zo.x) + c2 * (rv.x - a0),
+                                                         v_c.y + c1 * (v_c.y - zo.y) + c2 * (rv.y - a1));
       v_lo = v_c; v_c = v_hi; a3l = a3u;
     }
   }
 }
 
-// Last stencil pass (i = k-2) + the two trailing z updates + rho = r.z (Alg. 1 lines 10-11).
+// Last pass (i = k-2): z = Z_k in fp64 for the outer loop, and rho = r.z (Alg. 1 lines 10-11).
 template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                         int step) {
@@ -242,16 +245,14 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
-  const T* __restrict__ din = (const T*)ctxp->cd[step & 1];
-  const T* __restrict__ rc = (const T*)c.crc;
-  const T* __restrict__ zc = (const T*)c.czc;
+  const T* __restrict__ zcur = (const T*)ctxp->cd[(step + 1) & 1];
+  const T* __restrict__ zold = (const T*)ctxp->cd[step & 1];
   double acc[1] = {0.0};
-  apply_A_t<T, T, M>(c.A, din, [&](int64_t i, T di, T Ad) {
-    const T rci = rc[i] - Ad;
-    const T dl = c1 * di + c2 * rci;             // d_{k-1}
-    const double zi = (double)(zc[i] + di + dl);
-    c.cz[i] = zi;
-    acc[0] = fma(c.r[i], zi, acc[0]);
+  apply_A_t<T, T, M>(c.A, zcur, [&](int64_t i, T zi, T Az) {
+    const double rd = c.r[i];
+    const double zk = (double)(zi + c1 * (zi - zold[i]) + c2 * ((T)rd - Az));
+    c.cz[i] = zk;
+    acc[0] = fma(rd, zk, acc[0]);
   });
   if (grid_sum_last_block<1>(acc, partials + 3 * kMaxBlocks, &ctl->ticket[5], smem, &s_flag) && threadIdx.x == 0) {
     const double rho_new = acc[0];
