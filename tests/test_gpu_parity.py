@@ -39,6 +39,9 @@ SMALL = [
 ]
 
 
+_POLICY_REF = {}
+
+
 def _true_rel_resid(A, b, x):
     r = b - O.spmv(A, x)
     return np.linalg.norm(r) / np.linalg.norm(b)
@@ -150,6 +153,37 @@ def test_pcg_mixed_vs_oracle(kw):
     assert np.abs(x - ref.x).max() <= 1e-4                     # kelvin, max-abs
     assert res.promotions in (0, 1)
     assert res.true_resid_evals >= 1
+
+
+@pytest.mark.parametrize("kw", [dict(cfg=1), dict(cfg=2, nx=64, ny=48, nz=16, n_hot=6),
+                                dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8), dict(cfg=6, nx=45, ny=38, nz=10, n_hot=6)])
+def test_mixed_policy_decisions_match_the_reference(kw):
+    """Row a5: the device-side policy (stage switch, true-residual cadence, restart) against the step-by-step
+    CPU reference written from PAPER.md §IV-D (oracle/policy.py): same switch criterion, switch within one
+    evaluation period, same promotion count, iteration counts and number of true-residual evaluations close
+    (fp64 summation order differs), temperatures within the MIXED bar."""
+    import paper_2606_17850_b200 as cu
+    from oracle import policy as P
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
+    s = np.zeros((w.nz, w.nx * w.ny))
+    s[w.nz - 1] += w.h_top * w.dx * w.dy
+    if w.transient:
+        s += (w.cvol * (w.dx * w.dy * w.dz) / w.dt)[:, None]
+    T = w.true_resid_period
+    key = tuple(sorted(kw.items()))
+    if key not in _POLICY_REF:                      # the numpy reference is slow; one run per case
+        _POLICY_REF[key] = P.pcg_mixed(A, s.reshape(-1), b, rtol=1e-8, period=T)
+    ref = _POLICY_REF[key]
+    x, res, _, _ = gpu_solve(w, b, cu.MIXED, period=T)
+    assert ref.status == 0 and res.status == 0
+    assert res.promotions == ref.promotions
+    assert res.switch_reason == ref.switch_reason
+    assert abs(res.switch_iteration - ref.switch_iteration) <= T
+    assert abs(res.iterations - ref.iterations) <= max(3, 0.03 * ref.iterations)
+    assert abs(res.true_resid_evals - ref.true_resid_evals) <= 2
+    assert np.abs(x - ref.x).max() <= 1e-4
 
 
 def test_pcg_unpreconditioned_reaches_same_x():
