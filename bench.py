@@ -70,11 +70,6 @@ def max_over_ranks(value_ms: float, world: int, device="cpu") -> float:
     return float(t.item())
 
 
-def replica_seed_offset(rank: int) -> int:
-    """Each replica solves the same configuration (weak scaling: per-GPU work fixed)."""
-    return 0
-
-
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown," \
         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown," \

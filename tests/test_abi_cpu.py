@@ -83,3 +83,15 @@ def test_tridiag_extremes_vs_lapack(cu):
     lo, hi = cu.cuth_tridiag_extremes(al, be[:len(al) - 1])
     lo_o, hi_o = O.ritz_extremes(al, be)
     assert lo == pytest.approx(lo_o, rel=1e-9) and hi == pytest.approx(hi_o, rel=1e-12)
+
+
+def test_layout_golden_sizes(cu):
+    """ptr[] of the C ABI against the element counts tabulated for the five BASELINE grids (tests/golden)."""
+    rows = np.loadtxt(os.path.join(ROOT, "tests", "golden", "layout_sizes.txt"), dtype=np.int64)
+    lib = cu.load_library()
+    for cfg, nx, ny, nz, n, e in rows:
+        g = cu.Grid(int(nx), int(ny), int(nz), 1e-6, 1e-6, np.full(int(nz), 1e-6), None, 1e4)
+        ptr = (C.c_int64 * 5)()
+        off = (C.c_int64 * 4)()
+        assert lib.cuth_dia_view(C.c_void_p(4096), g.ref(), None, None, None, ptr, off) == 0
+        assert nx * ny * nz == n and ptr[4] == e and ptr[1] == n
