@@ -321,7 +321,7 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
   }
   c->cheb = k;
   c->cheb_inv_theta = 1.0 / theta;
-  c->cz = w.cz; c->cd[0] = w.cd0; c->cd[1] = w.cd1; c->crc = w.crc; c->czc = w.czc;
+  c->cz = w.cz; c->cd[0] = w.cd0; c->cd[1] = w.cd1; c->crc = w.crc;
   c->jacobi = 0;
   c->precision = opts->precision;
 }
