@@ -109,13 +109,16 @@ def test_cfg6_paperlike_stack_full_size(mode):
     _check_invariants(w, A, w.power, x, res)
 
 
-def test_cfg5_full_size_200_steps():
+@pytest.mark.parametrize("precond", ["jacobi", "chebyshev"])
+def test_cfg5_full_size_200_steps(precond):
     import torch
     import paper_2606_17850_b200 as cu
     w = W.make_workload(5)
     A = O.assemble_workload(w)
     M = cu.DiaMatrix(grid_from_workload(w))
     S = cu.Solver(M, cu.Opts(precision=cu.MIXED, rtol=1e-8, true_resid_period=5))
+    if precond == "chebyshev":      # setup once, reused by all 200 steps
+        S.setup_chebyshev(to_dev(W.power_for_step(w, 1)), lanczos_steps=40, degree=30)
     T = torch.zeros(w.n, dtype=torch.float64, device="cuda")
     cap = np.repeat(w.cvol * (w.dx * w.dy * w.dz) / w.dt, w.nx * w.ny)
     T_prev = np.zeros(w.n)
