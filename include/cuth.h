@@ -178,6 +178,12 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
 
+/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes).  0 = automatic (today: one pass per
+ * kernel), 1 = one pass per kernel, 2 = two consecutive passes per kernel (k_cheb_pair_f32: 43 % fewer HBM
+ * bytes, correct and parity-tested, but measured ~2x slower than two single passes on B200 -- experimental).
+ * The polynomial is the same. */
+int cuth_set_cheb_fusion(int mode);
+
 /* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle
  * step).  0 = automatic: two x-adjacent columns per thread with 16-byte vector traffic when nx is even and the
  * plane still yields >= 2048 CTAs (cfg 3, cfg 4), one column otherwise; 1 = always one column per thread;
@@ -197,7 +203,7 @@ int cuth_set_loop_mode(int mode);
  * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual,
  * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path),
  * 6 / 7 / 8 = one middle step of the Chebyshev apply in fp64 / fp32 on A2 / fp32 on the fp16 copy A3 (only
- * after a CUTH_PRECOND_CHEBYSHEV solve).  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
+ * after a CUTH_PRECOND_CHEBYSHEV solve); 9 / 10 = one fused PAIR of Chebyshev passes on A2 / A3.  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
 int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
 
 #ifdef __cplusplus

@@ -51,7 +51,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion"]
 
 _lib = None
 
@@ -241,6 +241,12 @@ def cuth_tridiag_extremes(alpha, beta):
     _check(L.cuth_tridiag_extremes(a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), C.c_int(a.size), out),
            "cuth_tridiag_extremes")
     return out[0], out[1]
+
+
+def cuth_set_cheb_fusion(mode: int):
+    L = load_library()
+    L.cuth_set_cheb_fusion.restype = C.c_int
+    _check(L.cuth_set_cheb_fusion(C.c_int(int(mode))), "cuth_set_cheb_fusion")
 
 
 def cuth_set_k1_variant(mode: int):

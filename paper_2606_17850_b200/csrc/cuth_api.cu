@@ -12,10 +12,12 @@
 #include <mutex>
 #include <string>
 #include <unordered_map>
+#include <vector>
 
 #include "cuth_fused.cuh"
 #include "cuth_fused_x2.cuh"
 #include "cuth_cheb.cuh"
+#include "cuth_cheb_pair.cuh"
 #include "cuth_persistent.cuh"
 
 namespace cuth {
@@ -148,9 +150,47 @@ static void* cheb_mid_fn(int code, bool x2) {
   if (x2) return code == 1 ? (void*)k_cheb_mid_f32x2<MatF32> : (void*)k_cheb_mid_f32x2<MatF16>;
   return code == 1 ? (void*)k_cheb_mid<float, MatF32> : (void*)k_cheb_mid<float, MatF16>;
 }
+static void* cheb_pair_fn(int code) {
+  return code == 2 ? (void*)k_cheb_pair_f32<MatF16> : (void*)k_cheb_pair_f32<MatF32>;
+}
+static std::atomic<int> g_cheb_pairs{0};   // 0 auto, 1 never, 2 always (fp32 modes): cuth_set_cheb_fusion
+static int cheb_pair_blocks(const DiaLayout& L) {
+  const int64_t tiles = ((L.nx + PTX - 1) / PTX) * ((L.ny + PTY - 1) / PTY);
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
+}
+static bool cheb_pairs(const DiaLayout& L, int code) {
+  const int mode = g_cheb_pairs.load();
+  if (code == 0 || mode == 1) return false;          // fp32 arithmetic only
+  // Measured (cfg 3 / cfg 4, B200): the straightforward two-pass kernel moves 43 % fewer HBM bytes but is
+  // latency-bound (three barrier-separated phases per plane, scalar loads, 3 CTAs/SM): 20.3 s vs 10.8 s at cfg 4.
+  // Until its phases are software-pipelined it stays an opt-in (mode 2); automatic = single passes.
+  (void)L;
+  return mode == 2;
+}
 static void* cheb_last_fn(int code) {
   return code == 0 ? (void*)k_cheb_last<double, MatF32> : code == 1 ? (void*)k_cheb_last<float, MatF32>
                                                                     : (void*)k_cheb_last<float, MatF16>;
+}
+
+// The passes of one Chebyshev apply after the first one: MID passes i = 1 .. k-3 (single, or fused in pairs),
+// then LAST (i = k-2).  State = which buffers hold Z_i (old) and Z_{i+1} (cur); k_cheb_first leaves old = 1, cur = 0.
+struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST
+static std::vector<ChebOp> cheb_schedule(int k, bool pairs) {
+  std::vector<ChebOp> ops;
+  int old = 1, cur = 0, i = 1;
+  while (i <= k - 3) {
+    if (pairs && i + 1 <= k - 3) {
+      int fr[2], nf = 0;
+      for (int b = 0; b < 4; ++b) if (b != old && b != cur) fr[nf++] = b;
+      ops.push_back({1, i, old, cur, fr[0], fr[1]});
+      old = fr[0]; cur = fr[1]; i += 2;
+    } else {
+      ops.push_back({0, i, old, cur, -1, -1});
+      const int t = old; old = cur; cur = t; i += 1;
+    }
+  }
+  ops.push_back({2, k - 2, old, cur, -1, -1});
+  return ops;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -163,6 +203,7 @@ struct GraphEntry {
   int chebkey = 0;
   int x2blocks = 0;
   int k1x2 = 0;
+  int pblocks = 0;
   int device = -1;
 };
 static std::mutex g_mu;
@@ -181,7 +222,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
 }
 
 static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
-                       int x2blocks, int k1x2, GraphEntry* out) {
+                       int x2blocks, int k1x2, int pblocks, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -214,19 +255,23 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
     const bool f32 = code != 0;
     { void* a[] = {&ctx};
       CU(add_kernel(body, &n_c, nullptr, 0, cheb_first_fn(code), cblocks, a)); }
-    for (int i = 1; i <= kdeg - 3; ++i) {
+    for (const ChebOp& op : cheb_schedule(kdeg, pblocks > 0)) {
       cudaGraphNode_t prev = n_c;
-      int step = i;
-      void* a[] = {&ctx, &step};
-      if (f32 && x2blocks > 0)
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, true), x2blocks, a));
-      else
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, false), cblocks, a));
+      int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
+      if (op.kind == 1) {
+        void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
+      } else if (op.kind == 0) {
+        void* a[] = {&ctx, &step, &old, &cur};
+        if (f32 && x2blocks > 0)
+          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, true), x2blocks, a));
+        else
+          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, false), cblocks, a));
+      } else {
+        void* a[] = {&ctx, &ctl, &partials, &step, &old, &cur};
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_last_fn(code), cblocks, a));
+      }
     }
-    { cudaGraphNode_t prev = n_c;
-      int step = kdeg - 2;
-      void* a[] = {&ctx, &ctl, &partials, &step};
-      CU(add_kernel(body, &n_c, &prev, 1, cheb_last_fn(code), cblocks, a)); }
   }
   const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
   const size_t ndep0 = n_c ? 1 : 0;
@@ -262,13 +307,13 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
 static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     int cblocks, int x2blocks, int k1x2, cudaGraphExec_t* ex) {
+                     int cblocks, int x2blocks, int k1x2, int pblocks, cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
@@ -276,7 +321,8 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
                                it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
-                               it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2)) {
+                               it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
+                               it->second.pblocks != pblocks)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -284,7 +330,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, pblocks, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -321,7 +367,7 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
   }
   c->cheb = k;
   c->cheb_inv_theta = 1.0 / theta;
-  c->cz = w.cz; c->cd[0] = w.cd0; c->cd[1] = w.cd1; c->crc = w.crc;
+  c->cz = w.cz; c->cd[0] = w.cd0; c->cd[1] = w.cd1; c->cd[2] = w.cd2; c->cd[3] = w.cd3; c->crc = w.crc;
   c->jacobi = 0;
   c->precision = opts->precision;
 }
@@ -403,7 +449,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   cudaGraphExec_t ex;
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
                  cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0,
-                 (use_zmarch(L) && fused_x2(L)) ? 1 : 0, &ex);
+                 (use_zmarch(L) && fused_x2(L)) ? 1 : 0,
+                 (cheb && cheb_pairs(L, cheb_code(opts))) ? cheb_pair_blocks(L) : 0, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -545,9 +592,14 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
     case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
       const int code = kernel_id - 6;
       const bool x2 = code != 0 && cheb_x2(L);
-      Ctx* ctxp = w.ctx; int step = 1;
-      void* args[] = {&ctxp, &step};
+      Ctx* ctxp = w.ctx; int step = 1, old = 1, cur = 0;
+      void* args[] = {&ctxp, &step, &old, &cur};
       CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : cheb_blocks(L)), dim3(kThreads), args, 0, st));
+    } break;
+    case 9: case 10: {            // one fused pair of Chebyshev passes, fp32 on A2 / on A3
+      Ctx* ctxp = w.ctx; int step = 1, old = 1, cur = 0, wo = 2, yo = 3;
+      void* args[] = {&ctxp, &step, &old, &cur, &wo, &yo};
+      CU(cudaLaunchKernel(cheb_pair_fn(kernel_id == 10 ? 2 : 1), dim3(cheb_pair_blocks(L)), dim3(kThreads), args, 0, st));
     } break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
@@ -624,14 +676,19 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   { void* a[] = {&ctxp};
     CU(cudaLaunchKernel(cheb_first_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
-  for (int i = 1; i <= k - 3; ++i) {
-    int step = i;
-    void* a[] = {&ctxp, &step};
-    CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : sb), dim3(kThreads), a, 0, st));
+  for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code))) {
+    int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
+    if (op.kind == 1) {
+      void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
+      CU(cudaLaunchKernel(cheb_pair_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st));
+    } else if (op.kind == 0) {
+      void* a[] = {&ctxp, &step, &old, &cur};
+      CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : sb), dim3(kThreads), a, 0, st));
+    } else {
+      void* a[] = {&ctxp, &ctlp, &part, &step, &old, &cur};
+      CU(cudaLaunchKernel(cheb_last_fn(code), dim3(sb), dim3(kThreads), a, 0, st));
+    }
   }
-  { int step = k - 2;
-    void* a[] = {&ctxp, &ctlp, &part, &step};
-    CU(cudaLaunchKernel(cheb_last_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
   (void)blocks;
   CU(cudaGetLastError());
   return CUTH_OK;
@@ -641,6 +698,12 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
   if (!alpha_H || !out_H || (m > 1 && !beta_H)) return CUTH_ERR_NULL;
   if (m < 1) return CUTH_ERR_VALUE;
   tridiag_extremes(alpha_H, beta_H, m, &out_H[0], &out_H[1]);
+  return CUTH_OK;
+}
+
+int cuth_set_cheb_fusion(int mode) {
+  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
+  g_cheb_pairs.store(mode);
   return CUTH_OK;
 }
 

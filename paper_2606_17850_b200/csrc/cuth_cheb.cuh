@@ -146,8 +146,9 @@ __device__ __forceinline__ void apply_A_t(const DiaDev& A, const VT* __restrict_
 // the same k-1 stencil passes, but a pass now reads Z_{i+1} (stencil), Z_i and r at its own cell and writes
 // Z_{i+2} over Z_i (in place: only the own cell of Z_i is ever read): M + 4s bytes per row instead of M + 6s
 // (s = sizeof(T)), and the residual is formed directly instead of by recurrence.  Two buffers Z[0], Z[1]
-// (Ctx.cd): at pass i the stencil input is Z[(i+1)&1], the old iterate / output is Z[i&1].  In fp32 mode the
-// first pass also leaves an fp32 copy of r (Ctx.crc) for the later passes.
+// (Ctx.cd), named by the `old` / `cur` kernel arguments: the stencil input is Z[cur], the old iterate / output is
+// Z[old]; the host schedule (cheb_schedule) swaps them after every pass.  In fp32 mode the first pass also
+// leaves an fp32 copy of r (Ctx.crc) for the later passes.
 //
 // First pass (i = 0): Z_1 = r/theta formed on the fly (A Z_1 = (A r)/theta), Z_2 = Z_1 + c1_0 Z_1 + c2_0 (r - A Z_1).
 template <class T, class M>
@@ -168,11 +169,12 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
 
 // Passes 0 < i < k-2.
 template <class T, class M>
-__global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step) {
+__global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 4) k_cheb_mid(const Ctx* __restrict__ ctxp, int step,
+                                                                                              int old, int cur) {
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
-  const T* __restrict__ zcur = (const T*)ctxp->cd[(step + 1) & 1];
-  T* __restrict__ zold = (T*)ctxp->cd[step & 1];
+  const T* __restrict__ zcur = (const T*)ctxp->cd[cur];
+  T* __restrict__ zold = (T*)ctxp->cd[old];
   const T* __restrict__ r32 = (const T*)c.crc;
   apply_A_t<T, T, M>(c.A, zcur, [&](int64_t i, T zi, T Az) {
     const T ri = sizeof(T) == 4 ? r32[i] : (T)c.r[i];
@@ -186,12 +188,12 @@ __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? CUTH_CHEB_MINB32 : 
 // 4-byte version is latency-bound (profiles/r1c_cfg3_cheb_mixed.md).  Matrix entries stay scalar loads: the
 // packed diagonals D2, D3 start at odd elements (R-G5b).  Tile = (2 ZTX) x ZTY columns per CTA.
 template <class M>
-__global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __restrict__ ctxp, int step) {
+__global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __restrict__ ctxp, int step, int old, int cur) {
   const Ctx c = *ctxp;
   const DiaDev& A = c.A;
   const float c1 = (float)ctxp->cheb_c1[step], c2 = (float)ctxp->cheb_c2[step];
-  const float* __restrict__ din = (const float*)ctxp->cd[(step + 1) & 1];     // Z_{i+1}: stencil input
-  float* __restrict__ zold = (float*)ctxp->cd[step & 1];                      // Z_i in, Z_{i+2} out (in place)
+  const float* __restrict__ din = (const float*)ctxp->cd[cur];                // Z_{i+1}: stencil input
+  float* __restrict__ zold = (float*)ctxp->cd[old];                           // Z_i in, Z_{i+2} out (in place)
   const float* __restrict__ r32 = (const float*)c.crc;
   const int tx = threadIdx.x % ZTX, ty = threadIdx.x / ZTX;
   const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
@@ -240,13 +242,13 @@ __global__ void __launch_bounds__(kThreads, 6) k_cheb_mid_f32x2(const Ctx* __res
 // Last pass (i = k-2): z = Z_k in fp64 for the outer loop, and rho = r.z (Alg. 1 lines 10-11).
 template <class T, class M>
 __global__ void __launch_bounds__(kThreads, sizeof(T) == 4 ? 6 : 4) k_cheb_last(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
-                                                        int step) {
+                                                        int step, int old, int cur) {
   __shared__ double smem[32];
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   const T c1 = (T)ctxp->cheb_c1[step], c2 = (T)ctxp->cheb_c2[step];
-  const T* __restrict__ zcur = (const T*)ctxp->cd[(step + 1) & 1];
-  const T* __restrict__ zold = (const T*)ctxp->cd[step & 1];
+  const T* __restrict__ zcur = (const T*)ctxp->cd[cur];
+  const T* __restrict__ zold = (const T*)ctxp->cd[old];
   double acc[1] = {0.0};
   apply_A_t<T, T, M>(c.A, zcur, [&](int64_t i, T zi, T Az) {
     const double rd = c.r[i];

@@ -84,9 +84,10 @@ struct Ctx {
   int32_t precision, max_iters, period, jacobi;
   int32_t soft_restart, cheb;     // cheb: degree k of the Chebyshev polynomial preconditioner, 0 = off
   // Chebyshev preconditioner (Alg. 3): z = q(A) r.  cz: z (fp64) handed to the outer
-  // loop; cd[2]: the two partial-sum buffers Z; crc: fp32 copy of r (MIXED only).  Element type T = double
-  // in FP64 mode, float in MIXED mode; buffers are sized for double.
-  double* cz; void* cd[2]; void* crc;
+  // loop; cd[4]: partial-sum buffers Z (two are live at any time; the fused two-pass kernel writes the other
+  // two); crc: fp32 copy of r (MIXED only).  Element type T = double in FP64 mode, float in MIXED mode;
+  // cd[0], cd[1] are sized for double, cd[2], cd[3] for float (the two-pass kernel is fp32 only).
+  double* cz; void* cd[4]; void* crc;
   double cheb_inv_theta;
   double cheb_c1[kMaxChebDegree], cheb_c2[kMaxChebDegree];   // d_{i+1} = c1[i] d_i + c2[i] r_c
 };
@@ -103,7 +104,7 @@ struct Ctl {
 
 struct Workspace {
   Ctx* ctx; Ctl* ctl; double* partials; double* r; double* p; double* p2; double* mu; double* b;
-  double* cz; double* cd0; double* cd1; double* crc;
+  double* cz; double* cd0; double* cd1; double* crc; float* cd2; float* cd3;
   size_t bytes;
 };
 
@@ -121,9 +122,12 @@ inline Workspace carve_workspace(void* base, int64_t n, bool with_b, bool with_c
   w.b = nullptr;
   if (with_b) { w.b = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
   w.cz = w.cd0 = w.cd1 = w.crc = nullptr;
+  w.cd2 = w.cd3 = nullptr;
   if (with_cheb) {
     double** v[4] = {&w.cz, &w.cd0, &w.cd1, &w.crc};
     for (int k = 0; k < 4; ++k) { *v[k] = (double*)(c + o); o = align_up(o + sizeof(double) * (size_t)n); }
+    w.cd2 = (float*)(c + o); o = align_up(o + sizeof(float) * (size_t)n);
+    w.cd3 = (float*)(c + o); o = align_up(o + sizeof(float) * (size_t)n);
   }
   w.bytes = o;
   return w;

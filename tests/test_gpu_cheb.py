@@ -19,14 +19,17 @@ CASES = [
 ]
 
 
-@pytest.fixture(params=["flat", "zmarch", "zmarch-x1"], autouse=True)
+@pytest.fixture(params=["flat", "flat-pairs", "zmarch", "zmarch-x1"], autouse=True)
 def traversal(request):
     import paper_2606_17850_b200 as cu
-    cu.cuth_set_traversal(1 if request.param == "flat" else 2)
+    cu.cuth_set_traversal(1 if request.param.startswith("flat") else 2)
+    # pairs: "flat" = one pass per kernel, "flat-pairs" and "zmarch" = fused pairs, "zmarch-x1" = single passes
+    cu.cuth_set_cheb_fusion({"flat": 1, "flat-pairs": 2, "zmarch": 2, "zmarch-x1": 1}[request.param])
     cu.cuth_set_k1_variant(1 if request.param == "zmarch-x1" else 2)       # 2: two columns per thread when nx is even
     yield request.param
     cu.cuth_set_traversal(0)
     cu.cuth_set_k1_variant(0)
+    cu.cuth_set_cheb_fusion(0)
 
 
 def _rhs(w):
