@@ -31,9 +31,8 @@ import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
-NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.4477e9,   # profiles/r1e (two-column K1)
-                     ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 12.055e9,     # profiles/r1d_cfg4_fp64.md
-                     }
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3114e9,   # profiles/r1f_cfg3_fp64_k1_nodinv.md
+                     }     # cfg 4: profiles/r1d predates the K1 that no longer reads 1/D0 -> null until recaptured
 
 METRIC = "pcg_time_to_solution"
 UNIT = "s"
@@ -54,8 +53,10 @@ def m_ratio(w):
 def bytes_per_row(w, what):
     """Algorithmic bytes per matrix row."""
     m = m_ratio(w)
+    # the fused K1 takes M = diag A from the D0 its SpMV reads (fp64 operator), so a fused fp64 iteration
+    # moves 8m + 80, not the 8m + 88 of the three-kernel path (which reads 1/D0 in k_pupdate)
     return {"spmv_fp64": 8 * m + 16, "spmv_mixed": 4 * (m - 1) + 16,
-            "iter_fp64": 8 * m + 88, "iter_mixed": 4 * (m - 1) + 88}[what]
+            "iter_fp64": 8 * m + 88, "iter_fp64_fused": 8 * m + 80, "iter_mixed": 4 * (m - 1) + 88}[what]
 
 
 def max_over_ranks(value_ms: float, world: int, device="cpu") -> float:
@@ -116,6 +117,11 @@ class ClockSampler:
         return out
 
 
+# Alg.-1 (Jacobi) iteration counts of the six workloads at their rtol, as the fp64 path of this repo measures
+# them on B200; what a window of oracle iterations is extrapolated to.
+NOMINAL_JACOBI_ITERS = {1: 288, 2: 1462, 3: 4500, 4: 9791, 5: 580, 6: 1500}
+
+
 def cpu_oracle_sample(w, iters_for_extrapolation, budget_iters=None, out=None):
     """Times the oracle (as it stands) on a bounded sample: a window of Alg.-1 iterations on the same
     workload, extrapolated to the iteration count the solve needs."""
@@ -149,7 +155,7 @@ def run_reference(args):
     A = O.assemble_workload(w)
     b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
     iters = int(max(3, min(200, 2.5e8 / w.n)))
-    nominal = {1: 288, 2: 1462, 3: 4500, 4: 9791, 5: 580, 6: 1500}[args.config]
+    nominal = NOMINAL_JACOBI_ITERS[args.config]
     for _ in range(args.warmup):
         O.pcg_window(A, b, np.zeros(w.n), 1)
     t0 = time.time()
@@ -359,7 +365,8 @@ def main():
     it = total_its
     early = int(early_acc.item()) if mixed else 0
     late = it - early
-    iter_bytes = (early * bytes_per_row(w, "iter_mixed") + late * bytes_per_row(w, "iter_fp64")) * w.n
+    iter_bytes = (early * bytes_per_row(w, "iter_mixed")
+                  + late * bytes_per_row(w, "iter_fp64_fused" if fused else "iter_fp64")) * w.n
     m = m_ratio(w)
     if cheb:
         # outer: K1 (matrix + z, p, x read + p', mu, x written) + K2 (r, mu read, r written); preconditioner:
@@ -368,14 +375,14 @@ def main():
         k, sT = args.cheb_degree, (4 if mixed else 8)
         Mc = (2 * (m - 1) if h16 else 4 * (m - 1)) if mixed else 8 * m
         apply_bytes = (k - 1) * Mc + ((3 if mixed else 2) * sT + 8) + (k - 3) * 4 * sT + (2 * sT + 16)
-        outer = lambda M_: M_ + 48 + 24
+        outer = lambda M_: M_ + 48 + 24          # no 1/D0 anywhere: z = q(A) r is a stored vector
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
     stage_fp64 = (not mixed) or res.promotions > 0     # operator the armed profile kernels ran with
     m = m_ratio(w)
-    if fused:      # K1: matrix + r, 1/D0, p, x read + p', mu, x written
+    if fused:      # K1: matrix + r, p, x read + p', mu, x written (+ 1/D0 read with the fp32-stored operator)
         dom_name, dom_ms = "k_fused_pspmv", kern["k_fused_pspmv"]
-        dom_bytes = ((8 * m if stage_fp64 else 4 * (m - 1)) + 56) * w.n
+        dom_bytes = ((8 * m + 48) if stage_fp64 else (4 * (m - 1) + 56)) * w.n
     else:
         dom_name, dom_ms = "k_spmv_dot", kern["k_spmv_dot"]
         dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
@@ -417,7 +424,7 @@ def main():
                                "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
                                "algorithmic_bytes_per_solve": iter_bytes,
                                "note": ("Chebyshev: outer K1+K2 plus (k-1)-kernel apply bytes per row per iteration " if cheb else "") +
-                                       "floor bytes (8m+88 fp64 / 4(m-1)+88 fp32-stored per row per iteration) "
+                                       "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
         "loop": "persistent cooperative kernel" if persistent else "cuda graph (conditional WHILE/IF nodes)",
@@ -427,7 +434,10 @@ def main():
     }
     if not args.no_cpu_baseline and world == 1:
         keep = {}
-        line["cpu_baseline"] = cpu_oracle_sample(w, it, out=keep)
+        # the oracle timed is Alg. 1 with Jacobi; a Chebyshev-preconditioned run is compared with the Jacobi
+        # iteration count of the same workload, not with its own (31 SpMVs each) count
+        cpu_its = NOMINAL_JACOBI_ITERS[args.config] if cheb else it
+        line["cpu_baseline"] = cpu_oracle_sample(w, cpu_its, out=keep)
         if not w.transient:
             # property check of the timed result against the ORACLE's matrix (not timed)
             from oracle import oracle as O

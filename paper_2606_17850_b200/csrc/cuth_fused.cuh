@@ -5,9 +5,10 @@
 //                        mu = A p', p'.mu       (Alg. 1 line 6 and the denominator of line 7)
 //   K2 = k_fused_update: r -= alpha mu, z = M^-1 r, r.z, ||r||^2   (lines 9-11)
 //
-// Algorithmic traffic per row and iteration: K1 = E/N matrix elements + r, 1/D0, p, x read +
-// p', mu, x written (8m + 56 B in fp64), K2 = r, mu, 1/D0 read + r written (32 B): 8m + 88 B, the
-// floor of SURVEY.md §8(d).
+// Algorithmic traffic per row and iteration, fp64 operator: K1 = E/N matrix elements + r, p, x read +
+// p', mu, x written (8m + 48 B; M^-1 comes from the D0 the SpMV reads anyway, one plane early), K2 = r, mu,
+// 1/D0 read + r written (32 B): 8m + 80 B, 8 B below the 8m + 88 floor SURVEY.md §8(d) counts.  fp32-stored
+// operator (early stage): D0 is not part of it, K1 reads 1/D0: 4(m-1) + 56 + 32 B.
 //
 // K1 walks the grid like zmarch_apply (a CTA owns a TX x TY tile of the x-y plane, a thread owns one
 // column and marches in z), but the vector it multiplies is produced on the fly: each thread forms
@@ -25,6 +26,17 @@ constexpr int FTX = 32, FTY = 8;     // FTX * FTY == kThreads
 static_assert(FTX * FTY == kThreads, "tile must match the block size");
 constexpr int kHalo = 2 * FTX + 2 * FTY;
 constexpr int kHaloPerWarp = (kHalo + kThreads / 32 - 1) / (kThreads / 32);
+
+// 1 / d for a positive normal d (a main-diagonal entry, R-G2), to within an ulp: hardware seed (>= 20 bits)
+// and two Newton steps; no special cases, hence no slow-path call and no extra registers.
+__device__ __forceinline__ double rcp_diag(double d) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  double e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-d, y, 1.0);
+  return fma(y, e, y);
+}
 
 template <bool MIXED>
 __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __restrict__ p_in,
@@ -61,17 +73,22 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
 
     __syncthreads();                       // previous tile's planes are dead
     double pn_lo = 0.0, pn_c = 0.0, a3l = 0.0;
+    double dnx = 1.0;                      // fp64 operator: D0 of the plane p' is being formed for (M, then SpMV)
     {   // plane 0 of p'
       double ro = 0.0, dio = 1.0, po = 0.0, xo = 0.0, rh = 0.0, dih = 1.0, ph = 0.0;
-      if (own) { ro = zs[col]; po = p_in[col]; if (jac) dio = A.dinv[col]; if (do_x) xo = c.x[col]; }
-      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = A.dinv[hcol]; }
       if (own) {
-        pn_c = fma(beta, po, ro * dio);
+        ro = zs[col]; po = p_in[col];
+        if (MIXED) { if (jac) dio = A.dinv[col]; } else { dnx = A.d0[col]; }
+        if (do_x) xo = c.x[col];
+      }
+      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? A.dinv[hcol] : A.d0[hcol]; }
+      if (own) {
+        pn_c = fma(beta, po, MIXED ? ro * dio : (jac ? ro * rcp_diag(dnx) : ro));
         p_out[col] = pn_c;
         if (do_x) c.x[col] = fma(xalpha, po, xo);
       }
       sp[0][ty + 1][tx + 1] = pn_c;
-      if (halo_role) sp[0][hr][hc] = halo_in ? fma(beta, ph, rh * dih) : 0.0;
+      if (halo_role) sp[0][hr][hc] = halo_in ? fma(beta, ph, MIXED ? rh * dih : rh * rcp_diag(dih)) : 0.0;
     }
 
     for (int z = 0; z < nz; ++z) {
@@ -85,7 +102,7 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
       if (own) {
         const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx;
         if (!MIXED) {
-          a0 = A.d0[i];
+          a0 = dnx;                                // loaded during the previous step
           a1u = up1 ? A.d1[i] : 0.0;  a1l = lo1 ? A.d1[i - 1] : 0.0;
           a2u = up2 ? A.d2[i] : 0.0;  a2l = lo2 ? A.d2[i - nx] : 0.0;
           a3u = up3 ? A.d3[i] : 0.0;
@@ -97,14 +114,14 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
         if (up3) {
           const int64_t j = i + np;
           ro = zs[j]; po = p_in[j];
-          if (jac) dio = A.dinv[j];
+          if (MIXED) { if (jac) dio = A.dinv[j]; } else { dnx = A.d0[j]; }
           if (do_x) xo = c.x[j];
         }
       }
       if (up3 && halo_in) {
         const int64_t j = hcol + (int64_t)(z + 1) * np;
         rh = zs[j]; ph = p_in[j];
-        if (jac) dih = A.dinv[j];
+        if (jac) dih = MIXED ? A.dinv[j] : A.d0[j];
       }
       // ---- 2. plane z of p' (written during the previous step) is complete; the loads above fly
       //         while the CTA waits here
@@ -113,12 +130,12 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
       double pn_hi = 0.0;
       if (up3) {
         if (own) {
-          pn_hi = fma(beta, po, ro * dio);
+          pn_hi = fma(beta, po, MIXED ? ro * dio : (jac ? ro * rcp_diag(dnx) : ro));
           p_out[i + np] = pn_hi;
           if (do_x) c.x[i + np] = fma(xalpha, po, xo);
         }
         sp[nxt][ty + 1][tx + 1] = pn_hi;
-        if (halo_role) sp[nxt][hr][hc] = halo_in ? fma(beta, ph, rh * dih) : 0.0;
+        if (halo_role) sp[nxt][hr][hc] = halo_in ? fma(beta, ph, MIXED ? rh * dih : rh * rcp_diag(dih)) : 0.0;
       }
       // ---- 4. row i of mu = A p'
       if (own) {

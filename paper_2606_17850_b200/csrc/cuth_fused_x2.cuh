@@ -53,18 +53,28 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
 
     __syncthreads();                              // previous tile's planes are dead
     double pc0 = 0.0, pc1 = 0.0, pl0 = 0.0, pl1 = 0.0, a3l0 = 0.0, a3l1 = 0.0;
+    // fp64 operator: the main diagonal of plane z+1 is loaded one step early and serves twice, as M = diag A
+    // of Alg. 1 line 10 (z = r / D0 as r * rcp(D0), rcp to within an ulp like the stored 1/D0) and then as the D0 term of the SpMV;
+    // 1/D0 is not read at all (8 B/row less).  fp32-stored operator: D0 is not part of it, 1/D0 is read.
+    double2 dnx = make_double2(1.0, 1.0);           // D0 of the plane p' is being formed for
     {   // plane 0 of p'
       double2 ro = make_double2(0.0, 0.0), po = ro, xo = ro, dio = make_double2(1.0, 1.0);
       double rh = 0.0, dih = 1.0, ph = 0.0;
-      if (own) { ro = ldd2(zs + col); po = ldd2(p_in + col); if (jac) dio = ldd2(A.dinv + col); if (do_x) xo = ldd2(c.x + col); }
-      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = A.dinv[hcol]; }
       if (own) {
-        pc0 = fma(beta, po.x, ro.x * dio.x); pc1 = fma(beta, po.y, ro.y * dio.y);
+        ro = ldd2(zs + col); po = ldd2(p_in + col);
+        if (MIXED) { if (jac) dio = ldd2(A.dinv + col); } else { dnx = ldd2(A.d0 + col); }
+        if (do_x) xo = ldd2(c.x + col);
+      }
+      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? A.dinv[hcol] : A.d0[hcol]; }
+      if (own) {
+        const double z0 = MIXED ? ro.x * dio.x : (jac ? ro.x * rcp_diag(dnx.x) : ro.x);
+        const double z1 = MIXED ? ro.y * dio.y : (jac ? ro.y * rcp_diag(dnx.y) : ro.y);
+        pc0 = fma(beta, po.x, z0); pc1 = fma(beta, po.y, z1);
         std2(p_out + col, pc0, pc1);
         if (do_x) std2(c.x + col, fma(xalpha, po.x, xo.x), fma(xalpha, po.y, xo.y));
       }
       std2(&sp[0][ty + 1][sc0], pc0, pc1);
-      if (halo_role) sp[0][hr][hc] = halo_in ? fma(beta, ph, rh * dih) : 0.0;
+      if (halo_role) sp[0][hr][hc] = halo_in ? fma(beta, ph, MIXED ? rh * dih : rh * rcp_diag(dih)) : 0.0;
     }
 
     for (int z = 0; z < nz; ++z) {
@@ -79,8 +89,7 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
       if (own) {
         const bool up1 = i + 2 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx;   // the pair shares up2 / lo2
         if (!MIXED) {
-          const double2 d0 = ldd2(A.d0 + i);
-          a00 = d0.x; a01 = d0.y;
+          a00 = dnx.x; a01 = dnx.y;               // loaded during the previous step
           if (up1) { const double2 d1 = ldd2(A.d1 + i); a1a = d1.x; a1b = d1.y; } else { a1a = A.d1[i]; }
           a1l = lo1 ? A.d1[i - 1] : 0.0;
           if (up2) { a2u0 = A.d2[i]; a2u1 = A.d2[i + 1]; }
@@ -97,14 +106,14 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
         if (up3) {
           const int64_t j = i + np;
           ro = ldd2(zs + j); po = ldd2(p_in + j);
-          if (jac) dio = ldd2(A.dinv + j);
+          if (MIXED) { if (jac) dio = ldd2(A.dinv + j); } else { dnx = ldd2(A.d0 + j); }
           if (do_x) xo = ldd2(c.x + j);
         }
       }
       if (up3 && halo_in) {
         const int64_t j = hcol + (int64_t)(z + 1) * np;
         rh = zs[j]; ph = p_in[j];
-        if (jac) dih = A.dinv[j];
+        if (jac) dih = MIXED ? A.dinv[j] : A.d0[j];
       }
       // ---- 2. plane z of p' is complete (written during the previous step); the loads fly meanwhile
       __syncthreads();
@@ -112,12 +121,14 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
       double ph0 = 0.0, ph1 = 0.0;
       if (up3) {
         if (own) {
-          ph0 = fma(beta, po.x, ro.x * dio.x); ph1 = fma(beta, po.y, ro.y * dio.y);
+          const double z0 = MIXED ? ro.x * dio.x : (jac ? ro.x * rcp_diag(dnx.x) : ro.x);
+          const double z1 = MIXED ? ro.y * dio.y : (jac ? ro.y * rcp_diag(dnx.y) : ro.y);
+          ph0 = fma(beta, po.x, z0); ph1 = fma(beta, po.y, z1);
           std2(p_out + i + np, ph0, ph1);
           if (do_x) std2(c.x + i + np, fma(xalpha, po.x, xo.x), fma(xalpha, po.y, xo.y));
         }
         std2(&sp[nxt][ty + 1][sc0], ph0, ph1);
-        if (halo_role) sp[nxt][hr][hc] = halo_in ? fma(beta, ph, rh * dih) : 0.0;
+        if (halo_role) sp[nxt][hr][hc] = halo_in ? fma(beta, ph, MIXED ? rh * dih : rh * rcp_diag(dih)) : 0.0;
       }
       // ---- 4. rows i, i+1 of mu = A p'
       if (own) {
