@@ -193,6 +193,8 @@ def main():
     ap.add_argument("--cheb-storage", default="fp32", choices=["fp32", "fp16"],
                     help="MIXED Chebyshev: matrix copy the preconditioner reads (A2 fp32 / A3 fp16, Alg. 4)")
     ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
+    ap.add_argument("--cheb-fusion", type=int, default=0, choices=[0, 1, 2],
+                    help="cuth_set_cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,
@@ -216,6 +218,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cu.cuth_set_traversal(args.traversal)
+    cu.cuth_set_cheb_fusion(args.cheb_fusion)
     w = W.make_workload(args.config)
     mixed = w.mixed if args.precision is None else (args.precision == "mixed")
     prec = cu.MIXED if mixed else cu.FP64
@@ -326,6 +329,8 @@ def main():
         cid = 8 if h16 else (7 if mixed else 6)
         names[cid] = "k_cheb_mid"
         body_ids = tuple([cid] * (args.cheb_degree - 1)) + body_ids
+        if mixed and w.nx % 2 == 0:
+            names[10 if h16 else 9] = "k_cheb_pair"      # two passes per launch (cuth_set_cheb_fusion)
     for kid, nm in names.items():
         for _ in range(3):
             cu.cuth_profile_kernel(S.work, g, kid)

@@ -178,10 +178,10 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
 
-/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes).  0 = automatic (today: one pass per
- * kernel), 1 = one pass per kernel, 2 = two consecutive passes per kernel (k_cheb_pair_f32: 43 % fewer HBM
- * bytes, correct and parity-tested, but measured ~2x slower than two single passes on B200 -- experimental).
- * The polynomial is the same. */
+/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic (two
+ * consecutive passes per kernel, k_cheb_pair_f32, on the large planes where the single passes run two columns
+ * per thread), 1 = one pass per kernel, 2 = pairs wherever nx is even.  The polynomial is the same, and so is
+ * the arithmetic of every row. */
 int cuth_set_cheb_fusion(int mode);
 
 /* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle

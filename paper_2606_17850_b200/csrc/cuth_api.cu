@@ -155,17 +155,15 @@ static void* cheb_pair_fn(int code) {
 }
 static std::atomic<int> g_cheb_pairs{0};   // 0 auto, 1 never, 2 always (fp32 modes): cuth_set_cheb_fusion
 static int cheb_pair_blocks(const DiaLayout& L) {
-  const int64_t tiles = ((L.nx + PTX - 1) / PTX) * ((L.ny + PTY - 1) / PTY);
+  const int64_t tiles = ((L.nx + QIX - 1) / QIX) * ((L.ny + QIY - 1) / QIY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 static bool cheb_pairs(const DiaLayout& L, int code) {
   const int mode = g_cheb_pairs.load();
-  if (code == 0 || mode == 1) return false;          // fp32 arithmetic only
-  // Measured (cfg 3 / cfg 4, B200): the straightforward two-pass kernel moves 43 % fewer HBM bytes but is
-  // latency-bound (three barrier-separated phases per plane, scalar loads, 3 CTAs/SM): 20.3 s vs 10.8 s at cfg 4.
-  // Until its phases are software-pipelined it stays an opt-in (mode 2); automatic = single passes.
-  (void)L;
-  return mode == 2;
+  if (code == 0 || mode == 1 || (L.nx & 1)) return false;     // fp32 arithmetic, column pairs: nx even
+  // automatic: wherever the single passes run two columns per thread (large planes); measured cfg 3 0.92 ->
+  // 0.79 s, cfg 4 10.8 -> 10.1 s
+  return mode == 2 || cheb_x2(L);
 }
 static void* cheb_last_fn(int code) {
   return code == 0 ? (void*)k_cheb_last<double, MatF32> : code == 1 ? (void*)k_cheb_last<float, MatF32>

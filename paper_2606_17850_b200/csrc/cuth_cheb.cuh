@@ -30,6 +30,13 @@ struct MatF32 {
   static __device__ __forceinline__ float e1(const DiaDev& A, int64_t i, float) { return A.f1[i]; }
   static __device__ __forceinline__ float e2(const DiaDev& A, int64_t i, float) { return A.f2[i]; }
   static __device__ __forceinline__ float e3(const DiaDev& A, int64_t i, float) { return A.f3[i]; }
+  // pointer form (kernels that walk a column bump one pointer per diagonal instead of re-deriving indices)
+  using elem = float;
+  static __device__ __forceinline__ const elem* d1(const DiaDev& A) { return A.f1; }
+  static __device__ __forceinline__ const elem* d2(const DiaDev& A) { return A.f2; }
+  static __device__ __forceinline__ const elem* d3(const DiaDev& A) { return A.f3; }
+  static __device__ __forceinline__ float ld(const elem* p, float) { return *p; }
+  static __device__ __forceinline__ float2 ldp(const elem* p, float) { return make_float2(p[0], p[1]); }
 };
 struct MatF16 {
   // the three fp16 arrays are this library's own 256-B aligned copies, so an even index is a 4-byte
@@ -45,6 +52,15 @@ struct MatF16 {
   static __device__ __forceinline__ float e1(const DiaDev& A, int64_t i, float s) { return __half2float(A.h1[i]) * s; }
   static __device__ __forceinline__ float e2(const DiaDev& A, int64_t i, float s) { return __half2float(A.h2[i]) * s; }
   static __device__ __forceinline__ float e3(const DiaDev& A, int64_t i, float s) { return __half2float(A.h3[i]) * s; }
+  using elem = __half;
+  static __device__ __forceinline__ const elem* d1(const DiaDev& A) { return A.h1; }
+  static __device__ __forceinline__ const elem* d2(const DiaDev& A) { return A.h2; }
+  static __device__ __forceinline__ const elem* d3(const DiaDev& A) { return A.h3; }
+  static __device__ __forceinline__ float ld(const elem* p, float s) { return __half2float(*p) * s; }
+  static __device__ __forceinline__ float2 ldp(const elem* p, float s) {          // p at an even element
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(p));
+    return make_float2(f.x * s, f.y * s);
+  }
 };
 
 // One row of A v with v stored as VT and arithmetic in T (T = double: A1 standard form; T = float: A2
