@@ -32,7 +32,7 @@ constexpr int QIX = QX - 4, QIY = QY - 2;              // interior written by th
 static_assert(QX / 2 * QY == kThreads, "one thread per column pair of the region");
 
 template <class M>
-__global__ void __launch_bounds__(kThreads, 3) k_cheb_pair_f32(const Ctx* __restrict__ ctxp, int step, int old, int cur,
+__global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_f32(const Ctx* __restrict__ ctxp, int step, int old, int cur,
                                                              int wout, int yout) {
   __shared__ __align__(8) float sW[2][QY][QX];
   const Ctx c = *ctxp;
