@@ -113,7 +113,10 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   const double* lay = (const double*)(base + L.o_layers);
   DiaDev A;
   A.d0 = v + L.ptr[0]; A.d1 = v + L.ptr[1]; A.d2 = v + L.ptr[2]; A.d3 = v + L.ptr[3];
-  A.f0 = f + L.ptr[0]; A.f1 = f + L.ptr[1]; A.f2 = f + L.ptr[2]; A.f3 = f + L.ptr[3];
+  A.f0 = f + L.ptr[0];
+  A.f1 = (const float*)(base + L.o_f32a);
+  A.f2 = (const float*)(base + L.o_f32a + L.f32a_stride);
+  A.f3 = (const float*)(base + L.o_f32a + 2 * L.f32a_stride);
   A.dinv = (const double*)(base + L.o_dinv);
   A.h1 = (const __half*)(base + L.o_h16);
   A.h2 = (const __half*)(base + L.o_h16 + L.h16_stride);

@@ -88,6 +88,17 @@ __global__ void __launch_bounds__(256) k_make_h16(BuildArgs a, const double* slo
   }
 }
 
+// The off-diagonals of A2 once more, one 256-B aligned array of n floats per diagonal (zero beyond the
+// diagonal's length): what the solver kernels read.  The packed fp32 copy stays what cuth_dia_view shows.
+__global__ void __launch_bounds__(256) k_make_f32a(BuildArgs a, float* g1, float* g2, float* g3) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+    g1[i] = i + 1 < a.n ? a.f1[i] : 0.f;
+    g2[i] = i + a.nx < a.n ? a.f2[i] : 0.f;
+    g3[i] = i + a.nxny < a.n ? a.f3[i] : 0.f;
+  }
+}
+
 // Host side: fills the per-layer arrays, launches the kernel.  Called from cuth_api.cu.
 int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStream_t st, cudaError_t* err) {
   char* base = (char*)dia_D;
@@ -137,6 +148,8 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   k_make_h16<<<(unsigned)blocks, 256, 0, st>>>(a, slot, (__half*)(base + L.o_h16),
                                                (__half*)(base + L.o_h16 + L.h16_stride),
                                                (__half*)(base + L.o_h16 + 2 * L.h16_stride));
+  k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(a, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
+                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride));
   e = cudaGetLastError();
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   return CUTH_OK;

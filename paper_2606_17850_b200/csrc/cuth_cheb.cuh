@@ -22,10 +22,10 @@ namespace cuth {
 // Where the fp32-arithmetic operator takes its off-diagonal entries from: A2 (fp32) or A3 (fp16
 // times a power-of-two scale, promoted to fp32 on load: "arithmetic decoupling", Alg. 4).
 struct MatF32 {
-  // the packed A2 diagonals D2, D3 start at odd elements (R-G5b): pairs are two scalar loads
-  static __device__ __forceinline__ float2 p1(const DiaDev& A, int64_t i, float) { return make_float2(A.f1[i], A.f1[i + 1]); }
-  static __device__ __forceinline__ float2 p2(const DiaDev& A, int64_t i, float) { return make_float2(A.f2[i], A.f2[i + 1]); }
-  static __device__ __forceinline__ float2 p3(const DiaDev& A, int64_t i, float) { return make_float2(A.f3[i], A.f3[i + 1]); }
+  // f1..f3 are the aligned per-diagonal copies: an even index is an 8-byte aligned pair, one load
+  static __device__ __forceinline__ float2 p1(const DiaDev& A, int64_t i, float) { return *reinterpret_cast<const float2*>(A.f1 + i); }
+  static __device__ __forceinline__ float2 p2(const DiaDev& A, int64_t i, float) { return *reinterpret_cast<const float2*>(A.f2 + i); }
+  static __device__ __forceinline__ float2 p3(const DiaDev& A, int64_t i, float) { return *reinterpret_cast<const float2*>(A.f3 + i); }
   static __device__ __forceinline__ float inv(const DiaDev&) { return 1.f; }
   static __device__ __forceinline__ float e1(const DiaDev& A, int64_t i, float) { return A.f1[i]; }
   static __device__ __forceinline__ float e2(const DiaDev& A, int64_t i, float) { return A.f2[i]; }
@@ -36,7 +36,7 @@ struct MatF32 {
   static __device__ __forceinline__ const elem* d2(const DiaDev& A) { return A.f2; }
   static __device__ __forceinline__ const elem* d3(const DiaDev& A) { return A.f3; }
   static __device__ __forceinline__ float ld(const elem* p, float) { return *p; }
-  static __device__ __forceinline__ float2 ldp(const elem* p, float) { return make_float2(p[0], p[1]); }
+  static __device__ __forceinline__ float2 ldp(const elem* p, float) { return *reinterpret_cast<const float2*>(p); }   // p at an even element
 };
 struct MatF16 {
   // the three fp16 arrays are this library's own 256-B aligned copies, so an even index is a 4-byte

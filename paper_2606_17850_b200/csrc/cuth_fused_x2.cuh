@@ -99,9 +99,10 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
           if (up1) { const float2 f = *reinterpret_cast<const float2*>(A.f1 + i); a1a = (double)f.x; a1b = (double)f.y; }
           else { a1a = (double)A.f1[i]; }
           a1l = lo1 ? (double)A.f1[i - 1] : 0.0;
-          if (up2) { a2u0 = (double)A.f2[i]; a2u1 = (double)A.f2[i + 1]; }
-          if (lo2) { a2l0 = (double)A.f2[i - nx]; a2l1 = (double)A.f2[i + 1 - nx]; }
-          if (up3) { a3u0 = (double)A.f3[i]; a3u1 = (double)A.f3[i + 1]; }
+          // aligned per-diagonal fp32 copies: every pair is one 8-byte load
+          if (up2) { const float2 f = *reinterpret_cast<const float2*>(A.f2 + i); a2u0 = (double)f.x; a2u1 = (double)f.y; }
+          if (lo2) { const float2 f = *reinterpret_cast<const float2*>(A.f2 + i - nx); a2l0 = (double)f.x; a2l1 = (double)f.y; }
+          if (up3) { const float2 f = *reinterpret_cast<const float2*>(A.f3 + i); a3u0 = (double)f.x; a3u1 = (double)f.y; }
         }
         if (up3) {
           const int64_t j = i + np;

@@ -27,6 +27,8 @@ struct DiaLayout {
   size_t o_dinv;     // fp64 [n]  1/D0
   size_t o_h16;      // fp16 3 x [n] (each 256-B aligned): off-diagonals D1, D2, D3 times a power-of-two scale (A3)
   size_t h16_stride; // bytes between the three fp16 arrays
+  size_t o_f32a;     // fp32 3 x [n] (each 256-B aligned): the off-diagonals of A2 again, one array per diagonal, so
+  size_t f32a_stride;//   that the pair (D_k[i], D_k[i+1]), i even, is one 8-byte load (packed D2, D3 start at odd elements)
   size_t bytes;
 };
 
@@ -49,6 +51,8 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
   L->o_dinv = o;   o = align_up(o + sizeof(double) * (size_t)L->n);
   L->h16_stride = align_up(sizeof(__half) * (size_t)L->n);
   L->o_h16 = o;    o = o + 3 * L->h16_stride;
+  L->f32a_stride = align_up(sizeof(float) * (size_t)L->n);
+  L->o_f32a = o;   o = o + 3 * L->f32a_stride;
   L->bytes = o;
   return true;
 }
@@ -57,7 +61,8 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
 struct DiaDev {
   const double* d0; const double* d1; const double* d2; const double* d3;   // fp64 diagonals (A1)
   const float* f0;                                                          // fp32 main diagonal (A2), ablation only
-  const float* f1; const float* f2; const float* f3;                        // fp32 off-diagonals (A2)
+  const float* f1; const float* f2; const float* f3;                        // fp32 off-diagonals (A2): the aligned
+                                                                            // per-diagonal copies, [n] each, zero tail
   const __half* h1; const __half* h2; const __half* h3;                     // fp16 off-diagonals x scale (A3)
   const double* h_scale;    // [0] absmax bits, [1] scale (power of two), [2] 1/scale
   const double* dinv;       // 1/D0

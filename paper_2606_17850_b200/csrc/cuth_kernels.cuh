@@ -157,9 +157,9 @@ __device__ __forceinline__ void zmarch_apply_x2(const DiaDev& A, const double* _
         if (up1) { const float2 g = *reinterpret_cast<const float2*>(A.f1 + i); a1a = (double)g.x; a1b = (double)g.y; }
         else { a1a = (double)A.f1[i]; }
         a1l = lo1 ? (double)A.f1[i - 1] : 0.0;
-        if (up2) { a2u0 = (double)A.f2[i]; a2u1 = (double)A.f2[i + 1]; }
-        if (lo2) { a2l0 = (double)A.f2[i - nx]; a2l1 = (double)A.f2[i + 1 - nx]; }
-        if (up3) { a3u0 = (double)A.f3[i]; a3u1 = (double)A.f3[i + 1]; }
+        if (up2) { const float2 g = *reinterpret_cast<const float2*>(A.f2 + i); a2u0 = (double)g.x; a2u1 = (double)g.y; }
+        if (lo2) { const float2 g = *reinterpret_cast<const float2*>(A.f2 + i - nx); a2l0 = (double)g.x; a2l1 = (double)g.y; }
+        if (up3) { const float2 g = *reinterpret_cast<const float2*>(A.f3 + i); a3u0 = (double)g.x; a3u1 = (double)g.y; }
       }
       // absent neighbours: their matrix entry is 0 (standard form) / they take the centre value (difference form)
       const double2 zero2 = make_double2(0.0, 0.0);
