@@ -377,9 +377,13 @@ def main():
         # outer: K1 (matrix + z, p, x read + p', mu, x written) + K2 (r, mu read, r written); preconditioner:
         # FIRST M+8+3s (2s in fp64), (k-3) x MID M+4s, LAST M+2s+16 with s = sizeof(T), M = matrix bytes per row
         #
+        # a two-pass launch (k_cheb_pair_f32) moves M + 5s for two MID passes
         k, sT = args.cheb_degree, (4 if mixed else 8)
         Mc = (2 * (m - 1) if h16 else 4 * (m - 1)) if mixed else 8 * m
-        apply_bytes = (k - 1) * Mc + ((3 if mixed else 2) * sT + 8) + (k - 3) * 4 * sT + (2 * sT + 16)
+        cheb_launches, cheb_npairs = cu.cuth_cheb_launches(g, S.opts)
+        singles = (k - 3) - 2 * cheb_npairs
+        apply_bytes = ((Mc + (3 if mixed else 2) * sT + 8) + singles * (Mc + 4 * sT) + cheb_npairs * (Mc + 5 * sT)
+                       + (Mc + 2 * sT + 16))
         outer = lambda M_: M_ + 48 + 24          # no 1/D0 anywhere: z = q(A) r is a stored vector
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
@@ -394,8 +398,11 @@ def main():
     if cheb:
         dom_name, dom_ms = "k_cheb_mid", kern["k_cheb_mid"]
         dom_bytes = (((2 if h16 else 4) * (m - 1) + 16) if mixed else (8 * m + 32)) * w.n
+        if cheb_npairs > 0:
+            dom_name, dom_ms = "k_cheb_pair", kern["k_cheb_pair"]
+            dom_bytes = ((2 if h16 else 4) * (m - 1) + 20) * w.n
         stage_fp64 = not mixed
-    per_it = (2 if fused else 3) + (args.cheb_degree - 1 if cheb else 0)
+    per_it = (2 if fused else 3) + (cheb_launches if cheb else 0)
     per_eval = 3 if fused else 2
     launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
     if persistent:

@@ -151,6 +151,12 @@ int cuth_version(void);
  * true-residual branches + epilogue. */
 int cuth_launches_per_iteration(const cuth_grid_t* grid);
 
+/* Kernel launches of ONE Chebyshev apply (Alg. 3) for this grid and these options: the first
+ * pass, the middle passes (single, or two per launch -- see cuth_set_cheb_fusion) and the last pass; 0 when the
+ * preconditioner is not Chebyshev, negative on bad arguments.  *pairs_out (may be NULL) = how many of them are
+ * two-pass launches.  Pure host. */
+int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pairs_out);
+
 /* Spectral-range estimate for the Chebyshev preconditioner: `steps` Lanczos iterations on
  * the device (start vector v0_D, e.g. the right-hand side), the tridiagonal T copied to the host and its
  * extreme eigenvalues found there in fp64 (bisection).  bounds_H[0] = smallest Ritz value, bounds_H[1] =

@@ -51,7 +51,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches"]
 
 _lib = None
 
@@ -241,6 +241,17 @@ def cuth_tridiag_extremes(alpha, beta):
     _check(L.cuth_tridiag_extremes(a.ctypes.data_as(C.c_void_p), b.ctypes.data_as(C.c_void_p), C.c_int(a.size), out),
            "cuth_tridiag_extremes")
     return out[0], out[1]
+
+
+def cuth_cheb_launches(grid: Grid, opts):
+    """(launches, pairs) of one Chebyshev apply for this grid and these options (include/cuth.h); pure host."""
+    L = load_library()
+    L.cuth_cheb_launches.restype = C.c_int
+    pairs = C.c_int(0)
+    rc = L.cuth_cheb_launches(grid.ref(), C.byref(opts), C.byref(pairs))
+    if rc < 0:
+        _check(rc, "cuth_cheb_launches")
+    return int(rc), int(pairs.value)
 
 
 def cuth_set_cheb_fusion(mode: int):

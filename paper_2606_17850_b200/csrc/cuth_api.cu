@@ -748,4 +748,18 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid) {
   return use_zmarch(L) ? 2 : 3;
 }
 
+int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pairs_out) {
+  DiaLayout L;
+  if (!opts) return CUTH_ERR_NULL;
+  if (!make_layout(grid, &L)) return CUTH_ERR_DIMS;
+  if (opts->preconditioner != CUTH_PRECOND_CHEBYSHEV) { if (pairs_out) *pairs_out = 0; return 0; }
+  int pairs = 0, launches = 1;                   // FIRST
+  for (const ChebOp& op : cheb_schedule(opts->cheb_degree, cheb_pairs(L, cheb_code(opts)))) {
+    ++launches;
+    if (op.kind == 1) ++pairs;
+  }
+  if (pairs_out) *pairs_out = pairs;
+  return launches;
+}
+
 }  // extern "C"
