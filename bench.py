@@ -194,8 +194,8 @@ def main():
     ap.add_argument("--cheb-storage", default="fp32", choices=["fp32", "fp16"],
                     help="MIXED Chebyshev: matrix copy the preconditioner reads (A2 fp32 / A3 fp16, Alg. 4)")
     ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
-    ap.add_argument("--cheb-fusion", type=int, default=0, choices=[0, 1, 2],
-                    help="cuth_set_cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel")
+    ap.add_argument("--cheb-fusion", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="cuth_set_cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel, 3 = 2 without TMA")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,

@@ -185,9 +185,11 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
 int cuth_set_traversal(int mode);
 
 /* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic (two
- * consecutive passes per kernel, k_cheb_pair_f32, on the large planes where the single passes run two columns
- * per thread), 1 = one pass per kernel, 2 = pairs wherever nx is even.  The polynomial is the same, and so is
- * the arithmetic of every row. */
+ * consecutive passes per kernel on the large planes where the single passes run two columns per thread),
+ * 1 = one pass per kernel, 2 = pairs wherever nx is even, 3 = like 2 but never the TMA version of the kernel.
+ * The two-pass kernel takes its operands through TMA (k_cheb_pair_tma) when nx is a multiple of 4 (fp32 A2) /
+ * 8 (fp16 A3), else through ordinary loads (k_cheb_pair_f32).  The polynomial is the same, and so is the
+ * arithmetic of every row. */
 int cuth_set_cheb_fusion(int mode);
 
 /* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle

@@ -18,6 +18,7 @@
 #include "cuth_fused_x2.cuh"
 #include "cuth_cheb.cuh"
 #include "cuth_cheb_pair.cuh"
+#include "cuth_cheb_pair_tma.cuh"
 #include "cuth_persistent.cuh"
 
 namespace cuth {
@@ -168,6 +169,71 @@ static bool cheb_pairs(const DiaLayout& L, int code) {
   // 0.79 s, cfg 4 10.8 -> 10.1 s
   return mode == 2 || cheb_x2(L);
 }
+struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST
+// ---- TMA version of the two-pass kernel: tensor maps over (x, y, z) for its six operand streams
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+static std::atomic<int> g_pair_tma{0};     // 0 auto (TMA when possible), 1 never (LDG version): cuth_set_cheb_fusion bit 2
+static bool cheb_pairs_tma(const DiaLayout& L, int code) {
+  if (!cheb_pairs(L, code) || g_pair_tma.load() == 1) return false;
+  const int64_t elems16 = code == 2 ? 8 : 4;           // tensor-map strides are multiples of 16 bytes
+  return (L.nx % elems16) == 0;
+}
+// box of `rows` rows x (QX + 16 bytes of) columns x 1 plane of an (nx, ny, nz) array of fp32 / fp16 elements; cells outside
+// the array read as zero
+static bool make_box_map(CUtensorMap* m, const void* base, bool half, const DiaLayout& L, int rows) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t es = half ? 2 : 4;
+  const cuuint64_t dims[3] = {(cuuint64_t)L.nx, (cuuint64_t)L.ny, (cuuint64_t)L.nz};
+  const cuuint64_t strides[2] = {(cuuint64_t)L.nx * es, (cuuint64_t)L.nxny * es};
+  const cuuint32_t box[3] = {(cuuint32_t)(QX + 16 / (int)es), (cuuint32_t)rows, 1u};   // PairBox<E>::W
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  return enc(m, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(base),
+             dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+struct PairMaps { CUtensorMap u, v, r, f1, f2, f3; };
+static bool make_pair_maps(PairMaps* pm, const DiaLayout& L, const void* dia_D, const Workspace& w, int code,
+                           int old, int cur) {
+  const DiaDev A = dev_view(dia_D, L);
+  const void* cd[4] = {w.cd0, w.cd1, w.cd2, w.cd3};
+  const bool h = code == 2;
+  return make_box_map(&pm->u, cd[cur], false, L, QY + 2) && make_box_map(&pm->v, cd[old], false, L, QY) &&
+         make_box_map(&pm->r, w.crc, false, L, QY) &&
+         make_box_map(&pm->f1, h ? (const void*)A.h1 : (const void*)A.f1, h, L, QY) &&
+         make_box_map(&pm->f2, h ? (const void*)A.h2 : (const void*)A.f2, h, L, QY + 1) &&
+         make_box_map(&pm->f3, h ? (const void*)A.h3 : (const void*)A.f3, h, L, QY);
+}
+static void* cheb_pair_tma_fn(int code) {
+  return code == 2 ? (void*)k_cheb_pair_tma<MatF16> : (void*)k_cheb_pair_tma<MatF32>;
+}
+// one two-pass launch outside a graph (cuth_cheb_apply, cuth_profile_kernel)
+static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Workspace& w, int code, const ChebOp& op,
+                               cudaStream_t st) {
+  Ctx* ctxp = w.ctx;
+  int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
+  PairMaps pm;
+  if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur)) {
+    void* a[] = {&ctxp, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
+    return cudaLaunchKernel(cheb_pair_tma_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
+  }
+  void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
+  return cudaLaunchKernel(cheb_pair_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
+}
+
 static void* cheb_last_fn(int code) {
   return code == 0 ? (void*)k_cheb_last<double, MatF32> : code == 1 ? (void*)k_cheb_last<float, MatF32>
                                                                     : (void*)k_cheb_last<float, MatF16>;
@@ -175,7 +241,6 @@ static void* cheb_last_fn(int code) {
 
 // The passes of one Chebyshev apply after the first one: MID passes i = 1 .. k-3 (single, or fused in pairs),
 // then LAST (i = k-2).  State = which buffers hold Z_i (old) and Z_{i+1} (cur); k_cheb_first leaves old = 1, cur = 0.
-struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST
 static std::vector<ChebOp> cheb_schedule(int k, bool pairs) {
   std::vector<ChebOp> ops;
   int old = 1, cur = 0, i = 1;
@@ -205,10 +270,12 @@ struct GraphEntry {
   int x2blocks = 0;
   int k1x2 = 0;
   int pblocks = 0;
+  const void* dia = nullptr;   // matrix the tensor maps of the TMA two-pass nodes were made for (else nullptr)
   int device = -1;
 };
 static std::mutex g_mu;
 static std::unordered_map<const void*, GraphEntry> g_graphs;
+static std::unordered_map<const void*, const void*> g_last_dia;   // workspace -> matrix of its last solve (profile hook)
 
 static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* deps, size_t ndeps,
                               void* func, int blocks, void** args) {
@@ -223,7 +290,7 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
 }
 
 static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
-                       int x2blocks, int k1x2, int pblocks, GraphEntry* out) {
+                       int x2blocks, int k1x2, int pblocks, const DiaLayout* Ltma, const void* dia_tma, GraphEntry* out) {
   const int blocks = grid_blocks(n);
   if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
   cudaGraph_t g;
@@ -259,7 +326,11 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
     for (const ChebOp& op : cheb_schedule(kdeg, pblocks > 0)) {
       cudaGraphNode_t prev = n_c;
       int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
-      if (op.kind == 1) {
+      PairMaps pm;
+      if (op.kind == 1 && dia_tma && make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur)) {
+        void* a[] = {&ctx, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code), pblocks, a));
+      } else if (op.kind == 1) {
         void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
         CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
       } else if (op.kind == 0) {
@@ -308,13 +379,14 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks;
+  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks; out->dia = dia_tma;
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
 
 static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     int cblocks, int x2blocks, int k1x2, int pblocks, cudaGraphExec_t* ex) {
+                     int cblocks, int x2blocks, int k1x2, int pblocks, const DiaLayout* Ltma, const void* dia_tma,
+                     cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
   int dev = -1;
@@ -323,7 +395,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
                                it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
                                it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
-                               it->second.pblocks != pblocks)) {
+                               it->second.pblocks != pblocks || it->second.dia != dia_tma)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -331,7 +403,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, pblocks, &e);
+    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, pblocks, Ltma, dia_tma, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -441,6 +513,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
+  { std::lock_guard<std::mutex> lk(g_mu); g_last_dia[work_D] = dia_D; }
   if (use_persistent(L, cheb)) {
     Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
     void* args[] = {&ctxp, &ctlp, &part};
@@ -451,7 +524,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
                  cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0,
                  (use_zmarch(L) && fused_x2(L)) ? 1 : 0,
-                 (cheb && cheb_pairs(L, cheb_code(opts))) ? cheb_pair_blocks(L) : 0, &ex);
+                 (cheb && cheb_pairs(L, cheb_code(opts))) ? cheb_pair_blocks(L) : 0, &L,
+                 (cheb && cheb_pairs_tma(L, cheb_code(opts))) ? dia_D : nullptr, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -598,9 +672,14 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
       CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : cheb_blocks(L)), dim3(kThreads), args, 0, st));
     } break;
     case 9: case 10: {            // one fused pair of Chebyshev passes, fp32 on A2 / on A3
-      Ctx* ctxp = w.ctx; int step = 1, old = 1, cur = 0, wo = 2, yo = 3;
-      void* args[] = {&ctxp, &step, &old, &cur, &wo, &yo};
-      CU(cudaLaunchKernel(cheb_pair_fn(kernel_id == 10 ? 2 : 1), dim3(cheb_pair_blocks(L)), dim3(kThreads), args, 0, st));
+      const void* dia = nullptr;
+      { std::lock_guard<std::mutex> lk(g_mu);
+        auto it = g_last_dia.find(work_D);
+        if (it != g_last_dia.end()) dia = it->second; }
+      if (!dia) return CUTH_ERR_VALUE;             // no solve has used this workspace yet
+      const ChebOp op = {1, 1, 1, 0, 2, 3};
+      const Workspace wc = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, true);   // with the Z buffers
+      CU(launch_pair(L, dia, wc, kernel_id == 10 ? 2 : 1, op, st));
     } break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
@@ -678,10 +757,9 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   { void* a[] = {&ctxp};
     CU(cudaLaunchKernel(cheb_first_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
   for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code))) {
-    int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
+    int step = op.step, old = op.old, cur = op.cur;
     if (op.kind == 1) {
-      void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
-      CU(cudaLaunchKernel(cheb_pair_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st));
+      CU(launch_pair(L, dia_D, w, code, op, st));
     } else if (op.kind == 0) {
       void* a[] = {&ctxp, &step, &old, &cur};
       CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : sb), dim3(kThreads), a, 0, st));
@@ -703,8 +781,9 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
 }
 
 int cuth_set_cheb_fusion(int mode) {
-  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
-  g_cheb_pairs.store(mode);
+  if (mode < 0 || mode > 3) return CUTH_ERR_VALUE;
+  g_cheb_pairs.store(mode == 3 ? 2 : mode);
+  g_pair_tma.store(mode == 3 ? 1 : 0);
   return CUTH_OK;
 }
 
@@ -734,6 +813,7 @@ int cuth_release_workspace(const void* work_D) {
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
   }
+  g_last_dia.erase(work_D);
   return CUTH_OK;
 }
 

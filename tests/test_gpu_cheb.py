@@ -16,15 +16,18 @@ CASES = [
     dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8),
     dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),
     dict(cfg=6, nx=45, ny=38, nz=10, n_hot=6),     # paper-like anisotropic stack
+    dict(cfg=4, nx=136, ny=67, nz=8, n_hot=6),     # nx % 8 == 0: three x-tiles of the TMA two-pass kernel, ragged in x and y
+    dict(cfg=1, nx=8, ny=4, nz=2, n_hot=1),        # two planes only: every plane of the march is a peeled one
 ]
 
 
-@pytest.fixture(params=["flat", "flat-pairs", "zmarch", "zmarch-x1"], autouse=True)
+@pytest.fixture(params=["flat", "flat-pairs", "flat-pairs-ldg", "zmarch", "zmarch-x1"], autouse=True)
 def traversal(request):
     import paper_2606_17850_b200 as cu
     cu.cuth_set_traversal(1 if request.param.startswith("flat") else 2)
-    # pairs: "flat" = one pass per kernel, "flat-pairs" and "zmarch" = fused pairs, "zmarch-x1" = single passes
-    cu.cuth_set_cheb_fusion({"flat": 1, "flat-pairs": 2, "zmarch": 2, "zmarch-x1": 1}[request.param])
+    # "flat", "zmarch-x1" = one pass per kernel; "flat-pairs", "zmarch" = two passes per kernel (operands by TMA
+    # when nx % 4 == 0 (fp16: % 8), by ordinary loads otherwise); "flat-pairs-ldg" = two passes, never TMA
+    cu.cuth_set_cheb_fusion({"flat": 1, "flat-pairs": 2, "flat-pairs-ldg": 3, "zmarch": 2, "zmarch-x1": 1}[request.param])
     cu.cuth_set_k1_variant(1 if request.param == "zmarch-x1" else 2)       # 2: two columns per thread when nx is even
     yield request.param
     cu.cuth_set_traversal(0)
