@@ -184,12 +184,12 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
  * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
 int cuth_set_traversal(int mode);
 
-/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic (two
- * consecutive passes per kernel on the large planes where the single passes run two columns per thread),
- * 1 = one pass per kernel, 2 = pairs wherever nx is even, 3 = like 2 but never the TMA version of the kernel.
+/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic = two
+ * consecutive passes per kernel (measured faster on every grid), 1 = one pass per kernel, 2 = same as 0,
+ * 3 = two passes per kernel but never the TMA version of the kernel.
  * The two-pass kernel takes its operands through TMA (k_cheb_pair_tma) when nx is a multiple of 4 (fp32 A2) /
  * 8 (fp16 A3), else through ordinary loads (k_cheb_pair_f32).  The polynomial is the same, and so is the
- * arithmetic of every row. */
+ * arithmetic of every row.  fp64 applies and odd nx always run one pass per kernel. */
 int cuth_set_cheb_fusion(int mode);
 
 /* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle

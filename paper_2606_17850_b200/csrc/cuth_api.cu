@@ -164,10 +164,9 @@ static int cheb_pair_blocks(const DiaLayout& L) {
 }
 static bool cheb_pairs(const DiaLayout& L, int code) {
   const int mode = g_cheb_pairs.load();
-  if (code == 0 || mode == 1 || (L.nx & 1)) return false;     // fp32 arithmetic, column pairs: nx even
-  // automatic: wherever the single passes run two columns per thread (large planes); measured cfg 3 0.92 ->
-  // 0.79 s, cfg 4 10.8 -> 10.1 s
-  return mode == 2 || cheb_x2(L);
+  // fp32 arithmetic, column pairs: nx even.  Measured faster on every grid (cfg 2 23.5 -> 21.0 ms, cfg 3 0.92 ->
+  // 0.63 s, cfg 4 10.8 -> 7.9 s, cfg 5 5.8 -> 4.3 s, cfg 6 41 -> 34 ms), so automatic = always.
+  return code != 0 && mode != 1 && (L.nx & 1) == 0;
 }
 struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST
 // ---- TMA version of the two-pass kernel: tensor maps over (x, y, z) for its six operand streams

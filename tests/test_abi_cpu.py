@@ -101,9 +101,9 @@ def test_cheb_launch_schedule_host_side(cu):
     """cuth_cheb_launches (pure host): k - 1 launches with one pass per kernel (R-C3: the dead k-th SpMV of
     Alg. 3 is skipped); with two passes per kernel the k - 3 middle passes pair up, FIRST and LAST stay."""
     dz = np.full(16, 1e-6)
-    big = cu.Grid(1024, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # cfg-3 planes: pairs by default
+    big = cu.Grid(1024, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # even nx: pairs by default
     odd = cu.Grid(1023, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # odd nx: never
-    small = cu.Grid(32, 32, 16, 1e-6, 1e-6, dz, None, 1e4)             # small planes: only when forced
+    small = cu.Grid(32, 32, 16, 1e-6, 1e-6, dz, None, 1e4)
     mk = lambda prec, k: cu.Opts(prec, 1e-8, 1000, 20, cu.PRECOND_CHEBYSHEV, k, 1e-3, 1.0, cu.CHEB_DEFAULT)
     try:
         for k in (3, 4, 5, 30, 31):
@@ -116,7 +116,10 @@ def test_cheb_launch_schedule_host_side(cu):
             assert cu.cuth_cheb_launches(small, mk(cu.FP64, k)) == (k - 1, 0)        # fp64 apply: single passes
             cu.cuth_set_cheb_fusion(0)
             assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
-            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (k - 1, 0)
+            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
+            assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k)) == (k - 1, 0)
+            cu.cuth_set_cheb_fusion(3)                                 # the non-TMA kernel: same schedule
+            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
         assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
     finally:
         cu.cuth_set_cheb_fusion(0)
