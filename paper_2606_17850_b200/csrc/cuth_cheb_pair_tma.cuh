@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
   }
   __syncthreads();
 
-  uint32_t seq0 = 0;                       // planes requested / consumed by this CTA before the current tile
+  uint32_t ph = 0;                         // bit S: parity of the next fill of stage S to wait for
   for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
     const int bx = t % tiles_x, by = t / tiles_x;
     const int x0 = bx * QIX - 2, y0 = by * QIY - 1;                    // region origin (x0 even)
@@ -120,47 +120,59 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
     // box starts: x0 rounded down to 16 bytes of elements (two's complement & works for x0 = -2 too)
     const int xs_f = x0 & ~(PairBox<float>::AL - 1), xs_e = x0 & ~(PairBox<E>::AL - 1);
     const int cf = (x0 - xs_f) + 2 * tx, ce = (x0 - xs_e) + 2 * tx;    // this thread's pair inside a staged row
-    auto request = [&](int kp) {           // thread 0: the six boxes of plane kp into its stage
-      const uint32_t seq = seq0 + (uint32_t)kp, s = seq % kPairStages;
-      mbar_expect_tx(&full[s], kStageBytes);
-      tma_load_3d(st[s].u, &tmU, &full[s], xs_f, y0 - 1, kp);
-      tma_load_3d(st[s].v, &tmV, &full[s], xs_f, y0, kp);
-      tma_load_3d(st[s].r, &tmR, &full[s], xs_f, y0, kp);
-      tma_load_3d(st[s].f1, &tm1, &full[s], xs_e, y0, kp);
-      tma_load_3d(st[s].f2, &tm2, &full[s], xs_e, y0 - 1, kp);
-      tma_load_3d(st[s].f3, &tm3, &full[s], xs_e, y0, kp);
+    // Plane kp lives in stage kp % 3 (every tile starts at stage 0, so the stage of a step is a compile-time
+    // constant in the three-fold unrolled march below); ph holds, per stage, the parity of its next fill.
+    auto request = [&](auto stage_t, int kp) {   // thread 0: the six boxes of plane kp into stage S
+      constexpr int S = decltype(stage_t)::value;
+      mbar_expect_tx(&full[S], kStageBytes);
+      tma_load_3d(st[S].u, &tmU, &full[S], xs_f, y0 - 1, kp);
+      tma_load_3d(st[S].v, &tmV, &full[S], xs_f, y0, kp);
+      tma_load_3d(st[S].r, &tmR, &full[S], xs_f, y0, kp);
+      tma_load_3d(st[S].f1, &tm1, &full[S], xs_e, y0, kp);
+      tma_load_3d(st[S].f2, &tm2, &full[S], xs_e, y0 - 1, kp);
+      tma_load_3d(st[S].f3, &tm3, &full[S], xs_e, y0, kp);
     };
-    auto arrived = [&](int kp) {           // everybody: block until plane kp has landed
-      const uint32_t seq = seq0 + (uint32_t)kp;
-      mbar_wait(&full[seq % kPairStages], (seq / kPairStages) & 1u);
+    auto arrived = [&](auto stage_t) {     // everybody: block until the pending fill of stage S has landed
+      constexpr int S = decltype(stage_t)::value;
+      mbar_wait(&full[S], (ph >> S) & 1u);
+      ph ^= 1u << S;
     };
+    constexpr std::integral_constant<int, 0> S0{};
+    constexpr std::integral_constant<int, 1> S1{};
+    constexpr std::integral_constant<int, 2> S2{};
 
     __syncthreads();                       // the previous tile's stages and W ring are dead
-    if (tid == 0)
-      for (int kp = 0; kp < kPairStages && kp < nz; ++kp) request(kp);
+    if (tid == 0) {
+      request(S0, 0);
+      request(S1, 1);                      // nz >= 2
+      if (nz > 2) request(S2, 2);
+    }
 
-    arrived(0);
-    float2 u_lo = z2, u_c = lds_pair(&st[seq0 % kPairStages].u[ty + 1][cf], 1.f);   // U on planes k-1, k
+    arrived(S0);
+    float2 u_lo = z2, u_c = lds_pair(&st[0].u[ty + 1][cf], 1.f);        // U on planes k-1, k
     float2 w_lo = z2, w_c = z2;                                         // W on planes k-2, k-1
     float2 a3l_w = z2, a3l_y = z2;                                      // D3 below plane k / below plane k-1
     float pf1l = 0.f, pf1a = 0.f, pf1b = 0.f, ps = 0.f;                 // row of plane k-1, kept for Y
     float2 pf2u = z2, pf2l = z2, pa3u = z2, pr = z2;
 
-    for (int k = 0; k <= nz; ++k) {
+    // One step of the march: W on plane k from stage S (HAS_W), the barrier, Y on plane k-1.
+    auto do_step = [&](auto stage_t, auto has_w_t, int k) {
+      constexpr int S = decltype(stage_t)::value, SN = (S + 1) % kPairStages;
+      constexpr bool HAS_W = decltype(has_w_t)::value;
       float2 w = z2, u_hi = z2, rv = z2, f1p = z2, f2u = z2, f2l = z2, a3u = z2;
       float f1l = 0.f, s = 0.f;
-      if (k < nz) {
+      if (HAS_W) {
         // ---- W on plane k: operands from the stage (no bounds predicates: absent = zero x zero)
-        const PairStage<E>& S = st[(seq0 + (uint32_t)k) % kPairStages];
-        const float2 v2u = lds_pair(&S.u[ty + 2][cf], 1.f), v2l = lds_pair(&S.u[ty][cf], 1.f);
-        const float2 zo = lds_pair(&S.v[ty][cf], 1.f);
-        rv = lds_pair(&S.r[ty][cf], 1.f);
-        f1p = lds_pair(&S.f1[ty][ce], ms);
-        f2u = lds_pair(&S.f2[ty + 1][ce], ms); f2l = lds_pair(&S.f2[ty][ce], ms);
-        a3u = lds_pair(&S.f3[ty][ce], ms);
+        const PairStage<E>& T = st[S];
+        const float2 v2u = lds_pair(&T.u[ty + 2][cf], 1.f), v2l = lds_pair(&T.u[ty][cf], 1.f);
+        const float2 zo = lds_pair(&T.v[ty][cf], 1.f);
+        rv = lds_pair(&T.r[ty][cf], 1.f);
+        f1p = lds_pair(&T.f1[ty][ce], ms);
+        f2u = lds_pair(&T.f2[ty + 1][ce], ms); f2l = lds_pair(&T.f2[ty][ce], ms);
+        a3u = lds_pair(&T.f3[ty][ce], ms);
         if (k + 1 < nz) {
-          arrived(k + 1);
-          u_hi = lds_pair(&st[(seq0 + (uint32_t)k + 1u) % kPairStages].u[ty + 1][cf], 1.f);
+          arrived(std::integral_constant<int, SN>{});
+          u_hi = lds_pair(&st[SN].u[ty + 1][cf], 1.f);
         }
         const float vl = __shfl_up_sync(kAll, u_c.y, 1), vr = __shfl_down_sync(kAll, u_c.x, 1);
         f1l = __shfl_up_sync(kAll, f1p.y, 1);
@@ -177,8 +189,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
         if (inner) *reinterpret_cast<float2*>(pW) = w;
       }
       __syncthreads();                     // W(k-1) complete, W(k-2) no longer read, stage of plane k consumed
-      if (k < nz) {
-        if (tid == 0 && k + kPairStages < nz) request(k + kPairStages);
+      if (HAS_W) {
+        if (tid == 0 && k + kPairStages < nz) request(stage_t, k + kPairStages);
         *reinterpret_cast<float2*>(&sW[k & 1][ty][2 * tx]) = w;
       }
       if (k >= 1) {
@@ -206,8 +218,21 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
       a3l_w = a3u;
       u_lo = u_c; u_c = u_hi;
       pW += np; pY += np;
+    };
+    constexpr std::true_type HW{};
+    constexpr std::false_type NW{};
+    int k = 0;
+    for (; k + kPairStages <= nz; k += kPairStages) {
+      do_step(S0, HW, k); do_step(S1, HW, k + 1); do_step(S2, HW, k + 2);
     }
-    seq0 += (uint32_t)nz;
+    // the last nz % 3 planes, then the step that only forms Y on the top plane
+    if (k < nz) {
+      do_step(S0, HW, k); ++k;
+      if (k < nz) { do_step(S1, HW, k); ++k; do_step(S2, NW, k); }
+      else do_step(S1, NW, k);
+    } else {
+      do_step(S0, NW, k);
+    }
   }
 }
 
