@@ -32,7 +32,8 @@ import workloads as W  # noqa: E402
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
 NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3114e9,   # profiles/r1f_cfg3_fp64_k1_nodinv.md
-                     ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 528.5e6,    # profiles/r1g_cfg3_cheb_pairs.md
+                     ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 516.7e6,    # profiles/r1h_cheb_pair_tma.md
+                     ("cfg4_steady_4096x4096x8", "k_cheb_pair", "mixed"): 4.477e9,                 # profiles/r1h_cheb_pair_tma.md
                      }     # cfg 4: profiles/r1d predates the K1 that no longer reads 1/D0 -> null until recaptured
 
 METRIC = "pcg_time_to_solution"
