@@ -193,3 +193,38 @@ def test_cheb_bad_interval_rejected_or_reported():
     S2 = cu.Solver(M, cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_degree=2, cheb_lmin=1e-6, cheb_lmax=1e-3))
     with pytest.raises(cu.CuthError):
         S2.solve(to_dev(w.power), x)
+
+
+SHAPES = [(4, 2, 2), (8, 6, 3), (12, 9, 5), (64, 8, 2), (60, 6, 4), (68, 10, 4), (124, 13, 3), (128, 7, 9),
+          (200, 31, 6), (256, 64, 16)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("degree", [5, 6, 30])
+@pytest.mark.parametrize("storage", ["fp32", "fp16"])
+@pytest.mark.parametrize("traversal", ["flat"], indirect=True)       # the test sets the schedule itself: once
+def test_cheb_apply_kernel_variants_agree(shape, degree, storage, traversal):
+    """The same polynomial through the three kernel schedules of the fp32 apply -- one pass per kernel, two
+    passes per kernel with ordinary loads, two passes per kernel with TMA-staged operands (taken when nx % 4 == 0,
+    fp16: % 8) -- on shapes below, at and above one 60 x 6 region, with per-cell conductivities: every row runs
+    the same arithmetic, so the results agree to fp32 rounding of the order of operations."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    nx, ny, nz = shape
+    w = W.make_workload(3, nx=nx, ny=ny, nz=nz, n_hot=2)
+    M, S, b, lo, hi, gersh = _setup(w, cu.MIXED, steps=min(20, w.n - 1), degree=degree,
+                                    storage=cu.CHEB_A3_FP16 if storage == "fp16" else cu.CHEB_DEFAULT)
+    r = W.normal01(w.seed, 52, 53, np.arange(w.n)) * 1e-7
+    out = {}
+    try:
+        for mode in (1, 3, 2):
+            cu.cuth_set_cheb_fusion(mode)
+            z = torch.full((w.n,), float("nan"), dtype=torch.float64, device="cuda")
+            S.cheb_apply(to_dev(r), z)
+            out[mode] = z.cpu().numpy()
+    finally:
+        cu.cuth_set_cheb_fusion(1)
+    assert np.isfinite(out[1]).all()
+    scale = np.abs(out[1]).max()
+    for mode in (3, 2):
+        assert np.abs(out[mode] - out[1]).max() <= 2e-5 * scale, (mode, shape)
