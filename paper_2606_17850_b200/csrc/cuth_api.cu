@@ -270,6 +270,7 @@ struct GraphEntry {
   int k1x2 = 0;
   int pblocks = 0;
   const void* dia = nullptr;   // matrix the tensor maps of the TMA two-pass nodes were made for (else nullptr)
+  int64_t tnx = 0, tny = 0;    // ... and its plane dimensions (the maps are baked into the kernel nodes)
   int device = -1;
 };
 static std::mutex g_mu;
@@ -379,6 +380,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
   out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks; out->dia = dia_tma;
+  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; }
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
@@ -394,7 +396,8 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
                                it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
                                it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
                                it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
-                               it->second.pblocks != pblocks || it->second.dia != dia_tma)) {
+                               it->second.pblocks != pblocks || it->second.dia != dia_tma ||
+                               (dia_tma && (it->second.tnx != Ltma->nx || it->second.tny != Ltma->ny)))) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);

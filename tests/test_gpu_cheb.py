@@ -228,3 +228,32 @@ def test_cheb_apply_kernel_variants_agree(shape, degree, storage, traversal):
     scale = np.abs(out[1]).max()
     for mode in (3, 2):
         assert np.abs(out[mode] - out[1]).max() <= 2e-5 * scale, (mode, shape)
+
+
+@pytest.mark.parametrize("traversal", ["flat-pairs"], indirect=True)
+def test_graph_cache_follows_plane_shape_and_matrix(traversal):
+    """The TMA two-pass nodes carry tensor maps baked into the cached graph of a workspace.  Re-using the SAME
+    workspace and the SAME matrix buffer for another grid with the same N (planes transposed: identical buffer
+    sizes, identical block counts are possible) must rebuild the graph, not reuse stale maps."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    shapes = [(120, 12, 6), (12, 120, 6), (120, 12, 6)]
+    copts = cu.Opts(cu.MIXED, 1e-8, 20000, 20, cu.PRECOND_CHEBYSHEV, 30, 1e-3, 1.0)
+    wls = [W.make_workload(3, nx=nx, ny=ny, nz=nz, n_hot=3) for (nx, ny, nz) in shapes]
+    grids = [grid_from_workload(w) for w in wls]
+    buf = torch.empty(max(cu.cuth_dia_bytes(g) for g in grids), dtype=torch.uint8, device="cuda")
+    work = torch.empty(max(cu.cuth_workspace_bytes(g, copts) for g in grids), dtype=torch.uint8, device="cuda")
+    res = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    for (nx, ny, nz), w, g in zip(shapes, wls, grids):
+        cu.cuth_build_dia(g, buf)
+        b = to_dev(w.power)
+        lo, hi, gersh, rlo, rhi = cu.cuth_lanczos_bounds(buf, g, b, 20, work)
+        opts = cu.Opts(cu.MIXED, 1e-8, 20000, 20, cu.PRECOND_CHEBYSHEV, 30, rlo, rhi)
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        cu.cuth_pcg_solve(buf, g, opts, b, x, work, res)
+        torch.cuda.synchronize()
+        A = O.assemble_workload(w)
+        xg = x.cpu().numpy()
+        rel = np.linalg.norm(w.power - O.spmv(A, xg)) / np.linalg.norm(w.power)
+        assert rel <= 1e-8, (nx, ny, nz, rel)
+    cu.cuth_release_workspace(work)
