@@ -387,8 +387,11 @@ def main():
         k, sT = args.cheb_degree, (4 if mixed else 8)
         Mc = (2 * (m - 1) if h16 else 4 * (m - 1)) if mixed else 8 * m
         singles = (k - 3) - 2 * cheb_npairs
-        apply_bytes = ((Mc + (3 if mixed else 2) * sT + 8) + singles * (Mc + 4 * sT) + cheb_npairs * (Mc + 5 * sT)
-                       + (Mc + 2 * sT + 16))
+        first_b, last_b = Mc + (3 if mixed else 2) * sT + 8, Mc + 2 * sT + 16
+        if singles < 0:     # the odd MID pass shares its launch with LAST: U, V, r32, r read, z written (M + 3s + 16)
+            apply_bytes = first_b + (cheb_npairs - 1) * (Mc + 5 * sT) + (Mc + 3 * sT + 16)
+        else:
+            apply_bytes = first_b + singles * (Mc + 4 * sT) + cheb_npairs * (Mc + 5 * sT) + last_b
         outer = lambda M_: M_ + 48 + 24          # no 1/D0 anywhere: z = q(A) r is a stored vector
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9

@@ -168,7 +168,7 @@ static bool cheb_pairs(const DiaLayout& L, int code) {
   // 0.63 s, cfg 4 10.8 -> 7.9 s, cfg 5 5.8 -> 4.3 s, cfg 6 41 -> 34 ms), so automatic = always.
   return code != 0 && mode != 1 && (L.nx & 1) == 0;
 }
-struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST
+struct ChebOp { int kind; int step, old, cur, w, y; };     // kind 0 = single MID, 1 = fused pair, 2 = LAST, 3 = MID + LAST
 // ---- TMA version of the two-pass kernel: tensor maps over (x, y, z) for its six operand streams
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -188,7 +188,7 @@ static std::atomic<int> g_pair_tma{0};     // 0 auto (TMA when possible), 1 neve
 static bool cheb_pairs_tma(const DiaLayout& L, int code) {
   if (!cheb_pairs(L, code) || g_pair_tma.load() == 1) return false;
   const int64_t elems16 = code == 2 ? 8 : 4;           // tensor-map strides are multiples of 16 bytes
-  return (L.nx % elems16) == 0;
+  return (L.nx % elems16) == 0 && encode_tiled_fn() != nullptr;
 }
 // box of `rows` rows x (QX + 16 bytes of) columns x 1 plane of an (nx, ny, nz) array of fp32 / fp16 elements; cells outside
 // the array read as zero
@@ -216,19 +216,21 @@ static bool make_pair_maps(PairMaps* pm, const DiaLayout& L, const void* dia_D, 
          make_box_map(&pm->f2, h ? (const void*)A.h2 : (const void*)A.f2, h, L, QY + 1) &&
          make_box_map(&pm->f3, h ? (const void*)A.h3 : (const void*)A.f3, h, L, QY);
 }
-static void* cheb_pair_tma_fn(int code) {
-  return code == 2 ? (void*)k_cheb_pair_tma<MatF16> : (void*)k_cheb_pair_tma<MatF32>;
+static void* cheb_pair_tma_fn(int code, bool last) {
+  if (last) return code == 2 ? (void*)k_cheb_pair_tma<MatF16, true> : (void*)k_cheb_pair_tma<MatF32, true>;
+  return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false> : (void*)k_cheb_pair_tma<MatF32, false>;
 }
 // one two-pass launch outside a graph (cuth_cheb_apply, cuth_profile_kernel)
 static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Workspace& w, int code, const ChebOp& op,
                                cudaStream_t st) {
-  Ctx* ctxp = w.ctx;
+  Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
   PairMaps pm;
   if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur)) {
-    void* a[] = {&ctxp, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
-    return cudaLaunchKernel(cheb_pair_tma_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
+    void* a[] = {&ctxp, &ctlp, &part, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
+    return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
   }
+  if (op.kind == 3) return cudaErrorInvalidValue;      // the fused MID + LAST launch exists only as a TMA kernel
   void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
   return cudaLaunchKernel(cheb_pair_fn(code), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
 }
@@ -240,10 +242,15 @@ static void* cheb_last_fn(int code) {
 
 // The passes of one Chebyshev apply after the first one: MID passes i = 1 .. k-3 (single, or fused in pairs),
 // then LAST (i = k-2).  State = which buffers hold Z_i (old) and Z_{i+1} (cur); k_cheb_first leaves old = 1, cur = 0.
-static std::vector<ChebOp> cheb_schedule(int k, bool pairs) {
+// kind 3 (only with the TMA kernel, fuse_last): the odd MID pass left over by the pairing and LAST in one launch.
+static std::vector<ChebOp> cheb_schedule(int k, bool pairs, bool fuse_last) {
   std::vector<ChebOp> ops;
   int old = 1, cur = 0, i = 1;
   while (i <= k - 3) {
+    if (pairs && fuse_last && i == k - 3) {
+      ops.push_back({3, i, old, cur, -1, -1});
+      return ops;
+    }
     if (pairs && i + 1 <= k - 3) {
       int fr[2], nf = 0;
       for (int b = 0; b < 4; ++b) if (b != old && b != cur) fr[nf++] = b;
@@ -323,13 +330,14 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
     const bool f32 = code != 0;
     { void* a[] = {&ctx};
       CU(add_kernel(body, &n_c, nullptr, 0, cheb_first_fn(code), cblocks, a)); }
-    for (const ChebOp& op : cheb_schedule(kdeg, pblocks > 0)) {
+    for (const ChebOp& op : cheb_schedule(kdeg, pblocks > 0, dia_tma != nullptr)) {
       cudaGraphNode_t prev = n_c;
       int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
       PairMaps pm;
-      if (op.kind == 1 && dia_tma && make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur)) {
-        void* a[] = {&ctx, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code), pblocks, a));
+      if ((op.kind == 1 || op.kind == 3) && dia_tma) {
+        if (!make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur)) return CUTH_ERR_CUDA;
+        void* a[] = {&ctx, &ctl, &partials, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3), pblocks, a));
       } else if (op.kind == 1) {
         void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
         CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
@@ -758,9 +766,9 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   { void* a[] = {&ctxp};
     CU(cudaLaunchKernel(cheb_first_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
-  for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code))) {
+  for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code), cheb_pairs_tma(L, code))) {
     int step = op.step, old = op.old, cur = op.cur;
-    if (op.kind == 1) {
+    if (op.kind == 1 || op.kind == 3) {
       CU(launch_pair(L, dia_D, w, code, op, st));
     } else if (op.kind == 0) {
       void* a[] = {&ctxp, &step, &old, &cur};
@@ -836,9 +844,10 @@ int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pa
   if (!make_layout(grid, &L)) return CUTH_ERR_DIMS;
   if (opts->preconditioner != CUTH_PRECOND_CHEBYSHEV) { if (pairs_out) *pairs_out = 0; return 0; }
   int pairs = 0, launches = 1;                   // FIRST
-  for (const ChebOp& op : cheb_schedule(opts->cheb_degree, cheb_pairs(L, cheb_code(opts)))) {
+  for (const ChebOp& op : cheb_schedule(opts->cheb_degree, cheb_pairs(L, cheb_code(opts)),
+                                        cheb_pairs_tma(L, cheb_code(opts)))) {
     ++launches;
-    if (op.kind == 1) ++pairs;
+    if (op.kind == 1 || op.kind == 3) ++pairs;
   }
   if (pairs_out) *pairs_out = pairs;
   return launches;

@@ -74,9 +74,12 @@ __device__ __forceinline__ float2 lds_pair(const __half* p, float s) {
   return make_float2(f.x * s, f.y * s);
 }
 
-template <class M>
+// LAST = true: the second pass is the last one of the apply (k_cheb_last's job): Y = Z_k goes to the fp64 vector
+// z of the outer loop, rho = r.z is reduced over the grid and the epilogue forms beta; W = Z_{k-1} is not stored.
+template <class M, bool LAST>
 __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
-    const Ctx* __restrict__ ctxp, int step, int wout, int yout, const __grid_constant__ CUtensorMap tmU,
+    const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials, int step, int wout, int yout,
+    const __grid_constant__ CUtensorMap tmU,
     const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmR,
     const __grid_constant__ CUtensorMap tm1, const __grid_constant__ CUtensorMap tm2,
     const __grid_constant__ CUtensorMap tm3) {
@@ -84,12 +87,18 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
   __shared__ PairStage<E> st[kPairStages];
   __shared__ __align__(8) float sW[2][QY][QX];
   __shared__ __align__(8) uint64_t full[kPairStages];
+  __shared__ double red[LAST ? 32 : 1];
+  __shared__ int s_flag;
   const DiaDev& A = ctxp->A;
   const float c1a = (float)ctxp->cheb_c1[step], c2a = (float)ctxp->cheb_c2[step];
   const float c1b = (float)ctxp->cheb_c1[step + 1], c2b = (float)ctxp->cheb_c2[step + 1];
-  float* __restrict__ Wg = (float*)ctxp->cd[wout];
-  float* __restrict__ Yg = (float*)ctxp->cd[yout];
+  float* __restrict__ Wg = (float*)ctxp->cd[LAST ? 0 : wout];
+  float* __restrict__ Yg = (float*)ctxp->cd[LAST ? 0 : yout];
+  double* __restrict__ Zg = ctxp->cz;                 // LAST: z = Z_k in fp64
+  const double* __restrict__ R64 = ctxp->r;           // LAST: r in fp64 for rho = r.z
   __builtin_assume(__isGlobal(Wg)); __builtin_assume(__isGlobal(Yg));
+  __builtin_assume(__isGlobal(Zg)); __builtin_assume(__isGlobal(R64));
+  double acc = 0.0;
   const double* __restrict__ s_layer = A.s_layer;
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
   const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
@@ -116,6 +125,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
     const bool inner = !rim && x >= 0 && x < nxi && y >= 0 && y < nyi;  // nx even: x + 1 < nx with x
     const int64_t c0 = inner ? x + nx * (int64_t)y : 0;
     float* pW = Wg + c0; float* pY = Yg + c0 - np;                       // Y trails W by a plane
+    double* pZ = Zg + c0 - np; const double* pR = R64 + c0 - np;
 
     // box starts: x0 rounded down to 16 bytes of elements (two's complement & works for x0 = -2 too)
     const int xs_f = x0 & ~(PairBox<float>::AL - 1), xs_e = x0 & ~(PairBox<E>::AL - 1);
@@ -161,6 +171,8 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
       constexpr bool HAS_W = decltype(has_w_t)::value;
       float2 w = z2, u_hi = z2, rv = z2, f1p = z2, f2u = z2, f2l = z2, a3u = z2;
       float f1l = 0.f, s = 0.f;
+      double2 rd = make_double2(0.0, 0.0);
+      if (LAST && inner && k >= 1) rd = *reinterpret_cast<const double2*>(pR);   // for Y below; flies during W
       if (HAS_W) {
         // ---- W on plane k: operands from the stage (no bounds predicates: absent = zero x zero)
         const PairStage<E>& T = st[S];
@@ -186,7 +198,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
         a0 += a3l_w.x * (u_lo.x - u_c.x); a1 += a3l_w.y * (u_lo.y - u_c.y);
         w = make_float2(u_c.x + c1a * (u_c.x - zo.x) + c2a * (rv.x - a0),
                         u_c.y + c1a * (u_c.y - zo.y) + c2a * (rv.y - a1));
-        if (inner) *reinterpret_cast<float2*>(pW) = w;
+        if (!LAST && inner) *reinterpret_cast<float2*>(pW) = w;
       }
       __syncthreads();                     // W(k-1) complete, W(k-2) no longer read, stage of plane k consumed
       if (HAS_W) {
@@ -207,8 +219,16 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
           a0 += pf2l.x * (wd.x - w_c.x);   a1 += pf2l.y * (wd.y - w_c.y);
           a0 += pa3u.x * (w.x - w_c.x);    a1 += pa3u.y * (w.y - w_c.y);     // pa3u = 0 on the top plane
           a0 += a3l_y.x * (w_lo.x - w_c.x); a1 += a3l_y.y * (w_lo.y - w_c.y);
-          *reinterpret_cast<float2*>(pY) = make_float2(w_c.x + c1b * (w_c.x - u_lo.x) + c2b * (pr.x - a0),
-                                                       w_c.y + c1b * (w_c.y - u_lo.y) + c2b * (pr.y - a1));
+          const float y0v = w_c.x + c1b * (w_c.x - u_lo.x) + c2b * (pr.x - a0);
+          const float y1v = w_c.y + c1b * (w_c.y - u_lo.y) + c2b * (pr.y - a1);
+          if (LAST) {
+            const double zk0 = (double)y0v, zk1 = (double)y1v;
+            *reinterpret_cast<double2*>(pZ) = make_double2(zk0, zk1);
+            acc = fma(rd.x, zk0, acc);
+            acc = fma(rd.y, zk1, acc);
+          } else {
+            *reinterpret_cast<float2*>(pY) = make_float2(y0v, y1v);
+          }
         }
       }
       // ---- rotate: plane k becomes plane k-1
@@ -217,7 +237,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
       w_lo = w_c; w_c = w;
       a3l_w = a3u;
       u_lo = u_c; u_c = u_hi;
-      pW += np; pY += np;
+      pW += np; pY += np; pZ += np; pR += np;
     };
     constexpr std::true_type HW{};
     constexpr std::false_type NW{};
@@ -232,6 +252,16 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
       else do_step(S1, NW, k);
     } else {
       do_step(S0, NW, k);
+    }
+  }
+  if (LAST) {
+    double a[1] = {acc};
+    if (grid_sum_last_block<1>(a, partials + 3 * kMaxBlocks, &ctl->ticket[5], red, &s_flag) && tid == 0) {
+      const double rho_new = a[0];
+      ctl->beta = ctl->beta_zero ? 0.0 : rho_new / ctl->rho;     // Alg. 1 line 11 (line 3 when restarting)
+      ctl->rho = rho_new;
+      ctl->beta_zero = 0;
+      if (!(rho_new == rho_new) || rho_new <= 0.0) ctl->status = CUTH_SOLVE_BREAKDOWN;   // q(A) not SPD: bad interval
     }
   }
 }

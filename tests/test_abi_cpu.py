@@ -99,27 +99,29 @@ def test_layout_golden_sizes(cu):
 
 def test_cheb_launch_schedule_host_side(cu):
     """cuth_cheb_launches (pure host): k - 1 launches with one pass per kernel (R-C3: the dead k-th SpMV of
-    Alg. 3 is skipped); with two passes per kernel the k - 3 middle passes pair up, FIRST and LAST stay."""
+    Alg. 3 is skipped); with two passes per kernel the k - 3 middle passes pair up, FIRST and LAST stay -- and
+    where the TMA kernel is available (nx % 4 == 0 and a driver that can encode tensor maps) an odd middle pass
+    left over shares its launch with LAST."""
     dz = np.full(16, 1e-6)
-    big = cu.Grid(1024, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # even nx: pairs by default
-    odd = cu.Grid(1023, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # odd nx: never
-    small = cu.Grid(32, 32, 16, 1e-6, 1e-6, dz, None, 1e4)
+    big = cu.Grid(1024, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # nx % 4 == 0
+    even = cu.Grid(34, 32, 16, 1e-6, 1e-6, dz, None, 1e4)              # even nx, not a multiple of 4: no TMA
+    odd = cu.Grid(1023, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # odd nx: never pairs
     mk = lambda prec, k: cu.Opts(prec, 1e-8, 1000, 20, cu.PRECOND_CHEBYSHEV, k, 1e-3, 1.0, cu.CHEB_DEFAULT)
     try:
         for k in (3, 4, 5, 30, 31):
             mids = k - 3
+            plain = (2 + mids // 2 + mids % 2, mids // 2)              # FIRST, pairs, odd MID, LAST
+            fused = (2 + mids // 2, mids // 2 + mids % 2) if mids % 2 else plain   # odd MID + LAST in one launch
             cu.cuth_set_cheb_fusion(1)
             assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == (k - 1, 0)
-            cu.cuth_set_cheb_fusion(2)
-            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
-            assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k)) == (k - 1, 0)
-            assert cu.cuth_cheb_launches(small, mk(cu.FP64, k)) == (k - 1, 0)        # fp64 apply: single passes
-            cu.cuth_set_cheb_fusion(0)
-            assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
-            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
-            assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k)) == (k - 1, 0)
-            cu.cuth_set_cheb_fusion(3)                                 # the non-TMA kernel: same schedule
-            assert cu.cuth_cheb_launches(small, mk(cu.MIXED, k)) == (2 + mids // 2 + mids % 2, mids // 2)
+            for mode in (0, 2):
+                cu.cuth_set_cheb_fusion(mode)
+                assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) in (plain, fused)
+                assert cu.cuth_cheb_launches(even, mk(cu.MIXED, k)) == plain
+                assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k)) == (k - 1, 0)
+                assert cu.cuth_cheb_launches(big, mk(cu.FP64, k)) == (k - 1, 0)          # fp64 apply: single passes
+            cu.cuth_set_cheb_fusion(3)                                 # never the TMA kernel
+            assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == plain
         assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
     finally:
         cu.cuth_set_cheb_fusion(0)
