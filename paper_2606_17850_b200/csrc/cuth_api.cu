@@ -220,6 +220,27 @@ static void* cheb_pair_tma_fn(int code, bool last) {
   if (last) return code == 2 ? (void*)k_cheb_pair_tma<MatF16, true> : (void*)k_cheb_pair_tma<MatF32, true>;
   return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false> : (void*)k_cheb_pair_tma<MatF32, false>;
 }
+// Resident CTAs per SM of the TMA two-pass kernel: built for 4 (64 registers, 47 KB of shared memory).  Fewer can
+// be forced (by requesting unused dynamic shared memory at launch) to study the partly filled last wave of
+// regions -- cfg 3 has 3078 regions = 5.2 waves of 592 but 6.9 waves of 444.  Measured: occupancy wins over wave
+// rounding (pair launch at cfg 3: 0.103 ms with 4, 0.109 with 3, 0.133 with 2; cfg 4: 0.73 / 0.83 ms), so
+// automatic = 4.
+static std::atomic<int> g_pair_occ{0};     // 0 automatic (4), 2..4 forced: cuth_set_pair_occupancy
+static int pair_tma_occupancy(const DiaLayout&) {
+  const int forced = g_pair_occ.load();
+  return (forced >= 2 && forced <= 4) ? forced : 4;
+}
+static unsigned pair_tma_dyn_smem(const DiaLayout& L, int code) {
+  const int occ = pair_tma_occupancy(L);
+  if (occ >= 4) return 0;
+  const size_t stat = (code == 2 ? sizeof(PairStage<__half>) : sizeof(PairStage<float>)) * kPairStages + 4608;
+  const size_t per_cta = (size_t)(227 * 1024) / (size_t)(occ + 1) + 1024;    // too much for occ + 1 CTAs
+  const size_t dyn = per_cta > stat ? per_cta - stat : 0;
+  for (int last = 0; last < 2; ++last)
+    cudaFuncSetAttribute(cheb_pair_tma_fn(code, last != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+  return (unsigned)dyn;
+}
+
 // one two-pass launch outside a graph (cuth_cheb_apply, cuth_profile_kernel)
 static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Workspace& w, int code, const ChebOp& op,
                                cudaStream_t st) {
@@ -228,7 +249,8 @@ static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Work
   PairMaps pm;
   if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur)) {
     void* a[] = {&ctxp, &ctlp, &part, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
-    return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3), dim3(cheb_pair_blocks(L)), dim3(kThreads), a, 0, st);
+    return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3), dim3(cheb_pair_blocks(L)), dim3(kThreads), a,
+                            pair_tma_dyn_smem(L, code), st);
   }
   if (op.kind == 3) return cudaErrorInvalidValue;      // the fused MID + LAST launch exists only as a TMA kernel
   void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
@@ -278,6 +300,7 @@ struct GraphEntry {
   int pblocks = 0;
   const void* dia = nullptr;   // matrix the tensor maps of the TMA two-pass nodes were made for (else nullptr)
   int64_t tnx = 0, tny = 0;    // ... and its plane dimensions (the maps are baked into the kernel nodes)
+  int tocc = 0;                // ... and the occupancy its TMA nodes were launched for
   int device = -1;
 };
 static std::mutex g_mu;
@@ -285,13 +308,13 @@ static std::unordered_map<const void*, GraphEntry> g_graphs;
 static std::unordered_map<const void*, const void*> g_last_dia;   // workspace -> matrix of its last solve (profile hook)
 
 static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* deps, size_t ndeps,
-                              void* func, int blocks, void** args) {
+                              void* func, int blocks, void** args, unsigned dyn_smem = 0) {
   cudaKernelNodeParams kp;
   memset(&kp, 0, sizeof kp);
   kp.func = func;
   kp.gridDim = dim3((unsigned)blocks);
   kp.blockDim = dim3(kThreads);
-  kp.sharedMemBytes = 0;
+  kp.sharedMemBytes = dyn_smem;
   kp.kernelParams = args;
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
@@ -337,7 +360,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
       if ((op.kind == 1 || op.kind == 3) && dia_tma) {
         if (!make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur)) return CUTH_ERR_CUDA;
         void* a[] = {&ctx, &ctl, &partials, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3), pblocks, a));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3), pblocks, a, pair_tma_dyn_smem(*Ltma, code)));
       } else if (op.kind == 1) {
         void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
         CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
@@ -388,7 +411,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
   out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks; out->dia = dia_tma;
-  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; }
+  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; out->tocc = pair_tma_occupancy(*Ltma); }
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
@@ -405,7 +428,8 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
                                it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
                                it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
                                it->second.pblocks != pblocks || it->second.dia != dia_tma ||
-                               (dia_tma && (it->second.tnx != Ltma->nx || it->second.tny != Ltma->ny)))) {
+                               (dia_tma && (it->second.tnx != Ltma->nx || it->second.tny != Ltma->ny ||
+                                            it->second.tocc != pair_tma_occupancy(*Ltma))))) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -794,6 +818,12 @@ int cuth_set_cheb_fusion(int mode) {
   if (mode < 0 || mode > 3) return CUTH_ERR_VALUE;
   g_cheb_pairs.store(mode == 3 ? 2 : mode);
   g_pair_tma.store(mode == 3 ? 1 : 0);
+  return CUTH_OK;
+}
+
+int cuth_set_pair_occupancy(int ctas_per_sm) {
+  if (ctas_per_sm != 0 && (ctas_per_sm < 2 || ctas_per_sm > 4)) return CUTH_ERR_VALUE;
+  g_pair_occ.store(ctas_per_sm);
   return CUTH_OK;
 }
 
