@@ -199,6 +199,8 @@ def main():
                     help="cuth_set_cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel, 3 = 2 without TMA")
     ap.add_argument("--pair-occupancy", type=int, default=0, choices=[0, 2, 3, 4],
                     help="cuth_set_pair_occupancy: resident CTAs/SM of the TMA two-pass Chebyshev kernel (0 auto)")
+    ap.add_argument("--pair-rows", type=int, default=0, choices=[0, 8, 16],
+                    help="cuth_set_pair_rows: region height of the TMA two-pass Chebyshev kernel (0 auto)")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
                     help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,
@@ -224,6 +226,7 @@ def main():
     cu.cuth_set_traversal(args.traversal)
     cu.cuth_set_cheb_fusion(args.cheb_fusion)
     cu.cuth_set_pair_occupancy(args.pair_occupancy)
+    cu.cuth_set_pair_rows(args.pair_rows)
     w = W.make_workload(args.config)
     mixed = w.mixed if args.precision is None else (args.precision == "mixed")
     prec = cu.MIXED if mixed else cu.FP64

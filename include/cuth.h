@@ -155,6 +155,10 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid);
  * fastest on every grid), 2..4 = forced (for studying occupancy against the partly filled last wave of regions). */
 int cuth_set_pair_occupancy(int ctas_per_sm);
 
+/* Tuning knob, process-wide: rows of a region of the TMA two-pass Chebyshev kernel (one warp per row): 8 (256
+ * threads, 4 CTAs/SM) or 16 (512 threads, 2 CTAs/SM, a sixth less rim recomputation); 0 = automatic. */
+int cuth_set_pair_rows(int rows);
+
 /* Kernel launches of ONE Chebyshev apply (Alg. 3) for this grid and these options: the first
  * pass, the middle passes (single, or two per launch -- see cuth_set_cheb_fusion) and the last pass; 0 when the
  * preconditioner is not Chebyshev, negative on bad arguments.  *pairs_out (may be NULL) = how many of them are

@@ -51,7 +51,7 @@ class cuth_result_t(C.Structure):
 
 EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy"]
+           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy", "cuth_set_pair_rows"]
 
 _lib = None
 
@@ -264,6 +264,12 @@ def cuth_set_pair_occupancy(ctas_per_sm: int):
     L = load_library()
     L.cuth_set_pair_occupancy.restype = C.c_int
     _check(L.cuth_set_pair_occupancy(C.c_int(int(ctas_per_sm))), "cuth_set_pair_occupancy")
+
+
+def cuth_set_pair_rows(rows: int):
+    L = load_library()
+    L.cuth_set_pair_rows.restype = C.c_int
+    _check(L.cuth_set_pair_rows(C.c_int(int(rows))), "cuth_set_pair_rows")
 
 
 def cuth_set_k1_variant(mode: int):

@@ -206,19 +206,36 @@ static bool make_box_map(CUtensorMap* m, const void* base, bool half, const DiaL
 }
 struct PairMaps { CUtensorMap u, v, r, f1, f2, f3; };
 static bool make_pair_maps(PairMaps* pm, const DiaLayout& L, const void* dia_D, const Workspace& w, int code,
-                           int old, int cur) {
+                           int old, int cur, int ry) {
   const DiaDev A = dev_view(dia_D, L);
   const void* cd[4] = {w.cd0, w.cd1, w.cd2, w.cd3};
   const bool h = code == 2;
-  return make_box_map(&pm->u, cd[cur], false, L, QY + 2) && make_box_map(&pm->v, cd[old], false, L, QY) &&
-         make_box_map(&pm->r, w.crc, false, L, QY) &&
-         make_box_map(&pm->f1, h ? (const void*)A.h1 : (const void*)A.f1, h, L, QY) &&
-         make_box_map(&pm->f2, h ? (const void*)A.h2 : (const void*)A.f2, h, L, QY + 1) &&
-         make_box_map(&pm->f3, h ? (const void*)A.h3 : (const void*)A.f3, h, L, QY);
+  return make_box_map(&pm->u, cd[cur], false, L, ry + 2) && make_box_map(&pm->v, cd[old], false, L, ry) &&
+         make_box_map(&pm->r, w.crc, false, L, ry) &&
+         make_box_map(&pm->f1, h ? (const void*)A.h1 : (const void*)A.f1, h, L, ry) &&
+         make_box_map(&pm->f2, h ? (const void*)A.h2 : (const void*)A.f2, h, L, ry + 1) &&
+         make_box_map(&pm->f3, h ? (const void*)A.h3 : (const void*)A.f3, h, L, ry);
 }
-static void* cheb_pair_tma_fn(int code, bool last) {
-  if (last) return code == 2 ? (void*)k_cheb_pair_tma<MatF16, true> : (void*)k_cheb_pair_tma<MatF32, true>;
-  return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false> : (void*)k_cheb_pair_tma<MatF32, false>;
+static void* cheb_pair_tma_fn(int code, bool last, int ry) {
+  if (ry == 16) {
+    if (last) return code == 2 ? (void*)k_cheb_pair_tma<MatF16, true, 16> : (void*)k_cheb_pair_tma<MatF32, true, 16>;
+    return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false, 16> : (void*)k_cheb_pair_tma<MatF32, false, 16>;
+  }
+  if (last) return code == 2 ? (void*)k_cheb_pair_tma<MatF16, true, 8> : (void*)k_cheb_pair_tma<MatF32, true, 8>;
+  return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false, 8> : (void*)k_cheb_pair_tma<MatF32, false, 8>;
+}
+// Region height of the TMA kernel: 16 rows (512 threads) recompute a sixth less than 8 rows; taken when the
+// plane still gives every SM several regions.  cuth_set_pair_rows forces it.
+static std::atomic<int> g_pair_rows{0};    // 0 automatic, 8, 16
+static int pair_tma_rows(const DiaLayout& L) {
+  const int forced = g_pair_rows.load();
+  if (forced == 8 || forced == 16) return forced;
+  const int64_t tiles16 = ((L.nx + QIX - 1) / QIX) * ((L.ny + 13) / 14);
+  return tiles16 >= 4 * 296 ? 16 : 8;
+}
+static int pair_tma_blocks(const DiaLayout& L, int ry) {
+  const int64_t tiles = ((L.nx + QIX - 1) / QIX) * ((L.ny + ry - 3) / (ry - 2));
+  return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 // Resident CTAs per SM of the TMA two-pass kernel: built for 4 (64 registers, 47 KB of shared memory).  Fewer can
 // be forced (by requesting unused dynamic shared memory at launch) to study the partly filled last wave of
@@ -230,15 +247,18 @@ static int pair_tma_occupancy(const DiaLayout&) {
   const int forced = g_pair_occ.load();
   return (forced >= 2 && forced <= 4) ? forced : 4;
 }
-static unsigned pair_tma_dyn_smem(const DiaLayout& L, int code) {
-  const int occ = pair_tma_occupancy(L);
-  if (occ >= 4) return 0;
-  const size_t stat = (code == 2 ? sizeof(PairStage<__half>) : sizeof(PairStage<float>)) * kPairStages + 4608;
-  const size_t per_cta = (size_t)(227 * 1024) / (size_t)(occ + 1) + 1024;    // too much for occ + 1 CTAs
-  const size_t dyn = per_cta > stat ? per_cta - stat : 0;
+static unsigned pair_tma_dyn_smem(const DiaLayout& L, int code, int ry) {
+  size_t need;
+  if (ry == 16) need = code == 2 ? sizeof(PairSmem<__half, 16>) : sizeof(PairSmem<float, 16>);
+  else need = code == 2 ? sizeof(PairSmem<__half, 8>) : sizeof(PairSmem<float, 8>);
+  const int full_occ = ry == 16 ? 2 : 4, occ = pair_tma_occupancy(L) * full_occ / 4;
+  if (occ >= 1 && occ < full_occ) {                   // forced lower occupancy: too much for occ + 1 CTAs
+    const size_t per_cta = (size_t)(227 * 1024) / (size_t)(occ + 1) + 1024;
+    if (per_cta > need) need = per_cta;
+  }
   for (int last = 0; last < 2; ++last)
-    cudaFuncSetAttribute(cheb_pair_tma_fn(code, last != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-  return (unsigned)dyn;
+    cudaFuncSetAttribute(cheb_pair_tma_fn(code, last != 0, ry), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need);
+  return (unsigned)need;
 }
 
 // one two-pass launch outside a graph (cuth_cheb_apply, cuth_profile_kernel)
@@ -247,10 +267,11 @@ static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Work
   Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
   PairMaps pm;
-  if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur)) {
+  const int ry = pair_tma_rows(L);
+  if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur, ry)) {
     void* a[] = {&ctxp, &ctlp, &part, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
-    return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3), dim3(cheb_pair_blocks(L)), dim3(kThreads), a,
-                            pair_tma_dyn_smem(L, code), st);
+    return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3, ry), dim3(pair_tma_blocks(L, ry)), dim3(32 * ry), a,
+                            pair_tma_dyn_smem(L, code, ry), st);
   }
   if (op.kind == 3) return cudaErrorInvalidValue;      // the fused MID + LAST launch exists only as a TMA kernel
   void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
@@ -308,12 +329,12 @@ static std::unordered_map<const void*, GraphEntry> g_graphs;
 static std::unordered_map<const void*, const void*> g_last_dia;   // workspace -> matrix of its last solve (profile hook)
 
 static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGraphNode_t* deps, size_t ndeps,
-                              void* func, int blocks, void** args, unsigned dyn_smem = 0) {
+                              void* func, int blocks, void** args, unsigned dyn_smem = 0, int threads = kThreads) {
   cudaKernelNodeParams kp;
   memset(&kp, 0, sizeof kp);
   kp.func = func;
   kp.gridDim = dim3((unsigned)blocks);
-  kp.blockDim = dim3(kThreads);
+  kp.blockDim = dim3((unsigned)threads);
   kp.sharedMemBytes = dyn_smem;
   kp.kernelParams = args;
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
@@ -358,9 +379,11 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
       int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
       PairMaps pm;
       if ((op.kind == 1 || op.kind == 3) && dia_tma) {
-        if (!make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur)) return CUTH_ERR_CUDA;
+        const int ry = pair_tma_rows(*Ltma);
+        if (!make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur, ry)) return CUTH_ERR_CUDA;
         void* a[] = {&ctx, &ctl, &partials, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3), pblocks, a, pair_tma_dyn_smem(*Ltma, code)));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3, ry), pair_tma_blocks(*Ltma, ry), a,
+                      pair_tma_dyn_smem(*Ltma, code, ry), 32 * ry));
       } else if (op.kind == 1) {
         void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
         CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
@@ -411,7 +434,7 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
   out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks; out->dia = dia_tma;
-  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; out->tocc = pair_tma_occupancy(*Ltma); }
+  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; out->tocc = pair_tma_occupancy(*Ltma) * 100 + pair_tma_rows(*Ltma); }
   cudaGetDevice(&out->device);
   return CUTH_OK;
 }
@@ -429,7 +452,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
                                it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
                                it->second.pblocks != pblocks || it->second.dia != dia_tma ||
                                (dia_tma && (it->second.tnx != Ltma->nx || it->second.tny != Ltma->ny ||
-                                            it->second.tocc != pair_tma_occupancy(*Ltma))))) {
+                                            it->second.tocc != pair_tma_occupancy(*Ltma) * 100 + pair_tma_rows(*Ltma))))) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -818,6 +841,12 @@ int cuth_set_cheb_fusion(int mode) {
   if (mode < 0 || mode > 3) return CUTH_ERR_VALUE;
   g_cheb_pairs.store(mode == 3 ? 2 : mode);
   g_pair_tma.store(mode == 3 ? 1 : 0);
+  return CUTH_OK;
+}
+
+int cuth_set_pair_rows(int rows) {
+  if (rows != 0 && rows != 8 && rows != 16) return CUTH_ERR_VALUE;
+  g_pair_rows.store(rows);
   return CUTH_OK;
 }
 

@@ -29,17 +29,28 @@ template <class E> struct PairBox {
   static constexpr int AL = 16 / (int)sizeof(E);     // elements per 16 bytes
   static constexpr int W = QX + AL;                  // box width in elements
 };
-template <class E>
+// RY = rows of the region (one warp each): 8 (256 threads, 4 CTAs/SM, 360 of 512 cells interior) or 16 (512
+// threads, 2 CTAs/SM, 840 of 1024 interior: a sixth less recomputation for the same number of resident warps).
+template <class E, int RY>
 struct PairStage {                         // every member starts on a 128-byte boundary (TMA destination)
-  alignas(128) float u[QY + 2][PairBox<float>::W];   // rows y0-1 .. y0+QY of U
-  alignas(128) float v[QY][PairBox<float>::W];
-  alignas(128) float r[QY][PairBox<float>::W];
-  alignas(128) E f1[QY][PairBox<E>::W];
-  alignas(128) E f2[QY + 1][PairBox<E>::W];          // rows y0-1 .. y0+QY-1: the entry towards y-1 is the row above's
-  alignas(128) E f3[QY][PairBox<E>::W];
+  alignas(128) float u[RY + 2][PairBox<float>::W];   // rows y0-1 .. y0+RY of U
+  alignas(128) float v[RY][PairBox<float>::W];
+  alignas(128) float r[RY][PairBox<float>::W];
+  alignas(128) E f1[RY][PairBox<E>::W];
+  alignas(128) E f2[RY + 1][PairBox<E>::W];          // rows y0-1 .. y0+RY-1: the entry towards y-1 is the row above's
+  alignas(128) E f3[RY][PairBox<E>::W];
   // bytes the six boxes deliver (the padding between members is not part of any box)
-  static constexpr uint32_t kTxBytes = sizeof(float) * PairBox<float>::W * (QY + 2 + QY + QY) +
-                                       sizeof(E) * PairBox<E>::W * (QY + QY + 1 + QY);
+  static constexpr uint32_t kTxBytes = sizeof(float) * PairBox<float>::W * (RY + 2 + RY + RY) +
+                                       sizeof(E) * PairBox<E>::W * (RY + RY + 1 + RY);
+};
+// dynamic shared memory of the kernel: stages | W ring | mbarriers | reduction scratch | flag
+template <class E, int RY>
+struct PairSmem {
+  PairStage<E, RY> st[kPairStages];
+  alignas(8) float sW[2][RY][QX];
+  alignas(8) uint64_t full[kPairStages];
+  double red[32];
+  int s_flag;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -76,19 +87,20 @@ __device__ __forceinline__ float2 lds_pair(const __half* p, float s) {
 
 // LAST = true: the second pass is the last one of the apply (k_cheb_last's job): Y = Z_k goes to the fp64 vector
 // z of the outer loop, rho = r.z is reduced over the grid and the epilogue forms beta; W = Z_{k-1} is not stored.
-template <class M, bool LAST>
-__global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
+template <class M, bool LAST, int RY>
+__global__ void __launch_bounds__(32 * RY, RY == 8 ? 4 : 2) k_cheb_pair_tma(
     const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials, int step, int wout, int yout,
     const __grid_constant__ CUtensorMap tmU,
     const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmR,
     const __grid_constant__ CUtensorMap tm1, const __grid_constant__ CUtensorMap tm2,
     const __grid_constant__ CUtensorMap tm3) {
   using E = typename M::elem;
-  __shared__ PairStage<E> st[kPairStages];
-  __shared__ __align__(8) float sW[2][QY][QX];
-  __shared__ __align__(8) uint64_t full[kPairStages];
-  __shared__ double red[LAST ? 32 : 1];
-  __shared__ int s_flag;
+  extern __shared__ __align__(128) unsigned char pair_smem_raw[];
+  PairSmem<E, RY>& sm = *reinterpret_cast<PairSmem<E, RY>*>(pair_smem_raw);
+  PairStage<E, RY>* st = sm.st;
+  float (*sW)[RY][QX] = sm.sW;
+  uint64_t* full = sm.full;
+  constexpr int QIYr = RY - 2;                        // interior rows written by this CTA
   const DiaDev& A = ctxp->A;
   const float c1a = (float)ctxp->cheb_c1[step], c2a = (float)ctxp->cheb_c2[step];
   const float c1b = (float)ctxp->cheb_c1[step + 1], c2b = (float)ctxp->cheb_c2[step + 1];
@@ -102,14 +114,14 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
   const double* __restrict__ s_layer = A.s_layer;
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
   const int nxi = (int)A.nx, nyi = A.ny, nz = A.nz;
-  const int tiles_x = (nxi + QIX - 1) / QIX, tiles_y = (nyi + QIY - 1) / QIY;
+  const int tiles_x = (nxi + QIX - 1) / QIX, tiles_y = (nyi + QIYr - 1) / QIYr;
   const int ntiles = tiles_x * tiles_y;
   const int64_t nx = A.nx, np = A.nxny;
   const float ms = M::inv(A);
   const float2 z2 = make_float2(0.f, 0.f);
-  const bool rim = tx == 0 || tx == 31 || ty == 0 || ty == QY - 1;
+  const bool rim = tx == 0 || tx == 31 || ty == 0 || ty == RY - 1;
   constexpr unsigned kAll = 0xffffffffu;
-  constexpr uint32_t kStageBytes = PairStage<E>::kTxBytes;
+  constexpr uint32_t kStageBytes = PairStage<E, RY>::kTxBytes;
 
   if (tid == 0) {
     for (int s = 0; s < kPairStages; ++s) mbar_init(&full[s], 1);
@@ -120,7 +132,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
   uint32_t ph = 0;                         // bit S: parity of the next fill of stage S to wait for
   for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
     const int bx = t % tiles_x, by = t / tiles_x;
-    const int x0 = bx * QIX - 2, y0 = by * QIY - 1;                    // region origin (x0 even)
+    const int x0 = bx * QIX - 2, y0 = by * QIYr - 1;                   // region origin (x0 even)
     const int x = x0 + 2 * tx, y = y0 + ty;
     const bool inner = !rim && x >= 0 && x < nxi && y >= 0 && y < nyi;  // nx even: x + 1 < nx with x
     const int64_t c0 = inner ? x + nx * (int64_t)y : 0;
@@ -175,7 +187,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
       if (LAST && inner && k >= 1) rd = *reinterpret_cast<const double2*>(pR);   // for Y below; flies during W
       if (HAS_W) {
         // ---- W on plane k: operands from the stage (no bounds predicates: absent = zero x zero)
-        const PairStage<E>& T = st[S];
+        const PairStage<E, RY>& T = st[S];
         const float2 v2u = lds_pair(&T.u[ty + 2][cf], 1.f), v2l = lds_pair(&T.u[ty][cf], 1.f);
         const float2 zo = lds_pair(&T.v[ty][cf], 1.f);
         rv = lds_pair(&T.r[ty][cf], 1.f);
@@ -256,7 +268,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_cheb_pair_tma(
   }
   if (LAST) {
     double a[1] = {acc};
-    if (grid_sum_last_block<1>(a, partials + 3 * kMaxBlocks, &ctl->ticket[5], red, &s_flag) && tid == 0) {
+    if (grid_sum_last_block<1>(a, partials + 3 * kMaxBlocks, &ctl->ticket[5], sm.red, &sm.s_flag) && tid == 0) {
       const double rho_new = a[0];
       ctl->beta = ctl->beta_zero ? 0.0 : rho_new / ctl->rho;     // Alg. 1 line 11 (line 3 when restarting)
       ctl->rho = rho_new;

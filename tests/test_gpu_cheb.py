@@ -206,7 +206,7 @@ SHAPES = [(4, 2, 2), (8, 6, 3), (12, 9, 5), (64, 8, 2), (60, 6, 4), (68, 10, 4),
 def test_cheb_apply_kernel_variants_agree(shape, degree, storage, traversal):
     """The same polynomial through the three kernel schedules of the fp32 apply -- one pass per kernel, two
     passes per kernel with ordinary loads, two passes per kernel with TMA-staged operands (taken when nx % 4 == 0,
-    fp16: % 8) -- on shapes below, at and above one 60 x 6 region, with per-cell conductivities: every row runs
+    fp16: % 8; regions of 8 and of 16 rows) -- on shapes below, at and above one 60 x 6 region, with per-cell conductivities: every row runs
     the same arithmetic, so the results agree to fp32 rounding of the order of operations."""
     import torch
     import paper_2606_17850_b200 as cu
@@ -217,17 +217,20 @@ def test_cheb_apply_kernel_variants_agree(shape, degree, storage, traversal):
     r = W.normal01(w.seed, 52, 53, np.arange(w.n)) * 1e-7
     out = {}
     try:
-        for mode in (1, 3, 2):
+        for mode, rows in ((1, 0), (3, 0), (2, 8), (2, 16)):      # rows: region height of the TMA kernel
             cu.cuth_set_cheb_fusion(mode)
+            cu.cuth_set_pair_rows(rows)
             z = torch.full((w.n,), float("nan"), dtype=torch.float64, device="cuda")
             S.cheb_apply(to_dev(r), z)
-            out[mode] = z.cpu().numpy()
+            out[(mode, rows)] = z.cpu().numpy()
     finally:
         cu.cuth_set_cheb_fusion(1)
-    assert np.isfinite(out[1]).all()
-    scale = np.abs(out[1]).max()
-    for mode in (3, 2):
-        assert np.abs(out[mode] - out[1]).max() <= 2e-5 * scale, (mode, shape)
+        cu.cuth_set_pair_rows(0)
+    ref = out[(1, 0)]
+    assert np.isfinite(ref).all()
+    scale = np.abs(ref).max()
+    for key in ((3, 0), (2, 8), (2, 16)):
+        assert np.abs(out[key] - ref).max() <= 2e-5 * scale, (key, shape)
 
 
 @pytest.mark.parametrize("traversal", ["flat-pairs"], indirect=True)
