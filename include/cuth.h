@@ -34,7 +34,9 @@ typedef enum {
   CUTH_ERR_SIZE = -4,        /* caller's buffer too small */
   CUTH_ERR_ALIGN = -5,       /* device pointer not 16-byte aligned */
   CUTH_ERR_CUDA = -6,        /* a CUDA runtime call failed (see cuth_last_cuda_error) */
-  CUTH_ERR_NOT_TRANSIENT = -7 /* cuth_transient_step on a matrix built without cvol/dt */
+  CUTH_ERR_NOT_TRANSIENT = -7,/* cuth_transient_step on a matrix built without cvol/dt (or on an imported matrix) */
+  CUTH_ERR_STRUCTURE = -8,    /* cuth_import_csr: the matrix is not a symmetric 7-point matrix of this grid (see the report) */
+  CUTH_ERR_FP64_ONLY = -9     /* MIXED requested on an imported matrix whose row sums are not constant per layer */
 } cuth_status_t;
 
 /* result_D->status values (device-side, numerical outcome of a solve) */
@@ -104,6 +106,39 @@ size_t cuth_workspace_bytes(const cuth_grid_t* grid, const cuth_opts_t* opts);
  * operator.  Arithmetic: fp64 without FMA contraction, in the order DESIGN.md §4 states, so
  * values are bit-identical to the oracle's.  dia_D: device buffer of >= cuth_dia_bytes(). */
 int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void* stream);
+
+/* What cuth_import_csr found.  The first four counts must all be zero for the import to succeed. */
+typedef struct {
+  int64_t off_stencil;        /* non-zero entries whose column is not row + {0, +-1, +-nx, +-nx*ny}, is out of range, or
+                                 couples x = nx-1 with x = 0 of the next line / y = ny-1 with y = 0 of the next plane */
+  int64_t asymmetric_rows;    /* rows with a lower-triangle entry that differs from its mirror (absent == 0) */
+  int64_t bad_diagonal;       /* rows whose main-diagonal entry is missing, not positive or not finite */
+  int64_t duplicates;         /* entries that repeat a column already seen in their row */
+  int64_t positive_offdiag;   /* off-diagonal entries > 0: information only (a conductance matrix has none) */
+  double max_rowsum_dev;      /* max over rows of |row sum - s(layer)| / (smallest diagonal entry of the layer) */
+  int32_t mixed_ok;           /* 1: the row sums are constant per layer to 1e-9, so CUTH_MIXED is available */
+} cuth_import_report_t;
+
+/* Importer (the paper's matrices are sparse matrices exported by 3D-ICE, which
+ * PAPER.md:219 then "decomposes and stores as a set of diagonal vectors").  Takes a square CSR matrix of order
+ * nx*ny*nz on the DEVICE (rowptr int64 [n+1], col int32 [nnz], val fp64 [nnz]; columns in any order within a row),
+ * checks that it is a symmetric matrix with a positive diagonal whose non-zeros all sit on the seven diagonals
+ * {0, +-1, +-nx, +-nx*ny} of the box and never couple across an x / y edge, and writes the same matrix object
+ * cuth_build_dia writes: the main and the three upper diagonals are copied BIT-EXACT into the packed layout (a
+ * missing entry is +0.0), then A2, 1/D0, A3 are derived as in the builder.  Only nx, ny, nz of `grid` are used
+ * (dx, dy, h_top must still be valid numbers).  rowsum_layer_H: NULL, or [nz] exact row sums s(z) of the operator
+ * per layer (physically h*dx*dy on the top layer plus C*V/dt); the MIXED operator is applied
+ * in difference form and needs them (DESIGN.md R-F3).  With NULL they are taken from the matrix (midrange of the
+ * layer's computed row sums, clamped at 0); if the rows of a layer do not agree to 1e-9 of the layer's smallest
+ * diagonal entry the matrix is usable in CUTH_FP64 only (report->mixed_ok = 0; MIXED calls return
+ * CUTH_ERR_FP64_ONLY), and if a supplied rowsum_layer_H disagrees the call fails with CUTH_ERR_STRUCTURE.
+ * Imported matrices are steady operators for this library: cuth_transient_step returns CUTH_ERR_NOT_TRANSIENT
+ * (form b = P + (C V/dt) T_n yourself and call cuth_pcg_solve).
+ * report_H (host, may be NULL) is always filled.  This call SYNCHRONISES `stream` (setup, not hot path).
+ * On CUTH_ERR_STRUCTURE the contents of dia_D are unspecified. */
+int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
+                    const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
+                    void* stream);
 
 /* View of the matrix object for the bit-exact layout test: device pointers to the packed fp64
  * values and to the fp32 copy (same ptr/off), and the host copies of ptr[5], off[4].

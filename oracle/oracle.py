@@ -94,6 +94,71 @@ def csr_to_dia(A: CSR, nx, ny, nz):
     return vals, ptr, off
 
 
+def stencil7_report(A: CSR, nx, ny, nz) -> dict:
+    """Is this CSR matrix a symmetric 7-point matrix of the nx x ny x nz box?  The definition written out entry by
+    entry (SURVEY.md §8(f) importer; the diagonals are those of PAPER.md:219 / Alg. 2):
+    an entry (i, j) is ON the stencil when j - i is one of {0, +-1, +-nx, +-nx*ny}, 0 <= j < n, and a +-1 / +-nx
+    step stays inside the line / plane of cell i.  Counts: non-zero entries off the stencil; repeats of an on-stencil
+    (i, j); rows whose first diagonal entry is missing, <= 0 or not finite; rows where a lower on-stencil entry
+    differs from its mirror (absent == 0); on-stencil off-diagonal entries > 0; and the largest deviation of a row
+    sum from the midrange row sum of its layer, relative to the layer's smallest diagonal entry."""
+    n = nx * ny * nz
+    nxny = nx * ny
+    first = {}
+    off_stencil = duplicates = positive = 0
+    for i in range(n):
+        x, y = i % nx, (i % nxny) // nx
+        for q in range(int(A.rowptr[i]), int(A.rowptr[i + 1])):
+            j, v = int(A.col[q]), float(A.val[q])
+            c = j - i
+            on = 0 <= j < n and c in (0, 1, -1, nx, -nx, nxny, -nxny)
+            if on and c == 1:
+                on = x + 1 < nx
+            if on and c == -1:
+                on = x > 0
+            if on and c == nx:
+                on = y + 1 < ny
+            if on and c == -nx:
+                on = y > 0
+            if not on:
+                off_stencil += 1 if v != 0.0 else 0
+                continue
+            if (i, j) in first:
+                duplicates += 1
+                continue
+            first[(i, j)] = v
+            if c != 0 and v > 0.0:
+                positive += 1
+    bad_diagonal = sum(1 for i in range(n) if not (first.get((i, i), 0.0) > 0.0 and np.isfinite(first[(i, i)])))
+    asymmetric_rows = 0
+    rowsum = np.zeros(n)
+    for i in range(n):
+        bad = False
+        rs = first.get((i, i), 0.0)
+        for o in (nxny, nx, 1):
+            if i - o >= 0:
+                bad = bad or first.get((i, i - o), 0.0) != first.get((i - o, i), 0.0)
+                rs += first.get((i - o, i), 0.0)
+        for o in (1, nx, nxny):
+            if i + o < n:
+                rs += first.get((i, i + o), 0.0)
+        asymmetric_rows += 1 if bad else 0
+        rowsum[i] = rs
+    dev = 0.0
+    s_layer = np.zeros(nz)
+    for z in range(nz):
+        rs = rowsum[z * nxny:(z + 1) * nxny]
+        d = np.array([first.get((i, i), 0.0) for i in range(z * nxny, (z + 1) * nxny)])
+        s = max(0.0, 0.5 * (rs.min() + rs.max()))
+        s_layer[z] = s
+        dmin = d.min() if d.min() > 0 else 1.0
+        dev = max(dev, max(abs(rs.max() - s), abs(rs.min() - s)) / dmin)
+    ok = off_stencil == 0 and duplicates == 0 and bad_diagonal == 0 and asymmetric_rows == 0
+    return dict(off_stencil=off_stencil, asymmetric_rows=asymmetric_rows, bad_diagonal=bad_diagonal,
+                duplicates=duplicates, positive_offdiag=positive, max_rowsum_dev=dev,
+                mixed_ok=int(ok and dev <= 1e-9), s_layer=s_layer)
+
+
 def transient_rhs(w, power: np.ndarray, t_n: np.ndarray) -> np.ndarray:
     b = np.empty(w.n, dtype=np.float64)
     power = np.ascontiguousarray(power, dtype=np.float64)

@@ -16,7 +16,8 @@ PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV = 0, 1, 2
 CHEB_DEFAULT, CHEB_A3_FP16 = 0, 1
 STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}
 _ERR = {-1: "CUTH_ERR_NULL", -2: "CUTH_ERR_DIMS", -3: "CUTH_ERR_VALUE", -4: "CUTH_ERR_SIZE",
-        -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT"}
+        -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT", -8: "CUTH_ERR_STRUCTURE",
+        -9: "CUTH_ERR_FP64_ONLY"}
 
 
 class CuthError(RuntimeError):
@@ -49,7 +50,13 @@ class cuth_result_t(C.Structure):
                 ("switch_iteration", C.c_int32)]
 
 
-EXPORTS = ["cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
+class cuth_import_report_t(C.Structure):
+    _fields_ = [("off_stencil", C.c_int64), ("asymmetric_rows", C.c_int64), ("bad_diagonal", C.c_int64),
+                ("duplicates", C.c_int64), ("positive_offdiag", C.c_int64), ("max_rowsum_dev", C.c_double),
+                ("mixed_ok", C.c_int32)]
+
+
+EXPORTS = ["cuth_import_csr", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
            "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy", "cuth_set_pair_rows"]
 
@@ -76,6 +83,8 @@ def load_library():
     L.cuth_workspace_bytes.argtypes = [gp, op]
     L.cuth_build_dia.restype = C.c_int
     L.cuth_build_dia.argtypes = [gp, vp, C.c_size_t, vp]
+    L.cuth_import_csr.restype = C.c_int
+    L.cuth_import_csr.argtypes = [gp, vp, vp, vp, vp, vp, C.c_size_t, C.POINTER(cuth_import_report_t), vp]
     L.cuth_dia_view.restype = C.c_int
     L.cuth_dia_view.argtypes = [vp, gp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                 C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -180,6 +189,22 @@ def cuth_workspace_bytes(grid: Grid, opts) -> int:
 def cuth_build_dia(grid: Grid, dia, stream=None):
     _check(load_library().cuth_build_dia(grid.ref(), _ptr(dia), dia.numel() * dia.element_size(),
                                          stream or _stream()), "cuth_build_dia")
+
+
+def cuth_import_csr(grid: Grid, rowptr, col, val, dia, rowsum_layer=None, stream=None, check=True):
+    """rowptr int64 / col int32 / val float64 CUDA tensors.  Returns the cuth_import_report_t; raises CuthError on
+    failure unless check=False (then returns (rc, report)).  Synchronises the stream."""
+    import torch
+    assert rowptr.dtype == torch.int64 and col.dtype == torch.int32 and val.dtype == torch.float64
+    rep = cuth_import_report_t()
+    rs = None if rowsum_layer is None else np.ascontiguousarray(rowsum_layer, dtype=np.float64)
+    rc = load_library().cuth_import_csr(grid.ref(), _ptr(rowptr), _ptr(col), _ptr(val),
+                                        None if rs is None else rs.ctypes.data_as(C.c_void_p), _ptr(dia),
+                                        dia.numel() * dia.element_size(), C.byref(rep), stream or _stream())
+    if not check:
+        return rc, rep
+    _check(rc, "cuth_import_csr")
+    return rep
 
 
 def cuth_dia_view(dia, grid: Grid):
@@ -296,9 +321,10 @@ def cuth_launches_per_iteration(grid: Grid) -> int:
 
 # ------------------------------------------------------------------ convenience holders (allocation only)
 class DiaMatrix:
-    """Allocates the matrix buffer with torch and calls cuth_build_dia."""
+    """Allocates the matrix buffer with torch and calls cuth_build_dia (or, with csr=(rowptr, col, val) CUDA
+    tensors, cuth_import_csr)."""
 
-    def __init__(self, grid: Grid):
+    def __init__(self, grid: Grid, csr=None, rowsum_layer=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("cuth needs a CUDA device (no CPU fallback)")
@@ -307,7 +333,11 @@ class DiaMatrix:
         if nbytes == 0:
             raise CuthError(-2, "cuth_dia_bytes")
         self.buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
-        cuth_build_dia(grid, self.buf)
+        self.import_report = None
+        if csr is None:
+            cuth_build_dia(grid, self.buf)
+        else:
+            self.import_report = cuth_import_csr(grid, csr[0], csr[1], csr[2], self.buf, rowsum_layer)
 
     def view(self):
         """(vals fp64 [E], vals32 fp32 [E], inv_diag fp64 [N], ptr, off) as torch views of the buffer."""

@@ -24,6 +24,9 @@
 namespace cuth {
 
 int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStream_t st, cudaError_t* err);
+int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowptr_D, const int32_t* col_D,
+                  const double* val_D, const double* rowsum_layer_H, void* dia_D, cuth_import_report_t* rep,
+                  cudaStream_t st, cudaError_t* err);
 
 static thread_local std::string g_last_err;
 
@@ -37,6 +40,16 @@ static int cuda_fail(cudaError_t e, const char* what) {
 #define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cuda_fail(e_, #x); } while (0)
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+// Matrix objects written by cuth_import_csr, by address: 1 = MIXED available, 0 = FP64 only.  Host-side knowledge
+// only (the solver never reads the device header back); cuth_build_dia on the same buffer removes the entry.
+static std::mutex g_imp_mu;
+static std::unordered_map<const void*, int> g_imported;
+static int imported_state(const void* dia_D) {   // -1 not imported
+  std::lock_guard<std::mutex> lk(g_imp_mu);
+  auto it = g_imported.find(dia_D);
+  return it == g_imported.end() ? -1 : it->second;
+}
 
 static int check_grid(const cuth_grid_t* g, DiaLayout* L) {
   if (!g) return CUTH_ERR_NULL;
@@ -543,6 +556,9 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
     return CUTH_ERR_ALIGN;
   const bool transient = power_D != nullptr;
   if (transient && !(grid->cvol_H && grid->dt > 0.0)) return CUTH_ERR_NOT_TRANSIENT;
+  const int imp = imported_state(dia_D);
+  if (transient && imp >= 0) return CUTH_ERR_NOT_TRANSIENT;
+  if (imp == 0 && opts->precision == CUTH_MIXED) return CUTH_ERR_FP64_ONLY;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
   const bool cheb = opts->preconditioner == CUTH_PRECOND_CHEBYSHEV;
@@ -650,8 +666,33 @@ int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void*
     if (grid->cvol_H && grid->dt > 0.0 && !(grid->cvol_H[z] > 0.0)) return CUTH_ERR_VALUE;
   }
   cudaError_t e = cudaSuccess;
+  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
   rc = launch_build(grid, L, dia_D, (cudaStream_t)stream, &e);
   if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_build_dia");
+  return rc;
+}
+
+int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
+                    const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
+                    void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  if (!dia_D || !rowptr_D || !col_D || !val_D) return CUTH_ERR_NULL;
+  if (!aligned16(dia_D) || ((uintptr_t)rowptr_D & 7u) || ((uintptr_t)col_D & 3u) || ((uintptr_t)val_D & 7u))
+    return CUTH_ERR_ALIGN;
+  if (dia_bytes < L.bytes) return CUTH_ERR_SIZE;
+  if (rowsum_layer_H)
+    for (int64_t z = 0; z < grid->nz; ++z)
+      if (!(rowsum_layer_H[z] >= 0.0) || std::isinf(rowsum_layer_H[z])) return CUTH_ERR_VALUE;
+  cuth_import_report_t rep;
+  memset(&rep, 0, sizeof rep);
+  cudaError_t e = cudaSuccess;
+  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
+  rc = launch_import(grid, L, rowptr_D, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e);
+  if (report_H) *report_H = rep;
+  if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_import_csr");
+  if (rc == CUTH_OK) { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported[dia_D] = rep.mixed_ok; }
   return rc;
 }
 
@@ -678,6 +719,7 @@ int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const d
   if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(y_D)) return CUTH_ERR_ALIGN;
   if (precision != CUTH_FP64 && precision != CUTH_MIXED && precision != CUTH_ABLATION_STD32) return CUTH_ERR_VALUE;
   if (x_D == y_D) return CUTH_ERR_VALUE;
+  if (precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
   DiaDev A = dev_view(dia_D, L);
   const int sb = stencil_blocks(L);
   const int blocks = sb > 0 ? sb : grid_blocks(L.n);
@@ -796,6 +838,7 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   if (!dia_D || !r_D || !z_D || !work_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(r_D) || !aligned16(z_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
+  if (opts->precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
   cudaStream_t st = (cudaStream_t)stream;
   Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, true);
   Ctx c;

@@ -3,6 +3,10 @@
 // three upper diagonals, the fp32 copy A2, and 1/D0.  Every fp64 operation is an explicit
 // round-to-nearest intrinsic (no FMA contraction), in the order stated in DESIGN.md §4, so the
 // stored values can be compared bit for bit with an independently assembled matrix.
+#include <cmath>
+#include <cstring>
+#include <vector>
+
 #include "cuth_internal.cuh"
 
 namespace cuth {
@@ -152,6 +156,219 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
                                                 (float*)(base + L.o_f32a + 2 * L.f32a_stride));
   e = cudaGetLastError();
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+  return CUTH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Importer ("CSR / COO import", PAPER.md:430 -- the paper's matrices arrive as sparse matrices
+// from 3D-ICE and are then "decomposed and stored as a set of diagonal vectors").  A CSR matrix
+// whose structure is the 7-point stencil of an nx x ny x nz box is checked and condensed into the same matrix
+// object cuth_build_dia writes: the four upper diagonals are COPIED (bit-exact), the lower triangle is only
+// compared with its mirror.
+struct ImportArgs {
+  int64_t n, nx, ny, nxny;
+  int32_t nz;
+  const int64_t* rowptr; const int32_t* col; const double* val;
+  double* d0; double* d1; double* d2; double* d3;
+  unsigned long long* cnt;     // [0] off-stencil, [1] asymmetric, [2] bad diagonal, [3] duplicates, [4] positive off-diagonals
+  unsigned long long* rs_min;  // [nz] order-preserving keys of the per-layer min / max row sum and min D0
+  unsigned long long* rs_max;
+  unsigned long long* d0_min;
+};
+
+__device__ __forceinline__ unsigned long long ordered_key(double v) {   // monotone map double -> uint64
+  const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+  return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+
+// Pass 1, one thread per row: the row's own diagonal and upper entries go to their slots (a missing entry is
+// +0.0, which is also what the builder stores where the +x / +y neighbour does not exist).
+__global__ void __launch_bounds__(256) k_import_upper(ImportArgs a) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned long long off_st = 0, bad = 0, dup = 0, pos = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+    const int64_t rem = i % a.nxny;
+    const int64_t x = rem % a.nx, y = rem / a.nx;
+    double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0;
+    unsigned seen = 0;
+    for (int64_t q = a.rowptr[i]; q < a.rowptr[i + 1]; ++q) {
+      const int64_t cq = (int64_t)a.col[q];
+      const int64_t c = cq - i;
+      const double v = a.val[q];
+      int slot = -1;
+      bool legal = cq >= 0 && cq < a.n;
+      if (c == 0) slot = 0;
+      else if (c == 1) { slot = 1; legal = legal && x + 1 < a.nx; }
+      else if (c == a.nx) { slot = 2; legal = legal && y + 1 < a.ny; }
+      else if (c == a.nxny) slot = 3;
+      else if (c == -1) { slot = 4; legal = legal && x > 0; }
+      else if (c == -a.nx) { slot = 5; legal = legal && y > 0; }
+      else if (c == -a.nxny) slot = 6;
+      if (slot < 0 || !legal) { if (v != 0.0) ++off_st; continue; }   // explicit zeros off the stencil are ignored
+      if (seen & (1u << slot)) { ++dup; continue; }
+      seen |= 1u << slot;
+      if (slot == 0) v0 = v; else if (slot == 1) v1 = v; else if (slot == 2) v2 = v; else if (slot == 3) v3 = v;
+      if (slot != 0 && v > 0.0) ++pos;
+    }
+    if (!(seen & 1u) || !(v0 > 0.0) || isinf(v0)) ++bad;
+    a.d0[i] = v0;
+    if (i + 1 < a.n) a.d1[i] = v1;
+    if (i + a.nx < a.n) a.d2[i] = v2;
+    if (i + a.nxny < a.n) a.d3[i] = v3;
+  }
+  if (off_st) atomicAdd(&a.cnt[0], off_st);
+  if (bad) atomicAdd(&a.cnt[2], bad);
+  if (dup) atomicAdd(&a.cnt[3], dup);
+  if (pos) atomicAdd(&a.cnt[4], pos);
+}
+
+// Pass 2, one thread per row: every lower entry must equal the stored mirror (absent == 0), and the row sum
+// D0 + sum of the six off-diagonal entries (fixed order -z, -y, -x, +x, +y, +z) feeds the per-layer min / max.
+__global__ void __launch_bounds__(256) k_import_lower(ImportArgs a) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned long long asym = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+    double l1 = 0.0, l2 = 0.0, l3 = 0.0;
+    unsigned seen = 0;
+    const int64_t rem = i % a.nxny;
+    const bool has_xm = rem % a.nx > 0, has_ym = rem / a.nx > 0;     // edge-crossing entries were counted in pass 1
+    for (int64_t q = a.rowptr[i]; q < a.rowptr[i + 1]; ++q) {
+      const int64_t c = (int64_t)a.col[q] - i;
+      const double v = a.val[q];
+      if (c == -1 && has_xm && !(seen & 1u)) { l1 = v; seen |= 1u; }
+      else if (c == -a.nx && has_ym && !(seen & 2u)) { l2 = v; seen |= 2u; }
+      else if (c == -a.nxny && !(seen & 4u)) { l3 = v; seen |= 4u; }
+    }
+    const double m1 = i >= 1 ? a.d1[i - 1] : 0.0;
+    const double m2 = i >= a.nx ? a.d2[i - a.nx] : 0.0;
+    const double m3 = i >= a.nxny ? a.d3[i - a.nxny] : 0.0;
+    if (!(l1 == m1) || !(l2 == m2) || !(l3 == m3)) ++asym;
+    const double d = a.d0[i];
+    double rs = d;
+    rs = __dadd_rn(rs, m3); rs = __dadd_rn(rs, m2); rs = __dadd_rn(rs, m1);
+    if (i + 1 < a.n) rs = __dadd_rn(rs, a.d1[i]);
+    if (i + a.nx < a.n) rs = __dadd_rn(rs, a.d2[i]);
+    if (i + a.nxny < a.n) rs = __dadd_rn(rs, a.d3[i]);
+    const int64_t z = i / a.nxny;
+    // a full warp inside one layer (the common case) reduces by shuffle: one atomic per warp and quantity
+    unsigned long long kmin = ordered_key(rs), kmax = kmin, kd = ordered_key(d);
+    const unsigned mask = __activemask();
+    bool uniform = false;
+    if (mask == 0xffffffffu) {
+      const int64_t z0 = __shfl_sync(mask, z, 0);
+      uniform = __all_sync(mask, z == z0);
+      if (uniform) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const unsigned long long t1 = __shfl_xor_sync(mask, kmin, o), t2 = __shfl_xor_sync(mask, kmax, o),
+                                   t3 = __shfl_xor_sync(mask, kd, o);
+          kmin = t1 < kmin ? t1 : kmin; kmax = t2 > kmax ? t2 : kmax; kd = t3 < kd ? t3 : kd;
+        }
+      }
+    }
+    if (!uniform || (threadIdx.x & 31) == 0) {
+      atomicMin(&a.rs_min[z], kmin); atomicMax(&a.rs_max[z], kmax); atomicMin(&a.d0_min[z], kd);
+    }
+  }
+  if (asym) atomicAdd(&a.cnt[1], asym);
+}
+
+// fp32 copy A2 (round-to-nearest-even of the packed values) and 1/D0, as the builder writes them.
+__global__ void __launch_bounds__(256) k_import_finish(const double* __restrict__ vals, float* __restrict__ f, int64_t e,
+                                                       double* __restrict__ dinv, int64_t n) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < e; i += stride) {
+    const double v = vals[i];
+    f[i] = __double2float_rn(v);
+    if (i < n) dinv[i] = __ddiv_rn(1.0, v);
+  }
+}
+
+static double key_to_double(unsigned long long k) {
+  const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+  double v;
+  memcpy(&v, &b, sizeof v);
+  return v;
+}
+
+// Host side of cuth_import_csr.  Synchronises `st` (setup call).  rowsum_layer_H may be nullptr.
+int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowptr_D, const int32_t* col_D,
+                  const double* val_D, const double* rowsum_layer_H, void* dia_D, cuth_import_report_t* rep,
+                  cudaStream_t st, cudaError_t* err) {
+  char* base = (char*)dia_D;
+  const int nz = (int)L.nz;
+  const size_t nlay = 4 * (size_t)nz + 4;
+  std::vector<unsigned long long> h(nlay, 0ull);
+  for (int z = 0; z < nz; ++z) { h[z] = ~0ull; h[2 * nz + z] = ~0ull; }   // min slots start at the largest key
+  unsigned long long hdr[kHeaderBytes / 8] = {0};
+  hdr[0] = kMagic; hdr[1] = (unsigned long long)L.nx; hdr[2] = (unsigned long long)L.ny;
+  hdr[3] = (unsigned long long)L.nz; hdr[4] = (unsigned long long)L.e; hdr[5] = 0ull;
+  for (int k = 0; k < 5; ++k) hdr[6 + k] = (unsigned long long)L.ptr[k];
+  for (int k = 0; k < 4; ++k) hdr[11 + k] = (unsigned long long)L.off[k];
+  hdr[15] = 1ull;   // imported
+  cudaError_t e = cudaMemcpyAsync(base, hdr, kHeaderBytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(base + L.o_layers, h.data(), nlay * 8, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+  unsigned long long* lay = (unsigned long long*)(base + L.o_layers);
+  double* v = (double*)(base + L.o_vals);
+  float* f = (float*)(base + L.o_vals32);
+  ImportArgs a;
+  a.n = L.n; a.nx = L.nx; a.ny = L.ny; a.nxny = L.nxny; a.nz = nz;
+  a.rowptr = rowptr_D; a.col = col_D; a.val = val_D;
+  a.d0 = v + L.ptr[0]; a.d1 = v + L.ptr[1]; a.d2 = v + L.ptr[2]; a.d3 = v + L.ptr[3];
+  a.cnt = (unsigned long long*)base + 32;     // header words 32..36
+  a.rs_min = lay; a.rs_max = lay + nz; a.d0_min = lay + 2 * nz;
+  int64_t blocks = (L.n + 255) / 256;
+  if (blocks > 148 * 64) blocks = 148 * 64;
+  k_import_upper<<<(unsigned)blocks, 256, 0, st>>>(a);
+  k_import_lower<<<(unsigned)blocks, 256, 0, st>>>(a);
+  k_import_finish<<<(unsigned)blocks, 256, 0, st>>>(v, f, L.e, (double*)(base + L.o_dinv), L.n);
+  BuildArgs b;
+  memset(&b, 0, sizeof b);
+  b.nx = L.nx; b.ny = L.ny; b.nz = L.nz; b.n = L.n; b.nxny = L.nxny;
+  b.d0 = a.d0; b.d1 = a.d1; b.d2 = a.d2; b.d3 = a.d3;
+  b.f0 = f + L.ptr[0]; b.f1 = f + L.ptr[1]; b.f2 = f + L.ptr[2]; b.f3 = f + L.ptr[3];
+  double* slot = (double*)(base + L.o_layers) + 4 * nz;
+  k_offdiag_absmax<<<(unsigned)blocks, 256, 0, st>>>(a.d1, L.e - L.n, slot);
+  k_h16_scale<<<1, 1, 0, st>>>(slot);
+  k_make_h16<<<(unsigned)blocks, 256, 0, st>>>(b, slot, (__half*)(base + L.o_h16), (__half*)(base + L.o_h16 + L.h16_stride),
+                                               (__half*)(base + L.o_h16 + 2 * L.h16_stride));
+  k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(b, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
+                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride));
+  e = cudaGetLastError();
+  unsigned long long cnt[5];
+  if (e == cudaSuccess) e = cudaMemcpyAsync(cnt, a.cnt, sizeof cnt, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h.data(), lay, 3 * (size_t)nz * 8, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+  // per-layer row sums s(z) of the MIXED operator (difference form, DESIGN.md R-F3): the caller's, else the
+  // midrange of the computed row sums of the layer (clamped at 0); usable only if every row of the layer agrees
+  // with it to 1e-9 of the layer's smallest diagonal entry.
+  std::vector<double> lay_out(4 * (size_t)nz, 0.0);
+  double dev = 0.0;
+  bool ok = true;
+  for (int z = 0; z < nz; ++z) {
+    const double lo = key_to_double(h[z]), hi = key_to_double(h[nz + z]), dmin = key_to_double(h[2 * nz + z]);
+    double s = rowsum_layer_H ? rowsum_layer_H[z] : 0.5 * (lo + hi);
+    if (!rowsum_layer_H && s < 0.0) s = 0.0;
+    const double dz = fmax(fabs(hi - s), fabs(lo - s)) / (dmin > 0.0 ? dmin : 1.0);
+    if (!(dz <= 1e-9) || !(s >= 0.0)) ok = false;
+    if (!(dz <= dev)) dev = dz;
+    lay_out[nz + z] = s;
+  }
+  const bool structure_ok = cnt[0] == 0 && cnt[1] == 0 && cnt[2] == 0 && cnt[3] == 0;
+  if (!ok || !structure_ok)
+    for (int z = 0; z < nz; ++z) lay_out[nz + z] = nan("");   // second line of defence: a MIXED solve breaks down loudly
+  e = cudaMemcpyAsync(lay, lay_out.data(), lay_out.size() * 8, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+  if (rep) {
+    rep->off_stencil = (int64_t)cnt[0]; rep->asymmetric_rows = (int64_t)cnt[1]; rep->bad_diagonal = (int64_t)cnt[2];
+    rep->duplicates = (int64_t)cnt[3]; rep->positive_offdiag = (int64_t)cnt[4];
+    rep->max_rowsum_dev = dev; rep->mixed_ok = (ok && structure_ok) ? 1 : 0;
+  }
+  if (!structure_ok) return CUTH_ERR_STRUCTURE;
+  if (rowsum_layer_H && !ok) return CUTH_ERR_STRUCTURE;
   return CUTH_OK;
 }
 

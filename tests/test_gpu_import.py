@@ -1,0 +1,208 @@
+"""GPU parity of the importer (PAPER.md:430 / :219): cuth_import_csr condenses a CSR matrix into the
+matrix object bit for bit, validates it like the oracle's entry-by-entry checker, and the solver runs on it."""
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import oracle as O
+from gpu_util import grid_from_workload, to_dev
+from import_faults import faults
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    dict(cfg=1, nx=2, ny=2, nz=2, n_hot=0),
+    dict(cfg=1, nx=7, ny=2, nz=5, n_hot=1),
+    dict(cfg=3, nx=37, ny=29, nz=16, n_hot=8),     # per-cell lognormal kappa
+    dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8),     # C/dt on the diagonal: every layer has a non-zero row sum
+    dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6),
+    dict(cfg=6, nx=45, ny=38, nz=10, n_hot=6),
+]
+
+
+def _csr_dev(A):
+    import torch
+    return (torch.from_numpy(A.rowptr).cuda(), torch.from_numpy(A.col).cuda(), torch.from_numpy(A.val).cuda())
+
+
+def _exact_rowsums(w):
+    s = np.zeros(w.nz)
+    s[-1] += w.h_top * (w.dx * w.dy)
+    if w.cvol is not None and w.dt > 0:
+        s += np.asarray(w.cvol) * ((w.dx * w.dy) * np.asarray(w.dz)) / w.dt
+    return s
+
+
+def _shuffle_rows(A, seed):
+    """Same matrix with the entries of every row in a different order."""
+    rng = np.random.default_rng(seed)
+    col, val = A.col.copy(), A.val.copy()
+    for i in range(A.n):
+        a, b = int(A.rowptr[i]), int(A.rowptr[i + 1])
+        p = rng.permutation(b - a)
+        col[a:b] = A.col[a:b][p]
+        val[a:b] = A.val[a:b][p]
+    return O.CSR(A.n, A.rowptr.copy(), col, val)
+
+
+@pytest.mark.parametrize("kw", CASES + [dict(cfg=2)])
+@pytest.mark.parametrize("given_rowsums", [False, True])
+def test_import_is_bit_exact(kw, given_rowsums):
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    vals_o, ptr_o, off_o = O.csr_to_dia(A, w.nx, w.ny, w.nz)
+    g = grid_from_workload(w)
+    A_sh = _shuffle_rows(A, 7) if w.n <= 100000 else A
+    M = cu.DiaMatrix(g, csr=_csr_dev(A_sh), rowsum_layer=_exact_rowsums(w) if given_rowsums else None)
+    rep = M.import_report
+    assert (rep.off_stencil, rep.asymmetric_rows, rep.bad_diagonal, rep.duplicates, rep.positive_offdiag) == (0,) * 5
+    assert rep.mixed_ok == 1 and rep.max_rowsum_dev <= 1e-9
+    vals, vals32, inv, ptr, off = M.view()
+    assert ptr == ptr_o.tolist() and off == off_o.tolist()
+    assert np.array_equal(vals.cpu().numpy().view(np.uint64), vals_o.view(np.uint64))
+    assert np.array_equal(vals32.cpu().numpy().view(np.uint32), vals_o.astype(np.float32).view(np.uint32))
+    assert np.array_equal(inv.cpu().numpy(), 1.0 / vals_o[:w.n])
+    # everything the solver kernels read besides the per-layer table is byte-identical to what the builder writes
+    B = cu.DiaMatrix(g)
+    lay_end = 512 + 256 * (((4 * w.nz + 4) * 8 + 255) // 256)
+    al = lambda v: (v + 255) // 256 * 256                    # section alignment of the matrix object
+    e, n = int(ptr[4]), w.n
+    o_h16 = al(al(al(lay_end + 8 * e) + 4 * e) + 8 * n)      # after A1, A2, 1/D0
+    o_f32a = o_h16 + 3 * al(2 * n)
+    for k in range(3):                                       # A3 (fp16, scaled) and the aligned per-diagonal copies of A2
+        a, b = o_h16 + k * al(2 * n), o_f32a + k * al(4 * n)
+        assert bool((M.buf[a:a + 2 * n] == B.buf[a:a + 2 * n]).all())
+        assert bool((M.buf[b:b + 4 * n] == B.buf[b:b + 4 * n]).all())
+    assert o_f32a + 3 * al(4 * n) == M.buf.numel()
+    sc = slice(512 + 32 * w.nz, 512 + 32 * w.nz + 24)        # |entry|max bits, fp16 scale, 1/scale
+    assert bool((M.buf[sc] == B.buf[sc]).all())
+    s_imp = M.buf[512 + 8 * w.nz: 512 + 16 * w.nz].view(np_to_torch_f64()).cpu().numpy()
+    s_bld = B.buf[512 + 8 * w.nz: 512 + 16 * w.nz].view(np_to_torch_f64()).cpu().numpy()
+    if given_rowsums:
+        assert np.array_equal(s_imp, s_bld)
+    else:
+        assert np.abs(s_imp - s_bld).max() <= 1e-9 * vals_o[:w.n].min()
+
+
+def np_to_torch_f64():
+    import torch
+    return torch.float64
+
+
+@pytest.mark.parametrize("kw", CASES)
+def test_solve_on_imported_matrix(kw):
+    """FP64 and MIXED solves on the imported object meet the same bars as on the built one (north_star)."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    ref = O.pcg(A, w.power, rtol=1e-10)
+    assert ref.status == 0
+    g = grid_from_workload(w)
+    M = cu.DiaMatrix(g, csr=_csr_dev(A))
+    B = cu.DiaMatrix(g)
+    for precision, bar in ((cu.FP64, 1e-6 * np.abs(ref.x).max()), (cu.MIXED, 1e-4)):
+        xs = []
+        for mat in (M, B):
+            S = cu.Solver(mat, cu.Opts(precision=precision, rtol=1e-8, true_resid_period=w.true_resid_period))
+            x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+            S.solve(to_dev(w.power), x)
+            res = S.result()
+            assert res.status == 0
+            xs.append(x.cpu().numpy())
+            S.close()
+        assert np.abs(xs[0] - ref.x).max() <= bar
+        r = w.power - O.spmv(A, xs[0])
+        assert np.linalg.norm(r) <= 1e-8 * np.linalg.norm(w.power)
+        if precision == cu.FP64:
+            assert np.array_equal(xs[0], xs[1])        # same bytes in, same kernels: identical iterates
+
+
+def test_validation_counts_match_the_oracle():
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(cfg=3, nx=12, ny=9, nz=5, n_hot=2)
+    A = O.assemble_workload(w)
+    g = grid_from_workload(w)
+    import torch
+    buf = torch.empty(cu.cuth_dia_bytes(g), dtype=torch.uint8, device="cuda")
+    for name, Af in faults(A, w.nx, w.ny, w.nz).items():
+        want = O.stencil7_report(Af, w.nx, w.ny, w.nz)
+        rc, rep = cu.cuth_import_csr(g, *_csr_dev(Af), buf, check=False)
+        got = dict(off_stencil=rep.off_stencil, asymmetric_rows=rep.asymmetric_rows, bad_diagonal=rep.bad_diagonal,
+                   duplicates=rep.duplicates, positive_offdiag=rep.positive_offdiag)
+        assert got == {k: want[k] for k in got}, name
+        healthy = name == "explicit_zero_off_stencil"
+        assert rc == (0 if healthy else -8), name
+
+
+def test_non_layered_row_sums_are_fp64_only():
+    """A diagonal shift that varies from cell to cell keeps A SPD but leaves no per-layer row sum: the import
+    succeeds, MIXED is refused on the host, and the FP64 solve matches the oracle on the same matrix."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(cfg=3, nx=20, ny=14, nz=6, n_hot=3)
+    A = O.assemble_workload(w)
+    rows = np.repeat(np.arange(A.n), np.diff(A.rowptr))
+    dq = np.flatnonzero(A.col == rows)
+    v = A.val.copy()
+    v[dq] *= 1.0 + 0.05 * W.uniform01(w.seed, 77, np.arange(A.n))
+    Ap = O.CSR(A.n, A.rowptr, A.col, v)
+    want = O.stencil7_report(Ap, w.nx, w.ny, w.nz)
+    assert want["mixed_ok"] == 0
+    g = grid_from_workload(w)
+    M = cu.DiaMatrix(g, csr=_csr_dev(Ap))
+    assert M.import_report.mixed_ok == 0
+    assert M.import_report.max_rowsum_dev == pytest.approx(want["max_rowsum_dev"], rel=1e-6)
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    S = cu.Solver(M, cu.Opts(precision=cu.MIXED))
+    with pytest.raises(cu.CuthError) as e:
+        S.solve(to_dev(w.power), x)
+    assert e.value.code == -9
+    with pytest.raises(cu.CuthError):
+        M.spmv(to_dev(w.power), cu.MIXED)
+    S = cu.Solver(M, cu.Opts(precision=cu.FP64))
+    S.solve(to_dev(w.power), x)
+    assert S.result().status == 0
+    ref = O.pcg(Ap, w.power, rtol=1e-10)
+    assert np.abs(x.cpu().numpy() - ref.x).max() <= 1e-6 * np.abs(ref.x).max()
+    # a supplied per-layer table that the matrix contradicts is an error
+    rc, rep = cu.cuth_import_csr(g, *_csr_dev(Ap), M.buf, rowsum_layer=_exact_rowsums(w), check=False)
+    assert rc == -8 and rep.mixed_ok == 0
+    # and the same buffer rebuilt by cuth_build_dia is a normal matrix again
+    cu.cuth_build_dia(g, M.buf)
+    S = cu.Solver(M, cu.Opts(precision=cu.MIXED))
+    S.solve(to_dev(w.power), x.zero_())
+    assert S.result().status == 0
+
+
+def test_import_argument_errors():
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(cfg=1, nx=4, ny=3, nz=2, n_hot=1)
+    A = O.assemble_workload(w)
+    g = grid_from_workload(w)
+    rp, col, val = _csr_dev(A)
+    buf = torch.empty(cu.cuth_dia_bytes(g), dtype=torch.uint8, device="cuda")
+    L = cu.load_library()
+    import ctypes as C
+    from paper_2606_17850_b200.binding import cuth_import_report_t
+    rep = cuth_import_report_t()
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    p = lambda t: C.c_void_p(t.data_ptr())
+    assert L.cuth_import_csr(g.ref(), None, p(col), p(val), None, p(buf), buf.numel(), C.byref(rep), st) == -1
+    assert L.cuth_import_csr(g.ref(), p(rp), p(col), p(val), None, p(buf), buf.numel() - 1, C.byref(rep), st) == -4
+    assert L.cuth_import_csr(g.ref(), p(rp), p(col), p(val), None, C.c_void_p(buf.data_ptr() + 8), buf.numel(),
+                             C.byref(rep), st) == -5
+    bad = np.full(w.nz, -1.0)
+    assert L.cuth_import_csr(g.ref(), p(rp), p(col), p(val), bad.ctypes.data_as(C.c_void_p), p(buf), buf.numel(),
+                             C.byref(rep), st) == -3
+    # an imported matrix is a steady operator for this library
+    wt = W.make_workload(cfg=5, nx=8, ny=6, nz=4, n_hot=2)
+    gt = grid_from_workload(wt)
+    M = cu.DiaMatrix(gt, csr=_csr_dev(O.assemble_workload(wt)))
+    S = cu.Solver(M, cu.Opts())
+    T = torch.zeros(wt.n, dtype=torch.float64, device="cuda")
+    with pytest.raises(cu.CuthError) as e:
+        S.step(to_dev(wt.power), T)
+    assert e.value.code == -7
