@@ -31,8 +31,8 @@ import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
-NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3114e9,   # profiles/r1f_cfg3_fp64_k1_nodinv.md
-                     ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 516.7e6,    # profiles/r1h_cheb_pair_tma.md
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3111e9,   # profiles/r1i_cfg3_default_and_cheb16.md
+                     ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 518.3e6,    # profiles/r1i_cfg3_default_and_cheb16.md
                      ("cfg4_steady_4096x4096x8", "k_cheb_pair", "mixed"): 4.477e9,                 # profiles/r1h_cheb_pair_tma.md
                      }     # cfg 4: profiles/r1d predates the K1 that no longer reads 1/D0 -> null until recaptured
 
@@ -178,6 +178,90 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_batch(args):
+    """`--batch NRHS`: cuth_pcg_solve_batch on NRHS seeded power maps of the workload (FP64, Jacobi) against the same
+    NRHS systems solved one after the other with cuth_pcg_solve.  One step = the whole batch."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    w = W.make_workload(args.config)
+    nrhs = args.batch
+    kap = w.kappa_cell if w.kappa_cell is not None else w.kappa_layer
+    g = cu.Grid(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, torch.from_numpy(np.ascontiguousarray(kap)).cuda(), w.h_top)
+    A = cu.DiaMatrix(g)
+    opts = cu.Opts(precision=cu.FP64, rtol=w.rtol, max_iters=200000)
+    idx = np.arange(w.n)
+    B = np.stack([w.power * (0.25 + 1.5 * W.uniform01(w.seed, 100 + s, idx)) if s else w.power for s in range(nrhs)])
+    b_host = torch.from_numpy(B).pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    b = b_host.cuda()
+    b_stage = torch.empty_like(b)
+    x = torch.zeros_like(b)
+    SB = cu.BatchSolver(A, nrhs, opts)
+    S1 = cu.Solver(A, opts)
+    stream = torch.cuda.current_stream()
+
+    def batch_pass(from_host):
+        x.zero_()
+        if from_host:
+            b_stage.copy_(b_host, non_blocking=True)
+        SB.solve(b_stage if from_host else b, x)
+        if from_host:
+            x_host.copy_(x, non_blocking=True)
+
+    def seq_pass():
+        x.zero_()
+        for s in range(nrhs):
+            S1.solve(b[s], x[s])
+
+    def timed(fn, *a):
+        for _ in range(args.warmup):
+            fn(*a)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for e0, e1 in ev:
+            e0.record(stream)
+            fn(*a)
+            e1.record(stream)
+        torch.cuda.synchronize()
+        return float(np.mean([e0.elapsed_time(e1) for e0, e1 in ev]))
+
+    sampler = ClockSampler(0)
+    ms_batch = timed(batch_pass, False)
+    clocks = sampler.stop()
+    res = SB.results()
+    xb = x.cpu().numpy().copy()
+    ms_e2e = timed(batch_pass, True)
+    ms_seq = timed(seq_pass)
+    xs = x.cpu().numpy()
+    its = [r.iterations for r in res]
+    peak, peak_src = peaks()
+    m = m_ratio(w)
+    # three phases per iteration (DESIGN.md §13): (8m + 8)/S matrix and 1/D0 bytes shared by S = 4 right-hand sides,
+    # 88 vector bytes per right-hand side
+    bytes_it = sum(its) * (88 + (8 * m + 16) / min(4, nrhs)) * w.n
+    line = {"metric": METRIC, "value": ms_batch * 1e-3, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_batch, "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz], "precision": "fp64",
+                       "preconditioner": "jacobi", "rtol": w.rtol, "batch_nrhs": nrhs,
+                       "l2_policy": "batched small-grid case: the working set of all right-hand sides is what it is; no flush",
+                       "parallelism": "1 GPU"},
+            "iterations": its, "status": [r.status_name for r in res],
+            "max_rel_resid_true": max(r.rel_resid_true for r in res),
+            "solves_per_s": nrhs / (ms_batch * 1e-3),
+            "sequential_single_solves_ms": ms_seq, "speedup_vs_sequential": ms_seq / ms_batch,
+            "max_rel_diff_vs_single_solves": float(np.abs(xb - xs).max() / np.abs(xs).max()),
+            "roofline": {"bound": "hbm", "kernel": "k_pcg_batch (whole solve, persistent)",
+                         "achieved": bytes_it / ms_batch / 1e6, "peak": peak, "unit": "GB/s",
+                         "frac": bytes_it / ms_batch / 1e6 / peak, "traffic": None, "peak_source": peak_src,
+                         "note": "algorithmic bytes of all iterations of all right-hand sides / whole-solve time; "
+                                 "L2-resident for small grids, where the fraction is not an HBM statement"},
+            "e2e": {"value": ms_e2e * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(B.nbytes), "d2h_bytes_per_step": int(B.nbytes)},
+            "gpu_launches": 2 * args.steps, "clocks": clocks, "loop": "persistent cooperative kernel (batched)"}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -206,9 +290,14 @@ def main():
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
                          "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="NRHS > 0: time cuth_pcg_solve_batch on NRHS power maps of --config (FP64, Jacobi) against "
+                         "NRHS single solves")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.batch > 0:
+        return run_batch(args)
 
     import torch
     import torch.distributed as dist

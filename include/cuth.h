@@ -165,6 +165,22 @@ int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const d
 int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
                    double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D, void* stream);
 
+/* Batched solve (SURVEY.md §8(f) "multi-RHS / batched solves sharing one A"; PAPER.md:473 observes that many
+ * right-hand sides on one matrix favour direct solvers -- this call amortises A on the iterative path instead).
+ * nrhs independent systems A x_s = b_s, 1 <= nrhs <= 32, each by its own Alg. 1 recurrence (own
+ * alpha, beta, stopping test on the true fp64 residual), advanced in lock-step by ONE persistent cooperative kernel:
+ * every matrix row is fetched once per 4 right-hand sides and every grid-wide barrier / reduction serves all of
+ * them, so small grids (where a single solve is bound by barrier latency) solve nrhs systems in little more than
+ * the time of one.  This is not block-CG: x_s is what cuth_pcg_solve would return for b_s, up to summation order.
+ * b_D, x_D: [nrhs][N] fp64, right-hand-side-major (x_D in: initial guesses, out: solutions).  result_D: [nrhs].
+ * opts: precision must be CUTH_FP64, preconditioner CUTH_PRECOND_JACOBI or CUTH_PRECOND_NONE (else CUTH_ERR_VALUE).
+ * work_D >= cuth_batch_workspace_bytes(grid, nrhs).  All CTAs must be co-resident: needs cooperative launch
+ * (CUTH_ERR_CUDA otherwise).  Asynchronous on `stream` like cuth_pcg_solve. */
+size_t cuth_batch_workspace_bytes(const cuth_grid_t* grid, int nrhs);
+int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, int nrhs,
+                         const double* b_D, double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D,
+                         void* stream);
+
 /* One backward-Euler step (step a6), eq. (5): forms b = P_{n+1} + (C V/dt) T_n in
  * one fused pass and solves A T_{n+1} = b warm-started from T_n.  power_D: W per cell [N];
  * T_D: in T_n, out T_{n+1}.  The matrix must have been built with cvol_H and dt > 0. */

@@ -56,7 +56,7 @@ class cuth_import_report_t(C.Structure):
                 ("mixed_ok", C.c_int32)]
 
 
-EXPORTS = ["cuth_import_csr", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
+EXPORTS = ["cuth_import_csr", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
            "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy", "cuth_set_pair_rows"]
 
@@ -92,6 +92,10 @@ def load_library():
     L.cuth_spmv.argtypes = [vp, gp, C.c_int, vp, vp, vp]
     L.cuth_pcg_solve.restype = C.c_int
     L.cuth_pcg_solve.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp, vp]
+    L.cuth_batch_workspace_bytes.restype = C.c_size_t
+    L.cuth_batch_workspace_bytes.argtypes = [gp, C.c_int]
+    L.cuth_pcg_solve_batch.restype = C.c_int
+    L.cuth_pcg_solve_batch.argtypes = [vp, gp, op, C.c_int, vp, vp, vp, C.c_size_t, vp, vp]
     L.cuth_transient_step.restype = C.c_int
     L.cuth_transient_step.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp, vp]
     L.cuth_release_workspace.restype = C.c_int
@@ -228,6 +232,17 @@ def cuth_pcg_solve(dia, grid: Grid, opts, b, x, work, result, stream=None):
            "cuth_pcg_solve")
 
 
+def cuth_batch_workspace_bytes(grid: Grid, nrhs: int) -> int:
+    return int(load_library().cuth_batch_workspace_bytes(grid.ref(), int(nrhs)))
+
+
+def cuth_pcg_solve_batch(dia, grid: Grid, opts, nrhs, b, x, work, result, stream=None):
+    """b, x: [nrhs, N] float64 CUDA tensors (contiguous); result: device buffer of nrhs cuth_result_t records."""
+    _check(load_library().cuth_pcg_solve_batch(_ptr(dia), grid.ref(), C.byref(opts), int(nrhs), _ptr(b), _ptr(x),
+                                               _ptr(work), work.numel() * work.element_size(), _ptr(result),
+                                               stream or _stream()), "cuth_pcg_solve_batch")
+
+
 def cuth_transient_step(dia, grid: Grid, opts, power, T, work, result, stream=None):
     _check(load_library().cuth_transient_step(_ptr(dia), grid.ref(), C.byref(opts), _ptr(power), _ptr(T), _ptr(work),
                                               work.numel() * work.element_size(), _ptr(result),
@@ -355,6 +370,35 @@ class DiaMatrix:
         y = torch.empty_like(x) if out is None else out
         cuth_spmv(self.buf, self.grid, precision, x, y)
         return y
+
+
+class BatchSolver:
+    """Workspace + result records for cuth_pcg_solve_batch (allocation only)."""
+
+    def __init__(self, A: "DiaMatrix", nrhs: int, opts=None):
+        import torch
+        self.A, self.nrhs = A, int(nrhs)
+        self.opts = opts or Opts()
+        nbytes = cuth_batch_workspace_bytes(A.grid, self.nrhs)
+        if nbytes == 0:
+            raise CuthError(-3, "cuth_batch_workspace_bytes")
+        self.work = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        self.result_dev = torch.zeros(self.nrhs * C.sizeof(cuth_result_t), dtype=torch.uint8, device="cuda")
+
+    def solve(self, b, x):
+        assert b.is_contiguous() and x.is_contiguous() and b.shape == x.shape == (self.nrhs, self.A.grid.n)
+        cuth_pcg_solve_batch(self.A.buf, self.A.grid, self.opts, self.nrhs, b, x, self.work, self.result_dev)
+
+    def results(self):
+        """Synchronising read-back of the nrhs device result records."""
+        raw = self.result_dev.cpu().numpy().tobytes()
+        sz = C.sizeof(cuth_result_t)
+        out = []
+        for s in range(self.nrhs):
+            r = cuth_result_t.from_buffer_copy(raw[s * sz:(s + 1) * sz])
+            out.append(Result(r.status, r.iterations, r.promotions, r.true_resid_evals, r.rel_resid_true,
+                              r.rel_resid_rec, r.switch_reason, r.switch_iteration))
+        return out
 
 
 class Solver:

@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcuth.so")
 SOURCES = ["cuth_api.cu", "cuth_build.cu"]
-HEADERS = ["cuth_internal.cuh", "cuth_kernels.cuh", "cuth_policy.cuh", "cuth_fused.cuh", "cuth_fused_x2.cuh", "cuth_cheb.cuh", "cuth_cheb_pair.cuh", "cuth_persistent.cuh", os.path.join("..", "..", "include", "cuth.h")]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh")) + [os.path.join("..", "..", "include", "cuth.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -20,6 +20,7 @@
 #include "cuth_cheb_pair.cuh"
 #include "cuth_cheb_pair_tma.cuh"
 #include "cuth_persistent.cuh"
+#include "cuth_batch.cuh"
 
 namespace cuth {
 
@@ -734,6 +735,63 @@ int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t
                    double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D, void* stream) {
   if (!b_D) return CUTH_ERR_NULL;
   return solve_common(dia_D, grid, opts, b_D, nullptr, x_D, work_D, work_bytes, result_D, stream);
+}
+
+size_t cuth_batch_workspace_bytes(const cuth_grid_t* grid, int nrhs) {
+  DiaLayout L;
+  if (!make_layout(grid, &L) || nrhs < 1 || nrhs > kBatchMaxRhs) return 0;
+  return carve_batch_workspace(nullptr, L.n, nrhs).bytes;
+}
+
+int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, int nrhs,
+                         const double* b_D, double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D,
+                         void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  rc = check_opts(opts);
+  if (rc) return rc;
+  if (nrhs < 1 || nrhs > kBatchMaxRhs) return CUTH_ERR_VALUE;
+  if (opts->precision != CUTH_FP64) return CUTH_ERR_VALUE;
+  if (opts->preconditioner != CUTH_PRECOND_JACOBI && opts->preconditioner != CUTH_PRECOND_NONE) return CUTH_ERR_VALUE;
+  if (!dia_D || !b_D || !x_D || !work_D || !result_D) return CUTH_ERR_NULL;
+  if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(work_D) || !aligned16(b_D) || ((uintptr_t)result_D & 7u))
+    return CUTH_ERR_ALIGN;
+  BatchWorkspace w = carve_batch_workspace(work_D, L.n, nrhs);
+  if (work_bytes < w.bytes) return CUTH_ERR_SIZE;
+  cudaStream_t st = (cudaStream_t)stream;
+  // co-resident CTAs available, split into ceil(nrhs / S) chunks x ntiles row tiles
+  static int max_blocks = -1;
+  if (max_blocks < 0) {
+    int dev = 0, sms = 0, coop = 0, occ = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pcg_batch, kThreads, 0);
+    if (occ > 3) occ = 3;
+    max_blocks = coop ? sms * occ : 0;
+  }
+  const int nchunks = (nrhs + kBatchChunk - 1) / kBatchChunk;
+  if (max_blocks < nchunks) { g_last_err = "cuth_pcg_solve_batch: cooperative launch unavailable"; return CUTH_ERR_CUDA; }
+  const int64_t need = (L.n + (int64_t)kThreads * kRows - 1) / ((int64_t)kThreads * kRows);
+  int64_t ntiles = max_blocks / nchunks;
+  if (ntiles > need) ntiles = need;
+  if (ntiles > kBatchMaxBlocks) ntiles = kBatchMaxBlocks;
+  BatchCtx c;
+  memset(&c, 0, sizeof c);
+  c.A = dev_view(dia_D, L);
+  c.b = b_D; c.x = x_D; c.r = w.r; c.p = w.p; c.mu = w.mu;
+  c.result = result_D;
+  c.rtol = opts->rtol;
+  c.nrhs = nrhs; c.max_iters = opts->max_iters;
+  c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
+  c.ntiles = (int32_t)ntiles;
+  k_batch_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
+  CU(cudaGetLastError());
+  BatchCtx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
+  void* args[] = {&ctxp, &ctlp, &part};
+  CU(cudaLaunchCooperativeKernel((void*)k_pcg_batch, dim3((unsigned)(ntiles * nchunks)), dim3(kThreads), args, 0, st));
+  return CUTH_OK;
 }
 
 int cuth_transient_step(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts,
