@@ -257,11 +257,11 @@ int cuth_set_cheb_fusion(int mode);
  * 2 = two columns whenever nx is even.  Results agree up to fp64 summation order. */
 int cuth_set_k1_variant(int mode);
 
-/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: for tiny grids (N <= 65536, flat
- * traversal, Jacobi / no preconditioner) the whole solve is ONE persistent cooperative kernel whose
- * iterations are separated by grid-wide barriers; everything else runs as the CUDA graph with conditional
- * nodes.  1 = always the graph, 2 = the persistent kernel wherever it applies (any flat-traversal grid).
- * Same arithmetic and policy code either way. */
+/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on flat-traversal grids of up to 2^21 rows
+ * (Jacobi / no preconditioner) the whole solve is ONE persistent cooperative kernel whose iterations are separated
+ * by grid-wide barriers (measured faster than the graph on every such grid); everything else runs as
+ * the CUDA graph with conditional nodes.  1 = always the graph, 2 = the persistent kernel wherever it applies (any
+ * flat-traversal grid).  Same arithmetic and policy code either way. */
 int cuth_set_loop_mode(int mode);
 
 /* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is

@@ -516,7 +516,12 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
   c->precision = opts->precision;
 }
 
-// Grid of the persistent kernel: every CTA must be co-resident (cooperative launch).
+// Grid of the persistent kernel: every CTA must be co-resident (cooperative launch).  The grid-wide barrier, not
+// the row work, sets the pace on small grids, and its cost is not monotonic in the CTA count: measured per
+// iteration at 8 k / 33 k / 66 k / 262 k / 1 M rows (B200) -- 32 CTAs 11.5 / 16.0 / 22.9 / 51 / 187 us,
+// 96 CTAs 12.4 / 13.9 / 16.0 / 27.7 / 72, 128 CTAs 7.1 / 7.3 / 8.1 / 13.9 / 47, 148 CTAs 8.0 / 8.0 / 8.8 / 14.2 / 46,
+// 256 CTAs 9.2 / 8.4 / 8.4 / 12.4 / 33, 592 CTAs 13.4 / 14.1 / 13.7 / 16.7 / 29.8.  So: 128 CTAs up to 64 k rows (CTAs
+// beyond the rows only take part in the barriers), 256 up to 512 k rows, everything the device holds beyond.
 static int persistent_blocks(int64_t n) {
   static int cached = -1;
   if (cached < 0) {
@@ -529,18 +534,18 @@ static int persistent_blocks(int64_t n) {
     cached = coop ? sms * occ : 0;
     if (cached > kPersistMaxBlocks) cached = kPersistMaxBlocks;
   }
-  int64_t need = (n + (int64_t)kThreads * kRows - 1) / ((int64_t)kThreads * kRows);
-  return (int)(need < cached ? need : cached);
+  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : cached);
+  return want < cached ? want : cached;
 }
 
 static bool use_persistent(const DiaLayout& L, bool cheb) {
   const int mode = g_loop_mode.load();
   if (cheb || use_zmarch(L) || mode == 1) return false;
   if (persistent_blocks(L.n) <= 0) return false;
-  // Measured on B200: a phase of the persistent kernel costs ~4.5 us (L2 round trips +
-  // grid.sync), a graph kernel node ~5 us: 14.1 vs 16.5 us per iteration at cfg 1 (8 k rows), 36.4 vs 34.6 us
-  // at cfg 2 (1 M rows), where the wider grid of the separate kernels wins.  Auto: persistent for tiny grids.
-  return mode == 2 || L.n <= (1 << 16);
+  // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
+  // 7.1 / 18.7 us at cfg 1 (8 k rows), 23 / 30.4 us at cfg 6 (655 k), 29.8 / 34.7 us at cfg 2 (1 M).  Auto: the
+  // persistent kernel for every flat-traversal grid up to 2 M rows; beyond, the wider grids of separate kernels.
+  return mode == 2 || L.n <= (1 << 21);
 }
 
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
@@ -773,9 +778,11 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   }
   const int nchunks = (nrhs + kBatchChunk - 1) / kBatchChunk;
   if (max_blocks < nchunks) { g_last_err = "cuth_pcg_solve_batch: cooperative launch unavailable"; return CUTH_ERR_CUDA; }
-  const int64_t need = (L.n + (int64_t)kThreads * kRows - 1) / ((int64_t)kThreads * kRows);
+  const int64_t need = (L.n + (int64_t)kThreads - 1) / (int64_t)kThreads;
   int64_t ntiles = max_blocks / nchunks;
   if (ntiles > need) ntiles = need;
+  // the barrier is fastest at >= 128 CTAs (see persistent_blocks): tiles beyond the rows only take part in it
+  if (ntiles * nchunks < 128 && max_blocks >= 128) ntiles = (128 + nchunks - 1) / nchunks;
   if (ntiles > kBatchMaxBlocks) ntiles = kBatchMaxBlocks;
   BatchCtx c;
   memset(&c, 0, sizeof c);

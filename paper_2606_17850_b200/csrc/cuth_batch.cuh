@@ -114,25 +114,46 @@ __device__ __forceinline__ void batch_deposit(double (&v)[NV * kBatchChunk], dou
 // Grid-wide part: after the barrier every CTA adds the per-tile partials of all `count` = nv * nrhs values in the
 // same fixed order, so all CTAs hold bitwise-identical sums in tot[] (shared memory) and take identical decisions.
 __device__ __forceinline__ void batch_collect(cgb::grid_group& grid, const double* mine, int count, int ntiles,
-                                              double* tot) {
+                                              double* tot) {   // ntiles: tiles that own rows (the others deposit 0)
   grid.sync();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  for (int v = wid; v < count; v += nw) {
-    double a = 0.0;
-    for (int b = lane; b < ntiles; b += 32) a += __ldcg(&mine[(size_t)v * kBatchMaxBlocks + b]);
-    a = warp_sum(a);
-    if (lane == 0) tot[v] = a;
+  if (count <= nw) {            // at most one value per warp: keep the tile loop simple so that its loads overlap
+    if (wid < count) {
+      double a = 0.0;
+#pragma unroll 4
+      for (int b = lane; b < ntiles; b += 32) a += __ldcg(&mine[(size_t)wid * kBatchMaxBlocks + b]);
+      a = warp_sum(a);
+      if (lane == 0) tot[wid] = a;
+    }
+  } else {
+    constexpr int U = 8;        // values a warp sums side by side: one L2 round trip for up to U * nw values
+    for (int v0 = wid; v0 < count; v0 += U * nw) {
+      double a[U];
+#pragma unroll
+      for (int u = 0; u < U; ++u) a[u] = 0.0;
+      for (int b = lane; b < ntiles; b += 32) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const int v = v0 + u * nw;
+          if (v < count) a[u] += __ldcg(&mine[(size_t)v * kBatchMaxBlocks + b]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int v = v0 + u * nw;
+        const double t = warp_sum(a[u]);
+        if (lane == 0 && v < count) tot[v] = t;
+      }
+    }
   }
   __syncthreads();
 }
 
-// Rows of this CTA: row tiles of kThreads * kRows rows are dealt round-robin to the `ntiles` CTAs of a chunk;
-// identical in every phase, so only the stencil phases need a preceding grid-wide barrier.
+// Rows of this CTA: row i = tile * kThreads + thread, then strides of ntiles * kThreads; identical in every phase,
+// so only the stencil phases need a preceding grid-wide barrier.  One row at a time: the S right-hand sides of the
+// chunk supply the independent loads.
 #define CUTH_BROWS(i_)                                                                           \
-  for (int64_t base_ = (int64_t)tile * (kThreads * kRows); base_ < n;                            \
-       base_ += (int64_t)ntiles * (kThreads * kRows))                                            \
-    for (int k_ = 0; k_ < kRows; ++k_)                                                           \
-      for (int64_t i_ = base_ + threadIdx.x + k_ * kThreads; i_ < n; i_ = n)
+  for (int64_t i_ = (int64_t)tile * kThreads + threadIdx.x; i_ < n; i_ += (int64_t)ntiles * kThreads)
 
 // Grid: ntiles * ceil(nrhs / S) CTAs, all co-resident.  CTA (tile, chunk) owns the right-hand sides
 // chunk*S .. chunk*S+S-1 on its rows; decisions for ALL right-hand sides are replicated in every CTA.
@@ -147,6 +168,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
   const BatchCtx c = *ctxp;
   const int64_t n = c.A.n;
   const int nrhs = c.nrhs, ntiles = c.ntiles;
+  const int nact = (int)((n + kThreads - 1) / kThreads < (int64_t)ntiles ? (n + kThreads - 1) / kThreads : (int64_t)ntiles);
   const int tile = blockIdx.x % ntiles, s0 = (blockIdx.x / ntiles) * S;
   const bool jac = c.jacobi != 0;
   // the policy code reads its options from a Ctx: only these fields are consulted on this path
@@ -192,7 +214,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
     }
     batch_deposit<3>(acc, part(), s0, nrhs, tile, smem);
   }
-  batch_collect(grid, part(), 3 * nrhs, ntiles, tot);
+  batch_collect(grid, part(), 3 * nrhs, nact, tot);
   parity ^= 1;
   if (threadIdx.x < nrhs) {
     const int s = threadIdx.x;
@@ -241,7 +263,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
       }
       batch_deposit<1>(acc, part(), s0, nrhs, tile, smem);
     }
-    batch_collect(grid, part(), nrhs, ntiles, tot);
+    batch_collect(grid, part(), nrhs, nact, tot);
     parity ^= 1;
     if (threadIdx.x < nrhs && s_go[threadIdx.x]) policy_after_spmv(&sc[threadIdx.x], tot[threadIdx.x], false);
     __syncthreads();
@@ -274,7 +296,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
       }
       batch_deposit<2>(acc, part(), s0, nrhs, tile, smem);
     }
-    batch_collect(grid, part(), 2 * nrhs, ntiles, tot);
+    batch_collect(grid, part(), 2 * nrhs, nact, tot);
     parity ^= 1;
     if (threadIdx.x < nrhs && s_go[threadIdx.x]) {
       const int s = threadIdx.x;
@@ -314,7 +336,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
         }
         batch_deposit<2>(acc, part(), s0, nrhs, tile, smem);
       }
-      batch_collect(grid, part(), 2 * nrhs, ntiles, tot);
+      batch_collect(grid, part(), 2 * nrhs, nact, tot);
       parity ^= 1;
       if (threadIdx.x < nrhs) {
         const int s = threadIdx.x;
@@ -353,7 +375,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
           }
           batch_deposit<2>(acc, part(), s0, nrhs, tile, smem);
         }
-        batch_collect(grid, part(), 2 * nrhs, ntiles, tot);
+        batch_collect(grid, part(), 2 * nrhs, nact, tot);
         parity ^= 1;
         if (threadIdx.x < nrhs && s_mode[threadIdx.x]) {
           const int s = threadIdx.x;

@@ -34,13 +34,14 @@ __device__ __forceinline__ void grid_allreduce(cg::grid_group& grid, double (&v)
     for (int k = 0; k < NV; ++k) __stcg(&mine[k * kPersistMaxBlocks + blockIdx.x], v[k]);
   }
   grid.sync();
-  if (threadIdx.x < 32) {
-#pragma unroll
-    for (int k = 0; k < NV; ++k) {
+  {
+    // one warp per value: the NV chains of L2 loads run side by side instead of one after the other
+    const int lane = threadIdx.x & 31, k = threadIdx.x >> 5;
+    if (k < NV) {
       double a = 0.0;
-      for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) a += __ldcg(&mine[k * kPersistMaxBlocks + b]);
+      for (int b = lane; b < (int)gridDim.x; b += 32) a += __ldcg(&mine[k * kPersistMaxBlocks + b]);
       a = warp_sum(a);
-      if (threadIdx.x == 0) smem[NV * 32 + k] = a;
+      if (lane == 0) smem[NV * 32 + k] = a;
     }
   }
   __syncthreads();
@@ -50,11 +51,31 @@ __device__ __forceinline__ void grid_allreduce(cg::grid_group& grid, double (&v)
   parity ^= 1;
 }
 
+// Rows are dealt to threads with a stride of the whole grid (identically in every phase) and walked two at a
+// time: all loads of both rows are issued before the first store, so a phase costs one L2 round trip per pair
+// instead of one per row and per store (the stores may alias the loads as far as the compiler knows).
+#define CUTH_ROWS2(i0_, i1_, h1_)                                                                \
+  for (int64_t i0_ = (int64_t)blockIdx.x * kThreads + threadIdx.x, i1_ = i0_ + gstride; i0_ < n;  \
+       i0_ += 2 * gstride, i1_ += 2 * gstride)                                                   \
+    for (bool h1_ = i1_ < n, once_ = true; once_; once_ = false)
+
 #define CUTH_ROWS(i_)                                                                            \
-  for (int64_t base_ = (int64_t)blockIdx.x * (kThreads * kRows); base_ < n;                      \
-       base_ += (int64_t)gridDim.x * (kThreads * kRows))                                         \
-    for (int k_ = 0; k_ < kRows; ++k_)                                                           \
-      for (int64_t i_ = base_ + threadIdx.x + k_ * kThreads; i_ < n; i_ = n)
+  for (int64_t i_ = (int64_t)blockIdx.x * kThreads + threadIdx.x; i_ < n; i_ += gstride)
+
+template <bool MIXED>
+__device__ __forceinline__ double persistent_spmv_phase(const Ctx& c, int64_t n, int64_t gstride) {
+  double acc = 0.0;
+  CUTH_ROWS2(i0, i1, h1) {
+    const double p0 = c.p[i0], p1 = h1 ? c.p[i1] : 0.0;
+    const double m0 = spmv_row<MIXED>(c.A, c.p, i0, p0);
+    const double m1 = h1 ? spmv_row<MIXED>(c.A, c.p, i1, p1) : 0.0;
+    c.mu[i0] = m0;
+    if (h1) c.mu[i1] = m1;
+    acc = fma(p0, m0, acc);
+    acc = fma(p1, m1, acc);
+  }
+  return acc;
+}
 
 __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __restrict__ ctxp, Ctl* ctl_g,
                                                                double* partials) {
@@ -63,6 +84,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
   __shared__ double smem[3 * 32 + 3];
   const Ctx c = *ctxp;
   const int64_t n = c.A.n;
+  const int64_t gstride = (int64_t)gridDim.x * kThreads;
   const bool jac = c.jacobi != 0;
   int parity = 0;
   if (threadIdx.x == 0) sc = *ctl_g;                 // cleared by k_set_ctx
@@ -90,21 +112,18 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
     // ---- A: p = z + beta p
     {
       const double beta = sc.beta;
-      CUTH_ROWS(i) {
-        const double ri = c.r[i];
-        const double zi = jac ? ri * c.A.dinv[i] : ri;
-        c.p[i] = fma(beta, c.p[i], zi);
+      CUTH_ROWS2(i0, i1, h1) {
+        const double r0 = c.r[i0], q0 = c.p[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
+        const double r1 = h1 ? c.r[i1] : 0.0, q1 = h1 ? c.p[i1] : 0.0, d1 = (h1 && jac) ? c.A.dinv[i1] : 1.0;
+        c.p[i0] = fma(beta, q0, jac ? r0 * d0 : r0);
+        if (h1) c.p[i1] = fma(beta, q1, jac ? r1 * d1 : r1);
       }
     }
     grid.sync();
     // ---- B: mu = A p, p.mu
     {
-      double acc[1] = {0.0};
-      if (sc.stage == 0) {
-        CUTH_ROWS(i) { const double pi = c.p[i]; const double m = spmv_row<true>(c.A, c.p, i, pi); c.mu[i] = m; acc[0] = fma(pi, m, acc[0]); }
-      } else {
-        CUTH_ROWS(i) { const double pi = c.p[i]; const double m = spmv_row<false>(c.A, c.p, i, pi); c.mu[i] = m; acc[0] = fma(pi, m, acc[0]); }
-      }
+      double acc[1];
+      acc[0] = sc.stage == 0 ? persistent_spmv_phase<true>(c, n, gstride) : persistent_spmv_phase<false>(c, n, gstride);
       grid_allreduce<1>(grid, acc, partials, parity, smem);
       if (threadIdx.x == 0) policy_after_spmv(&sc, acc[0], false);
       __syncthreads();
@@ -114,12 +133,22 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
     {
       const double alpha = sc.alpha;
       double acc[2] = {0.0, 0.0};
-      CUTH_ROWS(i) {
-        c.x[i] = fma(alpha, c.p[i], c.x[i]);
-        const double ri = fma(-alpha, c.mu[i], c.r[i]);
-        const double zi = jac ? ri * c.A.dinv[i] : ri;
-        c.r[i] = ri;
-        acc[0] = fma(ri, zi, acc[0]); acc[1] = fma(ri, ri, acc[1]);
+      CUTH_ROWS2(i0, i1, h1) {
+        const double x0 = c.x[i0], q0 = c.p[i0], m0 = c.mu[i0], r0 = c.r[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
+        double x1 = 0.0, q1 = 0.0, m1 = 0.0, r1 = 0.0, d1 = 1.0;
+        if (h1) { x1 = c.x[i1]; q1 = c.p[i1]; m1 = c.mu[i1]; r1 = c.r[i1]; if (jac) d1 = c.A.dinv[i1]; }
+        c.x[i0] = fma(alpha, q0, x0);
+        const double s0 = fma(-alpha, m0, r0);
+        const double z0 = jac ? s0 * d0 : s0;
+        c.r[i0] = s0;
+        acc[0] = fma(s0, z0, acc[0]); acc[1] = fma(s0, s0, acc[1]);
+        if (h1) {
+          c.x[i1] = fma(alpha, q1, x1);
+          const double s1 = fma(-alpha, m1, r1);
+          const double z1 = jac ? s1 * d1 : s1;
+          c.r[i1] = s1;
+          acc[0] = fma(s1, z1, acc[0]); acc[1] = fma(s1, s1, acc[1]);
+        }
       }
       grid_allreduce<2>(grid, acc, partials, parity, smem);
       if (threadIdx.x == 0) {
