@@ -140,3 +140,54 @@ def test_batch_argument_errors():
     assert code(cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_lmin=1.0, cheb_lmax=2.0)) == -3
     assert code(cu.Opts(), nrhs=0) == -3 and code(cu.Opts(), nrhs=33) == -3
     assert code(cu.Opts(), work=S.work[:S.work.numel() - 256]) == -4
+
+
+@pytest.mark.parametrize("kw", [dict(cfg=1, nx=7, ny=5, nz=3, n_hot=1), dict(cfg=4, nx=130, ny=67, nz=8, n_hot=6)])
+@pytest.mark.parametrize("nrhs", [3, 9])
+def test_batch_and_import_no_out_of_bounds_canaries(kw, nrhs):
+    """Same stand-in for memcheck as test_no_out_of_bounds_canaries (compute-sanitizer is closed on this pool), for
+    the two calls added last: every caller-owned buffer (CSR arrays, matrix object, b, x, workspace, result records) is
+    carved with exactly the size the ABI asks for out of a NaN-filled arena; guard words must survive bitwise, and the
+    results must be bit-identical to the run on ordinary allocations."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    g = grid_from_workload(w)
+    A = O.assemble_workload(w)
+    B = rhs_set(w, nrhs)
+    nanbits = torch.tensor([float("nan")], dtype=torch.float64, device="cuda").view(torch.int64)
+
+    def run(guarded):
+        pad = 4096 if guarded else 0
+        arenas, bufs = {}, {}
+
+        def carve(name, nbytes):
+            nb8 = (nbytes + 7) // 8 * 8
+            arena = torch.full(((nb8 + 2 * pad) // 8,), float("nan"), dtype=torch.float64, device="cuda").view(torch.uint8)
+            arenas[name] = (arena, nb8)
+            bufs[name] = arena[pad:pad + nbytes]
+
+        carve("rowptr", A.rowptr.nbytes); carve("col", A.col.nbytes); carve("val", A.val.nbytes)
+        carve("dia", cu.cuth_dia_bytes(g)); carve("b", B.nbytes); carve("x", B.nbytes)
+        carve("work", cu.cuth_batch_workspace_bytes(g, nrhs)); carve("res", nrhs * 40)
+        bufs["rowptr"].view(torch.int64).copy_(torch.from_numpy(A.rowptr))
+        bufs["col"].view(torch.int32).copy_(torch.from_numpy(A.col))
+        bufs["val"].view(torch.float64).copy_(torch.from_numpy(A.val))
+        rep = cu.cuth_import_csr(g, bufs["rowptr"].view(torch.int64), bufs["col"].view(torch.int32),
+                                 bufs["val"].view(torch.float64), bufs["dia"])
+        assert rep.mixed_ok == 1
+        bufs["b"].view(torch.float64).copy_(to_dev(B).reshape(-1))
+        x = bufs["x"].view(torch.float64)
+        x.zero_()
+        cu.cuth_pcg_solve_batch(bufs["dia"], g, cu.Opts(), nrhs, bufs["b"].view(torch.float64), x, bufs["work"], bufs["res"])
+        torch.cuda.synchronize()
+        if guarded:
+            for name, (arena, nb8) in arenas.items():
+                assert bool((arena[:pad].view(torch.int64) == nanbits).all()), f"guard below {name} overwritten"
+                assert bool((arena[pad + nb8:].view(torch.int64) == nanbits).all()), f"guard above {name} overwritten"
+        return x.clone().cpu().numpy(), bufs["res"].view(torch.int32).cpu().numpy().copy()
+
+    x0, r0 = run(False)
+    x1, r1 = run(True)
+    assert np.array_equal(r0, r1) and np.array_equal(x0.view(np.uint64), x1.view(np.uint64))
+    assert all(r0[10 * s] == 0 for s in range(nrhs))
