@@ -34,7 +34,8 @@ import workloads as W  # noqa: E402
 NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3111e9,   # profiles/r1i_cfg3_default_and_cheb16.md
                      ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 518.3e6,    # profiles/r1i_cfg3_default_and_cheb16.md
                      ("cfg4_steady_4096x4096x8", "k_cheb_pair", "mixed"): 4.477e9,                 # profiles/r1h_cheb_pair_tma.md
-                     }     # cfg 4: profiles/r1d predates the K1 that no longer reads 1/D0 -> null until recaptured
+                     ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 10.786e9,               # profiles/r1j_cfg4_fp64_k1.md
+                     }
 
 METRIC = "pcg_time_to_solution"
 UNIT = "s"
@@ -189,7 +190,9 @@ def run_batch(args):
     kap = w.kappa_cell if w.kappa_cell is not None else w.kappa_layer
     g = cu.Grid(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, torch.from_numpy(np.ascontiguousarray(kap)).cuda(), w.h_top)
     A = cu.DiaMatrix(g)
-    opts = cu.Opts(precision=cu.FP64, rtol=w.rtol, max_iters=200000)
+    mixed = args.precision == "mixed"
+    opts = cu.Opts(precision=cu.MIXED if mixed else cu.FP64, rtol=w.rtol, max_iters=200000,
+                   true_resid_period=w.true_resid_period)
     idx = np.arange(w.n)
     B = np.stack([w.power * (0.25 + 1.5 * W.uniform01(w.seed, 100 + s, idx)) if s else w.power for s in range(nrhs)])
     b_host = torch.from_numpy(B).pin_memory()
@@ -243,7 +246,8 @@ def run_batch(args):
     line = {"metric": METRIC, "value": ms_batch * 1e-3, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_batch, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz], "precision": "fp64",
+            "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz],
+                       "precision": "mixed" if mixed else "fp64",
                        "preconditioner": "jacobi", "rtol": w.rtol, "batch_nrhs": nrhs,
                        "l2_policy": "batched small-grid case: the working set of all right-hand sides is what it is; no flush",
                        "parallelism": "1 GPU"},

@@ -173,7 +173,9 @@ int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t
  * them, so small grids (where a single solve is bound by barrier latency) solve nrhs systems in little more than
  * the time of one.  This is not block-CG: x_s is what cuth_pcg_solve would return for b_s, up to summation order.
  * b_D, x_D: [nrhs][N] fp64, right-hand-side-major (x_D in: initial guesses, out: solutions).  result_D: [nrhs].
- * opts: precision must be CUTH_FP64, preconditioner CUTH_PRECOND_JACOBI or CUTH_PRECOND_NONE (else CUTH_ERR_VALUE).
+ * opts: CUTH_FP64 or CUTH_MIXED (every right-hand side runs the policy of cuth_pcg_solve on its own: own stage, own
+ * switch by eq. (14a)-(14c), own hot restart); preconditioner CUTH_PRECOND_JACOBI or CUTH_PRECOND_NONE (else
+ * CUTH_ERR_VALUE).
  * work_D >= cuth_batch_workspace_bytes(grid, nrhs).  All CTAs must be co-resident: needs cooperative launch
  * (CUTH_ERR_CUDA otherwise).  Asynchronous on `stream` like cuth_pcg_solve. */
 size_t cuth_batch_workspace_bytes(const cuth_grid_t* grid, int nrhs);

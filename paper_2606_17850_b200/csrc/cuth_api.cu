@@ -757,8 +757,8 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   rc = check_opts(opts);
   if (rc) return rc;
   if (nrhs < 1 || nrhs > kBatchMaxRhs) return CUTH_ERR_VALUE;
-  if (opts->precision != CUTH_FP64) return CUTH_ERR_VALUE;
   if (opts->preconditioner != CUTH_PRECOND_JACOBI && opts->preconditioner != CUTH_PRECOND_NONE) return CUTH_ERR_VALUE;
+  if (opts->precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
   if (!dia_D || !b_D || !x_D || !work_D || !result_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(work_D) || !aligned16(b_D) || ((uintptr_t)result_D & 7u))
     return CUTH_ERR_ALIGN;
@@ -793,6 +793,8 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   c.nrhs = nrhs; c.max_iters = opts->max_iters;
   c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
   c.ntiles = (int32_t)ntiles;
+  c.precision = opts->precision;
+  c.period = opts->true_resid_period > 0 ? opts->true_resid_period : 20;
   k_batch_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   BatchCtx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;

@@ -8,7 +8,8 @@
 //   * every grid-wide barrier and reduction serves all right-hand sides at once, so on the small grids where a
 //     single solve is bound by the ~4.5 us per phase of the barrier the batch costs little more
 //     than one solve.
-// FP64, M = diag(A) or I.  Vectors are stored right-hand-side-major: v[s * n + i].
+// FP64 or MIXED (each right-hand side has its own stage and switches on its own, eq. (14a)-(14c)), M = diag(A) or I.
+// Vectors are stored right-hand-side-major: v[s * n + i].
 // Phases per iteration (as cuth_persistent.cuh): A  p = z + beta p | B  mu = A p, p.mu | C  x, r, r.z, ||r||^2 |
 // D (on demand) t = b - A x | E (restart) r := t.  A right-hand side that has finished is skipped by every phase.
 #pragma once
@@ -30,6 +31,7 @@ struct BatchCtx {
   cuth_result_t* result;                                          // [nrhs]
   double rtol;
   int32_t nrhs, max_iters, jacobi, ntiles;   // ntiles: CTAs per chunk of S right-hand sides
+  int32_t precision, period;                 // CUTH_FP64 / CUTH_MIXED; true-residual period of the MIXED early stage
 };
 
 struct BatchWorkspace {
@@ -93,6 +95,42 @@ __device__ __forceinline__ double apply_row(const RowCoef& q, const DiaDev& A, c
   acc = fma(q.a2u, v2u, acc); acc = fma(q.a2l, v2l, acc);
   acc = fma(q.a3u, v3u, acc); acc = fma(q.a3l, v3l, acc);
   return acc;
+}
+
+// Row i of the fp32-stored operator (K3) applied in difference form (DESIGN.md R-F3); same loads and
+// order of operations as spmv_row<true>.
+struct RowCoef32 { float g1u, g1l, g2u, g2l, g3u, g3l; double s; };
+
+__device__ __forceinline__ RowCoef32 load_row32(const DiaDev& A, const RowCoef& q, int64_t i) {
+  RowCoef32 f;
+  const int64_t nx = A.nx, np = A.nxny;
+  f.g1u = q.up1 ? A.f1[i] : 0.f; f.g1l = q.lo1 ? A.f1[i - 1] : 0.f;
+  f.g2u = q.up2 ? A.f2[i] : 0.f; f.g2l = q.lo2 ? A.f2[i - nx] : 0.f;
+  f.g3u = q.up3 ? A.f3[i] : 0.f; f.g3l = q.lo3 ? A.f3[i - np] : 0.f;
+  f.s = A.s_layer[(unsigned)i / (unsigned)np];
+  return f;
+}
+
+__device__ __forceinline__ double apply_row32(const RowCoef32& f, const RowCoef& q, const DiaDev& A,
+                                              const double* __restrict__ v, int64_t i, double vi) {
+  const int64_t nx = A.nx, np = A.nxny;
+  const double v1u = q.up1 ? v[i + 1] : vi, v1l = q.lo1 ? v[i - 1] : vi;
+  const double v2u = q.up2 ? v[i + nx] : vi, v2l = q.lo2 ? v[i - nx] : vi;
+  const double v3u = q.up3 ? v[i + np] : vi, v3l = q.lo3 ? v[i - np] : vi;
+  double acc = f.s * vi;
+  acc = fma((double)f.g1u, v1u - vi, acc); acc = fma((double)f.g1l, v1l - vi, acc);
+  acc = fma((double)f.g2u, v2u - vi, acc); acc = fma((double)f.g2l, v2l - vi, acc);
+  acc = fma((double)f.g3u, v3u - vi, acc); acc = fma((double)f.g3l, v3l - vi, acc);
+  return acc;
+}
+
+// The index predicates of a row without its fp64 coefficients (early-stage-only chunks do not touch A1).
+__device__ __forceinline__ RowCoef row_predicates(const DiaDev& A, int64_t i) {
+  RowCoef q;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  q.up1 = i + 1 < n; q.lo1 = i >= 1; q.up2 = i + nx < n; q.lo2 = i >= nx; q.up3 = i + np < n; q.lo3 = i >= np;
+  q.a0 = q.a1u = q.a1l = q.a2u = q.a2l = q.a3u = q.a3l = 0.0;
+  return q;
 }
 
 // Block-level part of a batched reduction: NV values for each of the S right-hand sides of this CTA's chunk.
@@ -173,8 +211,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
   const bool jac = c.jacobi != 0;
   // the policy code reads its options from a Ctx: only these fields are consulted on this path
   Ctx pc;
-  pc.rtol = c.rtol; pc.precision = CUTH_FP64; pc.max_iters = c.max_iters; pc.period = 1 << 30; pc.cheb = 0;
-  pc.soft_restart = 0; pc.soft_drift2 = 0.0;
+  pc.rtol = c.rtol; pc.precision = c.precision; pc.max_iters = c.max_iters; pc.period = c.period; pc.cheb = 0;
+  pc.soft_restart = 1; pc.soft_drift2 = 1e-2;       // as cuth_pcg_solve (DESIGN.md R-G11)
   int parity = 0;
   if (threadIdx.x < nrhs) sc[threadIdx.x] = ctl_g[threadIdx.x];      // cleared by k_batch_set_ctx
   __syncthreads();
@@ -244,18 +282,30 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
       }
     }
     grid.sync();
-    // ---- B: mu = A p, p.mu
+    // ---- B: mu = A p, p.mu  (per right-hand side: the fp32-stored operator in its early stage, A1 after)
     {
       double acc[S];
+      bool early[S];
+      bool any_early = false, any_late = false;
 #pragma unroll
-      for (int s = 0; s < S; ++s) acc[s] = 0.0;
+      for (int s = 0; s < S; ++s) {
+        acc[s] = 0.0;
+        early[s] = live[s] && sc[s0 + s].stage == 0;
+        any_early = any_early || early[s];
+        any_late = any_late || (live[s] && !early[s]);
+      }
       CUTH_BROWS(i) {
-        const RowCoef rc = load_row(c.A, i);
+        const RowCoef rc = any_late ? load_row(c.A, i) : row_predicates(c.A, i);
+        RowCoef32 rf;
+        if (any_early) rf = load_row32(c.A, rc, i);
         double pi[S], m[S];
 #pragma unroll
         for (int s = 0; s < S; ++s) {
           pi[s] = 0.0; m[s] = 0.0;
-          if (live[s]) { pi[s] = c.p[o[s] + i]; m[s] = apply_row(rc, c.A, c.p + o[s], i, pi[s]); }
+          if (live[s]) {
+            pi[s] = c.p[o[s] + i];
+            m[s] = early[s] ? apply_row32(rf, rc, c.A, c.p + o[s], i, pi[s]) : apply_row(rc, c.A, c.p + o[s], i, pi[s]);
+          }
         }
 #pragma unroll
         for (int s = 0; s < S; ++s)

@@ -41,11 +41,12 @@ def rhs_set(w, nrhs):
     return B
 
 
-def _run(w, B, X0=None, precond=1, rtol=1e-8, max_iters=200000):
+def _run(w, B, X0=None, precond=1, rtol=1e-8, max_iters=200000, precision=0, period=20):
     import torch
     import paper_2606_17850_b200 as cu
     M = cu.DiaMatrix(grid_from_workload(w))
-    S = cu.BatchSolver(M, B.shape[0], cu.Opts(precision=cu.FP64, rtol=rtol, max_iters=max_iters, preconditioner=precond))
+    S = cu.BatchSolver(M, B.shape[0], cu.Opts(precision=precision, rtol=rtol, max_iters=max_iters, preconditioner=precond,
+                                              true_resid_period=period))
     x = torch.zeros(B.shape, dtype=torch.float64, device="cuda") if X0 is None else to_dev(X0)
     S.solve(to_dev(B), x)
     return x.cpu().numpy(), S.results(), M
@@ -72,6 +73,38 @@ def test_batch_vs_oracle(kw, nrhs):
         assert np.linalg.norm(r) <= 1e-8 * np.linalg.norm(B[s]), s
         assert abs(res[s].iterations - ref.iterations) <= max(5, 0.05 * ref.iterations), (s, res[s].iterations, ref.iterations)
         assert res[s].rel_resid_true == pytest.approx(np.linalg.norm(r) / np.linalg.norm(B[s]), rel=1e-3, abs=1e-10)
+
+
+@pytest.mark.parametrize("kw", GRIDS[1:])
+@pytest.mark.parametrize("nrhs", [2, 6])
+def test_batch_mixed_vs_oracle_and_single_policy(kw, nrhs):
+    """MIXED: north_star's bars per right-hand side (<= 1e-4 K, oracle-CSR true residual <= 1e-8), and every right-hand
+    side takes the stage decisions a single MIXED solve of it takes (same criterion; iteration of the switch and
+    iteration count up to the effect of the summation order on a threshold test: one true-residual period)."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    B = rhs_set(w, nrhs)
+    T = w.true_resid_period
+    X, res, M = _run(w, B, precision=cu.MIXED, period=T)
+    S1 = cu.Solver(M, cu.Opts(precision=cu.MIXED, true_resid_period=T))
+    for s in range(nrhs):
+        assert res[s].status == 0, s
+        if not B[s].any():
+            continue
+        ref = O.pcg(A, B[s], rtol=1e-10)
+        assert np.abs(X[s] - ref.x).max() <= 1e-4, s
+        r = B[s] - O.spmv(A, X[s])
+        assert np.linalg.norm(r) <= 1e-8 * np.linalg.norm(B[s]), s
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        S1.solve(to_dev(B[s]), x)
+        r1 = S1.result()
+        assert res[s].promotions == r1.promotions == 1
+        assert res[s].switch_reason == r1.switch_reason
+        assert abs(res[s].switch_iteration - r1.switch_iteration) <= T
+        assert abs(res[s].iterations - r1.iterations) <= max(3, T)
+        assert abs(res[s].true_resid_evals - r1.true_resid_evals) <= 2
 
 
 def test_batch_matches_single_solves():
@@ -136,7 +169,6 @@ def test_batch_argument_errors():
             cu.cuth_pcg_solve_batch(M.buf, g, opts, nrhs, b, x, work, S.result_dev)
         return e.value.code
 
-    assert code(cu.Opts(precision=cu.MIXED)) == -3
     assert code(cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_lmin=1.0, cheb_lmax=2.0)) == -3
     assert code(cu.Opts(), nrhs=0) == -3 and code(cu.Opts(), nrhs=33) == -3
     assert code(cu.Opts(), work=S.work[:S.work.numel() - 256]) == -4
