@@ -125,3 +125,34 @@ def test_cheb_launch_schedule_host_side(cu):
         assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
     finally:
         cu.cuth_set_cheb_fusion(0)
+
+
+def test_batch_and_import_host_side(cu):
+    """Pure-host behaviour of the two calls added last: batch workspace size (0 on a bad count, grows by three
+    vectors per right-hand side) and the argument checks that come before any CUDA call."""
+    g = cu.Grid(32, 32, 8, 1e-6, 1e-6, np.full(8, 1e-6), None, 1e4)
+    n = 32 * 32 * 8
+    assert cu.cuth_batch_workspace_bytes(g, 0) == 0 and cu.cuth_batch_workspace_bytes(g, 33) == 0
+    sizes = [cu.cuth_batch_workspace_bytes(g, k) for k in range(1, 33)]
+    assert all(b - a == 3 * 8 * n for a, b in zip(sizes, sizes[1:]))            # r, p, mu per right-hand side
+    assert sizes[0] >= 3 * 8 * n and sizes[0] % 256 == 0
+    lib = cu.load_library()
+    from paper_2606_17850_b200.binding import cuth_import_report_t
+    rep = cuth_import_report_t()
+    p = C.c_void_p(4096)
+    big = cu.cuth_dia_bytes(g)
+    assert lib.cuth_import_csr(g.ref(), None, p, p, None, p, big, C.byref(rep), None) == -1       # NULL rowptr
+    assert lib.cuth_import_csr(g.ref(), p, p, p, None, None, big, C.byref(rep), None) == -1       # NULL matrix
+    assert lib.cuth_import_csr(g.ref(), p, p, p, None, p, big - 1, C.byref(rep), None) == -4      # buffer too small
+    assert lib.cuth_import_csr(g.ref(), C.c_void_p(4100), p, p, None, p, big, C.byref(rep), None) == -5
+    neg = np.full(8, -1.0)
+    assert lib.cuth_import_csr(g.ref(), p, p, p, neg.ctypes.data_as(C.c_void_p), p, big, C.byref(rep), None) == -3
+    bad = cu.Grid(1, 4, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
+    assert lib.cuth_import_csr(bad.ref(), p, p, p, None, p, big, C.byref(rep), None) == -2
+    o = cu.Opts()
+    assert lib.cuth_pcg_solve_batch(p, g.ref(), C.byref(o), 0, p, p, p, 1 << 30, p, None) == -3   # nrhs out of range
+    assert lib.cuth_pcg_solve_batch(p, g.ref(), C.byref(o), 33, p, p, p, 1 << 30, p, None) == -3
+    oc = cu.Opts(preconditioner=cu.PRECOND_CHEBYSHEV, cheb_lmin=1.0, cheb_lmax=2.0)
+    assert lib.cuth_pcg_solve_batch(p, g.ref(), C.byref(oc), 2, p, p, p, 1 << 30, p, None) == -3  # no Chebyshev batch
+    assert lib.cuth_pcg_solve_batch(p, g.ref(), C.byref(o), 2, None, p, p, 1 << 30, p, None) == -1
+    assert lib.cuth_pcg_solve_batch(p, g.ref(), C.byref(o), 2, p, p, p, 1024, p, None) == -4      # workspace too small
