@@ -588,6 +588,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
   c.cheb = 0;
   if (cheb) fill_cheb(&c, opts, w);
+  c.persist_fuse = L.n <= (1 << 14) ? 1 : 0;   // persistent kernel: phases A and B in one on the smallest grids
   c.soft_restart = 1;         // promotion keeps p while the drift is small (DESIGN.md R-G11)
   c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);

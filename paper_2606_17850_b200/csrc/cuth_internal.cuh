@@ -88,6 +88,7 @@ struct Ctx {
   double soft_drift2;   // soft restart allowed while ||t - r||^2 <= soft_drift2 * ||t||^2
   int32_t precision, max_iters, period, jacobi;
   int32_t soft_restart, cheb;     // cheb: degree k of the Chebyshev polynomial preconditioner, 0 = off
+  int32_t persist_fuse, pad_pf;   // persistent kernel: phases A and B in one (p' recomputed at the six neighbours)
   // Chebyshev preconditioner (Alg. 3): z = q(A) r.  cz: z (fp64) handed to the outer
   // loop; cd[4]: partial-sum buffers Z (two are live at any time; the fused two-pass kernel writes the other
   // two); crc: fp32 copy of r (MIXED only).  Element type T = double in FP64 mode, float in MIXED mode;

@@ -77,6 +77,70 @@ __device__ __forceinline__ double persistent_spmv_phase(const Ctx& c, int64_t n,
   return acc;
 }
 
+// Phases A and B in one, for the smallest grids (a phase there is one barrier + one L2 round trip): row i forms
+// p' = z + beta p not only for itself but also for its six neighbours -- the same fma on the same operands as their
+// owners, hence bitwise the same values -- and applies A to them, which removes the barrier between A and B.  p' goes
+// to the other direction buffer (the neighbours still read the old one).  21 + 7 independent loads per row instead
+// of 3 and 7 + 7: pays only while the barrier outweighs them (measured: 8 k rows 7.26 -> 7.01 us per iteration,
+// 66 k rows 8.1 -> 8.9, 1 M rows 23 -> 32), so cuth_api.cu switches it on up to 16 k rows.
+template <bool MIXED>
+__device__ __forceinline__ double fused_dir_spmv_row(const Ctx& c, const double* __restrict__ pold,
+                                                     int64_t i, double beta, bool jac, double& p_i) {
+  const DiaDev& A = c.A;
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx, up3 = i + np < n, lo3 = i >= np;
+  auto dir = [&](int64_t j) {
+    const double rj = c.r[j];
+    return fma(beta, pold[j], jac ? rj * A.dinv[j] : rj);
+  };
+  const double vi = dir(i);
+  double acc;
+  if (!MIXED) {
+    const double a0 = A.d0[i];
+    const double a1u = up1 ? A.d1[i] : 0.0, a1l = lo1 ? A.d1[i - 1] : 0.0;
+    const double a2u = up2 ? A.d2[i] : 0.0, a2l = lo2 ? A.d2[i - nx] : 0.0;
+    const double a3u = up3 ? A.d3[i] : 0.0, a3l = lo3 ? A.d3[i - np] : 0.0;
+    const double v1u = up1 ? dir(i + 1) : 0.0, v1l = lo1 ? dir(i - 1) : 0.0;
+    const double v2u = up2 ? dir(i + nx) : 0.0, v2l = lo2 ? dir(i - nx) : 0.0;
+    const double v3u = up3 ? dir(i + np) : 0.0, v3l = lo3 ? dir(i - np) : 0.0;
+    acc = a0 * vi;
+    acc = fma(a1u, v1u, acc); acc = fma(a1l, v1l, acc);
+    acc = fma(a2u, v2u, acc); acc = fma(a2l, v2l, acc);
+    acc = fma(a3u, v3u, acc); acc = fma(a3l, v3l, acc);
+  } else {
+    const float g1u = up1 ? A.f1[i] : 0.f, g1l = lo1 ? A.f1[i - 1] : 0.f;
+    const float g2u = up2 ? A.f2[i] : 0.f, g2l = lo2 ? A.f2[i - nx] : 0.f;
+    const float g3u = up3 ? A.f3[i] : 0.f, g3l = lo3 ? A.f3[i - np] : 0.f;
+    const double v1u = up1 ? dir(i + 1) : vi, v1l = lo1 ? dir(i - 1) : vi;
+    const double v2u = up2 ? dir(i + nx) : vi, v2l = lo2 ? dir(i - nx) : vi;
+    const double v3u = up3 ? dir(i + np) : vi, v3l = lo3 ? dir(i - np) : vi;
+    const unsigned z = (unsigned)i / (unsigned)np;
+    acc = A.s_layer[z] * vi;
+    acc = fma((double)g1u, v1u - vi, acc); acc = fma((double)g1l, v1l - vi, acc);
+    acc = fma((double)g2u, v2u - vi, acc); acc = fma((double)g2l, v2l - vi, acc);
+    acc = fma((double)g3u, v3u - vi, acc); acc = fma((double)g3l, v3l - vi, acc);
+  }
+  p_i = vi;
+  return acc;
+}
+
+template <bool MIXED>
+__device__ __forceinline__ double persistent_fused_phase(const Ctx& c, const double* __restrict__ pold,
+                                                         double* __restrict__ pnew, double beta, bool jac, int64_t n,
+                                                         int64_t gstride) {
+  double acc = 0.0;
+  CUTH_ROWS2(i0, i1, h1) {
+    double p0, p1 = 0.0;
+    const double m0 = fused_dir_spmv_row<MIXED>(c, pold, i0, beta, jac, p0);
+    const double m1 = h1 ? fused_dir_spmv_row<MIXED>(c, pold, i1, beta, jac, p1) : 0.0;
+    pnew[i0] = p0; c.mu[i0] = m0;
+    if (h1) { pnew[i1] = p1; c.mu[i1] = m1; }
+    acc = fma(p0, m0, acc);
+    acc = fma(p1, m1, acc);
+  }
+  return acc;
+}
+
 __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __restrict__ ctxp, Ctl* ctl_g,
                                                                double* partials) {
   cg::grid_group grid = cg::this_grid();
@@ -107,23 +171,34 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
     __syncthreads();
   }
   bool go = sc.want_true != 0;
+  const bool fuse = c.persist_fuse != 0;
+  double* pcur = c.p;              // the buffer that holds p: the fused phase ping-pongs between c.p and c.p2
 
   while (go) {
-    // ---- A: p = z + beta p
-    {
+    double acc[1];
+    if (fuse) {
+      // ---- A + B: p' = z + beta p at the row and its six neighbours, mu = A p', p'.mu
       const double beta = sc.beta;
-      CUTH_ROWS2(i0, i1, h1) {
-        const double r0 = c.r[i0], q0 = c.p[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
-        const double r1 = h1 ? c.r[i1] : 0.0, q1 = h1 ? c.p[i1] : 0.0, d1 = (h1 && jac) ? c.A.dinv[i1] : 1.0;
-        c.p[i0] = fma(beta, q0, jac ? r0 * d0 : r0);
-        if (h1) c.p[i1] = fma(beta, q1, jac ? r1 * d1 : r1);
+      double* pnew = (pcur == c.p) ? c.p2 : c.p;
+      acc[0] = sc.stage == 0 ? persistent_fused_phase<true>(c, pcur, pnew, beta, jac, n, gstride)
+                             : persistent_fused_phase<false>(c, pcur, pnew, beta, jac, n, gstride);
+      pcur = pnew;
+    } else {
+      // ---- A: p = z + beta p
+      {
+        const double beta = sc.beta;
+        CUTH_ROWS2(i0, i1, h1) {
+          const double r0 = c.r[i0], q0 = c.p[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
+          const double r1 = h1 ? c.r[i1] : 0.0, q1 = h1 ? c.p[i1] : 0.0, d1 = (h1 && jac) ? c.A.dinv[i1] : 1.0;
+          c.p[i0] = fma(beta, q0, jac ? r0 * d0 : r0);
+          if (h1) c.p[i1] = fma(beta, q1, jac ? r1 * d1 : r1);
+        }
       }
-    }
-    grid.sync();
-    // ---- B: mu = A p, p.mu
-    {
-      double acc[1];
+      grid.sync();
+      // ---- B: mu = A p, p.mu
       acc[0] = sc.stage == 0 ? persistent_spmv_phase<true>(c, n, gstride) : persistent_spmv_phase<false>(c, n, gstride);
+    }
+    {
       grid_allreduce<1>(grid, acc, partials, parity, smem);
       if (threadIdx.x == 0) policy_after_spmv(&sc, acc[0], false);
       __syncthreads();
@@ -134,9 +209,9 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
       const double alpha = sc.alpha;
       double acc[2] = {0.0, 0.0};
       CUTH_ROWS2(i0, i1, h1) {
-        const double x0 = c.x[i0], q0 = c.p[i0], m0 = c.mu[i0], r0 = c.r[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
+        const double x0 = c.x[i0], q0 = pcur[i0], m0 = c.mu[i0], r0 = c.r[i0], d0 = jac ? c.A.dinv[i0] : 1.0;
         double x1 = 0.0, q1 = 0.0, m1 = 0.0, r1 = 0.0, d1 = 1.0;
-        if (h1) { x1 = c.x[i1]; q1 = c.p[i1]; m1 = c.mu[i1]; r1 = c.r[i1]; if (jac) d1 = c.A.dinv[i1]; }
+        if (h1) { x1 = c.x[i1]; q1 = pcur[i1]; m1 = c.mu[i1]; r1 = c.r[i1]; if (jac) d1 = c.A.dinv[i1]; }
         c.x[i0] = fma(alpha, q0, x0);
         const double s0 = fma(-alpha, m0, r0);
         const double z0 = jac ? s0 * d0 : s0;
