@@ -140,6 +140,13 @@ int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int3
                     const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
                     void* stream);
 
+/* The same import from COORDINATE format: nnz entries (row_D[q], col_D[q], val_D[q]) in any order (int32 indices,
+ * device).  Same checks, same report, same matrix object as cuth_import_csr (one thread per entry; a coordinate met
+ * twice counts as a duplicate whichever copy came first).  SYNCHRONISES `stream`. */
+int cuth_import_coo(const cuth_grid_t* grid, const int32_t* row_D, const int32_t* col_D, const double* val_D, int64_t nnz,
+                    const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
+                    void* stream);
+
 /* View of the matrix object for the bit-exact layout test: device pointers to the packed fp64
  * values and to the fp32 copy (same ptr/off), and the host copies of ptr[5], off[4].
  * Any output pointer may be NULL.  Pure host arithmetic, no CUDA call. */

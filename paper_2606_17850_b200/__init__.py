@@ -7,7 +7,7 @@ importing `binding` without the compiled library, or calling it without a CUDA d
 """
 from .binding import (  # noqa: F401
     CuthError, Grid, Opts, Result, DiaMatrix, Solver, BatchSolver, cuth_batch_workspace_bytes, cuth_pcg_solve_batch,
-    cuth_dia_bytes, cuth_workspace_bytes, cuth_build_dia, cuth_import_csr, cuth_dia_view, cuth_spmv,
+    cuth_dia_bytes, cuth_workspace_bytes, cuth_build_dia, cuth_import_csr, cuth_import_coo, cuth_dia_view, cuth_spmv,
     cuth_pcg_solve, cuth_transient_step, cuth_release_workspace, cuth_version,
     cuth_launches_per_iteration, cuth_profile_kernel, cuth_set_traversal, cuth_set_loop_mode, cuth_set_k1_variant, cuth_set_cheb_fusion, cuth_cheb_launches, cuth_set_pair_occupancy, cuth_set_pair_rows, cuth_lanczos_bounds, cuth_cheb_apply, cuth_tridiag_extremes, load_library, exported_symbols,
     FP64, MIXED, ABLATION_STD32, PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV, CHEB_DEFAULT, CHEB_A3_FP16,

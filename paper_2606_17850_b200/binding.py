@@ -56,7 +56,7 @@ class cuth_import_report_t(C.Structure):
                 ("mixed_ok", C.c_int32)]
 
 
-EXPORTS = ["cuth_import_csr", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
+EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
            "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
            "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy", "cuth_set_pair_rows"]
 
@@ -85,6 +85,8 @@ def load_library():
     L.cuth_build_dia.argtypes = [gp, vp, C.c_size_t, vp]
     L.cuth_import_csr.restype = C.c_int
     L.cuth_import_csr.argtypes = [gp, vp, vp, vp, vp, vp, C.c_size_t, C.POINTER(cuth_import_report_t), vp]
+    L.cuth_import_coo.restype = C.c_int
+    L.cuth_import_coo.argtypes = [gp, vp, vp, vp, C.c_int64, vp, vp, C.c_size_t, C.POINTER(cuth_import_report_t), vp]
     L.cuth_dia_view.restype = C.c_int
     L.cuth_dia_view.argtypes = [vp, gp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp),
                                 C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -208,6 +210,22 @@ def cuth_import_csr(grid: Grid, rowptr, col, val, dia, rowsum_layer=None, stream
     if not check:
         return rc, rep
     _check(rc, "cuth_import_csr")
+    return rep
+
+
+def cuth_import_coo(grid: Grid, row, col, val, dia, rowsum_layer=None, stream=None, check=True):
+    """row, col int32 / val float64 CUDA tensors of equal length (any order).  As cuth_import_csr."""
+    import torch
+    assert row.dtype == torch.int32 and col.dtype == torch.int32 and val.dtype == torch.float64
+    assert row.numel() == col.numel() == val.numel()
+    rep = cuth_import_report_t()
+    rs = None if rowsum_layer is None else np.ascontiguousarray(rowsum_layer, dtype=np.float64)
+    rc = load_library().cuth_import_coo(grid.ref(), _ptr(row), _ptr(col), _ptr(val), C.c_int64(val.numel()),
+                                        None if rs is None else rs.ctypes.data_as(C.c_void_p), _ptr(dia),
+                                        dia.numel() * dia.element_size(), C.byref(rep), stream or _stream())
+    if not check:
+        return rc, rep
+    _check(rc, "cuth_import_coo")
     return rep
 
 

@@ -27,7 +27,7 @@ namespace cuth {
 int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStream_t st, cudaError_t* err);
 int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowptr_D, const int32_t* col_D,
                   const double* val_D, const double* rowsum_layer_H, void* dia_D, cuth_import_report_t* rep,
-                  cudaStream_t st, cudaError_t* err);
+                  cudaStream_t st, cudaError_t* err, const int32_t* coo_row_D = nullptr, int64_t nnz = 0);
 
 static thread_local std::string g_last_err;
 
@@ -741,6 +741,31 @@ int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t
                    double* x_D, void* work_D, size_t work_bytes, cuth_result_t* result_D, void* stream) {
   if (!b_D) return CUTH_ERR_NULL;
   return solve_common(dia_D, grid, opts, b_D, nullptr, x_D, work_D, work_bytes, result_D, stream);
+}
+
+int cuth_import_coo(const cuth_grid_t* grid, const int32_t* row_D, const int32_t* col_D, const double* val_D, int64_t nnz,
+                    const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
+                    void* stream) {
+  DiaLayout L;
+  int rc = check_grid(grid, &L);
+  if (rc) return rc;
+  if (!dia_D || !row_D || !col_D || !val_D) return CUTH_ERR_NULL;
+  if (nnz < 0) return CUTH_ERR_VALUE;
+  if (!aligned16(dia_D) || ((uintptr_t)row_D & 3u) || ((uintptr_t)col_D & 3u) || ((uintptr_t)val_D & 7u))
+    return CUTH_ERR_ALIGN;
+  if (dia_bytes < L.bytes) return CUTH_ERR_SIZE;
+  if (rowsum_layer_H)
+    for (int64_t z = 0; z < grid->nz; ++z)
+      if (!(rowsum_layer_H[z] >= 0.0) || std::isinf(rowsum_layer_H[z])) return CUTH_ERR_VALUE;
+  cuth_import_report_t rep;
+  memset(&rep, 0, sizeof rep);
+  cudaError_t e = cudaSuccess;
+  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
+  rc = launch_import(grid, L, nullptr, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e, row_D, nnz);
+  if (report_H) *report_H = rep;
+  if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_import_coo");
+  if (rc == CUTH_OK) { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported[dia_D] = rep.mixed_ok; }
+  return rc;
 }
 
 size_t cuth_batch_workspace_bytes(const cuth_grid_t* grid, int nrhs) {

@@ -169,6 +169,7 @@ struct ImportArgs {
   int64_t n, nx, ny, nxny;
   int32_t nz;
   const int64_t* rowptr; const int32_t* col; const double* val;
+  const int32_t* coo_row; int64_t nnz; unsigned int* seen;   // COO input: row index per entry; seen[n]: slot bits per row
   double* d0; double* d1; double* d2; double* d3;
   unsigned long long* cnt;     // [0] off-stencil, [1] asymmetric, [2] bad diagonal, [3] duplicates, [4] positive off-diagonals
   unsigned long long* rs_min;  // [nz] order-preserving keys of the per-layer min / max row sum and min D0
@@ -222,6 +223,37 @@ __global__ void __launch_bounds__(256) k_import_upper(ImportArgs a) {
   if (pos) atomicAdd(&a.cnt[4], pos);
 }
 
+// Row sum D0 + the six off-diagonal entries of row i in the fixed order -z, -y, -x, +x, +y, +z (m1..m3: the stored
+// mirrors of the lower entries), folded into the per-layer min / max of the row sums and min of D0.
+__device__ __forceinline__ void rowsum_minmax(const ImportArgs& a, int64_t i, double m1, double m2, double m3) {
+  const double d = a.d0[i];
+  double rs = d;
+  rs = __dadd_rn(rs, m3); rs = __dadd_rn(rs, m2); rs = __dadd_rn(rs, m1);
+  if (i + 1 < a.n) rs = __dadd_rn(rs, a.d1[i]);
+  if (i + a.nx < a.n) rs = __dadd_rn(rs, a.d2[i]);
+  if (i + a.nxny < a.n) rs = __dadd_rn(rs, a.d3[i]);
+  const int64_t z = i / a.nxny;
+  // a full warp inside one layer (the common case) reduces by shuffle: one atomic per warp and quantity
+  unsigned long long kmin = ordered_key(rs), kmax = kmin, kd = ordered_key(d);
+  const unsigned mask = __activemask();
+  bool uniform = false;
+  if (mask == 0xffffffffu) {
+    const int64_t z0 = __shfl_sync(mask, z, 0);
+    uniform = __all_sync(mask, z == z0);
+    if (uniform) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long t1 = __shfl_xor_sync(mask, kmin, o), t2 = __shfl_xor_sync(mask, kmax, o),
+                                 t3 = __shfl_xor_sync(mask, kd, o);
+        kmin = t1 < kmin ? t1 : kmin; kmax = t2 > kmax ? t2 : kmax; kd = t3 < kd ? t3 : kd;
+      }
+    }
+  }
+  if (!uniform || (threadIdx.x & 31) == 0) {
+    atomicMin(&a.rs_min[z], kmin); atomicMax(&a.rs_max[z], kmax); atomicMin(&a.d0_min[z], kd);
+  }
+}
+
 // Pass 2, one thread per row: every lower entry must equal the stored mirror (absent == 0), and the row sum
 // D0 + sum of the six off-diagonal entries (fixed order -z, -y, -x, +x, +y, +z) feeds the per-layer min / max.
 __global__ void __launch_bounds__(256) k_import_lower(ImportArgs a) {
@@ -243,34 +275,81 @@ __global__ void __launch_bounds__(256) k_import_lower(ImportArgs a) {
     const double m2 = i >= a.nx ? a.d2[i - a.nx] : 0.0;
     const double m3 = i >= a.nxny ? a.d3[i - a.nxny] : 0.0;
     if (!(l1 == m1) || !(l2 == m2) || !(l3 == m3)) ++asym;
-    const double d = a.d0[i];
-    double rs = d;
-    rs = __dadd_rn(rs, m3); rs = __dadd_rn(rs, m2); rs = __dadd_rn(rs, m1);
-    if (i + 1 < a.n) rs = __dadd_rn(rs, a.d1[i]);
-    if (i + a.nx < a.n) rs = __dadd_rn(rs, a.d2[i]);
-    if (i + a.nxny < a.n) rs = __dadd_rn(rs, a.d3[i]);
-    const int64_t z = i / a.nxny;
-    // a full warp inside one layer (the common case) reduces by shuffle: one atomic per warp and quantity
-    unsigned long long kmin = ordered_key(rs), kmax = kmin, kd = ordered_key(d);
-    const unsigned mask = __activemask();
-    bool uniform = false;
-    if (mask == 0xffffffffu) {
-      const int64_t z0 = __shfl_sync(mask, z, 0);
-      uniform = __all_sync(mask, z == z0);
-      if (uniform) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          const unsigned long long t1 = __shfl_xor_sync(mask, kmin, o), t2 = __shfl_xor_sync(mask, kmax, o),
-                                   t3 = __shfl_xor_sync(mask, kd, o);
-          kmin = t1 < kmin ? t1 : kmin; kmax = t2 > kmax ? t2 : kmax; kd = t3 < kd ? t3 : kd;
-        }
-      }
-    }
-    if (!uniform || (threadIdx.x & 31) == 0) {
-      atomicMin(&a.rs_min[z], kmin); atomicMax(&a.rs_max[z], kmax); atomicMin(&a.d0_min[z], kd);
-    }
+    rowsum_minmax(a, i, m1, m2, m3);
   }
   if (asym) atomicAdd(&a.cnt[1], asym);
+}
+
+// ---- COO input (SURVEY.md §8(f) "CSR / COO import"): the same checks with one thread per ENTRY.
+// seen[i] bit s (s = 0 diagonal, 1..3 upper +1 / +nx / +nx*ny, 4..6 lower) = an on-stencil entry of row i was met in
+// slot s; bit 8 = a lower entry of row i differs from its mirror.
+__device__ __forceinline__ int coo_slot(const ImportArgs& a, int64_t i, int64_t j, bool* legal) {
+  *legal = i >= 0 && i < a.n && j >= 0 && j < a.n;
+  if (!*legal) return -1;
+  const int64_t c = j - i, rem = i % a.nxny, x = rem % a.nx, y = rem / a.nx;
+  if (c == 0) return 0;
+  if (c == 1) { *legal = x + 1 < a.nx; return 1; }
+  if (c == a.nx) { *legal = y + 1 < a.ny; return 2; }
+  if (c == a.nxny) return 3;
+  if (c == -1) { *legal = x > 0; return 4; }
+  if (c == -a.nx) { *legal = y > 0; return 5; }
+  if (c == -a.nxny) return 6;
+  return -1;
+}
+
+__global__ void __launch_bounds__(256) k_coo_scatter(ImportArgs a) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned long long off_st = 0, dup = 0, pos = 0;
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < a.nnz; q += stride) {
+    const int64_t i = a.coo_row[q], j = a.col[q];
+    const double v = a.val[q];
+    bool legal;
+    const int slot = coo_slot(a, i, j, &legal);
+    if (slot < 0 || !legal) { if (v != 0.0) ++off_st; continue; }
+    const unsigned old = atomicOr(&a.seen[i], 1u << slot);
+    if (old & (1u << slot)) { ++dup; continue; }
+    if (slot == 0) a.d0[i] = v; else if (slot == 1) a.d1[i] = v; else if (slot == 2) a.d2[i] = v; else if (slot == 3) a.d3[i] = v;
+    if (slot != 0 && v > 0.0) ++pos;
+  }
+  if (off_st) atomicAdd(&a.cnt[0], off_st);
+  if (dup) atomicAdd(&a.cnt[3], dup);
+  if (pos) atomicAdd(&a.cnt[4], pos);
+}
+
+__global__ void __launch_bounds__(256) k_coo_mirror(ImportArgs a) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < a.nnz; q += stride) {
+    const int64_t i = a.coo_row[q], j = a.col[q];
+    bool legal;
+    const int slot = coo_slot(a, i, j, &legal);
+    if (slot < 4 || !legal) continue;
+    const double m = slot == 4 ? a.d1[j] : (slot == 5 ? a.d2[j] : a.d3[j]);      // the mirror is element j of its diagonal
+    if (!(a.val[q] == m)) atomicOr(&a.seen[i], 1u << 8);
+  }
+}
+
+__global__ void __launch_bounds__(256) k_coo_rows(ImportArgs a) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned long long asym = 0, bad = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
+    const unsigned sn = a.seen[i];
+    const int64_t rem = i % a.nxny;
+    const bool has_xm = rem % a.nx > 0, has_ym = rem / a.nx > 0;
+    const double m1 = i >= 1 ? a.d1[i - 1] : 0.0;
+    const double m2 = i >= a.nx ? a.d2[i - a.nx] : 0.0;
+    const double m3 = i >= a.nxny ? a.d3[i - a.nxny] : 0.0;
+    bool as = (sn >> 8) & 1u;
+    // a mirror that is stored non-zero while row i has no lower entry there (absent == 0)
+    if (has_xm && !(sn & (1u << 4)) && m1 != 0.0) as = true;
+    if (has_ym && !(sn & (1u << 5)) && m2 != 0.0) as = true;
+    if (!(sn & (1u << 6)) && m3 != 0.0) as = true;
+    if (as) ++asym;
+    const double d = a.d0[i];
+    if (!(sn & 1u) || !(d > 0.0) || isinf(d)) ++bad;
+    rowsum_minmax(a, i, m1, m2, m3);
+  }
+  if (asym) atomicAdd(&a.cnt[1], asym);
+  if (bad) atomicAdd(&a.cnt[2], bad);
 }
 
 // fp32 copy A2 (round-to-nearest-even of the packed values) and 1/D0, as the builder writes them.
@@ -294,7 +373,7 @@ static double key_to_double(unsigned long long k) {
 // Host side of cuth_import_csr.  Synchronises `st` (setup call).  rowsum_layer_H may be nullptr.
 int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowptr_D, const int32_t* col_D,
                   const double* val_D, const double* rowsum_layer_H, void* dia_D, cuth_import_report_t* rep,
-                  cudaStream_t st, cudaError_t* err) {
+                  cudaStream_t st, cudaError_t* err, const int32_t* coo_row_D, int64_t nnz) {
   char* base = (char*)dia_D;
   const int nz = (int)L.nz;
   const size_t nlay = 4 * (size_t)nz + 4;
@@ -320,8 +399,21 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   a.rs_min = lay; a.rs_max = lay + nz; a.d0_min = lay + 2 * nz;
   int64_t blocks = (L.n + 255) / 256;
   if (blocks > 148 * 64) blocks = 148 * 64;
-  k_import_upper<<<(unsigned)blocks, 256, 0, st>>>(a);
-  k_import_lower<<<(unsigned)blocks, 256, 0, st>>>(a);
+  a.coo_row = coo_row_D; a.nnz = nnz; a.seen = (unsigned int*)(base + L.o_dinv);    // scratch until k_import_finish
+  if (coo_row_D) {
+    e = cudaMemsetAsync(v, 0, sizeof(double) * (size_t)L.e, st);                    // a missing entry is +0.0
+    if (e == cudaSuccess) e = cudaMemsetAsync(a.seen, 0, sizeof(unsigned int) * (size_t)L.n, st);
+    if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+    int64_t eb = (nnz + 255) / 256;
+    if (eb > 148 * 64) eb = 148 * 64;
+    if (eb < 1) eb = 1;
+    k_coo_scatter<<<(unsigned)eb, 256, 0, st>>>(a);
+    k_coo_mirror<<<(unsigned)eb, 256, 0, st>>>(a);
+    k_coo_rows<<<(unsigned)blocks, 256, 0, st>>>(a);
+  } else {
+    k_import_upper<<<(unsigned)blocks, 256, 0, st>>>(a);
+    k_import_lower<<<(unsigned)blocks, 256, 0, st>>>(a);
+  }
   k_import_finish<<<(unsigned)blocks, 256, 0, st>>>(v, f, L.e, (double*)(base + L.o_dinv), L.n);
   BuildArgs b;
   memset(&b, 0, sizeof b);

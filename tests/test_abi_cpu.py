@@ -147,6 +147,9 @@ def test_batch_and_import_host_side(cu):
     assert lib.cuth_import_csr(g.ref(), C.c_void_p(4100), p, p, None, p, big, C.byref(rep), None) == -5
     neg = np.full(8, -1.0)
     assert lib.cuth_import_csr(g.ref(), p, p, p, neg.ctypes.data_as(C.c_void_p), p, big, C.byref(rep), None) == -3
+    assert lib.cuth_import_coo(g.ref(), None, p, p, C.c_int64(10), None, p, big, C.byref(rep), None) == -1
+    assert lib.cuth_import_coo(g.ref(), p, p, p, C.c_int64(-1), None, p, big, C.byref(rep), None) == -3
+    assert lib.cuth_import_coo(g.ref(), p, p, p, C.c_int64(10), None, p, big - 1, C.byref(rep), None) == -4
     bad = cu.Grid(1, 4, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
     assert lib.cuth_import_csr(bad.ref(), p, p, p, None, p, big, C.byref(rep), None) == -2
     o = cu.Opts()

@@ -206,3 +206,82 @@ def test_import_argument_errors():
     with pytest.raises(cu.CuthError) as e:
         S.step(to_dev(wt.power), T)
     assert e.value.code == -7
+
+
+def _coo_dev(A, seed=None):
+    """The CSR matrix as (row, col, val) int32 / int32 / float64 device arrays, entries shuffled when seed is given."""
+    import torch
+    rows = np.repeat(np.arange(A.n, dtype=np.int32), np.diff(A.rowptr))
+    cols, vals = A.col.astype(np.int32), A.val
+    if seed is not None:
+        p = np.random.default_rng(seed).permutation(rows.size)
+        rows, cols, vals = rows[p], cols[p], vals[p]
+    return (torch.from_numpy(np.ascontiguousarray(rows)).cuda(), torch.from_numpy(np.ascontiguousarray(cols)).cuda(),
+            torch.from_numpy(np.ascontiguousarray(vals)).cuda())
+
+
+@pytest.mark.parametrize("kw", CASES + [dict(cfg=2)])
+def test_import_coo_is_bit_exact(kw):
+    """cuth_import_coo on the shuffled entries writes byte for byte the object cuth_import_csr writes."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    vals_o, _, _ = O.csr_to_dia(A, w.nx, w.ny, w.nz)
+    g = grid_from_workload(w)
+    M = cu.DiaMatrix(g, csr=_csr_dev(A))
+    buf = torch.empty_like(M.buf)
+    rep = cu.cuth_import_coo(g, *_coo_dev(A, seed=11), buf)
+    assert (rep.off_stencil, rep.asymmetric_rows, rep.bad_diagonal, rep.duplicates, rep.positive_offdiag) == (0,) * 5
+    assert rep.mixed_ok == 1 and rep.max_rowsum_dev == M.import_report.max_rowsum_dev
+    v, _, _, ptr, _ = cu.cuth_dia_view(buf, g)
+    e = ptr[4]
+    got = buf[v - buf.data_ptr(): v - buf.data_ptr() + 8 * e].view(torch.float64).cpu().numpy()
+    assert np.array_equal(got.view(np.uint64), vals_o.view(np.uint64))
+    lay_end = 512 + 256 * (((4 * w.nz + 4) * 8 + 255) // 256)
+    al = lambda q: (q + 255) // 256 * 256
+    n = w.n
+    sections = [(512 + 8 * w.nz, 8 * w.nz), (512 + 32 * w.nz, 24), (lay_end, 8 * e), (al(lay_end + 8 * e), 4 * e),
+                (al(al(lay_end + 8 * e) + 4 * e), 8 * n)]                  # s(z) | fp16 scale | A1 | A2 | 1/D0
+    o_h16 = al(al(al(lay_end + 8 * e) + 4 * e) + 8 * n)
+    o_f32a = o_h16 + 3 * al(2 * n)
+    sections += [(o_h16 + k * al(2 * n), 2 * n) for k in range(3)] + [(o_f32a + k * al(4 * n), 4 * n) for k in range(3)]
+    for a, nb in sections:
+        assert bool((buf[a:a + nb] == M.buf[a:a + nb]).all()), a
+    # and it solves: MIXED on the COO-imported object
+    x = torch.zeros(n, dtype=torch.float64, device="cuda")
+    opts = cu.Opts(precision=cu.MIXED, true_resid_period=w.true_resid_period)
+    work = torch.empty(cu.cuth_workspace_bytes(g, opts), dtype=torch.uint8, device="cuda")
+    res = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    cu.cuth_pcg_solve(buf, g, opts, to_dev(w.power), x, work, res)
+    torch.cuda.synchronize()
+    cu.cuth_release_workspace(work)
+    assert int(res[:4].view(torch.int32).item()) == 0
+    r = w.power - O.spmv(A, x.cpu().numpy())
+    assert np.linalg.norm(r) <= 1e-8 * np.linalg.norm(w.power)
+
+
+def test_coo_validation_counts_match_the_oracle():
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(cfg=3, nx=12, ny=9, nz=5, n_hot=2)
+    A = O.assemble_workload(w)
+    g = grid_from_workload(w)
+    buf = torch.empty(cu.cuth_dia_bytes(g), dtype=torch.uint8, device="cuda")
+    for name, Af in faults(A, w.nx, w.ny, w.nz).items():
+        want = O.stencil7_report(Af, w.nx, w.ny, w.nz)
+        rc, rep = cu.cuth_import_coo(g, *_coo_dev(Af, seed=5), buf, check=False)
+        got = dict(off_stencil=rep.off_stencil, asymmetric_rows=rep.asymmetric_rows, bad_diagonal=rep.bad_diagonal,
+                   duplicates=rep.duplicates, positive_offdiag=rep.positive_offdiag)
+        if name == "duplicate":        # which copy of a repeated coordinate is kept is unspecified: only its count is
+            assert got["duplicates"] == want["duplicates"] == 1
+        else:
+            assert got == {k: want[k] for k in got}, name
+        assert rc == (0 if name == "explicit_zero_off_stencil" else -8), name
+    # a lower triangle that is missing altogether: every row with a lower neighbour is asymmetric
+    rows = np.repeat(np.arange(A.n), np.diff(A.rowptr))
+    keep = A.col >= rows
+    up = (torch.from_numpy(rows[keep].astype(np.int32)).cuda(), torch.from_numpy(A.col[keep].astype(np.int32)).cuda(),
+          torch.from_numpy(A.val[keep]).cuda())
+    rc, rep = cu.cuth_import_coo(g, *up, buf, check=False)
+    assert rc == -8 and rep.asymmetric_rows == A.n - 1 and rep.off_stencil == 0
