@@ -5,7 +5,9 @@
  *   - "_D" pointers are DEVICE pointers owned by the caller (allocate them with torch or cudaMalloc),
  *     "_H" pointers are HOST pointers.  The library allocates no device memory of its own; its only
  *     hidden host-side state is a cache of instantiated CUDA graphs keyed by the workspace address
- *     (released by cuth_release_workspace / at process exit).
+ *     (released by cuth_release_workspace / at process exit) and a mutex-protected table, keyed by matrix
+ *     address, of the objects written by cuth_import_csr / cuth_import_coo (whether CUTH_MIXED is available on
+ *     them; an entry is dropped when cuth_build_dia or another import writes the same buffer).
  *   - Device buffers must be 16-byte aligned (torch gives 512).
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call is
  *     asynchronous on that stream and never synchronises with the host.
