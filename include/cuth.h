@@ -249,9 +249,10 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
 int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* r_D,
                     double* z_D, void* work_D, size_t work_bytes, void* stream);
 
-/* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching
- * when one x-y plane of the six streamed arrays no longer fits L2, flat 1-D streaming otherwise),
- * 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation order. */
+/* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching when one x-y
+ * plane of the six streamed arrays no longer fits L2 -- nx*ny >= 2^18 -- or from 2^17 columns on grids of more than
+ * 2^21 rows; flat 1-D streaming otherwise), 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation
+ * order. */
 int cuth_set_traversal(int mode);
 
 /* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic = two
@@ -268,11 +269,11 @@ int cuth_set_cheb_fusion(int mode);
  * 2 = two columns whenever nx is even.  Results agree up to fp64 summation order. */
 int cuth_set_k1_variant(int mode);
 
-/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on flat-traversal grids of up to 2^21 rows
- * (Jacobi / no preconditioner) the whole solve is ONE persistent cooperative kernel whose iterations are separated
- * by grid-wide barriers (measured faster than the graph on every such grid); everything else runs as
- * the CUDA graph with conditional nodes.  1 = always the graph, 2 = the persistent kernel wherever it applies (any
- * flat-traversal grid).  Same arithmetic and policy code either way. */
+/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on grids of up to 2^21 rows (Jacobi / no
+ * preconditioner, traversal not forced to z-marching) the whole solve is ONE persistent cooperative kernel whose
+ * iterations are separated by grid-wide barriers (measured faster than the graph on every such grid, whatever the
+ * plane shape); everything else runs as the CUDA graph with conditional nodes.  1 = always the graph,
+ * 2 = the persistent kernel wherever the flat traversal applies.  Same arithmetic and policy code either way. */
 int cuth_set_loop_mode(int mode);
 
 /* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is

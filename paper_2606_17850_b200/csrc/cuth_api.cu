@@ -63,12 +63,16 @@ static std::atomic<int> g_loop_mode{0};   // 0 auto, 1 CUDA graph, 2 persistent 
 static std::atomic<int> g_traversal{0};   // 0 auto, 1 flat, 2 z-march (cuth_set_traversal)
 
 // Traversal choice: the flat kernel relies on L2 to keep the +-nx*ny neighbours (two planes of six
-// arrays, 96 B per plane cell); beyond ~1/3 of the 126 MB L2 that fails and z-marching wins.
+// arrays, 96 B per plane cell); beyond ~1/3 of the 126 MB L2 that fails and z-marching wins.  On grids whose
+// vectors do not fit L2 anyway (> 2^21 rows) the fused two-kernel iteration of the z-marching path (8m + 80 B/row
+// against 8m + 104) already pays from 2^17 columns on: measured per Jacobi iteration, flat / z-marching,
+// 384x384x128 442 / 355 us, 512x256x128 393 / 329, 448x448x64 312 / 279, but 256x256x256 (2^16 columns: too few
+// CTAs) 383 / 413; the Chebyshev path is indifferent there (+-3 %).
 static bool use_zmarch(const DiaLayout& L) {
   const int mode = g_traversal.load();
   if (mode == 1) return false;
   if (mode == 2) return true;
-  return L.nxny >= (1 << 18);
+  return L.nxny >= (1 << 18) || (L.nxny >= (1 << 17) && L.n > (1 << 21));
 }
 
 static std::atomic<int> g_k1_variant{0};   // 0 auto (two columns per thread when nx is even), 1 one column, 2 two columns
@@ -539,13 +543,16 @@ static int persistent_blocks(int64_t n) {
 }
 
 static bool use_persistent(const DiaLayout& L, bool cheb) {
-  const int mode = g_loop_mode.load();
-  if (cheb || use_zmarch(L) || mode == 1) return false;
+  const int mode = g_loop_mode.load(), trav = g_traversal.load();
+  if (cheb || mode == 1 || trav == 2) return false;
   if (persistent_blocks(L.n) <= 0) return false;
+  if (mode == 2) return !use_zmarch(L);        // forced: wherever the flat traversal applies
   // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
-  // 7.1 / 18.7 us at cfg 1 (8 k rows), 23 / 30.4 us at cfg 6 (655 k), 29.8 / 34.7 us at cfg 2 (1 M).  Auto: the
-  // persistent kernel for every flat-traversal grid up to 2 M rows; beyond, the wider grids of separate kernels.
-  return mode == 2 || L.n <= (1 << 21);
+  // 7.0 / 18.7 us at cfg 1 (8 k rows), 19.3 / 30.4 us at cfg 6 (655 k), 23.2 / 34.7 us at cfg 2 (1 M); and on wide
+  // planes, against the z-marching graph: 512x512x4 23.2 / 36.1, 512x512x8 47.7 / 60.3, 1024x1024x2 47.0 / 66.1,
+  // 512x512x16 (4 M rows) 99.2 / 99.5.  Auto: the persistent kernel (its row access is flat whatever the plane shape;
+  // up to 2 M rows everything it touches stays in L2) for every grid of up to 2^21 rows; beyond, the graph.
+  return L.n <= (1 << 21);
 }
 
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
