@@ -294,6 +294,8 @@ def main():
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
                          "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
+    ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1, 2],
+                    help="cuth_set_loop_mode: 0 automatic, 1 CUDA graph, 2 persistent kernel wherever the flat traversal applies")
     ap.add_argument("--batch", type=int, default=0,
                     help="NRHS > 0: time cuth_pcg_solve_batch on NRHS power maps of --config (FP64, Jacobi) against "
                          "NRHS single solves")
@@ -317,6 +319,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cu.cuth_set_traversal(args.traversal)
+    cu.cuth_set_loop_mode(args.loop_mode)
     cu.cuth_set_cheb_fusion(args.cheb_fusion)
     cu.cuth_set_pair_occupancy(args.pair_occupancy)
     cu.cuth_set_pair_rows(args.pair_rows)

@@ -269,7 +269,7 @@ int cuth_set_cheb_fusion(int mode);
  * 2 = two columns whenever nx is even.  Results agree up to fp64 summation order. */
 int cuth_set_k1_variant(int mode);
 
-/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on grids of up to 2^21 rows (Jacobi / no
+/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on grids of up to 2^22 rows (Jacobi / no
  * preconditioner, traversal not forced to z-marching) the whole solve is ONE persistent cooperative kernel whose
  * iterations are separated by grid-wide barriers (measured faster than the graph on every such grid, whatever the
  * plane shape); everything else runs as the CUDA graph with conditional nodes.  1 = always the graph,

@@ -538,7 +538,7 @@ static int persistent_blocks(int64_t n) {
     cached = coop ? sms * occ : 0;
     if (cached > kPersistMaxBlocks) cached = kPersistMaxBlocks;
   }
-  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : cached);
+  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : cached);   // > 512 k rows: all co-resident CTAs
   return want < cached ? want : cached;
 }
 
@@ -550,9 +550,10 @@ static bool use_persistent(const DiaLayout& L, bool cheb) {
   // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
   // 7.0 / 18.7 us at cfg 1 (8 k rows), 19.3 / 30.4 us at cfg 6 (655 k), 23.2 / 34.7 us at cfg 2 (1 M); and on wide
   // planes, against the z-marching graph: 512x512x4 23.2 / 36.1, 512x512x8 47.7 / 60.3, 1024x1024x2 47.0 / 66.1,
-  // 512x512x16 (4 M rows) 99.2 / 99.5.  Auto: the persistent kernel (its row access is flat whatever the plane shape;
-  // up to 2 M rows everything it touches stays in L2) for every grid of up to 2^21 rows; beyond, the graph.
-  return L.n <= (1 << 21);
+  // 512x512x16 (4 M rows, cfg 5) 101.0 / 99.5 in FP64 but 103.9 / 112.6 in MIXED with T = 5 (the true-residual branch
+  // is three more kernels and an IF node in the graph, one more phase in the kernel).  Auto: the persistent kernel
+  // (its row access is flat whatever the plane shape) for every grid of up to 2^22 rows; beyond, the graph.
+  return L.n <= (1 << 22);
 }
 
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
