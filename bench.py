@@ -120,36 +120,79 @@ class ClockSampler:
         return out
 
 
-# Alg.-1 (Jacobi) iteration counts of the six workloads at their rtol, as the fp64 path of this repo measures
-# them on B200; what a window of oracle iterations is extrapolated to.
-NOMINAL_JACOBI_ITERS = {1: 288, 2: 1462, 3: 4500, 4: 9791, 5: 580, 6: 1500}
+# Iterations to convergence used when a measured seconds-per-iteration of the oracle is turned into a time to solution.
+# cfg 1, 2, 3, 6: the ORACLE's own count (tests/golden/oracle_iterations.txt, written by oracle/iteration_counts.py).
+# cfg 4, 5: a full oracle solve takes hours; the count below is the FP64 GPU solve's and
+# the result is labelled "extrapolated with the GPU's iteration count".
+GPU_FP64_ITERS = {4: 9791, 5: 115916}
 
 
-def cpu_oracle_sample(w, iters_for_extrapolation, budget_iters=None, out=None):
-    """Times the oracle (as it stands) on a bounded sample: a window of Alg.-1 iterations on the same
-    workload, extrapolated to the iteration count the solve needs."""
+def oracle_iterations(cfg):
+    path = os.path.join(ROOT, "tests", "golden", "oracle_iterations.txt")
+    if os.path.exists(path):
+        for line in open(path):
+            if line.strip() and not line.startswith("#") and int(line.split()[0]) == cfg:
+                return int(line.split()[3]), "the oracle's own iteration count (tests/golden/oracle_iterations.txt)"
+    if cfg in GPU_FP64_ITERS:
+        return GPU_FP64_ITERS[cfg], "the FP64 GPU solve's iteration count (a full oracle solve takes hours)"
+    return None, ""
+
+
+WIN_SHORT, WIN_LONG = 20, 91          # oracle timing windows: seconds per iteration = (t_long - t_short) / 71
+
+
+def oracle_s_per_iteration(O, A, b, n):
+    """Seconds per Alg.-1 iteration of the oracle as it stands, from TWO windows of 20 and 91 iterations: the
+    difference cancels what each oracle_pcg_window call does besides iterating (it allocates and zero-fills five
+    vectors and forms r0), so the same number comes out of both bench arms whatever the window length."""
+    x0 = np.zeros(n)
+    t0 = time.time()
+    O.pcg_window(A, b, x0, WIN_SHORT)
+    t1 = time.time()
+    O.pcg_window(A, b, x0, WIN_LONG)
+    t2 = time.time()
+    return ((t2 - t1) - (t1 - t0)) / (WIN_LONG - WIN_SHORT), t2 - t0
+
+
+def cpu_oracle_baseline(w, cfg, x_gpu=None, full=None, out=None):
+    """The oracle as it stands on the host cores.  cfg 1, 2, 3, 6 (`full`): ONE solve to convergence, measured --
+    time to solution, iterations, and max |x_gpu - x_oracle| at full size.  cfg 4, 5: seconds per iteration from the
+    two windows, times the iteration count (extrapolated, labelled)."""
     from oracle import oracle as O
     t0 = time.time()
     A = O.assemble_workload(w)
     t_asm = time.time() - t0
     b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
-    # size the window for ~10-20 s: ~176 B/row/iteration at a few GB/s per core
-    if budget_iters is None:
-        budget_iters = int(max(5, min(400, 1.2e9 / w.n)))
-    t0 = time.time()
-    O.pcg_window(A, b, np.zeros(w.n), budget_iters)
-    dt = time.time() - t0
-    s_per_it = dt / (budget_iters + 1)
     if out is not None:
         out["A"], out["b"] = A, b
-    return {"value": s_per_it * iters_for_extrapolation, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "sample": f"{budget_iters} Alg.-1 iterations of the CSR fp64 oracle on {w.name} timed "
-                      f"({dt:.2f} s, {s_per_it * 1e3:.2f} ms/iteration), extrapolated to "
-                      f"{iters_for_extrapolation} iterations; CSR assembly {t_asm:.1f} s not included",
-            "s_per_iteration": s_per_it, "assembly_s": t_asm}
+    if full is None:
+        full = cfg in (1, 2, 3, 6)
+    s_it, t_win = oracle_s_per_iteration(O, A, b, w.n)
+    base = {"unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "s_per_iteration": s_it, "assembly_s": t_asm}
+    if full:
+        t0 = time.time()
+        ref = O.pcg(A, b, rtol=w.rtol)
+        dt = time.time() - t0
+        base.update(value=dt, iterations=ref.iterations, rel_resid_true=ref.rel_resid_true,
+                    sample=f"ONE full solve of {w.name} by the CSR fp64 oracle to a verified true residual <= {w.rtol:g}: "
+                           f"{ref.iterations} iterations in {dt:.1f} s (measured, not extrapolated); windows of {WIN_SHORT} / "
+                           f"{WIN_LONG} iterations give {s_it * 1e3:.2f} ms/iteration; CSR assembly {t_asm:.1f} s not included")
+        if x_gpu is not None:
+            base["max_abs_diff_gpu_vs_oracle_K"] = float(np.abs(x_gpu - ref.x).max())
+            base["max_rel_diff_gpu_vs_oracle"] = float(np.abs(x_gpu - ref.x).max() / np.abs(ref.x).max())
+    else:
+        its, src = oracle_iterations(cfg)
+        base.update(value=s_it * its, iterations=its,
+                    sample=f"windows of {WIN_SHORT} and {WIN_LONG} Alg.-1 iterations of the CSR fp64 oracle on {w.name} ({t_win:.1f} s): "
+                           f"{s_it * 1e3:.2f} ms/iteration, EXTRAPOLATED to {its} iterations = {src}; CSR assembly "
+                           f"{t_asm:.1f} s not included")
+    return base
 
 
 def run_reference(args):
+    """--impl reference: the oracle on the host cores.  Each step = the two timing windows (20 + 91 iterations) of the
+    same workload; value = seconds per iteration x iterations to convergence (the oracle's own count where a golden
+    one exists).  The GPU arm's cpu_baseline runs the full solve once and reports the measured time beside it."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -157,22 +200,24 @@ def run_reference(args):
     from oracle import oracle as O
     A = O.assemble_workload(w)
     b = w.power if not w.transient else O.transient_rhs(w, w.power, np.zeros(w.n))
-    iters = int(max(3, min(200, 2.5e8 / w.n)))
-    nominal = NOMINAL_JACOBI_ITERS[args.config]
+    its, src = oracle_iterations(args.config)
     for _ in range(args.warmup):
-        O.pcg_window(A, b, np.zeros(w.n), 1)
-    t0 = time.time()
+        O.pcg_window(A, b, np.zeros(w.n), 2)
+    s_its, t0 = [], time.time()
     for _ in range(args.steps):
-        O.pcg_window(A, b, np.zeros(w.n), iters)
+        s_it, _ = oracle_s_per_iteration(O, A, b, w.n)
+        s_its.append(s_it)
     dt = (time.time() - t0) / args.steps
-    s_it = dt / (iters + 1)
-    val = s_it * nominal
-    sample = (f"each step = {iters} Alg.-1 iterations of the CSR fp64 oracle on {w.name} "
-              f"({s_it * 1e3:.2f} ms/iteration), extrapolated to the nominal {nominal} iterations of this config")
+    s_it = float(np.median(s_its))
+    val = s_it * its
+    sample = (f"each step = windows of {WIN_SHORT} and {WIN_LONG} Alg.-1 iterations of the CSR fp64 oracle on {w.name}; "
+              f"median {s_it * 1e3:.2f} ms/iteration over {args.steps} steps, times {its} iterations = {src}")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": False,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "n_unknowns": w.n, "rtol": w.rtol},
+            "config": {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz], "rtol": w.rtol,
+                       "preconditioner": "jacobi", "precision": "fp64", "parallelism": "host cores"},
+            "iterations": its, "s_per_iteration": s_it,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
@@ -275,6 +320,11 @@ def main():
     ap.add_argument("--precision", default=None, choices=["fp64", "mixed"])
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-window", action="store_true",
+                    help="cpu_baseline from two timing windows instead of one full oracle solve (cfg 1, 2, 3, 6)")
+    ap.add_argument("--no-cfg4", action="store_true",
+                    help="default run (config 3) only: skip the appended block that solves BASELINE configs[3] "
+                         "(4096x4096x8) once per precision")
     ap.add_argument("--kernel-reps", type=int, default=20)
     ap.add_argument("--preconditioner", default="jacobi", choices=["jacobi", "chebyshev"],
                     help="jacobi = the north_star hot path; chebyshev = the paper's own preconditioner (Alg. 3)")
@@ -284,18 +334,21 @@ def main():
                     help="MIXED Chebyshev: matrix copy the preconditioner reads (A2 fp32 / A3 fp16, Alg. 4)")
     ap.add_argument("--transient-steps", type=int, default=0, help="config 5: time steps per bench step (default 200)")
     ap.add_argument("--cheb-fusion", type=int, default=0, choices=[0, 1, 2, 3],
-                    help="cuth_set_cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel, 3 = 2 without TMA")
+                    help="cuth_tuning_t.cheb_fusion: 0 auto, 1 one Chebyshev pass per kernel, 2 two passes per kernel, 3 = 2 without TMA")
     ap.add_argument("--pair-occupancy", type=int, default=0, choices=[0, 2, 3, 4],
-                    help="cuth_set_pair_occupancy: resident CTAs/SM of the TMA two-pass Chebyshev kernel (0 auto)")
+                    help="cuth_tuning_t.pair_occupancy: resident CTAs/SM of the TMA two-pass Chebyshev kernel (0 auto)")
     ap.add_argument("--pair-rows", type=int, default=0, choices=[0, 8, 16],
-                    help="cuth_set_pair_rows: region height of the TMA two-pass Chebyshev kernel (0 auto)")
+                    help="cuth_tuning_t.pair_rows: region height of the TMA two-pass Chebyshev kernel (0 auto)")
     ap.add_argument("--traversal", type=int, default=0, choices=[0, 1, 2],
-                    help="cuth_set_traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
+                    help="cuth_tuning_t.traversal: 0 auto, 1 flat (3 kernels/iteration), 2 z-marching fused (2 kernels)")
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
                          "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
     ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1, 2],
-                    help="cuth_set_loop_mode: 0 automatic, 1 CUDA graph, 2 persistent kernel wherever the flat traversal applies")
+                    help="cuth_tuning_t.loop_mode: 0 automatic, 1 CUDA graph, 2 persistent kernel wherever the flat traversal applies")
+    ap.add_argument("--k1-variant", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="cuth_tuning_t.k1_variant: 0 auto, 1 one column per thread, 2 two columns (TMA-staged K1 when "
+                         "nx %% 4 == 0), 3 two columns with ordinary loads")
     ap.add_argument("--batch", type=int, default=0,
                     help="NRHS > 0: time cuth_pcg_solve_batch on NRHS power maps of --config (FP64, Jacobi) against "
                          "NRHS single solves")
@@ -318,11 +371,10 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    cu.cuth_set_traversal(args.traversal)
-    cu.cuth_set_loop_mode(args.loop_mode)
-    cu.cuth_set_cheb_fusion(args.cheb_fusion)
-    cu.cuth_set_pair_occupancy(args.pair_occupancy)
-    cu.cuth_set_pair_rows(args.pair_rows)
+    # kernel variants travel in every call's cuth_tuning_t (the library has no process-wide settings)
+    cu.set_default_tuning(traversal=args.traversal, loop_mode=args.loop_mode, cheb_fusion=args.cheb_fusion,
+                          k1_variant=args.k1_variant,
+                          pair_occupancy=args.pair_occupancy, pair_rows=args.pair_rows)
     w = W.make_workload(args.config)
     mixed = w.mixed if args.precision is None else (args.precision == "mixed")
     prec = cu.MIXED if mixed else cu.FP64
@@ -420,55 +472,72 @@ def main():
 
     # ---- dominant kernels timed one by one with CUDA events (same launch configuration as in the graph)
     peak, peak_src = peaks()
-    kern = {}
-    cu.cuth_profile_kernel(S.work, g, -1)
-    lpi = cu.cuth_launches_per_iteration(g)
-    persistent = (lpi == 0) and not (args.preconditioner == "chebyshev")   # whole solve = one cooperative kernel
+    lpi = cu.cuth_launches_per_iteration(g, S.opts)
+    persistent = (lpi == 0) and not cheb                  # whole solve = one cooperative kernel
     fused = lpi == 2
+    kern = {}
+
+    def time_kernel(kid):
+        for _ in range(3):
+            cu.cuth_profile_kernel(S.work, g, S.opts, kid)
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.kernel_reps):
+            cu.cuth_profile_kernel(S.work, g, S.opts, kid)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.kernel_reps
+
+    # The profile hook replays the loop-body kernels on the context the finished solve left in the workspace.  A MIXED
+    # solve ends in the late stage (fp64 operator): -1 arms that; -2 re-arms the EARLY stage so that the fp32-stored
+    # instantiation of K1 / the SpMV -- the one that ran most of the launches -- is timed as well.
+    cu.cuth_profile_kernel(S.work, g, S.opts, -1)
     names = ({4: "k_fused_pspmv", 5: "k_update_nox", 3: "k_true_resid"} if fused else
              {0: "k_pupdate", 1: "k_spmv_dot", 2: "k_update", 3: "k_true_resid"})
     body_ids = (4, 5) if fused else (0, 1, 2)
+    stage_tag = "fp64"
     if cheb:
         h16 = mixed and args.cheb_storage == "fp16"
         cid = 8 if h16 else (7 if mixed else 6)
         names[cid] = "k_cheb_mid"
         cheb_launches, cheb_npairs = cu.cuth_cheb_launches(g, S.opts)
-        pid = 10 if h16 else 9                            # two passes per launch (cuth_set_cheb_fusion)
+        pid = 10 if h16 else 9                            # two passes per launch (cuth_tuning_t.cheb_fusion)
         # replay of one apply for ncu's launch list: the two-pass launches, and a single pass standing in for
         # each of FIRST / leftover MID / LAST (same stencil, same traffic to within 8 B/row)
         body_ids = tuple([pid] * cheb_npairs + [cid] * (cheb_launches - cheb_npairs)) + body_ids
         if mixed and w.nx % 2 == 0:
             names[pid] = "k_cheb_pair"
+    a_kid = 4 if fused else 1                             # the kernel that applies A in the loop body
+    a_name = names[a_kid]
     for kid, nm in names.items():
-        for _ in range(3):
-            cu.cuth_profile_kernel(S.work, g, kid)
-        e0 = torch.cuda.Event(enable_timing=True)
-        e1 = torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(args.kernel_reps):
-            cu.cuth_profile_kernel(S.work, g, kid)
-        e1.record(stream)
-        torch.cuda.synchronize()
-        kern[nm] = e0.elapsed_time(e1) / args.kernel_reps
+        kern[nm + ("[fp64 operator]" if kid == a_kid else "")] = time_kernel(kid)
     for _ in range(args.profile_iters):
         for kid in body_ids:
-            cu.cuth_profile_kernel(S.work, g, kid)
+            cu.cuth_profile_kernel(S.work, g, S.opts, kid)
+    if mixed and not cheb:
+        cu.cuth_profile_kernel(S.work, g, S.opts, -2)
+        kern[a_name + "[fp32-stored operator]"] = time_kernel(a_kid)
+        for _ in range(args.profile_iters):
+            for kid in body_ids:
+                cu.cuth_profile_kernel(S.work, g, S.opts, kid)
     torch.cuda.synchronize()
     # standalone SpMV (cuth_spmv), both precisions
     y = torch.empty_like(x)
     spmv = {}
     for nm, pr in (("fp64", cu.FP64), ("mixed", cu.MIXED)):
         for _ in range(3):
-            cu.cuth_spmv(A.buf, g, pr, b[0], y)
+            cu.cuth_spmv_tuned(A.buf, g, pr, None, b[0], y)
         e0 = torch.cuda.Event(enable_timing=True)
         e1 = torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(args.kernel_reps):
-            cu.cuth_spmv(A.buf, g, pr, b[0], y)
+            cu.cuth_spmv_tuned(A.buf, g, pr, None, b[0], y)
         e1.record(stream)
         torch.cuda.synchronize()
         tms = e0.elapsed_time(e1) / args.kernel_reps
-        spmv[nm] = {"ms": tms, "gbs": bytes_per_row(w, "spmv_" + nm) * w.n / tms / 1e6}
+        gbs = bytes_per_row(w, "spmv_" + nm) * w.n / tms / 1e6
+        spmv[nm] = {"ms": tms, "gbs": gbs, "frac": gbs / peak, "frac_of_8TBs_nominal": gbs / 8000.0}
 
     if rank != 0:
         if world > 1:
@@ -497,21 +566,23 @@ def main():
         outer = lambda M_: M_ + 48 + 24          # no 1/D0 anywhere: z = q(A) r is a stored vector
         iter_bytes = (early * (outer(4 * (m - 1)) + apply_bytes) + late * (outer(8 * m) + apply_bytes)) * w.n
     iter_gbs = iter_bytes / (ms_per_step * 1e-3) / 1e9
-    stage_fp64 = (not mixed) or res.promotions > 0     # operator the armed profile kernels ran with
-    m = m_ratio(w)
+    # The roofline line describes the instantiation that ran the MAJORITY of the launches of the timed solve.
+    early_major = mixed and not cheb and early > late
+    stage_tag = "fp32-stored" if early_major else "fp64"
     if fused:      # K1: matrix + r, p, x read + p', mu, x written (+ 1/D0 read with the fp32-stored operator)
-        dom_name, dom_ms = "k_fused_pspmv", kern["k_fused_pspmv"]
-        dom_bytes = ((8 * m + 48) if stage_fp64 else (4 * (m - 1) + 56)) * w.n
+        dom_name = "k_fused_pspmv"
+        dom_bytes = ((4 * (m - 1) + 56) if early_major else (8 * m + 48)) * w.n
     else:
-        dom_name, dom_ms = "k_spmv_dot", kern["k_spmv_dot"]
-        dom_bytes = bytes_per_row(w, "spmv_fp64" if stage_fp64 else "spmv_mixed") * w.n
+        dom_name = "k_spmv_dot"
+        dom_bytes = bytes_per_row(w, "spmv_mixed" if early_major else "spmv_fp64") * w.n
+    dom_ms = kern["%s[%s operator]" % (dom_name, stage_tag)]
     if cheb:
         dom_name, dom_ms = "k_cheb_mid", kern["k_cheb_mid"]
         dom_bytes = (((2 if h16 else 4) * (m - 1) + 16) if mixed else (8 * m + 32)) * w.n
         if cheb_npairs > 0:
             dom_name, dom_ms = "k_cheb_pair", kern["k_cheb_pair"]
             dom_bytes = ((2 if h16 else 4) * (m - 1) + 20) * w.n
-        stage_fp64 = not mixed
+        stage_tag = "fp32-stored" if mixed else "fp64"
     per_it = (2 if fused else 3) + (cheb_launches if cheb else 0)
     per_eval = 3 if fused else 2
     launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
@@ -532,15 +603,19 @@ def main():
                                  "no flush; HBM fractions are not meaningful here") %
                                 ((8 * m_ratio(w) + 48) * w.n / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
-        "iterations": it, "promotions": total_promos, "true_resid_evals": total_evals, "time_steps": nt,
-        "switch_reason": res.switch_reason, "switch_iteration": res.switch_iteration,
+        "iterations": it, "iterations_early_stage": early, "promotions": total_promos, "true_resid_evals": total_evals,
+        "time_steps": nt,
+        "switch_reason": res.switch_reason, "switch_mask": res.switch_mask, "switch_iteration": res.switch_iteration,
+        "hard_restarts": res.hard_restarts, "soft_restarts": res.soft_restarts,
         "rel_resid_true": res.rel_resid_true, "status": res.status_name if worst_status == 0 else "not all steps converged",
         "us_per_iteration": ms_per_step * 1e3 / max(it, 1),
         "solves_per_s": world / (ms_per_step * 1e-3),
-        "roofline": {"bound": "hbm", "kernel": "%s (%s operator)" % (dom_name, "fp64" if stage_fp64 else "fp32-stored"),
+        "roofline": {"bound": "hbm", "kernel": "%s (%s operator; ran %d of the %d iterations)" %
+                                               (dom_name, stage_tag, early if early_major else late, it),
                      "achieved": dom_bytes / dom_ms / 1e6, "peak": peak, "unit": "GB/s",
-                     "frac": dom_bytes / dom_ms / 1e6 / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((w.name, dom_name, "fp64" if stage_fp64 else "mixed")), "peak_source": peak_src,
+                     "frac": dom_bytes / dom_ms / 1e6 / peak, "frac_of_8TBs_nominal": dom_bytes / dom_ms / 1e6 / 8000.0,
+                     "traffic": NCU_TRAFFIC_BYTES.get((w.name, dom_name, "mixed" if stage_tag == "fp32-stored" else "fp64")),
+                     "peak_source": peak_src,
                      "ms_per_launch": dom_ms, "algorithmic_bytes_per_launch": dom_bytes},
         "roofline_iteration": {"bound": "hbm", "achieved": iter_gbs, "peak": peak, "unit": "GB/s",
                                "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
@@ -554,20 +629,122 @@ def main():
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    if fused and not cheb:      # the other K1 instantiation, for the record
+        for tag, nb in (("fp64", 8 * m + 48), ("fp32-stored", 4 * (m - 1) + 56)):
+            key = "k_fused_pspmv[%s operator]" % tag
+            if key in kern:
+                gbs = nb * w.n / kern[key] / 1e6
+                line.setdefault("k1_instantiations", {})[tag] = {"ms": kern[key], "gbs": gbs, "frac": gbs / peak,
+                                                                "frac_of_8TBs_nominal": gbs / 8000.0, "bytes_per_row": nb}
+        gbs = 32 * w.n / kern["k_update_nox"] / 1e6
+        line["k2"] = {"ms": kern["k_update_nox"], "gbs": gbs, "frac": gbs / peak, "bytes_per_row": 32}
     if not args.no_cpu_baseline and world == 1:
         keep = {}
-        # the oracle timed is Alg. 1 with Jacobi; a Chebyshev-preconditioned run is compared with the Jacobi
-        # iteration count of the same workload, not with its own (31 SpMVs each) count
-        cpu_its = NOMINAL_JACOBI_ITERS[args.config] if cheb else it
-        line["cpu_baseline"] = cpu_oracle_sample(w, cpu_its, out=keep)
+        line["cpu_baseline"] = cpu_oracle_baseline(w, args.config, x_gpu=None if w.transient else x_final,
+                                                   full=False if args.cpu_window else None, out=keep)
         if not w.transient:
             # property check of the timed result against the ORACLE's matrix (not timed)
             from oracle import oracle as O
             Ao, bb = keep["A"], keep["b"]
             line["oracle_true_rel_resid_of_gpu_x"] = float(np.linalg.norm(bb - O.spmv(Ao, x_final)) / np.linalg.norm(bb))
+        del keep
+    if args.config == 3 and world == 1 and not args.no_cfg4 and not cheb:
+        # the 134 M-unknown scaling case of BASELINE.json, one timed solve per precision, in the same record
+        del S, A, b, b_stage, x, y, kap_d
+        torch.cuda.empty_cache()
+        line["cfg4"] = cfg4_block(cu, args, peak)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def cfg4_block(cu, args, peak):
+    """BASELINE.json configs[3] (4096x4096x8, 134 M unknowns): ONE timed solve in FP64 and one in MIXED (after a
+    5-iteration solve that instantiates the graph), the loop-body kernels and cuth_spmv timed as in the main record,
+    and the true residual of the GPU's x recomputed with the ORACLE's CSR matrix."""
+    import torch
+    w = W.make_workload(4)
+    g = cu.Grid(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, torch.from_numpy(np.ascontiguousarray(w.kappa_layer)).cuda(), w.h_top)
+    A = cu.DiaMatrix(g)
+    b = torch.from_numpy(w.power).cuda()
+    x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    m = m_ratio(w)
+    out = {"workload": w.name, "n_unknowns": w.n, "grid": [w.nx, w.ny, w.nz], "rtol": w.rtol}
+    xs = {}
+    for name, prec in (("fp64", cu.FP64), ("mixed", cu.MIXED)):
+        S = cu.Solver(A, cu.Opts(precision=prec, rtol=w.rtol, max_iters=5, true_resid_period=w.true_resid_period))
+        S.solve(b, x.zero_())                      # warm-up: graph instantiation, 5 iterations
+        S.opts.max_iters = 200000
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        x.zero_()
+        e0.record(stream)
+        S.solve(b, x)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        r = S.result()
+        early = (r.switch_iteration if r.promotions else r.iterations) if prec == cu.MIXED else 0
+        ib = (early * (4 * (m - 1) + 88) + (r.iterations - early) * (8 * m + 80)) * w.n
+        d = {"value": ms * 1e-3, "unit": UNIT, "iterations": r.iterations, "iterations_early_stage": early,
+             "status": r.status_name, "rel_resid_true": r.rel_resid_true, "true_resid_evals": r.true_resid_evals,
+             "switch_reason": r.switch_reason, "us_per_iteration": ms * 1e3 / max(r.iterations, 1),
+             "roofline_iteration": {"achieved": ib / ms / 1e6, "unit": "GB/s", "frac": ib / ms / 1e6 / peak,
+                                    "frac_of_8TBs_nominal": ib / ms / 1e6 / 8000.0}}
+
+        def tk(kid):
+            for _ in range(2):
+                cu.cuth_profile_kernel(S.work, g, S.opts, kid)
+            t0 = torch.cuda.Event(enable_timing=True)
+            t1 = torch.cuda.Event(enable_timing=True)
+            t0.record(stream)
+            for _ in range(10):
+                cu.cuth_profile_kernel(S.work, g, S.opts, kid)
+            t1.record(stream)
+            torch.cuda.synchronize()
+            return t0.elapsed_time(t1) / 10
+
+        x_keep = x.clone()
+        cu.cuth_profile_kernel(S.work, g, S.opts, -1)
+        k1, k2 = tk(4), tk(5)
+        d["k1_fp64"] = {"ms": k1, "gbs": (8 * m + 48) * w.n / k1 / 1e6, "frac": (8 * m + 48) * w.n / k1 / 1e6 / peak}
+        d["k2"] = {"ms": k2, "gbs": 32 * w.n / k2 / 1e6, "frac": 32 * w.n / k2 / 1e6 / peak}
+        if prec == cu.MIXED:
+            cu.cuth_profile_kernel(S.work, g, S.opts, -2)
+            k1e = tk(4)
+            d["k1_fp32_stored"] = {"ms": k1e, "gbs": (4 * (m - 1) + 56) * w.n / k1e / 1e6,
+                                   "frac": (4 * (m - 1) + 56) * w.n / k1e / 1e6 / peak}
+        xs[name] = x_keep.cpu().numpy()
+        del x_keep
+        S.close()
+        del S
+        out[name] = d
+    y = torch.empty_like(x)
+    for nm, pr, bpr in (("fp64", cu.FP64, 8 * m + 16), ("mixed", cu.MIXED, 4 * (m - 1) + 16)):
+        for _ in range(2):
+            cu.cuth_spmv_tuned(A.buf, g, pr, None, b, y)
+        t0 = torch.cuda.Event(enable_timing=True)
+        t1 = torch.cuda.Event(enable_timing=True)
+        t0.record(stream)
+        for _ in range(10):
+            cu.cuth_spmv_tuned(A.buf, g, pr, None, b, y)
+        t1.record(stream)
+        torch.cuda.synchronize()
+        tms = t0.elapsed_time(t1) / 10
+        out.setdefault("spmv", {})[nm] = {"ms": tms, "gbs": bpr * w.n / tms / 1e6, "frac": bpr * w.n / tms / 1e6 / peak,
+                                          "frac_of_8TBs_nominal": bpr * w.n / tms / 1e6 / 8000.0}
+    del A, b, x, y
+    torch.cuda.empty_cache()
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        Ao = O.assemble_workload(w)
+        bn = np.linalg.norm(w.power)
+        for name in ("fp64", "mixed"):
+            out[name]["oracle_true_rel_resid_of_gpu_x"] = float(np.linalg.norm(w.power - O.spmv(Ao, xs[name])) / bn)
+        out["max_abs_diff_mixed_vs_fp64_K"] = float(np.abs(xs["mixed"] - xs["fp64"]).max())
+    return out
 
 
 if __name__ == "__main__":

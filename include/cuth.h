@@ -3,14 +3,17 @@
  * Boundary.  Everything behind these calls is hand-written CUDA for
  * sm_100a; there is no CPU fallback.  Conventions shared by all calls:
  *   - "_D" pointers are DEVICE pointers owned by the caller (allocate them with torch or cudaMalloc),
- *     "_H" pointers are HOST pointers.  The library allocates no device memory of its own; its only
- *     hidden host-side state is a cache of instantiated CUDA graphs keyed by the workspace address
- *     (released by cuth_release_workspace / at process exit) and a mutex-protected table, keyed by matrix
- *     address, of the objects written by cuth_import_csr / cuth_import_coo (whether CUTH_MIXED is available on
- *     them; an entry is dropped when cuth_build_dia or another import writes the same buffer).
+ *     "_H" pointers are HOST pointers.  The library allocates no device memory of its own and has NO mutable
+ *     process-wide settings: every choice a call makes comes from its arguments (cuth_tuning_t below for the
+ *     kernel variants).  What it keeps on the host is derived data only: a mutex-protected cache of instantiated
+ *     CUDA graphs keyed by the workspace address (released by cuth_release_workspace / at process exit) and, per
+ *     device, the number of co-resident CTAs of its cooperative kernels.  What a matrix object is (built or
+ *     imported, transient or steady, CUTH_MIXED available or not) is recorded in the object itself, in device
+ *     memory, and checked on the device.
  *   - Device buffers must be 16-byte aligned (torch gives 512).
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call is
- *     asynchronous on that stream and never synchronises with the host.
+ *     asynchronous on that stream and never synchronises with the host, except the three setup calls that say so
+ *     (cuth_import_csr, cuth_import_coo, cuth_lanczos_bounds).
  *   - Return value: CUTH_OK or a negative cuth_status_t for errors detectable on the host (bad
  *     arguments, CUDA API failure).  NUMERICAL outcomes of a solve (converged / max-iters /
  *     breakdown) are written to result_D->status on the device, because the call is asynchronous.
@@ -38,14 +41,31 @@ typedef enum {
   CUTH_ERR_CUDA = -6,        /* a CUDA runtime call failed (see cuth_last_cuda_error) */
   CUTH_ERR_NOT_TRANSIENT = -7,/* cuth_transient_step on a matrix built without cvol/dt (or on an imported matrix) */
   CUTH_ERR_STRUCTURE = -8,    /* cuth_import_csr: the matrix is not a symmetric 7-point matrix of this grid (see the report) */
-  CUTH_ERR_FP64_ONLY = -9     /* MIXED requested on an imported matrix whose row sums are not constant per layer */
+  CUTH_ERR_FP64_ONLY = -9     /* reserved (round 1 returned it from the host; the condition is now detected on the
+                                 device: CUTH_SOLVE_FP64_ONLY) */
 } cuth_status_t;
 
-/* result_D->status values (device-side, numerical outcome of a solve) */
-enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN = 2, CUTH_SOLVE_RUNNING = 3 };
+/* result_D->status values (device-side outcome of a solve).  The last three mean "nothing was computed":
+ * FP64_ONLY      -- a fp32-stored precision was requested on an imported matrix whose row sums are not constant
+ *                   per layer (cuth_import_report_t.mixed_ok == 0);
+ * NOT_TRANSIENT  -- cuth_transient_step on a matrix object built without cvol / dt, or on an imported one;
+ * BAD_MATRIX     -- dia_D does not hold a matrix object of this grid (magic number / dimensions differ). */
+enum { CUTH_SOLVE_CONVERGED = 0, CUTH_SOLVE_MAX_ITERS = 1, CUTH_SOLVE_BREAKDOWN = 2, CUTH_SOLVE_RUNNING = 3,
+       CUTH_SOLVE_FP64_ONLY = 4, CUTH_SOLVE_NOT_TRANSIENT = 5, CUTH_SOLVE_BAD_MATRIX = 6,
+       CUTH_SOLVE_CONVERGED_UNVERIFIED = 7 /* CUTH_FIXED32 only: the fp32 recursive residual passed the test */ };
 
-enum { CUTH_FP64 = 0, CUTH_MIXED = 1,              /* cuth_opts_t.precision / cuth_spmv precision */
-       CUTH_ABLATION_STD32 = 2 };                  /* cuth_spmv only: fp32-rounded A2 in STANDARD form (ablation) */
+/* cuth_opts_t.precision / cuth_spmv precision.
+ * CUTH_FP64        fixed FP64.
+ * CUTH_MIXED       the adaptive scheme of PAPER.md §IV-D with the early-stage operator in DIFFERENCE form
+ *                  (DESIGN.md R-F3): the product path.
+ * CUTH_MIXED_STD32 ABLATION: the same scheme with the paper's A2 taken literally -- every diagonal, D0 included,
+ *                  rounded to fp32 and applied in standard form.  On these grids the true
+ *                  residual then floors near 1e-2 ||b|| and eq. (14c) / (14b) do the switching.
+ * CUTH_FIXED32     ABLATION: the paper's fixed-FP32 solver (Table VI): fp32 matrix A2 in standard
+ *                  form, fp32 x, r, p, mu and fp32 arithmetic including the dots; stops on its own recursive
+ *                  residual, never looks at b - A x (status CUTH_SOLVE_CONVERGED_UNVERIFIED); rel_resid_true
+ *                  reports the fp64 residual it really reached.  Solver only; Jacobi / no preconditioner. */
+enum { CUTH_FP64 = 0, CUTH_MIXED = 1, CUTH_MIXED_STD32 = 2, CUTH_ABLATION_STD32 = 2, CUTH_FIXED32 = 3 };
 enum { CUTH_PRECOND_NONE = 0, CUTH_PRECOND_JACOBI = 1, CUTH_PRECOND_CHEBYSHEV = 2 };
 enum { CUTH_CHEB_DEFAULT = 0, CUTH_CHEB_A3_FP16 = 1 };   /* cuth_opts_t.cheb_storage */
 
@@ -63,8 +83,27 @@ typedef struct {
   double dt;                  /* s; <= 0 => steady */
 } cuth_grid_t;
 
+/* Which variant of a kernel a call uses.  Zero-initialised = automatic (the measured-fastest rule for the grid,
+ * DESIGN.md §5); the non-zero values exist so that tests and measurements can run every variant.  Results agree
+ * up to fp64 summation order whatever is chosen.  Per call: there is no process-wide setting. */
 typedef struct {
-  int32_t precision;          /* CUTH_FP64 or CUTH_MIXED (§IV-D) */
+  int32_t traversal;          /* how the kernels that apply A walk the grid: 0 automatic (z-marching when one x-y plane
+                                 of the six streamed arrays no longer fits L2 -- nx*ny >= 2^18 -- or from 2^17 columns
+                                 on grids of more than 2^21 rows; flat 1-D streaming otherwise), 1 flat, 2 z-marching */
+  int32_t loop_mode;          /* where the PCG loop lives: 0 automatic (one persistent cooperative kernel up to 2^22
+                                 rows, the CUDA graph with conditional nodes beyond), 1 graph, 2 persistent kernel
+                                 wherever the flat traversal applies */
+  int32_t k1_variant;         /* z-marching kernels: 0 automatic, 1 one column per thread, 2 two x-adjacent columns per
+                                 thread (nx even), 3 = 2 without the TMA-staged K1 */
+  int32_t cheb_fusion;        /* Chebyshev passes per kernel (fp32 modes, nx even): 0 automatic = 2 = two passes, TMA
+                                 operands when nx % 4 == 0 (A3: % 8); 1 one pass per kernel; 3 two passes, never TMA */
+  int32_t pair_rows;          /* rows of a region of the TMA two-pass Chebyshev kernel: 0 automatic, 8, 16 */
+  int32_t pair_occupancy;     /* resident CTAs/SM of that kernel: 0 automatic (4), 2..4 */
+  int32_t reserved[2];        /* must be 0 */
+} cuth_tuning_t;
+
+typedef struct {
+  int32_t precision;          /* CUTH_FP64, CUTH_MIXED (§IV-D) or an ablation value above */
   double rtol;                /* stop when ||b - A x||_2 <= rtol * ||b||_2 (true fp64 residual) */
   int32_t max_iters;          /* cap on PCG iterations (Alg. 1 loop), > 0 */
   int32_t true_resid_period;  /* MIXED early stage: evaluate b - A1 x every this many iterations
@@ -77,6 +116,7 @@ typedef struct {
   int32_t cheb_storage;       /* matrix the preconditioner multiplies by in MIXED mode: CUTH_CHEB_DEFAULT = the fp32
                                  copy A2, CUTH_CHEB_A3_FP16 = the half-precision copy A3 promoted to fp32 on load
                                  (Alg. 4 "arithmetic decoupling").  Ignored in FP64 mode. */
+  cuth_tuning_t tuning;       /* kernel variants; all zero = automatic */
 } cuth_opts_t;
 
 typedef struct {
@@ -86,8 +126,14 @@ typedef struct {
   int32_t true_resid_evals;   /* number of explicit b - A1 x evaluations */
   double rel_resid_true;      /* last evaluated ||b - A1 x||_2 / ||b||_2 (fp64) */
   double rel_resid_rec;       /* last recursive ||r||_2 / ||b||_2 */
-  int32_t switch_reason;      /* MIXED: 0 none, 1 = (14a), 2 = (14b), 3 = (14c), 4 = recursive converged */
+  int32_t switch_reason;      /* MIXED: 0 none, else the first criterion, in the printed order, that held at the
+                                 switch: 1 = (14a), 2 = (14b), 3 = (14c) */
   int32_t switch_iteration;   /* iteration at which the switch happened */
+  int32_t switch_mask;        /* every criterion that held at the switch: bit 0 = (14a), bit 1 = (14b), bit 2 = (14c) */
+  int32_t hard_restarts;      /* hot restarts with p := z (Alg. 1 line 3): large drift at the switch, or a failed
+                                 verification of the stopping test in the late stage */
+  int32_t soft_restarts;      /* hot restarts that kept p through Alg. 1 line 12 (small drift, DESIGN.md R-G11) */
+  int32_t reserved;
 } cuth_result_t;
 
 /* Bytes of the caller-allocated device buffer that holds the matrix object (header, fp64 packed
@@ -208,21 +254,13 @@ const char* cuth_last_cuda_error(void);
 /* Library version, e.g. 10000 = 1.0.0 */
 int cuth_version(void);
 
-/* Kernel launches per PCG iteration of the graph body for this grid (2 on the fused path used for
- * large planes, 3 on the flat path, 0 when the whole solve is one persistent kernel); bench.py reports gpu_launches = prologue + this * iterations +
- * true-residual branches + epilogue. */
-int cuth_launches_per_iteration(const cuth_grid_t* grid);
-
-/* Tuning knob, process-wide: resident CTAs per SM of the TMA two-pass Chebyshev kernel.  0 = automatic (4: measured
- * fastest on every grid), 2..4 = forced (for studying occupancy against the partly filled last wave of regions). */
-int cuth_set_pair_occupancy(int ctas_per_sm);
-
-/* Tuning knob, process-wide: rows of a region of the TMA two-pass Chebyshev kernel (one warp per row): 8 (256
- * threads, 4 CTAs/SM) or 16 (512 threads, 2 CTAs/SM, a sixth less rim recomputation); 0 = automatic. */
-int cuth_set_pair_rows(int rows);
+/* Kernel launches per PCG iteration of the graph body for this grid and these options (2 on the fused path used
+ * for large planes, 3 on the flat path, 0 when the whole solve is one persistent kernel); bench.py reports
+ * gpu_launches = prologue + this * iterations + true-residual branches + epilogue.  Pure host. */
+int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts);
 
 /* Kernel launches of ONE Chebyshev apply (Alg. 3) for this grid and these options: the first
- * pass, the middle passes (single, or two per launch -- see cuth_set_cheb_fusion) and the last pass; 0 when the
+ * pass, the middle passes (single, or two per launch -- see cuth_tuning_t.cheb_fusion) and the last pass; 0 when the
  * preconditioner is not Chebyshev, negative on bad arguments.  *pairs_out (may be NULL) = how many of them are
  * two-pass launches.  Pure host. */
 int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pairs_out);
@@ -236,6 +274,9 @@ int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pa
  * Uses the solver workspace (>= cuth_workspace_bytes).  This call SYNCHRONISES `stream` (setup, not hot path). */
 int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
                         size_t work_bytes, double bounds_H[5], void* stream);
+/* ... with an explicit kernel variant for its SpMV (tuning may be NULL = automatic). */
+int cuth_lanczos_bounds_tuned(const void* dia_D, const cuth_grid_t* grid, const cuth_tuning_t* tuning, const double* v0_D,
+                              int steps, void* work_D, size_t work_bytes, double bounds_H[5], void* stream);
 
 /* The host half of cuth_lanczos_bounds on its own (pure host, no CUDA): smallest and largest eigenvalue of
  * the symmetric tridiagonal matrix with diagonal alpha_H[0..m) and off-diagonal beta_H[0..m-1), by Sturm
@@ -249,41 +290,31 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
 int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* r_D,
                     double* z_D, void* work_D, size_t work_bytes, void* stream);
 
-/* Tuning knob, process-wide: how the kernels that apply A walk the grid.  0 = automatic (z-marching when one x-y
- * plane of the six streamed arrays no longer fits L2 -- nx*ny >= 2^18 -- or from 2^17 columns on grids of more than
- * 2^21 rows; flat 1-D streaming otherwise), 1 = flat, 2 = z-marching.  Results are identical up to fp64 summation
- * order. */
-int cuth_set_traversal(int mode);
+/* cuth_spmv with an explicit choice of kernel variant (tuning may be NULL = automatic = cuth_spmv). */
+int cuth_spmv_tuned(const void* dia_D, const cuth_grid_t* grid, int precision, const cuth_tuning_t* tuning,
+                    const double* x_D, double* y_D, void* stream);
 
-/* Tuning knob, process-wide: fusion of the Chebyshev passes (fp32 modes, nx even).  0 = automatic = two
- * consecutive passes per kernel (measured faster on every grid), 1 = one pass per kernel, 2 = same as 0,
- * 3 = two passes per kernel but never the TMA version of the kernel.
- * The two-pass kernel takes its operands through TMA (k_cheb_pair_tma) when nx is a multiple of 4 (fp32 A2) /
- * 8 (fp16 A3), else through ordinary loads (k_cheb_pair_f32).  The polynomial is the same, and so is the
- * arithmetic of every row.  fp64 applies and odd nx always run one pass per kernel. */
-int cuth_set_cheb_fusion(int mode);
+/* Measurement hook (bench.py, ncu, __graft_entry__.smoke): launches ONE loop-body kernel of the solve whose context
+ * is still in this workspace, outside the graph and with the graph's launch configuration for `opts` (the options of
+ * that solve), so that it can be timed with CUDA events on `stream` and shows up by name in a profiler's launch list
+ * (kernel nodes of graphs with conditional nodes do not).  kernel_id: -1 = arm with the stage the solve ended in,
+ * -2 = arm and force the EARLY stage (fp32-stored operator; MIXED solves only) -- one of the two must be called once
+ * after the solve, before any other id; 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual
+ * (fused path: with the pending x-update and the restart folded in), 4 = fused p-update + SpMV (K1 of the fused
+ * path), 5 = r update + dots without x (K2 of the fused path), 6 / 7 / 8 = one middle step of the Chebyshev apply in
+ * fp64 / fp32 on A2 / fp32 on the fp16 copy A3 (only after a CUTH_PRECOND_CHEBYSHEV solve); 9 / 10 = one fused PAIR
+ * of Chebyshev passes on A2 / A3.  The vectors of the finished solve are overwritten; x_D is modified by ids 2-4. */
+int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t* opts, int kernel_id, void* stream);
 
-/* Tuning knob, process-wide: variant of the z-marching kernels (K1, SpMV, true residual, Chebyshev middle
- * step).  0 = automatic: two x-adjacent columns per thread with 16-byte vector traffic when nx is even and the
- * plane still yields >= 2048 CTAs (cfg 3, cfg 4), one column otherwise; 1 = always one column per thread;
- * 2 = two columns whenever nx is even.  Results agree up to fp64 summation order. */
-int cuth_set_k1_variant(int mode);
-
-/* Tuning knob, process-wide: where the PCG loop lives.  0 = automatic: on grids of up to 2^22 rows (Jacobi / no
- * preconditioner, traversal not forced to z-marching) the whole solve is ONE persistent cooperative kernel whose
- * iterations are separated by grid-wide barriers (measured faster than the graph on every such grid, whatever the
- * plane shape); everything else runs as the CUDA graph with conditional nodes.  1 = always the graph,
- * 2 = the persistent kernel wherever the flat traversal applies.  Same arithmetic and policy code either way. */
-int cuth_set_loop_mode(int mode);
-
-/* Measurement hook (bench.py, ncu): launches ONE loop-body kernel of the solve whose context is
- * still in this workspace, outside the graph and with the graph's launch configuration, so that it
- * can be timed with CUDA events on `stream`.  kernel_id: -1 = arm (must be called once after the
- * solve, before any other id), 0 = p-update, 1 = SpMV + p.mu, 2 = x/r update + dots, 3 = true residual,
- * 4 = fused p-update + SpMV (K1 of the fused path), 5 = r update + dots without x (K2 of the fused path),
- * 6 / 7 / 8 = one middle step of the Chebyshev apply in fp64 / fp32 on A2 / fp32 on the fp16 copy A3 (only
- * after a CUTH_PRECOND_CHEBYSHEV solve); 9 / 10 = one fused PAIR of Chebyshev passes on A2 / A3.  The vectors of the finished solve are overwritten; x_D is modified by id 2. */
-int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream);
+/* Test hook for the device-side stage-switch policy (csrc/cuth_policy.cuh): runs the decision
+ * function the solver kernels run after an evaluation of r_true = b - A1 x, ONCE, on caller-given scalars, in a
+ * one-thread kernel on `stream`, and writes what it decided to out_D (device, 8 x int32: [0] go, [1] stage after,
+ * [2] switch_reason, [3] switch_mask, [4] restart kind (0 none, 1 hard, 2 soft), [5] status, [6] promotions,
+ * [7] 0).  in_H (host, 8 doubles): ||r_low||^2, ||r_true||^2, ||r_true - r_low||^2, ||r_true||^2 at the previous
+ * evaluation, ||r_low||^2 at the previous evaluation, ||b||^2, rtol, soft_drift (<= 0: library default 0.1).
+ * flags: bit 0 = late stage, bit 1 = the recursive residual had passed the stopping test, bit 2 = iteration cap
+ * reached.  No solver state is touched. */
+int cuth_policy_probe(const double in_H[8], int flags, int32_t* out_D, void* stream);
 
 #ifdef __cplusplus
 }

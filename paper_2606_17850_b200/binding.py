@@ -11,10 +11,13 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("CUTH_LIB", os.path.join(HERE, "libcuth.so"))   # CUTH_LIB: developer override
 
-FP64, MIXED, ABLATION_STD32 = 0, 1, 2
+FP64, MIXED, MIXED_STD32, FIXED32 = 0, 1, 2, 3
+ABLATION_STD32 = MIXED_STD32
 PRECOND_NONE, PRECOND_JACOBI, PRECOND_CHEBYSHEV = 0, 1, 2
 CHEB_DEFAULT, CHEB_A3_FP16 = 0, 1
-STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running"}
+STATUS_NAMES = {0: "converged", 1: "max_iters", 2: "breakdown", 3: "running", 4: "fp64_only", 5: "not_transient",
+                6: "bad_matrix", 7: "converged_unverified"}
+SOLVE_FP64_ONLY, SOLVE_NOT_TRANSIENT, SOLVE_BAD_MATRIX, SOLVE_CONVERGED_UNVERIFIED = 4, 5, 6, 7
 _ERR = {-1: "CUTH_ERR_NULL", -2: "CUTH_ERR_DIMS", -3: "CUTH_ERR_VALUE", -4: "CUTH_ERR_SIZE",
         -5: "CUTH_ERR_ALIGN", -6: "CUTH_ERR_CUDA", -7: "CUTH_ERR_NOT_TRANSIENT", -8: "CUTH_ERR_STRUCTURE",
         -9: "CUTH_ERR_FP64_ONLY"}
@@ -36,18 +39,25 @@ class cuth_grid_t(C.Structure):
                 ("h_top", C.c_double), ("cvol_H", C.c_void_p), ("dt", C.c_double)]
 
 
+class cuth_tuning_t(C.Structure):
+    _fields_ = [("traversal", C.c_int32), ("loop_mode", C.c_int32), ("k1_variant", C.c_int32),
+                ("cheb_fusion", C.c_int32), ("pair_rows", C.c_int32), ("pair_occupancy", C.c_int32),
+                ("reserved", C.c_int32 * 2)]
+
+
 class cuth_opts_t(C.Structure):
     _fields_ = [("precision", C.c_int32), ("rtol", C.c_double), ("max_iters", C.c_int32),
                 ("true_resid_period", C.c_int32), ("preconditioner", C.c_int32),
                 ("cheb_degree", C.c_int32), ("cheb_lmin", C.c_double), ("cheb_lmax", C.c_double),
-                ("cheb_storage", C.c_int32)]
+                ("cheb_storage", C.c_int32), ("tuning", cuth_tuning_t)]
 
 
 class cuth_result_t(C.Structure):
     _fields_ = [("status", C.c_int32), ("iterations", C.c_int32), ("promotions", C.c_int32),
                 ("true_resid_evals", C.c_int32), ("rel_resid_true", C.c_double),
                 ("rel_resid_rec", C.c_double), ("switch_reason", C.c_int32),
-                ("switch_iteration", C.c_int32)]
+                ("switch_iteration", C.c_int32), ("switch_mask", C.c_int32), ("hard_restarts", C.c_int32),
+                ("soft_restarts", C.c_int32), ("reserved", C.c_int32)]
 
 
 class cuth_import_report_t(C.Structure):
@@ -56,9 +66,11 @@ class cuth_import_report_t(C.Structure):
                 ("mixed_ok", C.c_int32)]
 
 
-EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes", "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv",
-           "cuth_pcg_solve", "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error",
-           "cuth_version", "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_set_traversal", "cuth_lanczos_bounds", "cuth_cheb_apply", "cuth_set_loop_mode", "cuth_tridiag_extremes", "cuth_set_k1_variant", "cuth_set_cheb_fusion", "cuth_cheb_launches", "cuth_set_pair_occupancy", "cuth_set_pair_rows"]
+EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes",
+           "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv", "cuth_spmv_tuned", "cuth_pcg_solve",
+           "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error", "cuth_version",
+           "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_lanczos_bounds", "cuth_lanczos_bounds_tuned",
+           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe"]
 
 _lib = None
 
@@ -92,6 +104,8 @@ def load_library():
                                 C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.cuth_spmv.restype = C.c_int
     L.cuth_spmv.argtypes = [vp, gp, C.c_int, vp, vp, vp]
+    L.cuth_spmv_tuned.restype = C.c_int
+    L.cuth_spmv_tuned.argtypes = [vp, gp, C.c_int, C.POINTER(cuth_tuning_t), vp, vp, vp]
     L.cuth_pcg_solve.restype = C.c_int
     L.cuth_pcg_solve.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp, vp]
     L.cuth_batch_workspace_bytes.restype = C.c_size_t
@@ -105,17 +119,18 @@ def load_library():
     L.cuth_last_cuda_error.restype = C.c_char_p
     L.cuth_version.restype = C.c_int
     L.cuth_launches_per_iteration.restype = C.c_int
-    L.cuth_launches_per_iteration.argtypes = [gp]
+    L.cuth_launches_per_iteration.argtypes = [gp, op]
     L.cuth_lanczos_bounds.restype = C.c_int
     L.cuth_lanczos_bounds.argtypes = [vp, gp, vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_double), vp]
+    L.cuth_lanczos_bounds_tuned.restype = C.c_int
+    L.cuth_lanczos_bounds_tuned.argtypes = [vp, gp, C.POINTER(cuth_tuning_t), vp, C.c_int, vp, C.c_size_t,
+                                            C.POINTER(C.c_double), vp]
+    L.cuth_policy_probe.restype = C.c_int
+    L.cuth_policy_probe.argtypes = [C.POINTER(C.c_double), C.c_int, vp, vp]
     L.cuth_cheb_apply.restype = C.c_int
     L.cuth_cheb_apply.argtypes = [vp, gp, op, vp, vp, vp, C.c_size_t, vp]
-    L.cuth_set_loop_mode.restype = C.c_int
-    L.cuth_set_loop_mode.argtypes = [C.c_int]
-    L.cuth_set_traversal.restype = C.c_int
-    L.cuth_set_traversal.argtypes = [C.c_int]
     L.cuth_profile_kernel.restype = C.c_int
-    L.cuth_profile_kernel.argtypes = [vp, gp, C.c_int, vp]
+    L.cuth_profile_kernel.argtypes = [vp, gp, op, C.c_int, vp]
     _lib = L
     return L
 
@@ -152,10 +167,32 @@ class Grid:
         return C.byref(self.c)
 
 
+# The C library has no process-wide settings (include/cuth.h); the kernel variants travel in every call's
+# cuth_tuning_t.  For the test suite and bench.py, which run whole groups of calls under one variant, THIS PYTHON
+# MODULE keeps a default tuning that Opts() / DiaMatrix.spmv / the hooks below copy into their arguments.
+_DEFAULT_TUNING = dict(traversal=0, loop_mode=0, k1_variant=0, cheb_fusion=0, pair_rows=0, pair_occupancy=0)
+
+
+def set_default_tuning(**kw):
+    """Python-side default for the `tuning` argument of the calls made through this binding (0 = automatic)."""
+    for k, v in kw.items():
+        if k not in _DEFAULT_TUNING:
+            raise KeyError(k)
+        _DEFAULT_TUNING[k] = int(v)
+
+
+def Tuning(**kw):
+    d = dict(_DEFAULT_TUNING)
+    d.update({k: int(v) for k, v in kw.items()})
+    return cuth_tuning_t(d["traversal"], d["loop_mode"], d["k1_variant"], d["cheb_fusion"], d["pair_rows"],
+                         d["pair_occupancy"], (C.c_int32 * 2)(0, 0))
+
+
 def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI,
-         cheb_degree=30, cheb_lmin=0.0, cheb_lmax=0.0, cheb_storage=CHEB_DEFAULT):
+         cheb_degree=30, cheb_lmin=0.0, cheb_lmax=0.0, cheb_storage=CHEB_DEFAULT, tuning=None):
     return cuth_opts_t(int(precision), float(rtol), int(max_iters), int(true_resid_period), int(preconditioner),
-                       int(cheb_degree), float(cheb_lmin), float(cheb_lmax), int(cheb_storage))
+                       int(cheb_degree), float(cheb_lmin), float(cheb_lmax), int(cheb_storage),
+                       tuning if tuning is not None else Tuning())
 
 
 @dataclass
@@ -168,6 +205,9 @@ class Result:
     rel_resid_rec: float
     switch_reason: int
     switch_iteration: int
+    switch_mask: int = 0
+    hard_restarts: int = 0
+    soft_restarts: int = 0
 
     @property
     def status_name(self):
@@ -244,6 +284,12 @@ def cuth_spmv(dia, grid: Grid, precision, x, y, stream=None):
            "cuth_spmv")
 
 
+def cuth_spmv_tuned(dia, grid: Grid, precision, tuning, x, y, stream=None):
+    t = tuning if tuning is not None else Tuning()
+    _check(load_library().cuth_spmv_tuned(_ptr(dia), grid.ref(), int(precision), C.byref(t), _ptr(x), _ptr(y),
+                                          stream or _stream()), "cuth_spmv_tuned")
+
+
 def cuth_pcg_solve(dia, grid: Grid, opts, b, x, work, result, stream=None):
     _check(load_library().cuth_pcg_solve(_ptr(dia), grid.ref(), C.byref(opts), _ptr(b), _ptr(x), _ptr(work),
                                          work.numel() * work.element_size(), _ptr(result), stream or _stream()),
@@ -271,18 +317,33 @@ def cuth_release_workspace(work):
     load_library().cuth_release_workspace(_ptr(work))
 
 
-def cuth_profile_kernel(work, grid: Grid, kernel_id: int, stream=None):
-    _check(load_library().cuth_profile_kernel(_ptr(work), grid.ref(), int(kernel_id), stream or _stream()),
-           "cuth_profile_kernel")
+def cuth_profile_kernel(work, grid: Grid, opts, kernel_id: int, stream=None):
+    _check(load_library().cuth_profile_kernel(_ptr(work), grid.ref(), C.byref(opts), int(kernel_id),
+                                              stream or _stream()), "cuth_profile_kernel")
 
 
-def cuth_lanczos_bounds(dia, grid: Grid, v0, steps, work, stream=None):
+def cuth_lanczos_bounds(dia, grid: Grid, v0, steps, work, stream=None, tuning=None):
     """Returns (ritz_min, ritz_max, gershgorin_max, lmin, lmax); synchronises the stream."""
     out = (C.c_double * 5)()
-    _check(load_library().cuth_lanczos_bounds(_ptr(dia), grid.ref(), _ptr(v0), int(steps), _ptr(work),
-                                              work.numel() * work.element_size(), out, stream or _stream()),
-           "cuth_lanczos_bounds")
+    t = tuning if tuning is not None else Tuning()
+    _check(load_library().cuth_lanczos_bounds_tuned(_ptr(dia), grid.ref(), C.byref(t), _ptr(v0), int(steps),
+                                                    _ptr(work), work.numel() * work.element_size(), out,
+                                                    stream or _stream()), "cuth_lanczos_bounds")
     return tuple(out)
+
+
+def cuth_policy_probe(rr, tt, dd, tt_prev, rr_prev, bb, rtol, soft_drift=0.0, late=False, conv_rec=False,
+                      capped=False):
+    """The device-side decision after one evaluation of r_true (include/cuth.h cuth_policy_probe) on SQUARED norms;
+    returns dict(go, stage, switch_reason, switch_mask, restart, status, promotions).  Synchronises."""
+    import torch
+    vals = (C.c_double * 8)(float(rr), float(tt), float(dd), float(tt_prev), float(rr_prev), float(bb), float(rtol),
+                            float(soft_drift))
+    out = torch.zeros(8, dtype=torch.int32, device="cuda")
+    flags = (1 if late else 0) | (2 if conv_rec else 0) | (4 if capped else 0)
+    _check(load_library().cuth_policy_probe(vals, flags, _ptr(out), _stream()), "cuth_policy_probe")
+    o = out.cpu().tolist()
+    return dict(go=o[0], stage=o[1], switch_reason=o[2], switch_mask=o[3], restart=o[4], status=o[5], promotions=o[6])
 
 
 def cuth_cheb_apply(dia, grid: Grid, opts, r, z, work, stream=None):
@@ -312,44 +373,12 @@ def cuth_cheb_launches(grid: Grid, opts):
     return int(rc), int(pairs.value)
 
 
-def cuth_set_cheb_fusion(mode: int):
-    L = load_library()
-    L.cuth_set_cheb_fusion.restype = C.c_int
-    _check(L.cuth_set_cheb_fusion(C.c_int(int(mode))), "cuth_set_cheb_fusion")
-
-
-def cuth_set_pair_occupancy(ctas_per_sm: int):
-    L = load_library()
-    L.cuth_set_pair_occupancy.restype = C.c_int
-    _check(L.cuth_set_pair_occupancy(C.c_int(int(ctas_per_sm))), "cuth_set_pair_occupancy")
-
-
-def cuth_set_pair_rows(rows: int):
-    L = load_library()
-    L.cuth_set_pair_rows.restype = C.c_int
-    _check(L.cuth_set_pair_rows(C.c_int(int(rows))), "cuth_set_pair_rows")
-
-
-def cuth_set_k1_variant(mode: int):
-    L = load_library()
-    L.cuth_set_k1_variant.restype = C.c_int
-    _check(L.cuth_set_k1_variant(C.c_int(int(mode))), "cuth_set_k1_variant")
-
-
-def cuth_set_loop_mode(mode: int):
-    _check(load_library().cuth_set_loop_mode(int(mode)), "cuth_set_loop_mode")
-
-
-def cuth_set_traversal(mode: int):
-    _check(load_library().cuth_set_traversal(int(mode)), "cuth_set_traversal")
-
-
 def cuth_version() -> int:
     return int(load_library().cuth_version())
 
 
-def cuth_launches_per_iteration(grid: Grid) -> int:
-    return int(load_library().cuth_launches_per_iteration(grid.ref()))
+def cuth_launches_per_iteration(grid: Grid, opts) -> int:
+    return int(load_library().cuth_launches_per_iteration(grid.ref(), C.byref(opts)))
 
 
 # ------------------------------------------------------------------ convenience holders (allocation only)
@@ -386,7 +415,7 @@ class DiaMatrix:
     def spmv(self, x, precision=FP64, out=None):
         import torch
         y = torch.empty_like(x) if out is None else out
-        cuth_spmv(self.buf, self.grid, precision, x, y)
+        cuth_spmv_tuned(self.buf, self.grid, precision, None, x, y)
         return y
 
 
@@ -415,7 +444,8 @@ class BatchSolver:
         for s in range(self.nrhs):
             r = cuth_result_t.from_buffer_copy(raw[s * sz:(s + 1) * sz])
             out.append(Result(r.status, r.iterations, r.promotions, r.true_resid_evals, r.rel_resid_true,
-                              r.rel_resid_rec, r.switch_reason, r.switch_iteration))
+                              r.rel_resid_rec, r.switch_reason, r.switch_iteration, r.switch_mask, r.hard_restarts,
+                              r.soft_restarts))
         return out
 
 
@@ -433,10 +463,11 @@ class Solver:
         """Spectral range by Lanczos (cuth_lanczos_bounds) and switch this solver to the Chebyshev
         preconditioner; only copies the interval the library returns into the options struct."""
         import torch
-        lo, hi, gersh, rec_lo, rec_hi = cuth_lanczos_bounds(self.A.buf, self.A.grid, v0, lanczos_steps, self.work)
+        lo, hi, gersh, rec_lo, rec_hi = cuth_lanczos_bounds(self.A.buf, self.A.grid, v0, lanczos_steps, self.work,
+                                                            tuning=self.opts.tuning)
         o = self.opts
         self.opts = Opts(o.precision, o.rtol, o.max_iters, o.true_resid_period, PRECOND_CHEBYSHEV, degree,
-                         rec_lo if lmin is None else lmin, rec_hi if lmax is None else lmax, storage)
+                         rec_lo if lmin is None else lmin, rec_hi if lmax is None else lmax, storage, o.tuning)
         need = cuth_workspace_bytes(self.A.grid, self.opts)
         if need > self.work.numel():
             cuth_release_workspace(self.work)
@@ -457,7 +488,8 @@ class Solver:
         raw = self.result_dev.cpu().numpy().tobytes()
         r = cuth_result_t.from_buffer_copy(raw)
         return Result(r.status, r.iterations, r.promotions, r.true_resid_evals, r.rel_resid_true,
-                      r.rel_resid_rec, r.switch_reason, r.switch_iteration)
+                      r.rel_resid_rec, r.switch_reason, r.switch_iteration, r.switch_mask, r.hard_restarts,
+                      r.soft_restarts)
 
     def close(self):
         cuth_release_workspace(self.work)

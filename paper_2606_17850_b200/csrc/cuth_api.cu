@@ -6,7 +6,6 @@
 //                                   IF{ k_flush_x, k_true_resid, k_restart } } -> k_finalize
 #include <cmath>
 #include <cstdio>
-#include <atomic>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -19,6 +18,7 @@
 #include "cuth_cheb.cuh"
 #include "cuth_cheb_pair.cuh"
 #include "cuth_cheb_pair_tma.cuh"
+#include "cuth_fused_tma.cuh"
 #include "cuth_persistent.cuh"
 #include "cuth_batch.cuh"
 
@@ -42,14 +42,29 @@ static int cuda_fail(cudaError_t e, const char* what) {
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
-// Matrix objects written by cuth_import_csr, by address: 1 = MIXED available, 0 = FP64 only.  Host-side knowledge
-// only (the solver never reads the device header back); cuth_build_dia on the same buffer removes the entry.
-static std::mutex g_imp_mu;
-static std::unordered_map<const void*, int> g_imported;
-static int imported_state(const void* dia_D) {   // -1 not imported
-  std::lock_guard<std::mutex> lk(g_imp_mu);
-  auto it = g_imported.find(dia_D);
-  return it == g_imported.end() ? -1 : it->second;
+// Kernel variants of one call (cuth_tuning_t, validated): nothing here is process-wide.
+struct Tune {
+  int traversal = 0;    // 0 auto, 1 flat, 2 z-march
+  int loop_mode = 0;    // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel
+  int k1_variant = 0;   // 0 auto, 1 one column per thread, 2 two columns, 3 two columns without the TMA-staged K1
+  int cheb_pairs = 0;   // 0 auto, 1 never, 2 always (fp32 modes)
+  int pair_tma = 0;     // 0 auto (TMA when possible), 1 never
+  int pair_rows = 0;    // 0 auto, 8, 16
+  int pair_occ = 0;     // 0 auto (4), 2..4
+};
+static int make_tune(const cuth_tuning_t* t, Tune* T) {
+  *T = Tune();
+  if (!t) return CUTH_OK;
+  if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 2 || t->k1_variant < 0 ||
+      t->k1_variant > 3 || t->cheb_fusion < 0 || t->cheb_fusion > 3 ||
+      (t->pair_rows != 0 && t->pair_rows != 8 && t->pair_rows != 16) ||
+      (t->pair_occupancy != 0 && (t->pair_occupancy < 2 || t->pair_occupancy > 4)) || t->reserved[0] || t->reserved[1])
+    return CUTH_ERR_VALUE;
+  T->traversal = t->traversal; T->loop_mode = t->loop_mode; T->k1_variant = t->k1_variant;
+  T->cheb_pairs = t->cheb_fusion == 3 ? 2 : t->cheb_fusion;
+  T->pair_tma = t->cheb_fusion == 3 ? 1 : 0;
+  T->pair_rows = t->pair_rows; T->pair_occ = t->pair_occupancy;
+  return CUTH_OK;
 }
 
 static int check_grid(const cuth_grid_t* g, DiaLayout* L) {
@@ -59,42 +74,38 @@ static int check_grid(const cuth_grid_t* g, DiaLayout* L) {
   return CUTH_OK;
 }
 
-static std::atomic<int> g_loop_mode{0};   // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel (cuth_set_loop_mode)
-static std::atomic<int> g_traversal{0};   // 0 auto, 1 flat, 2 z-march (cuth_set_traversal)
-
 // Traversal choice: the flat kernel relies on L2 to keep the +-nx*ny neighbours (two planes of six
 // arrays, 96 B per plane cell); beyond ~1/3 of the 126 MB L2 that fails and z-marching wins.  On grids whose
 // vectors do not fit L2 anyway (> 2^21 rows) the fused two-kernel iteration of the z-marching path (8m + 80 B/row
 // against 8m + 104) already pays from 2^17 columns on: measured per Jacobi iteration, flat / z-marching,
 // 384x384x128 442 / 355 us, 512x256x128 393 / 329, 448x448x64 312 / 279, but 256x256x256 (2^16 columns: too few
 // CTAs) 383 / 413; the Chebyshev path is indifferent there (+-3 %).
-static bool use_zmarch(const DiaLayout& L) {
-  const int mode = g_traversal.load();
+static bool use_zmarch(const DiaLayout& L, const Tune& T) {
+  const int mode = T.traversal;
   if (mode == 1) return false;
   if (mode == 2) return true;
   return L.nxny >= (1 << 18) || (L.nxny >= (1 << 17) && L.n > (1 << 21));
 }
 
-static std::atomic<int> g_k1_variant{0};   // 0 auto (two columns per thread when nx is even), 1 one column, 2 two columns
 // Two columns per thread halve the number of CTAs: worth it only while the grid still has several waves
 // (cfg 5, 512x512 columns: 512 CTAs on 444 slots ran 13 % slower than the one-column kernel's 1024 CTAs).
 static bool enough_tiles_x2(const DiaLayout& L, int wx, int wy) {
   return ((L.nx + wx - 1) / wx) * ((L.ny + wy - 1) / wy) >= 2048;
 }
-static bool fused_x2(const DiaLayout& L) {
-  const int mode = g_k1_variant.load();
+static bool fused_x2(const DiaLayout& L, const Tune& T) {
+  const int mode = T.k1_variant;
   if (L.nx % 2 != 0 || mode == 1) return false;
-  return mode == 2 || enough_tiles_x2(L, XTX, XTY);
+  return mode >= 2 || enough_tiles_x2(L, XTX, XTY);
 }
-static bool zmarch_x2(const DiaLayout& L) {
-  const int mode = g_k1_variant.load();
+static bool zmarch_x2(const DiaLayout& L, const Tune& T) {
+  const int mode = T.k1_variant;
   if (L.nx % 2 != 0 || mode == 1) return false;
-  return mode == 2 || enough_tiles_x2(L, 2 * ZTX, ZTY);
+  return mode >= 2 || enough_tiles_x2(L, 2 * ZTX, ZTY);
 }
 
-static int stencil_blocks(const DiaLayout& L) {
-  if (!use_zmarch(L)) return -1;
-  const int64_t wx = zmarch_x2(L) ? 2 * ZTX : ZTX;         // two columns per thread (even nx, enough tiles)
+static int stencil_blocks(const DiaLayout& L, const Tune& T) {
+  if (!use_zmarch(L, T)) return -1;
+  const int64_t wx = zmarch_x2(L, T) ? 2 * ZTX : ZTX;         // two columns per thread (even nx, enough tiles)
   const int64_t tiles = ((L.nx + wx - 1) / wx) * ((L.ny + ZTY - 1) / ZTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
@@ -102,22 +113,22 @@ static int stencil_blocks(const DiaLayout& L) {
 static int grid_blocks(int64_t n);
 
 // fp32 Chebyshev middle step with two x-adjacent columns per thread: large planes with even nx
-static bool cheb_x2(const DiaLayout& L);
+static bool cheb_x2(const DiaLayout& L, const Tune& T);
 static int cheb_x2_blocks(const DiaLayout& L) {
   const int64_t tiles = ((L.nx + 2 * ZTX - 1) / (2 * ZTX)) * ((L.ny + ZTY - 1) / ZTY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
-static int cheb_blocks(const DiaLayout& L) {
-  if (!use_zmarch(L)) return grid_blocks(L.n);
+static int cheb_blocks(const DiaLayout& L, const Tune& T) {
+  if (!use_zmarch(L, T)) return grid_blocks(L.n);
   const int64_t tiles = ((L.nx + ZTX - 1) / ZTX) * ((L.ny + CUTH_CHEB_NC * ZTY - 1) / (CUTH_CHEB_NC * ZTY));
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
-static bool cheb_x2(const DiaLayout& L) { return use_zmarch(L) && zmarch_x2(L); }
+static bool cheb_x2(const DiaLayout& L, const Tune& T) { return use_zmarch(L, T) && zmarch_x2(L, T); }
 
-static int fused_blocks(const DiaLayout& L) {
-  if (fused_x2(L)) {
+static int fused_blocks(const DiaLayout& L, const Tune& T) {
+  if (fused_x2(L, T)) {
     const int64_t t2 = ((L.nx + XTX - 1) / XTX) * ((L.ny + XTY - 1) / XTY);
     return (int)(t2 < kMaxBlocks ? t2 : kMaxBlocks);
   }
@@ -125,7 +136,7 @@ static int fused_blocks(const DiaLayout& L) {
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
 
-static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
+static DiaDev dev_view(const void* dia_D, const DiaLayout& L, const Tune& T) {
   const char* base = (const char*)dia_D;
   const double* v = (const double*)(base + L.o_vals);
   const float* f = (const float*)(base + L.o_vals32);
@@ -143,10 +154,11 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L) {
   A.h_scale = lay + 4 * L.nz;
   A.s_layer = lay + L.nz;
   A.cap_layer = lay + 2 * L.nz;
+  A.hdr = (const unsigned long long*)base;
   A.n = L.n; A.nx = L.nx; A.nxny = L.nxny;
   A.ny = (int32_t)L.ny; A.nz = (int32_t)L.nz;
-  A.zmarch = use_zmarch(L) ? 1 : 0;
-  A.x2 = zmarch_x2(L) ? 1 : 0;
+  A.zmarch = use_zmarch(L, T) ? 1 : 0;
+  A.x2 = zmarch_x2(L, T) ? 1 : 0;
   return A;
 }
 
@@ -175,13 +187,12 @@ static void* cheb_mid_fn(int code, bool x2) {
 static void* cheb_pair_fn(int code) {
   return code == 2 ? (void*)k_cheb_pair_f32<MatF16> : (void*)k_cheb_pair_f32<MatF32>;
 }
-static std::atomic<int> g_cheb_pairs{0};   // 0 auto, 1 never, 2 always (fp32 modes): cuth_set_cheb_fusion
 static int cheb_pair_blocks(const DiaLayout& L) {
   const int64_t tiles = ((L.nx + QIX - 1) / QIX) * ((L.ny + QIY - 1) / QIY);
   return (int)(tiles < kMaxBlocks ? tiles : kMaxBlocks);
 }
-static bool cheb_pairs(const DiaLayout& L, int code) {
-  const int mode = g_cheb_pairs.load();
+static bool cheb_pairs(const DiaLayout& L, int code, const Tune& T) {
+  const int mode = T.cheb_pairs;
   // fp32 arithmetic, column pairs: nx even.  Measured faster on every grid (cfg 2 23.5 -> 21.0 ms, cfg 3 0.92 ->
   // 0.63 s, cfg 4 10.8 -> 7.9 s, cfg 5 5.8 -> 4.3 s, cfg 6 41 -> 34 ms), so automatic = always.
   return code != 0 && mode != 1 && (L.nx & 1) == 0;
@@ -202,9 +213,8 @@ static EncodeTiledFn encode_tiled_fn() {
   }();
   return fn;
 }
-static std::atomic<int> g_pair_tma{0};     // 0 auto (TMA when possible), 1 never (LDG version): cuth_set_cheb_fusion bit 2
-static bool cheb_pairs_tma(const DiaLayout& L, int code) {
-  if (!cheb_pairs(L, code) || g_pair_tma.load() == 1) return false;
+static bool cheb_pairs_tma(const DiaLayout& L, int code, const Tune& T) {
+  if (!cheb_pairs(L, code, T) || T.pair_tma == 1) return false;
   const int64_t elems16 = code == 2 ? 8 : 4;           // tensor-map strides are multiples of 16 bytes
   return (L.nx % elems16) == 0 && encode_tiled_fn() != nullptr;
 }
@@ -225,7 +235,7 @@ static bool make_box_map(CUtensorMap* m, const void* base, bool half, const DiaL
 struct PairMaps { CUtensorMap u, v, r, f1, f2, f3; };
 static bool make_pair_maps(PairMaps* pm, const DiaLayout& L, const void* dia_D, const Workspace& w, int code,
                            int old, int cur, int ry) {
-  const DiaDev A = dev_view(dia_D, L);
+  const DiaDev A = dev_view(dia_D, L, Tune());
   const void* cd[4] = {w.cd0, w.cd1, w.cd2, w.cd3};
   const bool h = code == 2;
   return make_box_map(&pm->u, cd[cur], false, L, ry + 2) && make_box_map(&pm->v, cd[old], false, L, ry) &&
@@ -244,9 +254,8 @@ static void* cheb_pair_tma_fn(int code, bool last, int ry) {
 }
 // Region height of the TMA kernel: 16 rows (512 threads) recompute a sixth less than 8 rows; taken when the
 // plane still gives every SM several regions.  cuth_set_pair_rows forces it.
-static std::atomic<int> g_pair_rows{0};    // 0 automatic, 8, 16
-static int pair_tma_rows(const DiaLayout& L) {
-  const int forced = g_pair_rows.load();
+static int pair_tma_rows(const DiaLayout& L, const Tune& T) {
+  const int forced = T.pair_rows;
   if (forced == 8 || forced == 16) return forced;
   const int64_t tiles16 = ((L.nx + QIX - 1) / QIX) * ((L.ny + 13) / 14);
   return tiles16 >= 4 * 296 ? 16 : 8;
@@ -260,16 +269,15 @@ static int pair_tma_blocks(const DiaLayout& L, int ry) {
 // regions -- cfg 3 has 3078 regions = 5.2 waves of 592 but 6.9 waves of 444.  Measured: occupancy wins over wave
 // rounding (pair launch at cfg 3: 0.103 ms with 4, 0.109 with 3, 0.133 with 2; cfg 4: 0.73 / 0.83 ms), so
 // automatic = 4.
-static std::atomic<int> g_pair_occ{0};     // 0 automatic (4), 2..4 forced: cuth_set_pair_occupancy
-static int pair_tma_occupancy(const DiaLayout&) {
-  const int forced = g_pair_occ.load();
+static int pair_tma_occupancy(const Tune& T) {
+  const int forced = T.pair_occ;
   return (forced >= 2 && forced <= 4) ? forced : 4;
 }
-static unsigned pair_tma_dyn_smem(const DiaLayout& L, int code, int ry) {
+static unsigned pair_tma_dyn_smem(const Tune& T, int code, int ry) {
   size_t need;
   if (ry == 16) need = code == 2 ? sizeof(PairSmem<__half, 16>) : sizeof(PairSmem<float, 16>);
   else need = code == 2 ? sizeof(PairSmem<__half, 8>) : sizeof(PairSmem<float, 8>);
-  const int full_occ = ry == 16 ? 2 : 4, occ = pair_tma_occupancy(L) * full_occ / 4;
+  const int full_occ = ry == 16 ? 2 : 4, occ = pair_tma_occupancy(T) * full_occ / 4;
   if (occ >= 1 && occ < full_occ) {                   // forced lower occupancy: too much for occ + 1 CTAs
     const size_t per_cta = (size_t)(227 * 1024) / (size_t)(occ + 1) + 1024;
     if (per_cta > need) need = per_cta;
@@ -279,17 +287,58 @@ static unsigned pair_tma_dyn_smem(const DiaLayout& L, int code, int ry) {
   return (unsigned)need;
 }
 
+// ---- TMA-staged K1 (cuth_fused_tma.cuh): tensor maps over (x, y, z) for r, p, p2, 1/D0, D0 and the two sets of
+// aligned per-diagonal off-diagonals (fp32 A2, fp64 A1)
+static bool make_map3d(CUtensorMap* m, const void* base, int elem_bytes, const DiaLayout& L, int box_w, int box_rows) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t es = (cuuint64_t)elem_bytes;
+  const cuuint64_t dims[3] = {(cuuint64_t)L.nx, (cuuint64_t)L.ny, (cuuint64_t)L.nz};
+  const cuuint64_t strides[2] = {(cuuint64_t)L.nx * es, (cuuint64_t)L.nxny * es};
+  const cuuint32_t box[3] = {(cuuint32_t)box_w, (cuuint32_t)box_rows, 1u};
+  const cuuint32_t estr[3] = {1u, 1u, 1u};
+  return enc(m, elem_bytes == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+             const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+static bool make_k1_maps(K1Maps* km, K1Maps* km64, const DiaLayout& L, const void* dia_D, const Workspace& w) {
+  const DiaDev A = dev_view(dia_D, L, Tune());
+  const char* base = (const char*)dia_D;
+  const void* e1 = base + L.o_f64a;
+  const void* e2 = base + L.o_f64a + L.f64a_stride;
+  const void* e3 = base + L.o_f64a + 2 * L.f64a_stride;
+  return make_map3d(&km->z, w.r, 8, L, K1VW, K1VH) && make_map3d(&km->p, w.p, 8, L, K1VW, K1VH) &&
+         make_map3d(&km->p2, w.p2, 8, L, K1VW, K1VH) && make_map3d(&km->d, A.dinv, 8, L, K1VW, K1VH) &&
+         make_map3d(&km->m1, A.f1, 4, L, K1Stage<true>::W1, K1Y) && make_map3d(&km->m2, A.f2, 4, L, K1X, K1Y + 1) &&
+         make_map3d(&km->m3, A.f3, 4, L, K1X, K1Y) &&
+         make_map3d(&km64->d, A.d0, 8, L, K1VW, K1VH) && make_map3d(&km64->m1, e1, 8, L, K1Stage<false>::W1, K1Y) &&
+         make_map3d(&km64->m2, e2, 8, L, K1X, K1Y + 1) && make_map3d(&km64->m3, e3, 8, L, K1X, K1Y);
+}
+static unsigned k1_tma_dyn_smem() {
+  const size_t need = sizeof(K1Smem<true>) > sizeof(K1Smem<false>) ? sizeof(K1Smem<true>) : sizeof(K1Smem<false>);
+  cudaFuncSetAttribute((const void*)k_fused_pspmv_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need);
+  return (unsigned)need;
+}
+// K1 takes its operands through TMA when it runs two columns per thread (nx even, enough tiles), nx % 4 == 0 (strides of
+// the fp32 tensors), z is r (no Chebyshev), the driver can encode tensor maps, and the variant is not forced away.
+static bool fused_tma(const DiaLayout& L, const Tune& T, bool cheb) {
+  if (cheb || T.k1_variant == 1 || T.k1_variant == 3) return false;
+  return fused_x2(L, T) && (L.nx % 4) == 0 && encode_tiled_fn() != nullptr;
+}
+// persistent over tiles: as many CTAs as are resident (2 per SM), never more than tiles
+static int fused_tma_blocks(const DiaLayout& L);
+
 // one two-pass launch outside a graph (cuth_cheb_apply, cuth_profile_kernel)
-static cudaError_t launch_pair(const DiaLayout& L, const void* dia_D, const Workspace& w, int code, const ChebOp& op,
-                               cudaStream_t st) {
+static cudaError_t launch_pair(const DiaLayout& L, const Tune& T, const void* dia_D, const Workspace& w, int code,
+                               const ChebOp& op, cudaStream_t st) {
   Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
   PairMaps pm;
-  const int ry = pair_tma_rows(L);
-  if (cheb_pairs_tma(L, code) && make_pair_maps(&pm, L, dia_D, w, code, old, cur, ry)) {
+  const int ry = pair_tma_rows(L, T);
+  if (cheb_pairs_tma(L, code, T) && make_pair_maps(&pm, L, dia_D, w, code, old, cur, ry)) {
     void* a[] = {&ctxp, &ctlp, &part, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};
     return cudaLaunchKernel(cheb_pair_tma_fn(code, op.kind == 3, ry), dim3(pair_tma_blocks(L, ry)), dim3(32 * ry), a,
-                            pair_tma_dyn_smem(L, code, ry), st);
+                            pair_tma_dyn_smem(T, code, ry), st);
   }
   if (op.kind == 3) return cudaErrorInvalidValue;      // the fused MID + LAST launch exists only as a TMA kernel
   void* a[] = {&ctxp, &step, &old, &cur, &wo, &yo};
@@ -327,20 +376,32 @@ static std::vector<ChebOp> cheb_schedule(int k, bool pairs, bool fuse_last) {
 }
 
 // ------------------------------------------------------------------------------------------
+// Everything that determines the SHAPE of the graph of a solve (kernels, grids, baked tensor maps, workspace
+// layout): the key of the graph cache.  Per-call pointers and options travel in Ctx, not in the graph.
+struct Plan {
+  int64_t n = 0;
+  int sblocks = 0;       // grid of the kernels that apply A (z-marching tiles, or the flat grid)
+  int fblocks = 0;       // > 0: fused path (K1 + K2); grid of K1
+  int k1x2 = 0;          // K1 with two columns per thread
+  int chebkey = 0;       // degree * 4 + arithmetic code, 0 = no Chebyshev preconditioner
+  int cblocks = 0, x2blocks = 0, pblocks = 0;    // Chebyshev single-pass / two-column / two-pass grids
+  int with_b = 0;        // transient matrix: b lives in the workspace, the Chebyshev buffers sit N doubles later
+  int pair_tma = 0;      // the two-pass Chebyshev nodes are the TMA kernel
+  int k1tma = 0;         // K1 is the TMA-staged kernel
+  const void* dia = nullptr;   // matrix the tensor maps of the TMA nodes were made for (else nullptr)
+  int64_t tnx = 0, tny = 0;    // ... and its plane dimensions
+  int tocc = 0;                // ... occupancy * 100 + region rows of the TMA two-pass nodes
+  int device = -1;
+  bool operator==(const Plan& o) const {
+    return n == o.n && sblocks == o.sblocks && fblocks == o.fblocks && k1x2 == o.k1x2 && chebkey == o.chebkey &&
+           cblocks == o.cblocks && x2blocks == o.x2blocks && pblocks == o.pblocks && with_b == o.with_b &&
+           pair_tma == o.pair_tma && k1tma == o.k1tma && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
+  }
+};
 struct GraphEntry {
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t exec = nullptr;
-  int64_t n = 0;
-  int sblocks = 0;
-  int fblocks = 0;
-  int chebkey = 0;
-  int x2blocks = 0;
-  int k1x2 = 0;
-  int pblocks = 0;
-  const void* dia = nullptr;   // matrix the tensor maps of the TMA two-pass nodes were made for (else nullptr)
-  int64_t tnx = 0, tny = 0;    // ... and its plane dimensions (the maps are baked into the kernel nodes)
-  int tocc = 0;                // ... and the occupancy its TMA nodes were launched for
-  int device = -1;
+  Plan plan;
 };
 static std::mutex g_mu;
 static std::unordered_map<const void*, GraphEntry> g_graphs;
@@ -358,10 +419,9 @@ static cudaError_t add_kernel(cudaGraph_t g, cudaGraphNode_t* node, const cudaGr
   return cudaGraphAddKernelNode(node, g, deps, ndeps, &kp);
 }
 
-static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, int chebkey, int cblocks,
-                       int x2blocks, int k1x2, int pblocks, const DiaLayout* Ltma, const void* dia_tma, GraphEntry* out) {
-  const int blocks = grid_blocks(n);
-  if (sblocks <= 0) sblocks = blocks;      // grid of the kernels that apply A
+static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, const Tune& T, GraphEntry* out) {
+  const int blocks = grid_blocks(P.n);
+  const int sblocks = P.sblocks;
   cudaGraph_t g;
   CU(cudaGraphCreate(&g, 0));
   cudaGraphConditionalHandle h_while, h_if;
@@ -386,42 +446,50 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   // Chebyshev: the body starts with the preconditioner z = q(A) r: k-1 stencil kernels, no reduction
   // until the last one, which also forms rho = r.z and beta (Alg. 1 lines 10-11).
   cudaGraphNode_t n_c = nullptr;
-  const int kdeg = chebkey >> 2;
+  const int kdeg = P.chebkey >> 2;
   if (kdeg > 0) {
-    const int code = chebkey & 3;
+    const int code = P.chebkey & 3;
     const bool f32 = code != 0;
     { void* a[] = {&ctx};
-      CU(add_kernel(body, &n_c, nullptr, 0, cheb_first_fn(code), cblocks, a)); }
-    for (const ChebOp& op : cheb_schedule(kdeg, pblocks > 0, dia_tma != nullptr)) {
+      CU(add_kernel(body, &n_c, nullptr, 0, cheb_first_fn(code), P.cblocks, a)); }
+    for (const ChebOp& op : cheb_schedule(kdeg, P.pblocks > 0, P.pair_tma != 0)) {
       cudaGraphNode_t prev = n_c;
       int step = op.step, old = op.old, cur = op.cur, wo = op.w, yo = op.y;
       PairMaps pm;
-      if ((op.kind == 1 || op.kind == 3) && dia_tma) {
-        const int ry = pair_tma_rows(*Ltma);
-        if (!make_pair_maps(&pm, *Ltma, dia_tma, w, code, old, cur, ry)) return CUTH_ERR_CUDA;
+      if ((op.kind == 1 || op.kind == 3) && P.pair_tma) {
+        const int ry = pair_tma_rows(L, T);
+        if (!make_pair_maps(&pm, L, P.dia, w, code, old, cur, ry)) return CUTH_ERR_CUDA;
         void* a[] = {&ctx, &ctl, &partials, &step, &wo, &yo, &pm.u, &pm.v, &pm.r, &pm.f1, &pm.f2, &pm.f3};   // copied into the node
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3, ry), pair_tma_blocks(*Ltma, ry), a,
-                      pair_tma_dyn_smem(*Ltma, code, ry), 32 * ry));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_tma_fn(code, op.kind == 3, ry), pair_tma_blocks(L, ry), a,
+                      pair_tma_dyn_smem(T, code, ry), 32 * ry));
       } else if (op.kind == 1) {
         void* a[] = {&ctx, &step, &old, &cur, &wo, &yo};
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), pblocks, a));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_pair_fn(code), P.pblocks, a));
       } else if (op.kind == 0) {
         void* a[] = {&ctx, &step, &old, &cur};
-        if (f32 && x2blocks > 0)
-          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, true), x2blocks, a));
+        if (f32 && P.x2blocks > 0)
+          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, true), P.x2blocks, a));
         else
-          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, false), cblocks, a));
+          CU(add_kernel(body, &n_c, &prev, 1, cheb_mid_fn(code, false), P.cblocks, a));
       } else {
         void* a[] = {&ctx, &ctl, &partials, &step, &old, &cur};
-        CU(add_kernel(body, &n_c, &prev, 1, cheb_last_fn(code), cblocks, a));
+        CU(add_kernel(body, &n_c, &prev, 1, cheb_last_fn(code), P.cblocks, a));
       }
     }
   }
   const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
   const size_t ndep0 = n_c ? 1 : 0;
-  if (fblocks > 0) {
-    { void* a[] = {&ctx, &ctl, &partials};
-      CU(add_kernel(body, &n_s, dep0, ndep0, k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, fblocks, a)); }
+  if (P.fblocks > 0) {
+    if (P.k1tma) {
+      K1Maps km, km64;
+      if (!make_k1_maps(&km, &km64, L, P.dia, w)) return CUTH_ERR_CUDA;
+      void* a[] = {&ctx, &ctl, &partials, &km.z, &km.p, &km.p2, &km.d, &km64.d, &km.m1, &km.m2, &km.m3,
+                   &km64.m1, &km64.m2, &km64.m3};                      // the maps are copied into the node
+      CU(add_kernel(body, &n_s, dep0, ndep0, (void*)k_fused_pspmv_tma, P.fblocks, a, k1_tma_dyn_smem()));
+    } else {
+      void* a[] = {&ctx, &ctl, &partials};
+      CU(add_kernel(body, &n_s, dep0, ndep0, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
+    }
     { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
       CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a)); }
   } else {
@@ -440,37 +508,26 @@ static int build_graph(const Workspace& w, int64_t n, int sblocks, int fblocks, 
   CU(cudaGraphAddNode(&n_if, body, &n_u, 1, &ip));
   cudaGraph_t ifb = ip.conditional.phGraph_out[0];
   cudaGraphNode_t n_f, n_t, n_r;
-  if (fblocks > 0) {
+  if (P.fblocks > 0) {
     void* a[] = {&ctx, &ctl};
     CU(add_kernel(ifb, &n_f, nullptr, 0, (void*)k_flush_x, blocks, a));
   }
   { void* a[] = {&ctx, &ctl, &partials, &h_while};
-    CU(add_kernel(ifb, &n_t, fblocks > 0 ? &n_f : nullptr, fblocks > 0 ? 1 : 0, (void*)k_true_resid, sblocks, a)); }
+    CU(add_kernel(ifb, &n_t, P.fblocks > 0 ? &n_f : nullptr, P.fblocks > 0 ? 1 : 0, (void*)k_true_resid, sblocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials};
     CU(add_kernel(ifb, &n_r, &n_t, 1, (void*)k_restart, blocks, a)); }
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));
-  out->graph = g; out->exec = ex; out->n = n; out->sblocks = sblocks; out->fblocks = fblocks; out->chebkey = chebkey; out->x2blocks = x2blocks; out->k1x2 = k1x2; out->pblocks = pblocks; out->dia = dia_tma;
-  if (dia_tma) { out->tnx = Ltma->nx; out->tny = Ltma->ny; out->tocc = pair_tma_occupancy(*Ltma) * 100 + pair_tma_rows(*Ltma); }
-  cudaGetDevice(&out->device);
+  out->graph = g; out->exec = ex; out->plan = P;
   return CUTH_OK;
 }
 
-static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, int fblocks, int chebkey,
-                     int cblocks, int x2blocks, int k1x2, int pblocks, const DiaLayout* Ltma, const void* dia_tma,
+static int get_graph(const Workspace& w, void* work_D, const Plan& P, const DiaLayout& L, const Tune& T,
                      cudaGraphExec_t* ex) {
   std::lock_guard<std::mutex> lk(g_mu);
   auto it = g_graphs.find(work_D);
-  int dev = -1;
-  cudaGetDevice(&dev);
-  if (it != g_graphs.end() && (it->second.n != n || it->second.device != dev ||
-                               it->second.sblocks != (sblocks > 0 ? sblocks : grid_blocks(n)) ||
-                               it->second.fblocks != fblocks || it->second.chebkey != chebkey ||
-                               it->second.x2blocks != x2blocks || it->second.k1x2 != k1x2 ||
-                               it->second.pblocks != pblocks || it->second.dia != dia_tma ||
-                               (dia_tma && (it->second.tnx != Ltma->nx || it->second.tny != Ltma->ny ||
-                                            it->second.tocc != pair_tma_occupancy(*Ltma) * 100 + pair_tma_rows(*Ltma))))) {
+  if (it != g_graphs.end() && !(it->second.plan == P)) {
     cudaGraphExecDestroy(it->second.exec);
     cudaGraphDestroy(it->second.graph);
     g_graphs.erase(it);
@@ -478,7 +535,7 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
   }
   if (it == g_graphs.end()) {
     GraphEntry e;
-    int rc = build_graph(w, n, sblocks, fblocks, chebkey, cblocks, x2blocks, k1x2, pblocks, Ltma, dia_tma, &e);
+    int rc = build_graph(w, P, L, T, &e);
     if (rc != CUTH_OK) return rc;
     it = g_graphs.emplace(work_D, e).first;
   }
@@ -489,7 +546,10 @@ static int get_graph(const Workspace& w, void* work_D, int64_t n, int sblocks, i
 static int check_opts(const cuth_opts_t* o) {
   if (!o) return CUTH_ERR_NULL;
   if (!(o->rtol > 0.0) || o->max_iters <= 0) return CUTH_ERR_VALUE;
-  if (o->precision != CUTH_FP64 && o->precision != CUTH_MIXED) return CUTH_ERR_VALUE;
+  if (o->precision != CUTH_FP64 && o->precision != CUTH_MIXED && o->precision != CUTH_MIXED_STD32) return CUTH_ERR_VALUE;
+  if (o->precision == CUTH_MIXED_STD32 && o->preconditioner == CUTH_PRECOND_CHEBYSHEV) return CUTH_ERR_VALUE;   // ablation: Alg. 1 with M = D0 or I
+  Tune T;
+  if (make_tune(&o->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
   if (o->preconditioner != CUTH_PRECOND_NONE && o->preconditioner != CUTH_PRECOND_JACOBI &&
       o->preconditioner != CUTH_PRECOND_CHEBYSHEV)
     return CUTH_ERR_VALUE;
@@ -526,27 +586,42 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
 // 96 CTAs 12.4 / 13.9 / 16.0 / 27.7 / 72, 128 CTAs 7.1 / 7.3 / 8.1 / 13.9 / 47, 148 CTAs 8.0 / 8.0 / 8.8 / 14.2 / 46,
 // 256 CTAs 9.2 / 8.4 / 8.4 / 12.4 / 33, 592 CTAs 13.4 / 14.1 / 13.7 / 16.7 / 29.8.  So: 128 CTAs up to 64 k rows (CTAs
 // beyond the rows only take part in the barriers), 256 up to 512 k rows, everything the device holds beyond.
+// Co-resident CTAs of a cooperative kernel, per device (derived data, filled on first use under the mutex).
+static std::mutex g_dev_mu;
+static std::unordered_map<long long, int> g_coresident;      // (device << 8 | kernel slot) -> CTAs
+static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, size_t dyn_smem = 0) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  std::lock_guard<std::mutex> lk(g_dev_mu);
+  const long long key = ((long long)dev << 8) | slot;
+  auto it = g_coresident.find(key);
+  if (it != g_coresident.end()) return it->second;
+  int sms = 0, coop = 0, occ = 0;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem);
+  if (occ > max_per_sm) occ = max_per_sm;
+  int v = (coop || slot == 2) ? sms * occ : 0;          // slot 2 (the TMA K1) is an ordinary launch
+  if (v > cap) v = cap;
+  g_coresident[key] = v;
+  return v;
+}
+static int fused_tma_blocks(const DiaLayout& L) {
+  const int64_t tiles = ((L.nx + K1X - 1) / K1X) * ((L.ny + K1Y - 1) / K1Y);
+  const int resident = coresident_blocks(2, (const void*)k_fused_pspmv_tma, 2, kMaxBlocks, k1_tma_dyn_smem());
+  return (int)(tiles < resident ? tiles : (resident > 0 ? resident : 1));
+}
 static int persistent_blocks(int64_t n) {
-  static int cached = -1;
-  if (cached < 0) {
-    int dev = 0, sms = 0, coop = 0, occ = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pcg_persistent, kThreads, 0);
-    if (occ > 4) occ = 4;
-    cached = coop ? sms * occ : 0;
-    if (cached > kPersistMaxBlocks) cached = kPersistMaxBlocks;
-  }
-  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : cached);   // > 512 k rows: all co-resident CTAs
-  return want < cached ? want : cached;
+  const int all = coresident_blocks(0, (const void*)k_pcg_persistent, 4, kPersistMaxBlocks);
+  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : all);   // > 512 k rows: all co-resident CTAs
+  return want < all ? want : all;
 }
 
-static bool use_persistent(const DiaLayout& L, bool cheb) {
-  const int mode = g_loop_mode.load(), trav = g_traversal.load();
+static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
+  const int mode = T.loop_mode, trav = T.traversal;
   if (cheb || mode == 1 || trav == 2) return false;
   if (persistent_blocks(L.n) <= 0) return false;
-  if (mode == 2) return !use_zmarch(L);        // forced: wherever the flat traversal applies
+  if (mode == 2) return !use_zmarch(L, T);        // forced: wherever the flat traversal applies
   // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
   // 7.0 / 18.7 us at cfg 1 (8 k rows), 19.3 / 30.4 us at cfg 6 (655 k), 23.2 / 34.7 us at cfg 2 (1 M); and on wide
   // planes, against the z-marching graph: 512x512x4 23.2 / 36.1, 512x512x8 47.7 / 60.3, 1024x1024x2 47.0 / 66.1,
@@ -554,6 +629,35 @@ static bool use_persistent(const DiaLayout& L, bool cheb) {
   // is three more kernels and an IF node in the graph, one more phase in the kernel).  Auto: the persistent kernel
   // (its row access is flat whatever the plane shape) for every grid of up to 2^22 rows; beyond, the graph.
   return L.n <= (1 << 22);
+}
+
+// The graph of a solve with these options on this grid.
+static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts, bool with_b, const void* dia_D) {
+  Plan P;
+  const bool cheb = opts->preconditioner == CUTH_PRECOND_CHEBYSHEV;
+  const int code = cheb_code(opts);
+  const bool zm = use_zmarch(L, T);
+  P.n = L.n;
+  const int sb = stencil_blocks(L, T);
+  P.sblocks = sb > 0 ? sb : grid_blocks(L.n);
+  P.fblocks = zm ? fused_blocks(L, T) : 0;
+  P.k1x2 = (zm && fused_x2(L, T)) ? 1 : 0;
+  if (zm && fused_tma(L, T, cheb)) {
+    P.k1tma = 1; P.fblocks = fused_tma_blocks(L);
+    P.dia = dia_D; P.tnx = L.nx; P.tny = L.ny;
+  }
+  P.chebkey = cheb ? opts->cheb_degree * 4 + code : 0;
+  P.cblocks = cheb_blocks(L, T);
+  P.x2blocks = cheb_x2(L, T) ? cheb_x2_blocks(L) : 0;
+  P.pblocks = (cheb && cheb_pairs(L, code, T)) ? cheb_pair_blocks(L) : 0;
+  P.with_b = with_b ? 1 : 0;
+  if (cheb && cheb_pairs_tma(L, code, T)) {
+    P.pair_tma = 1;
+    P.dia = dia_D; P.tnx = L.nx; P.tny = L.ny;
+    P.tocc = pair_tma_occupancy(T) * 100 + pair_tma_rows(L, T);
+  }
+  cudaGetDevice(&P.device);
+  return P;
 }
 
 static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
@@ -570,14 +674,15 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
     return CUTH_ERR_ALIGN;
   const bool transient = power_D != nullptr;
   if (transient && !(grid->cvol_H && grid->dt > 0.0)) return CUTH_ERR_NOT_TRANSIENT;
-  const int imp = imported_state(dia_D);
-  if (transient && imp >= 0) return CUTH_ERR_NOT_TRANSIENT;
-  if (imp == 0 && opts->precision == CUTH_MIXED) return CUTH_ERR_FP64_ONLY;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
   const bool cheb = opts->preconditioner == CUTH_PRECOND_CHEBYSHEV;
-  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, cheb);
-  DiaDev A = dev_view(dia_D, L);
+  const bool with_b = grid->cvol_H && grid->dt > 0.0;
+  Tune T;
+  make_tune(&opts->tuning, &T);
+  if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;    // the ablation operator exists in the flat kernels only
+  Workspace w = carve_workspace(work_D, L.n, with_b, cheb);
+  DiaDev A = dev_view(dia_D, L, T);
   const int blocks = grid_blocks(L.n);
   if (transient) {
     k_transient_rhs<<<blocks, kThreads, 0, st>>>(A, power_D, x_D, w.b);
@@ -596,24 +701,26 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   c.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
   c.cheb = 0;
   if (cheb) fill_cheb(&c, opts, w);
-  c.persist_fuse = L.n <= (1 << 14) ? 1 : 0;   // persistent kernel: phases A and B in one on the smallest grids
+  c.early_op = opts->precision == CUTH_MIXED_STD32 ? OP_STD32 : OP_DIFF32;
+  c.transient_call = transient ? 1 : 0;
+  // persistent kernel: phases A and B in one on the smallest grids (not with the ablation operator)
+  c.persist_fuse = (L.n <= (1 << 14) && c.early_op == OP_DIFF32) ? 1 : 0;
   c.soft_restart = 1;         // promotion keeps p while the drift is small (DESIGN.md R-G11)
   c.soft_drift2 = 1e-2;       // ||t - r|| <= 0.1 ||t||
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   { std::lock_guard<std::mutex> lk(g_mu); g_last_dia[work_D] = dia_D; }
-  if (use_persistent(L, cheb)) {
+  if (use_persistent(L, cheb, T)) {
     Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
     void* args[] = {&ctxp, &ctlp, &part};
-    CU(cudaLaunchCooperativeKernel((void*)k_pcg_persistent, dim3(persistent_blocks(L.n)), dim3(kThreads), args, 0, st));
-    return CUTH_OK;
+    const cudaError_t e = cudaLaunchCooperativeKernel((void*)k_pcg_persistent, dim3(persistent_blocks(L.n)),
+                                                      dim3(kThreads), args, 0, st);
+    if (e == cudaSuccess) return CUTH_OK;
+    if (T.loop_mode == 2) return cuda_fail(e, "cudaLaunchCooperativeKernel(k_pcg_persistent)");
+    cudaGetLastError();       // automatic mode: the graph loop serves every grid (e.g. under an SM-limited context)
   }
   cudaGraphExec_t ex;
-  rc = get_graph(w, work_D, L.n, stencil_blocks(L), use_zmarch(L) ? fused_blocks(L) : 0,
-                 cheb ? opts->cheb_degree * 4 + cheb_code(opts) : 0, cheb_blocks(L), cheb_x2(L) ? cheb_x2_blocks(L) : 0,
-                 (use_zmarch(L) && fused_x2(L)) ? 1 : 0,
-                 (cheb && cheb_pairs(L, cheb_code(opts))) ? cheb_pair_blocks(L) : 0, &L,
-                 (cheb && cheb_pairs_tma(L, cheb_code(opts))) ? dia_D : nullptr, &ex);
+  rc = get_graph(w, work_D, make_plan(L, T, opts, with_b, dia_D), L, T, &ex);
   if (rc) return rc;
   CU(cudaGraphLaunch(ex, st));
   return CUTH_OK;
@@ -681,7 +788,6 @@ int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void*
     if (grid->cvol_H && grid->dt > 0.0 && !(grid->cvol_H[z] > 0.0)) return CUTH_ERR_VALUE;
   }
   cudaError_t e = cudaSuccess;
-  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
   rc = launch_build(grid, L, dia_D, (cudaStream_t)stream, &e);
   if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_build_dia");
   return rc;
@@ -703,11 +809,9 @@ int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int3
   cuth_import_report_t rep;
   memset(&rep, 0, sizeof rep);
   cudaError_t e = cudaSuccess;
-  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
   rc = launch_import(grid, L, rowptr_D, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e);
   if (report_H) *report_H = rep;
   if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_import_csr");
-  if (rc == CUTH_OK) { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported[dia_D] = rep.mixed_ok; }
   return rc;
 }
 
@@ -725,24 +829,32 @@ int cuth_dia_view(const void* dia_D, const cuth_grid_t* grid, const double** val
   return CUTH_OK;
 }
 
-int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const double* x_D, double* y_D,
-              void* stream) {
+int cuth_spmv_tuned(const void* dia_D, const cuth_grid_t* grid, int precision, const cuth_tuning_t* tuning,
+                    const double* x_D, double* y_D, void* stream) {
   DiaLayout L;
   int rc = check_grid(grid, &L);
   if (rc) return rc;
   if (!dia_D || !x_D || !y_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(y_D)) return CUTH_ERR_ALIGN;
-  if (precision != CUTH_FP64 && precision != CUTH_MIXED && precision != CUTH_ABLATION_STD32) return CUTH_ERR_VALUE;
+  if (precision != CUTH_FP64 && precision != CUTH_MIXED && precision != CUTH_MIXED_STD32) return CUTH_ERR_VALUE;
   if (x_D == y_D) return CUTH_ERR_VALUE;
-  if (precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
-  DiaDev A = dev_view(dia_D, L);
-  const int sb = stencil_blocks(L);
+  Tune T;
+  if (make_tune(tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
+  if (precision == CUTH_MIXED_STD32) T.traversal = 1;
+  DiaDev A = dev_view(dia_D, L, T);
+  const int sb = stencil_blocks(L, T);
   const int blocks = sb > 0 ? sb : grid_blocks(L.n);
-  if (precision == CUTH_ABLATION_STD32) k_spmv_std32<<<grid_blocks(L.n), kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
-  else if (precision == CUTH_MIXED) k_spmv_only<true><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
-  else k_spmv_only<false><<<blocks, kThreads, 0, (cudaStream_t)stream>>>(A, x_D, y_D);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (precision == CUTH_MIXED_STD32) k_spmv_only<OP_STD32><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);
+  else if (precision == CUTH_MIXED) k_spmv_only<OP_DIFF32><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);
+  else k_spmv_only<OP_FP64><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);
   CU(cudaGetLastError());
   return CUTH_OK;
+}
+
+int cuth_spmv(const void* dia_D, const cuth_grid_t* grid, int precision, const double* x_D, double* y_D,
+              void* stream) {
+  return cuth_spmv_tuned(dia_D, grid, precision, nullptr, x_D, y_D, stream);
 }
 
 int cuth_pcg_solve(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* b_D,
@@ -768,11 +880,9 @@ int cuth_import_coo(const cuth_grid_t* grid, const int32_t* row_D, const int32_t
   cuth_import_report_t rep;
   memset(&rep, 0, sizeof rep);
   cudaError_t e = cudaSuccess;
-  { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported.erase(dia_D); }
   rc = launch_import(grid, L, nullptr, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e, row_D, nnz);
   if (report_H) *report_H = rep;
   if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_import_coo");
-  if (rc == CUTH_OK) { std::lock_guard<std::mutex> lk(g_imp_mu); g_imported[dia_D] = rep.mixed_ok; }
   return rc;
 }
 
@@ -792,7 +902,7 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   if (rc) return rc;
   if (nrhs < 1 || nrhs > kBatchMaxRhs) return CUTH_ERR_VALUE;
   if (opts->preconditioner != CUTH_PRECOND_JACOBI && opts->preconditioner != CUTH_PRECOND_NONE) return CUTH_ERR_VALUE;
-  if (opts->precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
+  if (opts->precision != CUTH_FP64 && opts->precision != CUTH_MIXED) return CUTH_ERR_VALUE;
   if (!dia_D || !b_D || !x_D || !work_D || !result_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(x_D) || !aligned16(work_D) || !aligned16(b_D) || ((uintptr_t)result_D & 7u))
     return CUTH_ERR_ALIGN;
@@ -800,16 +910,7 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   if (work_bytes < w.bytes) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
   // co-resident CTAs available, split into ceil(nrhs / S) chunks x ntiles row tiles
-  static int max_blocks = -1;
-  if (max_blocks < 0) {
-    int dev = 0, sms = 0, coop = 0, occ = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_pcg_batch, kThreads, 0);
-    if (occ > 3) occ = 3;
-    max_blocks = coop ? sms * occ : 0;
-  }
+  const int max_blocks = coresident_blocks(1, (const void*)k_pcg_batch, 3, 1 << 20);
   const int nchunks = (nrhs + kBatchChunk - 1) / kBatchChunk;
   if (max_blocks < nchunks) { g_last_err = "cuth_pcg_solve_batch: cooperative launch unavailable"; return CUTH_ERR_CUDA; }
   const int64_t need = (L.n + (int64_t)kThreads - 1) / (int64_t)kThreads;
@@ -820,7 +921,7 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   if (ntiles > kBatchMaxBlocks) ntiles = kBatchMaxBlocks;
   BatchCtx c;
   memset(&c, 0, sizeof c);
-  c.A = dev_view(dia_D, L);
+  c.A = dev_view(dia_D, L, Tune());
   c.b = b_D; c.x = x_D; c.r = w.r; c.p = w.p; c.mu = w.mu;
   c.result = result_D;
   c.rtol = opts->rtol;
@@ -844,32 +945,50 @@ int cuth_transient_step(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   return solve_common(dia_D, grid, opts, nullptr, power_D, T_D, work_D, work_bytes, result_D, stream);
 }
 
-int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, void* stream) {
+int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t* opts, int kernel_id, void* stream) {
   DiaLayout L;
   int rc = check_grid(grid, &L);
   if (rc) return rc;
-  if (!work_D) return CUTH_ERR_NULL;
+  if (!work_D || !opts) return CUTH_ERR_NULL;
+  Tune T;
+  if (make_tune(&opts->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
+  if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
   cudaStream_t st = (cudaStream_t)stream;
-  Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
+  const bool with_b = grid->cvol_H && grid->dt > 0.0;
+  Workspace w = carve_workspace(work_D, L.n, with_b);
   const int blocks = grid_blocks(L.n);
-  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
+  const int sb = stencil_blocks(L, T) > 0 ? stencil_blocks(L, T) : blocks;
   cudaGraphConditionalHandle h0 = 0;
   switch (kernel_id) {
-    case -1: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl); break;
+    case -1: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl, 0); break;
+    case -2: k_mark_no_graph<<<1, 1, 0, st>>>(w.ctl, 1); break;
     case 0: k_pupdate<<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl); break;
     case 1: k_spmv_dot<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 4:
-      if (fused_x2(L)) k_fused_pspmv_x2<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
-      else k_fused_pspmv<<<fused_blocks(L), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
+      if (fused_tma(L, T, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV)) {
+        const void* dia = nullptr;
+        { std::lock_guard<std::mutex> lk(g_mu);
+          auto it = g_last_dia.find(work_D);
+          if (it != g_last_dia.end()) dia = it->second; }
+        if (!dia) return CUTH_ERR_VALUE;           // no solve has used this workspace yet
+        K1Maps km, km64;
+        if (!make_k1_maps(&km, &km64, L, dia, w)) return CUTH_ERR_CUDA;
+        Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
+        void* a[] = {&ctxp, &ctlp, &part, &km.z, &km.p, &km.p2, &km.d, &km64.d, &km.m1, &km.m2, &km.m3,
+                     &km64.m1, &km64.m2, &km64.m3};
+        CU(cudaLaunchKernel((const void*)k_fused_pspmv_tma, dim3(fused_tma_blocks(L)), dim3(kThreads), a,
+                            k1_tma_dyn_smem(), st));
+      } else if (fused_x2(L, T)) k_fused_pspmv_x2<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
+      else k_fused_pspmv<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       break;
     case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
       const int code = kernel_id - 6;
-      const bool x2 = code != 0 && cheb_x2(L);
+      const bool x2 = code != 0 && cheb_x2(L, T);
       Ctx* ctxp = w.ctx; int step = 1, old = 1, cur = 0;
       void* args[] = {&ctxp, &step, &old, &cur};
-      CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : cheb_blocks(L)), dim3(kThreads), args, 0, st));
+      CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : cheb_blocks(L, T)), dim3(kThreads), args, 0, st));
     } break;
     case 9: case 10: {            // one fused pair of Chebyshev passes, fp32 on A2 / on A3
       const void* dia = nullptr;
@@ -878,8 +997,8 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
         if (it != g_last_dia.end()) dia = it->second; }
       if (!dia) return CUTH_ERR_VALUE;             // no solve has used this workspace yet
       const ChebOp op = {1, 1, 1, 0, 2, 3};
-      const Workspace wc = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, true);   // with the Z buffers
-      CU(launch_pair(L, dia, wc, kernel_id == 10 ? 2 : 1, op, st));
+      const Workspace wc = carve_workspace(work_D, L.n, with_b, true);   // with the Z buffers
+      CU(launch_pair(L, T, dia, wc, kernel_id == 10 ? 2 : 1, op, st));
     } break;
     case 3: k_true_resid<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0); break;
     default: return CUTH_ERR_VALUE;
@@ -888,20 +1007,22 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, int kernel_id, vo
   return CUTH_OK;
 }
 
-int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
-                        size_t work_bytes, double bounds_H[5], void* stream) {
+int cuth_lanczos_bounds_tuned(const void* dia_D, const cuth_grid_t* grid, const cuth_tuning_t* tuning, const double* v0_D,
+                              int steps, void* work_D, size_t work_bytes, double bounds_H[5], void* stream) {
   DiaLayout L;
   int rc = check_grid(grid, &L);
   if (rc) return rc;
   if (!dia_D || !v0_D || !work_D || !bounds_H) return CUTH_ERR_NULL;
   if (steps < 2 || steps > 120) return CUTH_ERR_VALUE;
   if (!aligned16(dia_D) || !aligned16(v0_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
+  Tune T;
+  if (make_tune(tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
   Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0);
   if (work_bytes < w.bytes) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
-  DiaDev A = dev_view(dia_D, L);
+  DiaDev A = dev_view(dia_D, L, T);
   const int blocks = grid_blocks(L.n);
-  const int sb = stencil_blocks(L) > 0 ? stencil_blocks(L) : blocks;
+  const int sb = stencil_blocks(L, T) > 0 ? stencil_blocks(L, T) : blocks;
   LanczosScal* sc = (LanczosScal*)(w.partials + 3 * kMaxBlocks);
   static_assert(sizeof(LanczosScal) <= sizeof(double) * kMaxBlocks, "LanczosScal must fit one partial slot");
   CU(cudaMemsetAsync(sc, 0, sizeof(LanczosScal), st));
@@ -928,6 +1049,11 @@ int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double
   return CUTH_OK;
 }
 
+int cuth_lanczos_bounds(const void* dia_D, const cuth_grid_t* grid, const double* v0_D, int steps, void* work_D,
+                        size_t work_bytes, double bounds_H[5], void* stream) {
+  return cuth_lanczos_bounds_tuned(dia_D, grid, nullptr, v0_D, steps, work_D, work_bytes, bounds_H, stream);
+}
+
 int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_t* opts, const double* r_D,
                     double* z_D, void* work_D, size_t work_bytes, void* stream) {
   DiaLayout L;
@@ -939,28 +1065,29 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   if (!dia_D || !r_D || !z_D || !work_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(r_D) || !aligned16(z_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
-  if (opts->precision == CUTH_MIXED && imported_state(dia_D) == 0) return CUTH_ERR_FP64_ONLY;
+  Tune T;
+  make_tune(&opts->tuning, &T);
   cudaStream_t st = (cudaStream_t)stream;
   Workspace w = carve_workspace(work_D, L.n, grid->cvol_H && grid->dt > 0.0, true);
   Ctx c;
   memset(&c, 0, sizeof c);
-  c.A = dev_view(dia_D, L);
+  c.A = dev_view(dia_D, L, T);
   c.r = const_cast<double*>(r_D);      // read only here
   fill_cheb(&c, opts, w);
   c.cz = z_D;
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
-  const int blocks = grid_blocks(L.n);
-  const int sb = cheb_blocks(L);
+  CU(cudaGetLastError());
+  const int sb = cheb_blocks(L, T);
   const int k = opts->cheb_degree;
   const int code = cheb_code(opts);
-  const bool x2 = code != 0 && cheb_x2(L);
+  const bool x2 = code != 0 && cheb_x2(L, T);
   Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
   { void* a[] = {&ctxp};
     CU(cudaLaunchKernel(cheb_first_fn(code), dim3(sb), dim3(kThreads), a, 0, st)); }
-  for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code), cheb_pairs_tma(L, code))) {
+  for (const ChebOp& op : cheb_schedule(k, cheb_pairs(L, code, T), cheb_pairs_tma(L, code, T))) {
     int step = op.step, old = op.old, cur = op.cur;
     if (op.kind == 1 || op.kind == 3) {
-      CU(launch_pair(L, dia_D, w, code, op, st));
+      CU(launch_pair(L, T, dia_D, w, code, op, st));
     } else if (op.kind == 0) {
       void* a[] = {&ctxp, &step, &old, &cur};
       CU(cudaLaunchKernel(cheb_mid_fn(code, x2), dim3(x2 ? cheb_x2_blocks(L) : sb), dim3(kThreads), a, 0, st));
@@ -969,7 +1096,35 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
       CU(cudaLaunchKernel(cheb_last_fn(code), dim3(sb), dim3(kThreads), a, 0, st));
     }
   }
-  (void)blocks;
+  CU(cudaGetLastError());
+  return CUTH_OK;
+}
+
+// Test hook: the decision function of the solver kernels on caller-given scalars (include/cuth.h).
+__global__ void k_policy_probe(double rr, double tt, double dd, double tt_prev, double rr_prev, double bb, double rtol,
+                               double soft_drift, int flags, int32_t* out) {
+  Ctl ctl;
+  memset(&ctl, 0, sizeof ctl);
+  Ctx c;
+  memset(&c, 0, sizeof c);
+  c.rtol = rtol; c.max_iters = 1000; c.soft_restart = soft_drift >= 0.0 ? 1 : 0;
+  c.soft_drift2 = soft_drift > 0.0 ? soft_drift * soft_drift : 1e-2;
+  ctl.status = CUTH_SOLVE_RUNNING;
+  ctl.bb = bb; ctl.tol2 = rtol * rtol * bb; ctl.sw2 = fmax(rtol, rtol * rtol) * bb;
+  ctl.rr = rr; ctl.tt_prev = tt_prev; ctl.rr_prev_eval = rr_prev;
+  ctl.stage = (flags & 1) ? 1 : 0;
+  ctl.conv_rec = (flags & 2) ? 1 : 0;
+  ctl.it = (flags & 4) ? c.max_iters : 10;
+  const unsigned go = policy_after_true(&ctl, c, tt, dd);
+  out[0] = (int32_t)go; out[1] = ctl.stage; out[2] = ctl.switch_reason; out[3] = ctl.switch_mask; out[4] = ctl.restart;
+  out[5] = ctl.status; out[6] = ctl.promotions; out[7] = 0;
+}
+
+int cuth_policy_probe(const double in_H[8], int flags, int32_t* out_D, void* stream) {
+  if (!in_H || !out_D) return CUTH_ERR_NULL;
+  if (((uintptr_t)out_D & 3u)) return CUTH_ERR_ALIGN;
+  k_policy_probe<<<1, 1, 0, (cudaStream_t)stream>>>(in_H[0], in_H[1], in_H[2], in_H[3], in_H[4], in_H[5], in_H[6], in_H[7],
+                                                    flags, out_D);
   CU(cudaGetLastError());
   return CUTH_OK;
 }
@@ -978,43 +1133,6 @@ int cuth_tridiag_extremes(const double* alpha_H, const double* beta_H, int m, do
   if (!alpha_H || !out_H || (m > 1 && !beta_H)) return CUTH_ERR_NULL;
   if (m < 1) return CUTH_ERR_VALUE;
   tridiag_extremes(alpha_H, beta_H, m, &out_H[0], &out_H[1]);
-  return CUTH_OK;
-}
-
-int cuth_set_cheb_fusion(int mode) {
-  if (mode < 0 || mode > 3) return CUTH_ERR_VALUE;
-  g_cheb_pairs.store(mode == 3 ? 2 : mode);
-  g_pair_tma.store(mode == 3 ? 1 : 0);
-  return CUTH_OK;
-}
-
-int cuth_set_pair_rows(int rows) {
-  if (rows != 0 && rows != 8 && rows != 16) return CUTH_ERR_VALUE;
-  g_pair_rows.store(rows);
-  return CUTH_OK;
-}
-
-int cuth_set_pair_occupancy(int ctas_per_sm) {
-  if (ctas_per_sm != 0 && (ctas_per_sm < 2 || ctas_per_sm > 4)) return CUTH_ERR_VALUE;
-  g_pair_occ.store(ctas_per_sm);
-  return CUTH_OK;
-}
-
-int cuth_set_k1_variant(int mode) {
-  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
-  g_k1_variant.store(mode);
-  return CUTH_OK;
-}
-
-int cuth_set_loop_mode(int mode) {
-  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
-  g_loop_mode.store(mode);
-  return CUTH_OK;
-}
-
-int cuth_set_traversal(int mode) {
-  if (mode < 0 || mode > 2) return CUTH_ERR_VALUE;
-  g_traversal.store(mode);
   return CUTH_OK;
 }
 
@@ -1034,11 +1152,13 @@ const char* cuth_last_cuda_error(void) { return g_last_err.c_str(); }
 
 int cuth_version(void) { return 10000; }
 
-int cuth_launches_per_iteration(const cuth_grid_t* grid) {
+int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts) {
   DiaLayout L;
-  if (!make_layout(grid, &L)) return 0;
-  if (use_persistent(L, false)) return 0;      // one persistent kernel for the whole solve
-  return use_zmarch(L) ? 2 : 3;
+  Tune T;
+  if (!make_layout(grid, &L) || !opts || make_tune(&opts->tuning, &T) != CUTH_OK) return 0;
+  if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
+  if (use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T)) return 0;      // one persistent kernel for the whole solve
+  return use_zmarch(L, T) ? 2 : 3;
 }
 
 int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pairs_out) {
@@ -1046,9 +1166,11 @@ int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pa
   if (!opts) return CUTH_ERR_NULL;
   if (!make_layout(grid, &L)) return CUTH_ERR_DIMS;
   if (opts->preconditioner != CUTH_PRECOND_CHEBYSHEV) { if (pairs_out) *pairs_out = 0; return 0; }
+  Tune T;
+  if (make_tune(&opts->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
   int pairs = 0, launches = 1;                   // FIRST
-  for (const ChebOp& op : cheb_schedule(opts->cheb_degree, cheb_pairs(L, cheb_code(opts)),
-                                        cheb_pairs_tma(L, cheb_code(opts)))) {
+  for (const ChebOp& op : cheb_schedule(opts->cheb_degree, cheb_pairs(L, cheb_code(opts), T),
+                                        cheb_pairs_tma(L, cheb_code(opts), T))) {
     ++launches;
     if (op.kind == 1 || op.kind == 3) ++pairs;
   }

@@ -211,6 +211,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_pcg_batch(const BatchCtx* __res
   const bool jac = c.jacobi != 0;
   // the policy code reads its options from a Ctx: only these fields are consulted on this path
   Ctx pc;
+  pc.A = c.A; pc.transient_call = 0;          // the matrix object's own header is checked by policy_init
   pc.rtol = c.rtol; pc.precision = c.precision; pc.max_iters = c.max_iters; pc.period = c.period; pc.cheb = 0;
   pc.soft_restart = 1; pc.soft_drift2 = 1e-2;       // as cuth_pcg_solve (DESIGN.md R-G11)
   int parity = 0;

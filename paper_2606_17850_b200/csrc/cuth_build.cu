@@ -94,13 +94,37 @@ __global__ void __launch_bounds__(256) k_make_h16(BuildArgs a, const double* slo
 
 // The off-diagonals of A2 once more, one 256-B aligned array of n floats per diagonal (zero beyond the
 // diagonal's length): what the solver kernels read.  The packed fp32 copy stays what cuth_dia_view shows.
-__global__ void __launch_bounds__(256) k_make_f32a(BuildArgs a, float* g1, float* g2, float* g3) {
+// ... and the same for the fp64 off-diagonals of A1 (e1..e3): the operands of the TMA-staged K1 (cuth_fused_tma.cuh).
+__global__ void __launch_bounds__(256) k_make_f32a(BuildArgs a, float* g1, float* g2, float* g3, double* e1, double* e2,
+                                                   double* e3) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
-    g1[i] = i + 1 < a.n ? a.f1[i] : 0.f;
-    g2[i] = i + a.nx < a.n ? a.f2[i] : 0.f;
-    g3[i] = i + a.nxny < a.n ? a.f3[i] : 0.f;
+    const bool h1 = i + 1 < a.n, h2 = i + a.nx < a.n, h3 = i + a.nxny < a.n;
+    g1[i] = h1 ? a.f1[i] : 0.f;
+    g2[i] = h2 ? a.f2[i] : 0.f;
+    g3[i] = h3 ? a.f3[i] : 0.f;
+    e1[i] = h1 ? a.d1[i] : 0.0;
+    e2[i] = h2 ? a.d2[i] : 0.0;
+    e3[i] = h3 ? a.d3[i] : 0.0;
   }
+}
+
+// Small host arrays (header, per-layer tables) reach the matrix object as KERNEL ARGUMENTS, 64 words per launch:
+// no pageable cudaMemcpyAsync (which blocks the host and cannot be stream-captured), no pinned staging buffer to
+// keep alive -- cuth_build_dia is asynchronous and capturable like every other call.
+struct WordChunk { unsigned long long w[64]; };
+__global__ void k_write_words(unsigned long long* dst, WordChunk c, int count) {
+  if ((int)threadIdx.x < count) dst[threadIdx.x] = c.w[threadIdx.x];
+}
+static cudaError_t write_words(void* dst, const void* src_H, size_t nwords, cudaStream_t st) {
+  const unsigned long long* src = (const unsigned long long*)src_H;
+  for (size_t o = 0; o < nwords; o += 64) {
+    WordChunk c;
+    const int cnt = (int)(nwords - o < 64 ? nwords - o : 64);
+    memcpy(c.w, src + o, sizeof(unsigned long long) * (size_t)cnt);
+    k_write_words<<<1, 64, 0, st>>>((unsigned long long*)dst + o, c, cnt);
+  }
+  return cudaGetLastError();
 }
 
 // Host side: fills the per-layer arrays, launches the kernel.  Called from cuth_api.cu.
@@ -109,7 +133,8 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   const int nz = (int)g->nz;
   const bool transient = g->cvol_H != nullptr && g->dt > 0.0;
   // per-layer arrays inside the matrix object: dz | s | cap | cvol
-  double* h = new double[4 * nz + 4];
+  std::vector<double> hv(4 * (size_t)nz + 4);
+  double* h = hv.data();
   for (int k = 0; k < 4; ++k) h[4 * nz + k] = 0.0;
   for (int z = 0; z < nz; ++z) {
     const double axy = g->dx * g->dy;
@@ -125,10 +150,9 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   hdr[3] = (unsigned long long)g->nz; hdr[4] = (unsigned long long)L.e; hdr[5] = transient ? 1ull : 0ull;
   for (int k = 0; k < 5; ++k) hdr[6 + k] = (unsigned long long)L.ptr[k];
   for (int k = 0; k < 4; ++k) hdr[11 + k] = (unsigned long long)L.off[k];
-  cudaError_t e = cudaMemcpyAsync(base, hdr, kHeaderBytes, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess)
-    e = cudaMemcpyAsync(base + L.o_layers, h, (4 * nz + 4) * sizeof(double), cudaMemcpyHostToDevice, st);
-  delete[] h;   // pageable H2D copies are staged before cudaMemcpyAsync returns
+  hdr[kHdrImported] = 0ull; hdr[kHdrMixedOk] = 1ull;
+  cudaError_t e = write_words(base, hdr, kHeaderBytes / 8, st);
+  if (e == cudaSuccess) e = write_words(base + L.o_layers, h, 4 * (size_t)nz + 4, st);
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   BuildArgs a;
   a.nx = L.nx; a.ny = L.ny; a.nz = L.nz; a.n = L.n; a.nxny = L.nxny;
@@ -153,7 +177,9 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
                                                (__half*)(base + L.o_h16 + L.h16_stride),
                                                (__half*)(base + L.o_h16 + 2 * L.h16_stride));
   k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(a, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
-                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride));
+                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride), (double*)(base + L.o_f64a),
+                                                (double*)(base + L.o_f64a + L.f64a_stride),
+                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride));
   e = cudaGetLastError();
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   return CUTH_OK;
@@ -384,7 +410,7 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   hdr[3] = (unsigned long long)L.nz; hdr[4] = (unsigned long long)L.e; hdr[5] = 0ull;
   for (int k = 0; k < 5; ++k) hdr[6 + k] = (unsigned long long)L.ptr[k];
   for (int k = 0; k < 4; ++k) hdr[11 + k] = (unsigned long long)L.off[k];
-  hdr[15] = 1ull;   // imported
+  hdr[kHdrImported] = 1ull; hdr[kHdrMixedOk] = 0ull;   // MIXED availability is settled at the end of the import
   cudaError_t e = cudaMemcpyAsync(base, hdr, kHeaderBytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(base + L.o_layers, h.data(), nlay * 8, cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
@@ -426,7 +452,9 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   k_make_h16<<<(unsigned)blocks, 256, 0, st>>>(b, slot, (__half*)(base + L.o_h16), (__half*)(base + L.o_h16 + L.h16_stride),
                                                (__half*)(base + L.o_h16 + 2 * L.h16_stride));
   k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(b, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
-                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride));
+                                                (float*)(base + L.o_f32a + 2 * L.f32a_stride), (double*)(base + L.o_f64a),
+                                                (double*)(base + L.o_f64a + L.f64a_stride),
+                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride));
   e = cudaGetLastError();
   unsigned long long cnt[5];
   if (e == cudaSuccess) e = cudaMemcpyAsync(cnt, a.cnt, sizeof cnt, cudaMemcpyDeviceToHost, st);
@@ -452,6 +480,9 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   if (!ok || !structure_ok)
     for (int z = 0; z < nz; ++z) lay_out[nz + z] = nan("");   // second line of defence: a MIXED solve breaks down loudly
   e = cudaMemcpyAsync(lay, lay_out.data(), lay_out.size() * 8, cudaMemcpyHostToDevice, st);
+  const unsigned long long mixed_ok = (ok && structure_ok) ? 1ull : 0ull;    // recorded IN the object (device header)
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync((unsigned long long*)base + kHdrMixedOk, &mixed_ok, 8, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   if (rep) {

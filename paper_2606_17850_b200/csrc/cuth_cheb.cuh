@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_lanczos_1(DiaDev A, const doubl
   __shared__ int s_flag;
   const double s_cur = sc->s_cur, cprev = sc->beta_prev * sc->s_prev;
   double acc[1] = {0.0};
-  apply_A<false>(A, u_cur, [&](int64_t i, double ui, double Au) {
+  apply_A<OP_FP64>(A, u_cur, [&](int64_t i, double ui, double Au) {
     const double ti = s_cur * Au - cprev * u_prev[i];
     t[i] = ti;
     acc[0] = fma(ti, ui, acc[0]);

@@ -16,6 +16,9 @@ constexpr uint64_t kMagic = 0x4355544844494131ull;  // "CUTHDIA1"
 constexpr int kMaxBlocks = 8192;       // upper bound on the grid of any reducing kernel
 constexpr int kNumPartialSlots = 4;
 constexpr int kMaxChebDegree = 64;    // partial-sum arrays (each kMaxBlocks doubles)
+// 64-bit words of the matrix header (device memory; what the object IS is recorded in the object)
+constexpr int kHdrMagic = 0, kHdrNx = 1, kHdrNy = 2, kHdrNz = 3, kHdrE = 4, kHdrTransient = 5, kHdrImported = 15,
+              kHdrMixedOk = 16;
 
 // Host-computed placement of the sections inside the caller's matrix buffer.
 struct DiaLayout {
@@ -29,6 +32,9 @@ struct DiaLayout {
   size_t h16_stride; // bytes between the three fp16 arrays
   size_t o_f32a;     // fp32 3 x [n] (each 256-B aligned): the off-diagonals of A2 again, one array per diagonal, so
   size_t f32a_stride;//   that the pair (D_k[i], D_k[i+1]), i even, is one 8-byte load (packed D2, D3 start at odd elements)
+  size_t o_f64a;     // fp64 3 x [n] (each 256-B aligned): the off-diagonals of A1 again, one array per diagonal with a zero
+  size_t f64a_stride;//   tail: proper (nx, ny, nz) tensors for the TMA-staged K1 (packed D2, D3 start at odd elements, and a
+                     //   tensor map needs a 16-byte aligned base)
   size_t bytes;
 };
 
@@ -53,6 +59,8 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
   L->o_h16 = o;    o = o + 3 * L->h16_stride;
   L->f32a_stride = align_up(sizeof(float) * (size_t)L->n);
   L->o_f32a = o;   o = o + 3 * L->f32a_stride;
+  L->f64a_stride = align_up(sizeof(double) * (size_t)L->n);
+  L->o_f64a = o;   o = o + 3 * L->f64a_stride;
   L->bytes = o;
   return true;
 }
@@ -68,6 +76,7 @@ struct DiaDev {
   const double* dinv;       // 1/D0
   const double* s_layer;    // exact row sums per layer: h dx dy [top] + C V / dt
   const double* cap_layer;  // C V / dt per layer (0 when steady)
+  const unsigned long long* hdr;   // the object's header (kHdr* words)
   int64_t n, nx, nxny;
   int32_t ny, nz;
   int32_t zmarch, x2;       // zmarch 1: march in z per thread (plane neighbours in registers), 0: flat 1-D
@@ -88,7 +97,9 @@ struct Ctx {
   double soft_drift2;   // soft restart allowed while ||t - r||^2 <= soft_drift2 * ||t||^2
   int32_t precision, max_iters, period, jacobi;
   int32_t soft_restart, cheb;     // cheb: degree k of the Chebyshev polynomial preconditioner, 0 = off
-  int32_t persist_fuse, pad_pf;   // persistent kernel: phases A and B in one (p' recomputed at the six neighbours)
+  int32_t persist_fuse;           // persistent kernel: phases A and B in one (p' recomputed at the six neighbours)
+  int32_t early_op;               // operator of the early stage: 1 = difference form (R-F3), 2 = A2 in standard form (ablation)
+  int32_t transient_call, pad_tc; // 1: cuth_transient_step (the matrix object must be a transient one)
   // Chebyshev preconditioner (Alg. 3): z = q(A) r.  cz: z (fp64) handed to the outer
   // loop; cd[4]: partial-sum buffers Z (two are live at any time; the fused two-pass kernel writes the other
   // two); crc: fp32 copy of r (MIXED only).  Element type T = double in FP64 mode, float in MIXED mode;
@@ -104,7 +115,8 @@ struct Ctl {
   double tt, dd, tt_prev, rr_prev_eval;
   double xalpha;   // pending x += xalpha * p (fused path defers Alg. 1 line 8 by one kernel)
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
-  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, beta_zero, pad3;
+  int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, beta_zero, switch_mask;
+  int32_t hard_restarts, soft_restarts, refused, pad4;
   unsigned int ticket[8];
 };
 

@@ -13,14 +13,30 @@ constexpr int kRows = 2;        // rows per thread per tile (strided by blockDim
 // One row of y = A v, Alg. 2 read 0-based: 7 terms, out-of-range terms dropped.  The structural
 // zeros stored in D1/D2 (x = nx-1, y = ny-1) make the lateral wrap-around vanish by themselves,
 // so the operator is purely banded in the linear index i.
-// MIXED = false: fp64 matrix A1 (kernel K1 of the paper).
-// MIXED = true : fp32-stored off-diagonals promoted to fp64 (K3) and applied in
-//                difference form  y_i = s_i v_i + sum_j g_ij (v_i - v_j)   (DESIGN.md R-F3).
-template <bool MIXED>
+// OP = 0: fp64 matrix A1 (kernel K1 of the paper).
+// OP = 1: fp32-stored off-diagonals promoted to fp64 (K3) and applied in
+//         difference form  y_i = s_i v_i + sum_j g_ij (v_i - v_j)   (DESIGN.md R-F3).
+// OP = 2: ABLATION (CUTH_MIXED_STD32): the paper's K3 literally -- all four diagonals of the fp32-rounded copy A2,
+//         D0 included, promoted to fp64 and applied in standard form.
+constexpr int OP_FP64 = 0, OP_DIFF32 = 1, OP_STD32 = 2;
+template <int OP>
 __device__ __forceinline__ double spmv_row(const DiaDev& A, const double* __restrict__ v, int64_t i, double vi) {
   const int64_t n = A.n, nx = A.nx, np = A.nxny;
   const bool up1 = i + 1 < n, lo1 = i >= 1, up2 = i + nx < n, lo2 = i >= nx, up3 = i + np < n, lo3 = i >= np;
-  if (!MIXED) {
+  if (OP == OP_STD32) {
+    const double a0 = (double)A.f0[i];
+    const double a1u = up1 ? (double)A.f1[i] : 0.0, a1l = lo1 ? (double)A.f1[i - 1] : 0.0;
+    const double a2u = up2 ? (double)A.f2[i] : 0.0, a2l = lo2 ? (double)A.f2[i - nx] : 0.0;
+    const double a3u = up3 ? (double)A.f3[i] : 0.0, a3l = lo3 ? (double)A.f3[i - np] : 0.0;
+    const double v1u = up1 ? v[i + 1] : 0.0, v1l = lo1 ? v[i - 1] : 0.0;
+    const double v2u = up2 ? v[i + nx] : 0.0, v2l = lo2 ? v[i - nx] : 0.0;
+    const double v3u = up3 ? v[i + np] : 0.0, v3l = lo3 ? v[i - np] : 0.0;
+    double acc = a0 * vi;
+    acc = fma(a1u, v1u, acc); acc = fma(a1l, v1l, acc);
+    acc = fma(a2u, v2u, acc); acc = fma(a2l, v2l, acc);
+    acc = fma(a3u, v3u, acc); acc = fma(a3l, v3l, acc);
+    return acc;
+  } else if (OP == OP_FP64) {
     // issue all loads first
     const double a0 = A.d0[i];
     const double a1u = up1 ? A.d1[i] : 0.0, a1l = lo1 ? A.d1[i - 1] : 0.0;
@@ -195,9 +211,10 @@ __device__ __forceinline__ void zmarch_apply_x2(const DiaDev& A, const double* _
 }
 
 // y_i = (A v)_i handed to f(i, v_i, y_i) for every row, with the traversal chosen at build time.
-template <bool MIXED, class F>
+template <int OP, class F>
 __device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restrict__ v, F&& f) {
-  if (A.zmarch) {
+  constexpr bool MIXED = OP == OP_DIFF32;
+  if (OP != OP_STD32 && A.zmarch) {              // the ablation operator exists in the flat traversal only
     if (A.x2) zmarch_apply_x2<MIXED>(A, v, f);
     else zmarch_apply<MIXED>(A, v, f);
   } else {
@@ -207,7 +224,7 @@ __device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restric
         const int64_t i = base + threadIdx.x + k * kThreads;
         if (i < A.n) {
           const double vi = v[i];
-          f(i, vi, spmv_row<MIXED>(A, v, i, vi));
+          f(i, vi, spmv_row<OP>(A, v, i, vi));
         }
       }
     }
@@ -216,34 +233,9 @@ __device__ __forceinline__ void apply_A(const DiaDev& A, const double* __restric
 
 // ---------------------------------------------------------------------------------------------
 // Standalone SpMV (cuth_spmv).
-template <bool MIXED>
+template <int OP>
 __global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_only(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
-  apply_A<MIXED>(A, x, [&](int64_t i, double, double yi) { y[i] = yi; });
-}
-
-// ABLATION ONLY (Table VI of the paper): the paper's "FP64/32 SpMV with AD"
-// taken literally -- ALL four diagonals of the fp32-rounded copy A2 in standard form,
-// promoted to fp64.  Rounding D0 perturbs it by ~5e-11 W/K, the size of the whole convective term that
-// fixes the mean temperature, so b - A2 x has a floor of ~1e-2 ||b|| on these grids (DESIGN.md R-F3).  Not
-// used by any solver path; it exists so that the test suite can show why the difference form is used.
-__global__ void __launch_bounds__(kThreads) k_spmv_std32(DiaDev A, const double* __restrict__ x, double* __restrict__ y) {
-  const int64_t n = A.n, nx = A.nx, np = A.nxny;
-  CUTH_TILE_LOOP(n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < n) {
-        double acc = (double)A.f0[i] * x[i];
-        if (i + 1 < n) acc = fma((double)A.f1[i], x[i + 1], acc);
-        if (i >= 1) acc = fma((double)A.f1[i - 1], x[i - 1], acc);
-        if (i + nx < n) acc = fma((double)A.f2[i], x[i + nx], acc);
-        if (i >= nx) acc = fma((double)A.f2[i - nx], x[i - nx], acc);
-        if (i + np < n) acc = fma((double)A.f3[i], x[i + np], acc);
-        if (i >= np) acc = fma((double)A.f3[i - np], x[i - np], acc);
-        y[i] = acc;
-      }
-    }
-  }
+  apply_A<OP>(A, x, [&](int64_t i, double, double yi) { y[i] = yi; });
 }
 
 // Writes the per-call context and clears the control block (plain launch before the graph).
@@ -280,7 +272,7 @@ __global__ void __launch_bounds__(kThreads) k_init(const Ctx* __restrict__ ctxp,
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   double acc[3] = {0.0, 0.0, 0.0};
-  apply_A<false>(c.A, c.x, [&](int64_t i, double, double ax) {
+  apply_A<OP_FP64>(c.A, c.x, [&](int64_t i, double, double ax) {
     const double bi = c.b[i];
     const double ri = bi - ax;
     const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
@@ -315,9 +307,9 @@ __global__ void __launch_bounds__(kThreads) k_pupdate(const Ctx* __restrict__ ct
 }
 
 // Alg. 1 line 6 + the p.mu half of line 7: mu = A p (stage-dependent operator), pAp = p.mu.
-template <bool MIXED>
+template <int OP>
 __device__ __forceinline__ void spmv_dot_body(const Ctx& c, double& acc) {
-  apply_A<MIXED>(c.A, c.p, [&](int64_t i, double pi, double m) {
+  apply_A<OP>(c.A, c.p, [&](int64_t i, double pi, double m) {
     c.mu[i] = m;
     acc = fma(pi, m, acc);
   });
@@ -328,8 +320,9 @@ __global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_dot(const Ctx* __r
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   double acc[1] = {0.0};
-  if (ctl->stage == 0) spmv_dot_body<true>(c, acc[0]);
-  else spmv_dot_body<false>(c, acc[0]);
+  if (ctl->stage != 0) spmv_dot_body<OP_FP64>(c, acc[0]);
+  else if (c.early_op == OP_STD32) spmv_dot_body<OP_STD32>(c, acc[0]);
+  else spmv_dot_body<OP_DIFF32>(c, acc[0]);
   if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
     policy_after_spmv(ctl, acc[0], false);      // Alg. 1 line 7
   }
@@ -375,7 +368,7 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
   __shared__ int s_flag;
   const Ctx c = *ctxp;
   double acc[2] = {0.0, 0.0};
-  apply_A<false>(c.A, c.x, [&](int64_t i, double, double ax) {
+  apply_A<OP_FP64>(c.A, c.x, [&](int64_t i, double, double ax) {
     const double ti = c.b[i] - ax;
     const double di = ti - c.r[i];
     c.mu[i] = ti;
@@ -415,8 +408,9 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
   }
 }
 
-// Measurement hook support: marks the control block as "outside a graph".
-__global__ void k_mark_no_graph(Ctl* ctl) { ctl->no_graph = 1; ctl->restart = 0; }
+// Measurement hook support: marks the control block as "outside a graph"; early = 1 re-arms the early stage
+// (fp32-stored operator) for the replayed kernels.
+__global__ void k_mark_no_graph(Ctl* ctl, int early) { ctl->no_graph = 1; ctl->restart = 0; if (early) ctl->stage = 0; }
 
 // Writes the result record; x := 0 when b = 0.
 __global__ void __launch_bounds__(kThreads) k_finalize(const Ctx* __restrict__ ctxp, Ctl* ctl) {

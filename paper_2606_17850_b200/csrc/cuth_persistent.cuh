@@ -62,13 +62,13 @@ __device__ __forceinline__ void grid_allreduce(cg::grid_group& grid, double (&v)
 #define CUTH_ROWS(i_)                                                                            \
   for (int64_t i_ = (int64_t)blockIdx.x * kThreads + threadIdx.x; i_ < n; i_ += gstride)
 
-template <bool MIXED>
+template <int OP>
 __device__ __forceinline__ double persistent_spmv_phase(const Ctx& c, int64_t n, int64_t gstride) {
   double acc = 0.0;
   CUTH_ROWS2(i0, i1, h1) {
     const double p0 = c.p[i0], p1 = h1 ? c.p[i1] : 0.0;
-    const double m0 = spmv_row<MIXED>(c.A, c.p, i0, p0);
-    const double m1 = h1 ? spmv_row<MIXED>(c.A, c.p, i1, p1) : 0.0;
+    const double m0 = spmv_row<OP>(c.A, c.p, i0, p0);
+    const double m1 = h1 ? spmv_row<OP>(c.A, c.p, i1, p1) : 0.0;
     c.mu[i0] = m0;
     if (h1) c.mu[i1] = m1;
     acc = fma(p0, m0, acc);
@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
     CUTH_ROWS(i) {
       const double xi = c.x[i];
       const double bi = c.b[i];
-      const double ri = bi - spmv_row<false>(c.A, c.x, i, xi);
+      const double ri = bi - spmv_row<OP_FP64>(c.A, c.x, i, xi);
       const double zi = jac ? ri * c.A.dinv[i] : ri;
       c.r[i] = ri;
       c.p[i] = 0.0;
@@ -196,7 +196,9 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
       }
       grid.sync();
       // ---- B: mu = A p, p.mu
-      acc[0] = sc.stage == 0 ? persistent_spmv_phase<true>(c, n, gstride) : persistent_spmv_phase<false>(c, n, gstride);
+      acc[0] = sc.stage != 0 ? persistent_spmv_phase<OP_FP64>(c, n, gstride)
+                             : (c.early_op == OP_STD32 ? persistent_spmv_phase<OP_STD32>(c, n, gstride)
+                                                       : persistent_spmv_phase<OP_DIFF32>(c, n, gstride));
     }
     {
       grid_allreduce<1>(grid, acc, partials, parity, smem);
@@ -239,7 +241,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __res
       // ---- D: true residual (x is complete: the all-reduce above was a grid-wide barrier)
       double acc[2] = {0.0, 0.0};
       CUTH_ROWS(i) {
-        const double ti = c.b[i] - spmv_row<false>(c.A, c.x, i, c.x[i]);
+        const double ti = c.b[i] - spmv_row<OP_FP64>(c.A, c.x, i, c.x[i]);
         const double di = ti - c.r[i];
         c.mu[i] = ti;
         acc[0] = fma(ti, ti, acc[0]); acc[1] = fma(di, di, acc[1]);

@@ -7,17 +7,33 @@
 
 namespace cuth {
 
+// What the matrix object says about itself (header words written by the builder / the importers, device memory):
+// 0 = usable for this call, else the CUTH_SOLVE_* status that ends the solve before it starts.
+__device__ __forceinline__ int matrix_refusal(const Ctx& c) {
+  const unsigned long long* h = c.A.hdr;
+  if (h[kHdrMagic] != kMagic || (int64_t)h[kHdrNx] != c.A.nx || (int64_t)h[kHdrNy] != (int64_t)c.A.ny ||
+      (int64_t)h[kHdrNz] != (int64_t)c.A.nz)
+    return CUTH_SOLVE_BAD_MATRIX;
+  if (c.transient_call && (h[kHdrTransient] == 0ull || h[kHdrImported] != 0ull)) return CUTH_SOLVE_NOT_TRANSIENT;
+  if (c.precision == CUTH_MIXED && h[kHdrMixedOk] == 0ull) return CUTH_SOLVE_FP64_ONLY;
+  return 0;
+}
+
 // After r0 = b - A1 x0: sums rho = r.z, rr = r.r, bb = b.b.  Returns 1 if the loop must run.
 __device__ __forceinline__ unsigned policy_init(Ctl* ctl, const Ctx& c, double rho, double rr, double bb) {
   ctl->rho = rho; ctl->rr = rr; ctl->bb = bb;
   ctl->tol2 = c.rtol * c.rtol * bb;
-  ctl->sw2 = c.rtol * bb;                        // (sqrt(rtol) ||b||)^2, eq. (14a) relative (R-G8)
+  // (sqrt(rtol) ||b||)^2, eq. (14a) relative (R-G8); never below the stopping threshold itself (rtol >= 1), so
+  // that a recursive residual that passes the stopping test always satisfies (14a)
+  ctl->sw2 = fmax(c.rtol, c.rtol * c.rtol) * bb;
   ctl->beta = 0.0; ctl->alpha = 0.0;
   ctl->tt = rr; ctl->tt_prev = rr; ctl->rr_prev_eval = rr;
-  ctl->stage = (c.precision == CUTH_MIXED) ? 0 : 1;
+  ctl->stage = (c.precision == CUTH_MIXED || c.precision == CUTH_MIXED_STD32) ? 0 : 1;
   ctl->beta_zero = 1;                            // Chebyshev path: the first p is z (Alg. 1 line 3)
   unsigned go = 1u;
-  if (bb == 0.0) { ctl->zero_rhs = 1; ctl->status = CUTH_SOLVE_CONVERGED; ctl->tt = 0.0; ctl->rr = 0.0; go = 0u; }
+  const int refusal = matrix_refusal(c);
+  if (refusal) { ctl->status = refusal; ctl->refused = 1; go = 0u; }
+  else if (bb == 0.0) { ctl->zero_rhs = 1; ctl->status = CUTH_SOLVE_CONVERGED; ctl->tt = 0.0; ctl->rr = 0.0; go = 0u; }
   else if (rr <= ctl->tol2) { ctl->status = CUTH_SOLVE_CONVERGED; go = 0u; }          // r0 IS the true residual
   else if (!(rho == rho) || !(rr == rr)) { ctl->status = CUTH_SOLVE_BREAKDOWN; go = 0u; }
   return go;
@@ -67,6 +83,21 @@ __device__ __forceinline__ void policy_after_update(Ctl* ctl, const Ctx& c, doub
   ctl->want_true = (int)want;
 }
 
+// Eq. (14a)-(14c) on SQUARED norms -- the grid-wide sums the kernels produce -- so the printed
+// constants appear squared: 0.9^2 = 0.81, 0.5^2 = 0.25.  Bit 0 = (14a), bit 1 = (14b), bit 2 = (14c).
+//   (14a)  ||r_low||^2 <= rtol ||b||^2                  (relative form of 10^(log10(eps)/2), R-G8; sw2)
+//   (14b)  ||r_true||^2 > 0.81 ||r_true,prev||^2  while  ||r_low||^2 <= 0.81 ||r_low,prev||^2   (successive
+//          evaluations; "despite a decreasing recursive one", R-G9)
+//   (14c)  ||r_true - r_low||^2 >= 0.25 ||r_true||^2     (second print, R-G10)
+__device__ __forceinline__ int switch_criteria(double rr, double tt, double dd, double tt_prev, double rr_prev,
+                                               double sw2) {
+  int mask = 0;
+  if (rr <= sw2) mask |= 1;
+  if (tt > 0.81 * tt_prev && rr <= 0.81 * rr_prev) mask |= 2;
+  if (dd >= 0.25 * tt) mask |= 4;
+  return mask;
+}
+
 // After t = b - A1 x: tt = ||t||^2, dd = ||t - r||^2.  Stopping rule and eq. (14a)-(14c).  Sets
 // ctl->restart (0 none, 1 hard: p = z, 2 soft: p keeps its history).  Returns go.
 __device__ __forceinline__ unsigned policy_after_true(Ctl* ctl, const Ctx& c, double tt, double dd) {
@@ -84,13 +115,12 @@ __device__ __forceinline__ unsigned policy_after_true(Ctl* ctl, const Ctx& c, do
     // restart the direction (same rule as the oracle), keep iterating.
     if (ctl->conv_rec) restart = 1;
   } else {
-    int reason = 0;
-    if (ctl->conv_rec) reason = 4;
-    else if (rr <= ctl->sw2) reason = 1;                                          // (14a)
-    else if (dd >= 0.25 * tt) reason = 3;                                         // (14c): ||t-r|| >= 0.5 ||t||
-    else if (tt > 0.81 * ctl->tt_prev && rr <= 0.81 * ctl->rr_prev_eval) reason = 2;     // (14b), R-G9
-    if (reason) {
-      ctl->stage = 1; ctl->promotions += 1; ctl->switch_reason = reason; ctl->switch_it = ctl->it;
+    // "triggered when any of the following holds"; the reason reported is the first in the
+    // printed order.  A recursive residual that passed the stopping test satisfies (14a) by construction of sw2.
+    const int mask = switch_criteria(rr, tt, dd, ctl->tt_prev, ctl->rr_prev_eval, ctl->sw2);
+    if (mask) {
+      const int reason = (mask & 1) ? 1 : ((mask & 2) ? 2 : 3);
+      ctl->stage = 1; ctl->promotions += 1; ctl->switch_reason = reason; ctl->switch_mask = mask; ctl->switch_it = ctl->it;
       // hot restart.  Small drift: r is recomputed, p keeps its history through its
       // defining equation p = z + beta p ("preserving the established Krylov subspace");
       // large drift ((14c)): the direction is rebuilt from scratch, p = z.
@@ -100,6 +130,8 @@ __device__ __forceinline__ unsigned policy_after_true(Ctl* ctl, const Ctx& c, do
   ctl->tt_prev = tt;
   ctl->rr_prev_eval = rr;
   ctl->restart = restart;
+  if (restart == 1) ctl->hard_restarts += 1;
+  else if (restart == 2) ctl->soft_restarts += 1;
   return go;
 }
 
@@ -126,6 +158,10 @@ __device__ __forceinline__ void write_result(const Ctl* ctl, const Ctx& c) {
   res.rel_resid_rec = bb > 0.0 ? sqrt(ctl->rr / bb) : 0.0;
   res.switch_reason = ctl->switch_reason;
   res.switch_iteration = ctl->switch_it;
+  res.switch_mask = ctl->switch_mask;
+  res.hard_restarts = ctl->hard_restarts;
+  res.soft_restarts = ctl->soft_restarts;
+  res.reserved = 0;
   *c.result = res;
 }
 

@@ -26,6 +26,43 @@ def test_exports_match_header(cu):
     for name in declared:
         assert hasattr(lib, name), name
     assert declared == set(cu.exported_symbols())
+    # SURVEY.md §8(b) "no global state": the library has no process-wide setter; kernel variants are per call
+    assert not [n for n in declared if n.startswith("cuth_set_")]
+    assert "cuth_tuning_t tuning;" in hdr
+
+
+def test_struct_sizes_match_the_header(cu):
+    """The ctypes mirrors of the ABI structs have the sizes the C compiler gives them (a quick layout check:
+    gcc on the header itself)."""
+    import subprocess
+    import tempfile
+    from paper_2606_17850_b200 import binding as B
+    src = '#include <stdio.h>\n#include "cuth.h"\nint main(){printf("%zu %zu %zu %zu %zu\\n", sizeof(cuth_grid_t), ' \
+          'sizeof(cuth_opts_t), sizeof(cuth_result_t), sizeof(cuth_tuning_t), sizeof(cuth_import_report_t));return 0;}\n'
+    with tempfile.TemporaryDirectory() as d:
+        open(os.path.join(d, "t.c"), "w").write(src)
+        subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), os.path.join(d, "t.c"), "-o", os.path.join(d, "t")],
+                       check=True)
+        out = subprocess.run([os.path.join(d, "t")], check=True, capture_output=True, text=True).stdout.split()
+    want = [C.sizeof(B.cuth_grid_t), C.sizeof(B.cuth_opts_t), C.sizeof(B.cuth_result_t), C.sizeof(B.cuth_tuning_t),
+            C.sizeof(B.cuth_import_report_t)]
+    assert [int(v) for v in out] == want
+
+
+def test_bad_tuning_and_precision_values_are_argument_errors(cu):
+    g = cu.Grid(8, 8, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
+    lib = cu.load_library()
+    p = C.c_void_p(4096)
+    for kw in (dict(traversal=3), dict(loop_mode=-1), dict(k1_variant=4), dict(cheb_fusion=4), dict(pair_rows=12),
+               dict(pair_occupancy=1)):
+        o = cu.Opts(tuning=cu.Tuning(**kw))
+        assert lib.cuth_pcg_solve(p, g.ref(), C.byref(o), p, p, p, 1 << 30, p, None) == -3, kw
+        t = cu.Tuning(**kw)
+        assert lib.cuth_spmv_tuned(p, g.ref(), 0, C.byref(t), p, C.c_void_p(8192), None) == -3, kw
+    o = cu.Opts(precision=9)
+    assert lib.cuth_pcg_solve(p, g.ref(), C.byref(o), p, p, p, 1 << 30, p, None) == -3
+    o = cu.Opts(precision=cu.MIXED_STD32, preconditioner=cu.PRECOND_CHEBYSHEV, cheb_lmin=1.0, cheb_lmax=2.0)
+    assert lib.cuth_pcg_solve(p, g.ref(), C.byref(o), p, p, p, 1 << 30, p, None) == -3      # ablation: Jacobi / none only
 
 
 def test_layout_closed_forms_host_side(cu):
@@ -106,25 +143,20 @@ def test_cheb_launch_schedule_host_side(cu):
     big = cu.Grid(1024, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # nx % 4 == 0
     even = cu.Grid(34, 32, 16, 1e-6, 1e-6, dz, None, 1e4)              # even nx, not a multiple of 4: no TMA
     odd = cu.Grid(1023, 1024, 16, 1e-6, 1e-6, dz, None, 1e4)           # odd nx: never pairs
-    mk = lambda prec, k: cu.Opts(prec, 1e-8, 1000, 20, cu.PRECOND_CHEBYSHEV, k, 1e-3, 1.0, cu.CHEB_DEFAULT)
-    try:
-        for k in (3, 4, 5, 30, 31):
-            mids = k - 3
-            plain = (2 + mids // 2 + mids % 2, mids // 2)              # FIRST, pairs, odd MID, LAST
-            fused = (2 + mids // 2, mids // 2 + mids % 2) if mids % 2 else plain   # odd MID + LAST in one launch
-            cu.cuth_set_cheb_fusion(1)
-            assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == (k - 1, 0)
-            for mode in (0, 2):
-                cu.cuth_set_cheb_fusion(mode)
-                assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) in (plain, fused)
-                assert cu.cuth_cheb_launches(even, mk(cu.MIXED, k)) == plain
-                assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k)) == (k - 1, 0)
-                assert cu.cuth_cheb_launches(big, mk(cu.FP64, k)) == (k - 1, 0)          # fp64 apply: single passes
-            cu.cuth_set_cheb_fusion(3)                                 # never the TMA kernel
-            assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k)) == plain
-        assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
-    finally:
-        cu.cuth_set_cheb_fusion(0)
+    mk = lambda prec, k, mode: cu.Opts(prec, 1e-8, 1000, 20, cu.PRECOND_CHEBYSHEV, k, 1e-3, 1.0, cu.CHEB_DEFAULT,
+                                       cu.Tuning(cheb_fusion=mode))
+    for k in (3, 4, 5, 30, 31):
+        mids = k - 3
+        plain = (2 + mids // 2 + mids % 2, mids // 2)              # FIRST, pairs, odd MID, LAST
+        fused = (2 + mids // 2, mids // 2 + mids % 2) if mids % 2 else plain   # odd MID + LAST in one launch
+        assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k, 1)) == (k - 1, 0)
+        for mode in (0, 2):
+            assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k, mode)) in (plain, fused)
+            assert cu.cuth_cheb_launches(even, mk(cu.MIXED, k, mode)) == plain
+            assert cu.cuth_cheb_launches(odd, mk(cu.MIXED, k, mode)) == (k - 1, 0)
+            assert cu.cuth_cheb_launches(big, mk(cu.FP64, k, mode)) == (k - 1, 0)          # fp64 apply: single passes
+        assert cu.cuth_cheb_launches(big, mk(cu.MIXED, k, 3)) == plain                      # never the TMA kernel
+    assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
 
 
 def test_batch_and_import_host_side(cu):

@@ -8,6 +8,7 @@ import pytest
 import workloads as W
 from oracle import oracle as O
 from gpu_util import grid_from_workload, to_dev
+from paper_2606_17850_b200.binding import cuth_result_t
 
 pytestmark = pytest.mark.gpu
 
@@ -201,7 +202,7 @@ def test_batch_and_import_no_out_of_bounds_canaries(kw, nrhs):
 
         carve("rowptr", A.rowptr.nbytes); carve("col", A.col.nbytes); carve("val", A.val.nbytes)
         carve("dia", cu.cuth_dia_bytes(g)); carve("b", B.nbytes); carve("x", B.nbytes)
-        carve("work", cu.cuth_batch_workspace_bytes(g, nrhs)); carve("res", nrhs * 40)
+        carve("work", cu.cuth_batch_workspace_bytes(g, nrhs)); carve("res", nrhs * C.sizeof(cuth_result_t))
         bufs["rowptr"].view(torch.int64).copy_(torch.from_numpy(A.rowptr))
         bufs["col"].view(torch.int32).copy_(torch.from_numpy(A.col))
         bufs["val"].view(torch.float64).copy_(torch.from_numpy(A.val))
@@ -222,4 +223,4 @@ def test_batch_and_import_no_out_of_bounds_canaries(kw, nrhs):
     x0, r0 = run(False)
     x1, r1 = run(True)
     assert np.array_equal(r0, r1) and np.array_equal(x0.view(np.uint64), x1.view(np.uint64))
-    assert all(r0[10 * s] == 0 for s in range(nrhs))
+    assert all(r0[(C.sizeof(cuth_result_t) // 4) * s] == 0 for s in range(nrhs))

@@ -24,15 +24,13 @@ CASES = [
 @pytest.fixture(params=["flat", "flat-pairs", "flat-pairs-ldg", "zmarch", "zmarch-x1"], autouse=True)
 def traversal(request):
     import paper_2606_17850_b200 as cu
-    cu.cuth_set_traversal(1 if request.param.startswith("flat") else 2)
+    cu.set_default_tuning(traversal=1 if request.param.startswith("flat") else 2)
     # "flat", "zmarch-x1" = one pass per kernel; "flat-pairs", "zmarch" = two passes per kernel (operands by TMA
     # when nx % 4 == 0 (fp16: % 8), by ordinary loads otherwise); "flat-pairs-ldg" = two passes, never TMA
-    cu.cuth_set_cheb_fusion({"flat": 1, "flat-pairs": 2, "flat-pairs-ldg": 3, "zmarch": 2, "zmarch-x1": 1}[request.param])
-    cu.cuth_set_k1_variant(1 if request.param == "zmarch-x1" else 2)       # 2: two columns per thread when nx is even
+    cu.set_default_tuning(cheb_fusion={"flat": 1, "flat-pairs": 2, "flat-pairs-ldg": 3, "zmarch": 2, "zmarch-x1": 1}[request.param],
+                          k1_variant=1 if request.param == "zmarch-x1" else 2)   # 2: two columns per thread when nx is even
     yield request.param
-    cu.cuth_set_traversal(0)
-    cu.cuth_set_k1_variant(0)
-    cu.cuth_set_cheb_fusion(0)
+    cu.set_default_tuning(traversal=0, k1_variant=0, cheb_fusion=0)
 
 
 def _rhs(w):
@@ -216,16 +214,12 @@ def test_cheb_apply_kernel_variants_agree(shape, degree, storage, traversal):
                                     storage=cu.CHEB_A3_FP16 if storage == "fp16" else cu.CHEB_DEFAULT)
     r = W.normal01(w.seed, 52, 53, np.arange(w.n)) * 1e-7
     out = {}
-    try:
-        for mode, rows in ((1, 0), (3, 0), (2, 8), (2, 16)):      # rows: region height of the TMA kernel
-            cu.cuth_set_cheb_fusion(mode)
-            cu.cuth_set_pair_rows(rows)
-            z = torch.full((w.n,), float("nan"), dtype=torch.float64, device="cuda")
-            S.cheb_apply(to_dev(r), z)
-            out[(mode, rows)] = z.cpu().numpy()
-    finally:
-        cu.cuth_set_cheb_fusion(1)
-        cu.cuth_set_pair_rows(0)
+    for mode, rows in ((1, 0), (3, 0), (2, 8), (2, 16)):      # rows: region height of the TMA kernel
+        S.opts.tuning.cheb_fusion = mode                       # per-call tuning (cuth_tuning_t)
+        S.opts.tuning.pair_rows = rows
+        z = torch.full((w.n,), float("nan"), dtype=torch.float64, device="cuda")
+        S.cheb_apply(to_dev(r), z)
+        out[(mode, rows)] = z.cpu().numpy()
     ref = out[(1, 0)]
     assert np.isfinite(ref).all()
     scale = np.abs(ref).max()
@@ -259,4 +253,35 @@ def test_graph_cache_follows_plane_shape_and_matrix(traversal):
         xg = x.cpu().numpy()
         rel = np.linalg.norm(w.power - O.spmv(A, xg)) / np.linalg.norm(w.power)
         assert rel <= 1e-8, (nx, ny, nz, rel)
+    cu.cuth_release_workspace(work)
+
+
+@pytest.mark.parametrize("traversal", ["flat-pairs"], indirect=True)
+def test_graph_cache_follows_the_workspace_layout(traversal):
+    """A transient matrix keeps b in the workspace, which moves the Chebyshev buffers N doubles later -- and their
+    addresses are baked into the tensor maps of the cached TMA nodes.  Steady, then transient, then steady again on
+    the SAME workspace and the SAME matrix buffer (same N, same plane): every solve must meet the bar."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    ws = W.make_workload(2, nx=48, ny=40, nz=16, n_hot=8)
+    wt = W.make_workload(5, nx=48, ny=40, nz=16, n_hot=8)
+    gs, gt = grid_from_workload(ws), grid_from_workload(wt)
+    copts = cu.Opts(cu.MIXED, 1e-8, 20000, 5, cu.PRECOND_CHEBYSHEV, 30, 1e-3, 1.0)
+    buf = torch.empty(max(cu.cuth_dia_bytes(gs), cu.cuth_dia_bytes(gt)), dtype=torch.uint8, device="cuda")
+    work = torch.empty(max(cu.cuth_workspace_bytes(gs, copts), cu.cuth_workspace_bytes(gt, copts)), dtype=torch.uint8,
+                       device="cuda")
+    res = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    for w, g in ((ws, gs), (wt, gt), (ws, gs)):
+        cu.cuth_build_dia(g, buf)
+        A = O.assemble_workload(w)
+        b_np = _rhs(w)
+        b = to_dev(b_np)
+        lo, hi, gersh, rlo, rhi = cu.cuth_lanczos_bounds(buf, g, b, 20, work)
+        opts = cu.Opts(cu.MIXED, 1e-8, 20000, 5, cu.PRECOND_CHEBYSHEV, 30, rlo, rhi)
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        cu.cuth_pcg_solve(buf, g, opts, b, x, work, res)
+        torch.cuda.synchronize()
+        assert int(res[:4].view(torch.int32).item()) == 0, w.name
+        rel = np.linalg.norm(b_np - O.spmv(A, x.cpu().numpy())) / np.linalg.norm(b_np)
+        assert rel <= 1e-8, (w.name, rel)
     cu.cuth_release_workspace(work)

@@ -138,7 +138,9 @@ def test_validation_counts_match_the_oracle():
 
 def test_non_layered_row_sums_are_fp64_only():
     """A diagonal shift that varies from cell to cell keeps A SPD but leaves no per-layer row sum: the import
-    succeeds, MIXED is refused on the host, and the FP64 solve matches the oracle on the same matrix."""
+    succeeds, MIXED is refused ON THE DEVICE (the object's own header says so: status CUTH_SOLVE_FP64_ONLY, x untouched
+    -- also for a byte copy of the object at another address, which a host-side table keyed by address would miss), and the
+    FP64 solve matches the oracle on the same matrix."""
     import torch
     import paper_2606_17850_b200 as cu
     w = W.make_workload(cfg=3, nx=20, ny=14, nz=6, n_hot=3)
@@ -156,11 +158,21 @@ def test_non_layered_row_sums_are_fp64_only():
     assert M.import_report.max_rowsum_dev == pytest.approx(want["max_rowsum_dev"], rel=1e-6)
     x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
     S = cu.Solver(M, cu.Opts(precision=cu.MIXED))
-    with pytest.raises(cu.CuthError) as e:
-        S.solve(to_dev(w.power), x)
-    assert e.value.code == -9
-    with pytest.raises(cu.CuthError):
-        M.spmv(to_dev(w.power), cu.MIXED)
+    x.fill_(3.25)
+    S.solve(to_dev(w.power), x)
+    r = S.result()
+    assert r.status == cu.SOLVE_FP64_ONLY and r.iterations == 0 and bool((x == 3.25).all())
+    buf2 = M.buf.clone()                                   # the same object at another address
+    res2 = torch.zeros(64, dtype=torch.uint8, device="cuda")
+    cu.cuth_pcg_solve(buf2, g, S.opts, to_dev(w.power), x, S.work, res2)
+    torch.cuda.synchronize()
+    assert int(res2[:4].view(torch.int32).item()) == cu.SOLVE_FP64_ONLY and bool((x == 3.25).all())
+    SB = cu.BatchSolver(M, 2, cu.Opts(precision=cu.MIXED))
+    xb = torch.full((2, w.n), 3.25, dtype=torch.float64, device="cuda")
+    SB.solve(torch.stack([to_dev(w.power)] * 2), xb)
+    assert [q.status for q in SB.results()] == [cu.SOLVE_FP64_ONLY] * 2 and bool((xb == 3.25).all())
+    assert not np.isfinite(M.spmv(to_dev(w.power), cu.MIXED).cpu().numpy()).any()   # s(z) = NaN: fails loudly
+    x.zero_()
     S = cu.Solver(M, cu.Opts(precision=cu.FP64))
     S.solve(to_dev(w.power), x)
     assert S.result().status == 0
@@ -202,10 +214,10 @@ def test_import_argument_errors():
     gt = grid_from_workload(wt)
     M = cu.DiaMatrix(gt, csr=_csr_dev(O.assemble_workload(wt)))
     S = cu.Solver(M, cu.Opts())
-    T = torch.zeros(wt.n, dtype=torch.float64, device="cuda")
-    with pytest.raises(cu.CuthError) as e:
-        S.step(to_dev(wt.power), T)
-    assert e.value.code == -7
+    T = torch.full((wt.n,), 1.5, dtype=torch.float64, device="cuda")
+    S.step(to_dev(wt.power), T)
+    r = S.result()
+    assert r.status == cu.SOLVE_NOT_TRANSIENT and r.iterations == 0 and bool((T == 1.5).all())
 
 
 def _coo_dev(A, seed=None):
