@@ -90,11 +90,17 @@ typedef struct {
   int32_t traversal;          /* how the kernels that apply A walk the grid: 0 automatic (z-marching when one x-y plane
                                  of the six streamed arrays no longer fits L2 -- nx*ny >= 2^18 -- or from 2^17 columns
                                  on grids of more than 2^21 rows; flat 1-D streaming otherwise), 1 flat, 2 z-marching */
-  int32_t loop_mode;          /* where the PCG loop lives: 0 automatic (one persistent cooperative kernel up to 2^22
-                                 rows, the CUDA graph with conditional nodes beyond), 1 graph, 2 persistent kernel
-                                 wherever the flat traversal applies */
-  int32_t k1_variant;         /* z-marching kernels: 0 automatic, 1 one column per thread, 2 two x-adjacent columns per
-                                 thread (nx even), 3 = 2 without the TMA-staged K1 */
+  int32_t loop_mode;          /* where the PCG loop lives: 0 automatic (one persistent cooperative kernel up to 2^21
+                                 rows -- up to 2^22 where the TMA-staged K1 is not available --, the CUDA graph with
+                                 conditional nodes beyond; grids whose rows fit the shared memory of one 8-CTA
+                                 thread-block cluster -- about 13 k rows, BASELINE cfg 1 -- run as ONE cluster-resident
+                                 kernel, Jacobi / no preconditioner), 1 graph, 2 persistent kernel wherever the flat
+                                 traversal applies, 3 cluster-resident kernel (CUTH_ERR_VALUE when the grid does not fit) */
+  int32_t k1_variant;         /* z-marching kernels: 0 automatic (K1 with TMA-staged operands when nx % 4 == 0 and the
+                                 plane has >= 288 tiles of 64 x 8 columns; else two x-adjacent columns per thread when nx
+                                 is even and there are >= 2048 tiles; else one column), 1 one column per thread,
+                                 2 two columns per thread (nx even), K1 TMA-staged whenever nx % 4 == 0,
+                                 3 = 2 with ordinary loads everywhere */
   int32_t cheb_fusion;        /* Chebyshev passes per kernel (fp32 modes, nx even): 0 automatic = 2 = two passes, TMA
                                  operands when nx % 4 == 0 (A3: % 8); 1 one pass per kernel; 3 two passes, never TMA */
   int32_t pair_rows;          /* rows of a region of the TMA two-pass Chebyshev kernel: 0 automatic, 8, 16 */

@@ -20,6 +20,8 @@
 #include "cuth_cheb_pair_tma.cuh"
 #include "cuth_fused_tma.cuh"
 #include "cuth_persistent.cuh"
+#include "cuth_fixed32.cuh"
+#include "cuth_cluster.cuh"
 #include "cuth_batch.cuh"
 
 namespace cuth {
@@ -45,7 +47,7 @@ static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 // Kernel variants of one call (cuth_tuning_t, validated): nothing here is process-wide.
 struct Tune {
   int traversal = 0;    // 0 auto, 1 flat, 2 z-march
-  int loop_mode = 0;    // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel
+  int loop_mode = 0;    // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel, 3 cluster-resident kernel
   int k1_variant = 0;   // 0 auto, 1 one column per thread, 2 two columns, 3 two columns without the TMA-staged K1
   int cheb_pairs = 0;   // 0 auto, 1 never, 2 always (fp32 modes)
   int pair_tma = 0;     // 0 auto (TMA when possible), 1 never
@@ -55,7 +57,7 @@ struct Tune {
 static int make_tune(const cuth_tuning_t* t, Tune* T) {
   *T = Tune();
   if (!t) return CUTH_OK;
-  if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 2 || t->k1_variant < 0 ||
+  if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 3 || t->k1_variant < 0 ||
       t->k1_variant > 3 || t->cheb_fusion < 0 || t->cheb_fusion > 3 ||
       (t->pair_rows != 0 && t->pair_rows != 8 && t->pair_rows != 16) ||
       (t->pair_occupancy != 0 && (t->pair_occupancy < 2 || t->pair_occupancy > 4)) || t->reserved[0] || t->reserved[1])
@@ -321,9 +323,16 @@ static unsigned k1_tma_dyn_smem() {
 }
 // K1 takes its operands through TMA when it runs two columns per thread (nx even, enough tiles), nx % 4 == 0 (strides of
 // the fp32 tensors), z is r (no Chebyshev), the driver can encode tensor maps, and the variant is not forced away.
+// Automatic: from one wave of 64 x 8 tiles on (2 CTAs/SM x 148 SMs = 296; the kernel is persistent over tiles and
+// keeps its TMA ring running across them, so it does not need the >= 2048 tiles of the LDG two-column kernel).
+// Measured per iteration, graph loop, MIXED, TMA K1 / one-column LDG K1: 512x512x16 84.3 / 108.3 us, 768x768x8
+// 92.1 / 119.7, 640x640x10 83.0 / 107.5, 384x384x32 91.2 / 112.0, but 256x256x64 (128 tiles) 104.8 / 155.4 with the
+// persistent kernel at 101.1 (profiles/r2_loop_homes.md).
 static bool fused_tma(const DiaLayout& L, const Tune& T, bool cheb) {
   if (cheb || T.k1_variant == 1 || T.k1_variant == 3) return false;
-  return fused_x2(L, T) && (L.nx % 4) == 0 && encode_tiled_fn() != nullptr;
+  if ((L.nx % 4) != 0 || encode_tiled_fn() == nullptr) return false;
+  if (T.k1_variant == 2) return true;
+  return ((L.nx + K1X - 1) / K1X) * ((L.ny + K1Y - 1) / K1Y) >= 288;
 }
 // persistent over tiles: as many CTAs as are resident (2 per SM), never more than tiles
 static int fused_tma_blocks(const DiaLayout& L);
@@ -388,6 +397,7 @@ struct Plan {
   int with_b = 0;        // transient matrix: b lives in the workspace, the Chebyshev buffers sit N doubles later
   int pair_tma = 0;      // the two-pass Chebyshev nodes are the TMA kernel
   int k1tma = 0;         // K1 is the TMA-staged kernel
+  int unroll = 1;        // K1 + K2 pairs per pass of the WHILE body (fused path without Chebyshev)
   const void* dia = nullptr;   // matrix the tensor maps of the TMA nodes were made for (else nullptr)
   int64_t tnx = 0, tny = 0;    // ... and its plane dimensions
   int tocc = 0;                // ... occupancy * 100 + region rows of the TMA two-pass nodes
@@ -395,7 +405,7 @@ struct Plan {
   bool operator==(const Plan& o) const {
     return n == o.n && sblocks == o.sblocks && fblocks == o.fblocks && k1x2 == o.k1x2 && chebkey == o.chebkey &&
            cblocks == o.cblocks && x2blocks == o.x2blocks && pblocks == o.pblocks && with_b == o.with_b &&
-           pair_tma == o.pair_tma && k1tma == o.k1tma && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
+           pair_tma == o.pair_tma && k1tma == o.k1tma && unroll == o.unroll && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
   }
 };
 struct GraphEntry {
@@ -480,18 +490,26 @@ static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, co
   const cudaGraphNode_t* dep0 = n_c ? &n_c : nullptr;
   const size_t ndep0 = n_c ? 1 : 0;
   if (P.fblocks > 0) {
-    if (P.k1tma) {
-      K1Maps km, km64;
-      if (!make_k1_maps(&km, &km64, L, P.dia, w)) return CUTH_ERR_CUDA;
-      void* a[] = {&ctx, &ctl, &partials, &km.z, &km.p, &km.p2, &km.d, &km64.d, &km.m1, &km.m2, &km.m3,
-                   &km64.m1, &km64.m2, &km64.m3};                      // the maps are copied into the node
-      CU(add_kernel(body, &n_s, dep0, ndep0, (void*)k_fused_pspmv_tma, P.fblocks, a, k1_tma_dyn_smem()));
-    } else {
-      void* a[] = {&ctx, &ctl, &partials};
-      CU(add_kernel(body, &n_s, dep0, ndep0, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
+    // A pass of the WHILE node costs ~9 us of scheduling, so the body holds P.unroll iterations; once
+    // K2's epilogue decides that the loop must stop or that the true-residual branch must run (ctl->halt), the
+    // remaining K1 / K2 launches of the pass return at once and the IF node at the end of the body takes over.
+    K1Maps km, km64;
+    if (P.k1tma && !make_k1_maps(&km, &km64, L, P.dia, w)) return CUTH_ERR_CUDA;
+    const unsigned k1_smem = P.k1tma ? k1_tma_dyn_smem() : 0u;
+    for (int u = 0; u < P.unroll; ++u) {
+      const cudaGraphNode_t* dep = u == 0 ? dep0 : &n_u;
+      const size_t ndep = u == 0 ? ndep0 : 1;
+      if (P.k1tma) {
+        void* a[] = {&ctx, &ctl, &partials, &km.z, &km.p, &km.p2, &km.d, &km64.d, &km.m1, &km.m2, &km.m3,
+                     &km64.m1, &km64.m2, &km64.m3};                    // the maps are copied into the node
+        CU(add_kernel(body, &n_s, dep, ndep, (void*)k_fused_pspmv_tma, P.fblocks, a, k1_smem));
+      } else {
+        void* a[] = {&ctx, &ctl, &partials};
+        CU(add_kernel(body, &n_s, dep, ndep, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
+      }
+      void* a2[] = {&ctx, &ctl, &partials, &h_while, &h_if};
+      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a2));
     }
-    { void* a[] = {&ctx, &ctl, &partials, &h_while, &h_if};
-      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a)); }
   } else {
     { void* a[] = {&ctx, &ctl};
       CU(add_kernel(body, &n_p, dep0, ndep0, (void*)k_pupdate, blocks, a)); }
@@ -546,8 +564,11 @@ static int get_graph(const Workspace& w, void* work_D, const Plan& P, const DiaL
 static int check_opts(const cuth_opts_t* o) {
   if (!o) return CUTH_ERR_NULL;
   if (!(o->rtol > 0.0) || o->max_iters <= 0) return CUTH_ERR_VALUE;
-  if (o->precision != CUTH_FP64 && o->precision != CUTH_MIXED && o->precision != CUTH_MIXED_STD32) return CUTH_ERR_VALUE;
-  if (o->precision == CUTH_MIXED_STD32 && o->preconditioner == CUTH_PRECOND_CHEBYSHEV) return CUTH_ERR_VALUE;   // ablation: Alg. 1 with M = D0 or I
+  if (o->precision != CUTH_FP64 && o->precision != CUTH_MIXED && o->precision != CUTH_MIXED_STD32 &&
+      o->precision != CUTH_FIXED32)
+    return CUTH_ERR_VALUE;
+  if ((o->precision == CUTH_MIXED_STD32 || o->precision == CUTH_FIXED32) && o->preconditioner == CUTH_PRECOND_CHEBYSHEV)
+    return CUTH_ERR_VALUE;                               // ablations: Alg. 1 with M = D0 or I
   Tune T;
   if (make_tune(&o->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
   if (o->preconditioner != CUTH_PRECOND_NONE && o->preconditioner != CUTH_PRECOND_JACOBI &&
@@ -617,19 +638,36 @@ static int persistent_blocks(int64_t n) {
   return want < all ? want : all;
 }
 
+// The cluster-resident kernel (cuth_cluster.cuh): every row lives in the shared memory of one 8-CTA cluster.
+// Measured on B200 (profiles/r2_loop_homes.md): cfg 1 (8 192 rows) per iteration, cluster / persistent kernel / graph.
+static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune& T) {
+  if (T.loop_mode == 1 || T.loop_mode == 2 || T.traversal == 2) return false;
+  if (opts->preconditioner == CUTH_PRECOND_CHEBYSHEV) return false;
+  if (opts->precision != CUTH_FP64 && opts->precision != CUTH_MIXED) return false;
+  return cluster_fits(L.nx, L.ny, L.nz, kClusterMaxCtas);
+}
+
 static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
   const int mode = T.loop_mode, trav = T.traversal;
-  if (cheb || mode == 1 || trav == 2) return false;
+  if (cheb || mode == 1 || mode == 3 || trav == 2) return false;
   if (persistent_blocks(L.n) <= 0) return false;
   if (mode == 2) return !use_zmarch(L, T);        // forced: wherever the flat traversal applies
   // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
   // 7.0 / 18.7 us at cfg 1 (8 k rows), 19.3 / 30.4 us at cfg 6 (655 k), 23.2 / 34.7 us at cfg 2 (1 M); and on wide
   // planes, against the z-marching graph: 512x512x4 23.2 / 36.1, 512x512x8 47.7 / 60.3, 1024x1024x2 47.0 / 66.1,
   // 512x512x16 (4 M rows, cfg 5) 101.0 / 99.5 in FP64 but 103.9 / 112.6 in MIXED with T = 5 (the true-residual branch
-  // is three more kernels and an IF node in the graph, one more phase in the kernel).  Auto: the persistent kernel
-  // (its row access is flat whatever the plane shape) for every grid of up to 2^22 rows; beyond, the graph.
-  return L.n <= (1 << 22);
+  // is three more kernels and an IF node in the graph, one more phase in the kernel).
+  // Round 2, graph with the TMA-staged K1 and four iterations per WHILE pass / persistent kernel: 512x512x8 (2 M rows)
+  // 48.2 / 47.9 us (MIXED), 1024x1024x2 53.2 / 47.0, but from 4 M rows on 512x512x16 (cfg 5) 84.3 / 101.8, 1024x512x8
+  // 86.3 / 101.2, 640x640x10 83.0 / 99.5, 768x768x8 92.1 / 113.7 (profiles/r2_loop_homes.md).
+  // Auto: the persistent kernel (its row access is flat whatever the plane shape) up to 2^21 rows, and up to 2^22
+  // rows where the TMA-staged K1 is not available; the graph everywhere else.
+  if (L.n > (1 << 22)) return false;
+  if (L.n <= (1 << 21)) return true;
+  return !(use_zmarch(L, T) && fused_tma(L, T, false));
 }
+
+constexpr int kGraphUnroll = 4;   // iterations per pass of the WHILE body on the fused path
 
 // The graph of a solve with these options on this grid.
 static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts, bool with_b, const void* dia_D) {
@@ -651,6 +689,7 @@ static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts
   P.x2blocks = cheb_x2(L, T) ? cheb_x2_blocks(L) : 0;
   P.pblocks = (cheb && cheb_pairs(L, code, T)) ? cheb_pair_blocks(L) : 0;
   P.with_b = with_b ? 1 : 0;
+  P.unroll = (P.fblocks > 0 && !cheb) ? kGraphUnroll : 1;
   if (cheb && cheb_pairs_tma(L, code, T)) {
     P.pair_tma = 1;
     P.dia = dia_D; P.tnx = L.nx; P.tny = L.ny;
@@ -681,6 +720,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   Tune T;
   make_tune(&opts->tuning, &T);
   if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;    // the ablation operator exists in the flat kernels only
+  if (opts->precision == CUTH_FIXED32) T.traversal = 1;
   Workspace w = carve_workspace(work_D, L.n, with_b, cheb);
   DiaDev A = dev_view(dia_D, L, T);
   const int blocks = grid_blocks(L.n);
@@ -710,6 +750,48 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   k_set_ctx<<<1, 32, 0, st>>>(c, w.ctx, w.ctl);
   CU(cudaGetLastError());
   { std::lock_guard<std::mutex> lk(g_mu); g_last_dia[work_D] = dia_D; }
+  if (opts->precision == CUTH_FIXED32) {       // ablation: the paper's fixed-FP32 solver, one cooperative kernel
+    const int nb = coresident_blocks(3, (const void*)k_pcg_fixed32, 4, kPersistMaxBlocks);
+    if (nb <= 0) { g_last_err = "CUTH_FIXED32: cooperative launch unavailable"; return CUTH_ERR_CUDA; }
+    Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
+    void* args[] = {&ctxp, &ctlp, &part};
+    CU(cudaLaunchCooperativeKernel((void*)k_pcg_fixed32, dim3(nb), dim3(kThreads), args, 0, st));
+    return CUTH_OK;
+  }
+  if (use_cluster(L, opts, T)) {
+    // 8 CTAs when the rows fit them, else 16 (non-portable cluster size): measured at cfg 1 (8 192 rows) 4.41 us per
+    // iteration with 8 CTAs against 4.88 with 16 -- the all-reduce across CTAs costs more than the halved row work saves
+    cudaError_t e = cudaErrorInvalidValue;
+    for (int nc = 8; nc <= kClusterMaxCtas && e != cudaSuccess; nc *= 2) {
+      if (!cluster_fits(L.nx, L.ny, L.nz, nc)) continue;
+      const void* fn = nc == 16 ? (const void*)k_pcg_cluster<16> : (const void*)k_pcg_cluster<8>;
+      const int rows = (int)cluster_rows_per_cta(L.nx, L.ny, L.nz, nc);
+      const size_t smem = cluster_smem_bytes(rows);
+      if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+          (nc > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+        cudaGetLastError();
+        continue;
+      }
+      cudaLaunchConfig_t cfg;
+      memset(&cfg, 0, sizeof cfg);
+      cfg.gridDim = dim3(nc); cfg.blockDim = dim3(kClusterThreads);
+      cfg.dynamicSmemBytes = smem; cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      const Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl;
+      void* args[] = {(void*)&ctxp, (void*)&ctlp, (void*)&rows};
+      e = cudaLaunchKernelExC(&cfg, fn, args);
+      if (e != cudaSuccess) cudaGetLastError();
+    }
+    if (e == cudaSuccess) return CUTH_OK;
+    if (T.loop_mode == 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster)");
+    // automatic mode: fall through to the persistent kernel / the graph
+  } else if (T.loop_mode == 3) {
+    g_last_err = "loop_mode 3: the grid does not fit one cluster, or the options are not served by the cluster kernel";
+    return CUTH_ERR_VALUE;
+  }
   if (use_persistent(L, cheb, T)) {
     Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
     void* args[] = {&ctxp, &ctlp, &part};
@@ -1062,6 +1144,7 @@ int cuth_cheb_apply(const void* dia_D, const cuth_grid_t* grid, const cuth_opts_
   rc = check_opts(opts);
   if (rc) return rc;
   if (opts->preconditioner != CUTH_PRECOND_CHEBYSHEV) return CUTH_ERR_VALUE;
+  if (opts->precision != CUTH_FP64 && opts->precision != CUTH_MIXED) return CUTH_ERR_VALUE;
   if (!dia_D || !r_D || !z_D || !work_D) return CUTH_ERR_NULL;
   if (!aligned16(dia_D) || !aligned16(r_D) || !aligned16(z_D) || !aligned16(work_D)) return CUTH_ERR_ALIGN;
   if (work_bytes < cuth_workspace_bytes(grid, opts)) return CUTH_ERR_SIZE;
@@ -1157,6 +1240,7 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts
   Tune T;
   if (!make_layout(grid, &L) || !opts || make_tune(&opts->tuning, &T) != CUTH_OK) return 0;
   if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
+  if (use_cluster(L, opts, T)) return 0;                                                   // one cluster-resident kernel
   if (use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T)) return 0;      // one persistent kernel for the whole solve
   return use_zmarch(L, T) ? 2 : 3;
 }

@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(kThreads, 4) k_fused_pspmv(const Ctx* __restri
   __shared__ double sp[2][FTY + 2][FTX + 2];
   __shared__ double smem[32];
   __shared__ int s_flag;
+  if (ctl->halt) return;                     // unrolled graph body: this pass is over
   const Ctx c = *ctxp;
   const int pcur = ctl->pcur;
   const double* p_in = pcur ? c.p2 : c.p;

@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_fused_pspmv_tma(
     const __grid_constant__ CUtensorMap tmF3, const __grid_constant__ CUtensorMap tmE1,
     const __grid_constant__ CUtensorMap tmE2, const __grid_constant__ CUtensorMap tmE3) {
   extern __shared__ __align__(128) unsigned char k1_smem_raw[];
+  if (ctl->halt) return;                     // unrolled graph body: this pass is over
   const Ctx c = *ctxp;
   const int pcur = ctl->pcur;
   double* p_out = pcur ? c.p : c.p2;

@@ -168,6 +168,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_fused_pspmv_x2(const Ctx* __res
   __shared__ __align__(16) double sp[2][XTY + 2][XS];
   __shared__ double smem[32];
   __shared__ int s_flag;
+  if (ctl->halt) return;                     // unrolled graph body: this pass is over
   const Ctx c = *ctxp;
   const int pcur = ctl->pcur;
   const double* p_in = pcur ? c.p2 : c.p;

@@ -116,7 +116,9 @@ struct Ctl {
   double xalpha;   // pending x += xalpha * p (fused path defers Alg. 1 line 8 by one kernel)
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
   int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, beta_zero, switch_mask;
-  int32_t hard_restarts, soft_restarts, refused, pad4;
+  int32_t hard_restarts, soft_restarts, refused;
+  int32_t halt;    // graph loop with an unrolled body: the remaining K1 / K2 launches of this pass are no-ops
+                   // (the loop must stop, or the true-residual branch at the end of the body must run first)
   unsigned int ticket[8];
 };
 

@@ -81,6 +81,7 @@ __device__ __forceinline__ void policy_after_update(Ctl* ctl, const Ctx& c, doub
     else if (conv_rec || c14a || periodic || capped) want = 1u;
   }
   ctl->want_true = (int)want;
+  ctl->halt = ((!go || want) && !ctl->no_graph) ? 1 : 0;      // replays outside the graph never halt
 }
 
 // Eq. (14a)-(14c) on SQUARED norms -- the grid-wide sums the kernels produce -- so the printed
@@ -132,6 +133,7 @@ __device__ __forceinline__ unsigned policy_after_true(Ctl* ctl, const Ctx& c, do
   ctl->restart = restart;
   if (restart == 1) ctl->hard_restarts += 1;
   else if (restart == 2) ctl->soft_restarts += 1;
+  ctl->halt = go ? 0 : 1;
   return go;
 }
 

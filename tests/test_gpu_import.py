@@ -70,11 +70,18 @@ def test_import_is_bit_exact(kw, given_rowsums):
     e, n = int(ptr[4]), w.n
     o_h16 = al(al(al(lay_end + 8 * e) + 4 * e) + 8 * n)      # after A1, A2, 1/D0
     o_f32a = o_h16 + 3 * al(2 * n)
-    for k in range(3):                                       # A3 (fp16, scaled) and the aligned per-diagonal copies of A2
-        a, b = o_h16 + k * al(2 * n), o_f32a + k * al(4 * n)
+    o_f64a = o_f32a + 3 * al(4 * n)
+    for k in range(3):                          # A3 (fp16, scaled) and the aligned per-diagonal copies of A2 and of A1
+        a, b, c = o_h16 + k * al(2 * n), o_f32a + k * al(4 * n), o_f64a + k * al(8 * n)
         assert bool((M.buf[a:a + 2 * n] == B.buf[a:a + 2 * n]).all())
         assert bool((M.buf[b:b + 4 * n] == B.buf[b:b + 4 * n]).all())
-    assert o_f32a + 3 * al(4 * n) == M.buf.numel()
+        assert bool((M.buf[c:c + 8 * n] == B.buf[c:c + 8 * n]).all())
+        # the aligned fp64 copy of diagonal k+1 is the packed diagonal followed by a zero tail
+        dk = M.buf[c:c + 8 * n].view(np_to_torch_f64()).cpu().numpy()
+        lk = int(ptr[k + 2] - ptr[k + 1])
+        assert np.array_equal(dk[:lk].view(np.uint64), vals_o[int(ptr[k + 1]):int(ptr[k + 2])].view(np.uint64))
+        assert not dk[lk:].any()
+    assert o_f64a + 3 * al(8 * n) == M.buf.numel()
     sc = slice(512 + 32 * w.nz, 512 + 32 * w.nz + 24)        # |entry|max bits, fp16 scale, 1/scale
     assert bool((M.buf[sc] == B.buf[sc]).all())
     s_imp = M.buf[512 + 8 * w.nz: 512 + 16 * w.nz].view(np_to_torch_f64()).cpu().numpy()

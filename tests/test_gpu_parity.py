@@ -14,16 +14,19 @@ from gpu_util import grid_from_workload, to_dev, gpu_solve
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(params=["flat-graph", "flat-persistent", "zmarch", "zmarch-k1x1", "zmarch-k1ldg"], autouse=True)
+@pytest.fixture(params=["auto", "flat-graph", "flat-persistent", "zmarch", "zmarch-k1x1", "zmarch-k1ldg"], autouse=True)
 def traversal(request):
     """Every parity case runs with both grid traversals of the kernels that apply A, and on the flat
     traversal with both homes of the loop (CUDA graph with conditional nodes / one persistent kernel).  z-marching:
     "zmarch" = two columns per thread with the TMA-staged K1 wherever nx % 4 == 0, "zmarch-k1ldg" = two columns per
     thread with ordinary loads everywhere, "zmarch-k1x1" = one column per thread."""
     import paper_2606_17850_b200 as cu
-    cu.set_default_tuning(traversal=2 if request.param.startswith("zmarch") else 1,
-                          k1_variant={"zmarch-k1x1": 1, "zmarch-k1ldg": 3}.get(request.param, 2),
-                          loop_mode=1 if request.param == "flat-graph" else 2)
+    if request.param == "auto":      # everything automatic: grids of up to ~13 k rows run in the cluster-resident kernel
+        cu.set_default_tuning(traversal=0, k1_variant=0, loop_mode=0)
+    else:
+        cu.set_default_tuning(traversal=2 if request.param.startswith("zmarch") else 1,
+                              k1_variant={"zmarch-k1x1": 1, "zmarch-k1ldg": 3}.get(request.param, 2),
+                              loop_mode=1 if request.param == "flat-graph" else 2)
     yield request.param
     cu.set_default_tuning(traversal=0, loop_mode=0, k1_variant=0)
 
@@ -296,6 +299,42 @@ def test_solver_reuse_and_determinism():
         xs.append((x.cpu().numpy(), r.iterations))
     assert xs[0][1] == xs[1][1] == xs[2][1]
     assert np.array_equal(xs[0][0], xs[1][0]) and np.array_equal(xs[0][0], xs[2][0])   # fixed-order sums
+
+
+@pytest.mark.parametrize("traversal", ["flat-graph"], indirect=True)    # the test sets both tunings itself: once
+def test_two_solvers_with_different_tunings_run_concurrently(traversal):
+    """SURVEY.md §8(b) "no global state": one matrix object shared by two solves with DIFFERENT kernel variants (flat
+    persistent kernel / z-marching graph with the TMA-staged K1), enqueued alternately on two streams with their own
+    workspaces, give bit-identical results to the same solves run one after the other."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(3, nx=128, ny=48, nz=8, n_hot=6)
+    M = cu.DiaMatrix(grid_from_workload(w))
+    b = to_dev(w.power)
+    tunings = [cu.Tuning(traversal=1, loop_mode=2), cu.Tuning(traversal=2, loop_mode=1, k1_variant=2)]
+    solvers = [cu.Solver(M, cu.Opts(precision=cu.MIXED, rtol=1e-8, tuning=t)) for t in tunings]
+
+    def run(streams):
+        xs = [torch.zeros(w.n, dtype=torch.float64, device="cuda") for _ in solvers]
+        for rep in range(3):
+            for S, x, st in zip(solvers, xs, streams):
+                with torch.cuda.stream(st):
+                    x.zero_()
+                    S.solve(b, x)
+        torch.cuda.synchronize()
+        return [x.cpu().numpy() for x in xs], [S.result() for S in solvers]
+
+    cur = torch.cuda.current_stream()
+    serial_x, serial_r = run([cur, cur])
+    torch.cuda.synchronize()
+    par_x, par_r = run([torch.cuda.Stream(), torch.cuda.Stream()])
+    for k in range(2):
+        assert serial_r[k].status == 0 and par_r[k].status == 0
+        assert serial_r[k].iterations == par_r[k].iterations
+        assert np.array_equal(serial_x[k].view(np.uint64), par_x[k].view(np.uint64))
+    assert np.abs(serial_x[0] - serial_x[1]).max() <= 1e-6 * np.abs(serial_x[0]).max()
+    for S in solvers:
+        S.close()
 
 
 # ---------------------------------------------------------------- a6: transient

@@ -6,7 +6,7 @@
   * whole solves in which (14a)+soft restart, (14c)+hard, (14b)+hard, (14b)+soft, (14a)+(14c) together, and the
     late-stage hard restart are each the expected outcome, with the switch iteration derived by tests/policy_scan.py
     from a plain PCG history (no policy code); run in every home of the loop that has the operator: CUDA graph (flat
-    and z-marching / fused), persistent kernel, batched kernel.
+    and z-marching / fused), persistent kernel, cluster-resident kernel, batched kernel.
 Mutation check (done by hand on the device code, 2026-11): 0.25 -> 0.49 in switch_criteria (14c), 0.81 -> 0.9025 in
 (14b), sw2 = rtol -> rtol^(2/3), soft_drift2 1e-2 -> 0.49, or testing (14c) before (14b) when forming `reason`, each
 fail test_device_policy_truth_table and at least one scenario test."""
@@ -21,7 +21,7 @@ from policy_scan import expected_switch
 
 pytestmark = pytest.mark.gpu
 
-HOMES = ["flat-graph", "persistent", "zmarch-graph", "zmarch-k1x1", "batch"]
+HOMES = ["flat-graph", "persistent", "cluster", "zmarch-graph", "zmarch-k1x1", "batch"]
 
 
 def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
@@ -29,6 +29,7 @@ def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
     import torch
     import paper_2606_17850_b200 as cu
     tune = {"flat-graph": cu.Tuning(traversal=1, loop_mode=1), "persistent": cu.Tuning(traversal=1, loop_mode=2),
+            "cluster": cu.Tuning(loop_mode=3),
             "zmarch-graph": cu.Tuning(traversal=2, k1_variant=2), "zmarch-k1x1": cu.Tuning(traversal=2, k1_variant=1),
             "batch": cu.Tuning()}[home]
     opts = cu.Opts(precision=precision, rtol=rtol, max_iters=max_iters, true_resid_period=period, tuning=tune)
