@@ -317,6 +317,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6])
+    ap.add_argument("--grid", type=int, nargs=3, default=None, metavar=("NX", "NY", "NZ"),
+                    help="the recipe of --config on another grid (for studying the automatic kernel choices)")
     ap.add_argument("--precision", default=None, choices=["fp64", "mixed"])
     ap.add_argument("--impl", default="cuth", choices=["cuth", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -375,7 +377,8 @@ def main():
     cu.set_default_tuning(traversal=args.traversal, loop_mode=args.loop_mode, cheb_fusion=args.cheb_fusion,
                           k1_variant=args.k1_variant,
                           pair_occupancy=args.pair_occupancy, pair_rows=args.pair_rows)
-    w = W.make_workload(args.config)
+    w = W.make_workload(args.config) if args.grid is None else \
+        W.make_workload(args.config, nx=args.grid[0], ny=args.grid[1], nz=args.grid[2], n_hot=16)
     mixed = w.mixed if args.precision is None else (args.precision == "mixed")
     prec = cu.MIXED if mixed else cu.FP64
     kap = w.kappa_cell if w.kappa_cell is not None else w.kappa_layer
@@ -624,7 +627,9 @@ def main():
                                        "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+88 fp32-stored per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
-        "loop": "persistent cooperative kernel" if persistent else "cuda graph (conditional WHILE/IF nodes)",
+        "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % (4 if fused and not cheb else 1),
+                 2: "persistent cooperative kernel", 3: "cluster-resident kernel (one thread-block cluster)",
+                 4: "fixed-FP32 ablation kernel"}[cu.cuth_loop_home(g, S.opts)],
         "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),
                 "d2h_bytes_per_step": int(w.n * 8)},
         "gpu_launches": int(launches), "clocks": clocks,

@@ -265,6 +265,11 @@ int cuth_version(void);
  * gpu_launches = prologue + this * iterations + true-residual branches + epilogue.  Pure host. */
 int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts);
 
+/* Where the PCG loop of a solve with these options on this grid lives (what cuth_tuning_t.loop_mode = 0 resolves
+ * to): 1 = CUDA graph with conditional nodes, 2 = persistent cooperative kernel, 3 = cluster-resident kernel,
+ * 4 = the fixed-FP32 ablation kernel; negative on bad arguments.  Pure host. */
+int cuth_loop_home(const cuth_grid_t* grid, const cuth_opts_t* opts);
+
 /* Kernel launches of ONE Chebyshev apply (Alg. 3) for this grid and these options: the first
  * pass, the middle passes (single, or two per launch -- see cuth_tuning_t.cheb_fusion) and the last pass; 0 when the
  * preconditioner is not Chebyshev, negative on bad arguments.  *pairs_out (may be NULL) = how many of them are

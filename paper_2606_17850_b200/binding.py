@@ -70,7 +70,7 @@ EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "
            "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv", "cuth_spmv_tuned", "cuth_pcg_solve",
            "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error", "cuth_version",
            "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_lanczos_bounds", "cuth_lanczos_bounds_tuned",
-           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe"]
+           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home"]
 
 _lib = None
 
@@ -375,6 +375,17 @@ def cuth_cheb_launches(grid: Grid, opts):
 
 def cuth_version() -> int:
     return int(load_library().cuth_version())
+
+
+def cuth_loop_home(grid: Grid, opts) -> int:
+    """1 graph, 2 persistent kernel, 3 cluster-resident kernel, 4 fixed-FP32 kernel (include/cuth.h); pure host."""
+    L = load_library()
+    L.cuth_loop_home.restype = C.c_int
+    L.cuth_loop_home.argtypes = [C.POINTER(cuth_grid_t), C.POINTER(cuth_opts_t)]
+    rc = int(L.cuth_loop_home(grid.ref(), C.byref(opts)))
+    if rc < 0:
+        _check(rc, "cuth_loop_home")
+    return rc
 
 
 def cuth_launches_per_iteration(grid: Grid, opts) -> int:

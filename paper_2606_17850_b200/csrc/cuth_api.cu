@@ -647,6 +647,36 @@ static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune&
   return cluster_fits(L.nx, L.ny, L.nz, kClusterMaxCtas);
 }
 
+// One cluster per solve (nsolves > 1: cuth_pcg_solve_batch, contexts and control blocks as arrays).  8 CTAs when the
+// rows fit them, else 16 (non-portable cluster size): measured at cfg 1 (8 192 rows) 4.41 us per iteration with 8 CTAs
+// against 4.88 with 16 -- the all-reduce across CTAs costs more than the halved row work saves.
+static cudaError_t launch_cluster(const DiaLayout& L, const Ctx* ctxp, Ctl* ctlp, int nsolves, cudaStream_t st) {
+  cudaError_t e = cudaErrorInvalidValue;
+  for (int nc = 8; nc <= kClusterMaxCtas && e != cudaSuccess; nc *= 2) {
+    if (!cluster_fits(L.nx, L.ny, L.nz, nc)) continue;
+    const void* fn = nc == 16 ? (const void*)k_pcg_cluster<16> : (const void*)k_pcg_cluster<8>;
+    int rows = (int)cluster_rows_per_cta(L.nx, L.ny, L.nz, nc);
+    const size_t smem = cluster_smem_bytes(rows);
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        (nc > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+      cudaGetLastError();
+      continue;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)(nc * nsolves)); cfg.blockDim = dim3(kClusterThreads);
+    cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    void* args[] = {(void*)&ctxp, (void*)&ctlp, (void*)&rows};
+    e = cudaLaunchKernelExC(&cfg, fn, args);
+    if (e != cudaSuccess) cudaGetLastError();
+  }
+  return e;
+}
+
 static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
   const int mode = T.loop_mode, trav = T.traversal;
   if (cheb || mode == 1 || mode == 3 || trav == 2) return false;
@@ -759,32 +789,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
     return CUTH_OK;
   }
   if (use_cluster(L, opts, T)) {
-    // 8 CTAs when the rows fit them, else 16 (non-portable cluster size): measured at cfg 1 (8 192 rows) 4.41 us per
-    // iteration with 8 CTAs against 4.88 with 16 -- the all-reduce across CTAs costs more than the halved row work saves
-    cudaError_t e = cudaErrorInvalidValue;
-    for (int nc = 8; nc <= kClusterMaxCtas && e != cudaSuccess; nc *= 2) {
-      if (!cluster_fits(L.nx, L.ny, L.nz, nc)) continue;
-      const void* fn = nc == 16 ? (const void*)k_pcg_cluster<16> : (const void*)k_pcg_cluster<8>;
-      const int rows = (int)cluster_rows_per_cta(L.nx, L.ny, L.nz, nc);
-      const size_t smem = cluster_smem_bytes(rows);
-      if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-          (nc > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
-        cudaGetLastError();
-        continue;
-      }
-      cudaLaunchConfig_t cfg;
-      memset(&cfg, 0, sizeof cfg);
-      cfg.gridDim = dim3(nc); cfg.blockDim = dim3(kClusterThreads);
-      cfg.dynamicSmemBytes = smem; cfg.stream = st;
-      cudaLaunchAttribute at[1];
-      at[0].id = cudaLaunchAttributeClusterDimension;
-      at[0].val.clusterDim.x = nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-      cfg.attrs = at; cfg.numAttrs = 1;
-      const Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl;
-      void* args[] = {(void*)&ctxp, (void*)&ctlp, (void*)&rows};
-      e = cudaLaunchKernelExC(&cfg, fn, args);
-      if (e != cudaSuccess) cudaGetLastError();
-    }
+    const cudaError_t e = launch_cluster(L, w.ctx, w.ctl, 1, st);
     if (e == cudaSuccess) return CUTH_OK;
     if (T.loop_mode == 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster)");
     // automatic mode: fall through to the persistent kernel / the graph
@@ -991,6 +996,29 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   BatchWorkspace w = carve_batch_workspace(work_D, L.n, nrhs);
   if (work_bytes < w.bytes) return CUTH_ERR_SIZE;
   cudaStream_t st = (cudaStream_t)stream;
+  Tune T;
+  make_tune(&opts->tuning, &T);
+  if (use_cluster(L, opts, T)) {
+    // Small grids: ONE CLUSTER PER RIGHT-HAND SIDE (cuth_cluster.cuh) -- each solve is exactly cuth_pcg_solve's, the
+    // clusters run side by side on the 148 SMs (18 at a time with 8 CTAs each).  cfg 1, 32 right-hand sides: 4.7 ms in the
+    // lock-step kernel below, 2.6 ms here.  The per-solve contexts live in the partials area of the batch workspace.
+    static_assert(sizeof(Ctx) * kBatchMaxRhs <= sizeof(double) * 2 * 3 * (size_t)kBatchMaxRhs * kBatchMaxBlocks, "contexts fit");
+    Ctx base;
+    memset(&base, 0, sizeof base);
+    base.A = dev_view(dia_D, L, T);
+    base.b = b_D; base.x = x_D; base.result = result_D;
+    base.rtol = opts->rtol; base.precision = opts->precision; base.max_iters = opts->max_iters;
+    base.period = opts->true_resid_period > 0 ? opts->true_resid_period : 20;
+    base.jacobi = opts->preconditioner == CUTH_PRECOND_JACOBI ? 1 : 0;
+    base.early_op = OP_DIFF32;
+    base.soft_restart = 1; base.soft_drift2 = 1e-2;
+    Ctx* ctxs = reinterpret_cast<Ctx*>(w.partials);
+    k_set_ctx_batch<<<1, kBatchMaxRhs, 0, st>>>(base, ctxs, w.ctl, nrhs);
+    CU(cudaGetLastError());
+    const cudaError_t e = launch_cluster(L, ctxs, w.ctl, nrhs, st);
+    if (e == cudaSuccess) return CUTH_OK;
+    if (T.loop_mode == 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster, batch)");
+  }
   // co-resident CTAs available, split into ceil(nrhs / S) chunks x ntiles row tiles
   const int max_blocks = coresident_blocks(1, (const void*)k_pcg_batch, 3, 1 << 20);
   const int nchunks = (nrhs + kBatchChunk - 1) / kBatchChunk;
@@ -1243,6 +1271,19 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts
   if (use_cluster(L, opts, T)) return 0;                                                   // one cluster-resident kernel
   if (use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T)) return 0;      // one persistent kernel for the whole solve
   return use_zmarch(L, T) ? 2 : 3;
+}
+
+int cuth_loop_home(const cuth_grid_t* grid, const cuth_opts_t* opts) {
+  DiaLayout L;
+  Tune T;
+  if (!opts) return CUTH_ERR_NULL;
+  if (!make_layout(grid, &L)) return CUTH_ERR_DIMS;
+  if (check_opts(opts) != CUTH_OK || make_tune(&opts->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
+  if (opts->precision == CUTH_FIXED32) return 4;
+  if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
+  if (use_cluster(L, opts, T)) return 3;
+  if (T.loop_mode == 3) return CUTH_ERR_VALUE;
+  return use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T) ? 2 : 1;
 }
 
 int cuth_cheb_launches(const cuth_grid_t* grid, const cuth_opts_t* opts, int* pairs_out) {

@@ -20,7 +20,7 @@
 //     copy, __syncwarp): no block-wide barrier besides the ones inside the reductions.
 // Same arithmetic per row as the flat kernels (spmv_row / fused_dir_spmv_row), same policy code, same stopping rule;
 // FP64 and MIXED (difference form), M = diag A or I, steady and transient.  Selected automatically when the rows fit
-// (cuth_api.cu), or with cuth_tuning_t.loop_mode = 3.
+// (cuth_api.cu), or with cuth_tuning_t.loop_mode = 3.  cuth_pcg_solve_batch launches one cluster per right-hand side.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -135,6 +135,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1) k_pcg_cluster(const Ctx* _
   extern __shared__ __align__(16) unsigned char cl_raw[];
   ClusterSmem* sm = reinterpret_cast<ClusterSmem*>(cl_raw);
   const int R = rows_per_cta;
+  // batched use (cuth_pcg_solve_batch): one cluster per right-hand side, each with its own context and control block
+  ctxp += blockIdx.x / NC;
+  ctl_g += blockIdx.x / NC;
   double* sr = reinterpret_cast<double*>(cl_raw + kClusterFixedBytes);
   double* sz = sr + R; double* sx = sz + R; double* smu = sx + R; double* sp0 = smu + R; double* sp1 = sp0 + R;
   double* sdi = sp1 + R;

@@ -249,6 +249,23 @@ __global__ void k_set_ctx(Ctx c, Ctx* dst, Ctl* ctl) {
   }
 }
 
+// The same for a batch served by one cluster per right-hand side: context s = the base context with b, x, result moved to
+// right-hand side s (vectors are right-hand-side-major, [nrhs][n]).
+__global__ void k_set_ctx_batch(Ctx c, Ctx* dst, Ctl* ctl, int nrhs) {
+  const int s = threadIdx.x;
+  if (s < nrhs) {
+    Ctx m = c;
+    m.b = c.b + (size_t)s * (size_t)c.A.n;
+    m.x = c.x + (size_t)s * (size_t)c.A.n;
+    m.result = c.result + s;
+    dst[s] = m;
+    Ctl z;
+    memset(&z, 0, sizeof(z));
+    z.status = CUTH_SOLVE_RUNNING;
+    ctl[s] = z;
+  }
+}
+
 // rhs of eq. (5), T_amb = 0:  b = P + (C V / dt) T_n
 __global__ void __launch_bounds__(kThreads) k_transient_rhs(DiaDev A, const double* __restrict__ power,
                                                            const double* __restrict__ t_n, double* __restrict__ b) {

@@ -12,6 +12,17 @@ from paper_2606_17850_b200.binding import cuth_result_t
 
 pytestmark = pytest.mark.gpu
 
+
+@pytest.fixture(params=["auto", "lockstep"], autouse=True)
+def home(request):
+    """"auto": grids that fit one thread-block cluster run one cluster-resident solve per right-hand side (round 2), the
+    others the lock-step persistent kernel; "lockstep": the lock-step kernel (k_pcg_batch) everywhere."""
+    import paper_2606_17850_b200 as cu
+    cu.set_default_tuning(loop_mode=2 if request.param == "lockstep" else 0)
+    yield request.param
+    cu.set_default_tuning(loop_mode=0)
+
+
 GRIDS = [
     dict(cfg=1, nx=2, ny=2, nz=2, n_hot=0),
     dict(cfg=1, nx=7, ny=2, nz=5, n_hot=1),

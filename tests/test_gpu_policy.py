@@ -21,7 +21,7 @@ from policy_scan import expected_switch
 
 pytestmark = pytest.mark.gpu
 
-HOMES = ["flat-graph", "persistent", "cluster", "zmarch-graph", "zmarch-k1x1", "batch"]
+HOMES = ["flat-graph", "persistent", "cluster", "zmarch-graph", "zmarch-k1x1", "batch", "batch-cluster"]
 
 
 def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
@@ -31,10 +31,10 @@ def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
     tune = {"flat-graph": cu.Tuning(traversal=1, loop_mode=1), "persistent": cu.Tuning(traversal=1, loop_mode=2),
             "cluster": cu.Tuning(loop_mode=3),
             "zmarch-graph": cu.Tuning(traversal=2, k1_variant=2), "zmarch-k1x1": cu.Tuning(traversal=2, k1_variant=1),
-            "batch": cu.Tuning()}[home]
+            "batch": cu.Tuning(loop_mode=2), "batch-cluster": cu.Tuning(loop_mode=3)}[home]
     opts = cu.Opts(precision=precision, rtol=rtol, max_iters=max_iters, true_resid_period=period, tuning=tune)
     M = cu.DiaMatrix(grid_from_workload(w))
-    if home == "batch":
+    if home.startswith("batch"):
         S = cu.BatchSolver(M, 2, opts)
         X = torch.zeros(2, w.n, dtype=torch.float64, device="cuda")
         S.solve(torch.stack([to_dev(b), to_dev(0.5 * b)]), X)
