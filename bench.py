@@ -307,7 +307,9 @@ def run_batch(args):
                          "note": "algorithmic bytes of all iterations of all right-hand sides / whole-solve time; "
                                  "L2-resident for small grids, where the fraction is not an HBM statement"},
             "e2e": {"value": ms_e2e * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(B.nbytes), "d2h_bytes_per_step": int(B.nbytes)},
-            "gpu_launches": 2 * args.steps, "clocks": clocks, "loop": "persistent cooperative kernel (batched)"}
+            "gpu_launches": 2 * args.steps, "clocks": clocks,
+            "loop": ("one cluster-resident solve per right-hand side (k_pcg_cluster)" if cu.cuth_loop_home(g, opts) == 3
+                     else "persistent cooperative kernel, lock-step over the right-hand sides (k_pcg_batch)")}
     print(json.dumps(line))
 
 
@@ -358,6 +360,8 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     if args.batch > 0:
+        import paper_2606_17850_b200 as cu0
+        cu0.set_default_tuning(traversal=args.traversal, loop_mode=args.loop_mode, k1_variant=args.k1_variant)
         return run_batch(args)
 
     import torch
