@@ -327,6 +327,24 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t
  * reached.  No solver state is touched. */
 int cuth_policy_probe(const double in_H[8], int flags, int32_t* out_D, void* stream);
 
+/* The ONE entry point that needs no caller-allocated scratch and allocates nothing itself (for callers that cannot
+ * call cudaMalloc: code under CUDA-graph capture, tight serving loops, harnesses that forbid it): the true residual of
+ * the stopping rule (DESIGN.md R-G7), t = b - A1 x in fp64 on the packed diagonals, with
+ * out_D[0] = ||t||_2^2, out_D[1] = ||b||_2^2, out_D[2] = ||t||_2 / ||b||_2 (0 when b = 0), out_D[3] = 0 (device, 4 doubles).
+ * t_D: device [N] to receive t, or NULL when only the norms are wanted; must not alias x_D.  b_D, x_D: device [N].
+ * The per-CTA partial sums of the reduction live in a FILE-SCOPE device array of cuth_noalloc_max_rows()-dependent,
+ * fixed size (32 KB + 256 B) that every GPU loading this library holds until the process exits.  Hence:
+ *   - LIMIT: grids of more than cuth_noalloc_max_rows() = 16 777 216 rows (BASELINE cfg 3 fits exactly) are refused with
+ *     CUTH_ERR_SIZE before anything is launched; cuth_noalloc_last_error() says why;
+ *   - all calls on a GPU share that array: calls that may OVERLAP on the GPU (different streams) race on it and must be
+ *     serialised by the caller; back-to-back calls on one stream are fine (the call clears what must start at zero);
+ *   - results are bit-reproducible (fixed-order sums) and equal cuth_spmv followed by b - y up to the last bit of y.
+ * Calls no cudaMalloc / cudaFree / allocating library routine; asynchronous on `stream`. */
+int64_t cuth_noalloc_max_rows(void);
+const char* cuth_noalloc_last_error(void);
+int cuth_residual_noalloc(const void* dia_D, const cuth_grid_t* grid, const double* b_D, const double* x_D,
+                          double* t_D, double* out_D, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

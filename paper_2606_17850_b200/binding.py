@@ -70,7 +70,8 @@ EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "
            "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv", "cuth_spmv_tuned", "cuth_pcg_solve",
            "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error", "cuth_version",
            "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_lanczos_bounds", "cuth_lanczos_bounds_tuned",
-           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home"]
+           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home",
+           "cuth_residual_noalloc", "cuth_noalloc_max_rows", "cuth_noalloc_last_error"]
 
 _lib = None
 
@@ -375,6 +376,30 @@ def cuth_cheb_launches(grid: Grid, opts):
 
 def cuth_version() -> int:
     return int(load_library().cuth_version())
+
+
+def cuth_noalloc_max_rows() -> int:
+    L = load_library()
+    L.cuth_noalloc_max_rows.restype = C.c_int64
+    return int(L.cuth_noalloc_max_rows())
+
+
+def cuth_residual_noalloc(dia, grid: Grid, b, x, out, t=None, stream=None, check=True):
+    """t = b - A1 x, out[0..3] = ||t||^2, ||b||^2, ||t|| / ||b||, 0 -- without any workspace (include/cuth.h).  `out`: CUDA
+    float64 tensor of >= 4 elements.  Raises CuthError (with the library's message) unless check=False (returns rc)."""
+    L = load_library()
+    L.cuth_residual_noalloc.restype = C.c_int
+    L.cuth_residual_noalloc.argtypes = [C.c_void_p, C.POINTER(cuth_grid_t), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.c_void_p]
+    L.cuth_noalloc_last_error.restype = C.c_char_p
+    rc = L.cuth_residual_noalloc(_ptr(dia), grid.ref(), _ptr(b), _ptr(x), _ptr(t), _ptr(out), stream or _stream())
+    if not check:
+        return rc
+    if rc != 0:
+        e = CuthError(rc, "cuth_residual_noalloc")
+        e.args = (e.args[0] + ": " + L.cuth_noalloc_last_error().decode(),)
+        raise e
+    return rc
 
 
 def cuth_loop_home(grid: Grid, opts) -> int:
