@@ -31,7 +31,8 @@ import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
-NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3111e9,   # profiles/r1i_cfg3_default_and_cheb16.md
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3201e9,   # profiles/r2b_k1_tma.md (TMA-staged K1)
+                     ("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "mixed"): 1.1131e9,  # profiles/r2b_k1_tma.md (fp32-stored operator)
                      ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 518.3e6,    # profiles/r1i_cfg3_default_and_cheb16.md
                      ("cfg4_steady_4096x4096x8", "k_cheb_pair", "mixed"): 4.477e9,                 # profiles/r1h_cheb_pair_tma.md
                      ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 10.786e9,               # profiles/r1j_cfg4_fp64_k1.md
@@ -353,6 +354,8 @@ def main():
     ap.add_argument("--k1-variant", type=int, default=0, choices=[0, 1, 2, 3],
                     help="cuth_tuning_t.k1_variant: 0 auto, 1 one column per thread, 2 two columns (TMA-staged K1 when "
                          "nx %% 4 == 0), 3 two columns with ordinary loads")
+    ap.add_argument("--lanczos-fp32", action="store_true",
+                    help="Chebyshev setup: the paper's fp32 Lanczos on A2 (PAPER.md:340) instead of fp64 on A1")
     ap.add_argument("--batch", type=int, default=0,
                     help="NRHS > 0: time cuth_pcg_solve_batch on NRHS power maps of --config (FP64, Jacobi) against "
                          "NRHS single solves")
@@ -379,7 +382,7 @@ def main():
 
     # kernel variants travel in every call's cuth_tuning_t (the library has no process-wide settings)
     cu.set_default_tuning(traversal=args.traversal, loop_mode=args.loop_mode, cheb_fusion=args.cheb_fusion,
-                          k1_variant=args.k1_variant,
+                          k1_variant=args.k1_variant, lanczos_fp32=1 if args.lanczos_fp32 else 0,
                           pair_occupancy=args.pair_occupancy, pair_rows=args.pair_rows)
     w = W.make_workload(args.config) if args.grid is None else \
         W.make_workload(args.config, nx=args.grid[0], ny=args.grid[1], nz=args.grid[2], n_hot=16)

@@ -105,7 +105,9 @@ typedef struct {
                                  operands when nx % 4 == 0 (A3: % 8); 1 one pass per kernel; 3 two passes, never TMA */
   int32_t pair_rows;          /* rows of a region of the TMA two-pass Chebyshev kernel: 0 automatic, 8, 16 */
   int32_t pair_occupancy;     /* resident CTAs/SM of that kernel: 0 automatic (4), 2..4 */
-  int32_t reserved[2];        /* must be 0 */
+  int32_t lanczos_fp32;       /* cuth_lanczos_bounds: 0 = fp64 vectors on A1 (DESIGN.md R-C5), 1 = the paper's variant
+                                 (PAPER.md:315, 340): fp32 vectors and the fixed-FP32 SpMV on the fp32 copy A2 */
+  int32_t reserved;           /* must be 0 */
 } cuth_tuning_t;
 
 typedef struct {

@@ -72,3 +72,29 @@ def pcg_fixed(A: O.CSR, b, dtype=np.float32, rtol=1e-8, max_iters=200000, precon
     t = b64 - O.spmv(A, x64)
     return FixedResult(x64, status, it, float(np.sqrt(float(rr) / float(bb))),
                        float(np.linalg.norm(t) / np.linalg.norm(b64)))
+
+
+def lanczos_fixed(A: O.CSR, v0, m: int, dtype=np.float32):
+    """m Lanczos steps entirely in one working precision on A2 = the stored entries rounded to that
+    precision, standard form ("the N-step Lanczos algorithm ... in FP32 precision using the fixed FP32 SpMV
+    kernel").  Same recurrence as oracle_lanczos (C++): v normalised, no reorthogonalisation; returns alpha[m'], beta[m'].
+    `dtype=np.float64` must reproduce oracle_lanczos; that pins the recurrence."""
+    T = np.dtype(dtype).type
+    S = A.to_scipy().astype(dtype)
+    v = np.asarray(v0, dtype=np.float64).astype(dtype)
+    v = v / T(np.sqrt(T(v @ v)))
+    vp = np.zeros_like(v)
+    bprev = T(0)
+    alpha, beta = [], []
+    for _ in range(m):
+        w = S @ v - bprev * vp
+        a = T(w @ v)
+        w = w - a * v
+        b = T(np.sqrt(T(w @ w)))
+        alpha.append(float(a))
+        beta.append(float(b))
+        if not b > 0:
+            break
+        vp, v = v, w / b
+        bprev = b
+    return np.array(alpha), np.array(beta)

@@ -42,7 +42,7 @@ class cuth_grid_t(C.Structure):
 class cuth_tuning_t(C.Structure):
     _fields_ = [("traversal", C.c_int32), ("loop_mode", C.c_int32), ("k1_variant", C.c_int32),
                 ("cheb_fusion", C.c_int32), ("pair_rows", C.c_int32), ("pair_occupancy", C.c_int32),
-                ("reserved", C.c_int32 * 2)]
+                ("lanczos_fp32", C.c_int32), ("reserved", C.c_int32)]
 
 
 class cuth_opts_t(C.Structure):
@@ -171,7 +171,8 @@ class Grid:
 # The C library has no process-wide settings (include/cuth.h); the kernel variants travel in every call's
 # cuth_tuning_t.  For the test suite and bench.py, which run whole groups of calls under one variant, THIS PYTHON
 # MODULE keeps a default tuning that Opts() / DiaMatrix.spmv / the hooks below copy into their arguments.
-_DEFAULT_TUNING = dict(traversal=0, loop_mode=0, k1_variant=0, cheb_fusion=0, pair_rows=0, pair_occupancy=0)
+_DEFAULT_TUNING = dict(traversal=0, loop_mode=0, k1_variant=0, cheb_fusion=0, pair_rows=0, pair_occupancy=0,
+                       lanczos_fp32=0)
 
 
 def set_default_tuning(**kw):
@@ -186,7 +187,7 @@ def Tuning(**kw):
     d = dict(_DEFAULT_TUNING)
     d.update({k: int(v) for k, v in kw.items()})
     return cuth_tuning_t(d["traversal"], d["loop_mode"], d["k1_variant"], d["cheb_fusion"], d["pair_rows"],
-                         d["pair_occupancy"], (C.c_int32 * 2)(0, 0))
+                         d["pair_occupancy"], d["lanczos_fp32"], 0)
 
 
 def Opts(precision=FP64, rtol=1e-8, max_iters=200000, true_resid_period=20, preconditioner=PRECOND_JACOBI,

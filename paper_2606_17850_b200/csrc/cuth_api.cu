@@ -53,6 +53,7 @@ struct Tune {
   int pair_tma = 0;     // 0 auto (TMA when possible), 1 never
   int pair_rows = 0;    // 0 auto, 8, 16
   int pair_occ = 0;     // 0 auto (4), 2..4
+  int lanczos_fp32 = 0; // 1: the paper's fp32 Lanczos on A2
 };
 static int make_tune(const cuth_tuning_t* t, Tune* T) {
   *T = Tune();
@@ -60,12 +61,13 @@ static int make_tune(const cuth_tuning_t* t, Tune* T) {
   if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 3 || t->k1_variant < 0 ||
       t->k1_variant > 3 || t->cheb_fusion < 0 || t->cheb_fusion > 3 ||
       (t->pair_rows != 0 && t->pair_rows != 8 && t->pair_rows != 16) ||
-      (t->pair_occupancy != 0 && (t->pair_occupancy < 2 || t->pair_occupancy > 4)) || t->reserved[0] || t->reserved[1])
+      (t->pair_occupancy != 0 && (t->pair_occupancy < 2 || t->pair_occupancy > 4)) || t->lanczos_fp32 < 0 ||
+      t->lanczos_fp32 > 1 || t->reserved)
     return CUTH_ERR_VALUE;
   T->traversal = t->traversal; T->loop_mode = t->loop_mode; T->k1_variant = t->k1_variant;
   T->cheb_pairs = t->cheb_fusion == 3 ? 2 : t->cheb_fusion;
   T->pair_tma = t->cheb_fusion == 3 ? 1 : 0;
-  T->pair_rows = t->pair_rows; T->pair_occ = t->pair_occupancy;
+  T->pair_rows = t->pair_rows; T->pair_occ = t->pair_occupancy; T->lanczos_fp32 = t->lanczos_fp32;
   return CUTH_OK;
 }
 
@@ -1136,12 +1138,24 @@ int cuth_lanczos_bounds_tuned(const void* dia_D, const cuth_grid_t* grid, const 
   LanczosScal* sc = (LanczosScal*)(w.partials + 3 * kMaxBlocks);
   static_assert(sizeof(LanczosScal) <= sizeof(double) * kMaxBlocks, "LanczosScal must fit one partial slot");
   CU(cudaMemsetAsync(sc, 0, sizeof(LanczosScal), st));
-  double* u_cur = w.r; double* u_prev = w.p; double* t = w.mu;
-  k_lanczos_init<<<blocks, kThreads, 0, st>>>(A, v0_D, u_cur, u_prev, sc, w.partials);
-  for (int j = 0; j < steps; ++j) {
-    k_lanczos_1<<<sb, kThreads, 0, st>>>(A, u_cur, u_prev, t, sc, w.partials);
-    k_lanczos_2<<<blocks, kThreads, 0, st>>>(L.n, u_cur, t, u_prev, sc, w.partials);
-    double* tmp = u_prev; u_prev = u_cur; u_cur = tmp;     // u_{j+1} was written over u_{j-1}
+  if (T.lanczos_fp32) {
+    // the paper's variant (PAPER.md:315 "matrix A2 is used", :340 "in FP32 precision using the fixed FP32 SpMV kernel"):
+    // fp32 vectors in the same workspace buffers, A2 in standard form, fp32 arithmetic (flat traversal)
+    float* u_cur = (float*)w.r; float* u_prev = (float*)w.p; float* t = (float*)w.mu;
+    k_lanczos_init<float><<<blocks, kThreads, 0, st>>>(A, v0_D, u_cur, u_prev, sc, w.partials);
+    for (int j = 0; j < steps; ++j) {
+      k_lanczos_1_f32<<<blocks, kThreads, 0, st>>>(A, u_cur, u_prev, t, sc, w.partials);
+      k_lanczos_2<float><<<blocks, kThreads, 0, st>>>(L.n, u_cur, t, u_prev, sc, w.partials);
+      float* tmp = u_prev; u_prev = u_cur; u_cur = tmp;
+    }
+  } else {
+    double* u_cur = w.r; double* u_prev = w.p; double* t = w.mu;
+    k_lanczos_init<double><<<blocks, kThreads, 0, st>>>(A, v0_D, u_cur, u_prev, sc, w.partials);
+    for (int j = 0; j < steps; ++j) {
+      k_lanczos_1<<<sb, kThreads, 0, st>>>(A, u_cur, u_prev, t, sc, w.partials);
+      k_lanczos_2<double><<<blocks, kThreads, 0, st>>>(L.n, u_cur, t, u_prev, sc, w.partials);
+      double* tmp = u_prev; u_prev = u_cur; u_cur = tmp;     // u_{j+1} was written over u_{j-1}
+    }
   }
   CU(cudaGetLastError());
   LanczosScal h;

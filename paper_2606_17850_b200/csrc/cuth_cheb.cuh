@@ -303,24 +303,60 @@ __global__ void __launch_bounds__(kThreads, 4) k_lanczos_1(DiaDev A, const doubl
     sc->alpha = s_cur * acc[0];
 }
 
-__global__ void __launch_bounds__(kThreads) k_lanczos_2(int64_t n, const double* __restrict__ u_cur,
-                                                       const double* __restrict__ t, double* __restrict__ u_next,
-                                                       LanczosScal* sc, double* partials) {
+// The paper's variant of L1: fp32 vectors, the fixed-FP32 SpMV of Alg. 2 on the fp32 copy A2 (all four
+// diagonals, standard form), fp32 arithmetic; per-thread sums in fp32, widened only for the fixed-order grid reduction.
+__global__ void __launch_bounds__(kThreads, 4) k_lanczos_1_f32(DiaDev A, const float* __restrict__ u_cur,
+                                                             const float* __restrict__ u_prev, float* __restrict__ t,
+                                                             LanczosScal* sc, double* partials) {
   __shared__ double smem[32];
   __shared__ int s_flag;
-  const double a = sc->alpha * sc->s_cur;
-  double acc[1] = {0.0};
+  const float s_cur = (float)sc->s_cur, cprev = (float)(sc->beta_prev * sc->s_prev);
+  const int64_t n = A.n, nx = A.nx, np = A.nxny;
+  float facc = 0.f;
   CUTH_TILE_LOOP(n) {
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
       const int64_t i = base + threadIdx.x + k * kThreads;
       if (i < n) {
-        const double v = t[i] - a * u_cur[i];
-        u_next[i] = v;
-        acc[0] = fma(v, v, acc[0]);
+        const float ui = u_cur[i];
+        float au = A.f0[i] * ui;
+        if (i + 1 < n) au = fmaf(A.f1[i], u_cur[i + 1], au);
+        if (i >= 1) au = fmaf(A.f1[i - 1], u_cur[i - 1], au);
+        if (i + nx < n) au = fmaf(A.f2[i], u_cur[i + nx], au);
+        if (i >= nx) au = fmaf(A.f2[i - nx], u_cur[i - nx], au);
+        if (i + np < n) au = fmaf(A.f3[i], u_cur[i + np], au);
+        if (i >= np) au = fmaf(A.f3[i - np], u_cur[i - np], au);
+        const float ti = s_cur * au - cprev * u_prev[i];
+        t[i] = ti;
+        facc = fmaf(ti, ui, facc);
       }
     }
   }
+  double acc[1] = {(double)facc};
+  if (grid_sum_last_block<1>(acc, partials, &sc->ticket[0], smem, &s_flag) && threadIdx.x == 0)
+    sc->alpha = (double)(s_cur * (float)acc[0]);
+}
+
+template <class V>
+__global__ void __launch_bounds__(kThreads) k_lanczos_2(int64_t n, const V* __restrict__ u_cur,
+                                                       const V* __restrict__ t, V* __restrict__ u_next,
+                                                       LanczosScal* sc, double* partials) {
+  __shared__ double smem[32];
+  __shared__ int s_flag;
+  const V a = (V)(sc->alpha * sc->s_cur);
+  V vacc = (V)0;
+  CUTH_TILE_LOOP(n) {
+#pragma unroll
+    for (int k = 0; k < kRows; ++k) {
+      const int64_t i = base + threadIdx.x + k * kThreads;
+      if (i < n) {
+        const V v = t[i] - a * u_cur[i];
+        u_next[i] = v;
+        vacc = v * v + vacc;
+      }
+    }
+  }
+  double acc[1] = {(double)vacc};
   if (grid_sum_last_block<1>(acc, partials + kMaxBlocks, &sc->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
     const double beta = sqrt(acc[0]);
     const int j = sc->j;
@@ -334,8 +370,9 @@ __global__ void __launch_bounds__(kThreads) k_lanczos_2(int64_t n, const double*
 }
 
 // u_0 = v0, u_{-1} = 0, s_0 = 1/||v0||; also the Gershgorin bound max_i sum_j |a_ij| (into out_beta[127]).
+template <class V>
 __global__ void __launch_bounds__(kThreads) k_lanczos_init(DiaDev A, const double* __restrict__ v0,
-                                                          double* __restrict__ u_cur, double* __restrict__ u_prev,
+                                                          V* __restrict__ u_cur, V* __restrict__ u_prev,
                                                           LanczosScal* sc, double* partials) {
   __shared__ double smem[2 * 32];
   __shared__ int s_flag;
@@ -347,9 +384,10 @@ __global__ void __launch_bounds__(kThreads) k_lanczos_init(DiaDev A, const doubl
     for (int k = 0; k < kRows; ++k) {
       const int64_t i = base + threadIdx.x + k * kThreads;
       if (i < n) {
-        const double v = v0[i];
-        u_cur[i] = v;
-        u_prev[i] = 0.0;
+        const V vv = (V)v0[i];
+        const double v = (double)vv;
+        u_cur[i] = vv;
+        u_prev[i] = (V)0;
         acc[0] = fma(v, v, acc[0]);
         double g = fabs(A.d0[i]);
         if (i + 1 < n) g += fabs(A.d1[i]);

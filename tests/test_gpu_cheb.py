@@ -183,6 +183,38 @@ def test_cheb_fp16_matrix_apply_and_solve(kw):
     assert np.abs(xh - O.pcg(A, b).x).max() <= 1e-4
 
 
+@pytest.mark.parametrize("kw", [dict(cfg=1), dict(cfg=3, nx=37, ny=29, nz=16, n_hot=8), dict(cfg=5, nx=48, ny=40, nz=16, n_hot=8)])
+@pytest.mark.parametrize("traversal", ["flat-pairs"], indirect=True)
+def test_lanczos_fp32_variant_vs_reference_and_solve(kw, traversal):
+    """Lanczos in FP32 with the fixed-FP32 SpMV on A2 (`cuth_tuning_t.lanczos_fp32`).  Against the
+    step-by-step fp32 reference (oracle/ablation.py, whose fp64 instance reproduces oracle_lanczos): the spectral interval
+    agrees to a few per cent (unconverged Ritz values move with the summation order); the interval serves the
+    preconditioner as well as the fp64 one (R-C5): same outer iteration count to within 15 %, both bars met."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    from oracle import ablation as AB
+    w = W.make_workload(**kw)
+    A = O.assemble_workload(w)
+    b = _rhs(w)
+    M = cu.DiaMatrix(grid_from_workload(w))
+    out = {}
+    for f32 in (0, 1):
+        S = cu.Solver(M, cu.Opts(precision=cu.MIXED, rtol=1e-8, true_resid_period=w.true_resid_period,
+                                 tuning=cu.Tuning(lanczos_fp32=f32)))
+        lo, hi, gersh = S.setup_chebyshev(to_dev(b), lanczos_steps=20, degree=30)
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        S.solve(to_dev(b), x)
+        r = S.result()
+        assert r.status == 0 and np.linalg.norm(b - O.spmv(A, x.cpu().numpy())) <= 1e-8 * np.linalg.norm(b)
+        out[f32] = (lo, hi, r.iterations)
+        S.close()
+    a32, b32 = AB.lanczos_fixed(A, b, 20, dtype=np.float32)
+    lo_o, hi_o = O.ritz_extremes(a32, b32)
+    assert out[1][1] == pytest.approx(hi_o, rel=0.02) and out[1][0] == pytest.approx(lo_o, rel=0.1)
+    assert out[1][1] == pytest.approx(out[0][1], rel=0.02)
+    assert abs(out[1][2] - out[0][2]) <= max(3, 0.15 * out[0][2])
+
+
 def test_lanczos_invariant_subspace_on_a_tiny_grid():
     """N = 8 < requested Lanczos steps: the Krylov space is exhausted (beta_j -> 0); the bounds must still be
     the exact extreme eigenvalues and the Chebyshev solve must work."""

@@ -38,3 +38,21 @@ def test_fixed_fp32_drifts_like_table_vi():
     assert res.rel_resid_true >= 100 * res.rel_resid_rec
     assert np.abs(ref.x - xd).max() <= 1e-6 * np.abs(xd).max()    # fp64 on the same system is fine
     assert AB.pcg_fixed(A, np.zeros(w.n)).iterations == 0
+
+
+def test_lanczos_fixed_fp64_reproduces_oracle_lanczos_and_fp32_stays_close():
+    """Lanczos in FP32 on the fixed-FP32 SpMV.  The fp64 instance of the step-by-step reference is the C++
+    oracle's recurrence (same alpha, beta); the fp32 instance gives the same spectral interval to a per cent or two --
+    which is all the preconditioner needs."""
+    for kw in (dict(cfg=1), dict(cfg=3, nx=20, ny=16, nz=16, n_hot=4)):
+        w = W.make_workload(**kw)
+        A = O.assemble_workload(w)
+        a64, b64 = O.lanczos(A, w.power, 25)
+        a, b = AB.lanczos_fixed(A, w.power, 25, dtype=np.float64)
+        assert np.allclose(a, a64, rtol=1e-8, atol=0) and np.allclose(b[:-1], b64[:-1], rtol=1e-7, atol=0)
+        a32, b32 = AB.lanczos_fixed(A, w.power, 25, dtype=np.float32)
+        lo, hi = O.ritz_extremes(a64, b64)
+        lo32, hi32 = O.ritz_extremes(a32, b32)
+        assert abs(hi32 - hi) <= 0.02 * hi          # unconverged Ritz values after 25 steps move with the rounding
+        assert abs(lo32 - lo) <= 0.05 * lo
+        assert np.abs(a32[:5] - a64[:5]).max() <= 1e-5 * np.abs(a64).max()      # the first steps agree to fp32 rounding
