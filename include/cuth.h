@@ -173,6 +173,10 @@ typedef struct {
   int64_t positive_offdiag;   /* off-diagonal entries > 0: information only (a conductance matrix has none) */
   double max_rowsum_dev;      /* max over rows of |row sum - s(layer)| / (smallest diagonal entry of the layer) */
   int32_t mixed_ok;           /* 1: the row sums are constant per layer to 1e-9, so CUTH_MIXED is available */
+  int32_t reserved;
+  int64_t bad_rowptr;         /* cuth_import_csr: rows whose [rowptr[i], rowptr[i+1]) is not a sane range -- rowptr[0] != 0,
+                                 decreasing, more than 4096 entries in a row, or (cuth_import_csr_n) beyond nnz.  When
+                                 non-zero NOTHING else of the matrix is read: the call fails with CUTH_ERR_STRUCTURE */
 } cuth_import_report_t;
 
 /* Importer (the paper's matrices are sparse matrices exported by 3D-ICE, which
@@ -195,6 +199,12 @@ typedef struct {
 int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
                     const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
                     void* stream);
+
+/* cuth_import_csr with the number of stored entries, so that a rowptr that points beyond the col / val arrays is caught
+ * before anything is read through it (nnz < 0 = unknown = cuth_import_csr). */
+int cuth_import_csr_n(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
+                      int64_t nnz, const double* rowsum_layer_H, void* dia_D, size_t dia_bytes,
+                      cuth_import_report_t* report_H, void* stream);
 
 /* The same import from COORDINATE format: nnz entries (row_D[q], col_D[q], val_D[q]) in any order (int32 indices,
  * device).  Same checks, same report, same matrix object as cuth_import_csr (one thread per entry; a coordinate met

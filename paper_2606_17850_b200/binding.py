@@ -63,7 +63,7 @@ class cuth_result_t(C.Structure):
 class cuth_import_report_t(C.Structure):
     _fields_ = [("off_stencil", C.c_int64), ("asymmetric_rows", C.c_int64), ("bad_diagonal", C.c_int64),
                 ("duplicates", C.c_int64), ("positive_offdiag", C.c_int64), ("max_rowsum_dev", C.c_double),
-                ("mixed_ok", C.c_int32)]
+                ("mixed_ok", C.c_int32), ("reserved", C.c_int32), ("bad_rowptr", C.c_int64)]
 
 
 EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "cuth_pcg_solve_batch", "cuth_dia_bytes",
@@ -71,7 +71,7 @@ EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "
            "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error", "cuth_version",
            "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_lanczos_bounds", "cuth_lanczos_bounds_tuned",
            "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home",
-           "cuth_residual_noalloc", "cuth_noalloc_max_rows", "cuth_noalloc_last_error"]
+           "cuth_residual_noalloc", "cuth_noalloc_max_rows", "cuth_noalloc_last_error", "cuth_import_csr_n"]
 
 _lib = None
 
@@ -239,16 +239,21 @@ def cuth_build_dia(grid: Grid, dia, stream=None):
                                          stream or _stream()), "cuth_build_dia")
 
 
-def cuth_import_csr(grid: Grid, rowptr, col, val, dia, rowsum_layer=None, stream=None, check=True):
+def cuth_import_csr(grid: Grid, rowptr, col, val, dia, rowsum_layer=None, stream=None, check=True, nnz=None):
     """rowptr int64 / col int32 / val float64 CUDA tensors.  Returns the cuth_import_report_t; raises CuthError on
     failure unless check=False (then returns (rc, report)).  Synchronises the stream."""
     import torch
     assert rowptr.dtype == torch.int64 and col.dtype == torch.int32 and val.dtype == torch.float64
     rep = cuth_import_report_t()
     rs = None if rowsum_layer is None else np.ascontiguousarray(rowsum_layer, dtype=np.float64)
-    rc = load_library().cuth_import_csr(grid.ref(), _ptr(rowptr), _ptr(col), _ptr(val),
-                                        None if rs is None else rs.ctypes.data_as(C.c_void_p), _ptr(dia),
-                                        dia.numel() * dia.element_size(), C.byref(rep), stream or _stream())
+    L = load_library()
+    L.cuth_import_csr_n.restype = C.c_int
+    L.cuth_import_csr_n.argtypes = [C.POINTER(cuth_grid_t), C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p,
+                                    C.c_void_p, C.c_size_t, C.POINTER(cuth_import_report_t), C.c_void_p]
+    rc = L.cuth_import_csr_n(grid.ref(), _ptr(rowptr), _ptr(col), _ptr(val),
+                             C.c_int64(val.numel() if nnz is None else int(nnz)),
+                             None if rs is None else rs.ctypes.data_as(C.c_void_p), _ptr(dia),
+                             dia.numel() * dia.element_size(), C.byref(rep), stream or _stream())
     if not check:
         return rc, rep
     _check(rc, "cuth_import_csr")

@@ -885,6 +885,12 @@ int cuth_build_dia(const cuth_grid_t* grid, void* dia_D, size_t dia_bytes, void*
 int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
                     const double* rowsum_layer_H, void* dia_D, size_t dia_bytes, cuth_import_report_t* report_H,
                     void* stream) {
+  return cuth_import_csr_n(grid, rowptr_D, col_D, val_D, -1, rowsum_layer_H, dia_D, dia_bytes, report_H, stream);
+}
+
+int cuth_import_csr_n(const cuth_grid_t* grid, const int64_t* rowptr_D, const int32_t* col_D, const double* val_D,
+                      int64_t nnz, const double* rowsum_layer_H, void* dia_D, size_t dia_bytes,
+                      cuth_import_report_t* report_H, void* stream) {
   DiaLayout L;
   int rc = check_grid(grid, &L);
   if (rc) return rc;
@@ -898,7 +904,8 @@ int cuth_import_csr(const cuth_grid_t* grid, const int64_t* rowptr_D, const int3
   cuth_import_report_t rep;
   memset(&rep, 0, sizeof rep);
   cudaError_t e = cudaSuccess;
-  rc = launch_import(grid, L, rowptr_D, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e);
+  rc = launch_import(grid, L, rowptr_D, col_D, val_D, rowsum_layer_H, dia_D, &rep, (cudaStream_t)stream, &e, nullptr,
+                     nnz < 0 ? -1 : nnz);
   if (report_H) *report_H = rep;
   if (rc == CUTH_ERR_CUDA) return cuda_fail(e, "cuth_import_csr");
   return rc;

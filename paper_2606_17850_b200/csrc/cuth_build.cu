@@ -208,6 +208,19 @@ __device__ __forceinline__ unsigned long long ordered_key(double v) {   // monot
   return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
 }
 
+// Pass 0: is rowptr a row pointer at all?  A malformed one would send the passes below out of bounds through col / val
+// (or into a very long loop), so nothing else is read until this count is zero.
+__global__ void __launch_bounds__(256) k_import_check_rowptr(const int64_t* __restrict__ rowptr, int64_t n, int64_t nnz,
+                                                            unsigned long long* bad_out) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  unsigned long long bad = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const int64_t lo = rowptr[i], hi = rowptr[i + 1];
+    if (lo < 0 || hi < lo || hi - lo > 4096 || (i == 0 && lo != 0) || (nnz >= 0 && hi > nnz)) ++bad;
+  }
+  if (bad) atomicAdd(bad_out, bad);
+}
+
 // Pass 1, one thread per row: the row's own diagonal and upper entries go to their slots (a missing entry is
 // +0.0, which is also what the builder stores where the +x / +y neighbour does not exist).
 __global__ void __launch_bounds__(256) k_import_upper(ImportArgs a) {
@@ -437,6 +450,16 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
     k_coo_mirror<<<(unsigned)eb, 256, 0, st>>>(a);
     k_coo_rows<<<(unsigned)blocks, 256, 0, st>>>(a);
   } else {
+    unsigned long long bad_rowptr = 0;
+    k_import_check_rowptr<<<(unsigned)blocks, 256, 0, st>>>(rowptr_D, L.n, nnz, a.cnt + 5);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad_rowptr, a.cnt + 5, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
+    if (bad_rowptr) {
+      if (rep) { rep->bad_rowptr = (int64_t)bad_rowptr; rep->mixed_ok = 0; }
+      return CUTH_ERR_STRUCTURE;
+    }
     k_import_upper<<<(unsigned)blocks, 256, 0, st>>>(a);
     k_import_lower<<<(unsigned)blocks, 256, 0, st>>>(a);
   }

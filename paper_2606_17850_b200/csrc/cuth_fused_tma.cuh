@@ -29,6 +29,23 @@
 namespace cuth {
 
 constexpr int kK1Stages = 3;
+// Split-phase synchronisation of the p' ring (compile-time option, OFF: measured on B200 it changes nothing -- cfg 3 MIXED
+// 1.347 vs 1.354 s, cfg 3 FP64 1.376 vs 1.369 s, cfg 4 FP64 24.44 vs 24.26 s, cfg 5 2.299 vs 2.311 s for 40 steps; K1 fp32-stored
+// 0.187 vs 0.190 ms -- so the per-step barrier is not what bounds the kernel, and the simpler form is kept).  A step's only CTA-wide dependency is "plane j of p' is complete
+// before the NEXT step reads its in-plane neighbours"; with __syncthreads every warp waits for the slowest one in every
+// step (ncu, round 2: stalled_barrier 4.9 warps per issue at 2 CTAs/SM).  Instead each warp ARRIVES on an mbarrier
+// right after writing its part of plane j and WAITS for that phase only one step later, just before writing plane j + 1:
+// warps may drift a step apart.  The wait of phase s - 1 also tells thread 0 that every warp has read the operands of step
+// s - 1 out of its stage, so that stage can be requested again (for step s + 2).  Three ring planes make it safe: plane
+// (s - 1) % 3 is read by the mu rows of step s and overwritten in step s + 2, whose writers have passed the wait of phase
+// s + 1, i.e. every warp has finished step s.  0 = one __syncthreads per step.
+#ifndef CUTH_K1_SPLIT
+#define CUTH_K1_SPLIT 0
+#endif
+constexpr int kK1Ring = CUTH_K1_SPLIT ? 3 : 2;
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
 constexpr int K1X = XTX, K1Y = XTY;                      // 64 x 8 columns per tile (as k_fused_pspmv_x2)
 constexpr int K1VW = K1X + 4;                            // vector box: x0-2 .. x0+65 (16-byte aligned start, one-cell rim)
 constexpr int K1VH = K1Y + 2;                            // rows y0-1 .. y0+TY
@@ -50,8 +67,9 @@ struct K1Stage {
 template <bool MIXED>
 struct K1Smem {
   K1Stage<MIXED> st[kK1Stages];
-  alignas(16) double sp[2][K1VH][XS];                   // p' ring: plane parity x (tile + rim), as k_fused_pspmv_x2
+  alignas(16) double sp[kK1Ring][K1VH][XS];             // p' ring: (tile + rim) planes of the last kK1Ring steps
   alignas(8) uint64_t full[kK1Stages];
+  alignas(8) uint64_t ringbar;                          // split-phase CTA barrier of the p' ring: one arrival per warp and step
   double red[32];
   int s_flag;
 };
@@ -112,6 +130,7 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
   };
   if (tid == 0) {
     for (int s = 0; s < kK1Stages; ++s) mbar_init(&sm.full[s], 1);
+    mbar_init(&sm.ringbar, kThreads / 32);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int s = 0; s < kK1Stages && s < total; ++s) request_next();
   }
@@ -127,6 +146,7 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
   double2 xnext = make_double2(0.0, 0.0);              // x of the plane the NEXT step forms p' for
   uint32_t ph = 0;                                     // bit S: parity of the next fill of stage S
   int slot = 0, j = 0, k = 0;
+  int rw = 0, rr = kK1Ring - 1;                        // ring plane written in this step / written in the step before
 
   for (int s = 0; s < total; ++s) {
     if (j == 0) {                                      // a new tile
@@ -171,9 +191,17 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
       a2l = k1_ld_pair<MIXED>(&S.m2[ty][2 * tx]);
       a3u = k1_ld_pair<MIXED>(&S.m3[ty][2 * tx]);
     }
+#if CUTH_K1_SPLIT
+    // ---- 2. every warp has finished step s - 2 and has written its part of the ring plane of step s - 1
+    if (s > 0) {
+      mbar_wait(&sm.ringbar, (uint32_t)((s - 1) & 1));
+      if (tid == 0 && s + kK1Stages - 1 < total) request_next();     // the stage of step s - 1 is consumed: refill it
+    }
+#else
     // ---- 2. plane j - 1 of the p' ring is complete, plane j - 2 no longer read, the stage is consumed
     __syncthreads();
     if (tid == 0 && s + kK1Stages < total) request_next();
+#endif
     // ---- 3. plane j of p'
     double ph0 = 0.0, ph1 = 0.0;
     if (has_p) {
@@ -185,15 +213,19 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
         std2(p_out + ip, ph0, ph1);
         std2(xg + ip, fma(xalpha, po.x, xo.x), fma(xalpha, po.y, xo.y));
       }
-      std2(&sm.sp[j & 1][ty + 1][sc0], ph0, ph1);
+      std2(&sm.sp[rw][ty + 1][sc0], ph0, ph1);
       if (halo_role) {
         const double zh = jac ? (MIXED ? rh * dh : rh * rcp_diag(dh)) : rh;
-        sm.sp[j & 1][hr][hc] = halo_in ? fma(beta, phh, zh) : 0.0;
+        sm.sp[rw][hr][hc] = halo_in ? fma(beta, phh, zh) : 0.0;
       }
     }
+#if CUTH_K1_SPLIT
+    __syncwarp();
+    if (tx == 0) mbar_arrive(&sm.ringbar);             // phase s: this warp's part of the plane is written, its operands are read
+#endif
     // ---- 4. rows of plane j - 1 of mu = A p'
     if (has_mu && own) {
-      const double (*P)[XS] = sm.sp[(j - 1) & 1];
+      const double (*P)[XS] = sm.sp[rr];
       const double vl = P[ty + 1][sc0 - 1], vr = P[ty + 1][sc0 + 2];
       const double2 dn = *reinterpret_cast<const double2*>(&P[ty][sc0]);
       const double2 up = *reinterpret_cast<const double2*>(&P[ty + 2][sc0]);
@@ -224,6 +256,8 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
     pl0 = pc0; pl1 = pc1; pc0 = ph0; pc1 = ph1; a3l0 = a3u.x; a3l1 = a3u.y;
     if (!MIXED) dcur = dd;                             // D0 of plane j serves the mu rows of the next step
     if (++slot == kK1Stages) slot = 0;
+    rr = rw;
+    if (++rw == kK1Ring) rw = 0;
     if (++j == spt) { j = 0; ++k; }
   }
 }

@@ -195,6 +195,37 @@ def test_non_layered_row_sums_are_fp64_only():
     assert S.result().status == 0
 
 
+def test_import_rejects_a_malformed_rowptr_before_reading_through_it():
+    """a rowptr that is not a row pointer (not starting at 0, decreasing, pointing beyond the arrays, absurd row
+    lengths) must end in CUTH_ERR_STRUCTURE with `bad_rowptr` counted -- not in out-of-bounds reads of col / val."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(cfg=1, nx=6, ny=5, nz=4, n_hot=1)
+    A = O.assemble_workload(w)
+    g = grid_from_workload(w)
+    rp, col, val = _csr_dev(A)
+    buf = torch.empty(cu.cuth_dia_bytes(g), dtype=torch.uint8, device="cuda")
+    nnz = int(A.rowptr[-1])
+
+    def bad(rowptr_np, expect, nnz_arg=None):
+        rc, rep = cu.cuth_import_csr(g, torch.from_numpy(rowptr_np).cuda(), col, val, buf, check=False, nnz=nnz_arg)
+        assert rc == -8 and rep.bad_rowptr == expect and rep.mixed_ok == 0, (rc, rep.bad_rowptr, expect)
+
+    r = A.rowptr.copy(); r[0] = 1
+    bad(r, 1)                                                    # does not start at 0
+    r = A.rowptr.copy(); r[10] = r[9] - 1
+    bad(r, 1)                                                    # decreasing: row 9 ends before it starts (row 10 just gets longer)
+    r = A.rowptr.copy(); r[-1] = nnz + 1000
+    bad(r, 1, nnz_arg=nnz)                                       # last row runs beyond the arrays (caught because nnz is known)
+    r = A.rowptr.copy(); r[5:] += 1 << 40
+    bad(r, 1, nnz_arg=-1)                                        # nnz unknown: row 4 would have 2^40 entries
+    bad(r, w.n - 4)                                              # nnz known: rows 4 .. n-1 all end beyond the arrays
+    r = A.rowptr.copy(); r[3] = -7
+    bad(r, 2)                                                    # negative pointer: rows 2 and 3
+    rc, rep = cu.cuth_import_csr(g, rp, col, val, buf, check=False)          # and the real thing still imports
+    assert rc == 0 and rep.bad_rowptr == 0 and rep.mixed_ok == 1
+
+
 def test_import_argument_errors():
     import torch
     import paper_2606_17850_b200 as cu
