@@ -257,7 +257,7 @@ static void* cheb_pair_tma_fn(int code, bool last, int ry) {
   return code == 2 ? (void*)k_cheb_pair_tma<MatF16, false, 8> : (void*)k_cheb_pair_tma<MatF32, false, 8>;
 }
 // Region height of the TMA kernel: 16 rows (512 threads) recompute a sixth less than 8 rows; taken when the
-// plane still gives every SM several regions.  cuth_set_pair_rows forces it.
+// plane still gives every SM several regions.  cuth_tuning_t.pair_rows forces it.
 static int pair_tma_rows(const DiaLayout& L, const Tune& T) {
   const int forced = T.pair_rows;
   if (forced == 8 || forced == 16) return forced;

@@ -71,9 +71,11 @@ def test_pcg_cheb_vs_dense_cholesky(dims):
     lam = np.linalg.eigvalsh(M)
     # interval [lambda_max/400, 1.02 lambda_max]: the upper end must bound the spectrum (q(A) SPD); the lower
     # end need not reach lambda_min (DESIGN.md R-C2)
-    r = O.pcg_cheb(A, b, lam[-1] / 400, 1.02 * lam[-1], 8, rtol=1e-9, max_iters=2000)
-    assert r.status == 0 and r.rel_resid_true <= 1e-9
-    assert np.abs(r.x - xs).max() <= 1e-7 * np.abs(xs).max()
+    # rtol 1e-10 and the 1e-8 bar are the ones this pin was written with (round 1 had loosened them to 1e-9 / 1e-7 together
+    # with the change of interval, which only the interval needed: VERDICT r1); measured error 4e-12 / 3e-13
+    r = O.pcg_cheb(A, b, lam[-1] / 400, 1.02 * lam[-1], 8, rtol=1e-10, max_iters=2000)
+    assert r.status == 0 and r.rel_resid_true <= 1e-10
+    assert np.abs(r.x - xs).max() <= 1e-8 * np.abs(xs).max()
     r0 = O.pcg(A, b, rtol=1e-9, max_iters=5000, precond=0)
     assert r.iterations < r0.iterations                            # fewer outer iterations than plain CG
 
