@@ -329,7 +329,7 @@ static unsigned k1_tma_dyn_smem() {
 // keeps its TMA ring running across them, so it does not need the >= 2048 tiles of the LDG two-column kernel).
 // Measured per iteration, graph loop, MIXED, TMA K1 / one-column LDG K1: 512x512x16 84.3 / 108.3 us, 768x768x8
 // 92.1 / 119.7, 640x640x10 83.0 / 107.5, 384x384x32 91.2 / 112.0, but 256x256x64 (128 tiles) 104.8 / 155.4 with the
-// persistent kernel at 101.1 (profiles/r2_loop_homes.md).
+// persistent kernel at 101.1 (profiles/r2c_loop_homes.md).
 static bool fused_tma(const DiaLayout& L, const Tune& T, bool cheb) {
   if (cheb || T.k1_variant == 1 || T.k1_variant == 3) return false;
   if ((L.nx % 4) != 0 || encode_tiled_fn() == nullptr) return false;
@@ -641,7 +641,8 @@ static int persistent_blocks(int64_t n) {
 }
 
 // The cluster-resident kernel (cuth_cluster.cuh): every row lives in the shared memory of one 8-CTA cluster.
-// Measured on B200 (profiles/r2_loop_homes.md): cfg 1 (8 192 rows) per iteration, cluster / persistent kernel / graph.
+// Measured on B200 (profiles/r2c_loop_homes.md), per iteration, cluster / persistent kernel / graph: cfg 1 (8 192 rows)
+// 4.4 / 7.1 / 18.8 us, 2 048 rows 3.7 / 6.7 / 19.4, 12 800 rows 5.0 / 7.1 / 19.2.
 static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune& T) {
   if (T.loop_mode == 1 || T.loop_mode == 2 || T.traversal == 2) return false;
   if (opts->preconditioner == CUTH_PRECOND_CHEBYSHEV) return false;
@@ -691,7 +692,7 @@ static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
   // is three more kernels and an IF node in the graph, one more phase in the kernel).
   // Round 2, graph with the TMA-staged K1 and four iterations per WHILE pass / persistent kernel: 512x512x8 (2 M rows)
   // 48.2 / 47.9 us (MIXED), 1024x1024x2 53.2 / 47.0, but from 4 M rows on 512x512x16 (cfg 5) 84.3 / 101.8, 1024x512x8
-  // 86.3 / 101.2, 640x640x10 83.0 / 99.5, 768x768x8 92.1 / 113.7 (profiles/r2_loop_homes.md).
+  // 86.3 / 101.2, 640x640x10 83.0 / 99.5, 768x768x8 92.1 / 113.7 (profiles/r2c_loop_homes.md).
   // Auto: the persistent kernel (its row access is flat whatever the plane shape) up to 2^21 rows, and up to 2^22
   // rows where the TMA-staged K1 is not available; the graph everywhere else.
   if (L.n > (1 << 22)) return false;
