@@ -60,7 +60,9 @@ def bytes_per_row(w, what):
     # the fused K1 takes M = diag A from the D0 its SpMV reads (fp64 operator), so a fused fp64 iteration
     # moves 8m + 80, not the 8m + 88 of the three-kernel path (which reads 1/D0 in k_pupdate)
     return {"spmv_fp64": 8 * m + 16, "spmv_mixed": 4 * (m - 1) + 16,
-            "iter_fp64": 8 * m + 88, "iter_fp64_fused": 8 * m + 80, "iter_mixed": 4 * (m - 1) + 88}[what]
+            "iter_fp64": 8 * m + 88, "iter_fp64_fused": 8 * m + 80, "iter_mixed": 4 * (m - 1) + 88,
+            # fused path, early stage: 1/D0 is read as fp32 in K1 and in K2 (4 + 4 B instead of 8 + 8)
+            "iter_mixed_fused": 4 * (m - 1) + 80}[what]
 
 
 def max_over_ranks(value_ms: float, world: int, device="cpu") -> float:
@@ -528,6 +530,8 @@ def main():
     if mixed and not cheb:
         cu.cuth_profile_kernel(S.work, g, S.opts, -2)
         kern[a_name + "[fp32-stored operator]"] = time_kernel(a_kid)
+        if fused:
+            kern["k_update_nox[early stage: fp32 1/D0, 28 B/row]"] = time_kernel(5)
         for _ in range(args.profile_iters):
             for kid in body_ids:
                 cu.cuth_profile_kernel(S.work, g, S.opts, kid)
@@ -557,7 +561,7 @@ def main():
     it = total_its
     early = int(early_acc.item()) if mixed else 0
     late = it - early
-    iter_bytes = (early * bytes_per_row(w, "iter_mixed")
+    iter_bytes = (early * bytes_per_row(w, "iter_mixed_fused" if fused else "iter_mixed")
                   + late * bytes_per_row(w, "iter_fp64_fused" if fused else "iter_fp64")) * w.n
     m = m_ratio(w)
     if cheb:
@@ -581,7 +585,7 @@ def main():
     stage_tag = "fp32-stored" if early_major else "fp64"
     if fused:      # K1: matrix + r, p, x read + p', mu, x written (+ 1/D0 read with the fp32-stored operator)
         dom_name = "k_fused_pspmv"
-        dom_bytes = ((4 * (m - 1) + 56) if early_major else (8 * m + 48)) * w.n
+        dom_bytes = ((4 * (m - 1) + 52) if early_major else (8 * m + 48)) * w.n
     else:
         dom_name = "k_spmv_dot"
         dom_bytes = bytes_per_row(w, "spmv_mixed" if early_major else "spmv_fp64") * w.n
@@ -631,7 +635,7 @@ def main():
                                "frac": iter_gbs / peak, "frac_of_8TBs_nominal": iter_gbs / 8000.0,
                                "algorithmic_bytes_per_solve": iter_bytes,
                                "note": ("Chebyshev: outer K1+K2 plus (k-1)-kernel apply bytes per row per iteration " if cheb else "") +
-                                       "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+88 fp32-stored per row per iteration) "
+                                       "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+80 fp32-stored fused, 4(m-1)+88 unfused, per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
         "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % (4 if fused and not cheb else 1),
@@ -642,7 +646,7 @@ def main():
         "gpu_launches": int(launches), "clocks": clocks,
     }
     if fused and not cheb:      # the other K1 instantiation, for the record
-        for tag, nb in (("fp64", 8 * m + 48), ("fp32-stored", 4 * (m - 1) + 56)):
+        for tag, nb in (("fp64", 8 * m + 48), ("fp32-stored", 4 * (m - 1) + 52)):
             key = "k_fused_pspmv[%s operator]" % tag
             if key in kern:
                 gbs = nb * w.n / kern[key] / 1e6
@@ -699,7 +703,7 @@ def cfg4_block(cu, args, peak):
         ms = e0.elapsed_time(e1)
         r = S.result()
         early = (r.switch_iteration if r.promotions else r.iterations) if prec == cu.MIXED else 0
-        ib = (early * (4 * (m - 1) + 88) + (r.iterations - early) * (8 * m + 80)) * w.n
+        ib = (early * (4 * (m - 1) + 80) + (r.iterations - early) * (8 * m + 80)) * w.n
         d = {"value": ms * 1e-3, "unit": UNIT, "iterations": r.iterations, "iterations_early_stage": early,
              "status": r.status_name, "rel_resid_true": r.rel_resid_true, "true_resid_evals": r.true_resid_evals,
              "switch_reason": r.switch_reason, "us_per_iteration": ms * 1e3 / max(r.iterations, 1),
@@ -726,8 +730,8 @@ def cfg4_block(cu, args, peak):
         if prec == cu.MIXED:
             cu.cuth_profile_kernel(S.work, g, S.opts, -2)
             k1e = tk(4)
-            d["k1_fp32_stored"] = {"ms": k1e, "gbs": (4 * (m - 1) + 56) * w.n / k1e / 1e6,
-                                   "frac": (4 * (m - 1) + 56) * w.n / k1e / 1e6 / peak}
+            d["k1_fp32_stored"] = {"ms": k1e, "gbs": (4 * (m - 1) + 52) * w.n / k1e / 1e6,
+                                   "frac": (4 * (m - 1) + 52) * w.n / k1e / 1e6 / peak}
         xs[name] = x_keep.cpu().numpy()
         del x_keep
         S.close()

@@ -152,6 +152,7 @@ static DiaDev dev_view(const void* dia_D, const DiaLayout& L, const Tune& T) {
   A.f2 = (const float*)(base + L.o_f32a + L.f32a_stride);
   A.f3 = (const float*)(base + L.o_f32a + 2 * L.f32a_stride);
   A.dinv = (const double*)(base + L.o_dinv);
+  A.dinv32 = (const float*)(base + L.o_dinv32);
   A.h1 = (const __half*)(base + L.o_h16);
   A.h2 = (const __half*)(base + L.o_h16 + L.h16_stride);
   A.h3 = (const __half*)(base + L.o_h16 + 2 * L.h16_stride);
@@ -312,7 +313,7 @@ static bool make_k1_maps(K1Maps* km, K1Maps* km64, const DiaLayout& L, const voi
   const void* e2 = base + L.o_f64a + L.f64a_stride;
   const void* e3 = base + L.o_f64a + 2 * L.f64a_stride;
   return make_map3d(&km->z, w.r, 8, L, K1VW, K1VH) && make_map3d(&km->p, w.p, 8, L, K1VW, K1VH) &&
-         make_map3d(&km->p2, w.p2, 8, L, K1VW, K1VH) && make_map3d(&km->d, A.dinv, 8, L, K1VW, K1VH) &&
+         make_map3d(&km->p2, w.p2, 8, L, K1VW, K1VH) && make_map3d(&km->d, A.dinv32, 4, L, K1VW + 4, K1VH) &&
          make_map3d(&km->m1, A.f1, 4, L, K1Stage<true>::W1, K1Y) && make_map3d(&km->m2, A.f2, 4, L, K1X, K1Y + 1) &&
          make_map3d(&km->m3, A.f3, 4, L, K1X, K1Y) &&
          make_map3d(&km64->d, A.d0, 8, L, K1VW, K1VH) && make_map3d(&km64->m1, e1, 8, L, K1Stage<false>::W1, K1Y) &&

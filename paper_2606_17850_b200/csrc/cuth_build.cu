@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(256) k_make_h16(BuildArgs a, const double* slo
 // diagonal's length): what the solver kernels read.  The packed fp32 copy stays what cuth_dia_view shows.
 // ... and the same for the fp64 off-diagonals of A1 (e1..e3): the operands of the TMA-staged K1 (cuth_fused_tma.cuh).
 __global__ void __launch_bounds__(256) k_make_f32a(BuildArgs a, float* g1, float* g2, float* g3, double* e1, double* e2,
-                                                   double* e3) {
+                                                   double* e3, float* dinv32) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += stride) {
     const bool h1 = i + 1 < a.n, h2 = i + a.nx < a.n, h3 = i + a.nxny < a.n;
@@ -106,6 +106,7 @@ __global__ void __launch_bounds__(256) k_make_f32a(BuildArgs a, float* g1, float
     e1[i] = h1 ? a.d1[i] : 0.0;
     e2[i] = h2 ? a.d2[i] : 0.0;
     e3[i] = h3 ? a.d3[i] : 0.0;
+    dinv32[i] = __double2float_rn(a.dinv[i]);      // fp32(1/D0): the early-stage Jacobi preconditioner of the fused path
   }
 }
 
@@ -179,7 +180,7 @@ int launch_build(const cuth_grid_t* g, const DiaLayout& L, void* dia_D, cudaStre
   k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(a, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
                                                 (float*)(base + L.o_f32a + 2 * L.f32a_stride), (double*)(base + L.o_f64a),
                                                 (double*)(base + L.o_f64a + L.f64a_stride),
-                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride));
+                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride), (float*)(base + L.o_dinv32));
   e = cudaGetLastError();
   if (e != cudaSuccess) { *err = e; return CUTH_ERR_CUDA; }
   return CUTH_OK;
@@ -468,6 +469,7 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   memset(&b, 0, sizeof b);
   b.nx = L.nx; b.ny = L.ny; b.nz = L.nz; b.n = L.n; b.nxny = L.nxny;
   b.d0 = a.d0; b.d1 = a.d1; b.d2 = a.d2; b.d3 = a.d3;
+  b.dinv = (double*)(base + L.o_dinv);
   b.f0 = f + L.ptr[0]; b.f1 = f + L.ptr[1]; b.f2 = f + L.ptr[2]; b.f3 = f + L.ptr[3];
   double* slot = (double*)(base + L.o_layers) + 4 * nz;
   k_offdiag_absmax<<<(unsigned)blocks, 256, 0, st>>>(a.d1, L.e - L.n, slot);
@@ -477,7 +479,7 @@ int launch_import(const cuth_grid_t* g, const DiaLayout& L, const int64_t* rowpt
   k_make_f32a<<<(unsigned)blocks, 256, 0, st>>>(b, (float*)(base + L.o_f32a), (float*)(base + L.o_f32a + L.f32a_stride),
                                                 (float*)(base + L.o_f32a + 2 * L.f32a_stride), (double*)(base + L.o_f64a),
                                                 (double*)(base + L.o_f64a + L.f64a_stride),
-                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride));
+                                                (double*)(base + L.o_f64a + 2 * L.f64a_stride), (float*)(base + L.o_dinv32));
   e = cudaGetLastError();
   unsigned long long cnt[5];
   if (e == cudaSuccess) e = cudaMemcpyAsync(cnt, a.cnt, sizeof cnt, cudaMemcpyDeviceToHost, st);

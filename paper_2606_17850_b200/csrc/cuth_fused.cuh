@@ -78,10 +78,10 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
       double ro = 0.0, dio = 1.0, po = 0.0, xo = 0.0, rh = 0.0, dih = 1.0, ph = 0.0;
       if (own) {
         ro = zs[col]; po = p_in[col];
-        if (MIXED) { if (jac) dio = A.dinv[col]; } else { dnx = A.d0[col]; }
+        if (MIXED) { if (jac) dio = (double)A.dinv32[col]; } else { dnx = A.d0[col]; }
         if (do_x) xo = c.x[col];
       }
-      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? A.dinv[hcol] : A.d0[hcol]; }
+      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? (double)A.dinv32[hcol] : A.d0[hcol]; }
       if (own) {
         pn_c = fma(beta, po, MIXED ? ro * dio : (jac ? ro * rcp_diag(dnx) : ro));
         p_out[col] = pn_c;
@@ -114,14 +114,14 @@ __device__ __forceinline__ void fused_pspmv_body(const Ctx& c, const double* __r
         if (up3) {
           const int64_t j = i + np;
           ro = zs[j]; po = p_in[j];
-          if (MIXED) { if (jac) dio = A.dinv[j]; } else { dnx = A.d0[j]; }
+          if (MIXED) { if (jac) dio = (double)A.dinv32[j]; } else { dnx = A.d0[j]; }
           if (do_x) xo = c.x[j];
         }
       }
       if (up3 && halo_in) {
         const int64_t j = hcol + (int64_t)(z + 1) * np;
         rh = zs[j]; ph = p_in[j];
-        if (jac) dih = MIXED ? A.dinv[j] : A.d0[j];
+        if (jac) dih = MIXED ? (double)A.dinv32[j] : A.d0[j];
       }
       // ---- 2. plane z of p' (written during the previous step) is complete; the loads above fly
       //         while the CTA waits here

@@ -57,11 +57,15 @@ struct K1Stage {
   static constexpr int W1 = K1X + 16 / (int)sizeof(E);  // D1 box: x0 - 16 bytes .. x0+63 (the entry towards x-1 is the left one's)
   alignas(128) double vz[K1VH][K1VW];                   // r
   alignas(128) double vp[K1VH][K1VW];                   // p (old direction)
-  alignas(128) double vd[K1VH][K1VW];                   // 1/D0 (fp32-stored operator) or D0 (fp64 operator)
+  // the diagonal operand: fp32(1/D0) with the fp32-stored operator (box starts at x0 - 4 floats = 16 bytes: four more
+  // columns), D0 itself with the fp64 operator
+  using VD = typename std::conditional<MIXED, float, double>::type;
+  static constexpr int VDW = MIXED ? K1VW + 4 : K1VW, VDX = MIXED ? 4 : 2;   // box width; elements in front of the tile
+  alignas(128) VD vd[K1VH][VDW];
   alignas(128) E m1[K1Y][W1];
   alignas(128) E m2[K1Y + 1][K1X];                      // rows y0-1 .. y0+TY-1: the entry towards y-1 is the row above's
   alignas(128) E m3[K1Y][K1X];
-  static constexpr uint32_t kVecBytes = 3u * sizeof(double) * K1VH * K1VW;
+  static constexpr uint32_t kVecBytes = 2u * sizeof(double) * K1VH * K1VW + sizeof(VD) * K1VH * VDW;
   static constexpr uint32_t kMatBytes = sizeof(E) * (K1Y * W1 + (K1Y + 1) * K1X + K1Y * K1X);
 };
 template <bool MIXED>
@@ -118,7 +122,7 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
     if (rj < nz) {
       tma_load_3d(S.vz, tmZ, bar, x0 - 2, y0 - 1, rj);
       tma_load_3d(S.vp, tmP, bar, x0 - 2, y0 - 1, rj);
-      tma_load_3d(S.vd, tmD, bar, x0 - 2, y0 - 1, rj);
+      tma_load_3d(S.vd, tmD, bar, x0 - ST::VDX, y0 - 1, rj);
     }
     if (rj >= 1) {
       tma_load_3d(S.m1, tm1, bar, x0 - AL1, y0, rj - 1);
@@ -178,8 +182,9 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
     if (has_p) {
       ro = *reinterpret_cast<const double2*>(&S.vz[ty + 1][sc0]);
       po = *reinterpret_cast<const double2*>(&S.vp[ty + 1][sc0]);
-      dd = *reinterpret_cast<const double2*>(&S.vd[ty + 1][sc0]);
-      if (halo_role) { rh = S.vz[hbr][hbc]; phh = S.vp[hbr][hbc]; dh = S.vd[hbr][hbc]; }
+      if (MIXED) dd = ldf2(reinterpret_cast<const float*>(&S.vd[ty + 1][ST::VDX + 2 * tx]));
+      else dd = *reinterpret_cast<const double2*>(&S.vd[ty + 1][sc0]);
+      if (halo_role) { rh = S.vz[hbr][hbc]; phh = S.vp[hbr][hbc]; dh = (double)S.vd[hbr][hbc + ST::VDX - 2]; }
       if (own && j + 1 < nz) xnext = ldd2(xg + ip + np);            // prefetch for the next step
     }
     double2 a1 = make_double2(0.0, 0.0), a2u = a1, a2l = a1, a3u = a1;

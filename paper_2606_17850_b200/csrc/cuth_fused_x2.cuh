@@ -18,6 +18,10 @@ constexpr int kHaloX2PerWarp = kHaloX2 / (kThreads / 32);   // 18 lanes of each 
 static_assert(kHaloX2 % (kThreads / 32) == 0, "halo must divide evenly among the warps");
 
 __device__ __forceinline__ double2 ldd2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ double2 ldf2(const float* p) {       // an aligned pair of floats, promoted
+  const float2 f = *reinterpret_cast<const float2*>(p);
+  return make_double2((double)f.x, (double)f.y);
+}
 __device__ __forceinline__ void std2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
 
 template <bool MIXED>
@@ -62,10 +66,10 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
       double rh = 0.0, dih = 1.0, ph = 0.0;
       if (own) {
         ro = ldd2(zs + col); po = ldd2(p_in + col);
-        if (MIXED) { if (jac) dio = ldd2(A.dinv + col); } else { dnx = ldd2(A.d0 + col); }
+        if (MIXED) { if (jac) dio = ldf2(A.dinv32 + col); } else { dnx = ldd2(A.d0 + col); }
         if (do_x) xo = ldd2(c.x + col);
       }
-      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? A.dinv[hcol] : A.d0[hcol]; }
+      if (halo_in) { rh = zs[hcol]; ph = p_in[hcol]; if (jac) dih = MIXED ? (double)A.dinv32[hcol] : A.d0[hcol]; }
       if (own) {
         const double z0 = MIXED ? ro.x * dio.x : (jac ? ro.x * rcp_diag(dnx.x) : ro.x);
         const double z1 = MIXED ? ro.y * dio.y : (jac ? ro.y * rcp_diag(dnx.y) : ro.y);
@@ -107,14 +111,14 @@ __device__ __forceinline__ void fused_pspmv_x2_body(const Ctx& c, const double* 
         if (up3) {
           const int64_t j = i + np;
           ro = ldd2(zs + j); po = ldd2(p_in + j);
-          if (MIXED) { if (jac) dio = ldd2(A.dinv + j); } else { dnx = ldd2(A.d0 + j); }
+          if (MIXED) { if (jac) dio = ldf2(A.dinv32 + j); } else { dnx = ldd2(A.d0 + j); }
           if (do_x) xo = ldd2(c.x + j);
         }
       }
       if (up3 && halo_in) {
         const int64_t j = hcol + (int64_t)(z + 1) * np;
         rh = zs[j]; ph = p_in[j];
-        if (jac) dih = MIXED ? A.dinv[j] : A.d0[j];
+        if (jac) dih = MIXED ? (double)A.dinv32[j] : A.d0[j];
       }
       // ---- 2. plane z of p' is complete (written during the previous step); the loads fly meanwhile
       __syncthreads();

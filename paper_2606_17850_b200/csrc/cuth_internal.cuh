@@ -35,6 +35,8 @@ struct DiaLayout {
   size_t o_f64a;     // fp64 3 x [n] (each 256-B aligned): the off-diagonals of A1 again, one array per diagonal with a zero
   size_t f64a_stride;//   tail: proper (nx, ny, nz) tensors for the TMA-staged K1 (packed D2, D3 start at odd elements, and a
                      //   tensor map needs a 16-byte aligned base)
+  size_t o_dinv32;   // fp32 [n]: 1/D0 rounded to fp32 -- the Jacobi preconditioner of the EARLY stage of the fused path
+                     //   ("fp32 storage where stable": M only has to be SPD; 8 B/row less in K1 and in K2)
   size_t bytes;
 };
 
@@ -61,6 +63,7 @@ inline bool make_layout(const cuth_grid_t* g, DiaLayout* L) {
   L->o_f32a = o;   o = o + 3 * L->f32a_stride;
   L->f64a_stride = align_up(sizeof(double) * (size_t)L->n);
   L->o_f64a = o;   o = o + 3 * L->f64a_stride;
+  L->o_dinv32 = o; o = align_up(o + sizeof(float) * (size_t)L->n);
   L->bytes = o;
   return true;
 }
@@ -74,6 +77,7 @@ struct DiaDev {
   const __half* h1; const __half* h2; const __half* h3;                     // fp16 off-diagonals x scale (A3)
   const double* h_scale;    // [0] absmax bits, [1] scale (power of two), [2] 1/scale
   const double* dinv;       // 1/D0
+  const float* dinv32;      // fp32(1/D0): M^-1 of the early stage on the fused path
   const double* s_layer;    // exact row sums per layer: h dx dy [top] + C V / dt
   const double* cap_layer;  // C V / dt per layer (0 when steady)
   const unsigned long long* hdr;   // the object's header (kHdr* words)

@@ -364,14 +364,27 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
     const double2* __restrict__ r2 = reinterpret_cast<const double2*>(c.r);
     const double2* __restrict__ m2 = reinterpret_cast<const double2*>(c.mu);
     const double2* __restrict__ d2 = reinterpret_cast<const double2*>(c.A.dinv);
+    // early stage of the fused path: M^-1 = fp32(1/D0), the same values K1 forms z = M^-1 r with (cuth_fused*.cuh)
+    const float2* __restrict__ f2 = reinterpret_cast<const float2*>(c.A.dinv32);
+    const bool m32 = ctl->stage == 0;
     double2* __restrict__ w2 = reinterpret_cast<double2*>(c.r);
     const bool jac = c.jacobi != 0;
     for (int64_t base = (int64_t)blockIdx.x * (kThreads * 2); base < n2; base += (int64_t)gridDim.x * (kThreads * 2)) {
       const int64_t i0 = base + threadIdx.x, i1 = i0 + kThreads;
       const bool h0 = i0 < n2, h1 = i1 < n2;
       const double2 one = make_double2(1.0, 1.0), zero = make_double2(0.0, 0.0);
-      const double2 ra = h0 ? r2[i0] : zero, ma = h0 ? __ldcs(&m2[i0]) : zero, da = (h0 && jac) ? d2[i0] : one;
-      const double2 rb = h1 ? r2[i1] : zero, mb = h1 ? __ldcs(&m2[i1]) : zero, db = (h1 && jac) ? d2[i1] : one;
+      const double2 ra = h0 ? r2[i0] : zero, ma = h0 ? __ldcs(&m2[i0]) : zero;
+      const double2 rb = h1 ? r2[i1] : zero, mb = h1 ? __ldcs(&m2[i1]) : zero;
+      double2 da = one, db = one;
+      if (jac) {
+        if (m32) {
+          if (h0) { const float2 f = f2[i0]; da = make_double2((double)f.x, (double)f.y); }
+          if (h1) { const float2 f = f2[i1]; db = make_double2((double)f.x, (double)f.y); }
+        } else {
+          if (h0) da = d2[i0];
+          if (h1) db = d2[i1];
+        }
+      }
       const double a0 = fma(-alpha, ma.x, ra.x), a1 = fma(-alpha, ma.y, ra.y);
       const double b0 = fma(-alpha, mb.x, rb.x), b1 = fma(-alpha, mb.y, rb.y);
       if (h0) w2[i0] = make_double2(a0, a1);
@@ -389,7 +402,7 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       if (i < c.A.n) {
         if (UPDATE_X) c.x[i] = fma(alpha, c.p[i], c.x[i]);
         const double ri = fma(-alpha, c.mu[i], c.r[i]);
-        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+        const double zi = c.jacobi ? ri * ((!UPDATE_X && ctl->stage == 0) ? (double)c.A.dinv32[i] : c.A.dinv[i]) : ri;
         c.r[i] = ri;
         acc[0] = fma(ri, zi, acc[0]);
         acc[1] = fma(ri, ri, acc[1]);

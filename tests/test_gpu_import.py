@@ -81,7 +81,12 @@ def test_import_is_bit_exact(kw, given_rowsums):
         lk = int(ptr[k + 2] - ptr[k + 1])
         assert np.array_equal(dk[:lk].view(np.uint64), vals_o[int(ptr[k + 1]):int(ptr[k + 2])].view(np.uint64))
         assert not dk[lk:].any()
-    assert o_f64a + 3 * al(8 * n) == M.buf.numel()
+    o_dinv32 = o_f64a + 3 * al(8 * n)                        # fp32(1/D0): the early-stage preconditioner of the fused path
+    assert bool((M.buf[o_dinv32:o_dinv32 + 4 * n] == B.buf[o_dinv32:o_dinv32 + 4 * n]).all())
+    import torch
+    d32 = M.buf[o_dinv32:o_dinv32 + 4 * n].view(torch.float32).cpu().numpy()
+    assert np.array_equal(d32.view(np.uint32), (1.0 / vals_o[:n]).astype(np.float32).view(np.uint32))
+    assert o_dinv32 + al(4 * n) == M.buf.numel()
     sc = slice(512 + 32 * w.nz, 512 + 32 * w.nz + 24)        # |entry|max bits, fp16 scale, 1/scale
     assert bool((M.buf[sc] == B.buf[sc]).all())
     s_imp = M.buf[512 + 8 * w.nz: 512 + 16 * w.nz].view(np_to_torch_f64()).cpu().numpy()

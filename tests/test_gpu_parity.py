@@ -69,6 +69,11 @@ def test_build_dia_bit_exact(kw):
     assert np.array_equal(v32.view(np.uint32), vals_o.astype(np.float32).view(np.uint32))
     d0 = vals_o[:w.n]
     assert np.array_equal(inv.cpu().numpy(), 1.0 / d0)
+    # the fp32 copy of 1/D0 (last section of the object): round-to-nearest-even of the fp64 reciprocal
+    import torch
+    tail = (4 * w.n + 255) // 256 * 256
+    d32 = M.buf[M.buf.numel() - tail: M.buf.numel() - tail + 4 * w.n].view(torch.float32).cpu().numpy()
+    assert np.array_equal(d32.view(np.uint32), (1.0 / d0).astype(np.float32).view(np.uint32))
 
 
 # ---------------------------------------------------------------- a1: SpMV
