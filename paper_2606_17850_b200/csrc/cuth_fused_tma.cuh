@@ -147,7 +147,19 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
   int hr = 0, hc = 0, hbr = 0, hbc = 0;                // rim cell: place in the p' ring / in the vector boxes
   double pc0 = 0.0, pc1 = 0.0, pl0 = 0.0, pl1 = 0.0, a3l0 = 0.0, a3l1 = 0.0;
   double2 dcur = make_double2(0.0, 0.0);               // fp64 operator: D0 of the plane mu is formed for
-  double2 xnext = make_double2(0.0, 0.0);              // x of the plane the NEXT step forms p' for
+  // x is the caller's buffer (no tensor map): plain loads, issued TWO p'-planes ahead -- across tile boundaries too, so that
+  // no step ever waits for HBM (round 2a loaded plane 0 of every tile synchronously: ~1 us of the ~17 us of a tile)
+  double2 xq0 = make_double2(0.0, 0.0), xq1 = xq0;     // x of the plane of this step / of the next p'-step
+  auto tile_col = [&](int kk, bool* o) -> int64_t {    // first row of this thread's pair in tile kk; *o: inside the grid
+    const int t = (int)blockIdx.x + kk * (int)gridDim.x;
+    const int xx = (t % tiles_x) * K1X + 2 * tx, yy = (t / tiles_x) * K1Y + ty;
+    *o = xx < nxi && yy < nyi;
+    return *o ? xx + nx * (int64_t)yy : 0;
+  };
+  if (my_tiles > 0) {
+    bool on; const int64_t c0 = tile_col(0, &on);
+    if (on) { xq0 = ldd2(xg + c0); xq1 = ldd2(xg + c0 + np); }       // nz >= 2
+  }
   uint32_t ph = 0;                                     // bit S: parity of the next fill of stage S
   int slot = 0, j = 0, k = 0;
   int rw = 0, rr = kK1Ring - 1;                        // ring plane written in this step / written in the step before
@@ -169,7 +181,6 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
       halo_in = halo_role && hx >= 0 && hx < nxi && hy >= 0 && hy < nyi;
       hbr = hr; hbc = hc;                              // the ring and the boxes share their origin (x0-2, y0-1)
       pc0 = pc1 = pl0 = pl1 = a3l0 = a3l1 = 0.0;
-      if (own) xnext = ldd2(xg + col);                 // plane 0: no step before it to prefetch in
     }
     const bool has_p = j < nz, has_mu = j >= 1;
     const int64_t ip = col + (int64_t)j * np;          // rows of plane j (p', x) ; plane j - 1 is ip - np (mu)
@@ -177,7 +188,7 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
     mbar_wait(&sm.full[slot], (ph >> slot) & 1u);
     ph ^= 1u << slot;
     const ST& S = sm.st[slot];
-    double2 ro = make_double2(0.0, 0.0), po = ro, dd = make_double2(1.0, 1.0), xo = xnext;
+    double2 ro = make_double2(0.0, 0.0), po = ro, dd = make_double2(1.0, 1.0), xo = xq0;
     double rh = 0.0, phh = 0.0, dh = 1.0;
     if (has_p) {
       ro = *reinterpret_cast<const double2*>(&S.vz[ty + 1][sc0]);
@@ -185,7 +196,9 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
       if (MIXED) dd = ldf2(reinterpret_cast<const float*>(&S.vd[ty + 1][ST::VDX + 2 * tx]));
       else dd = *reinterpret_cast<const double2*>(&S.vd[ty + 1][sc0]);
       if (halo_role) { rh = S.vz[hbr][hbc]; phh = S.vp[hbr][hbc]; dh = (double)S.vd[hbr][hbc + ST::VDX - 2]; }
-      if (own && j + 1 < nz) xnext = ldd2(xg + ip + np);            // prefetch for the next step
+      xq0 = xq1;                                                    // x for the p'-plane two steps ahead
+      if (j + 2 < nz) { if (own) xq1 = ldd2(xg + ip + 2 * np); }
+      else if (k + 1 < my_tiles) { bool on; const int64_t cn = tile_col(k + 1, &on); if (on) xq1 = ldd2(xg + cn + (int64_t)(j + 2 - nz) * np); }
     }
     double2 a1 = make_double2(0.0, 0.0), a2u = a1, a2l = a1, a3u = a1;
     double a1l = 0.0;
