@@ -401,6 +401,7 @@ struct Plan {
   int pair_tma = 0;      // the two-pass Chebyshev nodes are the TMA kernel
   int k1tma = 0;         // K1 is the TMA-staged kernel
   int unroll = 1;        // K1 + K2 pairs per pass of the WHILE body (fused path without Chebyshev)
+  int k2blocks = 0;      // grid of K2 (one resident wave)
   const void* dia = nullptr;   // matrix the tensor maps of the TMA nodes were made for (else nullptr)
   int64_t tnx = 0, tny = 0;    // ... and its plane dimensions
   int tocc = 0;                // ... occupancy * 100 + region rows of the TMA two-pass nodes
@@ -408,7 +409,7 @@ struct Plan {
   bool operator==(const Plan& o) const {
     return n == o.n && sblocks == o.sblocks && fblocks == o.fblocks && k1x2 == o.k1x2 && chebkey == o.chebkey &&
            cblocks == o.cblocks && x2blocks == o.x2blocks && pblocks == o.pblocks && with_b == o.with_b &&
-           pair_tma == o.pair_tma && k1tma == o.k1tma && unroll == o.unroll && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
+           pair_tma == o.pair_tma && k1tma == o.k1tma && unroll == o.unroll && k2blocks == o.k2blocks && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
   }
 };
 struct GraphEntry {
@@ -511,7 +512,7 @@ static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, co
         CU(add_kernel(body, &n_s, dep, ndep, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
       }
       void* a2[] = {&ctx, &ctl, &partials, &h_while, &h_if};
-      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, blocks, a2));
+      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, P.k2blocks, a2));
     }
   } else {
     { void* a[] = {&ctx, &ctl};
@@ -625,7 +626,7 @@ static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, 
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem);
   if (occ > max_per_sm) occ = max_per_sm;
-  int v = (coop || slot == 2) ? sms * occ : 0;          // slot 2 (the TMA K1) is an ordinary launch
+  int v = (coop || slot == 2 || slot == 4) ? sms * occ : 0;   // slots 2, 4 (TMA K1, K2) are ordinary launches
   if (v > cap) v = cap;
   g_coresident[key] = v;
   return v;
@@ -634,6 +635,14 @@ static int fused_tma_blocks(const DiaLayout& L) {
   const int64_t tiles = ((L.nx + K1X - 1) / K1X) * ((L.ny + K1Y - 1) / K1Y);
   const int resident = coresident_blocks(2, (const void*)k_fused_pspmv_tma, 2, kMaxBlocks, k1_tma_dyn_smem());
   return (int)(tiles < resident ? tiles : (resident > 0 ? resident : 1));
+}
+// Grid of K2 (k_update<false>, a pure stream): exactly ONE wave of resident CTAs striding over the rows.  Measured at cfg 3
+// (B200): 1184 CTAs = two waves 0.0905 ms (late stage) / 0.0849 (early), 592 CTAs = one wave 0.0861 / 0.0809; four instead of
+// two row pairs per trip were slower in every combination.
+static int k2_blocks(int64_t n) {
+  const int resident = coresident_blocks(4, (const void*)k_update<false>, 8, kMaxBlocks);
+  const int want = grid_blocks(n);
+  return resident > 0 && resident < want ? resident : want;
 }
 static int persistent_blocks(int64_t n) {
   const int all = coresident_blocks(0, (const void*)k_pcg_persistent, 4, kPersistMaxBlocks);
@@ -724,6 +733,7 @@ static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts
   P.pblocks = (cheb && cheb_pairs(L, code, T)) ? cheb_pair_blocks(L) : 0;
   P.with_b = with_b ? 1 : 0;
   P.unroll = (P.fblocks > 0 && !cheb) ? kGraphUnroll : 1;
+  P.k2blocks = k2_blocks(L.n);
   if (cheb && cheb_pairs_tma(L, code, T)) {
     P.pair_tma = 1;
     P.dia = dia_D; P.tnx = L.nx; P.tny = L.ny;
@@ -1103,7 +1113,7 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t
       } else if (fused_x2(L, T)) k_fused_pspmv_x2<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       else k_fused_pspmv<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       break;
-    case 5: k_update<false><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 5: k_update<false><<<k2_blocks(L.n), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
       const int code = kernel_id - 6;
       const bool x2 = code != 0 && cheb_x2(L, T);

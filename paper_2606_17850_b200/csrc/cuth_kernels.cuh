@@ -369,30 +369,34 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
     const bool m32 = ctl->stage == 0;
     double2* __restrict__ w2 = reinterpret_cast<double2*>(c.r);
     const bool jac = c.jacobi != 0;
-    for (int64_t base = (int64_t)blockIdx.x * (kThreads * 2); base < n2; base += (int64_t)gridDim.x * (kThreads * 2)) {
-      const int64_t i0 = base + threadIdx.x, i1 = i0 + kThreads;
-      const bool h0 = i0 < n2, h1 = i1 < n2;
+#ifndef CUTH_K2_PAIRS
+#define CUTH_K2_PAIRS 2
+#endif
+    constexpr int NP = CUTH_K2_PAIRS;
+    for (int64_t base = (int64_t)blockIdx.x * (kThreads * NP); base < n2; base += (int64_t)gridDim.x * (kThreads * NP)) {
       const double2 one = make_double2(1.0, 1.0), zero = make_double2(0.0, 0.0);
-      const double2 ra = h0 ? r2[i0] : zero, ma = h0 ? __ldcs(&m2[i0]) : zero;
-      const double2 rb = h1 ? r2[i1] : zero, mb = h1 ? __ldcs(&m2[i1]) : zero;
-      double2 da = one, db = one;
-      if (jac) {
-        if (m32) {
-          if (h0) { const float2 f = f2[i0]; da = make_double2((double)f.x, (double)f.y); }
-          if (h1) { const float2 f = f2[i1]; db = make_double2((double)f.x, (double)f.y); }
-        } else {
-          if (h0) da = d2[i0];
-          if (h1) db = d2[i1];
+      double2 rv[NP], mv[NP], dv[NP];
+      bool h[NP];
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const int64_t i = base + threadIdx.x + (int64_t)q * kThreads;
+        h[q] = i < n2;
+        rv[q] = h[q] ? r2[i] : zero;
+        mv[q] = h[q] ? __ldcs(&m2[i]) : zero;
+        dv[q] = one;
+        if (jac && h[q]) {
+          if (m32) { const float2 f = f2[i]; dv[q] = make_double2((double)f.x, (double)f.y); }
+          else dv[q] = d2[i];
         }
       }
-      const double a0 = fma(-alpha, ma.x, ra.x), a1 = fma(-alpha, ma.y, ra.y);
-      const double b0 = fma(-alpha, mb.x, rb.x), b1 = fma(-alpha, mb.y, rb.y);
-      if (h0) w2[i0] = make_double2(a0, a1);
-      if (h1) w2[i1] = make_double2(b0, b1);
-      acc[0] = fma(a0, a0 * da.x, acc[0]); acc[1] = fma(a0, a0, acc[1]);
-      acc[0] = fma(a1, a1 * da.y, acc[0]); acc[1] = fma(a1, a1, acc[1]);
-      acc[0] = fma(b0, b0 * db.x, acc[0]); acc[1] = fma(b0, b0, acc[1]);
-      acc[0] = fma(b1, b1 * db.y, acc[0]); acc[1] = fma(b1, b1, acc[1]);
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const int64_t i = base + threadIdx.x + (int64_t)q * kThreads;
+        const double a0 = fma(-alpha, mv[q].x, rv[q].x), a1 = fma(-alpha, mv[q].y, rv[q].y);
+        if (h[q]) w2[i] = make_double2(a0, a1);
+        acc[0] = fma(a0, a0 * dv[q].x, acc[0]); acc[1] = fma(a0, a0, acc[1]);
+        acc[0] = fma(a1, a1 * dv[q].y, acc[0]); acc[1] = fma(a1, a1, acc[1]);
+      }
     }
   } else {
   CUTH_TILE_LOOP(c.A.n) {
