@@ -31,8 +31,8 @@ import workloads as W  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of the dominant
 # kernel (profiles/r1e_cfg3_fp64_k1x2.md, r1d, r1c); null for workloads/kernels not captured.
-NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3201e9,   # profiles/r2b_k1_tma.md (TMA-staged K1)
-                     ("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "mixed"): 1.1131e9,  # profiles/r2b_k1_tma.md (fp32-stored operator)
+NCU_TRAFFIC_BYTES = {("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "fp64"): 1.3200e9,   # profiles/r2d_cfg3_mixed_final.md (TMA-staged K1)
+                     ("cfg3_steady_1024x1024x16_lognormal", "k_fused_pspmv", "mixed"): 1.0412e9,  # profiles/r2d_cfg3_mixed_final.md (fp32-stored operator)
                      ("cfg3_steady_1024x1024x16_lognormal", "k_cheb_pair", "mixed"): 518.3e6,    # profiles/r1i_cfg3_default_and_cheb16.md
                      ("cfg4_steady_4096x4096x8", "k_cheb_pair", "mixed"): 4.477e9,                 # profiles/r1h_cheb_pair_tma.md
                      ("cfg4_steady_4096x4096x8", "k_fused_pspmv", "fp64"): 10.786e9,               # profiles/r1j_cfg4_fp64_k1.md
