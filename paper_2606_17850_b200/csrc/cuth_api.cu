@@ -733,6 +733,14 @@ static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts
   P.pblocks = (cheb && cheb_pairs(L, code, T)) ? cheb_pair_blocks(L) : 0;
   P.with_b = with_b ? 1 : 0;
   P.unroll = (P.fblocks > 0 && !cheb) ? kGraphUnroll : 1;
+  if (P.unroll > 1 && (opts->precision == CUTH_MIXED || opts->precision == CUTH_MIXED_STD32)) {
+    // Early stage: every `period` iterations the pass ends in the true-residual branch.  A body whose length divides
+    // the period has no halted (no-op) launches in front of that branch: T = 5 (transient) and T = 20 (steady) -> 5.
+    const int period = opts->true_resid_period > 0 ? opts->true_resid_period : 20;
+    if (period % 5 == 0) P.unroll = 5;
+    else if (period % 4 != 0 && period % 6 == 0) P.unroll = 6;
+    else if (period % 4 != 0 && period % 3 == 0) P.unroll = 3;
+  }
   P.k2blocks = k2_blocks(L.n);
   if (cheb && cheb_pairs_tma(L, code, T)) {
     P.pair_tma = 1;

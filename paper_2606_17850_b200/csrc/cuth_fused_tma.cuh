@@ -156,7 +156,8 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
     *o = xx < nxi && yy < nyi;
     return *o ? xx + nx * (int64_t)yy : 0;
   };
-  if (my_tiles > 0) {
+  const bool do_x = xalpha != 0.0;                     // nothing pending (first iteration, or K2 / k_flush_x applied it): x untouched
+  if (my_tiles > 0 && do_x) {
     bool on; const int64_t c0 = tile_col(0, &on);
     if (on) { xq0 = ldd2(xg + c0); xq1 = ldd2(xg + c0 + np); }       // nz >= 2
   }
@@ -197,7 +198,8 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
       else dd = *reinterpret_cast<const double2*>(&S.vd[ty + 1][sc0]);
       if (halo_role) { rh = S.vz[hbr][hbc]; phh = S.vp[hbr][hbc]; dh = (double)S.vd[hbr][hbc + ST::VDX - 2]; }
       xq0 = xq1;                                                    // x for the p'-plane two steps ahead
-      if (j + 2 < nz) { if (own) xq1 = ldd2(xg + ip + 2 * np); }
+      if (!do_x) {}
+      else if (j + 2 < nz) { if (own) xq1 = ldd2(xg + ip + 2 * np); }
       else if (k + 1 < my_tiles) { bool on; const int64_t cn = tile_col(k + 1, &on); if (on) xq1 = ldd2(xg + cn + (int64_t)(j + 2 - nz) * np); }
     }
     double2 a1 = make_double2(0.0, 0.0), a2u = a1, a2l = a1, a3u = a1;
@@ -229,7 +231,7 @@ __device__ __forceinline__ void fused_pspmv_tma_body(const Ctx& c, K1Smem<MIXED>
         const double z1 = jac ? (MIXED ? ro.y * dd.y : ro.y * rcp_diag(dd.y)) : ro.y;
         ph0 = fma(beta, po.x, z0); ph1 = fma(beta, po.y, z1);
         std2(p_out + ip, ph0, ph1);
-        std2(xg + ip, fma(xalpha, po.x, xo.x), fma(xalpha, po.y, xo.y));
+        if (do_x) std2(xg + ip, fma(xalpha, po.x, xo.x), fma(xalpha, po.y, xo.y));
       }
       std2(&sm.sp[rw][ty + 1][sc0], ph0, ph1);
       if (halo_role) {
@@ -308,7 +310,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_fused_pspmv_tma(
   }
   if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], red, flag) && threadIdx.x == 0) {
     ctl->pcur = pcur ^ 1;
-    policy_after_spmv(ctl, acc[0], true);       // Alg. 1 line 7; x += alpha p deferred to the next K1
+    policy_after_spmv(ctl, acc[0], true, &c);   // Alg. 1 line 7; x += alpha p deferred to the next K1 (or to K2: xnow)
   }
 }
 

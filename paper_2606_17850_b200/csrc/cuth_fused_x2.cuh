@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_fused_pspmv_x2(const Ctx* __res
   else fused_pspmv_x2_body<false>(c, p_in, p_out, beta, xalpha, sp, acc[0]);
   if (grid_sum_last_block<1>(acc, partials, &ctl->ticket[1], smem, &s_flag) && threadIdx.x == 0) {
     ctl->pcur = pcur ^ 1;
-    policy_after_spmv(ctl, acc[0], true);       // Alg. 1 line 7; x += alpha p deferred to the next K1
+    policy_after_spmv(ctl, acc[0], true, &c);   // Alg. 1 line 7; x += alpha p deferred to the next K1 (or to K2: xnow)
   }
 }
 

@@ -121,6 +121,7 @@ struct Ctl {
   int32_t it, stage, status, want_true, restart, exiting, promotions, evals, since_eval;
   int32_t switch_reason, switch_it, conv_rec, zero_rhs, no_graph, pcur, beta_zero, switch_mask;
   int32_t hard_restarts, soft_restarts, refused;
+  int32_t xnow;    // fused path: K2 of this iteration applies x += alpha p itself (an evaluation is certain to follow)
   int32_t halt;    // graph loop with an unrolled body: the remaining K1 / K2 launches of this pass are no-ops
                    // (the loop must stop, or the true-residual branch at the end of the body must run first)
   unsigned int ticket[8];

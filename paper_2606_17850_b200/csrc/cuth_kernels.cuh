@@ -357,6 +357,24 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
   const Ctx c = *ctxp;
   const double alpha = ctl->alpha;
   double acc[2] = {0.0, 0.0};
+  if (!UPDATE_X && ctl->xnow) {
+    // Fused path, an evaluation of the true residual is certain to follow this iteration (policy_after_spmv): Alg. 1
+    // line 8 here instead of in the next K1 -- p' is the buffer K1 has just written (most of it still in L2).
+    const double* __restrict__ pn = ctl->pcur ? c.p2 : c.p;
+    CUTH_TILE_LOOP(c.A.n) {
+      double xv[kRows], pv[kRows];
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        xv[k] = i < c.A.n ? c.x[i] : 0.0; pv[k] = i < c.A.n ? pn[i] : 0.0;
+      }
+#pragma unroll
+      for (int k = 0; k < kRows; ++k) {
+        const int64_t i = base + threadIdx.x + k * kThreads;
+        if (i < c.A.n) c.x[i] = fma(alpha, pv[k], xv[k]);
+      }
+    }
+  }
   if (!UPDATE_X && (c.A.n & 1) == 0) {
     // K2 of the fused path (32 B/row, nothing but streaming): rows in pairs as 16-byte accesses, two pairs per thread
     // per trip with all six loads issued before the first store -- 96 bytes in flight per thread instead of 48.

@@ -39,17 +39,26 @@ __device__ __forceinline__ unsigned policy_init(Ctl* ctl, const Ctx& c, double r
   return go;
 }
 
-// After mu = A p: Alg. 1 line 7.
-__device__ __forceinline__ void policy_after_spmv(Ctl* ctl, double pAp, bool defer_x) {
+// After mu = A p: Alg. 1 line 7.  defer_x (fused path): x += alpha p is left to the NEXT K1, which has p in registers
+// anyway -- unless this iteration is certain to end in a true-residual evaluation (period reached in the early stage,
+// or the iteration cap): then K2 applies it at once (ctl->xnow), k_flush_x finds nothing pending and the next K1,
+// seeing xalpha = 0, neither reads nor writes x.  Same fma on the same operands either way: identical iterates.
+__device__ __forceinline__ void policy_after_spmv(Ctl* ctl, double pAp, bool defer_x, const Ctx* c = nullptr) {
   ctl->pAp = pAp;
   const double rho = ctl->rho;
+  ctl->xnow = 0;
   if (!(pAp > 0.0) || !(pAp <= 1.79e308) || !(rho == rho)) {
     ctl->alpha = 0.0; ctl->xalpha = 0.0;
     ctl->status = CUTH_SOLVE_BREAKDOWN;
   } else {
     const double alpha = rho / pAp;
     ctl->alpha = alpha;
-    if (defer_x) ctl->xalpha = alpha;            // fused path: x += alpha p is applied by the next K1
+    if (defer_x) {
+      const bool now = c && !ctl->no_graph &&
+                       ((ctl->stage == 0 && ctl->since_eval + 1 >= c->period) || ctl->it + 1 >= c->max_iters);
+      ctl->xnow = now ? 1 : 0;
+      ctl->xalpha = now ? 0.0 : alpha;
+    }
   }
 }
 
