@@ -351,8 +351,9 @@ def main():
     ap.add_argument("--profile-iters", type=int, default=0,
                     help="after the timed solves, replay this many loop bodies kernel by kernel OUTSIDE the "
                          "graph (ncu cannot see kernel nodes of graphs with conditional nodes)")
-    ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1, 2],
-                    help="cuth_tuning_t.loop_mode: 0 automatic, 1 CUDA graph, 2 persistent kernel wherever the flat traversal applies")
+    ap.add_argument("--loop-mode", type=int, default=0, choices=[0, 1, 2, 3, 4],
+                    help="cuth_tuning_t.loop_mode: 0 automatic, 1 CUDA graph, 2 persistent kernel wherever the flat traversal applies, "
+                         "3 cluster-resident kernel, 4 its shared-memory form")
     ap.add_argument("--k1-variant", type=int, default=0, choices=[0, 1, 2, 3],
                     help="cuth_tuning_t.k1_variant: 0 auto, 1 one column per thread, 2 two columns (TMA-staged K1 when "
                          "nx %% 4 == 0), 3 two columns with ordinary loads")

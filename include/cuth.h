@@ -95,7 +95,9 @@ typedef struct {
                                  conditional nodes beyond; grids whose rows fit the shared memory of one 8-CTA
                                  thread-block cluster -- about 13 k rows, BASELINE cfg 1 -- run as ONE cluster-resident
                                  kernel, Jacobi / no preconditioner), 1 graph, 2 persistent kernel wherever the flat
-                                 traversal applies, 3 cluster-resident kernel (CUTH_ERR_VALUE when the grid does not fit) */
+                                 traversal applies, 3 cluster-resident kernel (CUTH_ERR_VALUE when the grid does not fit; rows
+                                 in registers up to 1024 rows per CTA, in shared memory beyond), 4 the cluster-resident
+                                 kernel with the rows in shared memory whatever the size */
   int32_t k1_variant;         /* z-marching kernels: 0 automatic (K1 with TMA-staged operands when nx % 4 == 0 and the
                                  plane has >= 288 tiles of 64 x 8 columns; else two x-adjacent columns per thread when nx
                                  is even and there are >= 2048 tiles; else one column), 1 one column per thread,

@@ -22,6 +22,7 @@
 #include "cuth_persistent.cuh"
 #include "cuth_fixed32.cuh"
 #include "cuth_cluster.cuh"
+#include "cuth_cluster_reg.cuh"
 #include "cuth_batch.cuh"
 
 namespace cuth {
@@ -47,7 +48,7 @@ static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 // Kernel variants of one call (cuth_tuning_t, validated): nothing here is process-wide.
 struct Tune {
   int traversal = 0;    // 0 auto, 1 flat, 2 z-march
-  int loop_mode = 0;    // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel, 3 cluster-resident kernel
+  int loop_mode = 0;    // 0 auto, 1 CUDA graph, 2 persistent cooperative kernel, 3 cluster-resident kernel, 4 its shared-memory form
   int k1_variant = 0;   // 0 auto, 1 one column per thread, 2 two columns, 3 two columns without the TMA-staged K1
   int cheb_pairs = 0;   // 0 auto, 1 never, 2 always (fp32 modes)
   int pair_tma = 0;     // 0 auto (TMA when possible), 1 never
@@ -58,7 +59,7 @@ struct Tune {
 static int make_tune(const cuth_tuning_t* t, Tune* T) {
   *T = Tune();
   if (!t) return CUTH_OK;
-  if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 3 || t->k1_variant < 0 ||
+  if (t->traversal < 0 || t->traversal > 2 || t->loop_mode < 0 || t->loop_mode > 4 || t->k1_variant < 0 ||
       t->k1_variant > 3 || t->cheb_fusion < 0 || t->cheb_fusion > 3 ||
       (t->pair_rows != 0 && t->pair_rows != 8 && t->pair_rows != 16) ||
       (t->pair_occupancy != 0 && (t->pair_occupancy < 2 || t->pair_occupancy > 4)) || t->lanczos_fp32 < 0 ||
@@ -663,28 +664,62 @@ static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune&
 // One cluster per solve (nsolves > 1: cuth_pcg_solve_batch, contexts and control blocks as arrays).  8 CTAs when the
 // rows fit them, else 16 (non-portable cluster size): measured at cfg 1 (8 192 rows) 4.41 us per iteration with 8 CTAs
 // against 4.88 with 16 -- the all-reduce across CTAs costs more than the halved row work saves.
-static cudaError_t launch_cluster(const DiaLayout& L, const Ctx* ctxp, Ctl* ctlp, int nsolves, cudaStream_t st) {
+// Up to 1024 rows per CTA the rows live in registers (cuth_cluster_reg.cuh); beyond, or with loop_mode = 4, in shared
+// memory (cuth_cluster.cuh).  The candidates are tried in the measured order of speed until one launches (a 16-CTA
+// cluster is a non-portable size and may be refused).  Measured at cfg 1 (8 192 rows, FP64 / MIXED, us per iteration):
+// 16 CTAs x 256 threads 2.17 / 2.32, 16 x 512 (one row per thread) 2.46 / 2.64, 8 x 512 2.59 / 2.78, shared-memory form
+// 8 x 1024 3.91 / 4.12 -- FP64 adds, 64-bit shuffles and distributed-shared-memory bytes per SM are the narrow resources,
+// so spreading the rows over 16 SMs wins although the all-reduce has twice the partners.  A batch is a different matter:
+// a 16-CTA cluster takes a whole GPC where two 8-CTA ones share it, so the form whose (waves of co-resident clusters) x
+// (relative time of one solve: 1 for 16 x 256, 1.2 for 8 x 512) is smaller goes first.
+struct ClusterForm { int nc, threads; const void* fn; };     // threads = 1024: the shared-memory form
+static bool cluster_form_config(const ClusterForm& f, const DiaLayout& L, int nsolves, cudaStream_t st, cudaLaunchConfig_t* cfg,
+                                cudaLaunchAttribute* at, int* rows) {
+  const bool reg = f.threads != kClusterThreads;
+  *rows = (int)cluster_rows_per_cta(L.nx, L.ny, L.nz, f.nc);
+  const size_t smem = reg ? cluster_reg_smem_bytes(*rows) : cluster_smem_bytes(*rows);
+  if (cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      (f.nc > 8 && cudaFuncSetAttribute(f.fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+    cudaGetLastError();
+    return false;
+  }
+  memset(cfg, 0, sizeof *cfg);
+  cfg->gridDim = dim3((unsigned)(f.nc * nsolves)); cfg->blockDim = dim3((unsigned)f.threads);
+  cfg->dynamicSmemBytes = smem; cfg->stream = st;
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = f.nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg->attrs = at; cfg->numAttrs = 1;
+  return true;
+}
+// Clusters of this form that can be resident at once on the current device (0: unknown).
+static int cluster_form_resident(const ClusterForm& f, const DiaLayout& L) {
+  cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1]; int rows = 0, nclu = 0;
+  if (!cluster_form_config(f, L, 1, nullptr, &cfg, at, &rows)) return 0;
+  if (cudaOccupancyMaxActiveClusters(&nclu, f.fn, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+  return nclu;
+}
+static cudaError_t launch_cluster(const DiaLayout& L, const Ctx* ctxp, Ctl* ctlp, int nsolves, cudaStream_t st,
+                                  bool allow_reg) {
+  const ClusterForm r8 = {8, 512, (const void*)k_pcg_cluster_reg<8, 512>}, r16h = {16, 256, (const void*)k_pcg_cluster_reg<16, 256>},
+                    r16 = {16, 512, (const void*)k_pcg_cluster_reg<16, 512>}, s8 = {8, kClusterThreads, (const void*)k_pcg_cluster<8>},
+                    s16 = {16, kClusterThreads, (const void*)k_pcg_cluster<16>};
+  const ClusterForm one[] = {r16h, r8, r16, s8, s16}, many[] = {r8, r16h, r16, s8, s16};
+  bool eight_first = false;
+  if (nsolves > 1 && allow_reg && cluster_reg_fits(L.nx, L.ny, L.nz, 16, 256) && cluster_reg_fits(L.nx, L.ny, L.nz, 8, 512)) {
+    const int c16 = cluster_form_resident(r16h, L), c8 = cluster_form_resident(r8, L);
+    if (c16 > 0 && c8 > 0) eight_first = 1.2 * ((nsolves + c8 - 1) / c8) < 1.0 * ((nsolves + c16 - 1) / c16);
+    else eight_first = nsolves > 8;
+  }
+  const ClusterForm (&forms)[5] = eight_first ? many : one;
   cudaError_t e = cudaErrorInvalidValue;
-  for (int nc = 8; nc <= kClusterMaxCtas && e != cudaSuccess; nc *= 2) {
-    if (!cluster_fits(L.nx, L.ny, L.nz, nc)) continue;
-    const void* fn = nc == 16 ? (const void*)k_pcg_cluster<16> : (const void*)k_pcg_cluster<8>;
-    int rows = (int)cluster_rows_per_cta(L.nx, L.ny, L.nz, nc);
-    const size_t smem = cluster_smem_bytes(rows);
-    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-        (nc > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
-      cudaGetLastError();
-      continue;
-    }
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
-    cfg.gridDim = dim3((unsigned)(nc * nsolves)); cfg.blockDim = dim3(kClusterThreads);
-    cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeClusterDimension;
-    at[0].val.clusterDim.x = nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+  for (const ClusterForm& f : forms) {
+    if (e == cudaSuccess) break;
+    const bool reg = f.threads != kClusterThreads;
+    if (reg ? !(allow_reg && cluster_reg_fits(L.nx, L.ny, L.nz, f.nc, f.threads)) : !cluster_fits(L.nx, L.ny, L.nz, f.nc)) continue;
+    cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1]; int rows = 0;
+    if (!cluster_form_config(f, L, nsolves, st, &cfg, at, &rows)) continue;
     void* args[] = {(void*)&ctxp, (void*)&ctlp, (void*)&rows};
-    e = cudaLaunchKernelExC(&cfg, fn, args);
+    e = cudaLaunchKernelExC(&cfg, f.fn, args);
     if (e != cudaSuccess) cudaGetLastError();
   }
   return e;
@@ -692,7 +727,7 @@ static cudaError_t launch_cluster(const DiaLayout& L, const Ctx* ctxp, Ctl* ctlp
 
 static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
   const int mode = T.loop_mode, trav = T.traversal;
-  if (cheb || mode == 1 || mode == 3 || trav == 2) return false;
+  if (cheb || mode == 1 || mode >= 3 || trav == 2) return false;
   if (persistent_blocks(L.n) <= 0) return false;
   if (mode == 2) return !use_zmarch(L, T);        // forced: wherever the flat traversal applies
   // Measured on B200: per iteration, persistent kernel / graph with conditional nodes:
@@ -811,12 +846,12 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
     return CUTH_OK;
   }
   if (use_cluster(L, opts, T)) {
-    const cudaError_t e = launch_cluster(L, w.ctx, w.ctl, 1, st);
+    const cudaError_t e = launch_cluster(L, w.ctx, w.ctl, 1, st, T.loop_mode != 4);
     if (e == cudaSuccess) return CUTH_OK;
-    if (T.loop_mode == 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster)");
+    if (T.loop_mode >= 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster)");
     // automatic mode: fall through to the persistent kernel / the graph
-  } else if (T.loop_mode == 3) {
-    g_last_err = "loop_mode 3: the grid does not fit one cluster, or the options are not served by the cluster kernel";
+  } else if (T.loop_mode >= 3) {
+    g_last_err = "loop_mode 3 / 4: the grid does not fit one cluster, or the options are not served by the cluster kernel";
     return CUTH_ERR_VALUE;
   }
   if (use_persistent(L, cheb, T)) {
@@ -1044,9 +1079,9 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
     Ctx* ctxs = reinterpret_cast<Ctx*>(w.partials);
     k_set_ctx_batch<<<1, kBatchMaxRhs, 0, st>>>(base, ctxs, w.ctl, nrhs);
     CU(cudaGetLastError());
-    const cudaError_t e = launch_cluster(L, ctxs, w.ctl, nrhs, st);
+    const cudaError_t e = launch_cluster(L, ctxs, w.ctl, nrhs, st, T.loop_mode != 4);
     if (e == cudaSuccess) return CUTH_OK;
-    if (T.loop_mode == 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster, batch)");
+    if (T.loop_mode >= 3) return cuda_fail(e, "cudaLaunchKernelExC(k_pcg_cluster, batch)");
   }
   // co-resident CTAs available, split into ceil(nrhs / S) chunks x ntiles row tiles
   const int max_blocks = coresident_blocks(1, (const void*)k_pcg_batch, 3, 1 << 20);
@@ -1323,7 +1358,7 @@ int cuth_loop_home(const cuth_grid_t* grid, const cuth_opts_t* opts) {
   if (opts->precision == CUTH_FIXED32) return 4;
   if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
   if (use_cluster(L, opts, T)) return 3;
-  if (T.loop_mode == 3) return CUTH_ERR_VALUE;
+  if (T.loop_mode >= 3) return CUTH_ERR_VALUE;
   return use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T) ? 2 : 1;
 }
 

@@ -38,7 +38,7 @@ struct ClusterSmem {
   Ctl ctl[kClusterThreads / 32];                        // one replica per warp
   double red[2][3][kClusterMaxCtas];                    // [parity][value][source CTA]
   double wsum[3][32];                                   // per-warp partial sums
-  uint64_t bar;                                         // mbarrier: NC arrivals per reduction phase
+  uint64_t bar[2];                                      // mbarriers of the all-reduce, used alternately
   Ctx ctx;                                              // the call's context: the policy code reads its options from
                                                         // here, not from global memory (every cluster barrier
                                                         // invalidates L1, an L2 round trip per field otherwise)
@@ -69,64 +69,125 @@ inline bool cluster_fits(int64_t nx, int64_t ny, int64_t nz, int nc) {
 
 #ifdef __CUDACC__
 
-// Sum of NV values over the whole cluster, identical in every thread of every CTA; also a cluster-wide barrier with
-// release / acquire semantics for every shared-memory write made before the call.
+// Sum of NV values over the whole cluster, identical in every thread of every CTA; also a cluster-wide barrier for every
+// shared-memory write made before the call.
 // NOT barrier.cluster: measured on B200 with 16 CTAs x 32 warps, an all-reduce built on cluster.sync() costs 2 700 -
-// 3 500 cycles (every warp of every CTA takes part in the hardware barrier).  Here only 16 lanes per CTA talk across
-// CTAs: after the block-level sum, lane q of warp 0 stores the CTA's partial into CTA q's slot (a remote store) and
-// ARRIVES on CTA q's mbarrier (mbarrier.arrive.release.cluster on a shared::cluster address); every thread then waits
-// on its OWN CTA's mbarrier (acquire.cluster) for the NC arrivals of the phase.  Nobody can pass before every CTA has
-// arrived -- which it does only after its __syncthreads, i.e. after all its reads and writes of the phase -- so it is
-// a full barrier; a CTA can be at most one phase ahead of another, hence two slots and one mbarrier.
+// 3 500 cycles (every warp of every CTA takes part in the hardware barrier).  Here only NC lanes per CTA talk across
+// CTAs: after the block-level sum, lane q of warp 0 sends the CTA's partial into CTA q's slot with st.async -- a remote
+// store that carries its own completion signal: the 8 bytes are counted on CTA q's mbarrier (complete_tx) when they have
+// landed -- and every thread waits on its OWN CTA's mbarrier, on which one local thread has announced the NC * NV * 8
+// bytes of the phase (arrive.expect_tx).
+//   * Round 2a used plain remote stores followed by mbarrier.arrive.release.cluster on the remote barrier: ptxas turns
+//     that release into MEMBAR.ALL.GPU (+ CCTL.IVALL after the acquire.cluster wait), a GPU-scope fence twice per
+//     iteration: cfg 1 in the register form 3.29 -> 2.64 us per iteration, in the shared-memory form 4.53 -> 3.97.
+//   * Barrier property: a CTA sends only after its __syncthreads, i.e. after all its reads and writes of the phase (the
+//     barrier instruction drains the CTA's shared-memory stores), and nobody passes before the bytes of every CTA have
+//     landed; what the others then read remotely are ordinary shared-memory words written before that barrier.
+//   * Two mbarriers, used alternately: a CTA can be one reduction ahead of another (never two -- to pass reduction n + 1
+//     it needs every CTA's bytes of n + 1, sent after their wait of n), so its bytes for n + 1 must not count towards a
+//     neighbour's still incomplete n.  `n` = index of the reduction: barrier n & 1, phase parity (n >> 1) & 1.
 __device__ __forceinline__ uint32_t cl_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cl_remote_arrive(uint64_t* local_bar, unsigned rank) {
-  uint32_t raddr;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(cl_smem_u32(local_bar)), "r"(rank));
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(raddr) : "memory");
+__device__ __forceinline__ uint32_t cl_mapa(uint32_t local_addr, unsigned rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cl_st_async(uint32_t remote_addr, double v, uint32_t remote_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(remote_addr), "d"(v),
+               "r"(remote_bar) : "memory");
+}
+__device__ __forceinline__ void cl_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(cl_smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void cl_wait(uint64_t* bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred p;\n"
       "CL_WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
       "@p bra CL_WAIT_DONE;\n"
       "bra CL_WAIT_LOOP;\n"
       "CL_WAIT_DONE:\n"
       "}\n" ::"r"(cl_smem_u32(bar)), "r"(parity) : "memory");
 }
+// Once per kernel, by one thread, before the cluster-wide barrier that precedes the first reduction.
+__device__ __forceinline__ void cluster_bars_init(ClusterSmem* sm) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(cl_smem_u32(&sm->bar[0])) : "memory");
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(cl_smem_u32(&sm->bar[1])) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
 
-template <int NC, int NV>
-__device__ __forceinline__ void cluster_allreduce(cg::cluster_group& cluster, ClusterSmem* sm, double (&v)[NV], int& parity) {
+// Butterfly over the low `W` lanes of each W-lane group (W a power of two <= 32): every lane ends with its group's sum.
+template <int W>
+__device__ __forceinline__ double group_sum(double v) {
+#pragma unroll
+  for (int o = W / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// FP64 adds and 64-bit shuffles are the narrow resources of this kernel (measured on B200: a dependent DADD ~25 cycles, a
+// 5-level fp64 shuffle tree 210-260 cycles, and with 16 warps per SM the pipes themselves saturate), so the reduction is
+// built to issue as few of them as possible:
+//   1. in the warp, NV = 2: after the first exchange half the lanes carry value 0 and the other half value 1 -- one
+//      butterfly for both values (10 shuffles + 5 adds per lane instead of 20 + 10);
+//   2. across the warps of the CTA: warp k sums value k's NW partials, log2(NW) levels;
+//   3. its lanes q < NC send the CTA's partial to CTA q (st.async, see above);
+//   4. after the wait, the NC partials of value k are summed by the lanes of a 16-lane group, log2(NC) levels, and
+//      broadcast -- NC loads and 2 NC adds per THREAD in round 2a.
+// Every sum is a balanced tree of fixed shape: bit-reproducible, identical in all threads of all CTAs.
+template <int NC, int NV, int NW = kClusterThreads / 32>      // NW: warps per CTA
+__device__ __forceinline__ void cluster_allreduce(cg::cluster_group& cluster, ClusterSmem* sm, double (&v)[NV], int& n, long long* pr = nullptr) {
+  static_assert(NV >= 1 && NV <= 3 && NC <= 16 && (NC & (NC - 1)) == 0 && (NW & (NW - 1)) == 0, "cluster_allreduce");
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int slot = n & 1;
+#ifdef CUTH_CLUSTER_PROF
+  long long q0 = clock64();
+#define ARK(i) if (pr) { long long q1 = clock64(); pr[i] += q1 - q0; q0 = q1; }
+#else
+#define ARK(i)
+#endif
+  // ---- 1. the warp
+  if (NV == 2) {
+    const bool hi = (lane & 16) != 0;
+    const double give = hi ? v[0] : v[1], keep = hi ? v[1] : v[0];
+    const double w = group_sum<16>(keep + __shfl_xor_sync(0xffffffffu, give, 16));     // lanes 0-15: value 0, lanes 16-31: value 1
+    if ((lane & 15) == 0) sm->wsum[lane >> 4][wid] = w;
+  } else {
 #pragma unroll
-  for (int k = 0; k < NV; ++k) v[k] = warp_sum(v[k]);
-  if (lane == 0) {
+    for (int k = 0; k < NV; ++k) v[k] = warp_sum(v[k]);
+    if (lane == 0) {
 #pragma unroll
-    for (int k = 0; k < NV; ++k) sm->wsum[k][wid] = v[k];
+      for (int k = 0; k < NV; ++k) sm->wsum[k][wid] = v[k];
+    }
   }
+  ARK(0)
   __syncthreads();
-  if (wid == 0) {
+  ARK(1)
+  // ---- 2, 3. the CTA, and out to the cluster
+  if (wid < NV) {
     const unsigned me = cluster.block_rank();
-    double t[NV];
-#pragma unroll
-    for (int k = 0; k < NV; ++k) t[k] = warp_sum(sm->wsum[k][lane]);   // 32 warps; butterfly: every lane holds the total
-    if (lane < NC) {
-      ClusterSmem* dst = cluster.map_shared_rank(sm, lane);
-#pragma unroll
-      for (int k = 0; k < NV; ++k) dst->red[parity][k][me] = t[k];     // remote stores into CTA `lane`
-      cl_remote_arrive(&sm->bar, (unsigned)lane);                      // release: the stores above, and (through the
-    }                                                                  // __syncthreads) every write of this CTA
+    const double t = group_sum<(NW > NC ? NW : NC)>(lane < NW ? sm->wsum[wid][lane] : 0.0);   // lanes < NC must all hold the sum
+    ARK(2)
+    if (wid == 0 && lane == 0) cl_expect_tx(&sm->bar[slot], (uint32_t)(NC * NV * 8));
+    if (lane < NC)
+      cl_st_async(cl_mapa(cl_smem_u32(&sm->red[slot][wid][me]), (unsigned)lane), t,
+                  cl_mapa(cl_smem_u32(&sm->bar[slot]), (unsigned)lane));                    // into CTA `lane`
   }
-  cl_wait(&sm->bar, (uint32_t)parity);
+  ARK(3)
+  cl_wait(&sm->bar[slot], (uint32_t)((n >> 1) & 1));
+  ARK(4)
+  // ---- 4. the cluster's sum
+  if (NV <= 2) {
+    const int k = NV == 2 ? lane >> 4 : 0, c = lane & 15;
+    const double w = group_sum<NC>(c < NC ? sm->red[slot][k][c] : 0.0);
+    v[0] = __shfl_sync(0xffffffffu, w, 0);
+    if (NV == 2) v[1] = __shfl_sync(0xffffffffu, w, 16);
+  } else {
 #pragma unroll
-  for (int k = 0; k < NV; ++k) {           // fixed order, four chains: ((0+4+8+12) + (1+5+..)) + ((2+..) + (3+..))
-    double a[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-    for (int c = 0; c < NC; ++c) a[c & 3] += sm->red[parity][k][c];
-    v[k] = (a[0] + a[1]) + (a[2] + a[3]);
+    for (int k = 0; k < NV; ++k) v[k] = __shfl_sync(0xffffffffu, group_sum<NC>(lane < NC ? sm->red[slot][k][lane] : 0.0), 0);
   }
-  parity ^= 1;
+  ARK(5)
+  n += 1;
 }
 
 template <int NC>
@@ -233,8 +294,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1) k_pcg_cluster(const Ctx* _
   }
   if (lane == 0) *my = *ctl_g;                         // cleared by k_set_ctx
   if (threadIdx.x == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(cl_smem_u32(&sm->bar)), "r"(NC) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    cluster_bars_init(sm);
   }
   load_coefs(false);                                   // r0 = b - A1 x0 needs the fp64 operator
   cluster.sync();

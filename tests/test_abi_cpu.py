@@ -53,7 +53,7 @@ def test_bad_tuning_and_precision_values_are_argument_errors(cu):
     g = cu.Grid(8, 8, 4, 1e-6, 1e-6, np.full(4, 1e-6), None, 1e4)
     lib = cu.load_library()
     p = C.c_void_p(4096)
-    for kw in (dict(traversal=3), dict(loop_mode=4), dict(k1_variant=4), dict(cheb_fusion=4), dict(pair_rows=12),
+    for kw in (dict(traversal=3), dict(loop_mode=5), dict(k1_variant=4), dict(cheb_fusion=4), dict(pair_rows=12),
                dict(pair_occupancy=1)):
         o = cu.Opts(tuning=cu.Tuning(**kw))
         assert lib.cuth_pcg_solve(p, g.ref(), C.byref(o), p, p, p, 1 << 30, p, None) == -3, kw

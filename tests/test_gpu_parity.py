@@ -342,6 +342,44 @@ def test_two_solvers_with_different_tunings_run_concurrently(traversal):
         S.close()
 
 
+@pytest.mark.parametrize("traversal", ["auto"], indirect=True)    # the test chooses the kernel itself: once
+@pytest.mark.parametrize("prec", ["fp64", "mixed"])
+@pytest.mark.parametrize("shape", [(1, 32, 32, 8), (1, 7, 2, 5), (3, 16, 8, 40), (3, 37, 29, 13), (5, 24, 20, 16)])
+def test_cluster_kernels_agree(shape, prec, traversal):
+    """The two forms of the cluster-resident solve -- rows in registers (cuth_cluster_reg.cuh, loop_mode 3 where at most
+    1024 rows fall to a CTA) and rows in shared memory (cuth_cluster.cuh, loop_mode 4) -- run the same arithmetic per
+    row and differ only in the order of the three sums: same decisions, iteration counts within one of each other, x
+    equal to 1e-9 relative; both against the persistent kernel as well.  Shapes: cfg 1 itself (8 x 1024 rows), a
+    14-row grid, slabs along z, a 16-CTA cluster with ragged slabs, a transient matrix."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    cfg, nx, ny, nz = shape
+    w = W.make_workload(cfg, nx=nx, ny=ny, nz=nz, n_hot=min(4, nz))
+    M = cu.DiaMatrix(grid_from_workload(w))
+    b = to_dev(w.power)
+    out = []
+    for mode in (3, 4, 2):
+        opts = cu.Opts(precision=cu.MIXED if prec == "mixed" else cu.FP64, rtol=1e-8,
+                       true_resid_period=w.true_resid_period, tuning=cu.Tuning(loop_mode=mode, traversal=1 if mode == 2 else 0))
+        if mode != 2:
+            assert cu.cuth_loop_home(grid_from_workload(w), opts) == 3
+        S = cu.Solver(M, opts)
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        S.solve(b, x)
+        out.append((x.cpu().numpy(), S.result()))
+        S.close()
+    (x3, r3), (x4, r4), (x2, r2) = out
+    for r in (r3, r4, r2):
+        assert r.status == 0 and r.rel_resid_true <= 1e-8
+    assert abs(r3.iterations - r4.iterations) <= 1 and abs(r3.iterations - r2.iterations) <= 1
+    assert (r3.promotions, r3.switch_reason, r3.switch_mask, r3.soft_restarts) == \
+           (r4.promotions, r4.switch_reason, r4.switch_mask, r4.soft_restarts)
+    # a late-stage verification that fails by a rounding error (one more hard restart) may happen in one and not the other
+    assert abs(r3.hard_restarts - r4.hard_restarts) <= 1
+    scale = np.abs(x4).max()
+    assert np.abs(x3 - x4).max() <= 1e-9 * scale and np.abs(x3 - x2).max() <= 1e-9 * scale
+
+
 # ---------------------------------------------------------------- a6: transient
 def test_transient_steps_vs_oracle():
     import torch

@@ -21,7 +21,8 @@ from policy_scan import expected_switch
 
 pytestmark = pytest.mark.gpu
 
-HOMES = ["flat-graph", "persistent", "cluster", "zmarch-graph", "zmarch-k1x1", "batch", "batch-cluster"]
+HOMES = ["flat-graph", "persistent", "cluster", "cluster-smem", "zmarch-graph", "zmarch-k1x1", "batch", "batch-cluster",
+         "batch-cluster-smem"]
 
 
 def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
@@ -29,9 +30,11 @@ def _solve(w, b, home, precision, rtol=1e-8, period=20, max_iters=200000):
     import torch
     import paper_2606_17850_b200 as cu
     tune = {"flat-graph": cu.Tuning(traversal=1, loop_mode=1), "persistent": cu.Tuning(traversal=1, loop_mode=2),
-            "cluster": cu.Tuning(loop_mode=3),
+            "cluster": cu.Tuning(loop_mode=3),                     # rows in registers where they fit (cuth_cluster_reg.cuh)
+            "cluster-smem": cu.Tuning(loop_mode=4),                # rows in shared memory (cuth_cluster.cuh)
             "zmarch-graph": cu.Tuning(traversal=2, k1_variant=2), "zmarch-k1x1": cu.Tuning(traversal=2, k1_variant=1),
-            "batch": cu.Tuning(loop_mode=2), "batch-cluster": cu.Tuning(loop_mode=3)}[home]
+            "batch": cu.Tuning(loop_mode=2), "batch-cluster": cu.Tuning(loop_mode=3),
+            "batch-cluster-smem": cu.Tuning(loop_mode=4)}[home]
     opts = cu.Opts(precision=precision, rtol=rtol, max_iters=max_iters, true_resid_period=period, tuning=tune)
     M = cu.DiaMatrix(grid_from_workload(w))
     if home.startswith("batch"):
