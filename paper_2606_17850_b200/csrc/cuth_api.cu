@@ -19,6 +19,7 @@
 #include "cuth_cheb_pair.cuh"
 #include "cuth_cheb_pair_tma.cuh"
 #include "cuth_fused_tma.cuh"
+#include "cuth_spmv_tma.cuh"
 #include "cuth_persistent.cuh"
 #include "cuth_fixed32.cuh"
 #include "cuth_cluster.cuh"
@@ -627,7 +628,7 @@ static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, 
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem);
   if (occ > max_per_sm) occ = max_per_sm;
-  int v = (coop || slot == 2 || slot == 4) ? sms * occ : 0;   // slots 2, 4 (TMA K1, K2) are ordinary launches
+  int v = (coop || slot == 2 || slot >= 4) ? sms * occ : 0;   // slots 2, 4, 5, 6 (TMA K1, K2, TMA SpMV) are ordinary launches
   if (v > cap) v = cap;
   g_coresident[key] = v;
   return v;
@@ -980,6 +981,54 @@ int cuth_dia_view(const void* dia_D, const cuth_grid_t* grid, const double** val
   return CUTH_OK;
 }
 
+}  // extern "C"
+
+// cuth_spmv with TMA-staged operands (cuth_spmv_tma.cuh): wherever the two-column z-marching kernel would run, nx % 4 == 0
+// (strides of the tensor maps), the plane has at least one resident wave of 64 x 8 tiles and the stack at least 12
+// layers; k1_variant 1 / 3 keep the LDG kernels, 2 forces it.  The kernel is persistent over tiles: as many CTAs as give every CTA the same number of
+// tiles (cfg 3: 2048 tiles, 592 resident -> 4 waves -> 512 CTAs of exactly 4 tiles).
+template <bool MIXED>
+static int spmv_tma_blocks(const DiaLayout& L) {
+  const void* fn = (const void*)k_spmv_tma<MIXED>;
+  static_assert(sizeof(SpSmem<MIXED>) <= 227 * 1024, "stages of the TMA SpMV");
+  cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpSmem<MIXED>));
+  const int resident = coresident_blocks(MIXED ? 5 : 6, fn, MIXED ? 4 : 2, kMaxBlocks, sizeof(SpSmem<MIXED>));
+  if (resident <= 0) return 0;
+  const int64_t tiles = ((L.nx + K1X - 1) / K1X) * ((L.ny + K1Y - 1) / K1Y);
+  const int64_t waves = (tiles + resident - 1) / resident;
+  return (int)((tiles + waves - 1) / waves);
+}
+static bool spmv_tma(const DiaLayout& L, const Tune& T) {
+  if (!use_zmarch(L, T) || !zmarch_x2(L, T) || T.k1_variant == 3) return false;
+  if ((L.nx % 4) != 0 || encode_tiled_fn() == nullptr) return false;
+  if (T.k1_variant == 2) return true;
+  // Measured on B200, TMA / LDG: cfg 3 (nz = 16) fp64 0.126 / 0.133 ms, fp32-stored 0.078 / 0.086 ms; cfg 4 (nz = 8: nine
+  // steps for eight planes) fp64 0.977 / 0.981 ms, fp32-stored 0.714 / 0.637 ms -- so thin stacks keep the LDG kernel.
+  return ((L.nx + K1X - 1) / K1X) * ((L.ny + K1Y - 1) / K1Y) >= 592 && L.nz >= 12;
+}
+template <bool MIXED>
+static cudaError_t launch_spmv_tma(const DiaLayout& L, const DiaDev& A, const void* dia_D, const double* x_D, double* y_D,
+                                   cudaStream_t st) {
+  using ST = SpStage<MIXED>;
+  const int blocks = spmv_tma_blocks<MIXED>(L);
+  if (blocks <= 0) return cudaErrorInvalidConfiguration;
+  const char* base = (const char*)dia_D;
+  CUtensorMap tx, td, t1, t2, t3;
+  bool ok = make_map3d(&tx, x_D, 8, L, K1VW, K1VH) && make_map3d(&td, A.d0, 8, L, K1X, K1Y);
+  if (MIXED)
+    ok = ok && make_map3d(&t1, A.f1, 4, L, ST::W1, K1Y) && make_map3d(&t2, A.f2, 4, L, K1X, K1Y + 1) &&
+         make_map3d(&t3, A.f3, 4, L, K1X, K1Y);
+  else
+    ok = ok && make_map3d(&t1, base + L.o_f64a, 8, L, ST::W1, K1Y) &&
+         make_map3d(&t2, base + L.o_f64a + L.f64a_stride, 8, L, K1X, K1Y + 1) &&
+         make_map3d(&t3, base + L.o_f64a + 2 * L.f64a_stride, 8, L, K1X, K1Y);
+  if (!ok) return cudaErrorInvalidValue;
+  k_spmv_tma<MIXED><<<blocks, kThreads, sizeof(SpSmem<MIXED>), st>>>(A, y_D, tx, td, t1, t2, t3);
+  return cudaGetLastError();
+}
+
+extern "C" {
+
 int cuth_spmv_tuned(const void* dia_D, const cuth_grid_t* grid, int precision, const cuth_tuning_t* tuning,
                     const double* x_D, double* y_D, void* stream) {
   DiaLayout L;
@@ -996,6 +1045,13 @@ int cuth_spmv_tuned(const void* dia_D, const cuth_grid_t* grid, int precision, c
   const int sb = stencil_blocks(L, T);
   const int blocks = sb > 0 ? sb : grid_blocks(L.n);
   cudaStream_t st = (cudaStream_t)stream;
+  if (precision != CUTH_MIXED_STD32 && spmv_tma(L, T)) {
+    const cudaError_t e = precision == CUTH_MIXED ? launch_spmv_tma<true>(L, A, dia_D, x_D, y_D, st)
+                                                  : launch_spmv_tma<false>(L, A, dia_D, x_D, y_D, st);
+    if (e == cudaSuccess) return CUTH_OK;
+    if (T.k1_variant == 2) return cuda_fail(e, "k_spmv_tma");
+    cudaGetLastError();                       // automatic: the LDG kernel serves every grid
+  }
   if (precision == CUTH_MIXED_STD32) k_spmv_only<OP_STD32><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);
   else if (precision == CUTH_MIXED) k_spmv_only<OP_DIFF32><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);
   else k_spmv_only<OP_FP64><<<blocks, kThreads, 0, st>>>(A, x_D, y_D);

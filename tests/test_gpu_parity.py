@@ -245,6 +245,33 @@ def test_k1_variants_agree_iterate_for_iterate(shape, prec, traversal):
         assert np.abs(out[variant] - out[1]).max() <= 1e-10 * scale, (variant, shape)
 
 
+@pytest.mark.parametrize("shape", [s for s in K1_SHAPES if s[0] % 4 == 0] + [(192, 24, 2), (320, 17, 5)])
+@pytest.mark.parametrize("prec", ["fp64", "mixed"])
+@pytest.mark.parametrize("traversal", ["zmarch"], indirect=True)       # the test picks the kernels itself: once
+def test_spmv_tma_is_bitwise_the_ldg_kernel(shape, prec, traversal):
+    """cuth_spmv with TMA-staged operands (cuth_spmv_tma.cuh, k1_variant 2, nx % 4 == 0) against the two-column LDG kernel
+    (k1_variant 3): the same operations in the same order on every row, so y agrees bit for bit -- shapes below, at and
+    above one 64 x 8 tile, ragged in x and y, several tiles per CTA -- and both agree with the oracle's CSR SpMV."""
+    import paper_2606_17850_b200 as cu
+    nx, ny, nz = shape
+    w = W.make_workload(3, nx=nx, ny=ny, nz=nz, n_hot=2)
+    g = grid_from_workload(w)
+    M = cu.DiaMatrix(g)
+    x = W.normal01(w.seed, 40, 41, np.arange(w.n))
+    xd = to_dev(x)
+    pr = cu.MIXED if prec == "mixed" else cu.FP64
+    ys = {}
+    for variant in (3, 2):
+        y = to_dev(np.full(w.n, np.nan))
+        cu.cuth_spmv_tuned(M.buf, g, pr, cu.Tuning(traversal=2, k1_variant=variant), xd, y)
+        ys[variant] = y.cpu().numpy()
+    assert np.array_equal(ys[2].view(np.uint64), ys[3].view(np.uint64))
+    A = O.assemble_workload(w)
+    ref = O.spmv(A, x)
+    tol = (1e-12 if prec == "fp64" else 5e-7) * np.abs(A.val).max() * np.abs(x).max()
+    assert np.abs(ys[2] - ref).max() <= tol
+
+
 # ---------------------------------------------------------------- edge cases
 def test_zero_rhs_gives_zero_x():
     import paper_2606_17850_b200 as cu
