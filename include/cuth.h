@@ -102,7 +102,10 @@ typedef struct {
                                  plane has >= 288 tiles of 64 x 8 columns; else two x-adjacent columns per thread when nx
                                  is even and there are >= 2048 tiles; else one column), 1 one column per thread,
                                  2 two columns per thread (nx even), K1 TMA-staged whenever nx % 4 == 0,
-                                 3 = 2 with ordinary loads everywhere */
+                                 3 = 2 with ordinary loads everywhere.  cuth_spmv follows the same field: automatic =
+                                 TMA-staged operands when nx % 4 == 0, the plane has >= 592 such tiles and nz >= 12; 2
+                                 forces them wherever nx % 4 == 0; 1 / 3 keep the kernels with ordinary loads (same y,
+                                 bit for bit) */
   int32_t cheb_fusion;        /* Chebyshev passes per kernel (fp32 modes, nx even): 0 automatic = 2 = two passes, TMA
                                  operands when nx % 4 == 0 (A3: % 8); 1 one pass per kernel; 3 two passes, never TMA */
   int32_t pair_rows;          /* rows of a region of the TMA two-pass Chebyshev kernel: 0 automatic, 8, 16 */
