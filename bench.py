@@ -487,7 +487,7 @@ def main():
     peak, peak_src = peaks()
     lpi = cu.cuth_launches_per_iteration(g, S.opts)
     persistent = (lpi == 0) and not cheb                  # whole solve = one cooperative kernel
-    fused = lpi == 2
+    fused = lpi > 0 and cu.cuth_traversal(g, S.opts) == 2     # z-marching graph loop: K1 (one or two nodes) + K2
     kern = {}
 
     def time_kernel(kid):
@@ -598,7 +598,7 @@ def main():
             dom_name, dom_ms = "k_cheb_pair", kern["k_cheb_pair"]
             dom_bytes = ((2 if h16 else 4) * (m - 1) + 20) * w.n
         stage_tag = "fp32-stored" if mixed else "fp64"
-    per_it = (2 if fused else 3) + (cheb_launches if cheb else 0)
+    per_it = (lpi if fused else 3) + (cheb_launches if cheb else 0)
     per_eval = 3 if fused else 2
     launches = args.steps * (nt * (1 + 1 + 1 + (1 if w.transient else 0)) + per_it * it + per_eval * total_evals)
     if persistent:
@@ -639,7 +639,7 @@ def main():
                                        "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+80 fp32-stored fused, 4(m-1)+88 unfused, per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
-        "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % (4 if fused and not cheb else 1),
+        "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % ((5 if mixed and w.true_resid_period % 5 == 0 else 4) if fused and not cheb else 1),
                  2: "persistent cooperative kernel", 3: "cluster-resident kernel (one thread-block cluster)",
                  4: "fixed-FP32 ablation kernel"}[cu.cuth_loop_home(g, S.opts)],
         "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),

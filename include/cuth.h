@@ -278,9 +278,16 @@ const char* cuth_last_cuda_error(void);
 int cuth_version(void);
 
 /* Kernel launches per PCG iteration of the graph body for this grid and these options (2 on the fused path used
- * for large planes, 3 on the flat path, 0 when the whole solve is one persistent kernel); bench.py reports
+ * for large planes -- 3 there for a MIXED solve on a stack of fewer than 12 layers, whose K1 is two nodes, the
+ * TMA-staged kernel for the early stage and the two-column LDG kernel for the late stage, each returning at once in
+ * the other's stage --, 3 on the flat path, 0 when the whole solve is one persistent kernel); bench.py reports
  * gpu_launches = prologue + this * iterations + true-residual branches + epilogue.  Pure host. */
 int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts);
+
+/* How the kernels of a solve with these options walk this grid (what cuth_tuning_t.traversal = 0 resolves to):
+ * 1 = flat 1-D streaming (k_pupdate, k_spmv_dot, k_update in the graph loop), 2 = z-marching (the fused K1 + K2);
+ * negative on bad arguments.  Pure host. */
+int cuth_traversal(const cuth_grid_t* grid, const cuth_opts_t* opts);
 
 /* Where the PCG loop of a solve with these options on this grid lives (what cuth_tuning_t.loop_mode = 0 resolves
  * to): 1 = CUDA graph with conditional nodes, 2 = persistent cooperative kernel, 3 = cluster-resident kernel,

@@ -70,7 +70,7 @@ EXPORTS = ["cuth_import_csr", "cuth_import_coo", "cuth_batch_workspace_bytes", "
            "cuth_workspace_bytes", "cuth_build_dia", "cuth_dia_view", "cuth_spmv", "cuth_spmv_tuned", "cuth_pcg_solve",
            "cuth_transient_step", "cuth_release_workspace", "cuth_last_cuda_error", "cuth_version",
            "cuth_launches_per_iteration", "cuth_profile_kernel", "cuth_lanczos_bounds", "cuth_lanczos_bounds_tuned",
-           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home",
+           "cuth_cheb_apply", "cuth_tridiag_extremes", "cuth_cheb_launches", "cuth_policy_probe", "cuth_loop_home", "cuth_traversal",
            "cuth_residual_noalloc", "cuth_noalloc_max_rows", "cuth_noalloc_last_error", "cuth_import_csr_n"]
 
 _lib = None
@@ -416,6 +416,17 @@ def cuth_loop_home(grid: Grid, opts) -> int:
     rc = int(L.cuth_loop_home(grid.ref(), C.byref(opts)))
     if rc < 0:
         _check(rc, "cuth_loop_home")
+    return rc
+
+
+def cuth_traversal(grid: Grid, opts) -> int:
+    """1 flat, 2 z-marching (include/cuth.h); pure host."""
+    L = load_library()
+    L.cuth_traversal.restype = C.c_int
+    L.cuth_traversal.argtypes = [C.POINTER(cuth_grid_t), C.POINTER(cuth_opts_t)]
+    rc = int(L.cuth_traversal(grid.ref(), C.byref(opts)))
+    if rc < 0:
+        _check(rc, "cuth_traversal")
     return rc
 
 

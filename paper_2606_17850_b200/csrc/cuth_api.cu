@@ -402,6 +402,8 @@ struct Plan {
   int with_b = 0;        // transient matrix: b lives in the workspace, the Chebyshev buffers sit N doubles later
   int pair_tma = 0;      // the two-pass Chebyshev nodes are the TMA kernel
   int k1tma = 0;         // K1 is the TMA-staged kernel
+  int k1dual = 0;        // ... in the early stage only; in the late stage K1 is the two-column LDG kernel (fblocks2 CTAs)
+  int fblocks2 = 0;
   int unroll = 1;        // K1 + K2 pairs per pass of the WHILE body (fused path without Chebyshev)
   int k2blocks = 0;      // grid of K2 (one resident wave)
   const void* dia = nullptr;   // matrix the tensor maps of the TMA nodes were made for (else nullptr)
@@ -411,7 +413,7 @@ struct Plan {
   bool operator==(const Plan& o) const {
     return n == o.n && sblocks == o.sblocks && fblocks == o.fblocks && k1x2 == o.k1x2 && chebkey == o.chebkey &&
            cblocks == o.cblocks && x2blocks == o.x2blocks && pblocks == o.pblocks && with_b == o.with_b &&
-           pair_tma == o.pair_tma && k1tma == o.k1tma && unroll == o.unroll && k2blocks == o.k2blocks && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
+           pair_tma == o.pair_tma && k1tma == o.k1tma && k1dual == o.k1dual && fblocks2 == o.fblocks2 && unroll == o.unroll && k2blocks == o.k2blocks && dia == o.dia && tnx == o.tnx && tny == o.tny && tocc == o.tocc && device == o.device;
   }
 };
 struct GraphEntry {
@@ -509,6 +511,11 @@ static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, co
         void* a[] = {&ctx, &ctl, &partials, &km.z, &km.p, &km.p2, &km.d, &km64.d, &km.m1, &km.m2, &km.m3,
                      &km64.m1, &km64.m2, &km64.m3};                    // the maps are copied into the node
         CU(add_kernel(body, &n_s, dep, ndep, (void*)k_fused_pspmv_tma, P.fblocks, a, k1_smem));
+        if (P.k1dual) {        // thin stacks: the late stage's K1 (Ctx.k1_split makes each return in the other's stage)
+          cudaGraphNode_t n_e = n_s;
+          void* a2[] = {&ctx, &ctl, &partials};
+          CU(add_kernel(body, &n_s, &n_e, 1, (void*)k_fused_pspmv_x2, P.fblocks2, a2));
+        }
       } else {
         void* a[] = {&ctx, &ctl, &partials};
         CU(add_kernel(body, &n_s, dep, ndep, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
@@ -748,6 +755,16 @@ static bool use_persistent(const DiaLayout& L, bool cheb, const Tune& T) {
 
 constexpr int kGraphUnroll = 4;   // iterations per pass of the WHILE body on the fused path
 
+// Thin stacks (nz < 12: nz + 1 steps for nz planes) with the fp64 operator: the two-column LDG K1 beats the TMA-staged one
+// (cfg 4, nz = 8: 1.66 vs 1.82 ms; FP64 solve 23.45 vs 24.00 s), while with the fp32-stored operator the TMA-staged one wins
+// (1.57 ms).  Automatic choice only (k1_variant 0), where both kernels serve the grid:
+// 0 = nothing to do, 1 = FP64 solve: LDG K1 throughout, 2 = MIXED solve: TMA K1 in the early stage, LDG K1 in the late one.
+static int k1_thin_stack(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts) {
+  if (T.k1_variant != 0 || L.nz >= 12 || opts->preconditioner == CUTH_PRECOND_CHEBYSHEV || !fused_x2(L, T)) return 0;
+  if (!fused_tma(L, T, false)) return 0;
+  return opts->precision == CUTH_FP64 ? 1 : (opts->precision == CUTH_MIXED ? 2 : 0);
+}
+
 // The graph of a solve with these options on this grid.
 static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts, bool with_b, const void* dia_D) {
   Plan P;
@@ -762,6 +779,9 @@ static Plan make_plan(const DiaLayout& L, const Tune& T, const cuth_opts_t* opts
   if (zm && fused_tma(L, T, cheb)) {
     P.k1tma = 1; P.fblocks = fused_tma_blocks(L);
     P.dia = dia_D; P.tnx = L.nx; P.tny = L.ny;
+    const int split = k1_thin_stack(L, T, opts);
+    if (split == 1) { P.k1tma = 0; P.fblocks = fused_blocks(L, T); P.dia = nullptr; P.tnx = P.tny = 0; }
+    else if (split == 2) { P.k1dual = 1; P.fblocks2 = fused_blocks(L, T); }
   }
   P.chebkey = cheb ? opts->cheb_degree * 4 + code : 0;
   P.cblocks = cheb_blocks(L, T);
@@ -831,6 +851,7 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   if (cheb) fill_cheb(&c, opts, w);
   c.early_op = opts->precision == CUTH_MIXED_STD32 ? OP_STD32 : OP_DIFF32;
   c.transient_call = transient ? 1 : 0;
+  c.k1_split = (use_zmarch(L, T) && k1_thin_stack(L, T, opts) == 2) ? 1 : 0;
   // persistent kernel: phases A and B in one on the smallest grids (not with the ablation operator)
   c.persist_fuse = (L.n <= (1 << 14) && c.early_op == OP_DIFF32) ? 1 : 0;
   c.soft_restart = 1;         // promotion keeps p while the drift is small (DESIGN.md R-G11)
@@ -1196,7 +1217,7 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t
     case 1: k_spmv_dot<<<sb, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials); break;
     case 2: k_update<true><<<blocks, kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 4:
-      if (fused_tma(L, T, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV)) {
+      if (fused_tma(L, T, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV) && k1_thin_stack(L, T, opts) != 1) {
         const void* dia = nullptr;
         { std::lock_guard<std::mutex> lk(g_mu);
           auto it = g_last_dia.find(work_D);
@@ -1209,6 +1230,8 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t
                      &km64.m1, &km64.m2, &km64.m3};
         CU(cudaLaunchKernel((const void*)k_fused_pspmv_tma, dim3(fused_tma_blocks(L)), dim3(kThreads), a,
                             k1_tma_dyn_smem(), st));
+        if (k1_thin_stack(L, T, opts) == 2)        // as in the graph: one of the two returns at once
+          k_fused_pspmv_x2<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       } else if (fused_x2(L, T)) k_fused_pspmv_x2<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       else k_fused_pspmv<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       break;
@@ -1402,7 +1425,18 @@ int cuth_launches_per_iteration(const cuth_grid_t* grid, const cuth_opts_t* opts
   if (opts->precision == CUTH_MIXED_STD32) T.traversal = 1;
   if (use_cluster(L, opts, T)) return 0;                                                   // one cluster-resident kernel
   if (use_persistent(L, opts->preconditioner == CUTH_PRECOND_CHEBYSHEV, T)) return 0;      // one persistent kernel for the whole solve
-  return use_zmarch(L, T) ? 2 : 3;
+  if (!use_zmarch(L, T)) return 3;
+  return k1_thin_stack(L, T, opts) == 2 ? 3 : 2;   // thin stacks, MIXED: K1 is two nodes, one of which returns at once
+}
+
+int cuth_traversal(const cuth_grid_t* grid, const cuth_opts_t* opts) {
+  DiaLayout L;
+  Tune T;
+  if (!opts) return CUTH_ERR_NULL;
+  if (!make_layout(grid, &L)) return CUTH_ERR_DIMS;
+  if (check_opts(opts) != CUTH_OK || make_tune(&opts->tuning, &T) != CUTH_OK) return CUTH_ERR_VALUE;
+  if (opts->precision == CUTH_MIXED_STD32 || opts->precision == CUTH_FIXED32) T.traversal = 1;
+  return use_zmarch(L, T) ? 2 : 1;
 }
 
 int cuth_loop_home(const cuth_grid_t* grid, const cuth_opts_t* opts) {

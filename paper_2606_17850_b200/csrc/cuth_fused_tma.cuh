@@ -293,6 +293,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_fused_pspmv_tma(
   extern __shared__ __align__(128) unsigned char k1_smem_raw[];
   if (ctl->halt) return;                     // unrolled graph body: this pass is over
   const Ctx c = *ctxp;
+  if (c.k1_split && ctl->stage != 0) return; // thin stacks: the late stage belongs to k_fused_pspmv_x2 (cuth_api.cu make_plan)
   const int pcur = ctl->pcur;
   double* p_out = pcur ? c.p : c.p2;
   const CUtensorMap* tp = pcur ? &tmP2 : &tmP;

@@ -174,6 +174,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_fused_pspmv_x2(const Ctx* __res
   __shared__ int s_flag;
   if (ctl->halt) return;                     // unrolled graph body: this pass is over
   const Ctx c = *ctxp;
+  if (c.k1_split && ctl->stage == 0) return; // thin stacks: the early stage belongs to k_fused_pspmv_tma
   const int pcur = ctl->pcur;
   const double* p_in = pcur ? c.p2 : c.p;
   double* p_out = pcur ? c.p : c.p2;

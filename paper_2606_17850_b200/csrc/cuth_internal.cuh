@@ -103,7 +103,9 @@ struct Ctx {
   int32_t soft_restart, cheb;     // cheb: degree k of the Chebyshev polynomial preconditioner, 0 = off
   int32_t persist_fuse;           // persistent kernel: phases A and B in one (p' recomputed at the six neighbours)
   int32_t early_op;               // operator of the early stage: 1 = difference form (R-F3), 2 = A2 in standard form (ablation)
-  int32_t transient_call, pad_tc; // 1: cuth_transient_step (the matrix object must be a transient one)
+  int32_t transient_call;         // 1: cuth_transient_step (the matrix object must be a transient one)
+  int32_t k1_split;               // graph loop on thin stacks (nz < 12): the TMA-staged K1 serves the early stage only, the
+                                  // two-column LDG K1 the late stage; each returns at once in the other's stage
   // Chebyshev preconditioner (Alg. 3): z = q(A) r.  cz: z (fp64) handed to the outer
   // loop; cd[4]: partial-sum buffers Z (two are live at any time; the fused two-pass kernel writes the other
   // two); crc: fp32 copy of r (MIXED only).  Element type T = double in FP64 mode, float in MIXED mode;

@@ -272,6 +272,40 @@ def test_spmv_tma_is_bitwise_the_ldg_kernel(shape, prec, traversal):
     assert np.abs(ys[2] - ref).max() <= tol
 
 
+@pytest.mark.parametrize("traversal", ["auto"], indirect=True)       # the test picks the kernels itself: once
+def test_thin_stack_k1_split_agrees_with_either_kernel(traversal):
+    """Thin stacks (nz < 12) with everything automatic: a MIXED solve runs the TMA-staged K1 in the early stage and the
+    two-column LDG K1 in the late stage (two K1 nodes per iteration, each returning at once in the other's stage), an FP64
+    solve the LDG K1 throughout.  Same arithmetic per row in both kernels: same decisions, iteration counts within one,
+    x equal to 1e-9 relative to the solves that use one kernel throughout (k1_variant 2 / 3)."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(4, nx=1024, ny=1024, nz=5, n_hot=5)      # 5.2 M rows: the graph loop whatever K1
+    g = grid_from_workload(w)
+    M = cu.DiaMatrix(g)
+    b = to_dev(w.power)
+    for prec, launches in ((cu.MIXED, 3), (cu.FP64, 2)):
+        out = []
+        for variant in (0, 2, 3):
+            opts = cu.Opts(precision=prec, rtol=1e-8, true_resid_period=w.true_resid_period, tuning=cu.Tuning(k1_variant=variant))
+            assert cu.cuth_loop_home(g, opts) == 1 and cu.cuth_traversal(g, opts) == 2
+            assert cu.cuth_launches_per_iteration(g, opts) == (launches if variant == 0 else 2)
+            S = cu.Solver(M, opts)
+            x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+            S.solve(b, x)
+            out.append((x.cpu().numpy(), S.result()))
+            S.close()
+        (x0, r0), (x2, r2), (x3, r3) = out
+        scale = np.abs(x2).max()
+        for x, r in ((x0, r0), (x3, r3)):
+            assert r.status == 0 and r.rel_resid_true <= 1e-8
+            assert abs(r.iterations - r2.iterations) <= 1
+            assert (r.promotions, r.switch_reason, r.soft_restarts) == (r2.promotions, r2.switch_reason, r2.soft_restarts)
+            assert np.abs(x - x2).max() <= 1e-9 * scale
+        if prec == cu.MIXED:
+            assert r0.promotions == 1 and 0 < r0.switch_iteration < r0.iterations     # both stages ran
+
+
 # ---------------------------------------------------------------- edge cases
 def test_zero_rhs_gives_zero_x():
     import paper_2606_17850_b200 as cu
