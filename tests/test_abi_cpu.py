@@ -159,6 +159,33 @@ def test_cheb_launch_schedule_host_side(cu):
     assert cu.cuth_cheb_launches(big, cu.Opts(cu.MIXED, 1e-8, 1000, 20)) == (0, 0)   # Jacobi: no apply
 
 
+def test_kernel_choice_queries_host_side(cu):
+    """cuth_traversal / cuth_loop_home / cuth_launches_per_iteration (pure host) on the BASELINE grids: the rules stated in
+    include/cuth.h (cuth_tuning_t).  Where the driver cannot encode tensor maps (this CPU box) the TMA-dependent choices
+    fall back, and without a device there is no cooperative launch: hence the sets."""
+    mk = lambda nx, ny, nz: cu.Grid(nx, ny, nz, 1e-6, 1e-6, np.full(nz, 1e-6), None, 1e4)
+    o64, omx = cu.Opts(cu.FP64), cu.Opts(cu.MIXED)
+    cfg1, cfg2, cfg3, cfg4, cfg5 = mk(32, 32, 8), mk(256, 256, 16), mk(1024, 1024, 16), mk(4096, 4096, 8), mk(512, 512, 16)
+    # cfg 1 fits one thread-block cluster; cfg 2 is flat in one persistent kernel; cfg 3 / 4 z-march in the graph
+    assert (cu.cuth_traversal(cfg1, omx), cu.cuth_loop_home(cfg1, omx), cu.cuth_launches_per_iteration(cfg1, omx)) == (1, 3, 0)
+    # (without a device there is no cooperative launch: the graph loop with its three flat kernels)
+    assert (cu.cuth_traversal(cfg2, omx), cu.cuth_loop_home(cfg2, omx), cu.cuth_launches_per_iteration(cfg2, omx)) in ((1, 2, 0), (1, 1, 3))
+    for g in (cfg3, cfg4):
+        for o in (o64, omx):
+            assert (cu.cuth_traversal(g, o), cu.cuth_loop_home(g, o)) == (2, 1)
+    assert cu.cuth_launches_per_iteration(cfg3, omx) == 2 and cu.cuth_launches_per_iteration(cfg4, o64) == 2
+    assert cu.cuth_launches_per_iteration(cfg4, omx) in (2, 3)          # 3 = thin stack: TMA K1 early + LDG K1 late
+    assert cu.cuth_loop_home(cfg5, omx) in (1, 2)                       # graph with the TMA K1, else the persistent kernel
+    # forced variants
+    assert cu.cuth_traversal(cfg3, cu.Opts(cu.FP64, tuning=cu.Tuning(traversal=1))) == 1
+    assert cu.cuth_traversal(cfg2, cu.Opts(cu.FP64, tuning=cu.Tuning(traversal=2))) == 2
+    assert cu.cuth_loop_home(cfg1, cu.Opts(cu.FP64, tuning=cu.Tuning(loop_mode=4))) == 3
+    assert cu.cuth_loop_home(cfg1, cu.Opts(cu.FP64, tuning=cu.Tuning(loop_mode=2))) in (2, 1)
+    assert cu.cuth_loop_home(cfg1, cu.Opts(cu.FP64, tuning=cu.Tuning(loop_mode=1))) == 1
+    assert cu.cuth_launches_per_iteration(cfg4, cu.Opts(cu.MIXED, tuning=cu.Tuning(k1_variant=2))) == 2
+    assert cu.cuth_traversal(cfg3, cu.Opts(cu.MIXED_STD32)) == 1          # the ablation operator exists in the flat traversal only
+
+
 def test_batch_and_import_host_side(cu):
     """Pure-host behaviour of the two calls added last: batch workspace size (0 on a bad count, grows by three
     vectors per right-hand side) and the argument checks that come before any CUDA call."""
