@@ -272,6 +272,40 @@ def test_spmv_tma_is_bitwise_the_ldg_kernel(shape, prec, traversal):
     assert np.abs(ys[2] - ref).max() <= tol
 
 
+@pytest.mark.parametrize("traversal", ["auto"], indirect=True)    # the test chooses the kernel itself: once
+@pytest.mark.parametrize("mode", [3, 4])
+def test_cluster_solve_is_bit_reproducible_over_many_runs_and_placements(mode, traversal):
+    """The cluster-resident kernels exchange data between CTAs through distributed shared memory ordered only by the
+    st.async / mbarrier all-reduce: a missing ordering would show up as run-to-run differences.  40 solves
+    of cfg 1 one after the other, then 7 at once as a batch (seven clusters on different SMs): every x bit-identical,
+    every iteration count the same."""
+    import torch
+    import paper_2606_17850_b200 as cu
+    w = W.make_workload(1)
+    M = cu.DiaMatrix(grid_from_workload(w))
+    b = to_dev(w.power)
+    opts = cu.Opts(precision=cu.MIXED, rtol=1e-8, tuning=cu.Tuning(loop_mode=mode))
+    S = cu.Solver(M, opts)
+    first = None
+    for rep in range(40):
+        x = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        S.solve(b, x)
+        r = S.result()
+        cur = (x.cpu().numpy().view(np.uint64).copy(), r.iterations, r.switch_iteration)
+        assert r.status == 0
+        if first is None:
+            first = cur
+        else:
+            assert cur[1:] == first[1:] and np.array_equal(cur[0], first[0]), rep
+    S.close()
+    SB = cu.BatchSolver(M, 7, opts)
+    X = torch.zeros(7, w.n, dtype=torch.float64, device="cuda")
+    SB.solve(torch.stack([b] * 7), X)
+    Xh = X.cpu().numpy().view(np.uint64)
+    for s_, r in enumerate(SB.results()):
+        assert r.status == 0 and r.iterations == first[1] and np.array_equal(Xh[s_], first[0]), s_
+
+
 @pytest.mark.parametrize("traversal", ["auto"], indirect=True)       # the test picks the kernels itself: once
 def test_thin_stack_k1_split_agrees_with_either_kernel(traversal):
     """Thin stacks (nz < 12) with everything automatic: a MIXED solve runs the TMA-staged K1 in the early stage and the
