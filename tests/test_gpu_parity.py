@@ -261,10 +261,16 @@ def test_spmv_tma_is_bitwise_the_ldg_kernel(shape, prec, traversal):
     xd = to_dev(x)
     pr = cu.MIXED if prec == "mixed" else cu.FP64
     ys = {}
+    guard = 64                                      # doubles of canary on either side of y (16-byte aligned start)
     for variant in (3, 2):
-        y = to_dev(np.full(w.n, np.nan))
+        buf = to_dev(np.full(w.n + 2 * guard, 1234.5))
+        y = buf[guard:guard + w.n]
+        y.fill_(float("nan"))
         cu.cuth_spmv_tuned(M.buf, g, pr, cu.Tuning(traversal=2, k1_variant=variant), xd, y)
-        ys[variant] = y.cpu().numpy()
+        out = buf.cpu().numpy()
+        assert np.all(out[:guard] == 1234.5) and np.all(out[guard + w.n:] == 1234.5), "write outside y"
+        ys[variant] = out[guard:guard + w.n].copy()
+        assert not np.isnan(ys[variant]).any()
     assert np.array_equal(ys[2].view(np.uint64), ys[3].view(np.uint64))
     A = O.assemble_workload(w)
     ref = O.spmv(A, x)
