@@ -616,14 +616,14 @@ static void fill_cheb(Ctx* c, const cuth_opts_t* opts, const Workspace& w) {
 
 // Grid of the persistent kernel: every CTA must be co-resident (cooperative launch).  The grid-wide barrier, not
 // the row work, sets the pace on small grids, and its cost is not monotonic in the CTA count: measured per
-// iteration at 8 k / 33 k / 66 k / 262 k / 1 M rows (B200) -- 32 CTAs 11.5 / 16.0 / 22.9 / 51 / 187 us,
-// 96 CTAs 12.4 / 13.9 / 16.0 / 27.7 / 72, 128 CTAs 7.1 / 7.3 / 8.1 / 13.9 / 47, 148 CTAs 8.0 / 8.0 / 8.8 / 14.2 / 46,
-// 256 CTAs 9.2 / 8.4 / 8.4 / 12.4 / 33, 592 CTAs 13.4 / 14.1 / 13.7 / 16.7 / 29.8.  So: 128 CTAs up to 64 k rows (CTAs
-// beyond the rows only take part in the barriers), 256 up to 512 k rows, everything the device holds beyond.
+// iteration at 8 k / 33 k / 66 k / 262 k / 1 M rows with 256-thread CTAs (B200, round 1) -- 32 CTAs
+// 11.5 / 16.0 / 22.9 / 51 / 187 us, 96 CTAs 12.4 / 13.9 / 16.0 / 27.7 / 72, 128 CTAs 7.1 / 7.3 / 8.1 / 13.9 / 47, 148 CTAs
+// 8.0 / 8.0 / 8.8 / 14.2 / 46, 256 CTAs 9.2 / 8.4 / 8.4 / 12.4 / 33, 592 CTAs 13.4 / 14.1 / 13.7 / 16.7 / 29.8.  Round 2c keeps
+// the 128 CTAs and grows the CTAs instead of their number: persistent_config below.
 // Co-resident CTAs of a cooperative kernel, per device (derived data, filled on first use under the mutex).
 static std::mutex g_dev_mu;
 static std::unordered_map<long long, int> g_coresident;      // (device << 8 | kernel slot) -> CTAs
-static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, size_t dyn_smem = 0) {
+static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, size_t dyn_smem = 0, int threads = kThreads) {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return 0;
   std::lock_guard<std::mutex> lk(g_dev_mu);
@@ -633,7 +633,7 @@ static int coresident_blocks(int slot, const void* fn, int max_per_sm, int cap, 
   int sms = 0, coop = 0, occ = 0;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kThreads, dyn_smem);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, dyn_smem);
   if (occ > max_per_sm) occ = max_per_sm;
   int v = (coop || slot == 2 || slot >= 4) ? sms * occ : 0;   // slots 2, 4, 5, 6 (TMA K1, K2, TMA SpMV) are ordinary launches
   if (v > cap) v = cap;
@@ -653,11 +653,30 @@ static int k2_blocks(int64_t n) {
   const int want = grid_blocks(n);
   return resident > 0 && resident < want ? resident : want;
 }
-static int persistent_blocks(int64_t n) {
-  const int all = coresident_blocks(0, (const void*)k_pcg_persistent, 4, kPersistMaxBlocks);
-  const int want = n <= (1 << 16) ? 128 : (n <= (1 << 19) ? 256 : all);   // > 512 k rows: all co-resident CTAs
-  return want < all ? want : all;
+// Launch configuration of the persistent kernel (and of the fixed-FP32 ablation kernel, which shares its row loops).
+// What a grid-wide barrier costs grows with the CTAs that take part in it, so the kernel runs FEW, LARGE CTAs: always 128
+// CTAs (a power of two: 148 is slower everywhere), of 256 threads up to 64 k rows, 512 up to 128 k, 1024 beyond (round 2b
+// ran 128 / 256 / 592 CTAs of 256 threads up to 64 k / 512 k rows / beyond).  Measured on B200, us per iteration, MIXED,
+// 128 CTAs of 256 / 512 / 1024 threads: 8 k rows 6.9 / 7.2 / 8.5; 37 k 7.9 / 8.3 / 9.3; 65 k 8.4 / 8.3 / 9.8; 131 k 10.5 /
+// 9.4 / 10.0; 262 k 14.6 / 12.1 / 11.5; cfg 6 (655 k) 25.1 / 17.6 / 16.6; and 1024-thread CTAs x 32 / 64 / 96 / 128 / 148:
+// 262 k 21.1 / 17.0 / 15.8 / 11.0 / 12.1; cfg 6 40.2 / 25.4 / 22.3 / 16.3 / 17.1; cfg 2 (1 M) 58.6 / 36.1 / 29.9 / 21.8 /
+// 22.1 -- against 12.5 (262 k), 20.3 (cfg 6) and 25.2 (cfg 2) with round 2b's configuration.
+struct PersistConfig { int blocks, threads; };
+static PersistConfig persistent_config(int64_t n) {
+#ifdef CUTH_PERSIST_THREADS
+  const int threads = CUTH_PERSIST_THREADS;
+#else
+  const int threads = n <= (1 << 16) ? 256 : (n <= (1 << 17) ? 512 : kPersistMaxThreads);
+#endif
+#ifdef CUTH_PERSIST_CTAS
+  const int want = CUTH_PERSIST_CTAS;
+#else
+  const int want = n > 3 * (1 << 19) ? kPersistMaxBlocks : 128;      // beyond 1.5 M rows: every SM (2 M rows: 45.6 vs 48.4 us)
+#endif
+  const int all = coresident_blocks(0, (const void*)k_pcg_persistent, 1, kPersistMaxBlocks, 0, kPersistMaxThreads);
+  return {want < all ? want : all, threads};
 }
+static int persistent_blocks(int64_t n) { return persistent_config(n).blocks; }
 
 // The cluster-resident kernel (cuth_cluster.cuh): every row lives in the shared memory of one 8-CTA cluster.
 // Measured on B200 (profiles/r2c_loop_homes.md), per iteration, cluster / persistent kernel / graph: cfg 1 (8 192 rows)
@@ -860,11 +879,12 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   CU(cudaGetLastError());
   { std::lock_guard<std::mutex> lk(g_mu); g_last_dia[work_D] = dia_D; }
   if (opts->precision == CUTH_FIXED32) {       // ablation: the paper's fixed-FP32 solver, one cooperative kernel
-    const int nb = coresident_blocks(3, (const void*)k_pcg_fixed32, 4, kPersistMaxBlocks);
+    int nb = coresident_blocks(3, (const void*)k_pcg_fixed32, 1, kPersistMaxBlocks, 0, kPersistMaxThreads);
+    if (nb > 128) nb = 128;
     if (nb <= 0) { g_last_err = "CUTH_FIXED32: cooperative launch unavailable"; return CUTH_ERR_CUDA; }
     Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
     void* args[] = {&ctxp, &ctlp, &part};
-    CU(cudaLaunchCooperativeKernel((void*)k_pcg_fixed32, dim3(nb), dim3(kThreads), args, 0, st));
+    CU(cudaLaunchCooperativeKernel((void*)k_pcg_fixed32, dim3(nb), dim3(kPersistMaxThreads), args, 0, st));
     return CUTH_OK;
   }
   if (use_cluster(L, opts, T)) {
@@ -879,8 +899,8 @@ static int solve_common(const void* dia_D, const cuth_grid_t* grid, const cuth_o
   if (use_persistent(L, cheb, T)) {
     Ctx* ctxp = w.ctx; Ctl* ctlp = w.ctl; double* part = w.partials;
     void* args[] = {&ctxp, &ctlp, &part};
-    const cudaError_t e = cudaLaunchCooperativeKernel((void*)k_pcg_persistent, dim3(persistent_blocks(L.n)),
-                                                      dim3(kThreads), args, 0, st);
+    const PersistConfig pc = persistent_config(L.n);
+    const cudaError_t e = cudaLaunchCooperativeKernel((void*)k_pcg_persistent, dim3(pc.blocks), dim3(pc.threads), args, 0, st);
     if (e == cudaSuccess) return CUTH_OK;
     if (T.loop_mode == 2) return cuda_fail(e, "cudaLaunchCooperativeKernel(k_pcg_persistent)");
     cudaGetLastError();       // automatic mode: the graph loop serves every grid (e.g. under an SM-limited context)
@@ -1167,7 +1187,7 @@ int cuth_pcg_solve_batch(const void* dia_D, const cuth_grid_t* grid, const cuth_
   const int64_t need = (L.n + (int64_t)kThreads - 1) / (int64_t)kThreads;
   int64_t ntiles = max_blocks / nchunks;
   if (ntiles > need) ntiles = need;
-  // the barrier is fastest at >= 128 CTAs (see persistent_blocks): tiles beyond the rows only take part in it
+  // the barrier is fastest at >= 128 CTAs (see persistent_config): tiles beyond the rows only take part in it
   if (ntiles * nchunks < 128 && max_blocks >= 128) ntiles = (128 + nchunks - 1) / nchunks;
   if (ntiles > kBatchMaxBlocks) ntiles = kBatchMaxBlocks;
   BatchCtx c;

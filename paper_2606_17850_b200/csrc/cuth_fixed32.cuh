@@ -68,13 +68,13 @@ __device__ __forceinline__ float spmv_row_f32(const DiaDev& A, const float* __re
   return acc;
 }
 
-__global__ void __launch_bounds__(kThreads, 4) k_pcg_fixed32(const Ctx* __restrict__ ctxp, Ctl* ctl_g, double* partials_d) {
+__global__ void __launch_bounds__(kPersistMaxThreads, 1) k_pcg_fixed32(const Ctx* __restrict__ ctxp, Ctl* ctl_g, double* partials_d) {
   cg::grid_group grid = cg::this_grid();
   __shared__ float smem[3 * 32 + 3];
   __shared__ double dsm[3 * 32 + 3];
   const Ctx c = *ctxp;
   const int64_t n = c.A.n;
-  const int64_t gstride = (int64_t)gridDim.x * kThreads;
+  const int64_t gstride = (int64_t)gridDim.x * blockDim.x;
   const bool jac = c.jacobi != 0;
   float* partials = reinterpret_cast<float*>(partials_d);
   // fp32 vectors live in the fp64 workspace buffers (half of each is used)

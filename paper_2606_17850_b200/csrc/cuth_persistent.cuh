@@ -20,6 +20,10 @@ namespace cuth {
 
 namespace cg = cooperative_groups;
 
+// Threads per CTA are a launch parameter (the row loops stride by blockDim.x): 256 on grids of up to 64 k rows, 1024
+// beyond -- what a grid-wide barrier costs grows with the number of CTAs that take part in it, so the larger grids run
+// 128 CTAs of 1024 threads instead of 592 of 256 (cuth_api.cu persistent_config).
+constexpr int kPersistMaxThreads = 1024;
 constexpr int kPersistMaxBlocks = 1024;   // 2 parities x 3 values x 1024 doubles fit the 4 x 8192 partials area
 
 // Sums NV per-thread values over the whole grid; result valid in ALL threads of ALL CTAs.
@@ -55,12 +59,12 @@ __device__ __forceinline__ void grid_allreduce(cg::grid_group& grid, double (&v)
 // time: all loads of both rows are issued before the first store, so a phase costs one L2 round trip per pair
 // instead of one per row and per store (the stores may alias the loads as far as the compiler knows).
 #define CUTH_ROWS2(i0_, i1_, h1_)                                                                \
-  for (int64_t i0_ = (int64_t)blockIdx.x * kThreads + threadIdx.x, i1_ = i0_ + gstride; i0_ < n;  \
+  for (int64_t i0_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, i1_ = i0_ + gstride; i0_ < n;  \
        i0_ += 2 * gstride, i1_ += 2 * gstride)                                                   \
     for (bool h1_ = i1_ < n, once_ = true; once_; once_ = false)
 
 #define CUTH_ROWS(i_)                                                                            \
-  for (int64_t i_ = (int64_t)blockIdx.x * kThreads + threadIdx.x; i_ < n; i_ += gstride)
+  for (int64_t i_ = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i_ < n; i_ += gstride)
 
 template <int OP>
 __device__ __forceinline__ double persistent_spmv_phase(const Ctx& c, int64_t n, int64_t gstride) {
@@ -141,14 +145,14 @@ __device__ __forceinline__ double persistent_fused_phase(const Ctx& c, const dou
   return acc;
 }
 
-__global__ void __launch_bounds__(kThreads, 4) k_pcg_persistent(const Ctx* __restrict__ ctxp, Ctl* ctl_g,
+__global__ void __launch_bounds__(kPersistMaxThreads, 1) k_pcg_persistent(const Ctx* __restrict__ ctxp, Ctl* ctl_g,
                                                                double* partials) {
   cg::grid_group grid = cg::this_grid();
   __shared__ Ctl sc;
   __shared__ double smem[3 * 32 + 3];
   const Ctx c = *ctxp;
   const int64_t n = c.A.n;
-  const int64_t gstride = (int64_t)gridDim.x * kThreads;
+  const int64_t gstride = (int64_t)gridDim.x * blockDim.x;
   const bool jac = c.jacobi != 0;
   int parity = 0;
   if (threadIdx.x == 0) sc = *ctl_g;                 // cleared by k_set_ctx
