@@ -118,6 +118,12 @@ static int stencil_blocks(const DiaLayout& L, const Tune& T) {
 
 static int grid_blocks(int64_t n);
 
+// Threads per CTA of K2 (k_update<false>); see k2_blocks.
+#ifndef CUTH_K2_THREADS
+#define CUTH_K2_THREADS 512
+#endif
+constexpr int kK2Threads = CUTH_K2_THREADS;
+
 // fp32 Chebyshev middle step with two x-adjacent columns per thread: large planes with even nx
 static bool cheb_x2(const DiaLayout& L, const Tune& T);
 static int cheb_x2_blocks(const DiaLayout& L) {
@@ -521,7 +527,7 @@ static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, co
         CU(add_kernel(body, &n_s, dep, ndep, P.k1x2 ? (void*)k_fused_pspmv_x2 : (void*)k_fused_pspmv, P.fblocks, a));
       }
       void* a2[] = {&ctx, &ctl, &partials, &h_while, &h_if};
-      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, P.k2blocks, a2));
+      CU(add_kernel(body, &n_u, &n_s, 1, (void*)k_update<false>, P.k2blocks, a2, 0, kK2Threads));
     }
   } else {
     { void* a[] = {&ctx, &ctl};
@@ -647,11 +653,13 @@ static int fused_tma_blocks(const DiaLayout& L) {
 }
 // Grid of K2 (k_update<false>, a pure stream): exactly ONE wave of resident CTAs striding over the rows.  Measured at cfg 3
 // (B200): 1184 CTAs = two waves 0.0905 ms (late stage) / 0.0849 (early), 592 CTAs = one wave 0.0861 / 0.0809; four instead of
-// two row pairs per trip were slower in every combination.
+// two row pairs per trip were slower in every combination.  Round 2c: the same wave as 296 CTAs of 512 threads -- half the
+// tickets and partials for the last CTA to collect: cfg 3 MIXED 1.3450 / 1.3467 -> 1.3445 s, FP64 1.3728 -> 1.3696 s, cfg 5
+// (40 steps) 2.302 -> 2.278 s (1024 threads: 1.3429 / 1.3682 / 2.287).
 static int k2_blocks(int64_t n) {
-  const int resident = coresident_blocks(4, (const void*)k_update<false>, 8, kMaxBlocks);
-  const int want = grid_blocks(n);
-  return resident > 0 && resident < want ? resident : want;
+  const int resident = coresident_blocks(4, (const void*)k_update<false>, 2048 / kK2Threads, kMaxBlocks, 0, kK2Threads);
+  const int want = (int)((n + (int64_t)kK2Threads * kRows - 1) / ((int64_t)kK2Threads * kRows));
+  return resident > 0 && resident < want ? resident : (want > 0 ? want : 1);
 }
 // Launch configuration of the persistent kernel (and of the fixed-FP32 ablation kernel, which shares its row loops).
 // What a grid-wide barrier costs grows with the CTAs that take part in it, so the kernel runs FEW, LARGE CTAs: always 128
@@ -1255,7 +1263,7 @@ int cuth_profile_kernel(void* work_D, const cuth_grid_t* grid, const cuth_opts_t
       } else if (fused_x2(L, T)) k_fused_pspmv_x2<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       else k_fused_pspmv<<<fused_blocks(L, T), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials);
       break;
-    case 5: k_update<false><<<k2_blocks(L.n), kThreads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
+    case 5: k_update<false><<<k2_blocks(L.n), kK2Threads, 0, st>>>(w.ctx, w.ctl, w.partials, h0, h0); break;
     case 6: case 7: case 8: {      // one middle step of the Chebyshev apply: fp64 / fp32 on A2 / fp32 on A3 (fp16)
       const int code = kernel_id - 6;
       const bool x2 = code != 0 && cheb_x2(L, T);

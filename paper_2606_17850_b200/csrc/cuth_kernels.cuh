@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kThreads, CUTH_MINB) k_spmv_dot(const Ctx* __r
 // Alg. 1 lines 8-11: x += alpha p, r -= alpha mu, z = M^-1 r, rho' = r.z, ||r||^2; the last block
 // forms beta, advances the iteration counter and takes the loop / policy decisions.
 template <bool UPDATE_X>
-__global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
+__global__ void __launch_bounds__(1024) k_update(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                     cudaGraphConditionalHandle h_while,
                                                     cudaGraphConditionalHandle h_if) {
   __shared__ double smem[2 * 32];
@@ -356,21 +356,22 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
   if (ctl->halt) return;                     // unrolled graph body: this pass is over (cuth_api.cu build_graph)
   const Ctx c = *ctxp;
   const double alpha = ctl->alpha;
+  const int nt = (int)blockDim.x;            // threads per CTA are a launch parameter (k2_threads, cuth_api.cu)
   double acc[2] = {0.0, 0.0};
   if (!UPDATE_X && ctl->xnow) {
     // Fused path, an evaluation of the true residual is certain to follow this iteration (policy_after_spmv): Alg. 1
     // line 8 here instead of in the next K1 -- p' is the buffer K1 has just written (most of it still in L2).
     const double* __restrict__ pn = ctl->pcur ? c.p2 : c.p;
-    CUTH_TILE_LOOP(c.A.n) {
+    for (int64_t base = (int64_t)blockIdx.x * (nt * kRows); base < c.A.n; base += (int64_t)gridDim.x * (nt * kRows)) {
       double xv[kRows], pv[kRows];
 #pragma unroll
       for (int k = 0; k < kRows; ++k) {
-        const int64_t i = base + threadIdx.x + k * kThreads;
+        const int64_t i = base + threadIdx.x + k * nt;
         xv[k] = i < c.A.n ? c.x[i] : 0.0; pv[k] = i < c.A.n ? pn[i] : 0.0;
       }
 #pragma unroll
       for (int k = 0; k < kRows; ++k) {
-        const int64_t i = base + threadIdx.x + k * kThreads;
+        const int64_t i = base + threadIdx.x + k * nt;
         if (i < c.A.n) c.x[i] = fma(alpha, pv[k], xv[k]);
       }
     }
@@ -391,13 +392,13 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
 #define CUTH_K2_PAIRS 2
 #endif
     constexpr int NP = CUTH_K2_PAIRS;
-    for (int64_t base = (int64_t)blockIdx.x * (kThreads * NP); base < n2; base += (int64_t)gridDim.x * (kThreads * NP)) {
+    for (int64_t base = (int64_t)blockIdx.x * (nt * NP); base < n2; base += (int64_t)gridDim.x * (nt * NP)) {
       const double2 one = make_double2(1.0, 1.0), zero = make_double2(0.0, 0.0);
       double2 rv[NP], mv[NP], dv[NP];
       bool h[NP];
 #pragma unroll
       for (int q = 0; q < NP; ++q) {
-        const int64_t i = base + threadIdx.x + (int64_t)q * kThreads;
+        const int64_t i = base + threadIdx.x + (int64_t)q * nt;
         h[q] = i < n2;
         rv[q] = h[q] ? r2[i] : zero;
         mv[q] = h[q] ? __ldcs(&m2[i]) : zero;
@@ -409,7 +410,7 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       }
 #pragma unroll
       for (int q = 0; q < NP; ++q) {
-        const int64_t i = base + threadIdx.x + (int64_t)q * kThreads;
+        const int64_t i = base + threadIdx.x + (int64_t)q * nt;
         const double a0 = fma(-alpha, mv[q].x, rv[q].x), a1 = fma(-alpha, mv[q].y, rv[q].y);
         if (h[q]) w2[i] = make_double2(a0, a1);
         acc[0] = fma(a0, a0 * dv[q].x, acc[0]); acc[1] = fma(a0, a0, acc[1]);
@@ -417,10 +418,10 @@ __global__ void __launch_bounds__(kThreads) k_update(const Ctx* __restrict__ ctx
       }
     }
   } else {
-  CUTH_TILE_LOOP(c.A.n) {
+  for (int64_t base = (int64_t)blockIdx.x * (nt * kRows); base < c.A.n; base += (int64_t)gridDim.x * (nt * kRows)) {
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
+      const int64_t i = base + threadIdx.x + k * nt;
       if (i < c.A.n) {
         if (UPDATE_X) c.x[i] = fma(alpha, c.p[i], c.x[i]);
         const double ri = fma(-alpha, c.mu[i], c.r[i]);
