@@ -686,9 +686,9 @@ static PersistConfig persistent_config(int64_t n) {
 }
 static int persistent_blocks(int64_t n) { return persistent_config(n).blocks; }
 
-// The cluster-resident kernel (cuth_cluster.cuh): every row lives in the shared memory of one 8-CTA cluster.
-// Measured on B200 (profiles/r2c_loop_homes.md), per iteration, cluster / persistent kernel / graph: cfg 1 (8 192 rows)
-// 4.4 / 7.1 / 18.8 us, 2 048 rows 3.7 / 6.7 / 19.4, 12 800 rows 5.0 / 7.1 / 19.2.
+// The cluster-resident kernels (cuth_cluster_reg.cuh, cuth_cluster.cuh): every row lives in the registers / the shared memory
+// of one 8- or 16-CTA cluster.  Measured on B200 (profiles/r2e_cluster.md), per iteration, cluster / persistent kernel /
+// graph: cfg 1 (8 192 rows) 2.2 / 6.9 / 18.8 us, 2 048 rows 2.1 / 6.4 / 19.4, 12 800 rows 2.7 / 7.2 / 19.2.
 static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune& T) {
   if (T.loop_mode == 1 || T.loop_mode == 2 || T.traversal == 2) return false;
   if (opts->preconditioner == CUTH_PRECOND_CHEBYSHEV) return false;
@@ -696,9 +696,7 @@ static bool use_cluster(const DiaLayout& L, const cuth_opts_t* opts, const Tune&
   return cluster_fits(L.nx, L.ny, L.nz, kClusterMaxCtas);
 }
 
-// One cluster per solve (nsolves > 1: cuth_pcg_solve_batch, contexts and control blocks as arrays).  8 CTAs when the
-// rows fit them, else 16 (non-portable cluster size): measured at cfg 1 (8 192 rows) 4.41 us per iteration with 8 CTAs
-// against 4.88 with 16 -- the all-reduce across CTAs costs more than the halved row work saves.
+// One cluster per solve (nsolves > 1: cuth_pcg_solve_batch, contexts and control blocks as arrays).
 // Up to 1024 rows per CTA the rows live in registers (cuth_cluster_reg.cuh); beyond, or with loop_mode = 4, in shared
 // memory (cuth_cluster.cuh).  The candidates are tried in the measured order of speed until one launches (a 16-CTA
 // cluster is a non-portable size and may be refused).  Measured at cfg 1 (8 192 rows, FP64 / MIXED, us per iteration):
