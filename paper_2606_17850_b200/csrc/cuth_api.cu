@@ -726,9 +726,16 @@ static bool cluster_form_config(const ClusterForm& f, const DiaLayout& L, int ns
 }
 // Clusters of this form that can be resident at once on the current device (0: unknown).
 static int cluster_form_resident(const ClusterForm& f, const DiaLayout& L) {
-  cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1]; int rows = 0, nclu = 0;
-  if (!cluster_form_config(f, L, 1, nullptr, &cfg, at, &rows)) return 0;
-  if (cudaOccupancyMaxActiveClusters(&nclu, f.fn, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+  cudaLaunchConfig_t cfg; cudaLaunchAttribute at[1]; int rows = 0, nclu = 0, dev = 0;
+  if (!cluster_form_config(f, L, 1, nullptr, &cfg, at, &rows) || cudaGetDevice(&dev) != cudaSuccess) return 0;
+  // derived data, cached per (device, form, shared-memory size) like the co-resident CTA counts
+  const long long key = ((long long)dev << 40) | ((long long)f.nc << 32) | ((long long)f.threads << 20) | (long long)(rows & 0xfffff);
+  static std::unordered_map<long long, int> cache;
+  std::lock_guard<std::mutex> lk(g_dev_mu);
+  auto it = cache.find(key);
+  if (it != cache.end()) return it->second;
+  if (cudaOccupancyMaxActiveClusters(&nclu, f.fn, &cfg) != cudaSuccess) { cudaGetLastError(); nclu = 0; }
+  cache[key] = nclu;
   return nclu;
 }
 static cudaError_t launch_cluster(const DiaLayout& L, const Ctx* ctxp, Ctl* ctlp, int nsolves, cudaStream_t st,
