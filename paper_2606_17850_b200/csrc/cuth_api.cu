@@ -552,7 +552,7 @@ static int build_graph(const Workspace& w, const Plan& P, const DiaLayout& L, co
   { void* a[] = {&ctx, &ctl, &partials, &h_while};
     CU(add_kernel(ifb, &n_t, P.fblocks > 0 ? &n_f : nullptr, P.fblocks > 0 ? 1 : 0, (void*)k_true_resid, sblocks, a)); }
   { void* a[] = {&ctx, &ctl, &partials};
-    CU(add_kernel(ifb, &n_r, &n_t, 1, (void*)k_restart, blocks, a)); }
+    CU(add_kernel(ifb, &n_r, &n_t, 1, (void*)k_restart, sblocks, a)); }      // applies A1 itself: the stencil grid
 
   cudaGraphExec_t ex;
   CU(cudaGraphInstantiate(&ex, g, 0));

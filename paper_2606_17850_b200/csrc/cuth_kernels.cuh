@@ -440,8 +440,9 @@ __global__ void __launch_bounds__(1024) k_update(const Ctx* __restrict__ ctxp, C
   }
 }
 
-// True residual: t = b - A1 x in fp64 (stored in the mu buffer, which is dead here),
-// ||t||^2 and the drift ||t - r||^2; the last block applies the stopping rule and eq. (14a)-(14c).
+// True residual: t = b - A1 x in fp64, ||t||^2 and the drift ||t - r||^2; the last block applies the
+// stopping rule and eq. (14a)-(14c).  t itself is not stored (round 2b wrote it to the mu buffer for k_restart: 8 of the
+// 64 B/row of every evaluation for a restart that happens once or twice per solve): k_restart forms it again.
 __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials,
                                                         cudaGraphConditionalHandle h_while) {
   __shared__ double smem[2 * 32];
@@ -451,7 +452,6 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
   apply_A<OP_FP64>(c.A, c.x, [&](int64_t i, double, double ax) {
     const double ti = c.b[i] - ax;
     const double di = ti - c.r[i];
-    c.mu[i] = ti;
     acc[0] = fma(ti, ti, acc[0]);
     acc[1] = fma(di, di, acc[1]);
   });
@@ -461,8 +461,9 @@ __global__ void __launch_bounds__(kThreads) k_true_resid(const Ctx* __restrict__
   }
 }
 
-// Hot restart: r := t (= b - A1 x, sitting in mu), z = M^-1 r, rho = r.z, beta := 0 so that
-// the next k_pupdate gives p = z (p's defining equation, Alg. 1 line 3).  No-op unless ctl->restart.
+// Hot restart: r := t = b - A1 x (the same operations on the same x as in k_true_resid: the same bits),
+// z = M^-1 r, rho = r.z, beta := 0 so that the next k_pupdate gives p = z (p's defining equation, Alg. 1 line 3).
+// No-op unless ctl->restart.
 __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ctxp, Ctl* ctl, double* partials) {
   __shared__ double smem[2 * 32];
   __shared__ int s_flag;
@@ -470,19 +471,13 @@ __global__ void __launch_bounds__(kThreads) k_restart(const Ctx* __restrict__ ct
   if (!mode) return;
   const Ctx c = *ctxp;
   double acc[2] = {0.0, 0.0};
-  CUTH_TILE_LOOP(c.A.n) {
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-      const int64_t i = base + threadIdx.x + k * kThreads;
-      if (i < c.A.n) {
-        const double ri = c.mu[i];
-        const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
-        c.r[i] = ri;
-        acc[0] = fma(ri, zi, acc[0]);
-        acc[1] = fma(ri, ri, acc[1]);
-      }
-    }
-  }
+  apply_A<OP_FP64>(c.A, c.x, [&](int64_t i, double, double ax) {
+    const double ri = c.b[i] - ax;
+    const double zi = c.jacobi ? ri * c.A.dinv[i] : ri;
+    c.r[i] = ri;
+    acc[0] = fma(ri, zi, acc[0]);
+    acc[1] = fma(ri, ri, acc[1]);
+  });
   if (grid_sum_last_block<2>(acc, partials + 2 * kMaxBlocks, &ctl->ticket[4], smem, &s_flag) && threadIdx.x == 0) {
     policy_after_restart(ctl, c, mode, acc[0], acc[1]);
   }
