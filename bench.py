@@ -639,7 +639,7 @@ def main():
                                        "floor bytes (8m+88 fp64 three-kernel, 8m+80 fp64 fused / 4(m-1)+80 fp32-stored fused, 4(m-1)+88 unfused, per row per iteration) "
                                        "x iterations / whole-solve time, true-residual checks included in the time"},
         "kernels_ms": kern, "spmv": spmv, "setup_ms": setup_ms,
-        "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % ((5 if mixed and w.true_resid_period % 5 == 0 else 4) if fused and not cheb else 1),
+        "loop": {1: "cuda graph (conditional WHILE/IF nodes, %d iterations per pass)" % ((next((u for u in (10, 8, 6, 5, 4, 3) if w.true_resid_period % u == 0), 4) if mixed else 8) if fused and not cheb else 1),
                  2: "persistent cooperative kernel", 3: "cluster-resident kernel (one thread-block cluster)",
                  4: "fixed-FP32 ablation kernel"}[cu.cuth_loop_home(g, S.opts)],
         "e2e": {"value": e2e_ms_max * 1e-3, "unit": UNIT, "h2d_bytes_per_step": int(w.n * 8 * nt),
